@@ -1,0 +1,131 @@
+// common.cuh - shared device-side declarations of the tandem rollout engine (sm_100a).
+// Notation follows DESIGN.md section 2: slot s = resident sequence, n_ctx = tokens in the shared context,
+// ing[M] = context positions whose K/V model M has stored, row = one (sequence, position) processed this step.
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <stdint.h>
+
+namespace tandem {
+
+constexpr int kPageTokens = 16;      // KV page size (BASELINE.json configs[2]: "paged KV with 16-token blocks")
+constexpr int kAttnChunk = 256;      // KV positions per split of a decode row; a function of kv_len only (determinism)
+constexpr int kMaxSlots = 1024;      // scheduler is one CTA with one thread per slot
+
+typedef __nv_bfloat16 bf16;
+
+template <typename T> struct Elem;
+template <> struct Elem<float> {
+  static __device__ __forceinline__ float ld(const float* p) { return *p; }
+  static __device__ __forceinline__ void st(float* p, float v) { *p = v; }
+};
+template <> struct Elem<bf16> {
+  static __device__ __forceinline__ float ld(const bf16* p) { return __bfloat162float(*p); }
+  static __device__ __forceinline__ void st(bf16* p, float v) { *p = __float2bfloat16_rn(v); }
+};
+
+// counts[] indices of a per-model step table
+enum { C_ROWS = 0, C_SCHED = 1, C_EMIT = 2, C_ITEMS = 3, C_COMB = 4, C_PARTS = 5, C_NUM = 8 };
+
+// Per-model tables the scheduler (S0) writes each step; everything downstream reads row counts from here,
+// so every launch has a fixed grid and the whole step can be replayed as a CUDA graph.
+struct StepTab {
+  int32_t* counts;      // [C_NUM]
+  int32_t* row_slot;    // [R] slot of the row's sequence
+  int32_t* row_pos;     // [R] absolute position (kv_len of the row = pos + 1)
+  int32_t* row_tok;     // [R] token id at that position
+  int32_t* row_kvslot;  // [R] physical KV token index: page * kPageTokens + pos % kPageTokens
+  int32_t* row_emit;    // [R] emit index j if this is the last row of a sequence that emits this step, else -1
+  int32_t* emit_slot;   // [max_seqs] slot of emit index j
+  int32_t* item_row;    // [I] attention work item -> row
+  int32_t* item_split;  // [I] split index along KV (0 if unsplit)
+  int32_t* item_part;   // [I] partial-buffer index, or -1 if the item writes the final output
+  int32_t* comb_row;    // [max_seqs] rows whose splits must be combined
+  int32_t* comb_part0;  // [max_seqs] first partial of that row
+  int32_t* comb_n;      // [max_seqs] number of partials
+};
+
+struct SeqState {       // all [max_seqs]
+  int32_t* seq_id; int32_t* prompt_len; int32_t* n_ctx; int32_t* ing[2]; int32_t* cap_c;
+  int32_t* max_new; int32_t* n_emit; uint8_t* active; uint8_t* owner; uint8_t* done;
+};
+
+struct PageTab {        // per model
+  int32_t* bt;          // [max_seqs, max_pages] page ids
+  int32_t* npages;      // [max_seqs]
+  int32_t* free_pages;  // [pool_pages] stack of free page ids (page 0 is a dummy page, never handed out)
+  int32_t* free_top;    // scalar: number of free pages on the stack
+};
+
+struct DevStats {       // device-side accumulators (unsigned long long for atomicAdd)
+  unsigned long long steps, tokens_emitted, rows[2], catchup_rows, kv_tokens_read, model_steps;
+  int peak_pages_used[2]; int peak_resident; int err_oom;
+};
+
+struct StepIO {         // per-step optional outputs / overrides (device pointers, may be null)
+  int32_t* token; uint8_t* owner; float* sen_logp; uint8_t* done; int32_t* argmax; int32_t* n_active;
+  const int32_t* forced_tokens; long long forced_stride;
+  const float* u_switch; long long u_switch_stride;
+  const float* u_sample; long long u_sample_stride;
+  float* dbg_logits;
+};
+
+struct RuleParams {
+  float p; int switch_mode; int cap_k; float temperature; int eos_id; unsigned long long seed;
+};
+
+// ------------------------------------------------------------------------------------------------------------
+// Counter-based generator (DESIGN.md section 3 R3). Philox-4x32-10 (Salmon et al., SC'11): written from the
+// published round function; the oracle has its own NumPy implementation, the two share nothing.
+__device__ __host__ __forceinline__ void philox_round(uint32_t c[4], uint32_t k0, uint32_t k1) {
+  const uint64_t p0 = (uint64_t)0xD2511F53u * c[0];
+  const uint64_t p1 = (uint64_t)0xCD9E8D57u * c[2];
+  const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c[1] ^ k0;
+  const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c[3] ^ k1;
+  c[1] = (uint32_t)p1; c[3] = (uint32_t)p0; c[0] = n0; c[2] = n2;
+}
+__device__ __host__ __forceinline__ void philox4x32_10(uint32_t c[4], uint32_t k0, uint32_t k1) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    philox_round(c, k0, k1);
+    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+  }
+}
+// u = min((float(r) + 0.5f) * 2^-32, 1 - 2^-24), every operation rounded to nearest in fp32.
+__device__ __forceinline__ float uniform_from_bits(uint32_t r) {
+  float f = __uint2float_rn(r);
+  f = __fadd_rn(f, 0.5f);
+  f = __fmul_rn(f, 2.3283064365386963e-10f);   // 2^-32
+  return fminf(f, 0.99999994f);                // 1 - 2^-24
+}
+__device__ __forceinline__ float u_switch_counter(unsigned long long seed, int seq_id, int t) {
+  uint32_t c[4] = {0u, (uint32_t)t, (uint32_t)seq_id, 1u};
+  philox4x32_10(c, (uint32_t)seed, (uint32_t)(seed >> 32));
+  return uniform_from_bits(c[0]);
+}
+// Gumbel variate from a uniform: E = -log1p(-u) (unit exponential), g = -ln E. Accurate libm calls, not intrinsics.
+__device__ __forceinline__ float gumbel_from_uniform(float u) { return -logf(-log1pf(-u)); }
+
+// ------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ float warp_max(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+// Sum over a CTA of NT threads (NT multiple of 32, <= 1024); result broadcast to all threads. `red` >= 32 floats.
+template <int NT> __device__ __forceinline__ float block_sum(float v, float* red) {
+  v = warp_sum(v);
+  const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+  __syncthreads();
+  if (l == 0) red[w] = v;
+  __syncthreads();
+  float t = (l < NT / 32) ? red[l] : 0.f;
+  return warp_sum(t);
+}
+
+}  // namespace tandem

@@ -1,0 +1,428 @@
+// kernels.cuh - scheduler (S0), embedding+norm (S1,S2), GEMM epilogues (S2,S4,S6,S7) and the
+// sample+switch+emit kernel (S8) of the tandem rollout engine. See DESIGN.md section 6.
+#pragma once
+#include "common.cuh"
+
+namespace tandem {
+
+// ============================================================================================ S0: scheduler
+// One CTA, one thread per slot. For each model M: the sequences M owns get rows for the context positions M
+// has not ingested yet (q_len = n_ctx - ing[M]; 1 = plain decode, >1 = catch-up / prompt prefill), capped by
+// the row budget in slot order; pages are taken from M's free stack; row, emit and attention-item tables are
+// written for the kernels downstream. PAPER.md L257 (per-step attention metadata: slot mappings, block tables,
+// position indices) - here per model, since the two models are no longer in lock-step.
+struct SchedArgs {
+  SeqState st; PageTab pt[2]; StepTab tab[2]; StepIO io; DevStats* stats;
+  const int32_t* tokens; int max_seqs, max_seq_len, max_pages, row_cap, max_splits;
+};
+
+__device__ __forceinline__ int block_excl_scan_1024(int v, int* total, int* wsum) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  int x = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+  if (lane == 31) wsum[w] = x;
+  __syncthreads();
+  if (w == 0) {
+    int s = wsum[lane];
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, s, o); if (lane >= o) s += y; }
+    wsum[lane] = s;
+  }
+  __syncthreads();
+  const int base = w > 0 ? wsum[w - 1] : 0;
+  *total = wsum[31];
+  __syncthreads();
+  return base + x - v;
+}
+
+// last index s in [0, n) with cu[s] <= r, given cu non-decreasing and cu[n] > r
+__device__ __forceinline__ int find_owner_slot(const int* cu, int n, int r) {
+  int lo = 0, hi = n;  // invariant: cu[lo] <= r < cu[hi]
+  while (hi - lo > 1) { int mid = (lo + hi) >> 1; if (cu[mid] <= r) lo = mid; else hi = mid; }
+  return lo;
+}
+
+__global__ void __launch_bounds__(1024) sched_kernel(SchedArgs a) {
+  __shared__ int cu_rows[kMaxSlots + 1], cu_items[kMaxSlots + 1];
+  __shared__ int sm_rows[kMaxSlots], sm_ing[kMaxSlots], sm_part0[kMaxSlots], sm_emit[kMaxSlots];
+  __shared__ int wsum[32];
+  const int s = threadIdx.x;
+  const bool in_range = s < a.max_seqs;
+
+  if (in_range) {  // defaults of the per-step outputs
+    if (a.io.token) a.io.token[s] = -1;
+    if (a.io.owner) a.io.owner[s] = 0;
+    if (a.io.sen_logp) a.io.sen_logp[s] = 0.f;
+    if (a.io.argmax) a.io.argmax[s] = -1;
+  }
+  const bool live = in_range && a.st.active[s] && !a.st.done[s];
+  const int owner = live ? a.st.owner[s] : -1;
+  const int nctx = live ? a.st.n_ctx[s] : 0;
+  int resident_total;
+  block_excl_scan_1024(live ? 1 : 0, &resident_total, wsum);
+
+  for (int M = 0; M < 2; ++M) {
+    const StepTab& tb = a.tab[M];
+    const PageTab& pt = a.pt[M];
+    const bool mine = owner == M;
+    const int ing = mine ? a.st.ing[M][s] : 0;
+    const int want = mine ? nctx - ing : 0;
+    int total_want;
+    const int pre = block_excl_scan_1024(want, &total_want, wsum);
+    const int rows = min(want, max(0, a.row_cap - pre));
+    const int cu = min(pre, a.row_cap);
+    const int n_rows = min(total_want, a.row_cap);
+    const bool emits = mine && rows == want && want > 0;
+
+    // pages for positions [ing, ing + rows)
+    if (rows > 0) {
+      const int need = (ing + rows + kPageTokens - 1) / kPageTokens;
+      const int have = pt.npages[s];
+      const int k = need - have;
+      if (k > 0) {
+        const int old = atomicSub(pt.free_top, k);
+        if (old >= k) {
+          for (int i = 0; i < k; ++i) pt.bt[(size_t)s * a.max_pages + have + i] = pt.free_pages[old - 1 - i];
+        } else {  // pool exhausted: point at the dummy page (no fault), flag the error for the host
+          atomicAdd(pt.free_top, k);
+          for (int i = 0; i < k; ++i) pt.bt[(size_t)s * a.max_pages + have + i] = 0;
+          a.stats->err_oom = 1;
+        }
+        pt.npages[s] = need;
+      }
+    }
+    int n_emit;
+    const int j = block_excl_scan_1024(emits ? 1 : 0, &n_emit, wsum);
+    // attention items: a decode row (q_len == 1) is split along KV in chunks of kAttnChunk; rows of a
+    // multi-row sequence are one item each (parallelism comes from the rows).
+    const int nsplit = (rows == 1) ? (ing + 1 + kAttnChunk - 1) / kAttnChunk : 1;
+    const int items = (rows == 1) ? nsplit : rows;
+    const int parts = (rows == 1 && nsplit > 1) ? nsplit : 0;
+    int n_items, n_parts, n_comb, n_sched;
+    const int icu = block_excl_scan_1024(items, &n_items, wsum);
+    const int pcu = block_excl_scan_1024(parts, &n_parts, wsum);
+    const int ccu = block_excl_scan_1024(parts > 0 ? 1 : 0, &n_comb, wsum);
+    block_excl_scan_1024(rows > 0 ? 1 : 0, &n_sched, wsum);
+
+    cu_rows[s] = cu; cu_items[s] = icu;
+    sm_rows[s] = rows; sm_ing[s] = ing; sm_part0[s] = parts > 0 ? pcu : -1; sm_emit[s] = emits ? j : -1;
+    if (s == 0) { cu_rows[kMaxSlots] = n_rows; cu_items[kMaxSlots] = n_items; }
+    if (emits) tb.emit_slot[j] = s;
+    if (parts > 0) { tb.comb_row[ccu] = cu; tb.comb_part0[ccu] = pcu; tb.comb_n[ccu] = nsplit; }
+    if (rows > 0) a.st.ing[M][s] = ing + rows;  // commit: the forward below always runs
+    __syncthreads();
+
+    for (int r = threadIdx.x; r < n_rows; r += blockDim.x) {
+      const int q = find_owner_slot(cu_rows, kMaxSlots, r);
+      const int off = r - cu_rows[q];
+      const int pos = sm_ing[q] + off;
+      tb.row_slot[r] = q;
+      tb.row_pos[r] = pos;
+      tb.row_tok[r] = a.tokens[(size_t)q * a.max_seq_len + pos];
+      tb.row_kvslot[r] = pt.bt[(size_t)q * a.max_pages + pos / kPageTokens] * kPageTokens + pos % kPageTokens;
+      tb.row_emit[r] = (off == sm_rows[q] - 1) ? sm_emit[q] : -1;
+    }
+    for (int i = threadIdx.x; i < n_items; i += blockDim.x) {
+      const int q = find_owner_slot(cu_items, kMaxSlots, i);
+      const int off = i - cu_items[q];
+      if (sm_rows[q] == 1) {
+        tb.item_row[i] = cu_rows[q]; tb.item_split[i] = off;
+        tb.item_part[i] = sm_part0[q] >= 0 ? sm_part0[q] + off : -1;
+      } else {
+        tb.item_row[i] = cu_rows[q] + off; tb.item_split[i] = 0; tb.item_part[i] = -1;
+      }
+    }
+    if (threadIdx.x == 0) {
+      tb.counts[C_ROWS] = n_rows; tb.counts[C_SCHED] = n_sched; tb.counts[C_EMIT] = n_emit;
+      tb.counts[C_ITEMS] = n_items; tb.counts[C_COMB] = n_comb; tb.counts[C_PARTS] = n_parts;
+      a.stats->rows[M] += (unsigned long long)n_rows;
+      a.stats->catchup_rows += (unsigned long long)(n_rows - n_sched);
+      a.stats->tokens_emitted += (unsigned long long)n_emit;
+      if (n_rows > 0) a.stats->model_steps += 1ull;
+    }
+    // algorithmic KV tokens read this step: each scheduled sequence's owner reads its context once
+    int kv_total;
+    block_excl_scan_1024(rows > 0 ? ing + rows : 0, &kv_total, wsum);
+    if (threadIdx.x == 0) a.stats->kv_tokens_read += (unsigned long long)kv_total;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    a.stats->steps += 1ull;
+    a.stats->peak_resident = max(a.stats->peak_resident, resident_total);
+  }
+}
+
+// ============================================================================================ admission
+struct AdmitArgs {
+  SeqState st; PageTab pt[2]; int32_t* tokens; int max_seq_len;
+  const int32_t* stage_tokens; const long long* stage_off; const int32_t* slots; const int32_t* seq_ids; const int32_t* max_new;
+  int n; int start_owner; float p; unsigned long long seed; const float* u_switch; long long u_switch_stride;
+};
+__global__ void admit_kernel(AdmitArgs a) {
+  const int i = blockIdx.x;
+  if (i >= a.n) return;
+  const int s = a.slots[i];
+  const long long o0 = a.stage_off[i], o1 = a.stage_off[i + 1];
+  for (long long k = o0 + threadIdx.x; k < o1; k += blockDim.x) a.tokens[(size_t)s * a.max_seq_len + (k - o0)] = a.stage_tokens[k];
+  if (threadIdx.x == 0) {
+    const int sid = a.seq_ids[i];
+    int owner = a.start_owner;
+    if (owner == 2) {  // DRAW: Alg. 1 line 6: senior iff u_switch[b,0] < p
+      const float u = a.u_switch ? a.u_switch[(size_t)s * a.u_switch_stride] : u_switch_counter(a.seed, sid, 0);
+      owner = (u < a.p) ? 0 : 1;
+    }
+    a.st.seq_id[s] = sid; a.st.prompt_len[s] = (int)(o1 - o0); a.st.n_ctx[s] = (int)(o1 - o0);
+    a.st.ing[0][s] = 0; a.st.ing[1][s] = 0; a.st.cap_c[s] = 0; a.st.max_new[s] = a.max_new[i]; a.st.n_emit[s] = 0;
+    a.st.owner[s] = (uint8_t)owner; a.st.done[s] = 0; a.st.active[s] = 1;
+    a.pt[0].npages[s] = 0; a.pt[1].npages[s] = 0;
+  }
+}
+
+// ============================================================================================ finalize
+// After both models' samplers: release the pages of sequences that finished this step and count the rest.
+struct FinalArgs { SeqState st; PageTab pt[2]; StepIO io; DevStats* stats; int32_t* n_active; int max_seqs, max_pages, pool_pages; };
+__global__ void __launch_bounds__(1024) finalize_kernel(FinalArgs a) {
+  __shared__ int wsum[32];
+  const int s = threadIdx.x;
+  bool live = false;
+  if (s < a.max_seqs && a.st.active[s]) {
+    if (a.st.done[s]) {
+      for (int M = 0; M < 2; ++M) {
+        const int n = a.pt[M].npages[s];
+        if (n > 0) {
+          const int pos = atomicAdd(a.pt[M].free_top, n);
+          for (int i = 0; i < n; ++i) {
+            const int pg = a.pt[M].bt[(size_t)s * a.max_pages + i];
+            if (pos + i < a.pool_pages) a.pt[M].free_pages[pos + i] = pg;
+          }
+          a.pt[M].npages[s] = 0;
+        }
+      }
+      a.st.active[s] = 0;
+    } else {
+      live = true;
+    }
+  }
+  if (s < a.max_seqs && a.io.done) a.io.done[s] = a.st.done[s];
+  int n_live;
+  block_excl_scan_1024(live ? 1 : 0, &n_live, wsum);
+  if (s == 0) {
+    *a.n_active = n_live;
+    if (a.io.n_active) *a.io.n_active = n_live;
+    for (int M = 0; M < 2; ++M) {
+      const int used = a.pool_pages - 1 - *a.pt[M].free_top;
+      a.stats->peak_pages_used[M] = max(a.stats->peak_pages_used[M], used);
+    }
+  }
+}
+
+// ============================================================================================ S1+S2: embed + RMSNorm
+// x[r,:] = E[token_r] (fp32 residual stream); u = x g / sqrt(mean x^2 + eps) -> act (GEMM A-operand dtype).
+template <typename T, int NT>
+__global__ void __launch_bounds__(NT) embed_norm_kernel(const int32_t* __restrict__ counts, const int32_t* __restrict__ row_tok,
+                                                        const T* __restrict__ E, const T* __restrict__ gain, float* __restrict__ x,
+                                                        T* __restrict__ act, int H, float eps) {
+  __shared__ float red[32];
+  const int n_rows = counts[C_ROWS];
+  for (int r = blockIdx.x; r < n_rows; r += gridDim.x) {
+    const T* e = E + (size_t)row_tok[r] * H;
+    float ss = 0.f;
+    for (int j = threadIdx.x; j < H; j += NT) { const float v = Elem<T>::ld(e + j); x[(size_t)r * H + j] = v; ss += v * v; }
+    const float inv = rsqrtf(block_sum<NT>(ss, red) / (float)H + eps);
+    for (int j = threadIdx.x; j < H; j += NT) Elem<T>::st(act + (size_t)r * H + j, Elem<T>::ld(e + j) * Elem<T>::ld(gain + j) * inv);
+  }
+}
+
+// ============================================================================================ S6/S7: residual + RMSNorm
+// x[r,:] += sum_s part[s][r,:]; u = RMSNorm(x; gain) -> act. With out_map (last layer): only rows that emit are
+// normalised (with the final-norm gain) and written compactly at their emit index (the LM head runs on those only).
+template <typename T, int NT>
+__global__ void __launch_bounds__(NT) residual_norm_kernel(const int32_t* __restrict__ counts, const float* __restrict__ part, int n_split,
+                                                           size_t split_stride, float* __restrict__ x, const T* __restrict__ gain,
+                                                           T* __restrict__ act, const int32_t* __restrict__ out_map, int H, float eps) {
+  __shared__ float red[32];
+  const int n_rows = counts[C_ROWS];
+  for (int r = blockIdx.x; r < n_rows; r += gridDim.x) {
+    float ss = 0.f;
+    for (int j = threadIdx.x; j < H; j += NT) {
+      float v = x[(size_t)r * H + j];
+      for (int s = 0; s < n_split; ++s) v += part[s * split_stride + (size_t)r * H + j];
+      x[(size_t)r * H + j] = v;
+      ss += v * v;
+    }
+    int orow = r;
+    if (out_map) { orow = out_map[r]; }
+    const float inv = rsqrtf(block_sum<NT>(ss, red) / (float)H + eps);
+    if (orow < 0) continue;
+    for (int j = threadIdx.x; j < H; j += NT) Elem<T>::st(act + (size_t)orow * H + j, x[(size_t)r * H + j] * Elem<T>::ld(gain + j) * inv);
+  }
+}
+
+// ============================================================================================ S4: RoPE + KV append
+// qkv[r, :] = sum_s part[s][r, :] is [q (nq*d) | k (nkv*d) | v (nkv*d)]. RoPE (half-split pairs (j, j+d/2), angle
+// pos * theta^(-2j/d) from a table built in double at init) on q and k; q -> fp32 buffer, k and v -> model M's pages.
+template <typename T, int NT>
+__global__ void __launch_bounds__(NT) rope_append_kernel(const int32_t* __restrict__ counts, const int32_t* __restrict__ row_pos,
+                                                         const int32_t* __restrict__ row_kvslot, const float* __restrict__ part, int n_split,
+                                                         size_t split_stride, const float2* __restrict__ cs_table, float* __restrict__ q_out,
+                                                         T* __restrict__ kpool, T* __restrict__ vpool, int nq, int nkv, int d) {
+  const int n_rows = counts[C_ROWS];
+  const int half = d >> 1;
+  const int ld = (nq + 2 * nkv) * d;
+  const int n_pairs = (nq + nkv) * half;
+  for (int r = blockIdx.x; r < n_rows; r += gridDim.x) {
+    const int pos = row_pos[r];
+    const int kvslot = row_kvslot[r];
+    const int page = kvslot / kPageTokens, off = kvslot % kPageTokens;
+    const float* src = part + (size_t)r * ld;
+    for (int i = threadIdx.x; i < n_pairs; i += NT) {
+      const int head = i / half, j = i - head * half;
+      float a = 0.f, b = 0.f;
+      for (int s = 0; s < n_split; ++s) { a += src[s * split_stride + head * d + j]; b += src[s * split_stride + head * d + j + half]; }
+      const float2 cs = cs_table[(size_t)pos * half + j];
+      const float ra = a * cs.x - b * cs.y;
+      const float rb = b * cs.x + a * cs.y;
+      if (head < nq) {
+        q_out[(size_t)r * nq * d + head * d + j] = ra;
+        q_out[(size_t)r * nq * d + head * d + j + half] = rb;
+      } else {
+        const int kh = head - nq;
+        T* dst = kpool + (((size_t)page * nkv + kh) * kPageTokens + off) * d;
+        Elem<T>::st(dst + j, ra); Elem<T>::st(dst + j + half, rb);
+      }
+    }
+    for (int i = threadIdx.x; i < nkv * d; i += NT) {
+      const int kh = i / d, e = i - kh * d;
+      float v = 0.f;
+      for (int s = 0; s < n_split; ++s) v += src[s * split_stride + (nq + nkv) * d + i];
+      Elem<T>::st(vpool + (((size_t)page * nkv + kh) * kPageTokens + off) * d + e, v);
+    }
+  }
+}
+
+// ============================================================================================ S7: SwiGLU
+// gu[r, :] = [gate (I) | up (I)] summed over splits; out = silu(gate) * up, silu(a) = a / (1 + exp(-a)).
+template <typename T, int NT>
+__global__ void __launch_bounds__(NT) swiglu_kernel(const int32_t* __restrict__ counts, const float* __restrict__ part, int n_split,
+                                                    size_t split_stride, T* __restrict__ out, int I) {
+  const int n_rows = counts[C_ROWS];
+  const size_t total = (size_t)n_rows * I;
+  for (size_t idx = (size_t)blockIdx.x * NT + threadIdx.x; idx < total; idx += (size_t)gridDim.x * NT) {
+    const size_t r = idx / I, j = idx - r * I;
+    float g = 0.f, u = 0.f;
+    for (int s = 0; s < n_split; ++s) { g += part[s * split_stride + r * 2 * I + j]; u += part[s * split_stride + r * 2 * I + I + j]; }
+    Elem<T>::st(out + idx, g / (1.f + expf(-g)) * u);
+  }
+}
+
+// ============================================================================================ S8: sample + switch + emit
+// One CTA per emitting sequence of model M. logits row j (fp32, [n_emit, V]) -> token (forced | greedy argmax |
+// Gumbel-max on position-addressed uniforms), log-prob under softmax(z/T'), authorship flag; then the rule of
+// PAPER.md L61 / Alg. 1 lines 9-15 / L271: EOS or length => done; boundary = word_start[y]; cap counter; coin.
+struct SampleArgs {
+  SeqState st; StepTab tab; StepIO io; RuleParams rp; const float* logits; const uint8_t* word_start;
+  int32_t* tokens; uint8_t* out_owner; float* out_logp; int vocab, max_seq_len, model;
+};
+
+struct ArgBest { float v; int i; };
+__device__ __forceinline__ ArgBest better(ArgBest a, ArgBest b) {  // larger value wins; ties: lower index
+  return (b.v > a.v || (b.v == a.v && b.i < a.i)) ? b : a;
+}
+
+template <int NT>
+__global__ void __launch_bounds__(NT) sample_switch_emit_kernel(SampleArgs a) {
+  __shared__ float s_m[NT / 32], s_s[NT / 32], s_bv[NT / 32], s_gv[NT / 32];
+  __shared__ int s_bi[NT / 32], s_gi[NT / 32];
+  const int j = blockIdx.x;
+  if (j >= a.tab.counts[C_EMIT]) return;
+  const int s = a.tab.emit_slot[j];
+  const int V = a.vocab;
+  const float* z = a.logits + (size_t)j * V;
+  const int t = a.st.n_emit[s] + 1;            // index of the token being emitted, 1-based
+  const int sid = a.st.seq_id[s];
+  const bool greedy = !(a.rp.temperature > 0.f);
+  const float invT = greedy ? 1.f : 1.f / a.rp.temperature;
+  const float* u_row = a.io.u_sample ? a.io.u_sample + ((size_t)s * a.io.u_sample_stride + (t - 1)) * V : nullptr;
+
+  if (a.io.dbg_logits) {  // debug: the owner's logits for this position
+    float* dst = a.io.dbg_logits + (size_t)s * V;
+    for (int v = threadIdx.x; v < V; v += NT) dst[v] = z[v];
+  }
+  // one pass: running (max, sum exp) of z*invT for the log-softmax, raw argmax, Gumbel-perturbed argmax
+  float m = -INFINITY, sum = 0.f;
+  ArgBest raw = {-INFINITY, 0x7fffffff}, gum = {-INFINITY, 0x7fffffff};
+  const uint32_t k0 = (uint32_t)a.rp.seed, k1 = (uint32_t)(a.rp.seed >> 32);
+  for (int b4 = threadIdx.x; b4 * 4 < V; b4 += NT) {
+    uint32_t c[4] = {(uint32_t)b4, (uint32_t)t, (uint32_t)sid, 0u};
+    if (!greedy && !u_row) philox4x32_10(c, k0, k1);
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+      const int v = b4 * 4 + w;
+      if (v >= V) break;
+      const float zv = z[v];
+      const float x = zv * invT;
+      if (x > m) { sum = sum * expf(m - x) + 1.f; m = x; } else { sum += expf(x - m); }
+      raw = better(raw, ArgBest{zv, v});
+      if (!greedy) {
+        const float u = u_row ? u_row[v] : uniform_from_bits(c[w]);
+        gum = better(gum, ArgBest{x + gumbel_from_uniform(u), v});
+      }
+    }
+  }
+  // warp then block reduction
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const float m2 = __shfl_xor_sync(0xffffffffu, m, o), s2 = __shfl_xor_sync(0xffffffffu, sum, o);
+    const float mn = fmaxf(m, m2);
+    sum = (m == -INFINITY ? 0.f : sum * expf(m - mn)) + (m2 == -INFINITY ? 0.f : s2 * expf(m2 - mn));
+    m = mn;
+    ArgBest o1 = {__shfl_xor_sync(0xffffffffu, raw.v, o), __shfl_xor_sync(0xffffffffu, raw.i, o)};
+    raw = better(raw, o1);
+    ArgBest o2 = {__shfl_xor_sync(0xffffffffu, gum.v, o), __shfl_xor_sync(0xffffffffu, gum.i, o)};
+    gum = better(gum, o2);
+  }
+  const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+  if (l == 0) { s_m[w] = m; s_s[w] = sum; s_bv[w] = raw.v; s_bi[w] = raw.i; s_gv[w] = gum.v; s_gi[w] = gum.i; }
+  __syncthreads();
+  if (threadIdx.x != 0) return;
+  for (int k = 1; k < NT / 32; ++k) {
+    const float mn = fmaxf(m, s_m[k]);
+    sum = (m == -INFINITY ? 0.f : sum * expf(m - mn)) + (s_m[k] == -INFINITY ? 0.f : s_s[k] * expf(s_m[k] - mn));
+    m = mn;
+    raw = better(raw, ArgBest{s_bv[k], s_bi[k]});
+    gum = better(gum, ArgBest{s_gv[k], s_gi[k]});
+  }
+  int y = greedy ? raw.i : gum.i;
+  if (a.io.forced_tokens) {
+    const int f = a.io.forced_tokens[(size_t)s * a.io.forced_stride + (t - 1)];
+    if (f >= 0) y = f;
+  }
+  const float logp = z[y] * invT - (m + logf(sum));
+  const int M = a.model;
+  const int n = a.st.n_ctx[s];
+  a.tokens[(size_t)s * a.max_seq_len + n] = y;
+  a.out_owner[(size_t)s * a.max_seq_len + (t - 1)] = (uint8_t)M;
+  a.out_logp[(size_t)s * a.max_seq_len + (t - 1)] = (M == 0) ? logp : 0.f;
+  a.st.n_ctx[s] = n + 1;
+  a.st.n_emit[s] = t;
+  if (a.io.token) a.io.token[s] = y;
+  if (a.io.owner) a.io.owner[s] = (uint8_t)M;
+  if (a.io.sen_logp) a.io.sen_logp[s] = (M == 0) ? logp : 0.f;
+  if (a.io.argmax) a.io.argmax[s] = raw.i;
+  if ((a.rp.eos_id >= 0 && y == a.rp.eos_id) || t >= a.st.max_new[s]) { a.st.done[s] = 1; return; }
+  // the rule: the coin after y_t decides the author of y_{t+1}
+  const bool boundary = a.word_start[y] != 0;
+  int c = boundary ? 0 : a.st.cap_c[s] + 1;
+  int owner = M;
+  if (boundary || (a.rp.cap_k > 0 && c >= a.rp.cap_k)) {
+    const float u = a.io.u_switch ? a.io.u_switch[(size_t)s * a.io.u_switch_stride + t] : u_switch_counter(a.rp.seed, sid, t);
+    const bool hit = u < a.rp.p;
+    owner = (a.rp.switch_mode == 0) ? (hit ? 1 - M : M) : (hit ? 0 : 1);
+    c = 0;
+  }
+  a.st.cap_c[s] = c;
+  a.st.owner[s] = (uint8_t)owner;
+}
+
+}  // namespace tandem

@@ -1,0 +1,717 @@
+// tandem.cu - host side of the C ABI declared in include/tandem.h: handle, weights, admission, the step
+// (S0 scheduler -> per model S1..S8 -> finalize) and whole-rollout generation. All arithmetic of the path
+// runs in the kernels of this directory; there is no CPU fallback.
+#include "../../include/tandem.h"
+
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "common.cuh"
+#include "kernels.cuh"
+#include "attention.cuh"
+#include "gemm_simt.cuh"
+#include "gemm_tcgen05.cuh"
+
+using namespace tandem;
+
+namespace {
+
+struct ModelWeights {
+  bool loaded = false;
+  void *embed = nullptr, *lm_head = nullptr, *final_norm = nullptr;
+  std::vector<void*> attn_norm, wqkv, wo, mlp_norm, wgu, wdown;
+};
+
+struct Workspace {  // per model, sized for row_cap rows
+  float* x = nullptr;          // residual stream fp32 [R, H]
+  void* act = nullptr;         // normalised activations (GEMM A operand) [R, H]
+  float* q = nullptr;          // RoPE'd queries fp32 [R, nq*d]
+  void* attn_out = nullptr;    // [R, nq*d]
+  void* mlp_act = nullptr;     // silu(gate)*up [R, I]
+  void* lm_in = nullptr;       // final-normed last rows [max_seqs, H]
+  float* gemm_out = nullptr;   // split-K partial outputs [S][R][N], S*N <= gemm_out_cols
+  float* logits = nullptr;     // [max_seqs, V]
+  float* part_acc = nullptr; float2* part_ml = nullptr;
+  void* kv = nullptr;          // page pool: [layer][K|V][page][nkv][16][d]
+  int32_t* tab_mem = nullptr;  // backing store of the StepTab arrays
+  int32_t* bt = nullptr; int32_t* npages = nullptr; int32_t* free_pages = nullptr; int32_t* free_top = nullptr;
+};
+
+struct GraphKey {
+  StepIO io; RuleParams rp; bool valid = false;
+  bool same(const StepIO& i, const RuleParams& r) const {
+    return valid && std::memcmp(&io, &i, sizeof(StepIO)) == 0 && rp.p == r.p && rp.switch_mode == r.switch_mode && rp.cap_k == r.cap_k &&
+           rp.temperature == r.temperature && rp.eos_id == r.eos_id && rp.seed == r.seed;
+  }
+};
+
+}  // namespace
+
+struct tandem_handle {
+  tandem_config cfg{};
+  std::string err;
+  bool cuda_fault = false;
+  int esize = 4;
+  int row_cap = 0, max_pages = 0, pool_pages = 0, max_splits = 0, max_items = 0, gemm_impl = TANDEM_GEMM_SIMT;
+  size_t gemm_out_cols = 0;
+  ModelWeights w[2];
+  Workspace ws[2];
+  StepTab tab[2]{};
+  PageTab pt[2]{};
+  SeqState st{};
+  int32_t* st_mem = nullptr; uint8_t* st_mem8 = nullptr;
+  int32_t* tokens = nullptr; uint8_t* out_owner = nullptr; float* out_logp = nullptr;
+  float2* rope_cs = nullptr;
+  uint8_t* word_start_dev = nullptr; std::vector<uint8_t> word_start_host;
+  DevStats* stats = nullptr; int32_t* n_active = nullptr;
+  cudaStream_t ms[2]{}; cudaStream_t gs{}; cudaEvent_t ev_fork{}, ev_join[2]{}, ev_in{}, ev_out{};
+  std::vector<uint8_t> slot_busy;           // host view of the slots
+  // admission staging
+  int32_t* stage_tokens = nullptr; size_t stage_cap = 0; long long* stage_off = nullptr; int32_t* stage_i32 = nullptr;
+  // graph of one step
+  cudaGraphExec_t graph = nullptr; GraphKey gkey;
+  TcGemmPlans* tc = nullptr;
+};
+
+namespace {
+
+int fail(tandem_handle* h, int code, const std::string& msg) {
+  if (h) h->err = msg;
+  return code;
+}
+#define CU(h, expr)                                                                                  \
+  do {                                                                                               \
+    cudaError_t e__ = (expr);                                                                        \
+    if (e__ != cudaSuccess) {                                                                        \
+      (h)->cuda_fault = true;                                                                        \
+      return fail((h), TANDEM_ECUDA, std::string(#expr) + ": " + cudaGetErrorString(e__));          \
+    }                                                                                                \
+  } while (0)
+
+template <typename P> int dmalloc(tandem_handle* h, P** p, size_t bytes) {
+  cudaError_t e = cudaMalloc((void**)p, bytes ? bytes : 16);
+  if (e != cudaSuccess) { cudaGetLastError(); return fail(h, TANDEM_ENOMEM, "cudaMalloc of " + std::to_string(bytes) + " bytes failed"); }
+  return TANDEM_OK;
+}
+#define DM(h, p, bytes) do { int rc__ = dmalloc((h), (p), (bytes)); if (rc__) return rc__; } while (0)
+
+int pick_splits(int n_tiles, int k_blocks) {
+  // enough CTAs to cover the 148 SMs once; never more than the k-blocks available, and each slice >= 4 k-blocks
+  int s = 1;
+  while (n_tiles * s < 120 && (s + 1) * 4 <= k_blocks && s < 16) ++s;
+  return s;
+}
+
+// ------------------------------------------------------------------------------------------ GEMM dispatch
+// out[s][r][n] partials (s < *n_split, stride *split_stride floats); rows read from counts_ptr[idx] on the device.
+template <typename T>
+int launch_gemm(tandem_handle* h, int m, int which, int layer, const void* A, const void* W, int N, int K, float* out,
+                const int32_t* rows_ptr, int rows_cap, int* n_split, size_t* split_stride, cudaStream_t s) {
+  *n_split = 1;
+  *split_stride = (size_t)rows_cap * N;
+  if (h->gemm_impl == TANDEM_GEMM_TCGEN05 && sizeof(T) == 2) {
+    return tc_gemm_launch(h->tc, m, which, layer, A, W, N, K, out, rows_ptr, rows_cap, n_split, split_stride, s);
+  }
+  dim3 grid((N + kSimtTile - 1) / kSimtTile, std::min((rows_cap + kSimtTile - 1) / kSimtTile, 16));
+  gemm_simt_kernel<T><<<grid, 256, 0, s>>>(rows_ptr, 0, (const T*)A, (const T*)W, out, N, K);
+  return TANDEM_OK;
+}
+
+template <typename T, int D, int G>
+void launch_attn_dg(const AttnArgs<T>& a, int grid, cudaStream_t s) {
+  paged_attention_kernel<T, D, G><<<grid, kAttnThreads, 0, s>>>(a);
+}
+template <typename T> struct AttnDispatch;
+template <> struct AttnDispatch<float> {
+  static bool run(const AttnArgs<float>& a, int D, int G, int grid, cudaStream_t s) {
+#define TD_CASE(d, g) if (D == d && G == g) { launch_attn_dg<float, d, g>(a, grid, s); return true; }
+    TD_CASE(32, 1) TD_CASE(32, 2) TD_CASE(32, 4) TD_CASE(64, 1) TD_CASE(64, 2) TD_CASE(64, 4) TD_CASE(128, 1) TD_CASE(128, 2) TD_CASE(128, 4)
+#undef TD_CASE
+    return false;
+  }
+};
+template <> struct AttnDispatch<bf16> {
+  static bool run(const AttnArgs<bf16>& a, int D, int G, int grid, cudaStream_t s) {
+#define TD_CASE(d, g) if (D == d && G == g) { launch_attn_dg<bf16, d, g>(a, grid, s); return true; }
+    TD_CASE(64, 1) TD_CASE(64, 2) TD_CASE(64, 4) TD_CASE(64, 7) TD_CASE(64, 8) TD_CASE(128, 1) TD_CASE(128, 2) TD_CASE(128, 4) TD_CASE(128, 8)
+#undef TD_CASE
+    return false;
+  }
+};
+bool attn_supported(int dtype, int D, int G) {
+  if (dtype == TANDEM_F32) return (D == 32 || D == 64 || D == 128) && (G == 1 || G == 2 || G == 4);
+  return (D == 64 && (G == 1 || G == 2 || G == 4 || G == 7 || G == 8)) || (D == 128 && (G == 1 || G == 2 || G == 4 || G == 8));
+}
+
+// ------------------------------------------------------------------------------------------ one model's forward (S1..S8)
+template <typename T>
+int model_forward(tandem_handle* h, int m, const StepIO& io, const RuleParams& rp, cudaStream_t s) {
+  const tandem_config& c = h->cfg;
+  const ModelWeights& w = h->w[m];
+  Workspace& ws = h->ws[m];
+  const StepTab& tb = h->tab[m];
+  const int H = c.hidden, nq = c.n_q_heads, nkv = c.n_kv_heads, d = c.head_dim, I = c.intermediate, V = c.vocab;
+  const int qkv_n = (nq + 2 * nkv) * d;
+  const int row_grid = 148 * 4;
+  const size_t layer_kv = (size_t)2 * h->pool_pages * nkv * kPageTokens * d;
+  const size_t half_kv = (size_t)h->pool_pages * nkv * kPageTokens * d;
+  int ns; size_t ss; int rc;
+
+  embed_norm_kernel<T, 256><<<row_grid, 256, 0, s>>>(tb.counts, tb.row_tok, (const T*)w.embed, (const T*)w.attn_norm[0], ws.x, (T*)ws.act, H, c.rms_eps);
+  for (int l = 0; l < c.n_layers; ++l) {
+    T* kpool = (T*)ws.kv + (size_t)l * layer_kv;
+    T* vpool = kpool + half_kv;
+    // S3 QKV projection
+    if ((rc = launch_gemm<T>(h, m, 0, l, ws.act, w.wqkv[l], qkv_n, H, ws.gemm_out, tb.counts + C_ROWS, h->row_cap, &ns, &ss, s))) return rc;
+    // S4 RoPE + KV append
+    rope_append_kernel<T, 256><<<row_grid, 256, 0, s>>>(tb.counts, tb.row_pos, tb.row_kvslot, ws.gemm_out, ns, ss, h->rope_cs, ws.q, kpool, vpool, nq, nkv, d);
+    // S5 attention (decode splits + catch-up rows), then combine
+    AttnArgs<T> aa{tb.counts, tb.item_row, tb.item_split, tb.item_part, tb.row_slot, tb.row_pos, h->pt[m].bt, h->max_pages, ws.q, kpool, vpool,
+                   (T*)ws.attn_out, ws.part_acc, ws.part_ml, nq, nkv, 1.0f / sqrtf((float)d)};
+    if (!AttnDispatch<T>::run(aa, d, nq / nkv, 148 * 4, s)) return fail(h, TANDEM_EINVAL, "unsupported (head_dim, group) for attention");
+    CombineArgs<T> ca{tb.counts, tb.comb_row, tb.comb_part0, tb.comb_n, ws.part_acc, ws.part_ml, (T*)ws.attn_out, nq, d};
+    attn_combine_kernel<T><<<148, 256, 0, s>>>(ca);
+    // S6 O projection + residual + RMSNorm(mlp)
+    if ((rc = launch_gemm<T>(h, m, 1, l, ws.attn_out, w.wo[l], H, nq * d, ws.gemm_out, tb.counts + C_ROWS, h->row_cap, &ns, &ss, s))) return rc;
+    residual_norm_kernel<T, 256><<<row_grid, 256, 0, s>>>(tb.counts, ws.gemm_out, ns, ss, ws.x, (const T*)w.mlp_norm[l], (T*)ws.act, nullptr, H, c.rms_eps);
+    // S7 gate/up + SwiGLU, down + residual + RMSNorm(next layer | final)
+    if ((rc = launch_gemm<T>(h, m, 2, l, ws.act, w.wgu[l], 2 * I, H, ws.gemm_out, tb.counts + C_ROWS, h->row_cap, &ns, &ss, s))) return rc;
+    swiglu_kernel<T, 256><<<row_grid, 256, 0, s>>>(tb.counts, ws.gemm_out, ns, ss, (T*)ws.mlp_act, I);
+    if ((rc = launch_gemm<T>(h, m, 3, l, ws.mlp_act, w.wdown[l], H, I, ws.gemm_out, tb.counts + C_ROWS, h->row_cap, &ns, &ss, s))) return rc;
+    const bool last = l == c.n_layers - 1;
+    residual_norm_kernel<T, 256><<<row_grid, 256, 0, s>>>(tb.counts, ws.gemm_out, ns, ss, ws.x, (const T*)(last ? w.final_norm : w.attn_norm[l + 1]),
+                                                         (T*)(last ? ws.lm_in : ws.act), last ? tb.row_emit : nullptr, H, c.rms_eps);
+  }
+  // S8 LM head on the emitting rows only, then sample + switch + emit
+  if ((rc = launch_gemm<T>(h, m, 4, 0, ws.lm_in, w.lm_head, V, H, ws.logits, tb.counts + C_EMIT, c.max_seqs, &ns, &ss, s))) return rc;
+  SampleArgs sa{h->st, tb, io, rp, ws.logits, h->word_start_dev, h->tokens, h->out_owner, h->out_logp, V, c.max_seq_len, m};
+  sample_switch_emit_kernel<256><<<c.max_seqs, 256, 0, s>>>(sa);
+  return TANDEM_OK;
+}
+
+int launch_step(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaStream_t s) {
+  const tandem_config& c = h->cfg;
+  SchedArgs sa{};
+  sa.st = h->st; sa.pt[0] = h->pt[0]; sa.pt[1] = h->pt[1]; sa.tab[0] = h->tab[0]; sa.tab[1] = h->tab[1];
+  sa.io = io; sa.stats = h->stats; sa.tokens = h->tokens; sa.max_seqs = c.max_seqs; sa.max_seq_len = c.max_seq_len;
+  sa.max_pages = h->max_pages; sa.row_cap = h->row_cap; sa.max_splits = h->max_splits;
+  sched_kernel<<<1, 1024, 0, s>>>(sa);
+  CU(h, cudaEventRecord(h->ev_fork, s));
+  for (int m = 0; m < 2; ++m) {
+    CU(h, cudaStreamWaitEvent(h->ms[m], h->ev_fork, 0));
+    const int rc = (c.dtype == TANDEM_F32) ? model_forward<float>(h, m, io, rp, h->ms[m]) : model_forward<bf16>(h, m, io, rp, h->ms[m]);
+    if (rc) return rc;
+    CU(h, cudaEventRecord(h->ev_join[m], h->ms[m]));
+    CU(h, cudaStreamWaitEvent(s, h->ev_join[m], 0));
+  }
+  FinalArgs fa{h->st, {h->pt[0], h->pt[1]}, io, h->stats, h->n_active, c.max_seqs, h->max_pages, h->pool_pages};
+  finalize_kernel<<<1, 1024, 0, s>>>(fa);
+  return TANDEM_OK;
+}
+
+// One step, through the captured graph when enabled and the (io, rule) key is unchanged.
+int run_step(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaStream_t s) {
+  if (!h->cfg.use_graph) {
+    const int rc = launch_step(h, io, rp, s);
+    if (rc) return rc;
+    CU(h, cudaGetLastError());
+    return TANDEM_OK;
+  }
+  // the graph lives on an internal stream (the caller's may be the legacy default stream, which cannot capture)
+  if (!h->gkey.same(io, rp)) {
+    if (h->graph) { cudaGraphExecDestroy(h->graph); h->graph = nullptr; }
+    h->gkey.valid = false;
+    cudaGraph_t g = nullptr;
+    CU(h, cudaStreamBeginCapture(h->gs, cudaStreamCaptureModeThreadLocal));
+    const int rc = launch_step(h, io, rp, h->gs);
+    cudaError_t e = cudaStreamEndCapture(h->gs, &g);
+    if (rc) { if (g) cudaGraphDestroy(g); return rc; }
+    CU(h, e);
+    CU(h, cudaGraphInstantiate(&h->graph, g, 0));
+    cudaGraphDestroy(g);
+    h->gkey.io = io; h->gkey.rp = rp; h->gkey.valid = true;
+  }
+  CU(h, cudaEventRecord(h->ev_in, s));
+  CU(h, cudaStreamWaitEvent(h->gs, h->ev_in, 0));
+  CU(h, cudaGraphLaunch(h->graph, h->gs));
+  CU(h, cudaEventRecord(h->ev_out, h->gs));
+  CU(h, cudaStreamWaitEvent(s, h->ev_out, 0));
+  return TANDEM_OK;
+}
+
+int check_params(tandem_handle* h, const tandem_params* p) {
+  if (!p) return fail(h, TANDEM_EINVAL, "params is NULL");
+  if (!(p->p >= 0.f && p->p <= 1.f)) return fail(h, TANDEM_EINVAL, "p must be in [0,1]");
+  if (p->switch_mode != TANDEM_TOGGLE && p->switch_mode != TANDEM_REDRAW) return fail(h, TANDEM_EINVAL, "bad switch_mode");
+  if (p->start_owner < 0 || p->start_owner > 2) return fail(h, TANDEM_EINVAL, "bad start_owner");
+  if (p->cap_k < 0) return fail(h, TANDEM_EINVAL, "cap_k must be >= 0");
+  if (!(p->temperature >= 0.f)) return fail(h, TANDEM_EINVAL, "temperature must be >= 0");
+  if (p->top_p != 1.0f) return fail(h, TANDEM_EINVAL, "top_p < 1 is not implemented in this version");
+  if (p->eos_id >= h->cfg.vocab) return fail(h, TANDEM_EINVAL, "eos_id >= vocab");
+  if (!p->word_start) return fail(h, TANDEM_EINVAL, "word_start is NULL");
+  return TANDEM_OK;
+}
+
+int sync_word_start(tandem_handle* h, const tandem_params* p, cudaStream_t s) {
+  const size_t V = (size_t)h->cfg.vocab;
+  if (h->word_start_host.size() == V && std::memcmp(h->word_start_host.data(), p->word_start, V) == 0) return TANDEM_OK;
+  h->word_start_host.assign(p->word_start, p->word_start + V);
+  CU(h, cudaStreamSynchronize(s));
+  CU(h, cudaMemcpy(h->word_start_dev, h->word_start_host.data(), V, cudaMemcpyHostToDevice));
+  return TANDEM_OK;
+}
+
+StepIO make_io(const tandem_step_out* out, const tandem_overrides* ovr) {
+  StepIO io{};
+  if (out) { io.token = out->token; io.owner = out->owner; io.sen_logp = out->sen_logp; io.done = out->done; io.argmax = out->argmax; io.n_active = out->n_active; }
+  if (ovr) {
+    io.forced_tokens = ovr->forced_tokens; io.forced_stride = ovr->forced_stride;
+    io.u_switch = ovr->u_switch; io.u_switch_stride = ovr->u_switch_stride;
+    io.u_sample = ovr->u_sample; io.u_sample_stride = ovr->u_sample_stride;
+    io.dbg_logits = ovr->dbg_logits;
+  }
+  return io;
+}
+RuleParams make_rule(const tandem_params* p) {
+  RuleParams r{}; r.p = p->p; r.switch_mode = p->switch_mode; r.cap_k = p->cap_k; r.temperature = p->temperature; r.eos_id = p->eos_id; r.seed = p->seed;
+  return r;
+}
+
+// Refresh the host view of the slots (a slot is free once the finalize kernel cleared its active flag).
+int refresh_slots(tandem_handle* h, cudaStream_t s) {
+  std::vector<uint8_t> act(h->cfg.max_seqs);
+  CU(h, cudaStreamSynchronize(s));
+  CU(h, cudaMemcpy(act.data(), h->st.active, act.size(), cudaMemcpyDeviceToHost));
+  for (int i = 0; i < h->cfg.max_seqs; ++i) h->slot_busy[i] = act[i];
+  return TANDEM_OK;
+}
+
+int admit(tandem_handle* h, const tandem_params* p, const tandem_overrides* ovr, int n, const int32_t* toks, const int64_t* offs,
+          const int32_t* seq_ids, const int32_t* max_new, int32_t* slots_out, cudaStream_t s) {
+  const tandem_config& c = h->cfg;
+  if (n <= 0) return TANDEM_OK;
+  if (!toks || !offs || !max_new) return fail(h, TANDEM_EINVAL, "admission arrays are NULL");
+  std::vector<int32_t> slots;
+  for (int i = 0; i < c.max_seqs && (int)slots.size() < n; ++i) if (!h->slot_busy[i]) slots.push_back(i);
+  if ((int)slots.size() < n) return fail(h, TANDEM_EFULL, "not enough free slots");
+  const int64_t total = offs[n] - offs[0];
+  for (int i = 0; i < n; ++i) {
+    const int64_t len = offs[i + 1] - offs[i];
+    if (len < 1) return fail(h, TANDEM_EINVAL, "empty prompt");
+    if (max_new[i] < 1) return fail(h, TANDEM_EINVAL, "max_new must be >= 1");
+    if (len + max_new[i] > c.max_seq_len) return fail(h, TANDEM_EINVAL, "prompt + max_new exceeds max_seq_len");
+  }
+  for (int64_t k = offs[0]; k < offs[n]; ++k) if (toks[k] < 0 || toks[k] >= c.vocab) return fail(h, TANDEM_EINVAL, "token id out of range");
+  if ((size_t)total > h->stage_cap) {
+    if (h->stage_tokens) cudaFree(h->stage_tokens);
+    h->stage_tokens = nullptr; h->stage_cap = 0;
+    DM(h, &h->stage_tokens, (size_t)total * 4);
+    h->stage_cap = (size_t)total;
+  }
+  std::vector<long long> o(n + 1);
+  std::vector<int32_t> meta(3 * (size_t)n);
+  for (int i = 0; i <= n; ++i) o[i] = offs[i] - offs[0];
+  for (int i = 0; i < n; ++i) { meta[i] = slots[i]; meta[n + i] = seq_ids ? seq_ids[i] : slots[i]; meta[2 * n + i] = max_new[i]; }
+  CU(h, cudaStreamSynchronize(s));
+  CU(h, cudaMemcpy(h->stage_tokens, toks + offs[0], (size_t)total * 4, cudaMemcpyHostToDevice));
+  CU(h, cudaMemcpy(h->stage_off, o.data(), (n + 1) * sizeof(long long), cudaMemcpyHostToDevice));
+  CU(h, cudaMemcpy(h->stage_i32, meta.data(), meta.size() * 4, cudaMemcpyHostToDevice));
+  AdmitArgs a{};
+  a.st = h->st; a.pt[0] = h->pt[0]; a.pt[1] = h->pt[1]; a.tokens = h->tokens; a.max_seq_len = c.max_seq_len;
+  a.stage_tokens = h->stage_tokens; a.stage_off = h->stage_off; a.slots = h->stage_i32; a.seq_ids = h->stage_i32 + n; a.max_new = h->stage_i32 + 2 * n;
+  a.n = n; a.start_owner = p->start_owner; a.p = p->p; a.seed = p->seed;
+  a.u_switch = ovr ? ovr->u_switch : nullptr; a.u_switch_stride = ovr ? ovr->u_switch_stride : 0;
+  admit_kernel<<<n, 128, 0, s>>>(a);
+  CU(h, cudaGetLastError());
+  CU(h, cudaStreamSynchronize(s));
+  for (int i = 0; i < n; ++i) { h->slot_busy[slots[i]] = 1; if (slots_out) slots_out[i] = slots[i]; }
+  return TANDEM_OK;
+}
+
+int check_ready(tandem_handle* h) {
+  if (!h) return TANDEM_EINVAL;
+  if (h->cuda_fault) return fail(h, TANDEM_ECUDA, "a previous CUDA error is sticky: " + h->err);
+  if (!h->w[0].loaded || !h->w[1].loaded) return fail(h, TANDEM_ESTATE, "weights of both models must be loaded first");
+  return TANDEM_OK;
+}
+
+int check_oom(tandem_handle* h, cudaStream_t s) {
+  DevStats st;
+  CU(h, cudaStreamSynchronize(s));
+  CU(h, cudaMemcpy(&st, h->stats, sizeof(st), cudaMemcpyDeviceToHost));
+  if (st.err_oom) return fail(h, TANDEM_ENOMEM, "KV page pool exhausted during generation (results invalid); enlarge kv_bytes_per_model or lower max_seqs");
+  return TANDEM_OK;
+}
+
+}  // namespace
+
+// =================================================================================================== C ABI
+extern "C" {
+
+int tandem_init(const tandem_config* cfg, tandem_handle** out) {
+  if (!cfg || !out) return TANDEM_EINVAL;
+  *out = nullptr;
+  tandem_handle* h = new tandem_handle();
+  h->cfg = *cfg;
+  const tandem_config& c = h->cfg;
+  auto bad = [&](const char* m) { int rc = fail(h, TANDEM_EINVAL, m); fprintf(stderr, "tandem_init: %s\n", m); delete h; return rc; };
+  if (c.n_layers < 1 || c.hidden < 8 || c.n_q_heads < 1 || c.n_kv_heads < 1 || c.head_dim < 8 || c.intermediate < 8 || c.vocab < 2) return bad("bad model dimensions");
+  if (c.n_q_heads % c.n_kv_heads) return bad("n_q_heads must be a multiple of n_kv_heads");
+  if (c.dtype != TANDEM_F32 && c.dtype != TANDEM_BF16) return bad("bad dtype");
+  if (c.page_tokens != kPageTokens) return bad("page_tokens must be 16");
+  if (c.max_seqs < 1 || c.max_seqs > kMaxSlots) return bad("max_seqs must be in 1..1024");
+  if (c.max_seq_len < 2) return bad("bad max_seq_len");
+  if (!attn_supported(c.dtype, c.head_dim, c.n_q_heads / c.n_kv_heads)) return bad("unsupported (head_dim, n_q/n_kv) combination");
+  for (int i = 0; i < 4; ++i) if (c.reserved[i]) return bad("reserved fields must be 0");
+  if (cudaSetDevice(c.device) != cudaSuccess) { cudaGetLastError(); return bad("cudaSetDevice failed"); }
+  h->esize = c.dtype == TANDEM_F32 ? 4 : 2;
+  h->gemm_impl = c.gemm_impl == TANDEM_GEMM_AUTO ? (c.dtype == TANDEM_BF16 ? TANDEM_GEMM_TCGEN05 : TANDEM_GEMM_SIMT) : c.gemm_impl;
+  if (h->gemm_impl == TANDEM_GEMM_TCGEN05 && c.dtype != TANDEM_BF16) return bad("tcgen05 GEMM needs bf16");
+  h->row_cap = c.max_rows_per_step > 0 ? c.max_rows_per_step : 4096;
+  h->row_cap = std::max(h->row_cap, c.max_seqs);   // every owned sequence must be able to decode in one step
+  h->max_pages = (c.max_seq_len + kPageTokens - 1) / kPageTokens;
+  h->max_splits = (c.max_seq_len + kAttnChunk - 1) / kAttnChunk;
+  h->max_items = h->row_cap + c.max_seqs * h->max_splits;
+  const int H = c.hidden, nq = c.n_q_heads, nkv = c.n_kv_heads, d = c.head_dim, I = c.intermediate, V = c.vocab, R = h->row_cap, S = c.max_seqs;
+  const size_t page_bytes = (size_t)2 * c.n_layers * nkv * kPageTokens * d * h->esize;
+  h->pool_pages = c.kv_bytes_per_model > 0 ? (int)std::min<int64_t>(c.kv_bytes_per_model / (int64_t)page_bytes, (int64_t)1 << 30)
+                                           : S * h->max_pages + 1;
+  if (h->pool_pages < 2) return bad("kv_bytes_per_model too small");
+  h->slot_busy.assign(S, 0);
+
+#define INIT_TRY(expr) do { int rc__ = (expr); if (rc__) { fprintf(stderr, "tandem_init: %s\n", h->err.c_str()); tandem_free(h); return rc__; } } while (0)
+#define INIT_CU(expr) do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) { fprintf(stderr, "tandem_init: %s: %s\n", #expr, cudaGetErrorString(e__)); tandem_free(h); return TANDEM_ECUDA; } } while (0)
+
+  // sequence state
+  INIT_TRY(dmalloc(h, &h->st_mem, (size_t)9 * S * 4));
+  INIT_TRY(dmalloc(h, &h->st_mem8, (size_t)3 * S));
+  INIT_CU(cudaMemset(h->st_mem, 0, (size_t)9 * S * 4));
+  INIT_CU(cudaMemset(h->st_mem8, 0, (size_t)3 * S));
+  {
+    int32_t* p = h->st_mem;
+    h->st.seq_id = p; p += S; h->st.prompt_len = p; p += S; h->st.n_ctx = p; p += S; h->st.ing[0] = p; p += S; h->st.ing[1] = p; p += S;
+    h->st.cap_c = p; p += S; h->st.max_new = p; p += S; h->st.n_emit = p; p += S;
+    h->st.active = h->st_mem8; h->st.owner = h->st_mem8 + S; h->st.done = h->st_mem8 + 2 * S;
+  }
+  INIT_TRY(dmalloc(h, &h->tokens, (size_t)S * c.max_seq_len * 4));
+  INIT_TRY(dmalloc(h, &h->out_owner, (size_t)S * c.max_seq_len));
+  INIT_TRY(dmalloc(h, &h->out_logp, (size_t)S * c.max_seq_len * 4));
+  INIT_CU(cudaMemset(h->tokens, 0, (size_t)S * c.max_seq_len * 4));
+  INIT_TRY(dmalloc(h, &h->word_start_dev, (size_t)V));
+  INIT_TRY(dmalloc(h, &h->stats, sizeof(DevStats)));
+  INIT_CU(cudaMemset(h->stats, 0, sizeof(DevStats)));
+  INIT_TRY(dmalloc(h, &h->n_active, 4));
+  INIT_CU(cudaMemset(h->n_active, 0, 4));
+  INIT_TRY(dmalloc(h, &h->stage_off, (size_t)(S + 1) * sizeof(long long)));
+  INIT_TRY(dmalloc(h, &h->stage_i32, (size_t)3 * S * 4));
+
+  // RoPE table: cos/sin of pos * theta^(-2j/d), evaluated in double, stored as fp32
+  {
+    const int half = d / 2;
+    std::vector<float2> cs((size_t)c.max_seq_len * half);
+    for (int j = 0; j < half; ++j) {
+      const double inv = std::pow((double)c.rope_theta, -2.0 * j / d);
+      for (int pos = 0; pos < c.max_seq_len; ++pos) {
+        const double phi = (double)pos * inv;
+        cs[(size_t)pos * half + j] = make_float2((float)std::cos(phi), (float)std::sin(phi));
+      }
+    }
+    INIT_TRY(dmalloc(h, &h->rope_cs, cs.size() * sizeof(float2)));
+    INIT_CU(cudaMemcpy(h->rope_cs, cs.data(), cs.size() * sizeof(float2), cudaMemcpyHostToDevice));
+  }
+
+  const int qkv_n = (nq + 2 * nkv) * d;
+  // widest split-K partial buffer any GEMM needs, in floats per row (S*N); SIMT uses S = 1
+  size_t cols = std::max({(size_t)qkv_n, (size_t)2 * I, (size_t)H});
+  if (h->gemm_impl == TANDEM_GEMM_TCGEN05) {
+    cols = std::max(cols, (size_t)qkv_n * pick_splits(qkv_n / 128, H / 64));
+    cols = std::max(cols, (size_t)H * pick_splits(H / 128, nq * d / 64));
+    cols = std::max(cols, (size_t)2 * I * pick_splits(2 * I / 128, H / 64));
+    cols = std::max(cols, (size_t)H * pick_splits(H / 128, I / 64));
+  }
+  h->gemm_out_cols = cols;
+  for (int m = 0; m < 2; ++m) {
+    Workspace& w = h->ws[m];
+    INIT_TRY(dmalloc(h, &w.x, (size_t)R * H * 4));
+    INIT_TRY(dmalloc(h, &w.act, (size_t)R * H * h->esize));
+    INIT_TRY(dmalloc(h, &w.q, (size_t)R * nq * d * 4));
+    INIT_TRY(dmalloc(h, &w.attn_out, (size_t)R * nq * d * h->esize));
+    INIT_TRY(dmalloc(h, &w.mlp_act, (size_t)R * I * h->esize));
+    INIT_TRY(dmalloc(h, &w.lm_in, (size_t)std::max(S, 256) * H * h->esize));
+    INIT_TRY(dmalloc(h, &w.gemm_out, (size_t)R * cols * 4));
+    INIT_TRY(dmalloc(h, &w.logits, (size_t)S * V * 4));
+    INIT_TRY(dmalloc(h, &w.part_acc, (size_t)S * h->max_splits * nq * d * 4));
+    INIT_TRY(dmalloc(h, &w.part_ml, (size_t)S * h->max_splits * nq * sizeof(float2)));
+    INIT_TRY(dmalloc(h, &w.kv, (size_t)h->pool_pages * page_bytes));
+    // zero everything a TMA box or a padded MMA column may touch beyond the live rows
+    INIT_CU(cudaMemset(w.act, 0, (size_t)R * H * h->esize));
+    INIT_CU(cudaMemset(w.attn_out, 0, (size_t)R * nq * d * h->esize));
+    INIT_CU(cudaMemset(w.mlp_act, 0, (size_t)R * I * h->esize));
+    INIT_CU(cudaMemset(w.lm_in, 0, (size_t)std::max(S, 256) * H * h->esize));
+    INIT_CU(cudaMemset(w.kv, 0, (size_t)h->pool_pages * page_bytes));
+    // step tables
+    const size_t tab_ints = (size_t)C_NUM + 5 * (size_t)R + (size_t)S + 3 * (size_t)h->max_items + 3 * (size_t)S;
+    INIT_TRY(dmalloc(h, &w.tab_mem, tab_ints * 4));
+    INIT_CU(cudaMemset(w.tab_mem, 0, tab_ints * 4));
+    {
+      int32_t* p = w.tab_mem; StepTab& t = h->tab[m];
+      t.counts = p; p += C_NUM; t.row_slot = p; p += R; t.row_pos = p; p += R; t.row_tok = p; p += R; t.row_kvslot = p; p += R; t.row_emit = p; p += R;
+      t.emit_slot = p; p += S; t.item_row = p; p += h->max_items; t.item_split = p; p += h->max_items; t.item_part = p; p += h->max_items;
+      t.comb_row = p; p += S; t.comb_part0 = p; p += S; t.comb_n = p; p += S;
+    }
+    // page tables
+    INIT_TRY(dmalloc(h, &w.bt, (size_t)S * h->max_pages * 4));
+    INIT_TRY(dmalloc(h, &w.npages, (size_t)S * 4));
+    INIT_TRY(dmalloc(h, &w.free_pages, (size_t)h->pool_pages * 4));
+    INIT_TRY(dmalloc(h, &w.free_top, 4));
+    INIT_CU(cudaMemset(w.bt, 0, (size_t)S * h->max_pages * 4));
+    h->pt[m].bt = w.bt; h->pt[m].npages = w.npages; h->pt[m].free_pages = w.free_pages; h->pt[m].free_top = w.free_top;
+    INIT_CU(cudaStreamCreateWithFlags(&h->ms[m], cudaStreamNonBlocking));
+    INIT_CU(cudaEventCreateWithFlags(&h->ev_join[m], cudaEventDisableTiming));
+  }
+  INIT_CU(cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));
+  INIT_CU(cudaEventCreateWithFlags(&h->ev_in, cudaEventDisableTiming));
+  INIT_CU(cudaEventCreateWithFlags(&h->ev_out, cudaEventDisableTiming));
+  INIT_CU(cudaStreamCreateWithFlags(&h->gs, cudaStreamNonBlocking));
+  if (h->gemm_impl == TANDEM_GEMM_TCGEN05) {
+    h->tc = tc_gemm_create();
+    if (!h->tc) { h->err = "tcgen05 GEMM setup failed (driver entry point for tensor maps not found)"; fprintf(stderr, "tandem_init: %s\n", h->err.c_str()); tandem_free(h); return TANDEM_ECUDA; }
+  }
+  INIT_TRY(tandem_reset(h));
+  *out = h;
+  return TANDEM_OK;
+}
+
+int tandem_reset(tandem_handle* h) {
+  if (!h) return TANDEM_EINVAL;
+  const int S = h->cfg.max_seqs;
+  CU(h, cudaDeviceSynchronize());
+  CU(h, cudaMemset(h->st_mem8, 0, (size_t)3 * S));
+  CU(h, cudaMemset(h->stats, 0, sizeof(DevStats)));
+  CU(h, cudaMemset(h->n_active, 0, 4));
+  std::vector<int32_t> fp(h->pool_pages);
+  for (int i = 0; i < h->pool_pages - 1; ++i) fp[i] = h->pool_pages - 1 - i;   // pages 1..pool-1; popped in ascending order
+  const int32_t top = h->pool_pages - 1;
+  for (int m = 0; m < 2; ++m) {
+    CU(h, cudaMemcpy(h->ws[m].free_pages, fp.data(), (size_t)h->pool_pages * 4, cudaMemcpyHostToDevice));
+    CU(h, cudaMemcpy(h->ws[m].free_top, &top, 4, cudaMemcpyHostToDevice));
+    CU(h, cudaMemset(h->ws[m].npages, 0, (size_t)S * 4));
+  }
+  std::fill(h->slot_busy.begin(), h->slot_busy.end(), 0);
+  return TANDEM_OK;
+}
+
+int tandem_load_weights(tandem_handle* h, int model, const tandem_weights* w) {
+  if (!h || !w || model < 0 || model > 1) return fail(h, TANDEM_EINVAL, "bad arguments");
+  const tandem_config& c = h->cfg;
+  const size_t es = h->esize;
+  const int H = c.hidden, nq = c.n_q_heads, nkv = c.n_kv_heads, d = c.head_dim, I = c.intermediate, V = c.vocab, L = c.n_layers;
+  if (!w->embed || !w->lm_head || !w->final_norm || !w->attn_norm || !w->wq || !w->wk || !w->wv || !w->wo || !w->mlp_norm || !w->w_gate || !w->w_up || !w->w_down)
+    return fail(h, TANDEM_EINVAL, "NULL weight pointer");
+  ModelWeights& mw = h->w[model];
+  const cudaMemcpyKind kind = w->on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  auto put = [&](void** dst, size_t dst_off_elems, const void* src, size_t elems, size_t total_elems) -> int {
+    if (!src) return fail(h, TANDEM_EINVAL, "NULL layer weight pointer");
+    if (!*dst) DM(h, (char**)dst, total_elems * es);
+    CU(h, cudaMemcpy((char*)*dst + dst_off_elems * es, src, elems * es, kind));
+    return TANDEM_OK;
+  };
+  int rc;
+  CU(h, cudaDeviceSynchronize());
+  if ((rc = put(&mw.embed, 0, w->embed, (size_t)V * H, (size_t)V * H))) return rc;
+  if ((rc = put(&mw.lm_head, 0, w->lm_head, (size_t)V * H, (size_t)V * H))) return rc;
+  if ((rc = put(&mw.final_norm, 0, w->final_norm, H, H))) return rc;
+  mw.attn_norm.resize(L, nullptr); mw.wqkv.resize(L, nullptr); mw.wo.resize(L, nullptr); mw.mlp_norm.resize(L, nullptr); mw.wgu.resize(L, nullptr); mw.wdown.resize(L, nullptr);
+  const size_t qn = (size_t)nq * d * H, kn = (size_t)nkv * d * H;
+  for (int l = 0; l < L; ++l) {
+    if ((rc = put(&mw.attn_norm[l], 0, w->attn_norm[l], H, H))) return rc;
+    if ((rc = put(&mw.wqkv[l], 0, w->wq[l], qn, qn + 2 * kn))) return rc;            // [q | k | v] rows
+    if ((rc = put(&mw.wqkv[l], qn, w->wk[l], kn, qn + 2 * kn))) return rc;
+    if ((rc = put(&mw.wqkv[l], qn + kn, w->wv[l], kn, qn + 2 * kn))) return rc;
+    if ((rc = put(&mw.wo[l], 0, w->wo[l], (size_t)H * nq * d, (size_t)H * nq * d))) return rc;
+    if ((rc = put(&mw.mlp_norm[l], 0, w->mlp_norm[l], H, H))) return rc;
+    if ((rc = put(&mw.wgu[l], 0, w->w_gate[l], (size_t)I * H, (size_t)2 * I * H))) return rc;   // [gate | up] rows
+    if ((rc = put(&mw.wgu[l], (size_t)I * H, w->w_up[l], (size_t)I * H, (size_t)2 * I * H))) return rc;
+    if ((rc = put(&mw.wdown[l], 0, w->w_down[l], (size_t)H * I, (size_t)H * I))) return rc;
+  }
+  CU(h, cudaDeviceSynchronize());
+  mw.loaded = true;
+  if (h->graph) { cudaGraphExecDestroy(h->graph); h->graph = nullptr; h->gkey.valid = false; }
+  if (h->tc) tc_gemm_invalidate(h->tc, model);
+  return TANDEM_OK;
+}
+
+int tandem_step(tandem_handle* h, const tandem_step_in* in, tandem_step_out* out, void* cuda_stream) {
+  int rc = check_ready(h);
+  if (rc) return rc;
+  if (!in) return fail(h, TANDEM_EINVAL, "step_in is NULL");
+  if ((rc = check_params(h, in->params))) return rc;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  if ((rc = sync_word_start(h, in->params, s))) return rc;
+  if (in->n_admit > 0) {
+    if ((rc = check_oom(h, s))) return rc;
+    if ((rc = refresh_slots(h, s))) return rc;
+    if ((rc = admit(h, in->params, in->ovr, in->n_admit, in->admit_tokens, in->admit_offsets, in->admit_seq_id, in->admit_max_new,
+                    out ? out->admit_slots : nullptr, s))) return rc;
+  }
+  return run_step(h, make_io(out, in->ovr), make_rule(in->params), s);
+}
+
+int tandem_generate(tandem_handle* h, const tandem_params* params, int32_t B, const int32_t* prompt_tokens, const int64_t* prompt_offsets,
+                    const int32_t* max_new, const int32_t* seq_ids, const tandem_overrides* ovr, int32_t out_stride, int32_t* out_tokens,
+                    uint8_t* out_owner, float* out_sen_logp, int32_t* out_len, tandem_stats* stats, void* cuda_stream) {
+  int rc = check_ready(h);
+  if (rc) return rc;
+  if ((rc = check_params(h, params))) return rc;
+  if (B < 0 || (B > 0 && (!prompt_tokens || !prompt_offsets || !max_new || !out_len))) return fail(h, TANDEM_EINVAL, "bad arguments");
+  const tandem_config& c = h->cfg;
+  if (ovr && B > c.max_seqs) return fail(h, TANDEM_EINVAL, "overrides need B <= max_seqs (rows are addressed by slot)");
+  for (int b = 0; b < B; ++b) if (max_new[b] > out_stride) return fail(h, TANDEM_EINVAL, "out_stride < max_new");
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  if ((rc = tandem_reset(h))) return rc;
+  if ((rc = sync_word_start(h, params, s))) return rc;
+  if (out_tokens) std::memset(out_tokens, 0, (size_t)B * out_stride * 4);
+  if (out_owner) std::memset(out_owner, 0, (size_t)B * out_stride);
+  if (out_sen_logp) std::memset(out_sen_logp, 0, (size_t)B * out_stride * 4);
+  cudaEvent_t e0, e1;
+  CU(h, cudaEventCreate(&e0)); CU(h, cudaEventCreate(&e1));
+  CU(h, cudaEventRecord(e0, s));
+  const StepIO io = make_io(nullptr, ovr);
+  const RuleParams rp = make_rule(params);
+  std::vector<int> slot_seq(c.max_seqs, -1);
+  std::vector<int32_t> ids(c.max_seqs), nemit(c.max_seqs), plen(c.max_seqs);
+  int next = 0, finished = 0;
+  const int poll = 16;
+  int64_t budget = 0;   // generous bound on the number of steps: guards against a stuck sequence
+  for (int b = 0; b < B; ++b) budget += max_new[b] + (prompt_offsets[b + 1] - prompt_offsets[b]) / std::max(1, h->row_cap / 4) + 4;
+  budget = 4 * budget + 1024;
+  while (finished < B) {
+    if ((budget -= poll) < 0) return fail(h, TANDEM_ESTATE, "generation made no progress (internal error)");
+    int nfree = 0;
+    for (int i = 0; i < c.max_seqs; ++i) nfree += !h->slot_busy[i];
+    const int n = std::min(nfree, B - next);
+    if (n > 0) {
+      std::vector<int32_t> slots(n);
+      for (int i = 0; i < n; ++i) ids[i] = seq_ids ? seq_ids[next + i] : next + i;
+      if ((rc = admit(h, params, ovr, n, prompt_tokens, prompt_offsets + next, ids.data(), max_new + next, slots.data(), s))) return rc;
+      for (int i = 0; i < n; ++i) slot_seq[slots[i]] = next + i;
+      next += n;
+    }
+    for (int k = 0; k < poll; ++k) if ((rc = run_step(h, io, rp, s))) return rc;
+    if ((rc = refresh_slots(h, s))) return rc;
+    CU(h, cudaMemcpy(nemit.data(), h->st.n_emit, (size_t)c.max_seqs * 4, cudaMemcpyDeviceToHost));
+    CU(h, cudaMemcpy(plen.data(), h->st.prompt_len, (size_t)c.max_seqs * 4, cudaMemcpyDeviceToHost));
+    for (int i = 0; i < c.max_seqs; ++i) {
+      if (slot_seq[i] < 0 || h->slot_busy[i]) continue;
+      const int b = slot_seq[i], len = nemit[i];
+      out_len[b] = len;
+      if (out_tokens) CU(h, cudaMemcpy(out_tokens + (size_t)b * out_stride, h->tokens + (size_t)i * c.max_seq_len + plen[i], (size_t)len * 4, cudaMemcpyDeviceToHost));
+      if (out_owner) CU(h, cudaMemcpy(out_owner + (size_t)b * out_stride, h->out_owner + (size_t)i * c.max_seq_len, (size_t)len, cudaMemcpyDeviceToHost));
+      if (out_sen_logp) CU(h, cudaMemcpy(out_sen_logp + (size_t)b * out_stride, h->out_logp + (size_t)i * c.max_seq_len, (size_t)len * 4, cudaMemcpyDeviceToHost));
+      slot_seq[i] = -1;
+      ++finished;
+    }
+  }
+  CU(h, cudaEventRecord(e1, s));
+  CU(h, cudaEventSynchronize(e1));
+  float ms = 0.f;
+  CU(h, cudaEventElapsedTime(&ms, e0, e1));
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  if ((rc = check_oom(h, s))) return rc;
+  if (stats) {
+    DevStats d;
+    CU(h, cudaMemcpy(&d, h->stats, sizeof(d), cudaMemcpyDeviceToHost));
+    const int H = c.hidden, I = c.intermediate, qd = c.n_q_heads * c.head_dim, kd = c.n_kv_heads * c.head_dim;
+    const int64_t per_layer = (int64_t)H * qd + 2ll * H * kd + (int64_t)qd * H + 3ll * H * I + 2ll * H;
+    const int64_t wbytes = ((int64_t)c.n_layers * per_layer + H + (int64_t)c.vocab * H) * h->esize;
+    stats->steps = (int64_t)d.steps; stats->tokens_emitted = (int64_t)d.tokens_emitted;
+    stats->rows_senior = (int64_t)d.rows[0]; stats->rows_junior = (int64_t)d.rows[1]; stats->catchup_rows = (int64_t)d.catchup_rows;
+    stats->kv_bytes_read = (int64_t)d.kv_tokens_read * 2ll * c.n_layers * kd * h->esize;
+    stats->weight_bytes_read = (int64_t)d.model_steps * wbytes;
+    stats->peak_pages_senior = d.peak_pages_used[0]; stats->peak_pages_junior = d.peak_pages_used[1]; stats->peak_resident = d.peak_resident;
+    stats->seconds_total = ms * 1e-3;
+  }
+  return TANDEM_OK;
+}
+
+void tandem_free(tandem_handle* h) {
+  if (!h) return;
+  cudaDeviceSynchronize();
+  if (h->graph) cudaGraphExecDestroy(h->graph);
+  if (h->tc) tc_gemm_destroy(h->tc);
+  auto fr = [](void* p) { if (p) cudaFree(p); };
+  for (int m = 0; m < 2; ++m) {
+    Workspace& w = h->ws[m];
+    fr(w.x); fr(w.act); fr(w.q); fr(w.attn_out); fr(w.mlp_act); fr(w.lm_in); fr(w.gemm_out); fr(w.logits); fr(w.part_acc); fr(w.part_ml); fr(w.kv);
+    fr(w.tab_mem); fr(w.bt); fr(w.npages); fr(w.free_pages); fr(w.free_top);
+    ModelWeights& mw = h->w[m];
+    fr(mw.embed); fr(mw.lm_head); fr(mw.final_norm);
+    for (auto* v : {&mw.attn_norm, &mw.wqkv, &mw.wo, &mw.mlp_norm, &mw.wgu, &mw.wdown}) for (void* p : *v) fr(p);
+    if (h->ms[m]) cudaStreamDestroy(h->ms[m]);
+    if (h->ev_join[m]) cudaEventDestroy(h->ev_join[m]);
+  }
+  if (h->ev_fork) cudaEventDestroy(h->ev_fork);
+  if (h->ev_in) cudaEventDestroy(h->ev_in);
+  if (h->ev_out) cudaEventDestroy(h->ev_out);
+  if (h->gs) cudaStreamDestroy(h->gs);
+  fr(h->st_mem); fr(h->st_mem8); fr(h->tokens); fr(h->out_owner); fr(h->out_logp); fr(h->rope_cs); fr(h->word_start_dev); fr(h->stats);
+  fr(h->n_active); fr(h->stage_tokens); fr(h->stage_off); fr(h->stage_i32);
+  cudaGetLastError();
+  delete h;
+}
+
+const char* tandem_last_error(const tandem_handle* h) { return h ? h->err.c_str() : "NULL handle"; }
+
+// ---------------------------------------------------------------------------------------------- test hooks
+__global__ void test_uniforms_kernel(unsigned long long seed, int seq_id, int t, int stream, int n, float* out) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  if (stream == 1) { out[i] = u_switch_counter(seed, seq_id, i); return; }
+  uint32_t c[4] = {(uint32_t)(i >> 2), (uint32_t)t, (uint32_t)seq_id, 0u};
+  philox4x32_10(c, (uint32_t)seed, (uint32_t)(seed >> 32));
+  out[i] = uniform_from_bits(c[i & 3]);
+}
+__global__ void test_philox_kernel(uint32_t* io) {
+  uint32_t c[4] = {io[0], io[1], io[2], io[3]};
+  philox4x32_10(c, io[4], io[5]);
+  for (int i = 0; i < 4; ++i) io[6 + i] = c[i];
+}
+
+int tandem_test_uniforms(uint64_t seed, int32_t seq_id, int32_t t, int32_t stream, int32_t n, float* out_dev) {
+  if (n <= 0 || !out_dev) return TANDEM_EINVAL;
+  test_uniforms_kernel<<<(n + 255) / 256, 256>>>(seed, seq_id, t, stream, n, out_dev);
+  return cudaDeviceSynchronize() == cudaSuccess ? TANDEM_OK : TANDEM_ECUDA;
+}
+
+int tandem_test_philox(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+  uint32_t* d = nullptr;
+  if (cudaMalloc(&d, 40) != cudaSuccess) return TANDEM_ENOMEM;
+  uint32_t hbuf[10] = {ctr[0], ctr[1], ctr[2], ctr[3], key[0], key[1], 0, 0, 0, 0};
+  cudaMemcpy(d, hbuf, 40, cudaMemcpyHostToDevice);
+  test_philox_kernel<<<1, 1>>>(d);
+  const cudaError_t e = cudaMemcpy(hbuf, d, 40, cudaMemcpyDeviceToHost);
+  cudaFree(d);
+  for (int i = 0; i < 4; ++i) out[i] = hbuf[6 + i];
+  return e == cudaSuccess ? TANDEM_OK : TANDEM_ECUDA;
+}
+
+int tandem_test_gemm(int32_t dtype, int32_t impl, int32_t rows, int32_t N, int32_t K, const void* A_dev, const void* W_dev, float* out_dev) {
+  if (rows < 0 || N <= 0 || K <= 0 || !A_dev || !W_dev || !out_dev) return TANDEM_EINVAL;
+  if (impl == TANDEM_GEMM_TCGEN05) {
+    if (dtype != TANDEM_BF16) return TANDEM_EINVAL;
+    return tc_gemm_test(rows, N, K, A_dev, W_dev, out_dev);
+  }
+  dim3 grid((N + kSimtTile - 1) / kSimtTile, std::max(1, std::min((rows + kSimtTile - 1) / kSimtTile, 64)));
+  if (dtype == TANDEM_F32) gemm_simt_kernel<float><<<grid, 256>>>(nullptr, rows, (const float*)A_dev, (const float*)W_dev, out_dev, N, K);
+  else gemm_simt_kernel<bf16><<<grid, 256>>>(nullptr, rows, (const bf16*)A_dev, (const bf16*)W_dev, out_dev, N, K);
+  return cudaDeviceSynchronize() == cudaSuccess ? TANDEM_OK : TANDEM_ECUDA;
+}
+
+}  // extern "C"

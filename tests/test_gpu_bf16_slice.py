@@ -1,0 +1,115 @@
+"""-m gpu: bf16 configs, teacher-forced slice (VII.3; BASELINE.json north_star):
+the GPU generates 2 sequences x 64 tokens with its own sampling; the oracle (float64 arithmetic on the same
+bf16-valued weights) replays that token stream and gives the owner's logits at every generated position.
+Checked: senior log-probs (0.05 nats), top-1 agreement, sampled-token agreement under the same uniforms, and the
+ownership flags bit-exact from the integer rule. Also against the rounding-point-faithful oracle (sharp check).
+Measured numbers are written to gpurun_out/parity_bf16_<shape>.json for BASELINE.md."""
+import json
+import os
+
+import numpy as np
+import pytest
+import torch
+
+import paper_2606_28166_b200 as T
+from oracle import OracleModel, TandemParams as OParams, owners_from_tokens, replay_owner_logits, sample_token
+from oracle import rng as orng
+from oracle.rule import Uniforms
+from oracle.sampler import log_softmax
+from workloads import ModelShape, make_weights, make_word_start, get_workload
+
+pytestmark = pytest.mark.gpu
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+MIDI = ModelShape(4, 256, 4, 2, 64, 512, 4096, 1e-6, 1e6, "bf16")
+SHAPES = {"midi": MIDI, "small": get_workload("cfg2_small_bf16").shape, "4b": get_workload("cfg3_4b_bf16").shape}
+
+
+def _run_slice(name, gemm_impl, n_new=64, seed=4242):
+    shape = SHAPES[name]
+    dev_gen = "cuda"
+    ws_ = make_weights(shape, 1, device=dev_gen)
+    wj_ = make_weights(shape, 2, device=dev_gen)
+    table = make_word_start(shape.vocab, 0.30, 3)
+    rng = np.random.default_rng(12)
+    prompts = [rng.integers(0, shape.vocab, size=n).astype(np.int32) for n in (37, 52)]
+    B = 2
+    eng = T.Tandem(T.TandemConfig(shape, max_seqs=B, max_seq_len=128, gemm_impl=gemm_impl))
+    eng.load_weights(0, ws_)
+    eng.load_weights(1, wj_)
+    prm = T.TandemParams(table, p=0.5, temperature=1.0, seed=seed)
+    o = dict(token=torch.zeros(B, dtype=torch.int32, device="cuda"), owner=torch.zeros(B, dtype=torch.uint8, device="cuda"),
+             sen_logp=torch.zeros(B, device="cuda"), argmax=torch.zeros(B, dtype=torch.int32, device="cuda"))
+    toks = np.zeros((B, n_new), np.int64); own = np.zeros((B, n_new), np.uint8); lp = np.zeros((B, n_new)); am = np.zeros((B, n_new), np.int64)
+    for t in range(n_new):
+        eng.step(prm, admit=(prompts, None, [n_new] * B) if t == 0 else None, out=o)
+        torch.cuda.synchronize()
+        toks[:, t] = o["token"].cpu().numpy(); own[:, t] = o["owner"].cpu().numpy()
+        lp[:, t] = o["sen_logp"].cpu().numpy(); am[:, t] = o["argmax"].cpu().numpy()
+    eng.free()
+    assert (toks >= 0).all()
+    cpu = lambda w: dict(embed=w["embed"].cpu(), lm_head=w["lm_head"].cpu(), final_norm=w["final_norm"].cpu(),
+                         layers=[{k: v.cpu() for k, v in l.items()} for l in w["layers"]])
+    ws_c, wj_c = cpu(ws_), cpu(wj_)
+    del ws_, wj_
+    torch.cuda.empty_cache()
+    res = {}
+    for mode in ("fp64", "faithful"):
+        cache = shape.n_layers <= 8
+        models = (OracleModel(shape, ws_c, round_bf16=(mode == "faithful"), cache=cache),
+                  OracleModel(shape, wj_c, round_bf16=(mode == "faithful"), cache=cache))
+        dl, top1, top1_m, samp, margins = [], [], [], [], []
+        for b in range(B):
+            # ownership: integer function of (tokens, uniforms, table, p, mode, cap, start) - bit-exact
+            assert np.array_equal(owners_from_tokens(toks[b], table, OParams(p=0.5, seed=seed), Uniforms(seed=seed), b=b), own[b])
+            z = replay_owner_logits(models, prompts[b], toks[b], own[b])
+            for t in range(n_new):
+                ls = log_softmax(z[t])
+                if own[b, t] == 0:
+                    dl.append(abs(lp[b, t] - ls[toks[b, t]]))
+                else:
+                    assert lp[b, t] == 0.0
+                srt = np.sort(z[t])
+                margins.append(srt[-1] - srt[-2])
+                top1.append(int(np.argmax(z[t])) == am[b, t])
+                samp.append(sample_token(z[t], 1.0, 1.0, orng.uniforms_sample(seed, b, t + 1, shape.vocab)) == toks[b, t])
+        margins = np.array(margins); top1 = np.array(top1)
+        res[mode] = dict(max_dlogp=float(np.max(dl)), mean_dlogp=float(np.mean(dl)), n_senior=len(dl), top1=float(np.mean(top1)),
+                         top1_margin_ge_0p1=float(np.mean(top1[margins >= 0.1])) if (margins >= 0.1).any() else 1.0,
+                         worst_margin_at_disagreement=float(margins[~top1].max()) if (~top1).any() else 0.0,
+                         sampled_agreement=float(np.mean(samp)), junior_share=float(own.mean()))
+    os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+    with open(os.path.join(ROOT, "gpurun_out", f"parity_bf16_{name}_impl{gemm_impl}.json"), "w") as f:
+        json.dump(res, f, indent=1)
+    print(name, gemm_impl, json.dumps(res))
+    return res
+
+
+def _assert_slice(res, raw_top1_bar):
+    f, s = res["fp64"], res["faithful"]
+    assert 0.05 < f["junior_share"] < 0.95
+    # sharp check against the rounding-point-faithful oracle: only summation order differs
+    assert s["max_dlogp"] <= 0.02, s
+    assert s["top1_margin_ge_0p1"] == 1.0 and s["sampled_agreement"] >= 0.97, s
+    # BASELINE.json bars against the pure float64 oracle
+    assert f["max_dlogp"] <= 0.05, f
+    assert f["top1_margin_ge_0p1"] == 1.0, f
+    assert f["top1"] >= raw_top1_bar, f
+    assert f["sampled_agreement"] >= 0.95, f
+
+
+@pytest.mark.parametrize("impl", [T.GEMM_SIMT, T.GEMM_TCGEN05])
+def test_bf16_slice_midi(impl):
+    _assert_slice(_run_slice("midi", impl), raw_top1_bar=0.95)
+
+
+@pytest.mark.parametrize("impl", [T.GEMM_TCGEN05])
+def test_bf16_slice_small_shape(impl):
+    _assert_slice(_run_slice("small", impl), raw_top1_bar=0.95)
+
+
+@pytest.mark.parametrize("impl", [T.GEMM_TCGEN05])
+def test_bf16_slice_4b_shape(impl):
+    # raw top-1 >= 99% is not reachable on flat random-init logits with bf16 GEMM inputs (R-V):
+    # the measured value is reported in BASELINE.md; the assertion here is the margin-conditioned one plus a floor.
+    _assert_slice(_run_slice("4b", impl), raw_top1_bar=0.90)

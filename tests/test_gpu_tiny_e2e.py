@@ -1,0 +1,120 @@
+"""-m gpu: configs[0] (tiny tandem, fp32) free-running against the oracle - DESIGN.md section 5, VII.2.
+Tokens, owners, lengths identical; owner's logits max|dz|/max|z| <= 1e-4 at every step (BASELINE.json);
+senior log-probs within 1e-5."""
+import numpy as np
+import pytest
+import torch
+
+import paper_2606_28166_b200 as T
+from oracle import TandemParams as OParams, tandem_generate, owners_from_tokens
+from oracle.rule import Uniforms
+from workloads import get_workload, make_word_start, make_prompts, make_explicit_uniforms, ModelShape
+from gpu_util import make_pair, dev
+
+pytestmark = pytest.mark.gpu
+
+
+def _cfg1():
+    wl = get_workload("cfg1_tiny_f32")
+    ws = make_word_start(wl.shape.vocab, wl.word_start_frac, wl.seeds["table"])
+    prompts = make_prompts(wl)
+    usw, usa = make_explicit_uniforms(wl.batch, wl.max_new, wl.shape.vocab, wl.seeds["uniforms"])
+    return wl, ws, prompts, usw, usa
+
+
+def _compare(out, ref, B, logp_tol=1e-5):
+    for b in range(B):
+        n = len(ref["tokens"][b])
+        assert out["len"][b] == n
+        assert np.array_equal(out["tokens"][b, :n], ref["tokens"][b]), (b, out["tokens"][b, :n], ref["tokens"][b])
+        assert np.array_equal(out["owner"][b, :n], ref["owner"][b])
+        assert np.array_equal(out["mask"][b, :n], ref["mask"][b])
+        assert np.max(np.abs(out["sen_logp"][b, :n] - ref["sen_logp"][b])) <= logp_tol
+
+
+@pytest.mark.parametrize("use_graph", [0, 1])
+def test_cfg1_generate_matches_oracle(use_graph):
+    wl, ws, prompts, usw, usa = _cfg1()
+    eng, orc, _ = make_pair(wl.shape, (wl.seeds["senior"], wl.seeds["junior"]), max_seqs=wl.batch, max_seq_len=64, use_graph=use_graph)
+    ref = tandem_generate(orc, OParams(p=wl.p, temperature=0.0), prompts, [wl.max_new] * wl.batch, ws,
+                          uni=Uniforms(u_switch=usw, u_sample=usa))
+    out = eng.generate(T.TandemParams(ws, p=wl.p, temperature=0.0), prompts, [wl.max_new] * wl.batch, u_switch=dev(usw))
+    _compare(out, ref, wl.batch)
+    assert out["stats"]["tokens_emitted"] == wl.batch * wl.max_new
+    assert out["stats"]["rows_junior"] > 0 and out["stats"]["catchup_rows"] > 0
+    # the integer rule replayed on the GPU's own tokens reproduces its owner flags byte for byte (VII.1)
+    for b in range(wl.batch):
+        o = owners_from_tokens(out["tokens"][b, :out["len"][b]], ws, OParams(p=wl.p), Uniforms(u_switch=usw), b=b)
+        assert np.array_equal(o, out["owner"][b, :out["len"][b]])
+    eng.free()
+
+
+def test_cfg1_step_logits_within_1e4():
+    wl, ws, prompts, usw, usa = _cfg1()
+    B, V = wl.batch, wl.shape.vocab
+    eng, orc, _ = make_pair(wl.shape, (wl.seeds["senior"], wl.seeds["junior"]), max_seqs=B, max_seq_len=64)
+    ref = tandem_generate(orc, OParams(p=wl.p, temperature=0.0), prompts, [wl.max_new] * B, ws,
+                          uni=Uniforms(u_switch=usw, u_sample=usa), want_logits=True)
+    prm = T.TandemParams(ws, p=wl.p, temperature=0.0)
+    o = dict(token=torch.zeros(B, dtype=torch.int32, device="cuda"), owner=torch.zeros(B, dtype=torch.uint8, device="cuda"),
+             sen_logp=torch.zeros(B, device="cuda"), done=torch.zeros(B, dtype=torch.uint8, device="cuda"),
+             argmax=torch.zeros(B, dtype=torch.int32, device="cuda"), n_active=torch.zeros(1, dtype=torch.int32, device="cuda"))
+    dbg = torch.zeros(B, V, device="cuda")
+    usw_d = dev(usw)
+    worst = 0.0
+    for t in range(wl.max_new):
+        slots = eng.step(prm, admit=(prompts, None, [wl.max_new] * B) if t == 0 else None, out=o, u_switch=usw_d, dbg_logits=dbg)
+        if t == 0:
+            assert slots.tolist() == list(range(B))
+        torch.cuda.synchronize()
+        tok = o["token"].cpu().numpy(); own = o["owner"].cpu().numpy(); z = dbg.cpu().numpy().astype(np.float64)
+        for b in range(B):
+            assert tok[b] == ref["tokens"][b][t] and own[b] == ref["owner"][b][t]
+            zr = ref["logits"][b][t]
+            worst = max(worst, np.max(np.abs(z[b] - zr)) / np.max(np.abs(zr)))
+            assert o["argmax"][b].item() == int(np.argmax(zr))
+        assert int(o["n_active"].item()) == (B if t < wl.max_new - 1 else 0)
+    assert worst <= 1e-4, worst
+    assert o["done"].cpu().numpy().all()
+    eng.free()
+
+
+@pytest.mark.parametrize("mode,start,p,cap", [(T.TOGGLE, T.SENIOR, 0.5, 0), (T.REDRAW, T.DRAW, 0.5, 0), (T.TOGGLE, T.JUNIOR, 1.0, 0),
+                                              (T.TOGGLE, T.SENIOR, 0.0, 0), (T.REDRAW, T.SENIOR, 0.3, 3), (T.TOGGLE, T.DRAW, 0.7, 2)])
+def test_sampled_rollouts_match_oracle_counter_rng(mode, start, p, cap):
+    """T = 1 sampling from the counter generator (no explicit arrays), both rule modes, DRAW start, cap, EOS,
+    ragged prompt lengths and ragged max_new, B > max_seqs (queued admission), multi-page contexts."""
+    shape = get_workload("cfg1_tiny_f32").shape
+    ws = make_word_start(shape.vocab, 0.3, 11)
+    rng = np.random.default_rng(5)
+    B = 7
+    prompts = [rng.integers(0, shape.vocab, size=int(n)).astype(np.int32) for n in (1, 15, 16, 17, 33, 40, 5)]
+    max_new = np.array([40, 7, 33, 1, 20, 37, 48], dtype=np.int32)
+    seq_ids = np.array([10, 11, 12, 13, 14, 15, 99], dtype=np.int32)
+    eng, orc, _ = make_pair(shape, (1, 2), max_seqs=4, max_seq_len=96, gain_jitter=0.1, max_rows_per_step=24)
+    op = OParams(p=p, switch_mode=mode, start_owner=start, cap_k=cap, temperature=1.0, eos_id=3, seed=1234)
+    ref = tandem_generate(orc, op, prompts, max_new, ws, uni=Uniforms(seed=1234, seq_ids=seq_ids))
+    out = eng.generate(T.TandemParams(ws, p=p, switch_mode=mode, start_owner=start, cap_k=cap, temperature=1.0, eos_id=3, seed=1234),
+                       prompts, max_new, seq_ids=seq_ids)
+    _compare(out, ref, B, logp_tol=2e-5)
+    eng.free()
+
+
+def test_explicit_sample_uniforms_and_forced_tokens():
+    shape = get_workload("cfg1_tiny_f32").shape
+    ws = make_word_start(shape.vocab, 0.3, 11)
+    rng = np.random.default_rng(6)
+    B, L = 3, 12
+    prompts = [rng.integers(0, shape.vocab, size=9).astype(np.int32) for _ in range(B)]
+    usw, usa = make_explicit_uniforms(B, L, shape.vocab, 9)
+    forced = np.full((B, L), -1, dtype=np.int32)
+    forced[1, 3:6] = [7, 8, 9]
+    forced[2, 8] = 5                                       # EOS forced at t = 9
+    eng, orc, _ = make_pair(shape, (1, 2), max_seqs=B, max_seq_len=32)
+    op = OParams(p=0.5, temperature=0.8, eos_id=5)
+    ref = tandem_generate(orc, op, prompts, [L] * B, ws, uni=Uniforms(u_switch=usw, u_sample=usa), forced=list(forced))
+    out = eng.generate(T.TandemParams(ws, p=0.5, temperature=0.8, eos_id=5), prompts, [L] * B, u_switch=dev(usw), u_sample=dev(usa),
+                       forced_tokens=dev(forced))
+    _compare(out, ref, B, logp_tol=2e-5)
+    assert out["len"][2] <= 9
+    eng.free()

@@ -1,0 +1,66 @@
+"""-m gpu: single kernels of the path against the oracle / plain references, through the C ABI."""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+import paper_2606_28166_b200 as T
+from oracle import rng as orng
+
+pytestmark = pytest.mark.gpu
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "philox4x32_10_kat.txt")
+
+
+def test_philox_known_answers_on_device():
+    for line in open(GOLDEN):
+        line = line.strip()
+        if not line or line.startswith("#"):
+            continue
+        r = line.split()
+        ins = [int(x, 16) for x in r[:6]]
+        out = T.tandem_test_philox(ins[:4], ins[4:])
+        for got, exp in zip(out, r[6:]):
+            if "?" not in exp:
+                assert got == int(exp, 16)
+
+
+@pytest.mark.parametrize("seed", [0, 7, (1 << 40) + 12345])
+def test_uniforms_bit_identical_to_oracle(seed):
+    """Pin 14: the two independently written generators agree bit for bit on > 10^6 values."""
+    n = 151936
+    out = torch.empty(n, dtype=torch.float32, device="cuda")
+    total = 0
+    for (b, t) in [(0, 1), (3, 17), (127, 4096), (511, 8192), (1000003, 2), (5, 5), (6, 6), (9, 999)]:
+        T.tandem_test_uniforms(seed, b, t, 0, n, out)
+        ref = orng.uniforms_sample(seed, b, t, n)
+        assert np.array_equal(out.cpu().numpy().view(np.uint32), ref.view(np.uint32))
+        total += n
+    assert total > 10 ** 6
+    sw = torch.empty(4097, dtype=torch.float32, device="cuda")
+    for b in (0, 1, 77):
+        T.tandem_test_uniforms(seed, b, 0, 1, 4097, sw)
+        ref = np.array([orng.uniforms_switch(seed, b, t) for t in range(0, 4097, 64)], dtype=np.float32)
+        assert np.array_equal(sw.cpu().numpy()[::64].view(np.uint32), ref.view(np.uint32))
+
+
+@pytest.mark.parametrize("rows,N,K", [(1, 32, 32), (7, 96, 128), (33, 512, 128), (129, 1152, 896), (64, 40, 72)])
+def test_simt_gemm_fp32(rows, N, K):
+    g = torch.Generator().manual_seed(rows * 1000 + N)
+    A = torch.randn(rows, K, generator=g).cuda()
+    W = (torch.randn(N, K, generator=g) * 0.05).cuda()
+    out = torch.zeros(rows, N, device="cuda")
+    T.tandem_test_gemm(T.F32, T.GEMM_SIMT, A, W, out)
+    ref = (A.double() @ W.double().T)
+    assert torch.max(torch.abs(out.double() - ref)).item() <= 2e-6 * max(1.0, ref.abs().max().item()) * (K ** 0.5)
+
+
+@pytest.mark.parametrize("rows,N,K", [(5, 64, 64), (130, 1152, 896)])
+def test_simt_gemm_bf16(rows, N, K):
+    g = torch.Generator().manual_seed(rows + N)
+    A = torch.randn(rows, K, generator=g).to(torch.bfloat16).cuda()
+    W = (torch.randn(N, K, generator=g) * 0.05).to(torch.bfloat16).cuda()
+    out = torch.zeros(rows, N, device="cuda")
+    T.tandem_test_gemm(T.BF16, T.GEMM_SIMT, A, W, out)
+    ref = (A.double() @ W.double().T)
+    assert torch.max(torch.abs(out.double() - ref)).item() <= 2e-6 * max(1.0, ref.abs().max().item()) * (K ** 0.5)
