@@ -66,7 +66,7 @@ def test_api_errors():
     eng, _, _ = make_pair(SHAPE, max_seqs=2, max_seq_len=32)
     for bad in (dict(p=1.5), dict(top_p=0.9), dict(temperature=-1.0), dict(cap_k=-1), dict(eos_id=SHAPE.vocab)):
         with pytest.raises(T.TandemError) as e:
-            eng.generate(T.TandemParams(ws, **bad), _prompts(1), [4])
+            eng.generate(T.TandemParams(ws, **bad), [np.arange(4, dtype=np.int32)], [4])
         assert e.value.code == -1
     with pytest.raises(T.TandemError) as e:                     # prompt + max_new > max_seq_len
         eng.generate(prm, [np.zeros(30, np.int32)], [4])
@@ -75,9 +75,9 @@ def test_api_errors():
         eng.generate(prm, [np.array([1, SHAPE.vocab], np.int32)], [4])
     assert e.value.code == -1
     with pytest.raises(T.TandemError) as e:                     # more admissions than slots through tandem_step
-        eng.step(prm, admit=(_prompts(3), None, [2, 2, 2]))
+        eng.step(prm, admit=([p[:4] for p in _prompts(3)], None, [2, 2, 2]))
     assert e.value.code == -5
-    out = eng.generate(prm, _prompts(2), [4, 4])                # the handle is still usable
+    out = eng.generate(prm, [p[:8] for p in _prompts(2)], [4, 4])   # the handle is still usable
     assert out["len"].tolist() == [4, 4]
     assert eng.generate(prm, [], np.zeros(0, np.int32))["len"].shape == (0,)     # empty batch
     eng.free()
