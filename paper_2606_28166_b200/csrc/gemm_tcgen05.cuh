@@ -1,11 +1,340 @@
-// placeholder, replaced below
+// gemm_tcgen05.cuh - out[r, n] = sum_k A[r, k] W[n, k] for bf16 A, W with fp32 accumulation on the 5th-generation
+// tensor cores (S3, S6, S7 and the LM head of the bf16 configs; BASELINE.json north_star (e)).
+//
+// Shape of the problem: W is [N, K] row-major (K contiguous), A is [rows, K] row-major, rows is small in decode
+// (~64-256 per model per step) and only known on the device. So the kernel is "swap-AB": the weight tile is the
+// M operand of tcgen05.mma (128 weight rows = 128 TMEM lanes) and the token rows are the N operand (32..256, a
+// runtime field of the instruction descriptor), which makes ragged row counts free and turns the kernel into a
+// weight streamer: every weight byte crosses HBM once (TMA, L2 evict-first), the activation tile is re-read from L2.
+//   grid = (N/128 weight tiles, S K-splits); each CTA accumulates its K-slice for all rows in TMEM and writes an
+//   fp32 partial out[s][r][n]; the consumer kernel sums the S partials in a fixed order (deterministic, no atomics).
+//   warp 0: TMA producer   warp 1: MMA issuer   warps 2-5: epilogue (tcgen05.ld -> coalesced global stores)
+//   smem ring: stage = 16 KB of W (128 x 64 bf16, 128B swizzle) + nbox x 4 KB of A (32-row boxes), as many stages
+//   as fit in 200 KB (4 at 256 rows, 6 at 128 rows, 9 at 32 rows).
 #pragma once
+#include <cuda.h>   // CUtensorMap and its enums only; the encode entry point is fetched at run time (no libcuda link)
+#include <map>
+#include <tuple>
 #include "common.cuh"
+
 namespace tandem {
-struct TcGemmPlans;
-inline TcGemmPlans* tc_gemm_create() { return nullptr; }
-inline void tc_gemm_destroy(TcGemmPlans*) {}
-inline void tc_gemm_invalidate(TcGemmPlans*, int) {}
-inline int tc_gemm_launch(TcGemmPlans*, int, int, int, const void*, const void*, int, int, float*, const int32_t*, int, int*, size_t*, cudaStream_t) { return -3; }
-inline int tc_gemm_test(int, int, int, const void*, const void*, float*) { return -3; }
+
+constexpr int kTcTileN = 128;        // weight rows per CTA = UMMA M
+constexpr int kTcBlockK = 64;        // bf16 elements per k-block = one 128-byte swizzle row
+constexpr int kTcRowBox = 32;        // token rows per TMA box of A
+constexpr int kTcMaxRows = 256;      // token rows per accumulator pass = max UMMA N
+constexpr int kTcMaxStages = 10;
+constexpr int kTcRingBytes = 200 * 1024;
+constexpr int kTcSmemBytes = kTcRingBytes + 1024;   // + alignment slack
+constexpr int kTcThreads = 192;
+constexpr int kTcWBytes = kTcTileN * kTcBlockK * 2;     // 16384
+constexpr int kTcABoxBytes = kTcRowBox * kTcBlockK * 2; // 4096
+
+// ---------------------------------------------------------------------------------------------- PTX wrappers
+namespace ptx {
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
 }
+__device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t done;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}" : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+  } while (!done);
+}
+__device__ __forceinline__ uint64_t policy_evict_first() {
+  uint64_t p; asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p)); return p;
+}
+__device__ __forceinline__ uint64_t policy_evict_last() {
+  uint64_t p; asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p)); return p;
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar, uint64_t policy) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3}], [%4], %5;"
+               ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar), "l"(policy) : "memory");
+}
+__device__ __forceinline__ void prefetch_tmap(const CUtensorMap* map) { asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+template <int COLS> __device__ __forceinline__ void tmem_alloc(uint32_t smem_dst) {
+  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "n"(COLS) : "memory");
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+template <int COLS> __device__ __forceinline__ void tmem_dealloc(uint32_t taddr) {
+  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "n"(COLS) : "memory");
+}
+// D[tmem] (+)= A[smem desc] * B[smem desc], bf16 inputs, fp32 accumulate, one CTA.
+__device__ __forceinline__ void umma_bf16(uint32_t d_tmem, uint64_t desc_a, uint64_t desc_b, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem), "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+// arrives on the mbarrier once all previously issued tcgen05.mma of this thread have completed
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]), "=r"(v[9]),
+        "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]), "=r"(v[17]), "=r"(v[18]),
+        "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]),
+        "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+      : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+}  // namespace ptx
+
+// Shared-memory matrix descriptor of a K-major bf16 tile whose rows are 128 bytes (64 elements) with the 128-byte
+// swizzle TMA wrote: 8-row groups are 1024 bytes apart (SBO), descriptor version 1 (sm_100), layout type 2.
+__device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t smem_addr) {
+  uint64_t d = 0;
+  d |= (uint64_t)((smem_addr & 0x3FFFFu) >> 4);        // start address, bits [0,14)
+  d |= (uint64_t)1 << 16;                              // leading byte offset (unused for swizzled K-major), bits [16,30)
+  d |= (uint64_t)(1024u >> 4) << 32;                   // stride byte offset, bits [32,46)
+  d |= (uint64_t)1 << 46;                              // version
+  d |= (uint64_t)2 << 61;                              // SWIZZLE_128B
+  return d;
+}
+// Instruction descriptor, kind::f16: D fp32, A and B bf16, both K-major, M = 128, N = n (multiple of 16, <= 256).
+__device__ __forceinline__ uint32_t umma_idesc_bf16(int n) {
+  return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(kTcTileN >> 4) << 24);
+}
+
+struct TcGemmArgs {
+  float* out;                 // [n_split][row_cap][N] fp32 partials
+  const int32_t* rows_ptr;    // device scalar with the live row count, or null
+  int rows_fixed;
+  int N, K, n_split;
+  size_t split_stride;        // floats between partials
+};
+
+// ---------------------------------------------------------------------------------------------- the kernel
+__global__ void __launch_bounds__(kTcThreads, 1)
+gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_constant__ CUtensorMap tmap_a, TcGemmArgs g) {
+  extern __shared__ uint8_t tc_smem_raw[];
+  __shared__ __align__(8) uint64_t bars[2 * kTcMaxStages + 2];
+  __shared__ uint32_t tmem_base_smem;
+
+  const int rows = g.rows_ptr ? *g.rows_ptr : g.rows_fixed;
+  if (rows <= 0) return;                                   // uniform over the grid: nothing was scheduled for this model
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int n0 = blockIdx.x * kTcTileN;
+  const int split = blockIdx.y;
+  const int kb_total = (g.K + kTcBlockK - 1) / kTcBlockK;
+  const int kb0 = (int)((long long)kb_total * split / g.n_split);
+  const int kb1 = (int)((long long)kb_total * (split + 1) / g.n_split);
+  const int n_chunks = (rows + kTcMaxRows - 1) / kTcMaxRows;
+  const int nbox_max = (min(rows, kTcMaxRows) + kTcRowBox - 1) / kTcRowBox;
+  const int stage_bytes = kTcWBytes + nbox_max * kTcABoxBytes;
+  const int n_stages = min(kTcMaxStages, kTcRingBytes / stage_bytes);
+
+  const uint32_t ring = (ptx::smem_u32(tc_smem_raw) + 1023u) & ~1023u;   // 128B swizzle atoms are 1024-byte aligned
+  const uint32_t bar0 = ptx::smem_u32(bars);
+  auto full_bar = [&](int s) { return bar0 + 8u * (uint32_t)s; };
+  auto empty_bar = [&](int s) { return bar0 + 8u * (uint32_t)(kTcMaxStages + s); };
+  const uint32_t tmem_full_bar = bar0 + 8u * (2 * kTcMaxStages);
+  const uint32_t tmem_empty_bar = tmem_full_bar + 8u;
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < n_stages; ++s) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
+    ptx::mbar_init(tmem_full_bar, 1);
+    ptx::mbar_init(tmem_empty_bar, 4);
+    ptx::fence_mbar_init();
+    ptx::prefetch_tmap(&tmap_w);
+    ptx::prefetch_tmap(&tmap_a);
+  }
+  if (warp == 2) ptx::tmem_alloc<kTcMaxRows>(ptx::smem_u32(&tmem_base_smem));
+  ptx::tc_fence_before();
+  __syncthreads();
+  ptx::tc_fence_after();
+  const uint32_t tmem_base = tmem_base_smem;
+
+  if (warp == 0) {
+    // ===== TMA producer: weights stream once (evict-first), activations are re-read by every CTA (evict-last)
+    if (lane == 0) {
+      const uint64_t pol_w = ptx::policy_evict_first(), pol_a = ptx::policy_evict_last();
+      int it = 0;
+      for (int c = 0; c < n_chunks; ++c) {
+        const int r0 = c * kTcMaxRows;
+        const int nbox = (min(rows - r0, kTcMaxRows) + kTcRowBox - 1) / kTcRowBox;
+        for (int kb = kb0; kb < kb1; ++kb, ++it) {
+          const int s = it % n_stages;
+          const uint32_t ph = (uint32_t)(it / n_stages) & 1u;
+          ptx::mbar_wait(empty_bar(s), ph ^ 1u);
+          const uint32_t dst = ring + (uint32_t)(s * stage_bytes);
+          ptx::mbar_expect_tx(full_bar(s), (uint32_t)(kTcWBytes + nbox * kTcABoxBytes));
+          ptx::tma_load_2d(dst, &tmap_w, kb * kTcBlockK, n0, full_bar(s), pol_w);
+          for (int j = 0; j < nbox; ++j)
+            ptx::tma_load_2d(dst + kTcWBytes + j * kTcABoxBytes, &tmap_a, kb * kTcBlockK, r0 + j * kTcRowBox, full_bar(s), pol_a);
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===== MMA issuer: one thread drives the tensor core for the whole CTA
+    if (lane == 0) {
+      int it = 0;
+      for (int c = 0; c < n_chunks; ++c) {
+        const int r0 = c * kTcMaxRows;
+        const int ncols = ((min(rows - r0, kTcMaxRows) + kTcRowBox - 1) / kTcRowBox) * kTcRowBox;
+        const uint32_t idesc = umma_idesc_bf16(ncols);
+        ptx::mbar_wait(tmem_empty_bar, ((uint32_t)c & 1u) ^ 1u);
+        ptx::tc_fence_after();
+        for (int kb = kb0; kb < kb1; ++kb, ++it) {
+          const int s = it % n_stages;
+          const uint32_t ph = (uint32_t)(it / n_stages) & 1u;
+          ptx::mbar_wait(full_bar(s), ph);
+          ptx::tc_fence_after();
+          const uint32_t sw = ring + (uint32_t)(s * stage_bytes);
+          const uint64_t dw = umma_desc_sw128(sw), da = umma_desc_sw128(sw + kTcWBytes);
+#pragma unroll
+          for (int k = 0; k < kTcBlockK / 16; ++k)   // UMMA K = 16 bf16 = 32 bytes: advance the start address inside the swizzle row
+            ptx::umma_bf16(tmem_base, dw + (uint64_t)(2 * k), da + (uint64_t)(2 * k), idesc, (kb > kb0 || k > 0) ? 1u : 0u);
+          ptx::umma_commit(empty_bar(s));            // frees the smem stage once these MMAs have read it
+        }
+        ptx::umma_commit(tmem_full_bar);             // accumulator of this chunk complete
+      }
+    }
+  } else {
+    // ===== epilogue: warp w may touch TMEM lanes 32*(w%4)..+31; lane = weight row n, column = token row r
+    const int q = warp & 3;
+    const int n = n0 + q * 32 + lane;
+    float* outp = g.out + (size_t)split * g.split_stride;
+    for (int c = 0; c < n_chunks; ++c) {
+      const int r0 = c * kTcMaxRows;
+      const int crow = min(rows - r0, kTcMaxRows);
+      ptx::mbar_wait(tmem_full_bar, (uint32_t)c & 1u);
+      ptx::tc_fence_after();
+      for (int c0 = 0; c0 < crow; c0 += 32) {
+        uint32_t v[32];
+        ptx::tmem_ld32(tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)c0, v);
+        ptx::tmem_ld_wait();
+        if (n < g.N) {
+#pragma unroll
+          for (int j = 0; j < 32; ++j)
+            if (c0 + j < crow) outp[(size_t)(r0 + c0 + j) * g.N + n] = __uint_as_float(v[j]);
+        }
+      }
+      ptx::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(tmem_empty_bar);
+    }
+  }
+  ptx::tc_fence_before();
+  __syncthreads();
+  if (warp == 2) ptx::tmem_dealloc<kTcMaxRows>(tmem_base);
+}
+
+// ---------------------------------------------------------------------------------------------- host side
+// K-splits: enough CTAs to put one on (almost) every SM, never more than one wave of 148, each slice >= 4 k-blocks.
+// A function of the shape only, so the reduction order (and every logit) is independent of the batch.
+inline int tc_gemm_splits(int N, int K) {
+  const int tiles = (N + kTcTileN - 1) / kTcTileN, kb = (K + kTcBlockK - 1) / kTcBlockK;
+  int s = 1;
+  while (tiles * (s + 1) <= 148 && (s + 1) * 4 <= kb && s < 16) ++s;
+  return s;
+}
+
+typedef CUresult (*TcEncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                               const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                               CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+struct TcGemmPlans {
+  TcEncodeFn encode = nullptr;
+  std::map<std::tuple<const void*, int, int, int>, CUtensorMap> maps;   // (base, rows, K, box_rows) -> descriptor
+};
+
+inline TcGemmPlans* tc_gemm_create() {
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult q;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess || !fn || q != cudaDriverEntryPointSuccess) {
+    cudaGetLastError();
+    return nullptr;
+  }
+  if (cudaFuncSetAttribute(gemm_tcgen05_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes) != cudaSuccess) {
+    cudaGetLastError();
+    return nullptr;
+  }
+  TcGemmPlans* p = new TcGemmPlans();
+  p->encode = (TcEncodeFn)fn;
+  return p;
+}
+inline void tc_gemm_destroy(TcGemmPlans* p) { delete p; }
+inline void tc_gemm_invalidate(TcGemmPlans* p, int) { if (p) p->maps.clear(); }
+
+// Descriptor of a row-major bf16 matrix [n_rows, K] tiled in boxes of box_rows x 64 elements, 128-byte swizzle;
+// out-of-bounds elements read as zero (ragged K tails and row tails need no special case).
+inline const CUtensorMap* tc_gemm_map(TcGemmPlans* p, const void* base, int n_rows, int K, int box_rows) {
+  auto key = std::make_tuple(base, n_rows, K, box_rows);
+  auto it = p->maps.find(key);
+  if (it != p->maps.end()) return &it->second;
+  CUtensorMap m;
+  const cuuint64_t dims[2] = {(cuuint64_t)K, (cuuint64_t)n_rows};
+  const cuuint64_t strides[1] = {(cuuint64_t)K * 2};
+  const cuuint32_t box[2] = {(cuuint32_t)kTcBlockK, (cuuint32_t)box_rows};
+  const cuuint32_t estr[2] = {1, 1};
+  const CUresult r = p->encode(&m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr,
+                               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return nullptr;
+  return &(p->maps[key] = m);
+}
+
+// Launch on `s`. out receives *n_split partials, *split_stride floats apart. Returns 0, or -1 (TANDEM_EINVAL) / -3 (TANDEM_ECUDA).
+// which == 4 (LM head) never splits: the sampler reads the logits in place.
+inline int tc_gemm_launch(TcGemmPlans* p, int /*model*/, int which, int /*layer*/, const void* A, const void* W, int N, int K, float* out,
+                          const int32_t* rows_ptr, int rows_cap, int* n_split, size_t* split_stride, cudaStream_t s) {
+  if (!p || (K % 8) != 0) return -1;                       // TMA needs 16-byte row strides
+  const CUtensorMap* mw = tc_gemm_map(p, W, N, K, kTcTileN);
+  const CUtensorMap* ma = tc_gemm_map(p, A, rows_cap, K, kTcRowBox);
+  if (!mw || !ma) return -3;
+  const int S = which == 4 ? 1 : tc_gemm_splits(N, K);
+  *n_split = S;
+  *split_stride = (size_t)rows_cap * N;
+  TcGemmArgs g{out, rows_ptr, rows_cap, N, K, S, *split_stride};
+  if (!rows_ptr) g.rows_fixed = rows_cap;
+  dim3 grid((N + kTcTileN - 1) / kTcTileN, S);
+  gemm_tcgen05_kernel<<<grid, kTcThreads, kTcSmemBytes, s>>>(*mw, *ma, g);
+  return 0;
+}
+
+// Unit-test hook: out[rows, N] = A W^T (partials summed here), synchronous.
+__global__ void tc_sum_partials_kernel(const float* __restrict__ part, int n_split, size_t stride, float* __restrict__ out, size_t n) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    float v = 0.f;
+    for (int s = 0; s < n_split; ++s) v += part[s * stride + i];
+    out[i] = v;
+  }
+}
+inline int tc_gemm_test(int rows, int N, int K, const void* A, const void* W, float* out) {
+  if (rows == 0) return 0;
+  TcGemmPlans* p = tc_gemm_create();
+  if (!p) return -3;
+  const int S = tc_gemm_splits(N, K);
+  float* part = nullptr;
+  if (cudaMalloc(&part, (size_t)S * rows * N * sizeof(float)) != cudaSuccess) { tc_gemm_destroy(p); return -2; }
+  int ns; size_t ss;
+  int rc = tc_gemm_launch(p, 0, 0, 0, A, W, N, K, part, nullptr, rows, &ns, &ss, 0);
+  if (rc == 0) {
+    tc_sum_partials_kernel<<<296, 256>>>(part, ns, ss, out, (size_t)rows * N);
+    rc = cudaDeviceSynchronize() == cudaSuccess ? 0 : -3;
+  }
+  cudaFree(part);
+  tc_gemm_destroy(p);
+  return rc;
+}
+
+}  // namespace tandem

@@ -102,13 +102,6 @@ template <typename P> int dmalloc(tandem_handle* h, P** p, size_t bytes) {
 }
 #define DM(h, p, bytes) do { int rc__ = dmalloc((h), (p), (bytes)); if (rc__) return rc__; } while (0)
 
-int pick_splits(int n_tiles, int k_blocks) {
-  // enough CTAs to cover the 148 SMs once; never more than the k-blocks available, and each slice >= 4 k-blocks
-  int s = 1;
-  while (n_tiles * s < 120 && (s + 1) * 4 <= k_blocks && s < 16) ++s;
-  return s;
-}
-
 // ------------------------------------------------------------------------------------------ GEMM dispatch
 // out[s][r][n] partials (s < *n_split, stride *split_stride floats); rows read from counts_ptr[idx] on the device.
 template <typename T>
@@ -431,10 +424,10 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
   // widest split-K partial buffer any GEMM needs, in floats per row (S*N); SIMT uses S = 1
   size_t cols = std::max({(size_t)qkv_n, (size_t)2 * I, (size_t)H});
   if (h->gemm_impl == TANDEM_GEMM_TCGEN05) {
-    cols = std::max(cols, (size_t)qkv_n * pick_splits(qkv_n / 128, H / 64));
-    cols = std::max(cols, (size_t)H * pick_splits(H / 128, nq * d / 64));
-    cols = std::max(cols, (size_t)2 * I * pick_splits(2 * I / 128, H / 64));
-    cols = std::max(cols, (size_t)H * pick_splits(H / 128, I / 64));
+    cols = std::max(cols, (size_t)qkv_n * tc_gemm_splits(qkv_n, H));
+    cols = std::max(cols, (size_t)H * tc_gemm_splits(H, nq * d));
+    cols = std::max(cols, (size_t)2 * I * tc_gemm_splits(2 * I, H));
+    cols = std::max(cols, (size_t)H * tc_gemm_splits(H, I));
   }
   h->gemm_out_cols = cols;
   for (int m = 0; m < 2; ++m) {

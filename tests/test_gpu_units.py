@@ -64,3 +64,20 @@ def test_simt_gemm_bf16(rows, N, K):
     T.tandem_test_gemm(T.BF16, T.GEMM_SIMT, A, W, out)
     ref = (A.double() @ W.double().T)
     assert torch.max(torch.abs(out.double() - ref)).item() <= 2e-6 * max(1.0, ref.abs().max().item()) * (K ** 0.5)
+
+
+@pytest.mark.parametrize("rows,N,K", [(1, 128, 64), (7, 256, 128), (32, 128, 256), (33, 384, 192), (64, 512, 256), (128, 6144, 2560),
+                                      (129, 2560, 4096), (300, 1152, 896), (256, 2560, 9728), (257, 1024, 512), (61, 4096, 2560),
+                                      (5, 200, 72), (1000, 640, 1024)])
+def test_tcgen05_gemm_bf16(rows, N, K):
+    """tcgen05/TMEM/TMA GEMM (swap-AB, split-K) against a float64 matmul of the same bf16 values: the seven projection
+    shapes of the configs plus ragged rows (1, 33, 257, 1000), N not a multiple of the 128-row tile and K not a multiple of 64."""
+    g = torch.Generator().manual_seed(rows * 7919 + N + K)
+    A = torch.randn(rows, K, generator=g).to(torch.bfloat16).cuda()
+    W = (torch.randn(N, K, generator=g) * 0.05).to(torch.bfloat16).cuda()
+    out = torch.full((rows, N), float("nan"), device="cuda")
+    T.tandem_test_gemm(T.BF16, T.GEMM_TCGEN05, A, W, out)
+    ref = (A.double() @ W.double().T)
+    err = torch.max(torch.abs(out.double() - ref)).item()
+    assert np.isfinite(err)
+    assert err <= 2e-6 * max(1.0, ref.abs().max().item()) * (K ** 0.5), (err, ref.abs().max().item())
