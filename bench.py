@@ -1,0 +1,401 @@
+#!/usr/bin/env python
+"""bench.py - tandem rollout throughput on B200 (BASELINE.json metric: "tandem rollout tokens/s (4B-shape bf16, 1 B200)").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME] [--fast-forward G]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P bench.py --gpus N ...
+
+One "step" = one pass of the whole hot path (S0-S8) over the resident batch: every unfinished
+sequence of the workload emits exactly one token (`tandem_step`). The workload is BASELINE.json configs[2]
+(cfg3_4b_bf16: two 36-layer 4B-shape models, batch 128 = 16 prompts x 8 rollouts, prompts U[64,512], p = 0.5,
+T = 1, 16-token KV pages), synthetic and seeded (workloads/). Phases of the default arm:
+  setup   (untimed) weights -> engine, admission, prompt prefill, `--ramp` steps so that both models hold KV
+  warmup  W steps (>= 3 enforced)
+  timed   exactly K steps between CUDA events on the launching stream; barrier + synchronize on both sides; max over ranks
+  profile `--profile-steps` more steps in the library's per-kernel timing mode -> "roofline" of the dominant kernel
+  e2e     `tandem_generate` on HOST buffers (prompts H2D, tokens/owner/log-probs D2H inside the timed region)
+  cpu     the oracle (oracle/, float64 NumPy) on a bounded sample of the same workload, rank 0, N = 1 only
+`--impl reference` times the oracle alone (rank 0; other ranks exit 0) and prints the same JSON line shape.
+Prints ONE JSON line on rank 0.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "tandem rollout tokens/s (4B-shape bf16, 1 B200)"
+NOMINAL_HBM_GBS = 8000.0            # BASELINE.json: "decode HBM GB/s vs 8 TB/s"
+FALLBACK_HBM_GBS = 6650.0           # /opt/skills/guides/B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+FALLBACK_BF16_TFLOPS = 1590.0
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=128)
+    ap.add_argument("--warmup", type=int, default=8)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg3_4b_bf16")
+    ap.add_argument("--fast-forward", type=int, default=0,
+                    help="tokens already generated per sequence before the timed window (ingested as context by prefill)")
+    ap.add_argument("--ramp", type=int, default=48, help="untimed steps after prefill so that both models own KV")
+    ap.add_argument("--profile-steps", type=int, default=4)
+    ap.add_argument("--e2e-new", type=int, default=32, help="new tokens per sequence in the end-to-end tandem_generate leg")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--cpu-new", type=int, default=4, help="new tokens of the oracle's bounded sample")
+    return ap.parse_args()
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        p = json.load(open(path))
+        return dict(hbm_gbs=float(p["hbm_gbs"]), bf16_tflops=float(p["bf16_tflops"]),
+                    bf16_tflops_sustained=float(p.get("bf16_tflops_sustained", p["bf16_tflops"])), source="measured")
+    return dict(hbm_gbs=FALLBACK_HBM_GBS, bf16_tflops=FALLBACK_BF16_TFLOPS, bf16_tflops_sustained=1400.0, source="fallback")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md's clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------ workload
+def build_inputs(wl, fast_forward, rank):
+    """Seeded synthetic inputs of the workload for this rank: prompts (+ `fast_forward` already-generated ids appended
+    as context), the word-start table and the per-sequence ids that address the counter RNG."""
+    from workloads import make_prompts, make_word_start
+    prompts = make_prompts(wl, seed=wl.seeds["prompts"] + 1000 * rank)
+    if fast_forward > 0:
+        rng = np.random.default_rng(wl.seeds["prompts"] + 1000 * rank + 77)
+        prompts = [np.concatenate([p, rng.integers(0, wl.shape.vocab, size=fast_forward).astype(np.int32)]) for p in prompts]
+    table = make_word_start(wl.shape.vocab, wl.word_start_frac, wl.seeds["table"])
+    seq_ids = np.arange(wl.batch, dtype=np.int32) + wl.batch * rank
+    return prompts, table, seq_ids
+
+
+def weight_bytes_per_model(shape):
+    return shape.params_read_per_step * (4 if shape.dtype == "f32" else 2)
+
+
+def class_bytes(shape, cls, rows, kv_bytes_per_layer_launch, emit_rows):
+    """ALGORITHMIC HBM bytes of one launch of kernel class `cls` at `rows` rows: the operand
+    that must be streamed (weights / KV) + activations in + one copy of the result. bf16 = 2 bytes, fp32 = 4."""
+    H, I, V = shape.hidden, shape.intermediate, shape.vocab
+    qd, kd = shape.n_q_heads * shape.head_dim, shape.n_kv_heads * shape.head_dim
+    es = 4 if shape.dtype == "f32" else 2
+    g = lambda N, K, r: N * K * es + r * K * es + r * N * 4
+    if cls == "gemm_qkv":
+        return g(qd + 2 * kd, H, rows)
+    if cls == "gemm_o":
+        return g(H, qd, rows)
+    if cls == "gemm_gateup":
+        return g(2 * I, H, rows)
+    if cls == "gemm_down":
+        return g(H, I, rows)
+    if cls == "gemm_lmhead":
+        return g(V, H, emit_rows)
+    if cls == "attention":
+        return kv_bytes_per_layer_launch + rows * qd * (4 + es)
+    if cls == "rope_append":
+        return rows * (qd + 2 * kd) * 4 + rows * qd * 4 + rows * 2 * kd * es
+    if cls == "residual_norm":
+        return rows * H * (4 + 4 + 4 + es)
+    if cls == "swiglu":
+        return rows * 2 * I * 4 + rows * I * es
+    if cls == "embed_norm":
+        return rows * H * (es + 4 + es)
+    if cls == "sample_switch_emit":
+        return emit_rows * V * 4
+    return 0
+
+
+def run_ours(args):
+    import torch
+    import paper_2606_28166_b200 as T
+    from workloads import get_workload, make_weights
+
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    T.build()
+    wl = get_workload(args.workload)
+    shape, B = wl.shape, wl.batch
+    W, K = max(3, args.warmup), args.steps
+    prompts, table, seq_ids = build_inputs(wl, args.fast_forward, rank)
+    max_prompt = max(len(p) for p in prompts)
+    prefill_rows = sum(len(p) for p in prompts)
+    row_cap = 4096
+    prefill_steps = (prefill_rows + row_cap - 1) // row_cap + 2
+    gen_budget = prefill_steps + args.ramp + W + K + args.profile_steps + 64
+    max_seq_len = ((max_prompt + max(gen_budget, args.e2e_new) + 15) // 16) * 16
+    eng = T.Tandem(T.TandemConfig(shape, max_seqs=B, max_seq_len=max_seq_len, device=local, max_rows_per_step=row_cap, use_graph=1))
+    w_cpu = []
+    for m, seed in enumerate((wl.seeds["senior"], wl.seeds["junior"])):
+        w = make_weights(shape, seed, device="cuda")
+        eng.load_weights(m, w)
+        if rank == 0 and world == 1 and not args.no_cpu:
+            w_cpu.append(dict(embed=w["embed"].cpu(), lm_head=w["lm_head"].cpu(), final_norm=w["final_norm"].cpu(),
+                              layers=[{k: v.cpu() for k, v in l.items()} for l in w["layers"]]))
+        del w
+        torch.cuda.empty_cache()
+    prm = T.TandemParams(table, p=wl.p, temperature=wl.temperature, top_p=wl.top_p, seed=20260628)
+    out = dict(token=torch.zeros(B, dtype=torch.int32, device="cuda"), owner=torch.zeros(B, dtype=torch.uint8, device="cuda"),
+               sen_logp=torch.zeros(B, device="cuda"), done=torch.zeros(B, dtype=torch.uint8, device="cuda"))
+    stream = torch.cuda.current_stream().cuda_stream
+
+    # ---- setup: admission, prompt prefill (row-capped chunks), ramp
+    t0 = time.perf_counter()
+    eng.step(prm, admit=(prompts, seq_ids, [gen_budget] * B), out=out, stream=stream)
+    n_setup = 1
+    while True:
+        st = eng.get_stats()
+        if st["tokens_emitted"] >= B or n_setup > 4 * prefill_steps + 16:
+            break
+        eng.step(prm, out=out, stream=stream); n_setup += 1
+    for _ in range(args.ramp):
+        eng.step(prm, out=out, stream=stream)
+    torch.cuda.synchronize()
+    setup_s = time.perf_counter() - t0
+
+    # ---- warmup + timed region
+    for _ in range(W):
+        eng.step(prm, out=out, stream=stream)
+    torch.cuda.synchronize()
+    s0 = eng.get_stats()
+    if dist: dist.barrier()
+    torch.cuda.synchronize()
+    clocks = ClockSampler(local); clocks.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(K):
+        eng.step(prm, out=out, stream=stream)
+    e1.record()
+    torch.cuda.synchronize()
+    if dist: dist.barrier()
+    ms = e0.elapsed_time(e1)
+    clk = clocks.stop()
+    s1 = eng.get_stats()
+    d = {k: s1[k] - s0[k] for k in ("steps", "tokens_emitted", "rows_senior", "rows_junior", "catchup_rows", "kv_bytes_read",
+                                    "weight_bytes_read", "kernel_launches")}
+    tokens = d["tokens_emitted"]
+    if dist:
+        t = torch.tensor([ms, float(tokens)], dtype=torch.float64, device="cuda")
+        tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
+        ms_all, tokens_all = float(tmax[0]), float(tsum[1])
+    else:
+        ms_all, tokens_all = ms, float(tokens)
+    pk = peaks()
+    step_bytes = (d["weight_bytes_read"] + d["kv_bytes_read"]) / max(1, K)
+    step_gbs = step_bytes / (ms / K * 1e-3) / 1e9
+    ctx_mean = d["kv_bytes_read"] / max(1, tokens) / (shape.kv_elems_per_token * 2)
+
+    # ---- per-kernel pass (library profile mode: one stream, events around every launch)
+    roofline, kernels = None, {}
+    if args.profile_steps > 0:
+        p0 = eng.get_stats()
+        eng.set_profile(True)
+        for _ in range(args.profile_steps):
+            eng.step(prm, out=out, stream=stream)
+        prof = eng.get_profile()
+        eng.set_profile(False)
+        p1 = eng.get_stats()
+        msteps = max(1, (p1["weight_bytes_read"] - p0["weight_bytes_read"]) // weight_bytes_per_model(shape))
+        rows = (p1["rows_senior"] + p1["rows_junior"] - p0["rows_senior"] - p0["rows_junior"]) / msteps
+        emit_rows = (p1["tokens_emitted"] - p0["tokens_emitted"]) / msteps
+        kv_launch = (p1["kv_bytes_read"] - p0["kv_bytes_read"]) / msteps / shape.n_layers
+        total_ms = sum(v[0] for v in prof.values())
+        for name, (kms, n) in prof.items():
+            if n == 0:
+                continue
+            b = class_bytes(shape, name, rows, kv_launch, emit_rows)
+            kernels[name] = {"ms_per_launch": kms / n, "launches_per_step": n / args.profile_steps, "share": kms / total_ms,
+                             "alg_bytes_per_launch": b, "gbs": b / (kms / n * 1e-3) / 1e9 if kms > 0 else None}
+        top = max(kernels, key=lambda k: kernels[k]["share"])
+        kt = kernels[top]
+        roofline = {"kernel": top, "bound": "hbm", "achieved": kt["gbs"], "peak": pk["hbm_gbs"], "unit": "GB/s",
+                    "frac": kt["gbs"] / pk["hbm_gbs"], "traffic": None, "peak_source": pk["source"] + " burst copy (kernel timed alone)",
+                    "share_of_step": kt["share"], "rows_per_launch": rows, "profile_steps": args.profile_steps,
+                    "profile_ms_per_step": total_ms / args.profile_steps}
+
+    res = {"metric": METRIC, "value": tokens_all / (ms_all * 1e-3), "unit": "tokens/s", "n_gpus": world, "steps": K, "warmup": W,
+           "ms_per_step": ms_all / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+           "config": {"workload": wl.name, "batch_per_gpu": B, "prompt_len": list(wl.prompt_len), "fast_forward": args.fast_forward,
+                      "ctx_mean_timed": ctx_mean, "p": wl.p, "word_start_frac": wl.word_start_frac, "temperature": wl.temperature,
+                      "page_tokens": 16, "parallelism": "dp%d (independent sequences, replicated weights, no collective)" % world,
+                      "l2": "inputs larger than L2 (16.1 GB of weights + KV streamed per step vs 126 MB L2)",
+                      "setup_steps": n_setup + args.ramp, "setup_seconds": setup_s, "cuda_graph": True},
+           "clocks": clk, "gpu_launches": int(d["kernel_launches"]),
+           "step_roofline": {"bound": "hbm", "alg_bytes_per_step": step_bytes, "weights_bytes_per_step": d["weight_bytes_read"] / K,
+                             "kv_bytes_per_step": d["kv_bytes_read"] / K, "achieved": step_gbs, "unit": "GB/s",
+                             "frac_of_measured": step_gbs / pk["hbm_gbs"], "frac_of_8TBs": step_gbs / NOMINAL_HBM_GBS,
+                             "rows_per_step": (d["rows_senior"] + d["rows_junior"]) / K, "catchup_rows_per_step": d["catchup_rows"] / K},
+           "roofline": roofline, "kernels": kernels}
+
+    # ---- end to end through tandem_generate with HOST buffers
+    if not args.no_e2e:
+        new = args.e2e_new
+        for it in range(2):                      # first call warms the graph for this parameter set
+            if dist: dist.barrier()
+            t0 = time.perf_counter()
+            g = eng.generate(prm, prompts, [new] * B, seq_ids=seq_ids, stream=stream)
+            torch.cuda.synchronize()
+            dt = time.perf_counter() - t0
+        tok = float(g["len"].sum())
+        if dist:
+            t = torch.tensor([dt, tok], dtype=torch.float64, device="cuda")
+            tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+            tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
+            dt, tok = float(tmax[0]), float(tsum[1])
+        steps_e = max(1, g["stats"]["steps"])
+        h2d = prefill_rows * 4 + (B + 1) * 8 + 3 * B * 4 + shape.vocab
+        d2h = B * new * (4 + 1 + 4) + B * 4
+        res["e2e"] = {"value": tok / dt, "unit": "tokens/s", "h2d_bytes_per_step": h2d / steps_e, "d2h_bytes_per_step": d2h / steps_e,
+                      "call": "tandem_generate(B=%d host prompts, max_new=%d): prompt prefill + %d engine steps, host buffers in and out"
+                              % (B, new, steps_e), "seconds": dt, "device_seconds": g["stats"]["seconds_total"]}
+    eng.free()
+    torch.cuda.empty_cache()
+
+    if rank == 0 and world == 1 and not args.no_cpu:
+        res["cpu_baseline"] = oracle_sample(wl, w_cpu, prompts, table, seq_ids, args.cpu_new, prm_seed=20260628)
+    if rank == 0:
+        print(json.dumps(res))
+    if dist:
+        dist.destroy_process_group()
+
+
+# ------------------------------------------------------------------------------------------------ the oracle, timed
+def blas_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        n = [p.get("num_threads", 1) for p in threadpool_info() if p.get("user_api") == "blas"]
+        return max(n) if n else 1
+    except Exception:
+        return 1
+
+
+def oracle_rollout(wl, w_cpu, prompt, table, seq_id, n_new, prm_seed, models=None):
+    """One sequence of the workload through the oracle as it stands (incremental KV, float64 NumPy): returns
+    (seconds, tokens emitted, models). The oracle is test infrastructure; this is the one place bench.py executes it."""
+    from oracle import OracleModel, TandemParams as OParams, tandem_generate
+    from oracle.rule import Uniforms
+    if models is None:
+        try:
+            import psutil
+            roomy = psutil.virtual_memory().available > 2.6 * 8 * wl.shape.params_read_per_step * 2
+        except Exception:
+            roomy = False
+        models = (OracleModel(wl.shape, w_cpu[0], cache=roomy), OracleModel(wl.shape, w_cpu[1], cache=roomy))
+    op = OParams(p=wl.p, temperature=wl.temperature, top_p=wl.top_p, seed=prm_seed)
+    t0 = time.perf_counter()
+    r = tandem_generate(models, op, [prompt], [n_new], table, uni=Uniforms(seed=prm_seed, seq_ids=[int(seq_id)]))
+    dt = time.perf_counter() - t0
+    return dt, len(r["tokens"][0]), models
+
+
+def oracle_sample(wl, w_cpu, prompts, table, seq_ids, n_new, prm_seed):
+    b = int(np.argmin([len(p) for p in prompts]))
+    dt, n, _ = oracle_rollout(wl, w_cpu, prompts[b], table, seq_ids[b], n_new, prm_seed)
+    return {"value": n / dt, "unit": "tokens/s", "cores": blas_threads(), "host_cpus": os.cpu_count(), "kind": "oracle",
+            "sample": "1 of the %d sequences (the shortest prompt, %d ids), prompt prefill + %d new tokens, oracle.tandem_generate "
+                      "incremental-KV float64 NumPy on the same bf16-valued weights; %.1f s" % (len(prompts), len(prompts[b]), n, dt)}
+
+
+def run_reference(args):
+    """--impl reference: for this tier the reference arm is the oracle, timed on the host cores. A step = one token of a
+    one-sequence rollout of the workload (its prompt prefill is inside the timed region and amortised over the K tokens)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from workloads import get_workload, make_weights
+    wl = get_workload(args.workload)
+    W, K = max(1, args.warmup), args.steps
+    prompts, table, seq_ids = build_inputs(wl, 0, 0)
+    try:
+        import torch
+        dev = "cuda" if torch.cuda.is_available() else "cpu"   # the generator only: random weights are inputs, not arithmetic
+    except Exception:
+        dev = "cpu"
+    w_cpu = []
+    for seed in (wl.seeds["senior"], wl.seeds["junior"]):
+        w = make_weights(wl.shape, seed, device=dev)
+        w_cpu.append(dict(embed=w["embed"].cpu(), lm_head=w["lm_head"].cpu(), final_norm=w["final_norm"].cpu(),
+                          layers=[{k: v.cpu() for k, v in l.items()} for l in w["layers"]]))
+        del w
+    order = np.argsort([len(p) for p in prompts])
+    b0, b1 = int(order[0]), int(order[1])
+    _, _, models = oracle_rollout(wl, w_cpu, prompts[b0], table, seq_ids[b0], W, 20260628)          # warm-up
+    dt, n, _ = oracle_rollout(wl, w_cpu, prompts[b1], table, seq_ids[b1], K, 20260628, models=models)
+    v = n / dt
+    sample = ("1 of the %d sequences (prompt %d ids): prompt prefill + %d new tokens per timed run, oracle.tandem_generate "
+              "incremental-KV float64 NumPy" % (len(prompts), len(prompts[b1]), n))
+    print(json.dumps({"impl": "reference", "metric": METRIC, "value": v, "unit": "tokens/s", "n_gpus": args.gpus, "steps": K, "warmup": W,
+                      "ms_per_step": dt / max(1, n) * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+                      "data": "synthetic", "config": {"workload": wl.name, "sample": sample},
+                      "cpu_baseline": {"value": v, "unit": "tokens/s", "cores": blas_threads(), "host_cpus": os.cpu_count(), "kind": "oracle",
+                                       "sample": sample},
+                      "e2e": {"value": v, "unit": "tokens/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
+if __name__ == "__main__":
+    a = parse_args()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)

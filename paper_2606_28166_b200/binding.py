@@ -15,7 +15,9 @@ GEMM_AUTO, GEMM_SIMT, GEMM_TCGEN05 = 0, 1, 2
 _ERR = {0: "OK", -1: "EINVAL", -2: "ENOMEM", -3: "ECUDA", -4: "ESTATE", -5: "EFULL"}
 
 EXPORTED_SYMBOLS = ["tandem_init", "tandem_load_weights", "tandem_step", "tandem_generate", "tandem_reset",
-                    "tandem_free", "tandem_last_error", "tandem_test_uniforms", "tandem_test_philox", "tandem_test_gemm"]
+                    "tandem_free", "tandem_last_error", "tandem_get_stats", "tandem_set_profile", "tandem_get_profile",
+                    "tandem_kernel_class_name", "tandem_test_uniforms", "tandem_test_philox", "tandem_test_gemm"]
+KC_NUM = 14
 
 
 class TandemError(RuntimeError):
@@ -63,7 +65,8 @@ class _StepOut(C.Structure):
 
 class _Stats(C.Structure):
     _fields_ = [(n, C.c_int64) for n in ("steps", "tokens_emitted", "rows_senior", "rows_junior", "catchup_rows", "kv_bytes_read", "weight_bytes_read")] + \
-               [("peak_pages_senior", C.c_int32), ("peak_pages_junior", C.c_int32), ("peak_resident", C.c_int32), ("seconds_total", C.c_double)]
+               [("peak_pages_senior", C.c_int32), ("peak_pages_junior", C.c_int32), ("peak_resident", C.c_int32), ("seconds_total", C.c_double),
+                ("kernel_launches", C.c_int64)]
 
 
 _lib = None
@@ -83,6 +86,11 @@ def lib():
                                       C.POINTER(_Overrides), C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                       C.POINTER(_Stats), C.c_void_p]
         L.tandem_reset.argtypes = [C.c_void_p]
+        L.tandem_get_stats.argtypes = [C.c_void_p, C.POINTER(_Stats)]
+        L.tandem_set_profile.argtypes = [C.c_void_p, C.c_int]
+        L.tandem_get_profile.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
+        L.tandem_kernel_class_name.argtypes = [C.c_int]
+        L.tandem_kernel_class_name.restype = C.c_char_p
         L.tandem_free.argtypes = [C.c_void_p]
         L.tandem_free.restype = None
         L.tandem_last_error.argtypes = [C.c_void_p]
@@ -208,6 +216,20 @@ class Tandem:
 
     def reset(self):
         self._check(lib().tandem_reset(self._h))
+
+    def get_stats(self):
+        st = _Stats()
+        self._check(lib().tandem_get_stats(self._h, C.byref(st)))
+        return {n: getattr(st, n) for n, _ in _Stats._fields_}
+
+    def set_profile(self, enable):
+        self._check(lib().tandem_set_profile(self._h, 1 if enable else 0))
+
+    def get_profile(self):
+        """dict kernel class name -> (device milliseconds, launches) accumulated while profiling was enabled."""
+        ms = (C.c_double * KC_NUM)(); n = (C.c_int64 * KC_NUM)()
+        self._check(lib().tandem_get_profile(self._h, ms, n))
+        return {lib().tandem_kernel_class_name(i).decode(): (ms[i], n[i]) for i in range(KC_NUM)}
 
     def free(self):
         if self._h:

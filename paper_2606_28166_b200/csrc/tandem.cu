@@ -78,6 +78,13 @@ struct tandem_handle {
   // graph of one step
   cudaGraphExec_t graph = nullptr; GraphKey gkey;
   TcGemmPlans* tc = nullptr;
+  // launch accounting and the optional per-kernel-class timing mode (tandem_set_profile)
+  int64_t launches = 0, graph_launches = 0;
+  bool profile = false;
+  std::vector<cudaEvent_t> ev_pool; size_t ev_used = 0;
+  struct ProfRec { int cls; cudaEvent_t e0, e1; };
+  std::vector<ProfRec> prof_pending;
+  double prof_ms[TANDEM_KC_NUM] = {}; int64_t prof_n[TANDEM_KC_NUM] = {};
 };
 
 namespace {
@@ -102,6 +109,26 @@ template <typename P> int dmalloc(tandem_handle* h, P** p, size_t bytes) {
 }
 #define DM(h, p, bytes) do { int rc__ = dmalloc((h), (p), (bytes)); if (rc__) return rc__; } while (0)
 
+// Every kernel launch of a step goes through KL: it counts the launch and, in profile mode, brackets it with a
+// pair of timing events on its stream (the step then runs un-captured on one stream, see run_step).
+cudaEvent_t prof_event(tandem_handle* h) {
+  if (h->ev_used == h->ev_pool.size()) { cudaEvent_t e; cudaEventCreate(&e); h->ev_pool.push_back(e); }
+  return h->ev_pool[h->ev_used++];
+}
+#define KL(h, cls, stream, ...)                                                   \
+  do {                                                                            \
+    ++(h)->launches;                                                              \
+    if ((h)->profile) {                                                           \
+      cudaEvent_t e0__ = prof_event(h), e1__ = prof_event(h);                     \
+      cudaEventRecord(e0__, (stream));                                            \
+      __VA_ARGS__;                                                                \
+      cudaEventRecord(e1__, (stream));                                            \
+      (h)->prof_pending.push_back({(cls), e0__, e1__});                           \
+    } else {                                                                      \
+      __VA_ARGS__;                                                                \
+    }                                                                             \
+  } while (0)
+
 // ------------------------------------------------------------------------------------------ GEMM dispatch
 // out[s][r][n] partials (s < *n_split, stride *split_stride floats); rows read from counts_ptr[idx] on the device.
 template <typename T>
@@ -109,11 +136,14 @@ int launch_gemm(tandem_handle* h, int m, int which, int layer, const void* A, co
                 const int32_t* rows_ptr, int rows_cap, int* n_split, size_t* split_stride, cudaStream_t s) {
   *n_split = 1;
   *split_stride = (size_t)rows_cap * N;
+  static const int cls_of[5] = {TANDEM_KC_GEMM_QKV, TANDEM_KC_GEMM_O, TANDEM_KC_GEMM_GATEUP, TANDEM_KC_GEMM_DOWN, TANDEM_KC_GEMM_LMHEAD};
   if (h->gemm_impl == TANDEM_GEMM_TCGEN05 && sizeof(T) == 2) {
-    return tc_gemm_launch(h->tc, m, which, layer, A, W, N, K, out, rows_ptr, rows_cap, n_split, split_stride, s);
+    int rc = 0;
+    KL(h, cls_of[which], s, rc = tc_gemm_launch(h->tc, m, which, layer, A, W, N, K, out, rows_ptr, rows_cap, n_split, split_stride, s));
+    return rc == 0 ? TANDEM_OK : fail(h, rc, "tcgen05 GEMM launch failed (tensor map encode or K % 8 != 0)");
   }
   dim3 grid((N + kSimtTile - 1) / kSimtTile, std::min((rows_cap + kSimtTile - 1) / kSimtTile, 16));
-  gemm_simt_kernel<T><<<grid, 256, 0, s>>>(rows_ptr, 0, (const T*)A, (const T*)W, out, N, K);
+  KL(h, cls_of[which], s, (gemm_simt_kernel<T><<<grid, 256, 0, s>>>(rows_ptr, 0, (const T*)A, (const T*)W, out, N, K)));
   return TANDEM_OK;
 }
 
@@ -157,35 +187,37 @@ int model_forward(tandem_handle* h, int m, const StepIO& io, const RuleParams& r
   const size_t half_kv = (size_t)h->pool_pages * nkv * kPageTokens * d;
   int ns; size_t ss; int rc;
 
-  embed_norm_kernel<T, 256><<<row_grid, 256, 0, s>>>(tb.counts, tb.row_tok, (const T*)w.embed, (const T*)w.attn_norm[0], ws.x, (T*)ws.act, H, c.rms_eps);
+  KL(h, TANDEM_KC_EMBED, s, (embed_norm_kernel<T, 256><<<row_grid, 256, 0, s>>>(tb.counts, tb.row_tok, (const T*)w.embed, (const T*)w.attn_norm[0], ws.x, (T*)ws.act, H, c.rms_eps)));
   for (int l = 0; l < c.n_layers; ++l) {
     T* kpool = (T*)ws.kv + (size_t)l * layer_kv;
     T* vpool = kpool + half_kv;
     // S3 QKV projection
     if ((rc = launch_gemm<T>(h, m, 0, l, ws.act, w.wqkv[l], qkv_n, H, ws.gemm_out, tb.counts + C_ROWS, h->row_cap, &ns, &ss, s))) return rc;
     // S4 RoPE + KV append
-    rope_append_kernel<T, 256><<<row_grid, 256, 0, s>>>(tb.counts, tb.row_pos, tb.row_kvslot, ws.gemm_out, ns, ss, h->rope_cs, ws.q, kpool, vpool, nq, nkv, d);
+    KL(h, TANDEM_KC_ROPE_APPEND, s, (rope_append_kernel<T, 256><<<row_grid, 256, 0, s>>>(tb.counts, tb.row_pos, tb.row_kvslot, ws.gemm_out, ns, ss, h->rope_cs, ws.q, kpool, vpool, nq, nkv, d)));
     // S5 attention (decode splits + catch-up rows), then combine
     AttnArgs<T> aa{tb.counts, tb.item_row, tb.item_split, tb.item_part, tb.row_slot, tb.row_pos, h->pt[m].bt, h->max_pages, ws.q, kpool, vpool,
                    (T*)ws.attn_out, ws.part_acc, ws.part_ml, nq, nkv, 1.0f / sqrtf((float)d)};
-    if (!AttnDispatch<T>::run(aa, d, nq / nkv, 148 * 4, s)) return fail(h, TANDEM_EINVAL, "unsupported (head_dim, group) for attention");
+    bool ok = true;
+    KL(h, TANDEM_KC_ATTENTION, s, ok = AttnDispatch<T>::run(aa, d, nq / nkv, 148 * 4, s));
+    if (!ok) return fail(h, TANDEM_EINVAL, "unsupported (head_dim, group) for attention");
     CombineArgs<T> ca{tb.counts, tb.comb_row, tb.comb_part0, tb.comb_n, ws.part_acc, ws.part_ml, (T*)ws.attn_out, nq, d};
-    attn_combine_kernel<T><<<148, 256, 0, s>>>(ca);
+    KL(h, TANDEM_KC_ATTN_COMBINE, s, (attn_combine_kernel<T><<<148, 256, 0, s>>>(ca)));
     // S6 O projection + residual + RMSNorm(mlp)
     if ((rc = launch_gemm<T>(h, m, 1, l, ws.attn_out, w.wo[l], H, nq * d, ws.gemm_out, tb.counts + C_ROWS, h->row_cap, &ns, &ss, s))) return rc;
-    residual_norm_kernel<T, 256><<<row_grid, 256, 0, s>>>(tb.counts, ws.gemm_out, ns, ss, ws.x, (const T*)w.mlp_norm[l], (T*)ws.act, nullptr, H, c.rms_eps);
+    KL(h, TANDEM_KC_RESIDUAL_NORM, s, (residual_norm_kernel<T, 256><<<row_grid, 256, 0, s>>>(tb.counts, ws.gemm_out, ns, ss, ws.x, (const T*)w.mlp_norm[l], (T*)ws.act, nullptr, H, c.rms_eps)));
     // S7 gate/up + SwiGLU, down + residual + RMSNorm(next layer | final)
     if ((rc = launch_gemm<T>(h, m, 2, l, ws.act, w.wgu[l], 2 * I, H, ws.gemm_out, tb.counts + C_ROWS, h->row_cap, &ns, &ss, s))) return rc;
-    swiglu_kernel<T, 256><<<row_grid, 256, 0, s>>>(tb.counts, ws.gemm_out, ns, ss, (T*)ws.mlp_act, I);
+    KL(h, TANDEM_KC_SWIGLU, s, (swiglu_kernel<T, 256><<<row_grid, 256, 0, s>>>(tb.counts, ws.gemm_out, ns, ss, (T*)ws.mlp_act, I)));
     if ((rc = launch_gemm<T>(h, m, 3, l, ws.mlp_act, w.wdown[l], H, I, ws.gemm_out, tb.counts + C_ROWS, h->row_cap, &ns, &ss, s))) return rc;
     const bool last = l == c.n_layers - 1;
-    residual_norm_kernel<T, 256><<<row_grid, 256, 0, s>>>(tb.counts, ws.gemm_out, ns, ss, ws.x, (const T*)(last ? w.final_norm : w.attn_norm[l + 1]),
-                                                         (T*)(last ? ws.lm_in : ws.act), last ? tb.row_emit : nullptr, H, c.rms_eps);
+    KL(h, TANDEM_KC_RESIDUAL_NORM, s, (residual_norm_kernel<T, 256><<<row_grid, 256, 0, s>>>(tb.counts, ws.gemm_out, ns, ss, ws.x, (const T*)(last ? w.final_norm : w.attn_norm[l + 1]),
+                                                         (T*)(last ? ws.lm_in : ws.act), last ? tb.row_emit : nullptr, H, c.rms_eps)));
   }
   // S8 LM head on the emitting rows only, then sample + switch + emit
   if ((rc = launch_gemm<T>(h, m, 4, 0, ws.lm_in, w.lm_head, V, H, ws.logits, tb.counts + C_EMIT, c.max_seqs, &ns, &ss, s))) return rc;
   SampleArgs sa{h->st, tb, io, rp, ws.logits, h->word_start_dev, h->tokens, h->out_owner, h->out_logp, V, c.max_seq_len, m};
-  sample_switch_emit_kernel<256><<<c.max_seqs, 256, 0, s>>>(sa);
+  KL(h, TANDEM_KC_SAMPLE, s, (sample_switch_emit_kernel<256><<<c.max_seqs, 256, 0, s>>>(sa)));
   return TANDEM_OK;
 }
 
@@ -195,7 +227,16 @@ int launch_step(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaSt
   sa.st = h->st; sa.pt[0] = h->pt[0]; sa.pt[1] = h->pt[1]; sa.tab[0] = h->tab[0]; sa.tab[1] = h->tab[1];
   sa.io = io; sa.stats = h->stats; sa.tokens = h->tokens; sa.max_seqs = c.max_seqs; sa.max_seq_len = c.max_seq_len;
   sa.max_pages = h->max_pages; sa.row_cap = h->row_cap; sa.max_splits = h->max_splits;
-  sched_kernel<<<1, 1024, 0, s>>>(sa);
+  KL(h, TANDEM_KC_SCHED, s, (sched_kernel<<<1, 1024, 0, s>>>(sa)));
+  if (h->profile) {   // one stream, one kernel at a time: each kernel's duration is its own
+    for (int m = 0; m < 2; ++m) {
+      const int rc = (c.dtype == TANDEM_F32) ? model_forward<float>(h, m, io, rp, s) : model_forward<bf16>(h, m, io, rp, s);
+      if (rc) return rc;
+    }
+    FinalArgs fa{h->st, {h->pt[0], h->pt[1]}, io, h->stats, h->n_active, c.max_seqs, h->max_pages, h->pool_pages};
+    KL(h, TANDEM_KC_FINALIZE, s, (finalize_kernel<<<1, 1024, 0, s>>>(fa)));
+    return TANDEM_OK;
+  }
   CU(h, cudaEventRecord(h->ev_fork, s));
   for (int m = 0; m < 2; ++m) {
     CU(h, cudaStreamWaitEvent(h->ms[m], h->ev_fork, 0));
@@ -205,12 +246,24 @@ int launch_step(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaSt
     CU(h, cudaStreamWaitEvent(s, h->ev_join[m], 0));
   }
   FinalArgs fa{h->st, {h->pt[0], h->pt[1]}, io, h->stats, h->n_active, c.max_seqs, h->max_pages, h->pool_pages};
-  finalize_kernel<<<1, 1024, 0, s>>>(fa);
+  KL(h, TANDEM_KC_FINALIZE, s, (finalize_kernel<<<1, 1024, 0, s>>>(fa)));
   return TANDEM_OK;
 }
 
 // One step, through the captured graph when enabled and the (io, rule) key is unchanged.
 int run_step(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaStream_t s) {
+  if (h->profile) {
+    h->ev_used = 0; h->prof_pending.clear();
+    const int rc = launch_step(h, io, rp, s);
+    if (rc) return rc;
+    CU(h, cudaStreamSynchronize(s));
+    for (const auto& r : h->prof_pending) {
+      float ms = 0.f;
+      CU(h, cudaEventElapsedTime(&ms, r.e0, r.e1));
+      h->prof_ms[r.cls] += ms; h->prof_n[r.cls] += 1;
+    }
+    return TANDEM_OK;
+  }
   if (!h->cfg.use_graph) {
     const int rc = launch_step(h, io, rp, s);
     if (rc) return rc;
@@ -222,6 +275,7 @@ int run_step(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaStrea
     if (h->graph) { cudaGraphExecDestroy(h->graph); h->graph = nullptr; }
     h->gkey.valid = false;
     cudaGraph_t g = nullptr;
+    const int64_t l0 = h->launches;
     CU(h, cudaStreamBeginCapture(h->gs, cudaStreamCaptureModeThreadLocal));
     const int rc = launch_step(h, io, rp, h->gs);
     cudaError_t e = cudaStreamEndCapture(h->gs, &g);
@@ -230,7 +284,10 @@ int run_step(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaStrea
     CU(h, cudaGraphInstantiate(&h->graph, g, 0));
     cudaGraphDestroy(g);
     h->gkey.io = io; h->gkey.rp = rp; h->gkey.valid = true;
+    h->graph_launches = h->launches - l0;
+    h->launches = l0;   // capturing launched nothing
   }
+  h->launches += h->graph_launches;
   CU(h, cudaEventRecord(h->ev_in, s));
   CU(h, cudaStreamWaitEvent(h->gs, h->ev_in, 0));
   CU(h, cudaGraphLaunch(h->graph, h->gs));
@@ -325,6 +382,23 @@ int admit(tandem_handle* h, const tandem_params* p, const tandem_overrides* ovr,
   CU(h, cudaGetLastError());
   CU(h, cudaStreamSynchronize(s));
   for (int i = 0; i < n; ++i) { h->slot_busy[slots[i]] = 1; if (slots_out) slots_out[i] = slots[i]; }
+  return TANDEM_OK;
+}
+
+int fill_stats(tandem_handle* h, tandem_stats* stats) {
+  const tandem_config& c = h->cfg;
+  DevStats d;
+  CU(h, cudaMemcpy(&d, h->stats, sizeof(d), cudaMemcpyDeviceToHost));
+  const int H = c.hidden, I = c.intermediate, qd = c.n_q_heads * c.head_dim, kd = c.n_kv_heads * c.head_dim;
+  const int64_t per_layer = (int64_t)H * qd + 2ll * H * kd + (int64_t)qd * H + 3ll * H * I + 2ll * H;
+  const int64_t wbytes = ((int64_t)c.n_layers * per_layer + H + (int64_t)c.vocab * H) * h->esize;
+  stats->steps = (int64_t)d.steps; stats->tokens_emitted = (int64_t)d.tokens_emitted;
+  stats->rows_senior = (int64_t)d.rows[0]; stats->rows_junior = (int64_t)d.rows[1]; stats->catchup_rows = (int64_t)d.catchup_rows;
+  stats->kv_bytes_read = (int64_t)d.kv_tokens_read * 2ll * c.n_layers * kd * h->esize;
+  stats->weight_bytes_read = (int64_t)d.model_steps * wbytes;
+  stats->peak_pages_senior = d.peak_pages_used[0]; stats->peak_pages_junior = d.peak_pages_used[1]; stats->peak_resident = d.peak_resident;
+  stats->seconds_total = 0.0;
+  stats->kernel_launches = h->launches;
   return TANDEM_OK;
 }
 
@@ -498,7 +572,34 @@ int tandem_reset(tandem_handle* h) {
     CU(h, cudaMemset(h->ws[m].npages, 0, (size_t)S * 4));
   }
   std::fill(h->slot_busy.begin(), h->slot_busy.end(), 0);
+  h->launches = 0;
   return TANDEM_OK;
+}
+
+int tandem_get_stats(tandem_handle* h, tandem_stats* out) {
+  if (!h || !out) return TANDEM_EINVAL;
+  CU(h, cudaDeviceSynchronize());
+  return fill_stats(h, out);
+}
+
+int tandem_set_profile(tandem_handle* h, int enable) {
+  if (!h) return TANDEM_EINVAL;
+  CU(h, cudaDeviceSynchronize());
+  h->profile = enable != 0;
+  if (enable) for (int i = 0; i < TANDEM_KC_NUM; ++i) { h->prof_ms[i] = 0.0; h->prof_n[i] = 0; }
+  return TANDEM_OK;
+}
+
+int tandem_get_profile(tandem_handle* h, double* ms, int64_t* launches) {
+  if (!h || !ms || !launches) return TANDEM_EINVAL;
+  for (int i = 0; i < TANDEM_KC_NUM; ++i) { ms[i] = h->prof_ms[i]; launches[i] = h->prof_n[i]; }
+  return TANDEM_OK;
+}
+
+const char* tandem_kernel_class_name(int kc) {
+  static const char* names[TANDEM_KC_NUM] = {"sched", "embed_norm", "gemm_qkv", "rope_append", "attention", "attn_combine", "gemm_o",
+                                             "residual_norm", "gemm_gateup", "swiglu", "gemm_down", "gemm_lmhead", "sample_switch_emit", "finalize"};
+  return (kc >= 0 && kc < TANDEM_KC_NUM) ? names[kc] : "?";
 }
 
 int tandem_load_weights(tandem_handle* h, int model, const tandem_weights* w) {
@@ -619,16 +720,7 @@ int tandem_generate(tandem_handle* h, const tandem_params* params, int32_t B, co
   cudaEventDestroy(e0); cudaEventDestroy(e1);
   if ((rc = check_oom(h, s))) return rc;
   if (stats) {
-    DevStats d;
-    CU(h, cudaMemcpy(&d, h->stats, sizeof(d), cudaMemcpyDeviceToHost));
-    const int H = c.hidden, I = c.intermediate, qd = c.n_q_heads * c.head_dim, kd = c.n_kv_heads * c.head_dim;
-    const int64_t per_layer = (int64_t)H * qd + 2ll * H * kd + (int64_t)qd * H + 3ll * H * I + 2ll * H;
-    const int64_t wbytes = ((int64_t)c.n_layers * per_layer + H + (int64_t)c.vocab * H) * h->esize;
-    stats->steps = (int64_t)d.steps; stats->tokens_emitted = (int64_t)d.tokens_emitted;
-    stats->rows_senior = (int64_t)d.rows[0]; stats->rows_junior = (int64_t)d.rows[1]; stats->catchup_rows = (int64_t)d.catchup_rows;
-    stats->kv_bytes_read = (int64_t)d.kv_tokens_read * 2ll * c.n_layers * kd * h->esize;
-    stats->weight_bytes_read = (int64_t)d.model_steps * wbytes;
-    stats->peak_pages_senior = d.peak_pages_used[0]; stats->peak_pages_junior = d.peak_pages_used[1]; stats->peak_resident = d.peak_resident;
+    if ((rc = fill_stats(h, stats))) return rc;
     stats->seconds_total = ms * 1e-3;
   }
   return TANDEM_OK;
@@ -650,6 +742,7 @@ void tandem_free(tandem_handle* h) {
     if (h->ms[m]) cudaStreamDestroy(h->ms[m]);
     if (h->ev_join[m]) cudaEventDestroy(h->ev_join[m]);
   }
+  for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
   if (h->ev_fork) cudaEventDestroy(h->ev_fork);
   if (h->ev_in) cudaEventDestroy(h->ev_in);
   if (h->ev_out) cudaEventDestroy(h->ev_out);
