@@ -1,8 +1,10 @@
 // attention.cuh - S5a split-KV GQA decode attention and S5b ragged catch-up attention over paged KV
 // (DESIGN.md section 6). Plain ALUs (fp32 FMA), 128-bit loads of K/V, warp-shuffle reductions.
 // One work unit = (attention item, kv head): all G = n_q/n_kv query heads of the group share every K/V load.
-//   item of a decode row (q_len = 1): one kAttnChunk-position split of its KV range -> partial (m, l, acc)
-//   item of a catch-up/prefill row:   the row's whole causal range [0, pos], written directly
+//   item = n_tok consecutive rows of one sequence x one KV range [kv0, kv1) (common.cuh StepTab): a single-q-tile
+//   sequence is split along KV -> partial (m, l, acc) per row and split; q-tiles of longer runs are written directly.
+// This kernel walks the rows of an item one by one on plain ALUs: it is the fp32 path (configs[0]) and the reference the
+// tensor-core kernel of attention_mma.cuh is tested against.
 // softmax(q.K^T / sqrt(d)) V with q-head a reading kv-head a / G (oracle/model.py states the same definition).
 #pragma once
 #include "common.cuh"
@@ -10,7 +12,7 @@
 namespace tandem {
 
 template <typename T> struct AttnArgs {
-  const int32_t* counts; const int32_t* item_row; const int32_t* item_split; const int32_t* item_part;
+  const int32_t* counts; const int32_t* item_row0; const int32_t* item_ntok; const int32_t* item_kv0; const int32_t* item_kv1; const int32_t* item_part;
   const int32_t* row_slot; const int32_t* row_pos; const int32_t* bt; int max_pages;
   const float* q;            // [rows, nq*D] fp32, RoPE applied
   const T* kpool; const T* vpool;  // this layer: [pages, nkv, kPageTokens, D]
@@ -59,12 +61,13 @@ __global__ void __launch_bounds__(kAttnThreads) paged_attention_kernel(AttnArgs<
 
   for (int unit = blockIdx.x; unit < n_units; unit += gridDim.x) {
     const int item = unit / a.nkv, kvh = unit - item * a.nkv;
-    const int row = a.item_row[item], part = a.item_part[item];
-    const int slot = a.row_slot[row];
-    const int kv_len = a.row_pos[row] + 1;
-    const int kv0 = part >= 0 ? a.item_split[item] * kAttnChunk : 0;
-    const int kv1 = part >= 0 ? min(kv_len, kv0 + kAttnChunk) : kv_len;
+    const int row0 = a.item_row0[item], n_tok = a.item_ntok[item], part0 = a.item_part[item];
+    const int slot = a.row_slot[row0];
+    const int kv0 = a.item_kv0[item];
     const int32_t* bt = a.bt + (size_t)slot * a.max_pages;
+   for (int tok = 0; tok < n_tok; ++tok) {
+    const int row = row0 + tok, part = part0 >= 0 ? part0 + tok : -1;
+    const int kv1 = min(a.item_kv1[item], a.row_pos[row] + 1);   // causal bound of this row; may be <= kv0 (empty partial)
 
     float qv[G][VEC], acc[G][VEC], m_run[G], l_run[G];
 #pragma unroll
@@ -194,12 +197,13 @@ __global__ void __launch_bounds__(kAttnThreads) paged_attention_kernel(AttnArgs<
       }
     }
     __syncthreads();
+   }
   }
 }
 
 // Combine the splits of a decode row: out = sum_i e^{m_i - m} acc_i / sum_i e^{m_i - m} l_i.
 template <typename T> struct CombineArgs {
-  const int32_t* counts; const int32_t* comb_row; const int32_t* comb_part0; const int32_t* comb_n;
+  const int32_t* counts; const int32_t* comb_row; const int32_t* comb_part0; const int32_t* comb_n; const int32_t* comb_stride;
   const float* part_acc; const float2* part_ml; T* out; int nq, d;
 };
 template <typename T>
@@ -207,17 +211,17 @@ __global__ void __launch_bounds__(256) attn_combine_kernel(CombineArgs<T> a) {
   const int n_units = a.counts[C_COMB] * a.nq;
   for (int unit = blockIdx.x * (blockDim.x / 32) + (threadIdx.x >> 5); unit < n_units; unit += gridDim.x * (blockDim.x / 32)) {
     const int c = unit / a.nq, head = unit - c * a.nq;
-    const int row = a.comb_row[c], p0 = a.comb_part0[c], n = a.comb_n[c];
+    const int row = a.comb_row[c], p0 = a.comb_part0[c], n = a.comb_n[c], ps = a.comb_stride[c];
     const int lane = threadIdx.x & 31;
     float m = -INFINITY;
-    for (int i = 0; i < n; ++i) m = fmaxf(m, a.part_ml[(size_t)(p0 + i) * a.nq + head].x);
+    for (int i = 0; i < n; ++i) m = fmaxf(m, a.part_ml[(size_t)(p0 + i * ps) * a.nq + head].x);
     float l = 0.f;
-    for (int i = 0; i < n; ++i) { const float2 ml = a.part_ml[(size_t)(p0 + i) * a.nq + head]; l += __expf(ml.x - m) * ml.y; }
+    for (int i = 0; i < n; ++i) { const float2 ml = a.part_ml[(size_t)(p0 + i * ps) * a.nq + head]; l += __expf(ml.x - m) * ml.y; }
     for (int e = lane; e < a.d; e += 32) {
       float v = 0.f;
       for (int i = 0; i < n; ++i) {
-        const float w = __expf(a.part_ml[(size_t)(p0 + i) * a.nq + head].x - m);
-        v += w * a.part_acc[((size_t)(p0 + i) * a.nq + head) * a.d + e];
+        const float w = __expf(a.part_ml[(size_t)(p0 + i * ps) * a.nq + head].x - m);
+        v += w * a.part_acc[((size_t)(p0 + i * ps) * a.nq + head) * a.d + e];
       }
       Elem<T>::st(a.out + (size_t)row * a.nq * a.d + head * a.d + e, v / l);
     }

@@ -9,7 +9,15 @@
 namespace tandem {
 
 constexpr int kPageTokens = 16;      // KV page size (BASELINE.json configs[2]: "paged KV with 16-token blocks")
-constexpr int kAttnChunk = 256;      // KV positions per split of a decode row; a function of kv_len only (determinism)
+constexpr int kAttnMinChunk = 256;   // smallest KV split of an attention item
+constexpr int kAttnMaxSplits = 8;    // an item is split along KV into at most this many chunks
+constexpr int kAttnTileRows = 64;    // (query token, q-head of the group) rows per attention item = 4 MMA m-tiles
+// KV positions per split for a context of kv_len positions: a function of kv_len only, so the reduction order of a row
+// never depends on what else is in the batch (batch invariance).
+__host__ __device__ __forceinline__ int attn_chunk(int kv_len) {
+  const int c = ((kv_len + kAttnMaxSplits - 1) / kAttnMaxSplits + 63) & ~63;
+  return c > kAttnMinChunk ? c : kAttnMinChunk;
+}
 constexpr int kMaxSlots = 1024;      // scheduler is one CTA with one thread per slot
 
 typedef __nv_bfloat16 bf16;
@@ -37,12 +45,16 @@ struct StepTab {
   int32_t* row_kvslot;  // [R] physical KV token index: page * kPageTokens + pos % kPageTokens
   int32_t* row_emit;    // [R] emit index j if this is the last row of a sequence that emits this step, else -1
   int32_t* emit_slot;   // [max_seqs] slot of emit index j
-  int32_t* item_row;    // [I] attention work item -> row
-  int32_t* item_split;  // [I] split index along KV (0 if unsplit)
-  int32_t* item_part;   // [I] partial-buffer index, or -1 if the item writes the final output
-  int32_t* comb_row;    // [max_seqs] rows whose splits must be combined
-  int32_t* comb_part0;  // [max_seqs] first partial of that row
-  int32_t* comb_n;      // [max_seqs] number of partials
+  // attention work items: item = n_tok consecutive rows of one sequence (one q-tile) x one KV range [kv0, kv1)
+  int32_t* item_row0;   // [I] first row of the item
+  int32_t* item_ntok;   // [I] rows (query tokens) in the item, <= tile_tok = kAttnTileRows / group
+  int32_t* item_kv0;    // [I] first KV position of the item's range
+  int32_t* item_kv1;    // [I] one past the last KV position (causal bound of the item's last row, or the split end)
+  int32_t* item_part;   // [I] partial index of the item's first row (row j writes part + j), or -1: writes the final output
+  int32_t* comb_row;    // [C] rows whose splits must be combined
+  int32_t* comb_part0;  // [C] first partial of that row
+  int32_t* comb_n;      // [C] number of partials
+  int32_t* comb_stride; // [C] distance between consecutive partials of that row
 };
 
 struct SeqState {       // all [max_seqs]

@@ -13,7 +13,7 @@ namespace tandem {
 // position indices) - here per model, since the two models are no longer in lock-step.
 struct SchedArgs {
   SeqState st; PageTab pt[2]; StepTab tab[2]; StepIO io; DevStats* stats;
-  const int32_t* tokens; int max_seqs, max_seq_len, max_pages, row_cap, max_splits;
+  const int32_t* tokens; int max_seqs, max_seq_len, max_pages, row_cap, tile_tok;
 };
 
 __device__ __forceinline__ int block_excl_scan_1024(int v, int* total, int* wsum) {
@@ -94,22 +94,28 @@ __global__ void __launch_bounds__(1024) sched_kernel(SchedArgs a) {
     }
     int n_emit;
     const int j = block_excl_scan_1024(emits ? 1 : 0, &n_emit, wsum);
-    // attention items: a decode row (q_len == 1) is split along KV in chunks of kAttnChunk; rows of a
-    // multi-row sequence are one item each (parallelism comes from the rows).
-    const int nsplit = (rows == 1) ? (ing + 1 + kAttnChunk - 1) / kAttnChunk : 1;
-    const int items = (rows == 1) ? nsplit : rows;
-    const int parts = (rows == 1 && nsplit > 1) ? nsplit : 0;
+    // attention items (S5): the rows of a sequence are cut into q-tiles of tile_tok tokens; a sequence with a single
+    // q-tile (plain decode and short catch-ups) is also split along KV into n_split chunks whose partial (m, l, acc)
+    // are combined afterwards; longer runs (prompt prefill) get their parallelism from the q-tiles.
+    const int kv_len = ing + rows;
+    const int n_qt = (rows + a.tile_tok - 1) / a.tile_tok;
+    const int chunk = attn_chunk(kv_len);
+    const int nsplit = (n_qt == 1) ? (kv_len + chunk - 1) / chunk : 1;
+    const int items = (rows == 0) ? 0 : (n_qt == 1 ? nsplit : n_qt);
+    const int parts = (n_qt == 1 && nsplit > 1) ? nsplit * rows : 0;
     int n_items, n_parts, n_comb, n_sched;
     const int icu = block_excl_scan_1024(items, &n_items, wsum);
     const int pcu = block_excl_scan_1024(parts, &n_parts, wsum);
-    const int ccu = block_excl_scan_1024(parts > 0 ? 1 : 0, &n_comb, wsum);
+    const int ccu = block_excl_scan_1024(parts > 0 ? rows : 0, &n_comb, wsum);
     block_excl_scan_1024(rows > 0 ? 1 : 0, &n_sched, wsum);
 
     cu_rows[s] = cu; cu_items[s] = icu;
     sm_rows[s] = rows; sm_ing[s] = ing; sm_part0[s] = parts > 0 ? pcu : -1; sm_emit[s] = emits ? j : -1;
     if (s == 0) { cu_rows[kMaxSlots] = n_rows; cu_items[kMaxSlots] = n_items; }
     if (emits) tb.emit_slot[j] = s;
-    if (parts > 0) { tb.comb_row[ccu] = cu; tb.comb_part0[ccu] = pcu; tb.comb_n[ccu] = nsplit; }
+    for (int t = 0; t < (parts > 0 ? rows : 0); ++t) {
+      tb.comb_row[ccu + t] = cu + t; tb.comb_part0[ccu + t] = pcu + t; tb.comb_n[ccu + t] = nsplit; tb.comb_stride[ccu + t] = rows;
+    }
     if (rows > 0) a.st.ing[M][s] = ing + rows;  // commit: the forward below always runs
     __syncthreads();
 
@@ -126,11 +132,17 @@ __global__ void __launch_bounds__(1024) sched_kernel(SchedArgs a) {
     for (int i = threadIdx.x; i < n_items; i += blockDim.x) {
       const int q = find_owner_slot(cu_items, kMaxSlots, i);
       const int off = i - cu_items[q];
-      if (sm_rows[q] == 1) {
-        tb.item_row[i] = cu_rows[q]; tb.item_split[i] = off;
-        tb.item_part[i] = sm_part0[q] >= 0 ? sm_part0[q] + off : -1;
-      } else {
-        tb.item_row[i] = cu_rows[q] + off; tb.item_split[i] = 0; tb.item_part[i] = -1;
+      const int qrows = sm_rows[q], qkv = sm_ing[q] + qrows;
+      if (qrows <= a.tile_tok) {          // one q-tile, split `off` of the KV range
+        const int ch = attn_chunk(qkv);
+        tb.item_row0[i] = cu_rows[q]; tb.item_ntok[i] = qrows;
+        tb.item_kv0[i] = off * ch; tb.item_kv1[i] = min(qkv, (off + 1) * ch);
+        tb.item_part[i] = sm_part0[q] >= 0 ? sm_part0[q] + off * qrows : -1;
+      } else {                            // q-tile `off`, whole causal range
+        const int t0 = off * a.tile_tok, nt = min(a.tile_tok, qrows - t0);
+        tb.item_row0[i] = cu_rows[q] + t0; tb.item_ntok[i] = nt;
+        tb.item_kv0[i] = 0; tb.item_kv1[i] = sm_ing[q] + t0 + nt;
+        tb.item_part[i] = -1;
       }
     }
     if (threadIdx.x == 0) {

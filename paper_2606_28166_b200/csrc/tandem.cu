@@ -59,7 +59,7 @@ struct tandem_handle {
   std::string err;
   bool cuda_fault = false;
   int esize = 4;
-  int row_cap = 0, max_pages = 0, pool_pages = 0, max_splits = 0, max_items = 0, gemm_impl = TANDEM_GEMM_SIMT;
+  int row_cap = 0, max_pages = 0, pool_pages = 0, tile_tok = 0, max_items = 0, max_comb = 0, part_cap = 0, gemm_impl = TANDEM_GEMM_SIMT;
   size_t gemm_out_cols = 0;
   ModelWeights w[2];
   Workspace ws[2];
@@ -196,12 +196,12 @@ int model_forward(tandem_handle* h, int m, const StepIO& io, const RuleParams& r
     // S4 RoPE + KV append
     KL(h, TANDEM_KC_ROPE_APPEND, s, (rope_append_kernel<T, 256><<<row_grid, 256, 0, s>>>(tb.counts, tb.row_pos, tb.row_kvslot, ws.gemm_out, ns, ss, h->rope_cs, ws.q, kpool, vpool, nq, nkv, d)));
     // S5 attention (decode splits + catch-up rows), then combine
-    AttnArgs<T> aa{tb.counts, tb.item_row, tb.item_split, tb.item_part, tb.row_slot, tb.row_pos, h->pt[m].bt, h->max_pages, ws.q, kpool, vpool,
+    AttnArgs<T> aa{tb.counts, tb.item_row0, tb.item_ntok, tb.item_kv0, tb.item_kv1, tb.item_part, tb.row_slot, tb.row_pos, h->pt[m].bt, h->max_pages, ws.q, kpool, vpool,
                    (T*)ws.attn_out, ws.part_acc, ws.part_ml, nq, nkv, 1.0f / sqrtf((float)d)};
     bool ok = true;
     KL(h, TANDEM_KC_ATTENTION, s, ok = AttnDispatch<T>::run(aa, d, nq / nkv, 148 * 4, s));
     if (!ok) return fail(h, TANDEM_EINVAL, "unsupported (head_dim, group) for attention");
-    CombineArgs<T> ca{tb.counts, tb.comb_row, tb.comb_part0, tb.comb_n, ws.part_acc, ws.part_ml, (T*)ws.attn_out, nq, d};
+    CombineArgs<T> ca{tb.counts, tb.comb_row, tb.comb_part0, tb.comb_n, tb.comb_stride, ws.part_acc, ws.part_ml, (T*)ws.attn_out, nq, d};
     KL(h, TANDEM_KC_ATTN_COMBINE, s, (attn_combine_kernel<T><<<148, 256, 0, s>>>(ca)));
     // S6 O projection + residual + RMSNorm(mlp)
     if ((rc = launch_gemm<T>(h, m, 1, l, ws.attn_out, w.wo[l], H, nq * d, ws.gemm_out, tb.counts + C_ROWS, h->row_cap, &ns, &ss, s))) return rc;
@@ -226,7 +226,7 @@ int launch_step(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaSt
   SchedArgs sa{};
   sa.st = h->st; sa.pt[0] = h->pt[0]; sa.pt[1] = h->pt[1]; sa.tab[0] = h->tab[0]; sa.tab[1] = h->tab[1];
   sa.io = io; sa.stats = h->stats; sa.tokens = h->tokens; sa.max_seqs = c.max_seqs; sa.max_seq_len = c.max_seq_len;
-  sa.max_pages = h->max_pages; sa.row_cap = h->row_cap; sa.max_splits = h->max_splits;
+  sa.max_pages = h->max_pages; sa.row_cap = h->row_cap; sa.tile_tok = h->tile_tok;
   KL(h, TANDEM_KC_SCHED, s, (sched_kernel<<<1, 1024, 0, s>>>(sa)));
   if (h->profile) {   // one stream, one kernel at a time: each kernel's duration is its own
     for (int m = 0; m < 2; ++m) {
@@ -444,8 +444,10 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
   h->row_cap = c.max_rows_per_step > 0 ? c.max_rows_per_step : 4096;
   h->row_cap = std::max(h->row_cap, c.max_seqs);   // every owned sequence must be able to decode in one step
   h->max_pages = (c.max_seq_len + kPageTokens - 1) / kPageTokens;
-  h->max_splits = (c.max_seq_len + kAttnChunk - 1) / kAttnChunk;
-  h->max_items = h->row_cap + c.max_seqs * h->max_splits;
+  h->tile_tok = std::max(1, kAttnTileRows / (c.n_q_heads / c.n_kv_heads));
+  h->max_items = c.max_seqs * kAttnMaxSplits + h->row_cap;          // split single-tile sequences + q-tiles of longer runs
+  h->max_comb = std::min(c.max_seqs * h->tile_tok, h->row_cap);     // rows whose splits are combined
+  h->part_cap = h->max_comb * kAttnMaxSplits;                       // (row, split) partials
   const int H = c.hidden, nq = c.n_q_heads, nkv = c.n_kv_heads, d = c.head_dim, I = c.intermediate, V = c.vocab, R = h->row_cap, S = c.max_seqs;
   const size_t page_bytes = (size_t)2 * c.n_layers * nkv * kPageTokens * d * h->esize;
   h->pool_pages = c.kv_bytes_per_model > 0 ? (int)std::min<int64_t>(c.kv_bytes_per_model / (int64_t)page_bytes, (int64_t)1 << 30)
@@ -514,8 +516,8 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
     INIT_TRY(dmalloc(h, &w.lm_in, (size_t)std::max(S, 256) * H * h->esize));
     INIT_TRY(dmalloc(h, &w.gemm_out, (size_t)R * cols * 4));
     INIT_TRY(dmalloc(h, &w.logits, (size_t)S * V * 4));
-    INIT_TRY(dmalloc(h, &w.part_acc, (size_t)S * h->max_splits * nq * d * 4));
-    INIT_TRY(dmalloc(h, &w.part_ml, (size_t)S * h->max_splits * nq * sizeof(float2)));
+    INIT_TRY(dmalloc(h, &w.part_acc, (size_t)h->part_cap * nq * d * 4));
+    INIT_TRY(dmalloc(h, &w.part_ml, (size_t)h->part_cap * nq * sizeof(float2)));
     INIT_TRY(dmalloc(h, &w.kv, (size_t)h->pool_pages * page_bytes));
     // zero everything a TMA box or a padded MMA column may touch beyond the live rows
     INIT_CU(cudaMemset(w.act, 0, (size_t)R * H * h->esize));
@@ -524,14 +526,15 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
     INIT_CU(cudaMemset(w.lm_in, 0, (size_t)std::max(S, 256) * H * h->esize));
     INIT_CU(cudaMemset(w.kv, 0, (size_t)h->pool_pages * page_bytes));
     // step tables
-    const size_t tab_ints = (size_t)C_NUM + 5 * (size_t)R + (size_t)S + 3 * (size_t)h->max_items + 3 * (size_t)S;
+    const size_t tab_ints = (size_t)C_NUM + 5 * (size_t)R + (size_t)S + 5 * (size_t)h->max_items + 4 * (size_t)h->max_comb;
     INIT_TRY(dmalloc(h, &w.tab_mem, tab_ints * 4));
     INIT_CU(cudaMemset(w.tab_mem, 0, tab_ints * 4));
     {
       int32_t* p = w.tab_mem; StepTab& t = h->tab[m];
       t.counts = p; p += C_NUM; t.row_slot = p; p += R; t.row_pos = p; p += R; t.row_tok = p; p += R; t.row_kvslot = p; p += R; t.row_emit = p; p += R;
-      t.emit_slot = p; p += S; t.item_row = p; p += h->max_items; t.item_split = p; p += h->max_items; t.item_part = p; p += h->max_items;
-      t.comb_row = p; p += S; t.comb_part0 = p; p += S; t.comb_n = p; p += S;
+      t.emit_slot = p; p += S; t.item_row0 = p; p += h->max_items; t.item_ntok = p; p += h->max_items; t.item_kv0 = p; p += h->max_items;
+      t.item_kv1 = p; p += h->max_items; t.item_part = p; p += h->max_items;
+      t.comb_row = p; p += h->max_comb; t.comb_part0 = p; p += h->max_comb; t.comb_n = p; p += h->max_comb; t.comb_stride = p; p += h->max_comb;
     }
     // page tables
     INIT_TRY(dmalloc(h, &w.bt, (size_t)S * h->max_pages * 4));
