@@ -7,11 +7,11 @@ the symbol-export test can run without a GPU), but every compute call needs the 
 """
 from .binding import (lib, lib_path, TandemConfig, TandemParams, Tandem, TandemError,
                       tandem_test_uniforms, tandem_test_philox, tandem_test_gemm,
-                      SENIOR, JUNIOR, DRAW, TOGGLE, REDRAW, F32, BF16, GEMM_AUTO, GEMM_SIMT, GEMM_TCGEN05,
+                      SENIOR, JUNIOR, DRAW, TOGGLE, REDRAW, F32, BF16, GEMM_AUTO, GEMM_SIMT, GEMM_TCGEN05, ATTN_AUTO, ATTN_ALU, ATTN_MMA,
                       EXPORTED_SYMBOLS)
 from .build import build
 
 __all__ = ["lib", "lib_path", "TandemConfig", "TandemParams", "Tandem", "TandemError", "build",
            "tandem_test_uniforms", "tandem_test_philox", "tandem_test_gemm",
            "SENIOR", "JUNIOR", "DRAW", "TOGGLE", "REDRAW", "F32", "BF16",
-           "GEMM_AUTO", "GEMM_SIMT", "GEMM_TCGEN05", "EXPORTED_SYMBOLS"]
+           "GEMM_AUTO", "GEMM_SIMT", "GEMM_TCGEN05", "ATTN_AUTO", "ATTN_ALU", "ATTN_MMA", "EXPORTED_SYMBOLS"]

@@ -12,6 +12,7 @@ SENIOR, JUNIOR, DRAW = 0, 1, 2
 TOGGLE, REDRAW = 0, 1
 F32, BF16 = 0, 1
 GEMM_AUTO, GEMM_SIMT, GEMM_TCGEN05 = 0, 1, 2
+ATTN_AUTO, ATTN_ALU, ATTN_MMA = 0, 1, 2
 _ERR = {0: "OK", -1: "EINVAL", -2: "ENOMEM", -3: "ECUDA", -4: "ESTATE", -5: "EFULL"}
 
 EXPORTED_SYMBOLS = ["tandem_init", "tandem_load_weights", "tandem_step", "tandem_generate", "tandem_reset",
@@ -30,7 +31,7 @@ class _Config(C.Structure):
     _fields_ = [(n, C.c_int32) for n in ("n_layers", "hidden", "n_q_heads", "n_kv_heads", "head_dim", "intermediate", "vocab")] + \
                [("rms_eps", C.c_float), ("rope_theta", C.c_float), ("dtype", C.c_int32), ("page_tokens", C.c_int32),
                 ("max_seqs", C.c_int32), ("max_seq_len", C.c_int32), ("kv_bytes_per_model", C.c_int64), ("device", C.c_int32),
-                ("max_rows_per_step", C.c_int32), ("gemm_impl", C.c_int32), ("use_graph", C.c_int32), ("reserved", C.c_int32 * 4)]
+                ("max_rows_per_step", C.c_int32), ("gemm_impl", C.c_int32), ("use_graph", C.c_int32), ("attn_impl", C.c_int32), ("reserved", C.c_int32 * 3)]
 
 
 _PP = C.POINTER(C.c_void_p)
@@ -106,11 +107,11 @@ class TandemConfig:
     """Mirror of tandem_config. `shape` is any object with the model dimensions (e.g. workloads.ModelShape)."""
 
     def __init__(self, shape, max_seqs, max_seq_len, kv_bytes_per_model=0, device=0, max_rows_per_step=0,
-                 gemm_impl=GEMM_AUTO, use_graph=0, page_tokens=16):
+                 gemm_impl=GEMM_AUTO, use_graph=0, page_tokens=16, attn_impl=ATTN_AUTO):
         self.shape = shape
         self.c = _Config(shape.n_layers, shape.hidden, shape.n_q_heads, shape.n_kv_heads, shape.head_dim, shape.intermediate,
                          shape.vocab, shape.rms_eps, shape.rope_theta, F32 if shape.dtype == "f32" else BF16, page_tokens,
-                         max_seqs, max_seq_len, kv_bytes_per_model, device, max_rows_per_step, gemm_impl, use_graph)
+                         max_seqs, max_seq_len, kv_bytes_per_model, device, max_rows_per_step, gemm_impl, use_graph, attn_impl)
 
 
 class TandemParams:

@@ -273,11 +273,12 @@ __global__ void __launch_bounds__(NT) residual_norm_kernel(const int32_t* __rest
 
 // ============================================================================================ S4: RoPE + KV append
 // qkv[r, :] = sum_s part[s][r, :] is [q (nq*d) | k (nkv*d) | v (nkv*d)]. RoPE (half-split pairs (j, j+d/2), angle
-// pos * theta^(-2j/d) from a table built in double at init) on q and k; q -> fp32 buffer, k and v -> model M's pages.
-template <typename T, int NT>
+// pos * theta^(-2j/d) from a table built in double at init) on q and k; q -> buffer of type QT (fp32 for the ALU attention
+// kernel, bf16 for the tensor-core one), k and v -> model M's pages.
+template <typename T, typename QT, int NT>
 __global__ void __launch_bounds__(NT) rope_append_kernel(const int32_t* __restrict__ counts, const int32_t* __restrict__ row_pos,
                                                          const int32_t* __restrict__ row_kvslot, const float* __restrict__ part, int n_split,
-                                                         size_t split_stride, const float2* __restrict__ cs_table, float* __restrict__ q_out,
+                                                         size_t split_stride, const float2* __restrict__ cs_table, QT* __restrict__ q_out,
                                                          T* __restrict__ kpool, T* __restrict__ vpool, int nq, int nkv, int d) {
   const int n_rows = counts[C_ROWS];
   const int half = d >> 1;
@@ -296,8 +297,8 @@ __global__ void __launch_bounds__(NT) rope_append_kernel(const int32_t* __restri
       const float ra = a * cs.x - b * cs.y;
       const float rb = b * cs.x + a * cs.y;
       if (head < nq) {
-        q_out[(size_t)r * nq * d + head * d + j] = ra;
-        q_out[(size_t)r * nq * d + head * d + j + half] = rb;
+        Elem<QT>::st(q_out + (size_t)r * nq * d + head * d + j, ra);
+        Elem<QT>::st(q_out + (size_t)r * nq * d + head * d + j + half, rb);
       } else {
         const int kh = head - nq;
         T* dst = kpool + (((size_t)page * nkv + kh) * kPageTokens + off) * d;

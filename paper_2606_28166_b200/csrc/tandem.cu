@@ -16,6 +16,7 @@
 #include "common.cuh"
 #include "kernels.cuh"
 #include "attention.cuh"
+#include "attention_mma.cuh"
 #include "gemm_simt.cuh"
 #include "gemm_tcgen05.cuh"
 
@@ -32,7 +33,7 @@ struct ModelWeights {
 struct Workspace {  // per model, sized for row_cap rows
   float* x = nullptr;          // residual stream fp32 [R, H]
   void* act = nullptr;         // normalised activations (GEMM A operand) [R, H]
-  float* q = nullptr;          // RoPE'd queries fp32 [R, nq*d]
+  void* q = nullptr;           // RoPE'd queries [R, nq*d]: fp32 (ALU attention) or bf16 (tensor-core attention)
   void* attn_out = nullptr;    // [R, nq*d]
   void* mlp_act = nullptr;     // silu(gate)*up [R, I]
   void* lm_in = nullptr;       // final-normed last rows [max_seqs, H]
@@ -59,7 +60,8 @@ struct tandem_handle {
   std::string err;
   bool cuda_fault = false;
   int esize = 4;
-  int row_cap = 0, max_pages = 0, pool_pages = 0, tile_tok = 0, max_items = 0, max_comb = 0, part_cap = 0, gemm_impl = TANDEM_GEMM_SIMT;
+  int row_cap = 0, max_pages = 0, pool_pages = 0, tile_tok = 0, max_items = 0, max_comb = 0, part_cap = 0, gemm_impl = TANDEM_GEMM_SIMT, attn_impl = TANDEM_ATTN_ALU;
+  int n_sms = 148;
   size_t gemm_out_cols = 0;
   ModelWeights w[2];
   Workspace ws[2];
@@ -78,6 +80,8 @@ struct tandem_handle {
   // graph of one step
   cudaGraphExec_t graph = nullptr; GraphKey gkey;
   TcGemmPlans* tc = nullptr;
+  CUtensorMap kv_map_store[2];
+  const CUtensorMap* kv_map[2] = {nullptr, nullptr};   // each model's whole KV pool as rows of head_dim bf16 (tensor-core attention)
   // launch accounting and the optional per-kernel-class timing mode (tandem_set_profile)
   int64_t launches = 0, graph_launches = 0;
   bool profile = false;
@@ -168,6 +172,22 @@ template <> struct AttnDispatch<bf16> {
     return false;
   }
 };
+template <int D, int G> struct AmStages { static constexpr int value = D == 128 ? 2 : 4; };
+template <int D, int G>
+bool launch_attn_mma_dg(const CUtensorMap& map, const AttnMmaArgs& a, int grid, cudaStream_t s, bool set_attr) {
+  constexpr int ST = AmStages<D, G>::value;
+  constexpr int smem = attn_mma_smem_bytes<D, ST>();
+  if (set_attr) return cudaFuncSetAttribute(paged_attention_mma_kernel<D, G, ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) == cudaSuccess;
+  paged_attention_mma_kernel<D, G, ST><<<grid, kAmThreads, smem, s>>>(map, a);
+  return true;
+}
+// set_attr = true: only raise the kernel's dynamic shared memory limit (called once from tandem_init)
+bool run_attn_mma(const CUtensorMap& map, const AttnMmaArgs& a, int D, int G, int grid, cudaStream_t s, bool set_attr) {
+#define TD_CASE(d, g) if (D == d && G == g) return launch_attn_mma_dg<d, g>(map, a, grid, s, set_attr);
+  TD_CASE(64, 1) TD_CASE(64, 2) TD_CASE(64, 4) TD_CASE(64, 7) TD_CASE(64, 8) TD_CASE(128, 1) TD_CASE(128, 2) TD_CASE(128, 4) TD_CASE(128, 8)
+#undef TD_CASE
+  return false;
+}
 bool attn_supported(int dtype, int D, int G) {
   if (dtype == TANDEM_F32) return (D == 32 || D == 64 || D == 128) && (G == 1 || G == 2 || G == 4);
   return (D == 64 && (G == 1 || G == 2 || G == 4 || G == 7 || G == 8)) || (D == 128 && (G == 1 || G == 2 || G == 4 || G == 8));
@@ -194,12 +214,22 @@ int model_forward(tandem_handle* h, int m, const StepIO& io, const RuleParams& r
     // S3 QKV projection
     if ((rc = launch_gemm<T>(h, m, 0, l, ws.act, w.wqkv[l], qkv_n, H, ws.gemm_out, tb.counts + C_ROWS, h->row_cap, &ns, &ss, s))) return rc;
     // S4 RoPE + KV append
-    KL(h, TANDEM_KC_ROPE_APPEND, s, (rope_append_kernel<T, 256><<<row_grid, 256, 0, s>>>(tb.counts, tb.row_pos, tb.row_kvslot, ws.gemm_out, ns, ss, h->rope_cs, ws.q, kpool, vpool, nq, nkv, d)));
+    const bool mma = h->attn_impl == TANDEM_ATTN_MMA;
+    if (mma) KL(h, TANDEM_KC_ROPE_APPEND, s, (rope_append_kernel<T, bf16, 256><<<row_grid, 256, 0, s>>>(tb.counts, tb.row_pos, tb.row_kvslot, ws.gemm_out, ns, ss, h->rope_cs, (bf16*)ws.q, kpool, vpool, nq, nkv, d)));
+    else KL(h, TANDEM_KC_ROPE_APPEND, s, (rope_append_kernel<T, float, 256><<<row_grid, 256, 0, s>>>(tb.counts, tb.row_pos, tb.row_kvslot, ws.gemm_out, ns, ss, h->rope_cs, (float*)ws.q, kpool, vpool, nq, nkv, d)));
     // S5 attention (decode splits + catch-up rows), then combine
-    AttnArgs<T> aa{tb.counts, tb.item_row0, tb.item_ntok, tb.item_kv0, tb.item_kv1, tb.item_part, tb.row_slot, tb.row_pos, h->pt[m].bt, h->max_pages, ws.q, kpool, vpool,
-                   (T*)ws.attn_out, ws.part_acc, ws.part_ml, nq, nkv, 1.0f / sqrtf((float)d)};
     bool ok = true;
-    KL(h, TANDEM_KC_ATTENTION, s, ok = AttnDispatch<T>::run(aa, d, nq / nkv, 148 * 4, s));
+    if (mma) {
+      const long long rows_per_half = (long long)h->pool_pages * nkv * kPageTokens;
+      AttnMmaArgs ma{tb.counts, tb.item_row0, tb.item_ntok, tb.item_kv0, tb.item_kv1, tb.item_part, tb.row_slot, tb.row_pos, h->pt[m].bt, h->max_pages,
+                     (const bf16*)ws.q, (bf16*)ws.attn_out, ws.part_acc, ws.part_ml, nq, nkv, 1.0f / sqrtf((float)d),
+                     (int)((2ll * l) * rows_per_half), (int)((2ll * l + 1) * rows_per_half)};
+      KL(h, TANDEM_KC_ATTENTION, s, ok = run_attn_mma(*h->kv_map[m], ma, d, nq / nkv, 2 * h->n_sms, s, false));
+    } else {
+      AttnArgs<T> aa{tb.counts, tb.item_row0, tb.item_ntok, tb.item_kv0, tb.item_kv1, tb.item_part, tb.row_slot, tb.row_pos, h->pt[m].bt, h->max_pages, (const float*)ws.q, kpool, vpool,
+                     (T*)ws.attn_out, ws.part_acc, ws.part_ml, nq, nkv, 1.0f / sqrtf((float)d)};
+      KL(h, TANDEM_KC_ATTENTION, s, ok = AttnDispatch<T>::run(aa, d, nq / nkv, 148 * 4, s));
+    }
     if (!ok) return fail(h, TANDEM_EINVAL, "unsupported (head_dim, group) for attention");
     CombineArgs<T> ca{tb.counts, tb.comb_row, tb.comb_part0, tb.comb_n, tb.comb_stride, ws.part_acc, ws.part_ml, (T*)ws.attn_out, nq, d};
     KL(h, TANDEM_KC_ATTN_COMBINE, s, (attn_combine_kernel<T><<<148, 256, 0, s>>>(ca)));
@@ -436,7 +466,10 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
   if (c.max_seqs < 1 || c.max_seqs > kMaxSlots) return bad("max_seqs must be in 1..1024");
   if (c.max_seq_len < 2) return bad("bad max_seq_len");
   if (!attn_supported(c.dtype, c.head_dim, c.n_q_heads / c.n_kv_heads)) return bad("unsupported (head_dim, n_q/n_kv) combination");
-  for (int i = 0; i < 4; ++i) if (c.reserved[i]) return bad("reserved fields must be 0");
+  for (int i = 0; i < 3; ++i) if (c.reserved[i]) return bad("reserved fields must be 0");
+  if (c.attn_impl < 0 || c.attn_impl > 2) return bad("bad attn_impl");
+  h->attn_impl = c.attn_impl == TANDEM_ATTN_AUTO ? (c.dtype == TANDEM_BF16 ? TANDEM_ATTN_MMA : TANDEM_ATTN_ALU) : c.attn_impl;
+  if (h->attn_impl == TANDEM_ATTN_MMA && c.dtype != TANDEM_BF16) return bad("tensor-core attention needs bf16");
   if (cudaSetDevice(c.device) != cudaSuccess) { cudaGetLastError(); return bad("cudaSetDevice failed"); }
   h->esize = c.dtype == TANDEM_F32 ? 4 : 2;
   h->gemm_impl = c.gemm_impl == TANDEM_GEMM_AUTO ? (c.dtype == TANDEM_BF16 ? TANDEM_GEMM_TCGEN05 : TANDEM_GEMM_SIMT) : c.gemm_impl;
@@ -511,6 +544,7 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
     INIT_TRY(dmalloc(h, &w.x, (size_t)R * H * 4));
     INIT_TRY(dmalloc(h, &w.act, (size_t)R * H * h->esize));
     INIT_TRY(dmalloc(h, &w.q, (size_t)R * nq * d * 4));
+    INIT_CU(cudaMemset(w.q, 0, (size_t)R * nq * d * 4));
     INIT_TRY(dmalloc(h, &w.attn_out, (size_t)R * nq * d * h->esize));
     INIT_TRY(dmalloc(h, &w.mlp_act, (size_t)R * I * h->esize));
     INIT_TRY(dmalloc(h, &w.lm_in, (size_t)std::max(S, 256) * H * h->esize));
@@ -550,9 +584,29 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
   INIT_CU(cudaEventCreateWithFlags(&h->ev_in, cudaEventDisableTiming));
   INIT_CU(cudaEventCreateWithFlags(&h->ev_out, cudaEventDisableTiming));
   INIT_CU(cudaStreamCreateWithFlags(&h->gs, cudaStreamNonBlocking));
-  if (h->gemm_impl == TANDEM_GEMM_TCGEN05) {
+  {
+    int dev_sms = 0;
+    if (cudaDeviceGetAttribute(&dev_sms, cudaDevAttrMultiProcessorCount, c.device) == cudaSuccess && dev_sms > 0) h->n_sms = dev_sms;
+  }
+  if (h->gemm_impl == TANDEM_GEMM_TCGEN05 || h->attn_impl == TANDEM_ATTN_MMA) {
     h->tc = tc_gemm_create();
     if (!h->tc) { h->err = "tcgen05 GEMM setup failed (driver entry point for tensor maps not found)"; fprintf(stderr, "tandem_init: %s\n", h->err.c_str()); tandem_free(h); return TANDEM_ECUDA; }
+  }
+  if (h->attn_impl == TANDEM_ATTN_MMA) {
+    const long long total_rows = 2ll * c.n_layers * h->pool_pages * nkv * kPageTokens;
+    if (total_rows >= (1ll << 31)) return bad("KV pool too large for the attention tensor map (2^31 rows)");
+    for (int m = 0; m < 2; ++m) {
+      const CUtensorMap* mp = tc_gemm_map(h->tc, h->ws[m].kv, (int)total_rows, d, kPageTokens);
+      if (!mp) { h->err = "tensor map encode failed for the KV pool"; fprintf(stderr, "tandem_init: %s\n", h->err.c_str()); tandem_free(h); return TANDEM_ECUDA; }
+      h->kv_map_store[m] = *mp;
+      h->kv_map[m] = &h->kv_map_store[m];
+    }
+    AttnMmaArgs dummy{};
+    if (!run_attn_mma(h->kv_map_store[0], dummy, d, nq / nkv, 1, 0, true)) {
+      cudaGetLastError();
+      h->err = "tensor-core attention: unsupported (head_dim, group) or shared-memory limit"; fprintf(stderr, "tandem_init: %s\n", h->err.c_str());
+      tandem_free(h); return TANDEM_EINVAL;
+    }
   }
   INIT_TRY(tandem_reset(h));
   *out = h;
