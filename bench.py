@@ -49,6 +49,8 @@ def parse_args():
     ap.add_argument("--ramp", type=int, default=48, help="untimed steps after prefill so that both models own KV")
     ap.add_argument("--profile-steps", type=int, default=4)
     ap.add_argument("--e2e-new", type=int, default=32, help="new tokens per sequence in the end-to-end tandem_generate leg")
+    ap.add_argument("--profiler-range", action="store_true",
+                    help="cudaProfilerStart/Stop around the timed region (for `ncu --profile-from-start off`)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-new", type=int, default=4, help="new tokens of the oracle's bounded sample")
@@ -222,11 +224,15 @@ def run_ours(args):
     torch.cuda.synchronize()
     clocks = ClockSampler(local); clocks.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if args.profiler_range:
+        torch.cuda.profiler.start()
     e0.record()
     for _ in range(K):
         eng.step(prm, out=out, stream=stream)
     e1.record()
     torch.cuda.synchronize()
+    if args.profiler_range:
+        torch.cuda.profiler.stop()
     if dist: dist.barrier()
     ms = e0.elapsed_time(e1)
     clk = clocks.stop()

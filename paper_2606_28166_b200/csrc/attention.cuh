@@ -206,24 +206,35 @@ template <typename T> struct CombineArgs {
   const int32_t* counts; const int32_t* comb_row; const int32_t* comb_part0; const int32_t* comb_n; const int32_t* comb_stride;
   const float* part_acc; const float2* part_ml; T* out; int nq, d;
 };
+// One warp per (row, head); lane = 4 consecutive dims; all partial loads of a row are independent (n <= kAttnMaxSplits).
 template <typename T>
 __global__ void __launch_bounds__(256) attn_combine_kernel(CombineArgs<T> a) {
   const int n_units = a.counts[C_COMB] * a.nq;
+  const int lane = threadIdx.x & 31;
   for (int unit = blockIdx.x * (blockDim.x / 32) + (threadIdx.x >> 5); unit < n_units; unit += gridDim.x * (blockDim.x / 32)) {
     const int c = unit / a.nq, head = unit - c * a.nq;
     const int row = a.comb_row[c], p0 = a.comb_part0[c], n = a.comb_n[c], ps = a.comb_stride[c];
-    const int lane = threadIdx.x & 31;
+    float2 ml[kAttnMaxSplits];
     float m = -INFINITY;
-    for (int i = 0; i < n; ++i) m = fmaxf(m, a.part_ml[(size_t)(p0 + i * ps) * a.nq + head].x);
-    float l = 0.f;
-    for (int i = 0; i < n; ++i) { const float2 ml = a.part_ml[(size_t)(p0 + i * ps) * a.nq + head]; l += __expf(ml.x - m) * ml.y; }
-    for (int e = lane; e < a.d; e += 32) {
-      float v = 0.f;
-      for (int i = 0; i < n; ++i) {
-        const float w = __expf(a.part_ml[(size_t)(p0 + i * ps) * a.nq + head].x - m);
-        v += w * a.part_acc[((size_t)(p0 + i * ps) * a.nq + head) * a.d + e];
+#pragma unroll
+    for (int i = 0; i < kAttnMaxSplits; ++i) {
+      ml[i] = i < n ? a.part_ml[(size_t)(p0 + i * ps) * a.nq + head] : make_float2(-INFINITY, 0.f);
+      m = fmaxf(m, ml[i].x);
+    }
+    float l = 0.f, w[kAttnMaxSplits];
+#pragma unroll
+    for (int i = 0; i < kAttnMaxSplits; ++i) { w[i] = i < n ? __expf(ml[i].x - m) : 0.f; l += w[i] * ml[i].y; }
+    for (int e = 4 * lane; e < a.d; e += 128) {
+      float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+      for (int i = 0; i < kAttnMaxSplits; ++i) {
+        if (i < n) {
+          const float4 t = ld4(a.part_acc + ((size_t)(p0 + i * ps) * a.nq + head) * a.d + e);
+          v.x += w[i] * t.x; v.y += w[i] * t.y; v.z += w[i] * t.z; v.w += w[i] * t.w;
+        }
       }
-      Elem<T>::st(a.out + (size_t)row * a.nq * a.d + head * a.d + e, v / l);
+      const float inv = 1.f / l;
+      st4(a.out + (size_t)row * a.nq * a.d + head * a.d + e, make_float4(v.x * inv, v.y * inv, v.z * inv, v.w * inv));
     }
   }
 }

@@ -32,6 +32,20 @@ template <> struct Elem<bf16> {
   static __device__ __forceinline__ void st(bf16* p, float v) { *p = __float2bfloat16_rn(v); }
 };
 
+// 4 consecutive elements <-> 4 floats (16-byte fp32 / 8-byte bf16 accesses; pointers must be aligned accordingly)
+__device__ __forceinline__ float4 ld4(const float* p) { return *reinterpret_cast<const float4*>(p); }
+__device__ __forceinline__ float4 ld4(const bf16* p) {
+  const uint2 t = *reinterpret_cast<const uint2*>(p);
+  return make_float4(__uint_as_float(t.x << 16), __uint_as_float(t.x & 0xffff0000u), __uint_as_float(t.y << 16), __uint_as_float(t.y & 0xffff0000u));
+}
+__device__ __forceinline__ void st4(float* p, float4 v) { *reinterpret_cast<float4*>(p) = v; }
+__device__ __forceinline__ void st4(bf16* p, float4 v) {
+  const __nv_bfloat162 a = __floats2bfloat162_rn(v.x, v.y), b = __floats2bfloat162_rn(v.z, v.w);
+  uint2 t; t.x = *reinterpret_cast<const uint32_t*>(&a); t.y = *reinterpret_cast<const uint32_t*>(&b);
+  *reinterpret_cast<uint2*>(p) = t;
+}
+__device__ __forceinline__ float4 add4(float4 a, float4 b) { return make_float4(a.x + b.x, a.y + b.y, a.z + b.z, a.w + b.w); }
+
 // counts[] indices of a per-model step table
 enum { C_ROWS = 0, C_SCHED = 1, C_EMIT = 2, C_ITEMS = 3, C_COMB = 4, C_PARTS = 5, C_NUM = 8 };
 

@@ -247,69 +247,99 @@ __global__ void __launch_bounds__(NT) embed_norm_kernel(const int32_t* __restric
 }
 
 // ============================================================================================ S6/S7: residual + RMSNorm
-// x[r,:] += sum_s part[s][r,:]; u = RMSNorm(x; gain) -> act. With out_map (last layer): only rows that emit are
-// normalised (with the final-norm gain) and written compactly at their emit index (the LM head runs on those only).
-template <typename T, int NT>
+// x[r,:] += sum_s part[s][r,:] (ascending s); u = RMSNorm(x; gain) -> act. With out_map (last layer): only rows that emit
+// are normalised (with the final-norm gain) and written compactly at their emit index (the LM head runs on those only).
+// One CTA per row; every thread keeps its VPT float4 of the row in registers, and the loads of all splits are
+// independent of each other, so a row costs ~one memory latency instead of n_split * H / NT of them.
+template <typename T, int NT, int VPT>
 __global__ void __launch_bounds__(NT) residual_norm_kernel(const int32_t* __restrict__ counts, const float* __restrict__ part, int n_split,
                                                            size_t split_stride, float* __restrict__ x, const T* __restrict__ gain,
                                                            T* __restrict__ act, const int32_t* __restrict__ out_map, int H, float eps) {
   __shared__ float red[32];
   const int n_rows = counts[C_ROWS];
+  const int H4 = H >> 2;
   for (int r = blockIdx.x; r < n_rows; r += gridDim.x) {
-    float ss = 0.f;
-    for (int j = threadIdx.x; j < H; j += NT) {
-      float v = x[(size_t)r * H + j];
-      for (int s = 0; s < n_split; ++s) v += part[s * split_stride + (size_t)r * H + j];
-      x[(size_t)r * H + j] = v;
-      ss += v * v;
+    float4 v[VPT];
+#pragma unroll
+    for (int i = 0; i < VPT; ++i) {
+      const int j4 = threadIdx.x + i * NT;
+      v[i] = j4 < H4 ? ld4(x + (size_t)r * H + 4 * j4) : make_float4(0.f, 0.f, 0.f, 0.f);
     }
-    int orow = r;
-    if (out_map) { orow = out_map[r]; }
+#pragma unroll 4
+    for (int s = 0; s < n_split; ++s) {
+#pragma unroll
+      for (int i = 0; i < VPT; ++i) {
+        const int j4 = threadIdx.x + i * NT;
+        if (j4 < H4) v[i] = add4(v[i], ld4(part + s * split_stride + (size_t)r * H + 4 * j4));
+      }
+    }
+    float ss = 0.f;
+#pragma unroll
+    for (int i = 0; i < VPT; ++i) {
+      const int j4 = threadIdx.x + i * NT;
+      if (j4 < H4) st4(x + (size_t)r * H + 4 * j4, v[i]);
+      ss += v[i].x * v[i].x + v[i].y * v[i].y + v[i].z * v[i].z + v[i].w * v[i].w;
+    }
+    const int orow = out_map ? out_map[r] : r;
     const float inv = rsqrtf(block_sum<NT>(ss, red) / (float)H + eps);
     if (orow < 0) continue;
-    for (int j = threadIdx.x; j < H; j += NT) Elem<T>::st(act + (size_t)orow * H + j, x[(size_t)r * H + j] * Elem<T>::ld(gain + j) * inv);
+#pragma unroll
+    for (int i = 0; i < VPT; ++i) {
+      const int j4 = threadIdx.x + i * NT;
+      if (j4 < H4) {
+        const float4 g = ld4(gain + 4 * j4);
+        st4(act + (size_t)orow * H + 4 * j4, make_float4(v[i].x * g.x * inv, v[i].y * g.y * inv, v[i].z * g.z * inv, v[i].w * g.w * inv));
+      }
+    }
   }
 }
 
 // ============================================================================================ S4: RoPE + KV append
 // qkv[r, :] = sum_s part[s][r, :] is [q (nq*d) | k (nkv*d) | v (nkv*d)]. RoPE (half-split pairs (j, j+d/2), angle
 // pos * theta^(-2j/d) from a table built in double at init) on q and k; q -> buffer of type QT (fp32 for the ALU attention
-// kernel, bf16 for the tensor-core one), k and v -> model M's pages.
+// kernel, bf16 for the tensor-core one), k and v -> model M's pages. Four pairs / four v elements per thread per step.
 template <typename T, typename QT, int NT>
 __global__ void __launch_bounds__(NT) rope_append_kernel(const int32_t* __restrict__ counts, const int32_t* __restrict__ row_pos,
                                                          const int32_t* __restrict__ row_kvslot, const float* __restrict__ part, int n_split,
                                                          size_t split_stride, const float2* __restrict__ cs_table, QT* __restrict__ q_out,
                                                          T* __restrict__ kpool, T* __restrict__ vpool, int nq, int nkv, int d) {
   const int n_rows = counts[C_ROWS];
-  const int half = d >> 1;
+  const int half = d >> 1, hq = half >> 2;                 // hq: groups of 4 pairs per head
   const int ld = (nq + 2 * nkv) * d;
-  const int n_pairs = (nq + nkv) * half;
+  const int n_rot = (nq + nkv) * hq, n_v = nkv * (d >> 2);
   for (int r = blockIdx.x; r < n_rows; r += gridDim.x) {
     const int pos = row_pos[r];
     const int kvslot = row_kvslot[r];
     const int page = kvslot / kPageTokens, off = kvslot % kPageTokens;
     const float* src = part + (size_t)r * ld;
-    for (int i = threadIdx.x; i < n_pairs; i += NT) {
-      const int head = i / half, j = i - head * half;
-      float a = 0.f, b = 0.f;
-      for (int s = 0; s < n_split; ++s) { a += src[s * split_stride + head * d + j]; b += src[s * split_stride + head * d + j + half]; }
-      const float2 cs = cs_table[(size_t)pos * half + j];
-      const float ra = a * cs.x - b * cs.y;
-      const float rb = b * cs.x + a * cs.y;
-      if (head < nq) {
-        Elem<QT>::st(q_out + (size_t)r * nq * d + head * d + j, ra);
-        Elem<QT>::st(q_out + (size_t)r * nq * d + head * d + j + half, rb);
+    for (int i = threadIdx.x; i < n_rot + n_v; i += NT) {
+      if (i < n_rot) {
+        const int head = i / hq, j = (i - head * hq) << 2;
+        float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a;
+#pragma unroll 4
+        for (int s = 0; s < n_split; ++s) {
+          a = add4(a, ld4(src + s * split_stride + head * d + j));
+          b = add4(b, ld4(src + s * split_stride + head * d + j + half));
+        }
+        const float4 c01 = *reinterpret_cast<const float4*>(cs_table + (size_t)pos * half + j);       // (cos, sin) of pairs j, j+1
+        const float4 c23 = *reinterpret_cast<const float4*>(cs_table + (size_t)pos * half + j + 2);
+        const float4 ra = make_float4(a.x * c01.x - b.x * c01.y, a.y * c01.z - b.y * c01.w, a.z * c23.x - b.z * c23.y, a.w * c23.z - b.w * c23.w);
+        const float4 rb = make_float4(b.x * c01.x + a.x * c01.y, b.y * c01.z + a.y * c01.w, b.z * c23.x + a.z * c23.y, b.w * c23.z + a.w * c23.w);
+        if (head < nq) {
+          st4(q_out + (size_t)r * nq * d + head * d + j, ra);
+          st4(q_out + (size_t)r * nq * d + head * d + j + half, rb);
+        } else {
+          T* dst = kpool + (((size_t)page * nkv + (head - nq)) * kPageTokens + off) * d;
+          st4(dst + j, ra); st4(dst + j + half, rb);
+        }
       } else {
-        const int kh = head - nq;
-        T* dst = kpool + (((size_t)page * nkv + kh) * kPageTokens + off) * d;
-        Elem<T>::st(dst + j, ra); Elem<T>::st(dst + j + half, rb);
+        const int e = (i - n_rot) << 2;                      // element index within [nkv * d)
+        float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll 4
+        for (int s = 0; s < n_split; ++s) v = add4(v, ld4(src + s * split_stride + (nq + nkv) * d + e));
+        const int kh = e / d;
+        st4(vpool + (((size_t)page * nkv + kh) * kPageTokens + off) * d + (e - kh * d), v);
       }
-    }
-    for (int i = threadIdx.x; i < nkv * d; i += NT) {
-      const int kh = i / d, e = i - kh * d;
-      float v = 0.f;
-      for (int s = 0; s < n_split; ++s) v += src[s * split_stride + (nq + nkv) * d + i];
-      Elem<T>::st(vpool + (((size_t)page * nkv + kh) * kPageTokens + off) * d + e, v);
     }
   }
 }
@@ -320,12 +350,18 @@ template <typename T, int NT>
 __global__ void __launch_bounds__(NT) swiglu_kernel(const int32_t* __restrict__ counts, const float* __restrict__ part, int n_split,
                                                     size_t split_stride, T* __restrict__ out, int I) {
   const int n_rows = counts[C_ROWS];
-  const size_t total = (size_t)n_rows * I;
+  const int I4 = I >> 2;
+  const size_t total = (size_t)n_rows * I4;
   for (size_t idx = (size_t)blockIdx.x * NT + threadIdx.x; idx < total; idx += (size_t)gridDim.x * NT) {
-    const size_t r = idx / I, j = idx - r * I;
-    float g = 0.f, u = 0.f;
-    for (int s = 0; s < n_split; ++s) { g += part[s * split_stride + r * 2 * I + j]; u += part[s * split_stride + r * 2 * I + I + j]; }
-    Elem<T>::st(out + idx, g / (1.f + expf(-g)) * u);
+    const size_t r = idx / I4, j = (idx - r * I4) << 2;
+    float4 g = make_float4(0.f, 0.f, 0.f, 0.f), u = g;
+#pragma unroll 4
+    for (int s = 0; s < n_split; ++s) {
+      g = add4(g, ld4(part + s * split_stride + r * 2 * I + j));
+      u = add4(u, ld4(part + s * split_stride + r * 2 * I + I + j));
+    }
+    st4(out + r * I + j, make_float4(g.x / (1.f + expf(-g.x)) * u.x, g.y / (1.f + expf(-g.y)) * u.y,
+                                     g.z / (1.f + expf(-g.z)) * u.z, g.w / (1.f + expf(-g.w)) * u.w));
   }
 }
 

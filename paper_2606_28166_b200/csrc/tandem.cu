@@ -151,6 +151,16 @@ int launch_gemm(tandem_handle* h, int m, int which, int layer, const void* A, co
   return TANDEM_OK;
 }
 
+template <typename T>
+void launch_residual_norm(tandem_handle* h, cudaStream_t s, int grid, const int32_t* counts, const float* part, int ns, size_t ss, float* x,
+                          const T* gain, T* act, const int32_t* out_map, int H, float eps) {
+  const int v = (H / 4 + 255) / 256;   // float4 per thread; tandem_init guarantees H % 8 == 0 and H <= 8192
+  if (v <= 1) KL(h, TANDEM_KC_RESIDUAL_NORM, s, (residual_norm_kernel<T, 256, 1><<<grid, 256, 0, s>>>(counts, part, ns, ss, x, gain, act, out_map, H, eps)));
+  else if (v <= 2) KL(h, TANDEM_KC_RESIDUAL_NORM, s, (residual_norm_kernel<T, 256, 2><<<grid, 256, 0, s>>>(counts, part, ns, ss, x, gain, act, out_map, H, eps)));
+  else if (v <= 4) KL(h, TANDEM_KC_RESIDUAL_NORM, s, (residual_norm_kernel<T, 256, 4><<<grid, 256, 0, s>>>(counts, part, ns, ss, x, gain, act, out_map, H, eps)));
+  else KL(h, TANDEM_KC_RESIDUAL_NORM, s, (residual_norm_kernel<T, 256, 8><<<grid, 256, 0, s>>>(counts, part, ns, ss, x, gain, act, out_map, H, eps)));
+}
+
 template <typename T, int D, int G>
 void launch_attn_dg(const AttnArgs<T>& a, int grid, cudaStream_t s) {
   paged_attention_kernel<T, D, G><<<grid, kAttnThreads, 0, s>>>(a);
@@ -235,14 +245,14 @@ int model_forward(tandem_handle* h, int m, const StepIO& io, const RuleParams& r
     KL(h, TANDEM_KC_ATTN_COMBINE, s, (attn_combine_kernel<T><<<148, 256, 0, s>>>(ca)));
     // S6 O projection + residual + RMSNorm(mlp)
     if ((rc = launch_gemm<T>(h, m, 1, l, ws.attn_out, w.wo[l], H, nq * d, ws.gemm_out, tb.counts + C_ROWS, h->row_cap, &ns, &ss, s))) return rc;
-    KL(h, TANDEM_KC_RESIDUAL_NORM, s, (residual_norm_kernel<T, 256><<<row_grid, 256, 0, s>>>(tb.counts, ws.gemm_out, ns, ss, ws.x, (const T*)w.mlp_norm[l], (T*)ws.act, nullptr, H, c.rms_eps)));
+    launch_residual_norm<T>(h, s, row_grid, tb.counts, ws.gemm_out, ns, ss, ws.x, (const T*)w.mlp_norm[l], (T*)ws.act, nullptr, H, c.rms_eps);
     // S7 gate/up + SwiGLU, down + residual + RMSNorm(next layer | final)
     if ((rc = launch_gemm<T>(h, m, 2, l, ws.act, w.wgu[l], 2 * I, H, ws.gemm_out, tb.counts + C_ROWS, h->row_cap, &ns, &ss, s))) return rc;
     KL(h, TANDEM_KC_SWIGLU, s, (swiglu_kernel<T, 256><<<row_grid, 256, 0, s>>>(tb.counts, ws.gemm_out, ns, ss, (T*)ws.mlp_act, I)));
     if ((rc = launch_gemm<T>(h, m, 3, l, ws.mlp_act, w.wdown[l], H, I, ws.gemm_out, tb.counts + C_ROWS, h->row_cap, &ns, &ss, s))) return rc;
     const bool last = l == c.n_layers - 1;
-    KL(h, TANDEM_KC_RESIDUAL_NORM, s, (residual_norm_kernel<T, 256><<<row_grid, 256, 0, s>>>(tb.counts, ws.gemm_out, ns, ss, ws.x, (const T*)(last ? w.final_norm : w.attn_norm[l + 1]),
-                                                         (T*)(last ? ws.lm_in : ws.act), last ? tb.row_emit : nullptr, H, c.rms_eps)));
+    launch_residual_norm<T>(h, s, row_grid, tb.counts, ws.gemm_out, ns, ss, ws.x, (const T*)(last ? w.final_norm : w.attn_norm[l + 1]),
+                            (T*)(last ? ws.lm_in : ws.act), last ? tb.row_emit : nullptr, H, c.rms_eps);
   }
   // S8 LM head on the emitting rows only, then sample + switch + emit
   if ((rc = launch_gemm<T>(h, m, 4, 0, ws.lm_in, w.lm_head, V, H, ws.logits, tb.counts + C_EMIT, c.max_seqs, &ns, &ss, s))) return rc;
@@ -461,6 +471,7 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
   auto bad = [&](const char* m) { int rc = fail(h, TANDEM_EINVAL, m); fprintf(stderr, "tandem_init: %s\n", m); delete h; return rc; };
   if (c.n_layers < 1 || c.hidden < 8 || c.n_q_heads < 1 || c.n_kv_heads < 1 || c.head_dim < 8 || c.intermediate < 8 || c.vocab < 2) return bad("bad model dimensions");
   if (c.n_q_heads % c.n_kv_heads) return bad("n_q_heads must be a multiple of n_kv_heads");
+  if ((c.hidden % 8) || (c.intermediate % 8) || (c.head_dim % 8) || c.hidden > 8192) return bad("hidden, intermediate, head_dim must be multiples of 8; hidden <= 8192");
   if (c.dtype != TANDEM_F32 && c.dtype != TANDEM_BF16) return bad("bad dtype");
   if (c.page_tokens != kPageTokens) return bad("page_tokens must be 16");
   if (c.max_seqs < 1 || c.max_seqs > kMaxSlots) return bad("max_seqs must be in 1..1024");
