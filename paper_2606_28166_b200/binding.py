@@ -17,7 +17,7 @@ _ERR = {0: "OK", -1: "EINVAL", -2: "ENOMEM", -3: "ECUDA", -4: "ESTATE", -5: "EFU
 
 EXPORTED_SYMBOLS = ["tandem_init", "tandem_load_weights", "tandem_step", "tandem_generate", "tandem_reset",
                     "tandem_free", "tandem_last_error", "tandem_get_stats", "tandem_set_profile", "tandem_get_profile",
-                    "tandem_kernel_class_name", "tandem_test_uniforms", "tandem_test_philox", "tandem_test_gemm"]
+                    "tandem_kernel_class_name", "tandem_test_uniforms", "tandem_test_philox", "tandem_test_gemm", "tandem_test_gemm_time"]
 KC_NUM = 14
 
 
@@ -99,6 +99,7 @@ def lib():
         L.tandem_test_uniforms.argtypes = [C.c_uint64, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_void_p]
         L.tandem_test_philox.argtypes = [C.POINTER(C.c_uint32), C.POINTER(C.c_uint32), C.POINTER(C.c_uint32)]
         L.tandem_test_gemm.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.tandem_test_gemm_time.argtypes = [C.c_int32] * 8 + [C.POINTER(C.c_float)]
         _lib = L
     return _lib
 
@@ -264,3 +265,11 @@ def tandem_test_gemm(dtype, impl, A, W, out):
     rc = lib().tandem_test_gemm(dtype, impl, rows, N, K, A.data_ptr(), W.data_ptr(), out.data_ptr())
     if rc:
         raise TandemError(rc)
+
+
+def tandem_test_gemm_time(rows, N, K, iters=50, cluster=0, ring_kb=0, splits=0, swiglu=0):
+    ms = C.c_float()
+    rc = lib().tandem_test_gemm_time(rows, N, K, iters, cluster, ring_kb, splits, swiglu, C.byref(ms))
+    if rc:
+        raise TandemError(rc)
+    return ms.value

@@ -13,7 +13,9 @@
 //   as fit in 200 KB (4 at 256 rows, 6 at 128 rows, 9 at 32 rows).
 #pragma once
 #include <cuda.h>   // CUtensorMap and its enums only; the encode entry point is fetched at run time (no libcuda link)
+#include <algorithm>
 #include <map>
+#include <vector>
 #include <tuple>
 #include "common.cuh"
 
@@ -120,9 +122,34 @@ struct TcGemmArgs {
   int rows_fixed;
   int N, K, n_split;
   size_t split_stride;        // floats between partials
+  int ring_bytes;             // shared-memory ring of this launch (200 KB: one CTA per SM; 98 KB: two)
 };
 
 // ---------------------------------------------------------------------------------------------- the kernel
+namespace ptx {
+__device__ __forceinline__ uint32_t cluster_ctarank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ void cluster_sync() {
+  asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+  asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// the box lands at the same CTA-relative smem offset, and signals the mbarrier at the same offset, in every CTA of `mask`
+__device__ __forceinline__ void tma_load_2d_mc(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar, uint16_t mask, uint64_t policy) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster.L2::cache_hint [%0], [%1, {%2, %3}], [%4], %5, %6;"
+               ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar), "h"(mask), "l"(policy) : "memory");
+}
+__device__ __forceinline__ void umma_commit_mc(uint32_t bar, uint16_t mask) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(bar), "h"(mask) : "memory");
+}
+}  // namespace ptx
+
+enum { kTcEpiPartial = 0, kTcEpiSwiGLU = 1 };
+
+// CL   = CTAs per cluster along the weight tiles: they need the same activation tile, so each loads 1/CL of its 32-row boxes
+//        and multicasts them to all (L2 -> SM traffic of the activations / CL); a stage is released to the producers only
+//        when the MMAs of all CL CTAs have read it (commit multicast to every CTA's empty barrier).
+// EPI  = kTcEpiPartial: fp32 partial out[split][r][n];
+//        kTcEpiSwiGLU : W rows interleaved (2i = gate_i, 2i+1 = up_i), n_split = 1: act[r][i] = silu(gate) * up as bf16.
+template <int CL, int EPI>
 __global__ void __launch_bounds__(kTcThreads, 1)
 gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_constant__ CUtensorMap tmap_a, TcGemmArgs g) {
   extern __shared__ uint8_t tc_smem_raw[];
@@ -140,7 +167,9 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_con
   const int n_chunks = (rows + kTcMaxRows - 1) / kTcMaxRows;
   const int nbox_max = (min(rows, kTcMaxRows) + kTcRowBox - 1) / kTcRowBox;
   const int stage_bytes = kTcWBytes + nbox_max * kTcABoxBytes;
-  const int n_stages = min(kTcMaxStages, kTcRingBytes / stage_bytes);
+  const int n_stages = min(kTcMaxStages, g.ring_bytes / stage_bytes);
+  const uint32_t cta_rank = CL > 1 ? ptx::cluster_ctarank() : 0u;
+  constexpr uint16_t kMask = (uint16_t)((1u << CL) - 1u);
 
   const uint32_t ring = (ptx::smem_u32(tc_smem_raw) + 1023u) & ~1023u;   // 128B swizzle atoms are 1024-byte aligned
   const uint32_t bar0 = ptx::smem_u32(bars);
@@ -150,7 +179,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_con
   const uint32_t tmem_empty_bar = tmem_full_bar + 8u;
 
   if (threadIdx.x == 0) {
-    for (int s = 0; s < n_stages; ++s) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
+    for (int s = 0; s < n_stages; ++s) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), CL); }
     ptx::mbar_init(tmem_full_bar, 1);
     ptx::mbar_init(tmem_empty_bar, 4);
     ptx::fence_mbar_init();
@@ -159,12 +188,12 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_con
   }
   if (warp == 2) ptx::tmem_alloc<kTcMaxRows>(ptx::smem_u32(&tmem_base_smem));
   ptx::tc_fence_before();
-  __syncthreads();
+  if (CL > 1) ptx::cluster_sync(); else __syncthreads();   // peers' barriers must exist before anything is multicast to them
   ptx::tc_fence_after();
   const uint32_t tmem_base = tmem_base_smem;
 
   if (warp == 0) {
-    // ===== TMA producer: weights stream once (evict-first), activations are re-read by every CTA (evict-last)
+    // ===== TMA producer: weights stream once (evict-first), activations are shared by every CTA (evict-last)
     if (lane == 0) {
       const uint64_t pol_w = ptx::policy_evict_first(), pol_a = ptx::policy_evict_last();
       int it = 0;
@@ -178,8 +207,10 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_con
           const uint32_t dst = ring + (uint32_t)(s * stage_bytes);
           ptx::mbar_expect_tx(full_bar(s), (uint32_t)(kTcWBytes + nbox * kTcABoxBytes));
           ptx::tma_load_2d(dst, &tmap_w, kb * kTcBlockK, n0, full_bar(s), pol_w);
-          for (int j = 0; j < nbox; ++j)
-            ptx::tma_load_2d(dst + kTcWBytes + j * kTcABoxBytes, &tmap_a, kb * kTcBlockK, r0 + j * kTcRowBox, full_bar(s), pol_a);
+          for (int j = (int)cta_rank; j < nbox; j += CL) {
+            if (CL > 1) ptx::tma_load_2d_mc(dst + kTcWBytes + j * kTcABoxBytes, &tmap_a, kb * kTcBlockK, r0 + j * kTcRowBox, full_bar(s), kMask, pol_a);
+            else ptx::tma_load_2d(dst + kTcWBytes + j * kTcABoxBytes, &tmap_a, kb * kTcBlockK, r0 + j * kTcRowBox, full_bar(s), pol_a);
+          }
         }
       }
     }
@@ -203,7 +234,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_con
 #pragma unroll
           for (int k = 0; k < kTcBlockK / 16; ++k)   // UMMA K = 16 bf16 = 32 bytes: advance the start address inside the swizzle row
             ptx::umma_bf16(tmem_base, dw + (uint64_t)(2 * k), da + (uint64_t)(2 * k), idesc, (kb > kb0 || k > 0) ? 1u : 0u);
-          ptx::umma_commit(empty_bar(s));            // frees the smem stage once these MMAs have read it
+          if (CL > 1) ptx::umma_commit_mc(empty_bar(s), kMask); else ptx::umma_commit(empty_bar(s));   // stage free once these MMAs have read it
         }
         ptx::umma_commit(tmem_full_bar);             // accumulator of this chunk complete
       }
@@ -222,10 +253,27 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_con
         uint32_t v[32];
         ptx::tmem_ld32(tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)c0, v);
         ptx::tmem_ld_wait();
-        if (n < g.N) {
+        if (EPI == kTcEpiPartial) {
+          if (n < g.N) {
 #pragma unroll
-          for (int j = 0; j < 32; ++j)
-            if (c0 + j < crow) outp[(size_t)(r0 + c0 + j) * g.N + n] = __uint_as_float(v[j]);
+            for (int j = 0; j < 32; ++j)
+              if (c0 + j < crow) outp[(size_t)(r0 + c0 + j) * g.N + n] = __uint_as_float(v[j]);
+          }
+        } else {
+          // even lane = gate row i, odd lane = up row i of the same intermediate index i: swap halves of the 32 columns so
+          // that the even lane finishes columns [0,16) and the odd lane columns [16,32)
+          const bool odd = lane & 1;
+          const int i = n >> 1, I = g.N >> 1;
+          bf16* act = reinterpret_cast<bf16*>(g.out);
+#pragma unroll
+          for (int j = 0; j < 16; ++j) {
+            const float mine = __uint_as_float(odd ? v[16 + j] : v[j]);
+            const float send = __uint_as_float(odd ? v[j] : v[16 + j]);
+            const float recv = __shfl_xor_sync(0xffffffffu, send, 1);
+            const float gate = odd ? recv : mine, up = odd ? mine : recv;
+            const int r = c0 + (odd ? 16 : 0) + j;
+            if (r < crow && n < g.N) act[(size_t)(r0 + r) * I + i] = __float2bfloat16_rn(gate / (1.f + expf(-gate)) * up);
+          }
         }
       }
       ptx::tc_fence_before();
@@ -234,7 +282,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_con
     }
   }
   ptx::tc_fence_before();
-  __syncthreads();
+  if (CL > 1) ptx::cluster_sync(); else __syncthreads();   // no CTA leaves while a peer may still multicast into it
   if (warp == 2) ptx::tmem_dealloc<kTcMaxRows>(tmem_base);
 }
 
@@ -264,7 +312,14 @@ inline TcGemmPlans* tc_gemm_create() {
     cudaGetLastError();
     return nullptr;
   }
-  if (cudaFuncSetAttribute(gemm_tcgen05_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes) != cudaSuccess) {
+  bool ok = true;
+  ok &= cudaFuncSetAttribute(gemm_tcgen05_kernel<1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes) == cudaSuccess;
+  ok &= cudaFuncSetAttribute(gemm_tcgen05_kernel<2, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes) == cudaSuccess;
+  ok &= cudaFuncSetAttribute(gemm_tcgen05_kernel<4, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes) == cudaSuccess;
+  ok &= cudaFuncSetAttribute(gemm_tcgen05_kernel<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes) == cudaSuccess;
+  ok &= cudaFuncSetAttribute(gemm_tcgen05_kernel<2, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes) == cudaSuccess;
+  ok &= cudaFuncSetAttribute(gemm_tcgen05_kernel<4, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes) == cudaSuccess;
+  if (!ok) {
     cudaGetLastError();
     return nullptr;
   }
@@ -293,22 +348,49 @@ inline const CUtensorMap* tc_gemm_map(TcGemmPlans* p, const void* base, int n_ro
   return &(p->maps[key] = m);
 }
 
-// Launch on `s`. out receives *n_split partials, *split_stride floats apart. Returns 0, or -1 (TANDEM_EINVAL) / -3 (TANDEM_ECUDA).
+// Launch on `s`. out receives *n_split partials, *split_stride floats apart (epi = kTcEpiPartial), or the bf16 SwiGLU
+// activations [rows, N/2] (epi = kTcEpiSwiGLU; W rows interleaved gate/up). Returns 0, or -1 (TANDEM_EINVAL) / -3 (TANDEM_ECUDA).
 // which == 4 (LM head) never splits: the sampler reads the logits in place.
+template <int CL, int EPI>
+inline int tc_gemm_launch_cl(const CUtensorMap* mw, const CUtensorMap* ma, const TcGemmArgs& g, dim3 grid, cudaStream_t s) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = grid; cfg.blockDim = dim3(kTcThreads); cfg.dynamicSmemBytes = (size_t)g.ring_bytes + 1024; cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, gemm_tcgen05_kernel<CL, EPI>, *mw, *ma, g) == cudaSuccess ? 0 : -3;
+}
+struct TcGemmTune { int cl = 0, ring_kb = 0, splits = 0; };   // 0 = automatic; overrides for tandem_test_gemm_time only
 inline int tc_gemm_launch(TcGemmPlans* p, int /*model*/, int which, int /*layer*/, const void* A, const void* W, int N, int K, float* out,
-                          const int32_t* rows_ptr, int rows_cap, int* n_split, size_t* split_stride, cudaStream_t s) {
+                          const int32_t* rows_ptr, int rows_cap, int* n_split, size_t* split_stride, cudaStream_t s, int epi = kTcEpiPartial,
+                          const TcGemmTune* tune = nullptr) {
   if (!p || (K % 8) != 0) return -1;                       // TMA needs 16-byte row strides
   const CUtensorMap* mw = tc_gemm_map(p, W, N, K, kTcTileN);
   const CUtensorMap* ma = tc_gemm_map(p, A, rows_cap, K, kTcRowBox);
   if (!mw || !ma) return -3;
-  const int S = which == 4 ? 1 : tc_gemm_splits(N, K);
+  int S = (which == 4 || epi == kTcEpiSwiGLU) ? 1 : tc_gemm_splits(N, K);
+  if (tune && tune->splits > 0) S = tune->splits;
   *n_split = S;
   *split_stride = (size_t)rows_cap * N;
-  TcGemmArgs g{out, rows_ptr, rows_cap, N, K, S, *split_stride};
+  const int tiles = (N + kTcTileN - 1) / kTcTileN;
+  // Clusters with activation multicast are implemented (CL = 2, 4) but measured no faster than CL = 1 on B200 at any of the
+  // projection shapes (profiles/gemm_sweep_r1.md), so the automatic choice is 1; tandem_test_gemm_time can still select them.
+  int cl = 1;
+  if (tune && tune->cl > 0) cl = tune->cl;
+  const int tiles_pad = (tiles + cl - 1) / cl * cl;
+  TcGemmArgs g{out, rows_ptr, rows_cap, N, K, S, *split_stride, 0};
   if (!rows_ptr) g.rows_fixed = rows_cap;
-  dim3 grid((N + kTcTileN - 1) / kTcTileN, S);
-  gemm_tcgen05_kernel<<<grid, kTcThreads, kTcSmemBytes, s>>>(*mw, *ma, g);
-  return 0;
+  g.ring_bytes = tiles_pad * S > 148 ? 98 * 1024 : kTcRingBytes;     // more CTAs than SMs: let two share an SM
+  if (tune && tune->ring_kb > 0) g.ring_bytes = tune->ring_kb * 1024;
+  dim3 grid(tiles_pad, S);
+  if (epi == kTcEpiSwiGLU) {
+    if (cl == 4) return tc_gemm_launch_cl<4, 1>(mw, ma, g, grid, s);
+    if (cl == 2) return tc_gemm_launch_cl<2, 1>(mw, ma, g, grid, s);
+    return tc_gemm_launch_cl<1, 1>(mw, ma, g, grid, s);
+  }
+  if (cl == 4) return tc_gemm_launch_cl<4, 0>(mw, ma, g, grid, s);
+  if (cl == 2) return tc_gemm_launch_cl<2, 0>(mw, ma, g, grid, s);
+  return tc_gemm_launch_cl<1, 0>(mw, ma, g, grid, s);
 }
 
 // Unit-test hook: out[rows, N] = A W^T (partials summed here), synchronous.
@@ -319,10 +401,17 @@ __global__ void tc_sum_partials_kernel(const float* __restrict__ part, int n_spl
     out[i] = v;
   }
 }
-inline int tc_gemm_test(int rows, int N, int K, const void* A, const void* W, float* out) {
+inline int tc_gemm_test(int rows, int N, int K, const void* A, const void* W, float* out, int epi = kTcEpiPartial) {
   if (rows == 0) return 0;
   TcGemmPlans* p = tc_gemm_create();
   if (!p) return -3;
+  if (epi == kTcEpiSwiGLU) {   // W rows interleaved gate/up; out is bf16 [rows, N/2]
+    int ns; size_t ss;
+    int rc = tc_gemm_launch(p, 0, 2, 0, A, W, N, K, out, nullptr, rows, &ns, &ss, 0, epi);
+    if (rc == 0) rc = cudaDeviceSynchronize() == cudaSuccess ? 0 : -3;
+    tc_gemm_destroy(p);
+    return rc;
+  }
   const int S = tc_gemm_splits(N, K);
   float* part = nullptr;
   if (cudaMalloc(&part, (size_t)S * rows * N * sizeof(float)) != cudaSuccess) { tc_gemm_destroy(p); return -2; }
@@ -334,6 +423,42 @@ inline int tc_gemm_test(int rows, int N, int K, const void* A, const void* W, fl
   }
   cudaFree(part);
   tc_gemm_destroy(p);
+  return rc;
+}
+
+// Timing hook: `iters` back-to-back launches of the [rows, K] x [N, K]^T GEMM, each on a different weight buffer (enough
+// buffers to exceed the L2), between two CUDA events; returns the mean milliseconds per launch.
+inline int tc_gemm_time(int rows, int N, int K, int iters, const TcGemmTune& tune, int epi, float* ms_out) {
+  TcGemmPlans* p = tc_gemm_create();
+  if (!p) return -3;
+  const size_t wbytes = (size_t)N * K * 2;
+  const int nbuf = (int)std::min<size_t>(64, (400ull << 20) / wbytes + 2);
+  std::vector<void*> wb(nbuf, nullptr);
+  void* A = nullptr; float* out = nullptr;
+  int rc = 0;
+  const int S = tune.splits > 0 ? tune.splits : tc_gemm_splits(N, K);
+  for (int i = 0; i < nbuf && !rc; ++i) { if (cudaMalloc(&wb[i], wbytes) != cudaSuccess) rc = -2; else cudaMemset(wb[i], 0x11, wbytes); }
+  if (!rc && cudaMalloc(&A, (size_t)rows * K * 2) != cudaSuccess) rc = -2;
+  if (!rc && cudaMalloc(&out, (size_t)S * rows * N * 4) != cudaSuccess) rc = -2;
+  if (!rc) {
+    cudaMemset(A, 0x11, (size_t)rows * K * 2);
+    cudaEvent_t e0, e1; cudaEventCreate(&e0); cudaEventCreate(&e1);
+    int ns; size_t ss;
+    for (int i = 0; i < nbuf + iters && !rc; ++i) {
+      if (i == nbuf) cudaEventRecord(e0, 0);
+      rc = tc_gemm_launch(p, 0, epi == kTcEpiSwiGLU ? 2 : 0, 0, A, wb[i % nbuf], N, K, out, nullptr, rows, &ns, &ss, 0, epi, &tune);
+    }
+    cudaEventRecord(e1, 0);
+    if (cudaDeviceSynchronize() != cudaSuccess) rc = -3;
+    float ms = 0.f; cudaEventElapsedTime(&ms, e0, e1);
+    *ms_out = ms / iters;
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+  }
+  for (void* b : wb) if (b) cudaFree(b);
+  if (A) cudaFree(A);
+  if (out) cudaFree(out);
+  tc_gemm_destroy(p);
+  cudaGetLastError();
   return rc;
 }
 

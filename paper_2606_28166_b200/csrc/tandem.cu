@@ -137,13 +137,13 @@ cudaEvent_t prof_event(tandem_handle* h) {
 // out[s][r][n] partials (s < *n_split, stride *split_stride floats); rows read from counts_ptr[idx] on the device.
 template <typename T>
 int launch_gemm(tandem_handle* h, int m, int which, int layer, const void* A, const void* W, int N, int K, float* out,
-                const int32_t* rows_ptr, int rows_cap, int* n_split, size_t* split_stride, cudaStream_t s) {
+                const int32_t* rows_ptr, int rows_cap, int* n_split, size_t* split_stride, cudaStream_t s, int epi = kTcEpiPartial) {
   *n_split = 1;
   *split_stride = (size_t)rows_cap * N;
   static const int cls_of[5] = {TANDEM_KC_GEMM_QKV, TANDEM_KC_GEMM_O, TANDEM_KC_GEMM_GATEUP, TANDEM_KC_GEMM_DOWN, TANDEM_KC_GEMM_LMHEAD};
   if (h->gemm_impl == TANDEM_GEMM_TCGEN05 && sizeof(T) == 2) {
     int rc = 0;
-    KL(h, cls_of[which], s, rc = tc_gemm_launch(h->tc, m, which, layer, A, W, N, K, out, rows_ptr, rows_cap, n_split, split_stride, s));
+    KL(h, cls_of[which], s, rc = tc_gemm_launch(h->tc, m, which, layer, A, W, N, K, out, rows_ptr, rows_cap, n_split, split_stride, s, epi));
     return rc == 0 ? TANDEM_OK : fail(h, rc, "tcgen05 GEMM launch failed (tensor map encode or K % 8 != 0)");
   }
   dim3 grid((N + kSimtTile - 1) / kSimtTile, std::min((rows_cap + kSimtTile - 1) / kSimtTile, 16));
@@ -247,8 +247,12 @@ int model_forward(tandem_handle* h, int m, const StepIO& io, const RuleParams& r
     if ((rc = launch_gemm<T>(h, m, 1, l, ws.attn_out, w.wo[l], H, nq * d, ws.gemm_out, tb.counts + C_ROWS, h->row_cap, &ns, &ss, s))) return rc;
     launch_residual_norm<T>(h, s, row_grid, tb.counts, ws.gemm_out, ns, ss, ws.x, (const T*)w.mlp_norm[l], (T*)ws.act, nullptr, H, c.rms_eps);
     // S7 gate/up + SwiGLU, down + residual + RMSNorm(next layer | final)
-    if ((rc = launch_gemm<T>(h, m, 2, l, ws.act, w.wgu[l], 2 * I, H, ws.gemm_out, tb.counts + C_ROWS, h->row_cap, &ns, &ss, s))) return rc;
-    KL(h, TANDEM_KC_SWIGLU, s, (swiglu_kernel<T, 256><<<row_grid, 256, 0, s>>>(tb.counts, ws.gemm_out, ns, ss, (T*)ws.mlp_act, I)));
+    if (h->gemm_impl == TANDEM_GEMM_TCGEN05) {   // SwiGLU in the GEMM epilogue (gate/up rows interleaved at load time)
+      if ((rc = launch_gemm<T>(h, m, 2, l, ws.act, w.wgu[l], 2 * I, H, (float*)ws.mlp_act, tb.counts + C_ROWS, h->row_cap, &ns, &ss, s, kTcEpiSwiGLU))) return rc;
+    } else {
+      if ((rc = launch_gemm<T>(h, m, 2, l, ws.act, w.wgu[l], 2 * I, H, ws.gemm_out, tb.counts + C_ROWS, h->row_cap, &ns, &ss, s))) return rc;
+      KL(h, TANDEM_KC_SWIGLU, s, (swiglu_kernel<T, 256><<<row_grid, 256, 0, s>>>(tb.counts, ws.gemm_out, ns, ss, (T*)ws.mlp_act, I)));
+    }
     if ((rc = launch_gemm<T>(h, m, 3, l, ws.mlp_act, w.wdown[l], H, I, ws.gemm_out, tb.counts + C_ROWS, h->row_cap, &ns, &ss, s))) return rc;
     const bool last = l == c.n_layers - 1;
     launch_residual_norm<T>(h, s, row_grid, tb.counts, ws.gemm_out, ns, ss, ws.x, (const T*)(last ? w.final_norm : w.attn_norm[l + 1]),
@@ -699,8 +703,15 @@ int tandem_load_weights(tandem_handle* h, int model, const tandem_weights* w) {
     if ((rc = put(&mw.wqkv[l], qn + kn, w->wv[l], kn, qn + 2 * kn))) return rc;
     if ((rc = put(&mw.wo[l], 0, w->wo[l], (size_t)H * nq * d, (size_t)H * nq * d))) return rc;
     if ((rc = put(&mw.mlp_norm[l], 0, w->mlp_norm[l], H, H))) return rc;
-    if ((rc = put(&mw.wgu[l], 0, w->w_gate[l], (size_t)I * H, (size_t)2 * I * H))) return rc;   // [gate | up] rows
-    if ((rc = put(&mw.wgu[l], (size_t)I * H, w->w_up[l], (size_t)I * H, (size_t)2 * I * H))) return rc;
+    if (h->gemm_impl == TANDEM_GEMM_TCGEN05) {   // rows interleaved: 2i = gate_i, 2i+1 = up_i (SwiGLU runs in the GEMM epilogue)
+      if (!w->w_gate[l] || !w->w_up[l]) return fail(h, TANDEM_EINVAL, "NULL layer weight pointer");
+      if (!mw.wgu[l]) DM(h, (char**)&mw.wgu[l], (size_t)2 * I * H * es);
+      CU(h, cudaMemcpy2D(mw.wgu[l], (size_t)2 * H * es, w->w_gate[l], (size_t)H * es, (size_t)H * es, I, kind));
+      CU(h, cudaMemcpy2D((char*)mw.wgu[l] + (size_t)H * es, (size_t)2 * H * es, w->w_up[l], (size_t)H * es, (size_t)H * es, I, kind));
+    } else {
+      if ((rc = put(&mw.wgu[l], 0, w->w_gate[l], (size_t)I * H, (size_t)2 * I * H))) return rc;   // [gate | up] rows
+      if ((rc = put(&mw.wgu[l], (size_t)I * H, w->w_up[l], (size_t)I * H, (size_t)2 * I * H))) return rc;
+    }
     if ((rc = put(&mw.wdown[l], 0, w->w_down[l], (size_t)H * I, (size_t)H * I))) return rc;
   }
   CU(h, cudaDeviceSynchronize());
@@ -858,14 +869,21 @@ int tandem_test_philox(const uint32_t ctr[4], const uint32_t key[2], uint32_t ou
 
 int tandem_test_gemm(int32_t dtype, int32_t impl, int32_t rows, int32_t N, int32_t K, const void* A_dev, const void* W_dev, float* out_dev) {
   if (rows < 0 || N <= 0 || K <= 0 || !A_dev || !W_dev || !out_dev) return TANDEM_EINVAL;
-  if (impl == TANDEM_GEMM_TCGEN05) {
+  if (impl == TANDEM_GEMM_TCGEN05 || impl == 3) {
     if (dtype != TANDEM_BF16) return TANDEM_EINVAL;
-    return tc_gemm_test(rows, N, K, A_dev, W_dev, out_dev);
+    return tc_gemm_test(rows, N, K, A_dev, W_dev, out_dev, impl == 3 ? kTcEpiSwiGLU : kTcEpiPartial);
   }
   dim3 grid((N + kSimtTile - 1) / kSimtTile, std::max(1, std::min((rows + kSimtTile - 1) / kSimtTile, 64)));
   if (dtype == TANDEM_F32) gemm_simt_kernel<float><<<grid, 256>>>(nullptr, rows, (const float*)A_dev, (const float*)W_dev, out_dev, N, K);
   else gemm_simt_kernel<bf16><<<grid, 256>>>(nullptr, rows, (const bf16*)A_dev, (const bf16*)W_dev, out_dev, N, K);
   return cudaDeviceSynchronize() == cudaSuccess ? TANDEM_OK : TANDEM_ECUDA;
+}
+
+int tandem_test_gemm_time(int32_t rows, int32_t N, int32_t K, int32_t iters, int32_t cluster, int32_t ring_kb, int32_t splits, int32_t swiglu,
+                          float* ms_per_launch) {
+  if (rows <= 0 || N <= 0 || K <= 0 || iters <= 0 || !ms_per_launch) return TANDEM_EINVAL;
+  TcGemmTune t; t.cl = cluster; t.ring_kb = ring_kb; t.splits = splits;
+  return tc_gemm_time(rows, N, K, iters, t, swiglu ? kTcEpiSwiGLU : kTcEpiPartial, ms_per_launch);
 }
 
 }  // extern "C"

@@ -81,3 +81,20 @@ def test_tcgen05_gemm_bf16(rows, N, K):
     err = torch.max(torch.abs(out.double() - ref)).item()
     assert np.isfinite(err)
     assert err <= 2e-6 * max(1.0, ref.abs().max().item()) * (K ** 0.5), (err, ref.abs().max().item())
+
+
+@pytest.mark.parametrize("rows,I,K", [(1, 64, 64), (37, 192, 128), (140, 9728, 2560), (300, 512, 256), (64, 4864, 896)])
+def test_tcgen05_gemm_swiglu_epilogue(rows, I, K):
+    """Gate/up projection with SwiGLU fused into the tcgen05 epilogue (rows of W interleaved gate/up) against float64."""
+    g = torch.Generator().manual_seed(rows * 31 + I + K)
+    A = torch.randn(rows, K, generator=g).to(torch.bfloat16).cuda()
+    Wg = (torch.randn(I, K, generator=g) * 0.05).to(torch.bfloat16)
+    Wu = (torch.randn(I, K, generator=g) * 0.05).to(torch.bfloat16)
+    W = torch.stack([Wg, Wu], dim=1).reshape(2 * I, K).contiguous().cuda()
+    out = torch.zeros(rows, I, dtype=torch.bfloat16, device="cuda")
+    T.tandem_test_gemm(T.BF16, 3, A, W, out)
+    gate = A.double() @ Wg.cuda().double().T
+    up = A.double() @ Wu.cuda().double().T
+    ref = gate / (1 + torch.exp(-gate)) * up
+    err = torch.max(torch.abs(out.double() - ref)).item()
+    assert err <= 2 ** -8 * max(1e-3, ref.abs().max().item()) + 1e-6, (err, ref.abs().max().item())   # one bf16 rounding of the result
