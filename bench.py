@@ -44,16 +44,19 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=8)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg3_4b_bf16")
-    ap.add_argument("--fast-forward", type=int, default=0,
-                    help="tokens already generated per sequence before the timed window (ingested as context by prefill)")
+    ap.add_argument("--fast-forward", type=int, default=-1,
+                    help="tokens already generated per sequence before the timed window (ingested as context by prefill); "
+                         "-1 = half of the workload's max_new: step time is affine in the context length, so a step at the "
+                         "rollout's midpoint costs what the whole rollout costs on average")
     ap.add_argument("--ramp", type=int, default=48, help="untimed steps after prefill so that both models own KV")
+    ap.add_argument("--max-drain", type=int, default=256, help="upper bound on the extra untimed steps that drain the first catch-ups")
     ap.add_argument("--profile-steps", type=int, default=4)
-    ap.add_argument("--e2e-new", type=int, default=32, help="new tokens per sequence in the end-to-end tandem_generate leg")
+    ap.add_argument("--e2e-new", type=int, default=64, help="new tokens per sequence in the end-to-end tandem_generate leg")
     ap.add_argument("--profiler-range", action="store_true",
                     help="cudaProfilerStart/Stop around the timed region (for `ncu --profile-from-start off`)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
-    ap.add_argument("--cpu-new", type=int, default=4, help="new tokens of the oracle's bounded sample")
+    ap.add_argument("--cpu-new", type=int, default=8, help="new tokens of the oracle's bounded sample")
     return ap.parse_args()
 
 
@@ -179,12 +182,14 @@ def run_ours(args):
     wl = get_workload(args.workload)
     shape, B = wl.shape, wl.batch
     W, K = max(3, args.warmup), args.steps
+    if args.fast_forward < 0:
+        args.fast_forward = wl.max_new // 2
     prompts, table, seq_ids = build_inputs(wl, args.fast_forward, rank)
     max_prompt = max(len(p) for p in prompts)
     prefill_rows = sum(len(p) for p in prompts)
     row_cap = 4096
     prefill_steps = (prefill_rows + row_cap - 1) // row_cap + 2
-    gen_budget = prefill_steps + args.ramp + W + K + args.profile_steps + 64
+    gen_budget = prefill_steps + args.ramp + args.max_drain + W + K + args.profile_steps + 64
     max_seq_len = ((max_prompt + max(gen_budget, args.e2e_new) + 15) // 16) * 16
     eng = T.Tandem(T.TandemConfig(shape, max_seqs=B, max_seq_len=max_seq_len, device=local, max_rows_per_step=row_cap, use_graph=1))
     w_cpu = []
@@ -212,6 +217,18 @@ def run_ours(args):
         eng.step(prm, out=out, stream=stream); n_setup += 1
     for _ in range(args.ramp):
         eng.step(prm, out=out, stream=stream)
+    # keep stepping until the partner's first catch-up over the (fast-forwarded) context has drained: steady state is
+    # ~2 rows per sequence per step; the budget above reserves room for these steps
+    n_drain, prev = 0, eng.get_stats()
+    while n_drain < args.max_drain:
+        for _ in range(8):
+            eng.step(prm, out=out, stream=stream)
+        n_drain += 8
+        cur = eng.get_stats()
+        rows8 = cur["rows_senior"] + cur["rows_junior"] - prev["rows_senior"] - prev["rows_junior"]
+        prev = cur
+        if rows8 <= 8 * 3 * B:
+            break
     torch.cuda.synchronize()
     setup_s = time.perf_counter() - t0
 
@@ -275,8 +292,15 @@ def run_ours(args):
                              "alg_bytes_per_launch": b, "gbs": b / (kms / n * 1e-3) / 1e9 if kms > 0 else None}
         top = max(kernels, key=lambda k: kernels[k]["share"])
         kt = kernels[top]
+        traffic = None        # DRAM bytes per launch of that kernel from the committed `ncu --set full` capture of this workload
+        tpath = os.path.join(ROOT, "profiles", "traffic_r1.json")
+        if os.path.exists(tpath):
+            tj = json.load(open(tpath))
+            for kname, tv in tj.items():
+                if top == "attention" and "attention" in kname and tv.get("workload") == wl.name and tv.get("fast_forward") == args.fast_forward:
+                    traffic = tv["dram_bytes_per_launch"]
         roofline = {"kernel": top, "bound": "hbm", "achieved": kt["gbs"], "peak": pk["hbm_gbs"], "unit": "GB/s",
-                    "frac": kt["gbs"] / pk["hbm_gbs"], "traffic": None, "peak_source": pk["source"] + " burst copy (kernel timed alone)",
+                    "frac": kt["gbs"] / pk["hbm_gbs"], "traffic": traffic, "alg_bytes_per_launch": kt["alg_bytes_per_launch"], "peak_source": pk["source"] + " burst copy (kernel timed alone)",
                     "share_of_step": kt["share"], "rows_per_launch": rows, "profile_steps": args.profile_steps,
                     "profile_ms_per_step": total_ms / args.profile_steps}
 
@@ -286,7 +310,7 @@ def run_ours(args):
                       "ctx_mean_timed": ctx_mean, "p": wl.p, "word_start_frac": wl.word_start_frac, "temperature": wl.temperature,
                       "page_tokens": 16, "parallelism": "dp%d (independent sequences, replicated weights, no collective)" % world,
                       "l2": "inputs larger than L2 (16.1 GB of weights + KV streamed per step vs 126 MB L2)",
-                      "setup_steps": n_setup + args.ramp, "setup_seconds": setup_s, "cuda_graph": True},
+                      "setup_steps": n_setup + args.ramp + n_drain, "setup_seconds": setup_s, "cuda_graph": True},
            "clocks": clk, "gpu_launches": int(d["kernel_launches"]),
            "step_roofline": {"bound": "hbm", "alg_bytes_per_step": step_bytes, "weights_bytes_per_step": d["weight_bytes_read"] / K,
                              "kv_bytes_per_step": d["kv_bytes_read"] / K, "achieved": step_gbs, "unit": "GB/s",
@@ -297,10 +321,12 @@ def run_ours(args):
     # ---- end to end through tandem_generate with HOST buffers
     if not args.no_e2e:
         new = args.e2e_new
+        e_prompts = build_inputs(wl, 0, rank)[0]   # the workload's own prompts: a rollout from its start, max_new capped
+        e_rows = sum(len(p) for p in e_prompts)
         for it in range(2):                      # first call warms the graph for this parameter set
             if dist: dist.barrier()
             t0 = time.perf_counter()
-            g = eng.generate(prm, prompts, [new] * B, seq_ids=seq_ids, stream=stream)
+            g = eng.generate(prm, e_prompts, [new] * B, seq_ids=seq_ids, stream=stream)
             torch.cuda.synchronize()
             dt = time.perf_counter() - t0
         tok = float(g["len"].sum())
@@ -310,16 +336,16 @@ def run_ours(args):
             tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
             dt, tok = float(tmax[0]), float(tsum[1])
         steps_e = max(1, g["stats"]["steps"])
-        h2d = prefill_rows * 4 + (B + 1) * 8 + 3 * B * 4 + shape.vocab
+        h2d = e_rows * 4 + (B + 1) * 8 + 3 * B * 4 + shape.vocab
         d2h = B * new * (4 + 1 + 4) + B * 4
         res["e2e"] = {"value": tok / dt, "unit": "tokens/s", "h2d_bytes_per_step": h2d / steps_e, "d2h_bytes_per_step": d2h / steps_e,
-                      "call": "tandem_generate(B=%d host prompts, max_new=%d): prompt prefill + %d engine steps, host buffers in and out"
+                      "call": "tandem_generate(B=%d host prompts of the workload, max_new=%d): prompt prefill + %d engine steps, host buffers in and out"
                               % (B, new, steps_e), "seconds": dt, "device_seconds": g["stats"]["seconds_total"]}
     eng.free()
     torch.cuda.empty_cache()
 
     if rank == 0 and world == 1 and not args.no_cpu:
-        res["cpu_baseline"] = oracle_sample(wl, w_cpu, prompts, table, seq_ids, args.cpu_new, prm_seed=20260628)
+        res["cpu_baseline"] = oracle_sample(wl, w_cpu, build_inputs(wl, 0, rank)[0], table, seq_ids, args.cpu_new, prm_seed=20260628)
     if rank == 0:
         print(json.dumps(res))
     if dist:
@@ -359,7 +385,7 @@ def oracle_sample(wl, w_cpu, prompts, table, seq_ids, n_new, prm_seed):
     b = int(np.argmin([len(p) for p in prompts]))
     dt, n, _ = oracle_rollout(wl, w_cpu, prompts[b], table, seq_ids[b], n_new, prm_seed)
     return {"value": n / dt, "unit": "tokens/s", "cores": blas_threads(), "host_cpus": os.cpu_count(), "kind": "oracle",
-            "sample": "1 of the %d sequences (the shortest prompt, %d ids), prompt prefill + %d new tokens, oracle.tandem_generate "
+            "sample": "1 of the %d sequences at the start of its rollout (the shortest prompt, %d ids), prompt prefill + %d new tokens, oracle.tandem_generate "
                       "incremental-KV float64 NumPy on the same bf16-valued weights; %.1f s" % (len(prompts), len(prompts[b]), n, dt)}
 
 
