@@ -3,9 +3,10 @@
 //
 // Work unit = (attention item, kv head): the item's n_tok query tokens x G q-heads of the group form up to 64 rows
 // (row = tok * G + g) that share every K/V byte of the unit's KV range [kv0, kv1).
-//   producer warp : walks the CTA's units, looks pages up in the block table and streams them with TMA
-//                   (cp.async.bulk.tensor, 128-byte swizzle, L2 evict-first) into a ring of 64-token stages;
-//                   it runs ahead across unit boundaries, so HBM never waits for a softmax.
+//   producer warp : claims units (the first statically, the rest from an atomic counter, so no SM idles in the tail), looks
+//                   pages up in the block table and streams them with TMA (cp.async.bulk.tensor, 128-byte swizzle, L2
+//                   evict-first) into a ring of 64-token stages, each tagged with (unit, tile); it runs ahead across unit
+//                   boundaries, so HBM never waits for a softmax.
 //   4 consumer warps: S = Q K^T and O += P V on mma.sync.m16n8k16 (bf16 in, fp32 accumulate), online softmax in fp32
 //                   registers. Rows <= 16 (decode, short catch-up): the warps split the pages of a stage and are merged at
 //                   the end of the unit; more rows (long catch-up, prompt prefill): one 16-row m-tile per warp.
@@ -32,6 +33,7 @@ struct AttnMmaArgs {
   float2* part_ml;           // [parts, nq] (max of the scaled scores, sum)
   int nq, nkv; float scale;
   int row_base_k, row_base_v;  // tensor-map row of (page 0, kv head 0, token 0) of this layer's K / V pool
+  int32_t* work_ctr;           // zeroed by the scheduler every step: units beyond the first gridDim.x are claimed dynamically
 };
 
 namespace ptx {
@@ -68,6 +70,7 @@ __global__ void __launch_bounds__(kAmThreads, 2) paged_attention_mma_kernel(cons
   extern __shared__ uint8_t am_smem_raw[];
   __shared__ __align__(8) uint64_t bars[2 * STAGES];
   __shared__ float2 s_ml[4][16];
+  __shared__ int2 s_meta[STAGES];                   // (unit, tile index) of the data in each stage; unit < 0: no more work
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int n_units = a.counts[C_ITEMS] * a.nkv;
@@ -88,31 +91,46 @@ __global__ void __launch_bounds__(kAmThreads, 2) paged_attention_mma_kernel(cons
     // ================================================================== producer
     const uint64_t pol = ptx::policy_evict_first();
     int it = 0;
-    for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
-      const int item = u / a.nkv, kvh = u - item * a.nkv;
-      const int slot = a.row_slot[a.item_row0[item]];
-      const int kv0 = a.item_kv0[item], kv1 = a.item_kv1[item];
-      const int n_tiles = (kv1 - kv0 + kAmTileTok - 1) / kAmTileTok;
-      const int32_t* btp = a.bt + (size_t)slot * a.max_pages + kv0 / kPageTokens;
-      for (int ti = 0; ti < n_tiles; ++ti, ++it) {
-        const int npg = min(4, (kv1 - kv0 - ti * kAmTileTok + kPageTokens - 1) / kPageTokens);
-        const int pg = lane < npg ? btp[ti * 4 + lane] : 0;
-        const int s = it % STAGES;
-        if (lane == 0) {
-          ptx::mbar_wait(empty_bar(s), (((uint32_t)(it / STAGES)) & 1u) ^ 1u);
-          ptx::mbar_expect_tx(full_bar(s), (uint32_t)(npg * 2 * PAGE_BYTES));
-        }
-        __syncwarp();
-        if (lane < npg) {
-          const int rk = a.row_base_k + (pg * a.nkv + kvh) * kPageTokens;
-          const int rv = a.row_base_v + (pg * a.nkv + kvh) * kPageTokens;
-          const uint32_t dk = ring + (uint32_t)(s * STAGE_BYTES + lane * PAGE_BYTES);
+    int u = blockIdx.x;
+    while (true) {
+      if (u < n_units) {
+        const int item = u / a.nkv, kvh = u - item * a.nkv;
+        const int slot = a.row_slot[a.item_row0[item]];
+        const int kv0 = a.item_kv0[item], kv1 = a.item_kv1[item];
+        const int n_tiles = (kv1 - kv0 + kAmTileTok - 1) / kAmTileTok;
+        const int32_t* btp = a.bt + (size_t)slot * a.max_pages + kv0 / kPageTokens;
+        for (int ti = 0; ti < n_tiles; ++ti, ++it) {
+          const int npg = min(4, (kv1 - kv0 - ti * kAmTileTok + kPageTokens - 1) / kPageTokens);
+          const int pg = lane < npg ? btp[ti * 4 + lane] : 0;
+          const int s = it % STAGES;
+          if (lane == 0) {
+            ptx::mbar_wait(empty_bar(s), (((uint32_t)(it / STAGES)) & 1u) ^ 1u);
+            s_meta[s] = make_int2(u, ti);
+            ptx::mbar_expect_tx(full_bar(s), (uint32_t)(npg * 2 * PAGE_BYTES));
+          }
+          __syncwarp();
+          if (lane < npg) {
+            const int rk = a.row_base_k + (pg * a.nkv + kvh) * kPageTokens;
+            const int rv = a.row_base_v + (pg * a.nkv + kvh) * kPageTokens;
+            const uint32_t dk = ring + (uint32_t)(s * STAGE_BYTES + lane * PAGE_BYTES);
 #pragma unroll
-          for (int hh = 0; hh < HALVES; ++hh) {
-            ptx::tma_load_2d(dk + hh * 2048, &tmap_kv, hh * 64, rk, full_bar(s), pol);
-            ptx::tma_load_2d(dk + KV_BYTES + hh * 2048, &tmap_kv, hh * 64, rv, full_bar(s), pol);
+            for (int hh = 0; hh < HALVES; ++hh) {
+              ptx::tma_load_2d(dk + hh * 2048, &tmap_kv, hh * 64, rk, full_bar(s), pol);
+              ptx::tma_load_2d(dk + KV_BYTES + hh * 2048, &tmap_kv, hh * 64, rv, full_bar(s), pol);
+            }
           }
         }
+        int nu = 0;
+        if (lane == 0) nu = atomicAdd(a.work_ctr, 1) + (int)gridDim.x;
+        u = __shfl_sync(0xffffffffu, nu, 0);
+      } else {
+        if (lane == 0) {   // sentinel stage: tells the consumers to stop
+          const int s = it % STAGES;
+          ptx::mbar_wait(empty_bar(s), (((uint32_t)(it / STAGES)) & 1u) ^ 1u);
+          s_meta[s] = make_int2(-1, 0);
+          ptx::mbar_arrive(full_bar(s));
+        }
+        break;
       }
     }
     return;
@@ -128,7 +146,10 @@ __global__ void __launch_bounds__(kAmThreads, 2) paged_attention_mma_kernel(cons
   const int v_t = (lane & 7) + ((kmat & 1) << 3);           // V (transposed): matrices (tok 0-7 | 8-15) x (chunk j | j+1)
   const int v_c = kmat >> 1;
   int it = 0;
-  for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
+  while (true) {
+    ptx::mbar_wait(full_bar(it % STAGES), ((uint32_t)(it / STAGES)) & 1u);    // first stage of the next unit (or the sentinel)
+    const int u = s_meta[it % STAGES].x;
+    if (u < 0) break;
     const int item = u / a.nkv, kvh = u - item * a.nkv;
     const int row0 = a.item_row0[item], n_tok = a.item_ntok[item], part = a.item_part[item];
     const int kv0 = a.item_kv0[item], kv1 = a.item_kv1[item];
@@ -169,7 +190,7 @@ __global__ void __launch_bounds__(kAmThreads, 2) paged_attention_mma_kernel(cons
       const int s = it % STAGES;
       const int tile0 = kv0 + ti * kAmTileTok;
       const int npg = min(4, (kv1 - tile0 + kPageTokens - 1) / kPageTokens);
-      ptx::mbar_wait(full_bar(s), ((uint32_t)(it / STAGES)) & 1u);
+      if (ti > 0) ptx::mbar_wait(full_bar(s), ((uint32_t)(it / STAGES)) & 1u);
       if (active) {
         for (int p = kl; p < npg; p += kvg) {
           const int t0 = tile0 + p * kPageTokens;

@@ -14,6 +14,7 @@ namespace tandem {
 struct SchedArgs {
   SeqState st; PageTab pt[2]; StepTab tab[2]; StepIO io; DevStats* stats;
   const int32_t* tokens; int max_seqs, max_seq_len, max_pages, row_cap, tile_tok;
+  int32_t* work_ctr; int n_work_ctr;   // dynamic-scheduling counters of the attention launches of this step
 };
 
 __device__ __forceinline__ int block_excl_scan_1024(int v, int* total, int* wsum) {
@@ -49,6 +50,7 @@ __global__ void __launch_bounds__(1024) sched_kernel(SchedArgs a) {
   __shared__ int wsum[32];
   const int s = threadIdx.x;
   const bool in_range = s < a.max_seqs;
+  for (int i = threadIdx.x; i < a.n_work_ctr; i += blockDim.x) a.work_ctr[i] = 0;
 
   if (in_range) {  // defaults of the per-step outputs
     if (a.io.token) a.io.token[s] = -1;

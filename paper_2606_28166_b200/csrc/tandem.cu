@@ -72,7 +72,7 @@ struct tandem_handle {
   int32_t* tokens = nullptr; uint8_t* out_owner = nullptr; float* out_logp = nullptr;
   float2* rope_cs = nullptr;
   uint8_t* word_start_dev = nullptr; std::vector<uint8_t> word_start_host;
-  DevStats* stats = nullptr; int32_t* n_active = nullptr;
+  DevStats* stats = nullptr; int32_t* n_active = nullptr; int32_t* work_ctr = nullptr;
   cudaStream_t ms[2]{}; cudaStream_t gs{}; cudaEvent_t ev_fork{}, ev_join[2]{}, ev_in{}, ev_out{};
   std::vector<uint8_t> slot_busy;           // host view of the slots
   // admission staging
@@ -233,7 +233,7 @@ int model_forward(tandem_handle* h, int m, const StepIO& io, const RuleParams& r
       const long long rows_per_half = (long long)h->pool_pages * nkv * kPageTokens;
       AttnMmaArgs ma{tb.counts, tb.item_row0, tb.item_ntok, tb.item_kv0, tb.item_kv1, tb.item_part, tb.row_slot, tb.row_pos, h->pt[m].bt, h->max_pages,
                      (const bf16*)ws.q, (bf16*)ws.attn_out, ws.part_acc, ws.part_ml, nq, nkv, 1.0f / sqrtf((float)d),
-                     (int)((2ll * l) * rows_per_half), (int)((2ll * l + 1) * rows_per_half)};
+                     (int)((2ll * l) * rows_per_half), (int)((2ll * l + 1) * rows_per_half), h->work_ctr + m * c.n_layers + l};
       KL(h, TANDEM_KC_ATTENTION, s, ok = run_attn_mma(*h->kv_map[m], ma, d, nq / nkv, 2 * h->n_sms, s, false));
     } else {
       AttnArgs<T> aa{tb.counts, tb.item_row0, tb.item_ntok, tb.item_kv0, tb.item_kv1, tb.item_part, tb.row_slot, tb.row_pos, h->pt[m].bt, h->max_pages, (const float*)ws.q, kpool, vpool,
@@ -271,6 +271,7 @@ int launch_step(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaSt
   sa.st = h->st; sa.pt[0] = h->pt[0]; sa.pt[1] = h->pt[1]; sa.tab[0] = h->tab[0]; sa.tab[1] = h->tab[1];
   sa.io = io; sa.stats = h->stats; sa.tokens = h->tokens; sa.max_seqs = c.max_seqs; sa.max_seq_len = c.max_seq_len;
   sa.max_pages = h->max_pages; sa.row_cap = h->row_cap; sa.tile_tok = h->tile_tok;
+  sa.work_ctr = h->work_ctr; sa.n_work_ctr = 2 * c.n_layers;
   KL(h, TANDEM_KC_SCHED, s, (sched_kernel<<<1, 1024, 0, s>>>(sa)));
   if (h->profile) {   // one stream, one kernel at a time: each kernel's duration is its own
     for (int m = 0; m < 2; ++m) {
@@ -524,6 +525,7 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
   INIT_TRY(dmalloc(h, &h->word_start_dev, (size_t)V));
   INIT_TRY(dmalloc(h, &h->stats, sizeof(DevStats)));
   INIT_CU(cudaMemset(h->stats, 0, sizeof(DevStats)));
+  INIT_TRY(dmalloc(h, &h->work_ctr, (size_t)2 * c.n_layers * 4));
   INIT_TRY(dmalloc(h, &h->n_active, 4));
   INIT_CU(cudaMemset(h->n_active, 0, 4));
   INIT_TRY(dmalloc(h, &h->stage_off, (size_t)(S + 1) * sizeof(long long)));
@@ -827,7 +829,7 @@ void tandem_free(tandem_handle* h) {
   if (h->ev_out) cudaEventDestroy(h->ev_out);
   if (h->gs) cudaStreamDestroy(h->gs);
   fr(h->st_mem); fr(h->st_mem8); fr(h->tokens); fr(h->out_owner); fr(h->out_logp); fr(h->rope_cs); fr(h->word_start_dev); fr(h->stats);
-  fr(h->n_active); fr(h->stage_tokens); fr(h->stage_off); fr(h->stage_i32);
+  fr(h->n_active); fr(h->work_ctr); fr(h->stage_tokens); fr(h->stage_off); fr(h->stage_i32);
   cudaGetLastError();
   delete h;
 }
