@@ -96,27 +96,44 @@ __global__ void __launch_bounds__(1024) sched_kernel(SchedArgs a) {
     }
     int n_emit;
     const int j = block_excl_scan_1024(emits ? 1 : 0, &n_emit, wsum);
-    // attention items (S5): the rows of a sequence are cut into q-tiles of tile_tok tokens; a sequence with a single
-    // q-tile (plain decode and short catch-ups) is also split along KV into n_split chunks whose partial (m, l, acc)
-    // are combined afterwards; longer runs (prompt prefill) get their parallelism from the q-tiles.
+    // attention items (S5): the rows of a sequence are cut into q-tiles of tile_tok tokens; q-tile t attends to the KV
+    // range [0, ing + t0 + nt). For a sequence with at most kAttnSplitTiles q-tiles (decode, catch-ups) every q-tile is
+    // also split along KV into chunks of attn_chunk(kv_len) positions whose partial (m, l, acc) are combined afterwards;
+    // longer runs (prompt prefill) get their parallelism from the q-tiles and write their output directly.
     const int kv_len = ing + rows;
     const int n_qt = (rows + a.tile_tok - 1) / a.tile_tok;
     const int chunk = attn_chunk(kv_len);
-    const int nsplit = (n_qt == 1) ? (kv_len + chunk - 1) / chunk : 1;
-    const int items = (rows == 0) ? 0 : (n_qt == 1 ? nsplit : n_qt);
-    const int parts = (n_qt == 1 && nsplit > 1) ? nsplit * rows : 0;
+    const bool use_parts = rows > 0 && n_qt <= kAttnSplitTiles && kv_len > chunk;
+    int items = rows > 0 ? n_qt : 0, parts = 0;
+    if (use_parts) {
+      items = 0;
+      for (int t = 0; t < n_qt; ++t) {
+        const int t0 = t * a.tile_tok, nt = min(a.tile_tok, rows - t0);
+        const int ns = (ing + t0 + nt + chunk - 1) / chunk;
+        items += ns; parts += ns * nt;
+      }
+    }
     int n_items, n_parts, n_comb, n_sched;
     const int icu = block_excl_scan_1024(items, &n_items, wsum);
     const int pcu = block_excl_scan_1024(parts, &n_parts, wsum);
-    const int ccu = block_excl_scan_1024(parts > 0 ? rows : 0, &n_comb, wsum);
+    const int ccu = block_excl_scan_1024(use_parts ? rows : 0, &n_comb, wsum);
     block_excl_scan_1024(rows > 0 ? 1 : 0, &n_sched, wsum);
 
     cu_rows[s] = cu; cu_items[s] = icu;
-    sm_rows[s] = rows; sm_ing[s] = ing; sm_part0[s] = parts > 0 ? pcu : -1; sm_emit[s] = emits ? j : -1;
+    sm_rows[s] = rows; sm_ing[s] = ing; sm_part0[s] = use_parts ? pcu : -1; sm_emit[s] = emits ? j : -1;
     if (s == 0) { cu_rows[kMaxSlots] = n_rows; cu_items[kMaxSlots] = n_items; }
     if (emits) tb.emit_slot[j] = s;
-    for (int t = 0; t < (parts > 0 ? rows : 0); ++t) {
-      tb.comb_row[ccu + t] = cu + t; tb.comb_part0[ccu + t] = pcu + t; tb.comb_n[ccu + t] = nsplit; tb.comb_stride[ccu + t] = rows;
+    if (use_parts) {
+      int poff = 0;
+      for (int t = 0; t < n_qt; ++t) {
+        const int t0 = t * a.tile_tok, nt = min(a.tile_tok, rows - t0);
+        const int ns = (ing + t0 + nt + chunk - 1) / chunk;
+        for (int k = 0; k < nt; ++k) {
+          tb.comb_row[ccu + t0 + k] = cu + t0 + k; tb.comb_part0[ccu + t0 + k] = pcu + poff + k;
+          tb.comb_n[ccu + t0 + k] = ns; tb.comb_stride[ccu + t0 + k] = nt;
+        }
+        poff += ns * nt;
+      }
     }
     if (rows > 0) a.st.ing[M][s] = ing + rows;  // commit: the forward below always runs
     __syncthreads();
@@ -135,12 +152,19 @@ __global__ void __launch_bounds__(1024) sched_kernel(SchedArgs a) {
       const int q = find_owner_slot(cu_items, kMaxSlots, i);
       const int off = i - cu_items[q];
       const int qrows = sm_rows[q], qkv = sm_ing[q] + qrows;
-      if (qrows <= a.tile_tok) {          // one q-tile, split `off` of the KV range
+      if (sm_part0[q] >= 0) {             // split sequence: walk its q-tiles to find (q-tile, split) number `off`
         const int ch = attn_chunk(qkv);
-        tb.item_row0[i] = cu_rows[q]; tb.item_ntok[i] = qrows;
-        tb.item_kv0[i] = off * ch; tb.item_kv1[i] = min(qkv, (off + 1) * ch);
-        tb.item_part[i] = sm_part0[q] >= 0 ? sm_part0[q] + off * qrows : -1;
-      } else {                            // q-tile `off`, whole causal range
+        int rem = off, poff = 0, t0 = 0, nt = 0, ns = 0;
+        for (;; t0 += a.tile_tok) {
+          nt = min(a.tile_tok, qrows - t0);
+          ns = (sm_ing[q] + t0 + nt + ch - 1) / ch;
+          if (rem < ns) break;
+          rem -= ns; poff += ns * nt;
+        }
+        tb.item_row0[i] = cu_rows[q] + t0; tb.item_ntok[i] = nt;
+        tb.item_kv0[i] = rem * ch; tb.item_kv1[i] = min(sm_ing[q] + t0 + nt, (rem + 1) * ch);
+        tb.item_part[i] = sm_part0[q] + poff + rem * nt;
+      } else {                            // q-tile `off`, whole causal range, written directly
         const int t0 = off * a.tile_tok, nt = min(a.tile_tok, qrows - t0);
         tb.item_row0[i] = cu_rows[q] + t0; tb.item_ntok[i] = nt;
         tb.item_kv0[i] = 0; tb.item_kv1[i] = sm_ing[q] + t0 + nt;

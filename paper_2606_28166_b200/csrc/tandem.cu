@@ -494,8 +494,8 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
   h->row_cap = std::max(h->row_cap, c.max_seqs);   // every owned sequence must be able to decode in one step
   h->max_pages = (c.max_seq_len + kPageTokens - 1) / kPageTokens;
   h->tile_tok = std::max(1, kAttnTileRows / (c.n_q_heads / c.n_kv_heads));
-  h->max_items = c.max_seqs * kAttnMaxSplits + h->row_cap;          // split single-tile sequences + q-tiles of longer runs
-  h->max_comb = std::min(c.max_seqs * h->tile_tok, h->row_cap);     // rows whose splits are combined
+  h->max_items = c.max_seqs * kAttnSplitTiles * kAttnMaxSplits + h->row_cap;   // (q-tile, split) of short runs + q-tiles of longer ones
+  h->max_comb = std::min(c.max_seqs * kAttnSplitTiles * h->tile_tok, h->row_cap);   // rows whose splits are combined
   h->part_cap = h->max_comb * kAttnMaxSplits;                       // (row, split) partials
   const int H = c.hidden, nq = c.n_q_heads, nkv = c.n_kv_heads, d = c.head_dim, I = c.intermediate, V = c.vocab, R = h->row_cap, S = c.max_seqs;
   const size_t page_bytes = (size_t)2 * c.n_layers * nkv * kPageTokens * d * h->esize;
