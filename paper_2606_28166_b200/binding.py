@@ -267,9 +267,9 @@ def tandem_test_gemm(dtype, impl, A, W, out):
         raise TandemError(rc)
 
 
-def tandem_test_gemm_time(rows, N, K, iters=50, cluster=0, ring_kb=0, splits=0, swiglu=0):
+def tandem_test_gemm_time(rows, N, K, iters=50, cluster=0, ring_kb=0, splits=0, swiglu=0, pdl=0):
     ms = C.c_float()
-    rc = lib().tandem_test_gemm_time(rows, N, K, iters, cluster, ring_kb, splits, swiglu, C.byref(ms))
+    rc = lib().tandem_test_gemm_time(rows, N, K, iters, cluster, ring_kb, splits, (1 if swiglu else 0) | (2 if pdl else 0), C.byref(ms))
     if rc:
         raise TandemError(rc)
     return ms.value

@@ -42,6 +42,7 @@ constexpr int kAttnTile = 64;   // KV positions per softmax tile
 
 template <typename T, int D, int G>
 __global__ void __launch_bounds__(kAttnThreads) paged_attention_kernel(AttnArgs<T> a) {
+  pdl_trigger(); pdl_wait();
   constexpr int VEC = 16 / (int)sizeof(T);
   constexpr int LPP = D / VEC;                   // lanes cooperating on one KV position
   constexpr int PPW = 32 / LPP;                  // positions per warp per iteration
@@ -209,6 +210,7 @@ template <typename T> struct CombineArgs {
 // One warp per (row, head); lane = 4 consecutive dims; all partial loads of a row are independent (n <= kAttnMaxSplits).
 template <typename T>
 __global__ void __launch_bounds__(256) attn_combine_kernel(CombineArgs<T> a) {
+  pdl_trigger(); pdl_wait();
   const int n_units = a.counts[C_COMB] * a.nq;
   const int lane = threadIdx.x & 31;
   for (int unit = blockIdx.x * (blockDim.x / 32) + (threadIdx.x >> 5); unit < n_units; unit += gridDim.x * (blockDim.x / 32)) {

@@ -72,9 +72,10 @@ __global__ void __launch_bounds__(kAmThreads, 2) paged_attention_mma_kernel(cons
   __shared__ float2 s_ml[4][16];
   __shared__ int2 s_meta[STAGES];                   // (unit, tile index) of the data in each stage; unit < 0: no more work
 
+  pdl_trigger();
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int n_units = a.counts[C_ITEMS] * a.nkv;
-  if ((int)blockIdx.x >= n_units) return;
+  const int n_units = a.counts[C_ITEMS] * a.nkv;   // written by the scheduler, complete long before this kernel can start
+  if ((int)blockIdx.x >= n_units) { pdl_wait(); return; }
   const uint32_t ring = (ptx::smem_u32(am_smem_raw) + 1023u) & ~1023u;
   float* scratch = reinterpret_cast<float*>(am_smem_raw + (ring - ptx::smem_u32(am_smem_raw)) + STAGES * STAGE_BYTES);   // [4][16][OSTRIDE]
   const uint32_t bar0 = ptx::smem_u32(bars);
@@ -86,6 +87,7 @@ __global__ void __launch_bounds__(kAmThreads, 2) paged_attention_mma_kernel(cons
     ptx::prefetch_tmap(&tmap_kv);
   }
   __syncthreads();
+  pdl_wait();                                       // q and this step's K/V come from the predecessor (rope_append)
 
   if (warp == 4) {
     // ================================================================== producer

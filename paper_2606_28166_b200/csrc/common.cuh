@@ -134,6 +134,24 @@ __device__ __forceinline__ float u_switch_counter(unsigned long long seed, int s
 __device__ __forceinline__ float gumbel_from_uniform(float u) { return -logf(-log1pf(-u)); }
 
 // ------------------------------------------------------------------------------------------------------------
+// Programmatic dependent launch (PDL): a kernel launched with the attribute may start while its predecessor in the stream
+// is still running; pdl_wait() blocks until the predecessor has completed and its writes are visible, pdl_trigger() lets
+// the successor start launching. Both are no-ops in a kernel launched without the attribute. Rule used throughout: before
+// pdl_wait() a kernel touches only constants (weights, tensor maps, the step tables written by the scheduler, which is
+// never the direct predecessor) and its own shared memory / TMEM; every global write comes after it.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <typename... P, typename... A>
+inline cudaError_t launch_ex(void (*kernel)(P...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, bool pdl, A&&... args) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kernel, P(args)...);
+}
+
 __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);

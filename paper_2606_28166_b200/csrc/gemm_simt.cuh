@@ -13,6 +13,7 @@ constexpr int kSimtTile = 32;
 template <typename T>
 __global__ void __launch_bounds__(256) gemm_simt_kernel(const int32_t* __restrict__ n_rows_ptr, int n_rows_fixed, const T* __restrict__ A,
                                                         const T* __restrict__ W, float* __restrict__ out, int N, int K) {
+  pdl_trigger(); pdl_wait();
   __shared__ float As[kSimtTile][kSimtTile + 1];
   __shared__ float Ws[kSimtTile][kSimtTile + 1];
   const int n_rows = n_rows_ptr ? *n_rows_ptr : n_rows_fixed;

@@ -156,8 +156,9 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_con
   __shared__ __align__(8) uint64_t bars[2 * kTcMaxStages + 2];
   __shared__ uint32_t tmem_base_smem;
 
-  const int rows = g.rows_ptr ? *g.rows_ptr : g.rows_fixed;
-  if (rows <= 0) return;                                   // uniform over the grid: nothing was scheduled for this model
+  pdl_trigger();
+  const int rows = g.rows_ptr ? *g.rows_ptr : g.rows_fixed;   // scheduler output: complete before any kernel of the chain starts
+  if (rows <= 0) { pdl_wait(); return; }                   // uniform over the grid: nothing was scheduled for this model
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int n0 = blockIdx.x * kTcTileN;
   const int split = blockIdx.y;
@@ -196,11 +197,28 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_con
     // ===== TMA producer: weights stream once (evict-first), activations are shared by every CTA (evict-last)
     if (lane == 0) {
       const uint64_t pol_w = ptx::policy_evict_first(), pol_a = ptx::policy_evict_last();
+      // Weights do not depend on the predecessor kernel: fill the ring with the first weight tiles right away, wait for
+      // the predecessor (PDL), then add the activation boxes of those stages and carry on normally.
+      const int npre = min(n_stages, kb1 - kb0);
+      const int nbox0 = (min(rows, kTcMaxRows) + kTcRowBox - 1) / kTcRowBox;
+      for (int i = 0; i < npre; ++i) {
+        ptx::mbar_expect_tx(full_bar(i), (uint32_t)(kTcWBytes + nbox0 * kTcABoxBytes));
+        ptx::tma_load_2d(ring + (uint32_t)(i * stage_bytes), &tmap_w, (kb0 + i) * kTcBlockK, n0, full_bar(i), pol_w);
+      }
+      pdl_wait();
+      for (int i = 0; i < npre; ++i) {
+        const uint32_t dst = ring + (uint32_t)(i * stage_bytes);
+        for (int j = (int)cta_rank; j < nbox0; j += CL) {
+          if (CL > 1) ptx::tma_load_2d_mc(dst + kTcWBytes + j * kTcABoxBytes, &tmap_a, (kb0 + i) * kTcBlockK, j * kTcRowBox, full_bar(i), kMask, pol_a);
+          else ptx::tma_load_2d(dst + kTcWBytes + j * kTcABoxBytes, &tmap_a, (kb0 + i) * kTcBlockK, j * kTcRowBox, full_bar(i), pol_a);
+        }
+      }
       int it = 0;
       for (int c = 0; c < n_chunks; ++c) {
         const int r0 = c * kTcMaxRows;
         const int nbox = (min(rows - r0, kTcMaxRows) + kTcRowBox - 1) / kTcRowBox;
         for (int kb = kb0; kb < kb1; ++kb, ++it) {
+          if (it < npre) continue;
           const int s = it % n_stages;
           const uint32_t ph = (uint32_t)(it / n_stages) & 1u;
           ptx::mbar_wait(empty_bar(s), ph ^ 1u);
@@ -244,6 +262,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_con
     const int q = warp & 3;
     const int n = n0 + q * 32 + lane;
     float* outp = g.out + (size_t)split * g.split_stride;
+    pdl_wait();                                            // the predecessor may still be reading the buffer this kernel writes
     for (int c = 0; c < n_chunks; ++c) {
       const int r0 = c * kTcMaxRows;
       const int crow = min(rows - r0, kTcMaxRows);
@@ -352,15 +371,16 @@ inline const CUtensorMap* tc_gemm_map(TcGemmPlans* p, const void* base, int n_ro
 // activations [rows, N/2] (epi = kTcEpiSwiGLU; W rows interleaved gate/up). Returns 0, or -1 (TANDEM_EINVAL) / -3 (TANDEM_ECUDA).
 // which == 4 (LM head) never splits: the sampler reads the logits in place.
 template <int CL, int EPI>
-inline int tc_gemm_launch_cl(const CUtensorMap* mw, const CUtensorMap* ma, const TcGemmArgs& g, dim3 grid, cudaStream_t s) {
+inline int tc_gemm_launch_cl(const CUtensorMap* mw, const CUtensorMap* ma, const TcGemmArgs& g, dim3 grid, cudaStream_t s, bool pdl) {
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = grid; cfg.blockDim = dim3(kTcThreads); cfg.dynamicSmemBytes = (size_t)g.ring_bytes + 1024; cfg.stream = s;
-  cudaLaunchAttribute at[1];
+  cudaLaunchAttribute at[2];
   at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-  cfg.attrs = at; cfg.numAttrs = 1;
+  at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[1].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = pdl ? 2 : 1;
   return cudaLaunchKernelEx(&cfg, gemm_tcgen05_kernel<CL, EPI>, *mw, *ma, g) == cudaSuccess ? 0 : -3;
 }
-struct TcGemmTune { int cl = 0, ring_kb = 0, splits = 0; };   // 0 = automatic; overrides for tandem_test_gemm_time only
+struct TcGemmTune { int cl = 0, ring_kb = 0, splits = 0; bool pdl = false; };   // 0 = automatic; overrides for tandem_test_gemm_time only
 inline int tc_gemm_launch(TcGemmPlans* p, int /*model*/, int which, int /*layer*/, const void* A, const void* W, int N, int K, float* out,
                           const int32_t* rows_ptr, int rows_cap, int* n_split, size_t* split_stride, cudaStream_t s, int epi = kTcEpiPartial,
                           const TcGemmTune* tune = nullptr) {
@@ -383,14 +403,15 @@ inline int tc_gemm_launch(TcGemmPlans* p, int /*model*/, int which, int /*layer*
   g.ring_bytes = tiles_pad * S > 148 ? 98 * 1024 : kTcRingBytes;     // more CTAs than SMs: let two share an SM
   if (tune && tune->ring_kb > 0) g.ring_bytes = tune->ring_kb * 1024;
   dim3 grid(tiles_pad, S);
+  const bool pdl = tune && tune->pdl;
   if (epi == kTcEpiSwiGLU) {
-    if (cl == 4) return tc_gemm_launch_cl<4, 1>(mw, ma, g, grid, s);
-    if (cl == 2) return tc_gemm_launch_cl<2, 1>(mw, ma, g, grid, s);
-    return tc_gemm_launch_cl<1, 1>(mw, ma, g, grid, s);
+    if (cl == 4) return tc_gemm_launch_cl<4, 1>(mw, ma, g, grid, s, pdl);
+    if (cl == 2) return tc_gemm_launch_cl<2, 1>(mw, ma, g, grid, s, pdl);
+    return tc_gemm_launch_cl<1, 1>(mw, ma, g, grid, s, pdl);
   }
-  if (cl == 4) return tc_gemm_launch_cl<4, 0>(mw, ma, g, grid, s);
-  if (cl == 2) return tc_gemm_launch_cl<2, 0>(mw, ma, g, grid, s);
-  return tc_gemm_launch_cl<1, 0>(mw, ma, g, grid, s);
+  if (cl == 4) return tc_gemm_launch_cl<4, 0>(mw, ma, g, grid, s, pdl);
+  if (cl == 2) return tc_gemm_launch_cl<2, 0>(mw, ma, g, grid, s, pdl);
+  return tc_gemm_launch_cl<1, 0>(mw, ma, g, grid, s, pdl);
 }
 
 // Unit-test hook: out[rows, N] = A W^T (partials summed here), synchronous.

@@ -261,6 +261,7 @@ template <typename T, int NT>
 __global__ void __launch_bounds__(NT) embed_norm_kernel(const int32_t* __restrict__ counts, const int32_t* __restrict__ row_tok,
                                                         const T* __restrict__ E, const T* __restrict__ gain, float* __restrict__ x,
                                                         T* __restrict__ act, int H, float eps) {
+  pdl_trigger(); pdl_wait();
   __shared__ float red[32];
   const int n_rows = counts[C_ROWS];
   for (int r = blockIdx.x; r < n_rows; r += gridDim.x) {
@@ -281,6 +282,7 @@ template <typename T, int NT, int VPT>
 __global__ void __launch_bounds__(NT) residual_norm_kernel(const int32_t* __restrict__ counts, const float* __restrict__ part, int n_split,
                                                            size_t split_stride, float* __restrict__ x, const T* __restrict__ gain,
                                                            T* __restrict__ act, const int32_t* __restrict__ out_map, int H, float eps) {
+  pdl_trigger(); pdl_wait();
   __shared__ float red[32];
   const int n_rows = counts[C_ROWS];
   const int H4 = H >> 2;
@@ -329,6 +331,7 @@ __global__ void __launch_bounds__(NT) rope_append_kernel(const int32_t* __restri
                                                          const int32_t* __restrict__ row_kvslot, const float* __restrict__ part, int n_split,
                                                          size_t split_stride, const float2* __restrict__ cs_table, QT* __restrict__ q_out,
                                                          T* __restrict__ kpool, T* __restrict__ vpool, int nq, int nkv, int d) {
+  pdl_trigger(); pdl_wait();
   const int n_rows = counts[C_ROWS];
   const int half = d >> 1, hq = half >> 2;                 // hq: groups of 4 pairs per head
   const int ld = (nq + 2 * nkv) * d;
@@ -375,6 +378,7 @@ __global__ void __launch_bounds__(NT) rope_append_kernel(const int32_t* __restri
 template <typename T, int NT>
 __global__ void __launch_bounds__(NT) swiglu_kernel(const int32_t* __restrict__ counts, const float* __restrict__ part, int n_split,
                                                     size_t split_stride, T* __restrict__ out, int I) {
+  pdl_trigger(); pdl_wait();
   const int n_rows = counts[C_ROWS];
   const int I4 = I >> 2;
   const size_t total = (size_t)n_rows * I4;
@@ -407,6 +411,7 @@ __device__ __forceinline__ ArgBest better(ArgBest a, ArgBest b) {  // larger val
 
 template <int NT>
 __global__ void __launch_bounds__(NT) sample_switch_emit_kernel(SampleArgs a) {
+  pdl_trigger(); pdl_wait();
   __shared__ float s_m[NT / 32], s_s[NT / 32], s_bv[NT / 32], s_gv[NT / 32];
   __shared__ int s_bi[NT / 32], s_gi[NT / 32];
   const int j = blockIdx.x;

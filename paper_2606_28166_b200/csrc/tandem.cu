@@ -9,6 +9,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -62,6 +63,8 @@ struct tandem_handle {
   int esize = 4;
   int row_cap = 0, max_pages = 0, pool_pages = 0, tile_tok = 0, max_items = 0, max_comb = 0, part_cap = 0, gemm_impl = TANDEM_GEMM_SIMT, attn_impl = TANDEM_ATTN_ALU;
   int n_sms = 148;
+  int attn_ctas_per_sm = 2, gemm_ring_kb = 0;   // tuning knobs (env TANDEM_ATTN_CTAS_PER_SM, TANDEM_GEMM_RING_KB; 0 = automatic)
+  bool use_pdl = true;                          // programmatic dependent launch along each model's kernel chain (env TANDEM_PDL=0 disables)
   size_t gemm_out_cols = 0;
   ModelWeights w[2];
   Workspace ws[2];
@@ -143,11 +146,12 @@ int launch_gemm(tandem_handle* h, int m, int which, int layer, const void* A, co
   static const int cls_of[5] = {TANDEM_KC_GEMM_QKV, TANDEM_KC_GEMM_O, TANDEM_KC_GEMM_GATEUP, TANDEM_KC_GEMM_DOWN, TANDEM_KC_GEMM_LMHEAD};
   if (h->gemm_impl == TANDEM_GEMM_TCGEN05 && sizeof(T) == 2) {
     int rc = 0;
-    KL(h, cls_of[which], s, rc = tc_gemm_launch(h->tc, m, which, layer, A, W, N, K, out, rows_ptr, rows_cap, n_split, split_stride, s, epi));
+    TcGemmTune tune; tune.ring_kb = h->gemm_ring_kb; tune.pdl = h->use_pdl;
+    KL(h, cls_of[which], s, rc = tc_gemm_launch(h->tc, m, which, layer, A, W, N, K, out, rows_ptr, rows_cap, n_split, split_stride, s, epi, &tune));
     return rc == 0 ? TANDEM_OK : fail(h, rc, "tcgen05 GEMM launch failed (tensor map encode or K % 8 != 0)");
   }
   dim3 grid((N + kSimtTile - 1) / kSimtTile, std::min((rows_cap + kSimtTile - 1) / kSimtTile, 16));
-  KL(h, cls_of[which], s, (gemm_simt_kernel<T><<<grid, 256, 0, s>>>(rows_ptr, 0, (const T*)A, (const T*)W, out, N, K)));
+  KL(h, cls_of[which], s, launch_ex(gemm_simt_kernel<T>, grid, dim3(256), 0, s, h->use_pdl, rows_ptr, 0, (const T*)A, (const T*)W, out, N, K));
   return TANDEM_OK;
 }
 
@@ -155,28 +159,28 @@ template <typename T>
 void launch_residual_norm(tandem_handle* h, cudaStream_t s, int grid, const int32_t* counts, const float* part, int ns, size_t ss, float* x,
                           const T* gain, T* act, const int32_t* out_map, int H, float eps) {
   const int v = (H / 4 + 255) / 256;   // float4 per thread; tandem_init guarantees H % 8 == 0 and H <= 8192
-  if (v <= 1) KL(h, TANDEM_KC_RESIDUAL_NORM, s, (residual_norm_kernel<T, 256, 1><<<grid, 256, 0, s>>>(counts, part, ns, ss, x, gain, act, out_map, H, eps)));
-  else if (v <= 2) KL(h, TANDEM_KC_RESIDUAL_NORM, s, (residual_norm_kernel<T, 256, 2><<<grid, 256, 0, s>>>(counts, part, ns, ss, x, gain, act, out_map, H, eps)));
-  else if (v <= 4) KL(h, TANDEM_KC_RESIDUAL_NORM, s, (residual_norm_kernel<T, 256, 4><<<grid, 256, 0, s>>>(counts, part, ns, ss, x, gain, act, out_map, H, eps)));
-  else KL(h, TANDEM_KC_RESIDUAL_NORM, s, (residual_norm_kernel<T, 256, 8><<<grid, 256, 0, s>>>(counts, part, ns, ss, x, gain, act, out_map, H, eps)));
+  if (v <= 1) KL(h, TANDEM_KC_RESIDUAL_NORM, s, launch_ex(residual_norm_kernel<T, 256, 1>, dim3(grid), dim3(256), 0, s, h->use_pdl, counts, part, ns, ss, x, gain, act, out_map, H, eps));
+  else if (v <= 2) KL(h, TANDEM_KC_RESIDUAL_NORM, s, launch_ex(residual_norm_kernel<T, 256, 2>, dim3(grid), dim3(256), 0, s, h->use_pdl, counts, part, ns, ss, x, gain, act, out_map, H, eps));
+  else if (v <= 4) KL(h, TANDEM_KC_RESIDUAL_NORM, s, launch_ex(residual_norm_kernel<T, 256, 4>, dim3(grid), dim3(256), 0, s, h->use_pdl, counts, part, ns, ss, x, gain, act, out_map, H, eps));
+  else KL(h, TANDEM_KC_RESIDUAL_NORM, s, launch_ex(residual_norm_kernel<T, 256, 8>, dim3(grid), dim3(256), 0, s, h->use_pdl, counts, part, ns, ss, x, gain, act, out_map, H, eps));
 }
 
 template <typename T, int D, int G>
-void launch_attn_dg(const AttnArgs<T>& a, int grid, cudaStream_t s) {
-  paged_attention_kernel<T, D, G><<<grid, kAttnThreads, 0, s>>>(a);
+void launch_attn_dg(const AttnArgs<T>& a, int grid, cudaStream_t s, bool pdl) {
+  launch_ex(paged_attention_kernel<T, D, G>, dim3(grid), dim3(kAttnThreads), 0, s, pdl, a);
 }
 template <typename T> struct AttnDispatch;
 template <> struct AttnDispatch<float> {
-  static bool run(const AttnArgs<float>& a, int D, int G, int grid, cudaStream_t s) {
-#define TD_CASE(d, g) if (D == d && G == g) { launch_attn_dg<float, d, g>(a, grid, s); return true; }
+  static bool run(const AttnArgs<float>& a, int D, int G, int grid, cudaStream_t s, bool pdl) {
+#define TD_CASE(d, g) if (D == d && G == g) { launch_attn_dg<float, d, g>(a, grid, s, pdl); return true; }
     TD_CASE(32, 1) TD_CASE(32, 2) TD_CASE(32, 4) TD_CASE(64, 1) TD_CASE(64, 2) TD_CASE(64, 4) TD_CASE(128, 1) TD_CASE(128, 2) TD_CASE(128, 4)
 #undef TD_CASE
     return false;
   }
 };
 template <> struct AttnDispatch<bf16> {
-  static bool run(const AttnArgs<bf16>& a, int D, int G, int grid, cudaStream_t s) {
-#define TD_CASE(d, g) if (D == d && G == g) { launch_attn_dg<bf16, d, g>(a, grid, s); return true; }
+  static bool run(const AttnArgs<bf16>& a, int D, int G, int grid, cudaStream_t s, bool pdl) {
+#define TD_CASE(d, g) if (D == d && G == g) { launch_attn_dg<bf16, d, g>(a, grid, s, pdl); return true; }
     TD_CASE(64, 1) TD_CASE(64, 2) TD_CASE(64, 4) TD_CASE(64, 7) TD_CASE(64, 8) TD_CASE(128, 1) TD_CASE(128, 2) TD_CASE(128, 4) TD_CASE(128, 8)
 #undef TD_CASE
     return false;
@@ -184,16 +188,15 @@ template <> struct AttnDispatch<bf16> {
 };
 template <int D, int G> struct AmStages { static constexpr int value = D == 128 ? 2 : 4; };
 template <int D, int G>
-bool launch_attn_mma_dg(const CUtensorMap& map, const AttnMmaArgs& a, int grid, cudaStream_t s, bool set_attr) {
+bool launch_attn_mma_dg(const CUtensorMap& map, const AttnMmaArgs& a, int grid, cudaStream_t s, bool set_attr, bool pdl) {
   constexpr int ST = AmStages<D, G>::value;
   constexpr int smem = attn_mma_smem_bytes<D, ST>();
   if (set_attr) return cudaFuncSetAttribute(paged_attention_mma_kernel<D, G, ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) == cudaSuccess;
-  paged_attention_mma_kernel<D, G, ST><<<grid, kAmThreads, smem, s>>>(map, a);
-  return true;
+  return launch_ex(paged_attention_mma_kernel<D, G, ST>, dim3(grid), dim3(kAmThreads), smem, s, pdl, map, a) == cudaSuccess;
 }
 // set_attr = true: only raise the kernel's dynamic shared memory limit (called once from tandem_init)
-bool run_attn_mma(const CUtensorMap& map, const AttnMmaArgs& a, int D, int G, int grid, cudaStream_t s, bool set_attr) {
-#define TD_CASE(d, g) if (D == d && G == g) return launch_attn_mma_dg<d, g>(map, a, grid, s, set_attr);
+bool run_attn_mma(const CUtensorMap& map, const AttnMmaArgs& a, int D, int G, int grid, cudaStream_t s, bool set_attr, bool pdl = false) {
+#define TD_CASE(d, g) if (D == d && G == g) return launch_attn_mma_dg<d, g>(map, a, grid, s, set_attr, pdl);
   TD_CASE(64, 1) TD_CASE(64, 2) TD_CASE(64, 4) TD_CASE(64, 7) TD_CASE(64, 8) TD_CASE(128, 1) TD_CASE(128, 2) TD_CASE(128, 4) TD_CASE(128, 8)
 #undef TD_CASE
   return false;
@@ -225,8 +228,8 @@ int model_forward(tandem_handle* h, int m, const StepIO& io, const RuleParams& r
     if ((rc = launch_gemm<T>(h, m, 0, l, ws.act, w.wqkv[l], qkv_n, H, ws.gemm_out, tb.counts + C_ROWS, h->row_cap, &ns, &ss, s))) return rc;
     // S4 RoPE + KV append
     const bool mma = h->attn_impl == TANDEM_ATTN_MMA;
-    if (mma) KL(h, TANDEM_KC_ROPE_APPEND, s, (rope_append_kernel<T, bf16, 256><<<row_grid, 256, 0, s>>>(tb.counts, tb.row_pos, tb.row_kvslot, ws.gemm_out, ns, ss, h->rope_cs, (bf16*)ws.q, kpool, vpool, nq, nkv, d)));
-    else KL(h, TANDEM_KC_ROPE_APPEND, s, (rope_append_kernel<T, float, 256><<<row_grid, 256, 0, s>>>(tb.counts, tb.row_pos, tb.row_kvslot, ws.gemm_out, ns, ss, h->rope_cs, (float*)ws.q, kpool, vpool, nq, nkv, d)));
+    if (mma) KL(h, TANDEM_KC_ROPE_APPEND, s, launch_ex(rope_append_kernel<T, bf16, 256>, dim3(row_grid), dim3(256), 0, s, h->use_pdl, tb.counts, tb.row_pos, tb.row_kvslot, ws.gemm_out, ns, ss, h->rope_cs, (bf16*)ws.q, kpool, vpool, nq, nkv, d));
+    else KL(h, TANDEM_KC_ROPE_APPEND, s, launch_ex(rope_append_kernel<T, float, 256>, dim3(row_grid), dim3(256), 0, s, h->use_pdl, tb.counts, tb.row_pos, tb.row_kvslot, ws.gemm_out, ns, ss, h->rope_cs, (float*)ws.q, kpool, vpool, nq, nkv, d));
     // S5 attention (decode splits + catch-up rows), then combine
     bool ok = true;
     if (mma) {
@@ -234,15 +237,15 @@ int model_forward(tandem_handle* h, int m, const StepIO& io, const RuleParams& r
       AttnMmaArgs ma{tb.counts, tb.item_row0, tb.item_ntok, tb.item_kv0, tb.item_kv1, tb.item_part, tb.row_slot, tb.row_pos, h->pt[m].bt, h->max_pages,
                      (const bf16*)ws.q, (bf16*)ws.attn_out, ws.part_acc, ws.part_ml, nq, nkv, 1.0f / sqrtf((float)d),
                      (int)((2ll * l) * rows_per_half), (int)((2ll * l + 1) * rows_per_half), h->work_ctr + m * c.n_layers + l};
-      KL(h, TANDEM_KC_ATTENTION, s, ok = run_attn_mma(*h->kv_map[m], ma, d, nq / nkv, 2 * h->n_sms, s, false));
+      KL(h, TANDEM_KC_ATTENTION, s, ok = run_attn_mma(*h->kv_map[m], ma, d, nq / nkv, h->attn_ctas_per_sm * h->n_sms, s, false, h->use_pdl));
     } else {
       AttnArgs<T> aa{tb.counts, tb.item_row0, tb.item_ntok, tb.item_kv0, tb.item_kv1, tb.item_part, tb.row_slot, tb.row_pos, h->pt[m].bt, h->max_pages, (const float*)ws.q, kpool, vpool,
                      (T*)ws.attn_out, ws.part_acc, ws.part_ml, nq, nkv, 1.0f / sqrtf((float)d)};
-      KL(h, TANDEM_KC_ATTENTION, s, ok = AttnDispatch<T>::run(aa, d, nq / nkv, 148 * 4, s));
+      KL(h, TANDEM_KC_ATTENTION, s, ok = AttnDispatch<T>::run(aa, d, nq / nkv, 148 * 4, s, h->use_pdl));
     }
     if (!ok) return fail(h, TANDEM_EINVAL, "unsupported (head_dim, group) for attention");
     CombineArgs<T> ca{tb.counts, tb.comb_row, tb.comb_part0, tb.comb_n, tb.comb_stride, ws.part_acc, ws.part_ml, (T*)ws.attn_out, nq, d};
-    KL(h, TANDEM_KC_ATTN_COMBINE, s, (attn_combine_kernel<T><<<148, 256, 0, s>>>(ca)));
+    KL(h, TANDEM_KC_ATTN_COMBINE, s, launch_ex(attn_combine_kernel<T>, dim3(148), dim3(256), 0, s, h->use_pdl, ca));
     // S6 O projection + residual + RMSNorm(mlp)
     if ((rc = launch_gemm<T>(h, m, 1, l, ws.attn_out, w.wo[l], H, nq * d, ws.gemm_out, tb.counts + C_ROWS, h->row_cap, &ns, &ss, s))) return rc;
     launch_residual_norm<T>(h, s, row_grid, tb.counts, ws.gemm_out, ns, ss, ws.x, (const T*)w.mlp_norm[l], (T*)ws.act, nullptr, H, c.rms_eps);
@@ -251,7 +254,7 @@ int model_forward(tandem_handle* h, int m, const StepIO& io, const RuleParams& r
       if ((rc = launch_gemm<T>(h, m, 2, l, ws.act, w.wgu[l], 2 * I, H, (float*)ws.mlp_act, tb.counts + C_ROWS, h->row_cap, &ns, &ss, s, kTcEpiSwiGLU))) return rc;
     } else {
       if ((rc = launch_gemm<T>(h, m, 2, l, ws.act, w.wgu[l], 2 * I, H, ws.gemm_out, tb.counts + C_ROWS, h->row_cap, &ns, &ss, s))) return rc;
-      KL(h, TANDEM_KC_SWIGLU, s, (swiglu_kernel<T, 256><<<row_grid, 256, 0, s>>>(tb.counts, ws.gemm_out, ns, ss, (T*)ws.mlp_act, I)));
+      KL(h, TANDEM_KC_SWIGLU, s, launch_ex(swiglu_kernel<T, 256>, dim3(row_grid), dim3(256), 0, s, h->use_pdl, tb.counts, ws.gemm_out, ns, ss, (T*)ws.mlp_act, I));
     }
     if ((rc = launch_gemm<T>(h, m, 3, l, ws.mlp_act, w.wdown[l], H, I, ws.gemm_out, tb.counts + C_ROWS, h->row_cap, &ns, &ss, s))) return rc;
     const bool last = l == c.n_layers - 1;
@@ -261,7 +264,7 @@ int model_forward(tandem_handle* h, int m, const StepIO& io, const RuleParams& r
   // S8 LM head on the emitting rows only, then sample + switch + emit
   if ((rc = launch_gemm<T>(h, m, 4, 0, ws.lm_in, w.lm_head, V, H, ws.logits, tb.counts + C_EMIT, c.max_seqs, &ns, &ss, s))) return rc;
   SampleArgs sa{h->st, tb, io, rp, ws.logits, h->word_start_dev, h->tokens, h->out_owner, h->out_logp, V, c.max_seq_len, m};
-  KL(h, TANDEM_KC_SAMPLE, s, (sample_switch_emit_kernel<256><<<c.max_seqs, 256, 0, s>>>(sa)));
+  KL(h, TANDEM_KC_SAMPLE, s, launch_ex(sample_switch_emit_kernel<256>, dim3(c.max_seqs), dim3(256), 0, s, h->use_pdl, sa));
   return TANDEM_OK;
 }
 
@@ -601,6 +604,9 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
   INIT_CU(cudaEventCreateWithFlags(&h->ev_in, cudaEventDisableTiming));
   INIT_CU(cudaEventCreateWithFlags(&h->ev_out, cudaEventDisableTiming));
   INIT_CU(cudaStreamCreateWithFlags(&h->gs, cudaStreamNonBlocking));
+  if (const char* e = getenv("TANDEM_ATTN_CTAS_PER_SM")) h->attn_ctas_per_sm = std::max(1, std::min(2, atoi(e)));
+  if (const char* e = getenv("TANDEM_PDL")) h->use_pdl = atoi(e) != 0;
+  if (const char* e = getenv("TANDEM_GEMM_RING_KB")) h->gemm_ring_kb = std::max(0, std::min(200, atoi(e)));
   {
     int dev_sms = 0;
     if (cudaDeviceGetAttribute(&dev_sms, cudaDevAttrMultiProcessorCount, c.device) == cudaSuccess && dev_sms > 0) h->n_sms = dev_sms;
@@ -881,11 +887,11 @@ int tandem_test_gemm(int32_t dtype, int32_t impl, int32_t rows, int32_t N, int32
   return cudaDeviceSynchronize() == cudaSuccess ? TANDEM_OK : TANDEM_ECUDA;
 }
 
-int tandem_test_gemm_time(int32_t rows, int32_t N, int32_t K, int32_t iters, int32_t cluster, int32_t ring_kb, int32_t splits, int32_t swiglu,
+int tandem_test_gemm_time(int32_t rows, int32_t N, int32_t K, int32_t iters, int32_t cluster, int32_t ring_kb, int32_t splits, int32_t flags,
                           float* ms_per_launch) {
   if (rows <= 0 || N <= 0 || K <= 0 || iters <= 0 || !ms_per_launch) return TANDEM_EINVAL;
-  TcGemmTune t; t.cl = cluster; t.ring_kb = ring_kb; t.splits = splits;
-  return tc_gemm_time(rows, N, K, iters, t, swiglu ? kTcEpiSwiGLU : kTcEpiPartial, ms_per_launch);
+  TcGemmTune t; t.cl = cluster; t.ring_kb = ring_kb; t.splits = splits; t.pdl = (flags & 2) != 0;
+  return tc_gemm_time(rows, N, K, iters, t, (flags & 1) ? kTcEpiSwiGLU : kTcEpiPartial, ms_per_launch);
 }
 
 }  // extern "C"
