@@ -41,8 +41,9 @@ constexpr int kAttnThreads = 128;
 constexpr int kAttnTile = 64;   // KV positions per softmax tile
 
 template <typename T, int D, int G>
-__global__ void __launch_bounds__(kAttnThreads) paged_attention_kernel(AttnArgs<T> a) {
+__global__ void __launch_bounds__(kAttnThreads) paged_attention_kernel(const __grid_constant__ Pair<AttnArgs<T>> pp) {
   pdl_trigger(); pdl_wait();
+  const AttnArgs<T>& a = pp.m[blockIdx.y];
   constexpr int VEC = 16 / (int)sizeof(T);
   constexpr int LPP = D / VEC;                   // lanes cooperating on one KV position
   constexpr int PPW = 32 / LPP;                  // positions per warp per iteration
@@ -209,8 +210,9 @@ template <typename T> struct CombineArgs {
 };
 // One warp per (row, head); lane = 4 consecutive dims; all partial loads of a row are independent (n <= kAttnMaxSplits).
 template <typename T>
-__global__ void __launch_bounds__(256) attn_combine_kernel(CombineArgs<T> a) {
+__global__ void __launch_bounds__(256) attn_combine_kernel(const __grid_constant__ Pair<CombineArgs<T>> pp) {
   pdl_trigger(); pdl_wait();
+  const CombineArgs<T>& a = pp.m[blockIdx.y];
   const int n_units = a.counts[C_COMB] * a.nq;
   const int lane = threadIdx.x & 31;
   for (int unit = blockIdx.x * (blockDim.x / 32) + (threadIdx.x >> 5); unit < n_units; unit += gridDim.x * (blockDim.x / 32)) {

@@ -57,7 +57,7 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
 }
 
 template <int D, int G, int STAGES>
-__global__ void __launch_bounds__(kAmThreads, 2) paged_attention_mma_kernel(const __grid_constant__ CUtensorMap tmap_kv, AttnMmaArgs a) {
+__global__ void __launch_bounds__(kAmThreads, 2) paged_attention_mma_kernel(const __grid_constant__ Pair<CUtensorMap> maps, const __grid_constant__ Pair<AttnMmaArgs> ap) {
   constexpr int HALVES = D / 64;                    // 128-byte swizzle rows per K/V row
   constexpr int PAGE_BYTES = kPageTokens * D * 2;   // one (page, kv head) block of K or V
   constexpr int KV_BYTES = 4 * PAGE_BYTES;          // K (or V) part of a stage
@@ -74,7 +74,10 @@ __global__ void __launch_bounds__(kAmThreads, 2) paged_attention_mma_kernel(cons
 
   pdl_trigger();
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int n_units = a.counts[C_ITEMS] * a.nkv;   // written by the scheduler, complete long before this kernel can start
+  // units of both models share one index space (senior first) and one work counter: the tail is balanced across models
+  const int nkv = ap.m[0].nkv;
+  const int n_units0 = ap.m[0].counts[C_ITEMS] * nkv;   // written by the scheduler, complete long before this kernel can start
+  const int n_units = n_units0 + ap.m[1].counts[C_ITEMS] * nkv;
   if ((int)blockIdx.x >= n_units) { pdl_wait(); return; }
   const uint32_t ring = (ptx::smem_u32(am_smem_raw) + 1023u) & ~1023u;
   float* scratch = reinterpret_cast<float*>(am_smem_raw + (ring - ptx::smem_u32(am_smem_raw)) + STAGES * STAGE_BYTES);   // [4][16][OSTRIDE]
@@ -84,7 +87,8 @@ __global__ void __launch_bounds__(kAmThreads, 2) paged_attention_mma_kernel(cons
   if (threadIdx.x == 0) {
     for (int s = 0; s < STAGES; ++s) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 4); }
     ptx::fence_mbar_init();
-    ptx::prefetch_tmap(&tmap_kv);
+    ptx::prefetch_tmap(&maps.m[0]);
+    ptx::prefetch_tmap(&maps.m[1]);
   }
   __syncthreads();
   pdl_wait();                                       // q and this step's K/V come from the predecessor (rope_append)
@@ -96,7 +100,11 @@ __global__ void __launch_bounds__(kAmThreads, 2) paged_attention_mma_kernel(cons
     int u = blockIdx.x;
     while (true) {
       if (u < n_units) {
-        const int item = u / a.nkv, kvh = u - item * a.nkv;
+        const int mdl = u >= n_units0 ? 1 : 0;
+        const AttnMmaArgs& a = ap.m[mdl];
+        const CUtensorMap* tmap_kv = &maps.m[mdl];
+        const int ul = u - mdl * n_units0;
+        const int item = ul / nkv, kvh = ul - item * nkv;
         const int slot = a.row_slot[a.item_row0[item]];
         const int kv0 = a.item_kv0[item], kv1 = a.item_kv1[item];
         const int n_tiles = (kv1 - kv0 + kAmTileTok - 1) / kAmTileTok;
@@ -117,13 +125,13 @@ __global__ void __launch_bounds__(kAmThreads, 2) paged_attention_mma_kernel(cons
             const uint32_t dk = ring + (uint32_t)(s * STAGE_BYTES + lane * PAGE_BYTES);
 #pragma unroll
             for (int hh = 0; hh < HALVES; ++hh) {
-              ptx::tma_load_2d(dk + hh * 2048, &tmap_kv, hh * 64, rk, full_bar(s), pol);
-              ptx::tma_load_2d(dk + KV_BYTES + hh * 2048, &tmap_kv, hh * 64, rv, full_bar(s), pol);
+              ptx::tma_load_2d(dk + hh * 2048, tmap_kv, hh * 64, rk, full_bar(s), pol);
+              ptx::tma_load_2d(dk + KV_BYTES + hh * 2048, tmap_kv, hh * 64, rv, full_bar(s), pol);
             }
           }
         }
         int nu = 0;
-        if (lane == 0) nu = atomicAdd(a.work_ctr, 1) + (int)gridDim.x;
+        if (lane == 0) nu = atomicAdd(ap.m[0].work_ctr, 1) + (int)gridDim.x;
         u = __shfl_sync(0xffffffffu, nu, 0);
       } else {
         if (lane == 0) {   // sentinel stage: tells the consumers to stop
@@ -139,7 +147,7 @@ __global__ void __launch_bounds__(kAmThreads, 2) paged_attention_mma_kernel(cons
   }
 
   // ==================================================================== consumers
-  const float c2 = a.scale * 1.4426950408889634f;          // scores are kept as raw dots; p = 2^((s - m) * c2)
+  const float c2 = ap.m[0].scale * 1.4426950408889634f;          // scores are kept as raw dots; p = 2^((s - m) * c2)
   const int quad = lane & 3, qrow = lane >> 2;
   // lane-constant parts of the ldmatrix addresses (see the layout notes in DESIGN.md section 6)
   const int kmat = lane >> 3;
@@ -152,7 +160,10 @@ __global__ void __launch_bounds__(kAmThreads, 2) paged_attention_mma_kernel(cons
     ptx::mbar_wait(full_bar(it % STAGES), ((uint32_t)(it / STAGES)) & 1u);    // first stage of the next unit (or the sentinel)
     const int u = s_meta[it % STAGES].x;
     if (u < 0) break;
-    const int item = u / a.nkv, kvh = u - item * a.nkv;
+    const int mdl = u >= n_units0 ? 1 : 0;
+    const AttnMmaArgs& a = ap.m[mdl];
+    const int ul = u - mdl * n_units0;
+    const int item = ul / nkv, kvh = ul - item * nkv;
     const int row0 = a.item_row0[item], n_tok = a.item_ntok[item], part = a.item_part[item];
     const int kv0 = a.item_kv0[item], kv1 = a.item_kv1[item];
     const int pos0 = a.row_pos[row0];

@@ -47,6 +47,11 @@ __device__ __forceinline__ void st4(bf16* p, float4 v) {
 }
 __device__ __forceinline__ float4 add4(float4 a, float4 b) { return make_float4(a.x + b.x, a.y + b.y, a.z + b.z, a.w + b.w); }
 
+// Every kernel of the model chain is launched once for BOTH models (senior = 0, junior = 1): the two argument sets travel as
+// one __grid_constant__ parameter and the model is a grid dimension (or, for attention, part of the unit index). Two
+// independent half-sized problems per launch hide each other's latencies and halve the launch count.
+template <typename A> struct Pair { A m[2]; };
+
 // counts[] indices of a per-model step table
 enum { C_ROWS = 0, C_SCHED = 1, C_EMIT = 2, C_ITEMS = 3, C_COMB = 4, C_PARTS = 5, C_NUM = 8 };
 

@@ -10,10 +10,13 @@ namespace tandem {
 constexpr int kSimtTile = 32;
 
 // grid: (ceil(N/32), row-tile lanes); each CTA walks row tiles r0 = blockIdx.y*32, += gridDim.y*32 while r0 < n_rows.
+template <typename T> struct SimtGemmArgs { const int32_t* n_rows_ptr; int n_rows_fixed; const T* A; const T* W; float* out; int N, K; };
 template <typename T>
-__global__ void __launch_bounds__(256) gemm_simt_kernel(const int32_t* __restrict__ n_rows_ptr, int n_rows_fixed, const T* __restrict__ A,
-                                                        const T* __restrict__ W, float* __restrict__ out, int N, int K) {
+__global__ void __launch_bounds__(256) gemm_simt_kernel(const __grid_constant__ Pair<SimtGemmArgs<T>> pp) {
   pdl_trigger(); pdl_wait();
+  const SimtGemmArgs<T>& a = pp.m[blockIdx.z];
+  const int32_t* __restrict__ n_rows_ptr = a.n_rows_ptr; const int n_rows_fixed = a.n_rows_fixed;
+  const T* __restrict__ A = a.A; const T* __restrict__ W = a.W; float* __restrict__ out = a.out; const int N = a.N, K = a.K;
   __shared__ float As[kSimtTile][kSimtTile + 1];
   __shared__ float Ws[kSimtTile][kSimtTile + 1];
   const int n_rows = n_rows_ptr ? *n_rows_ptr : n_rows_fixed;

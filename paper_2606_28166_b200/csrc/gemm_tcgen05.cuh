@@ -23,7 +23,7 @@ namespace tandem {
 
 constexpr int kTcTileN = 128;        // weight rows per CTA = UMMA M
 constexpr int kTcBlockK = 64;        // bf16 elements per k-block = one 128-byte swizzle row
-constexpr int kTcRowBox = 32;        // token rows per TMA box of A
+constexpr int kTcRowBox = 16;        // token rows per TMA box of A (= granularity of UMMA N)
 constexpr int kTcMaxRows = 256;      // token rows per accumulator pass = max UMMA N
 constexpr int kTcMaxStages = 10;
 constexpr int kTcRingBytes = 200 * 1024;
@@ -116,6 +116,8 @@ __device__ __forceinline__ uint32_t umma_idesc_bf16(int n) {
   return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(kTcTileN >> 4) << 24);
 }
 
+struct TcMaps { CUtensorMap w[2], a[2]; };   // weight and activation descriptors of the two models
+
 struct TcGemmArgs {
   float* out;                 // [n_split][row_cap][N] fp32 partials
   const int32_t* rows_ptr;    // device scalar with the live row count, or null
@@ -151,7 +153,10 @@ enum { kTcEpiPartial = 0, kTcEpiSwiGLU = 1 };
 //        kTcEpiSwiGLU : W rows interleaved (2i = gate_i, 2i+1 = up_i), n_split = 1: act[r][i] = silu(gate) * up as bf16.
 template <int CL, int EPI>
 __global__ void __launch_bounds__(kTcThreads, 1)
-gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_constant__ CUtensorMap tmap_a, TcGemmArgs g) {
+gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ Pair<TcGemmArgs> gp) {
+  const TcGemmArgs& g = gp.m[blockIdx.z];                  // blockIdx.z = model
+  const CUtensorMap* tmap_w = &maps.w[blockIdx.z];
+  const CUtensorMap* tmap_a = &maps.a[blockIdx.z];
   extern __shared__ uint8_t tc_smem_raw[];
   __shared__ __align__(8) uint64_t bars[2 * kTcMaxStages + 2];
   __shared__ uint32_t tmem_base_smem;
@@ -184,8 +189,8 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_con
     ptx::mbar_init(tmem_full_bar, 1);
     ptx::mbar_init(tmem_empty_bar, 4);
     ptx::fence_mbar_init();
-    ptx::prefetch_tmap(&tmap_w);
-    ptx::prefetch_tmap(&tmap_a);
+    ptx::prefetch_tmap(tmap_w);
+    ptx::prefetch_tmap(tmap_a);
   }
   if (warp == 2) ptx::tmem_alloc<kTcMaxRows>(ptx::smem_u32(&tmem_base_smem));
   ptx::tc_fence_before();
@@ -203,14 +208,14 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_con
       const int nbox0 = (min(rows, kTcMaxRows) + kTcRowBox - 1) / kTcRowBox;
       for (int i = 0; i < npre; ++i) {
         ptx::mbar_expect_tx(full_bar(i), (uint32_t)(kTcWBytes + nbox0 * kTcABoxBytes));
-        ptx::tma_load_2d(ring + (uint32_t)(i * stage_bytes), &tmap_w, (kb0 + i) * kTcBlockK, n0, full_bar(i), pol_w);
+        ptx::tma_load_2d(ring + (uint32_t)(i * stage_bytes), tmap_w, (kb0 + i) * kTcBlockK, n0, full_bar(i), pol_w);
       }
       pdl_wait();
       for (int i = 0; i < npre; ++i) {
         const uint32_t dst = ring + (uint32_t)(i * stage_bytes);
         for (int j = (int)cta_rank; j < nbox0; j += CL) {
-          if (CL > 1) ptx::tma_load_2d_mc(dst + kTcWBytes + j * kTcABoxBytes, &tmap_a, (kb0 + i) * kTcBlockK, j * kTcRowBox, full_bar(i), kMask, pol_a);
-          else ptx::tma_load_2d(dst + kTcWBytes + j * kTcABoxBytes, &tmap_a, (kb0 + i) * kTcBlockK, j * kTcRowBox, full_bar(i), pol_a);
+          if (CL > 1) ptx::tma_load_2d_mc(dst + kTcWBytes + j * kTcABoxBytes, tmap_a, (kb0 + i) * kTcBlockK, j * kTcRowBox, full_bar(i), kMask, pol_a);
+          else ptx::tma_load_2d(dst + kTcWBytes + j * kTcABoxBytes, tmap_a, (kb0 + i) * kTcBlockK, j * kTcRowBox, full_bar(i), pol_a);
         }
       }
       int it = 0;
@@ -224,10 +229,10 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_con
           ptx::mbar_wait(empty_bar(s), ph ^ 1u);
           const uint32_t dst = ring + (uint32_t)(s * stage_bytes);
           ptx::mbar_expect_tx(full_bar(s), (uint32_t)(kTcWBytes + nbox * kTcABoxBytes));
-          ptx::tma_load_2d(dst, &tmap_w, kb * kTcBlockK, n0, full_bar(s), pol_w);
+          ptx::tma_load_2d(dst, tmap_w, kb * kTcBlockK, n0, full_bar(s), pol_w);
           for (int j = (int)cta_rank; j < nbox; j += CL) {
-            if (CL > 1) ptx::tma_load_2d_mc(dst + kTcWBytes + j * kTcABoxBytes, &tmap_a, kb * kTcBlockK, r0 + j * kTcRowBox, full_bar(s), kMask, pol_a);
-            else ptx::tma_load_2d(dst + kTcWBytes + j * kTcABoxBytes, &tmap_a, kb * kTcBlockK, r0 + j * kTcRowBox, full_bar(s), pol_a);
+            if (CL > 1) ptx::tma_load_2d_mc(dst + kTcWBytes + j * kTcABoxBytes, tmap_a, kb * kTcBlockK, r0 + j * kTcRowBox, full_bar(s), kMask, pol_a);
+            else ptx::tma_load_2d(dst + kTcWBytes + j * kTcABoxBytes, tmap_a, kb * kTcBlockK, r0 + j * kTcRowBox, full_bar(s), pol_a);
           }
         }
       }
@@ -371,23 +376,21 @@ inline const CUtensorMap* tc_gemm_map(TcGemmPlans* p, const void* base, int n_ro
 // activations [rows, N/2] (epi = kTcEpiSwiGLU; W rows interleaved gate/up). Returns 0, or -1 (TANDEM_EINVAL) / -3 (TANDEM_ECUDA).
 // which == 4 (LM head) never splits: the sampler reads the logits in place.
 template <int CL, int EPI>
-inline int tc_gemm_launch_cl(const CUtensorMap* mw, const CUtensorMap* ma, const TcGemmArgs& g, dim3 grid, cudaStream_t s, bool pdl) {
+inline int tc_gemm_launch_cl(const TcMaps& maps, const Pair<TcGemmArgs>& g, dim3 grid, cudaStream_t s, bool pdl) {
   cudaLaunchConfig_t cfg{};
-  cfg.gridDim = grid; cfg.blockDim = dim3(kTcThreads); cfg.dynamicSmemBytes = (size_t)g.ring_bytes + 1024; cfg.stream = s;
+  cfg.gridDim = grid; cfg.blockDim = dim3(kTcThreads); cfg.dynamicSmemBytes = (size_t)g.m[0].ring_bytes + 1024; cfg.stream = s;
   cudaLaunchAttribute at[2];
   at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
   at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[1].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = at; cfg.numAttrs = pdl ? 2 : 1;
-  return cudaLaunchKernelEx(&cfg, gemm_tcgen05_kernel<CL, EPI>, *mw, *ma, g) == cudaSuccess ? 0 : -3;
+  return cudaLaunchKernelEx(&cfg, gemm_tcgen05_kernel<CL, EPI>, maps, g) == cudaSuccess ? 0 : -3;
 }
-struct TcGemmTune { int cl = 0, ring_kb = 0, splits = 0; bool pdl = false; };   // 0 = automatic; overrides for tandem_test_gemm_time only
-inline int tc_gemm_launch(TcGemmPlans* p, int /*model*/, int which, int /*layer*/, const void* A, const void* W, int N, int K, float* out,
-                          const int32_t* rows_ptr, int rows_cap, int* n_split, size_t* split_stride, cudaStream_t s, int epi = kTcEpiPartial,
+struct TcGemmTune { int cl = 0, ring_kb = 0, splits = 0; bool pdl = false; };   // 0 = automatic; overrides for tuning / tandem_test_gemm_time
+// One launch for n_models (1 or 2) problems of the same shape: out[m] = A[m] W[m]^T, rows of model m from rows_ptr[m].
+inline int tc_gemm_launch(TcGemmPlans* p, int n_models, int which, const void* const* A, const void* const* W, int N, int K, float* const* out,
+                          const int32_t* const* rows_ptr, int rows_cap, int* n_split, size_t* split_stride, cudaStream_t s, int epi = kTcEpiPartial,
                           const TcGemmTune* tune = nullptr) {
   if (!p || (K % 8) != 0) return -1;                       // TMA needs 16-byte row strides
-  const CUtensorMap* mw = tc_gemm_map(p, W, N, K, kTcTileN);
-  const CUtensorMap* ma = tc_gemm_map(p, A, rows_cap, K, kTcRowBox);
-  if (!mw || !ma) return -3;
   int S = (which == 4 || epi == kTcEpiSwiGLU) ? 1 : tc_gemm_splits(N, K);
   if (tune && tune->splits > 0) S = tune->splits;
   *n_split = S;
@@ -398,20 +401,28 @@ inline int tc_gemm_launch(TcGemmPlans* p, int /*model*/, int which, int /*layer*
   int cl = 1;
   if (tune && tune->cl > 0) cl = tune->cl;
   const int tiles_pad = (tiles + cl - 1) / cl * cl;
-  TcGemmArgs g{out, rows_ptr, rows_cap, N, K, S, *split_stride, 0};
-  if (!rows_ptr) g.rows_fixed = rows_cap;
-  g.ring_bytes = tiles_pad * S > 148 ? 98 * 1024 : kTcRingBytes;     // more CTAs than SMs: let two share an SM
-  if (tune && tune->ring_kb > 0) g.ring_bytes = tune->ring_kb * 1024;
-  dim3 grid(tiles_pad, S);
+  TcMaps maps;
+  Pair<TcGemmArgs> g;
+  const int ring = (tune && tune->ring_kb > 0) ? tune->ring_kb * 1024
+                                                : (tiles_pad * S * n_models > 148 ? 109 * 1024 : kTcRingBytes);   // more CTAs than SMs: two share an SM
+  for (int m = 0; m < 2; ++m) {
+    const int mm = m < n_models ? m : 0;
+    const CUtensorMap* mw = tc_gemm_map(p, W[mm], N, K, kTcTileN);
+    const CUtensorMap* ma = tc_gemm_map(p, A[mm], rows_cap, K, kTcRowBox);
+    if (!mw || !ma) return -3;
+    maps.w[m] = *mw; maps.a[m] = *ma;
+    g.m[m] = TcGemmArgs{out[mm], rows_ptr ? rows_ptr[mm] : nullptr, rows_cap, N, K, S, *split_stride, ring};
+  }
+  dim3 grid(tiles_pad, S, n_models);
   const bool pdl = tune && tune->pdl;
   if (epi == kTcEpiSwiGLU) {
-    if (cl == 4) return tc_gemm_launch_cl<4, 1>(mw, ma, g, grid, s, pdl);
-    if (cl == 2) return tc_gemm_launch_cl<2, 1>(mw, ma, g, grid, s, pdl);
-    return tc_gemm_launch_cl<1, 1>(mw, ma, g, grid, s, pdl);
+    if (cl == 4) return tc_gemm_launch_cl<4, 1>(maps, g, grid, s, pdl);
+    if (cl == 2) return tc_gemm_launch_cl<2, 1>(maps, g, grid, s, pdl);
+    return tc_gemm_launch_cl<1, 1>(maps, g, grid, s, pdl);
   }
-  if (cl == 4) return tc_gemm_launch_cl<4, 0>(mw, ma, g, grid, s, pdl);
-  if (cl == 2) return tc_gemm_launch_cl<2, 0>(mw, ma, g, grid, s, pdl);
-  return tc_gemm_launch_cl<1, 0>(mw, ma, g, grid, s, pdl);
+  if (cl == 4) return tc_gemm_launch_cl<4, 0>(maps, g, grid, s, pdl);
+  if (cl == 2) return tc_gemm_launch_cl<2, 0>(maps, g, grid, s, pdl);
+  return tc_gemm_launch_cl<1, 0>(maps, g, grid, s, pdl);
 }
 
 // Unit-test hook: out[rows, N] = A W^T (partials summed here), synchronous.
@@ -428,7 +439,7 @@ inline int tc_gemm_test(int rows, int N, int K, const void* A, const void* W, fl
   if (!p) return -3;
   if (epi == kTcEpiSwiGLU) {   // W rows interleaved gate/up; out is bf16 [rows, N/2]
     int ns; size_t ss;
-    int rc = tc_gemm_launch(p, 0, 2, 0, A, W, N, K, out, nullptr, rows, &ns, &ss, 0, epi);
+    int rc = tc_gemm_launch(p, 1, 2, &A, &W, N, K, &out, nullptr, rows, &ns, &ss, 0, epi);
     if (rc == 0) rc = cudaDeviceSynchronize() == cudaSuccess ? 0 : -3;
     tc_gemm_destroy(p);
     return rc;
@@ -437,7 +448,7 @@ inline int tc_gemm_test(int rows, int N, int K, const void* A, const void* W, fl
   float* part = nullptr;
   if (cudaMalloc(&part, (size_t)S * rows * N * sizeof(float)) != cudaSuccess) { tc_gemm_destroy(p); return -2; }
   int ns; size_t ss;
-  int rc = tc_gemm_launch(p, 0, 0, 0, A, W, N, K, part, nullptr, rows, &ns, &ss, 0);
+  int rc = tc_gemm_launch(p, 1, 0, &A, &W, N, K, &part, nullptr, rows, &ns, &ss, 0);
   if (rc == 0) {
     tc_sum_partials_kernel<<<296, 256>>>(part, ns, ss, out, (size_t)rows * N);
     rc = cudaDeviceSynchronize() == cudaSuccess ? 0 : -3;
@@ -467,7 +478,8 @@ inline int tc_gemm_time(int rows, int N, int K, int iters, const TcGemmTune& tun
     int ns; size_t ss;
     for (int i = 0; i < nbuf + iters && !rc; ++i) {
       if (i == nbuf) cudaEventRecord(e0, 0);
-      rc = tc_gemm_launch(p, 0, epi == kTcEpiSwiGLU ? 2 : 0, 0, A, wb[i % nbuf], N, K, out, nullptr, rows, &ns, &ss, 0, epi, &tune);
+      const void* Ap = A; const void* Wp = wb[i % nbuf];
+      rc = tc_gemm_launch(p, 1, epi == kTcEpiSwiGLU ? 2 : 0, &Ap, &Wp, N, K, &out, nullptr, rows, &ns, &ss, 0, epi, &tune);
     }
     cudaEventRecord(e1, 0);
     if (cudaDeviceSynchronize() != cudaSuccess) rc = -3;

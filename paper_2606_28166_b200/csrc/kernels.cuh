@@ -257,11 +257,14 @@ __global__ void __launch_bounds__(1024) finalize_kernel(FinalArgs a) {
 
 // ============================================================================================ S1+S2: embed + RMSNorm
 // x[r,:] = E[token_r] (fp32 residual stream); u = x g / sqrt(mean x^2 + eps) -> act (GEMM A-operand dtype).
+template <typename T> struct EmbedArgs { const int32_t* counts; const int32_t* row_tok; const T* E; const T* gain; float* x; T* act; int H; float eps; };
 template <typename T, int NT>
-__global__ void __launch_bounds__(NT) embed_norm_kernel(const int32_t* __restrict__ counts, const int32_t* __restrict__ row_tok,
-                                                        const T* __restrict__ E, const T* __restrict__ gain, float* __restrict__ x,
-                                                        T* __restrict__ act, int H, float eps) {
+__global__ void __launch_bounds__(NT) embed_norm_kernel(const __grid_constant__ Pair<EmbedArgs<T>> pp) {
   pdl_trigger(); pdl_wait();
+  const EmbedArgs<T>& a = pp.m[blockIdx.y];
+  const int32_t* __restrict__ counts = a.counts; const int32_t* __restrict__ row_tok = a.row_tok;
+  const T* __restrict__ E = a.E; const T* __restrict__ gain = a.gain; float* __restrict__ x = a.x; T* __restrict__ act = a.act;
+  const int H = a.H; const float eps = a.eps;
   __shared__ float red[32];
   const int n_rows = counts[C_ROWS];
   for (int r = blockIdx.x; r < n_rows; r += gridDim.x) {
@@ -278,11 +281,16 @@ __global__ void __launch_bounds__(NT) embed_norm_kernel(const int32_t* __restric
 // are normalised (with the final-norm gain) and written compactly at their emit index (the LM head runs on those only).
 // One CTA per row; every thread keeps its VPT float4 of the row in registers, and the loads of all splits are
 // independent of each other, so a row costs ~one memory latency instead of n_split * H / NT of them.
+template <typename T> struct ResNormArgs {
+  const int32_t* counts; const float* part; int n_split; size_t split_stride; float* x; const T* gain; T* act; const int32_t* out_map; int H; float eps;
+};
 template <typename T, int NT, int VPT>
-__global__ void __launch_bounds__(NT) residual_norm_kernel(const int32_t* __restrict__ counts, const float* __restrict__ part, int n_split,
-                                                           size_t split_stride, float* __restrict__ x, const T* __restrict__ gain,
-                                                           T* __restrict__ act, const int32_t* __restrict__ out_map, int H, float eps) {
+__global__ void __launch_bounds__(NT) residual_norm_kernel(const __grid_constant__ Pair<ResNormArgs<T>> pp) {
   pdl_trigger(); pdl_wait();
+  const ResNormArgs<T>& a = pp.m[blockIdx.y];
+  const int32_t* __restrict__ counts = a.counts; const float* __restrict__ part = a.part; const int n_split = a.n_split;
+  const size_t split_stride = a.split_stride; float* __restrict__ x = a.x; const T* __restrict__ gain = a.gain; T* __restrict__ act = a.act;
+  const int32_t* __restrict__ out_map = a.out_map; const int H = a.H; const float eps = a.eps;
   __shared__ float red[32];
   const int n_rows = counts[C_ROWS];
   const int H4 = H >> 2;
@@ -326,12 +334,18 @@ __global__ void __launch_bounds__(NT) residual_norm_kernel(const int32_t* __rest
 // qkv[r, :] = sum_s part[s][r, :] is [q (nq*d) | k (nkv*d) | v (nkv*d)]. RoPE (half-split pairs (j, j+d/2), angle
 // pos * theta^(-2j/d) from a table built in double at init) on q and k; q -> buffer of type QT (fp32 for the ALU attention
 // kernel, bf16 for the tensor-core one), k and v -> model M's pages. Four pairs / four v elements per thread per step.
+template <typename T, typename QT> struct RopeArgs {
+  const int32_t* counts; const int32_t* row_pos; const int32_t* row_kvslot; const float* part; int n_split; size_t split_stride;
+  const float2* cs_table; QT* q_out; T* kpool; T* vpool; int nq, nkv, d;
+};
 template <typename T, typename QT, int NT>
-__global__ void __launch_bounds__(NT) rope_append_kernel(const int32_t* __restrict__ counts, const int32_t* __restrict__ row_pos,
-                                                         const int32_t* __restrict__ row_kvslot, const float* __restrict__ part, int n_split,
-                                                         size_t split_stride, const float2* __restrict__ cs_table, QT* __restrict__ q_out,
-                                                         T* __restrict__ kpool, T* __restrict__ vpool, int nq, int nkv, int d) {
+__global__ void __launch_bounds__(NT) rope_append_kernel(const __grid_constant__ Pair<RopeArgs<T, QT>> pp) {
   pdl_trigger(); pdl_wait();
+  const RopeArgs<T, QT>& a = pp.m[blockIdx.y];
+  const int32_t* __restrict__ counts = a.counts; const int32_t* __restrict__ row_pos = a.row_pos; const int32_t* __restrict__ row_kvslot = a.row_kvslot;
+  const float* __restrict__ part = a.part; const int n_split = a.n_split; const size_t split_stride = a.split_stride;
+  const float2* __restrict__ cs_table = a.cs_table; QT* __restrict__ q_out = a.q_out; T* __restrict__ kpool = a.kpool; T* __restrict__ vpool = a.vpool;
+  const int nq = a.nq, nkv = a.nkv, d = a.d;
   const int n_rows = counts[C_ROWS];
   const int half = d >> 1, hq = half >> 2;                 // hq: groups of 4 pairs per head
   const int ld = (nq + 2 * nkv) * d;
@@ -375,10 +389,13 @@ __global__ void __launch_bounds__(NT) rope_append_kernel(const int32_t* __restri
 
 // ============================================================================================ S7: SwiGLU
 // gu[r, :] = [gate (I) | up (I)] summed over splits; out = silu(gate) * up, silu(a) = a / (1 + exp(-a)).
+template <typename T> struct SwigluArgs { const int32_t* counts; const float* part; int n_split; size_t split_stride; T* out; int I; };
 template <typename T, int NT>
-__global__ void __launch_bounds__(NT) swiglu_kernel(const int32_t* __restrict__ counts, const float* __restrict__ part, int n_split,
-                                                    size_t split_stride, T* __restrict__ out, int I) {
+__global__ void __launch_bounds__(NT) swiglu_kernel(const __grid_constant__ Pair<SwigluArgs<T>> pp) {
   pdl_trigger(); pdl_wait();
+  const SwigluArgs<T>& a = pp.m[blockIdx.y];
+  const int32_t* __restrict__ counts = a.counts; const float* __restrict__ part = a.part; const int n_split = a.n_split;
+  const size_t split_stride = a.split_stride; T* __restrict__ out = a.out; const int I = a.I;
   const int n_rows = counts[C_ROWS];
   const int I4 = I >> 2;
   const size_t total = (size_t)n_rows * I4;
@@ -410,8 +427,9 @@ __device__ __forceinline__ ArgBest better(ArgBest a, ArgBest b) {  // larger val
 }
 
 template <int NT>
-__global__ void __launch_bounds__(NT) sample_switch_emit_kernel(SampleArgs a) {
+__global__ void __launch_bounds__(NT) sample_switch_emit_kernel(const __grid_constant__ Pair<SampleArgs> pp) {
   pdl_trigger(); pdl_wait();
+  const SampleArgs& a = pp.m[blockIdx.y];
   __shared__ float s_m[NT / 32], s_s[NT / 32], s_bv[NT / 32], s_gv[NT / 32];
   __shared__ int s_bi[NT / 32], s_gi[NT / 32];
   const int j = blockIdx.x;

@@ -137,41 +137,44 @@ cudaEvent_t prof_event(tandem_handle* h) {
   } while (0)
 
 // ------------------------------------------------------------------------------------------ GEMM dispatch
-// out[s][r][n] partials (s < *n_split, stride *split_stride floats); rows read from counts_ptr[idx] on the device.
+// One launch for both models: out[m][s][r][n] partials (s < *n_split, stride *split_stride floats); rows of model m are
+// read from rows_ptr[m] on the device.
 template <typename T>
-int launch_gemm(tandem_handle* h, int m, int which, int layer, const void* A, const void* W, int N, int K, float* out,
-                const int32_t* rows_ptr, int rows_cap, int* n_split, size_t* split_stride, cudaStream_t s, int epi = kTcEpiPartial) {
+int launch_gemm(tandem_handle* h, int which, const void* const* A, const void* const* W, int N, int K, float* const* out,
+                const int32_t* const* rows_ptr, int rows_cap, int* n_split, size_t* split_stride, cudaStream_t s, int epi = kTcEpiPartial) {
   *n_split = 1;
   *split_stride = (size_t)rows_cap * N;
   static const int cls_of[5] = {TANDEM_KC_GEMM_QKV, TANDEM_KC_GEMM_O, TANDEM_KC_GEMM_GATEUP, TANDEM_KC_GEMM_DOWN, TANDEM_KC_GEMM_LMHEAD};
   if (h->gemm_impl == TANDEM_GEMM_TCGEN05 && sizeof(T) == 2) {
     int rc = 0;
     TcGemmTune tune; tune.ring_kb = h->gemm_ring_kb; tune.pdl = h->use_pdl;
-    KL(h, cls_of[which], s, rc = tc_gemm_launch(h->tc, m, which, layer, A, W, N, K, out, rows_ptr, rows_cap, n_split, split_stride, s, epi, &tune));
+    KL(h, cls_of[which], s, rc = tc_gemm_launch(h->tc, 2, which, A, W, N, K, out, rows_ptr, rows_cap, n_split, split_stride, s, epi, &tune));
     return rc == 0 ? TANDEM_OK : fail(h, rc, "tcgen05 GEMM launch failed (tensor map encode or K % 8 != 0)");
   }
-  dim3 grid((N + kSimtTile - 1) / kSimtTile, std::min((rows_cap + kSimtTile - 1) / kSimtTile, 16));
-  KL(h, cls_of[which], s, launch_ex(gemm_simt_kernel<T>, grid, dim3(256), 0, s, h->use_pdl, rows_ptr, 0, (const T*)A, (const T*)W, out, N, K));
+  dim3 grid((N + kSimtTile - 1) / kSimtTile, std::min((rows_cap + kSimtTile - 1) / kSimtTile, 16), 2);
+  Pair<SimtGemmArgs<T>> g;
+  for (int m = 0; m < 2; ++m) g.m[m] = SimtGemmArgs<T>{rows_ptr[m], 0, (const T*)A[m], (const T*)W[m], out[m], N, K};
+  KL(h, cls_of[which], s, launch_ex(gemm_simt_kernel<T>, grid, dim3(256), 0, s, h->use_pdl, g));
   return TANDEM_OK;
 }
 
 template <typename T>
-void launch_residual_norm(tandem_handle* h, cudaStream_t s, int grid, const int32_t* counts, const float* part, int ns, size_t ss, float* x,
-                          const T* gain, T* act, const int32_t* out_map, int H, float eps) {
-  const int v = (H / 4 + 255) / 256;   // float4 per thread; tandem_init guarantees H % 8 == 0 and H <= 8192
-  if (v <= 1) KL(h, TANDEM_KC_RESIDUAL_NORM, s, launch_ex(residual_norm_kernel<T, 256, 1>, dim3(grid), dim3(256), 0, s, h->use_pdl, counts, part, ns, ss, x, gain, act, out_map, H, eps));
-  else if (v <= 2) KL(h, TANDEM_KC_RESIDUAL_NORM, s, launch_ex(residual_norm_kernel<T, 256, 2>, dim3(grid), dim3(256), 0, s, h->use_pdl, counts, part, ns, ss, x, gain, act, out_map, H, eps));
-  else if (v <= 4) KL(h, TANDEM_KC_RESIDUAL_NORM, s, launch_ex(residual_norm_kernel<T, 256, 4>, dim3(grid), dim3(256), 0, s, h->use_pdl, counts, part, ns, ss, x, gain, act, out_map, H, eps));
-  else KL(h, TANDEM_KC_RESIDUAL_NORM, s, launch_ex(residual_norm_kernel<T, 256, 8>, dim3(grid), dim3(256), 0, s, h->use_pdl, counts, part, ns, ss, x, gain, act, out_map, H, eps));
+void launch_residual_norm(tandem_handle* h, cudaStream_t s, int grid_x, const Pair<ResNormArgs<T>>& a) {
+  const int v = (a.m[0].H / 4 + 255) / 256;   // float4 per thread; tandem_init guarantees H % 8 == 0 and H <= 8192
+  const dim3 grid(grid_x, 2);
+  if (v <= 1) KL(h, TANDEM_KC_RESIDUAL_NORM, s, launch_ex(residual_norm_kernel<T, 256, 1>, grid, dim3(256), 0, s, h->use_pdl, a));
+  else if (v <= 2) KL(h, TANDEM_KC_RESIDUAL_NORM, s, launch_ex(residual_norm_kernel<T, 256, 2>, grid, dim3(256), 0, s, h->use_pdl, a));
+  else if (v <= 4) KL(h, TANDEM_KC_RESIDUAL_NORM, s, launch_ex(residual_norm_kernel<T, 256, 4>, grid, dim3(256), 0, s, h->use_pdl, a));
+  else KL(h, TANDEM_KC_RESIDUAL_NORM, s, launch_ex(residual_norm_kernel<T, 256, 8>, grid, dim3(256), 0, s, h->use_pdl, a));
 }
 
 template <typename T, int D, int G>
-void launch_attn_dg(const AttnArgs<T>& a, int grid, cudaStream_t s, bool pdl) {
-  launch_ex(paged_attention_kernel<T, D, G>, dim3(grid), dim3(kAttnThreads), 0, s, pdl, a);
+void launch_attn_dg(const Pair<AttnArgs<T>>& a, int grid, cudaStream_t s, bool pdl) {
+  launch_ex(paged_attention_kernel<T, D, G>, dim3(grid, 2), dim3(kAttnThreads), 0, s, pdl, a);
 }
 template <typename T> struct AttnDispatch;
 template <> struct AttnDispatch<float> {
-  static bool run(const AttnArgs<float>& a, int D, int G, int grid, cudaStream_t s, bool pdl) {
+  static bool run(const Pair<AttnArgs<float>>& a, int D, int G, int grid, cudaStream_t s, bool pdl) {
 #define TD_CASE(d, g) if (D == d && G == g) { launch_attn_dg<float, d, g>(a, grid, s, pdl); return true; }
     TD_CASE(32, 1) TD_CASE(32, 2) TD_CASE(32, 4) TD_CASE(64, 1) TD_CASE(64, 2) TD_CASE(64, 4) TD_CASE(128, 1) TD_CASE(128, 2) TD_CASE(128, 4)
 #undef TD_CASE
@@ -179,7 +182,7 @@ template <> struct AttnDispatch<float> {
   }
 };
 template <> struct AttnDispatch<bf16> {
-  static bool run(const AttnArgs<bf16>& a, int D, int G, int grid, cudaStream_t s, bool pdl) {
+  static bool run(const Pair<AttnArgs<bf16>>& a, int D, int G, int grid, cudaStream_t s, bool pdl) {
 #define TD_CASE(d, g) if (D == d && G == g) { launch_attn_dg<bf16, d, g>(a, grid, s, pdl); return true; }
     TD_CASE(64, 1) TD_CASE(64, 2) TD_CASE(64, 4) TD_CASE(64, 7) TD_CASE(64, 8) TD_CASE(128, 1) TD_CASE(128, 2) TD_CASE(128, 4) TD_CASE(128, 8)
 #undef TD_CASE
@@ -188,14 +191,14 @@ template <> struct AttnDispatch<bf16> {
 };
 template <int D, int G> struct AmStages { static constexpr int value = D == 128 ? 2 : 4; };
 template <int D, int G>
-bool launch_attn_mma_dg(const CUtensorMap& map, const AttnMmaArgs& a, int grid, cudaStream_t s, bool set_attr, bool pdl) {
+bool launch_attn_mma_dg(const Pair<CUtensorMap>& map, const Pair<AttnMmaArgs>& a, int grid, cudaStream_t s, bool set_attr, bool pdl) {
   constexpr int ST = AmStages<D, G>::value;
   constexpr int smem = attn_mma_smem_bytes<D, ST>();
   if (set_attr) return cudaFuncSetAttribute(paged_attention_mma_kernel<D, G, ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) == cudaSuccess;
   return launch_ex(paged_attention_mma_kernel<D, G, ST>, dim3(grid), dim3(kAmThreads), smem, s, pdl, map, a) == cudaSuccess;
 }
 // set_attr = true: only raise the kernel's dynamic shared memory limit (called once from tandem_init)
-bool run_attn_mma(const CUtensorMap& map, const AttnMmaArgs& a, int D, int G, int grid, cudaStream_t s, bool set_attr, bool pdl = false) {
+bool run_attn_mma(const Pair<CUtensorMap>& map, const Pair<AttnMmaArgs>& a, int D, int G, int grid, cudaStream_t s, bool set_attr, bool pdl = false) {
 #define TD_CASE(d, g) if (D == d && G == g) return launch_attn_mma_dg<d, g>(map, a, grid, s, set_attr, pdl);
   TD_CASE(64, 1) TD_CASE(64, 2) TD_CASE(64, 4) TD_CASE(64, 7) TD_CASE(64, 8) TD_CASE(128, 1) TD_CASE(128, 2) TD_CASE(128, 4) TD_CASE(128, 8)
 #undef TD_CASE
@@ -206,65 +209,116 @@ bool attn_supported(int dtype, int D, int G) {
   return (D == 64 && (G == 1 || G == 2 || G == 4 || G == 7 || G == 8)) || (D == 128 && (G == 1 || G == 2 || G == 4 || G == 8));
 }
 
-// ------------------------------------------------------------------------------------------ one model's forward (S1..S8)
+// ------------------------------------------------------------------------------------------ both models' forward (S1..S8)
+// Every kernel is launched once for the two models (Pair arguments): the models advance layer by layer in lock-step on
+// one stream, each launch carrying the senior's and the junior's half of the work.
 template <typename T>
-int model_forward(tandem_handle* h, int m, const StepIO& io, const RuleParams& rp, cudaStream_t s) {
+int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaStream_t s) {
   const tandem_config& c = h->cfg;
-  const ModelWeights& w = h->w[m];
-  Workspace& ws = h->ws[m];
-  const StepTab& tb = h->tab[m];
   const int H = c.hidden, nq = c.n_q_heads, nkv = c.n_kv_heads, d = c.head_dim, I = c.intermediate, V = c.vocab;
   const int qkv_n = (nq + 2 * nkv) * d;
-  const int row_grid = 148 * 4;
+  const int row_grid = 148 * 2;
   const size_t layer_kv = (size_t)2 * h->pool_pages * nkv * kPageTokens * d;
   const size_t half_kv = (size_t)h->pool_pages * nkv * kPageTokens * d;
+  const bool mma = h->attn_impl == TANDEM_ATTN_MMA;
+  const bool pdl = h->use_pdl;
   int ns; size_t ss; int rc;
+  const void* A[2]; const void* W[2]; float* O[2]; const int32_t* RP[2];
+  auto set_gemm = [&](int m, const void* a_, const void* w_, float* o_, const int32_t* r_) { A[m] = a_; W[m] = w_; O[m] = o_; RP[m] = r_; };
 
-  KL(h, TANDEM_KC_EMBED, s, (embed_norm_kernel<T, 256><<<row_grid, 256, 0, s>>>(tb.counts, tb.row_tok, (const T*)w.embed, (const T*)w.attn_norm[0], ws.x, (T*)ws.act, H, c.rms_eps)));
+  {
+    Pair<EmbedArgs<T>> ea;
+    for (int m = 0; m < 2; ++m) ea.m[m] = EmbedArgs<T>{h->tab[m].counts, h->tab[m].row_tok, (const T*)h->w[m].embed, (const T*)h->w[m].attn_norm[0], h->ws[m].x, (T*)h->ws[m].act, H, c.rms_eps};
+    KL(h, TANDEM_KC_EMBED, s, launch_ex(embed_norm_kernel<T, 256>, dim3(row_grid, 2), dim3(256), 0, s, false, ea));
+  }
   for (int l = 0; l < c.n_layers; ++l) {
-    T* kpool = (T*)ws.kv + (size_t)l * layer_kv;
-    T* vpool = kpool + half_kv;
     // S3 QKV projection
-    if ((rc = launch_gemm<T>(h, m, 0, l, ws.act, w.wqkv[l], qkv_n, H, ws.gemm_out, tb.counts + C_ROWS, h->row_cap, &ns, &ss, s))) return rc;
+    for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].act, h->w[m].wqkv[l], h->ws[m].gemm_out, h->tab[m].counts + C_ROWS);
+    if ((rc = launch_gemm<T>(h, 0, A, W, qkv_n, H, O, RP, h->row_cap, &ns, &ss, s))) return rc;
     // S4 RoPE + KV append
-    const bool mma = h->attn_impl == TANDEM_ATTN_MMA;
-    if (mma) KL(h, TANDEM_KC_ROPE_APPEND, s, launch_ex(rope_append_kernel<T, bf16, 256>, dim3(row_grid), dim3(256), 0, s, h->use_pdl, tb.counts, tb.row_pos, tb.row_kvslot, ws.gemm_out, ns, ss, h->rope_cs, (bf16*)ws.q, kpool, vpool, nq, nkv, d));
-    else KL(h, TANDEM_KC_ROPE_APPEND, s, launch_ex(rope_append_kernel<T, float, 256>, dim3(row_grid), dim3(256), 0, s, h->use_pdl, tb.counts, tb.row_pos, tb.row_kvslot, ws.gemm_out, ns, ss, h->rope_cs, (float*)ws.q, kpool, vpool, nq, nkv, d));
+    if (mma) {
+      Pair<RopeArgs<T, bf16>> ra;
+      for (int m = 0; m < 2; ++m) {
+        T* kpool = (T*)h->ws[m].kv + (size_t)l * layer_kv;
+        ra.m[m] = RopeArgs<T, bf16>{h->tab[m].counts, h->tab[m].row_pos, h->tab[m].row_kvslot, h->ws[m].gemm_out, ns, ss, h->rope_cs, (bf16*)h->ws[m].q, kpool, kpool + half_kv, nq, nkv, d};
+      }
+      KL(h, TANDEM_KC_ROPE_APPEND, s, launch_ex(rope_append_kernel<T, bf16, 256>, dim3(row_grid, 2), dim3(256), 0, s, pdl, ra));
+    } else {
+      Pair<RopeArgs<T, float>> ra;
+      for (int m = 0; m < 2; ++m) {
+        T* kpool = (T*)h->ws[m].kv + (size_t)l * layer_kv;
+        ra.m[m] = RopeArgs<T, float>{h->tab[m].counts, h->tab[m].row_pos, h->tab[m].row_kvslot, h->ws[m].gemm_out, ns, ss, h->rope_cs, (float*)h->ws[m].q, kpool, kpool + half_kv, nq, nkv, d};
+      }
+      KL(h, TANDEM_KC_ROPE_APPEND, s, launch_ex(rope_append_kernel<T, float, 256>, dim3(row_grid, 2), dim3(256), 0, s, pdl, ra));
+    }
     // S5 attention (decode splits + catch-up rows), then combine
     bool ok = true;
     if (mma) {
       const long long rows_per_half = (long long)h->pool_pages * nkv * kPageTokens;
-      AttnMmaArgs ma{tb.counts, tb.item_row0, tb.item_ntok, tb.item_kv0, tb.item_kv1, tb.item_part, tb.row_slot, tb.row_pos, h->pt[m].bt, h->max_pages,
-                     (const bf16*)ws.q, (bf16*)ws.attn_out, ws.part_acc, ws.part_ml, nq, nkv, 1.0f / sqrtf((float)d),
-                     (int)((2ll * l) * rows_per_half), (int)((2ll * l + 1) * rows_per_half), h->work_ctr + m * c.n_layers + l};
-      KL(h, TANDEM_KC_ATTENTION, s, ok = run_attn_mma(*h->kv_map[m], ma, d, nq / nkv, h->attn_ctas_per_sm * h->n_sms, s, false, h->use_pdl));
+      Pair<AttnMmaArgs> ma; Pair<CUtensorMap> maps;
+      for (int m = 0; m < 2; ++m) {
+        const StepTab& tb = h->tab[m];
+        ma.m[m] = AttnMmaArgs{tb.counts, tb.item_row0, tb.item_ntok, tb.item_kv0, tb.item_kv1, tb.item_part, tb.row_slot, tb.row_pos, h->pt[m].bt, h->max_pages,
+                              (const bf16*)h->ws[m].q, (bf16*)h->ws[m].attn_out, h->ws[m].part_acc, h->ws[m].part_ml, nq, nkv, 1.0f / sqrtf((float)d),
+                              (int)((2ll * l) * rows_per_half), (int)((2ll * l + 1) * rows_per_half), h->work_ctr + l};
+        maps.m[m] = h->kv_map_store[m];
+      }
+      KL(h, TANDEM_KC_ATTENTION, s, ok = run_attn_mma(maps, ma, d, nq / nkv, h->attn_ctas_per_sm * h->n_sms, s, false, pdl));
     } else {
-      AttnArgs<T> aa{tb.counts, tb.item_row0, tb.item_ntok, tb.item_kv0, tb.item_kv1, tb.item_part, tb.row_slot, tb.row_pos, h->pt[m].bt, h->max_pages, (const float*)ws.q, kpool, vpool,
-                     (T*)ws.attn_out, ws.part_acc, ws.part_ml, nq, nkv, 1.0f / sqrtf((float)d)};
-      KL(h, TANDEM_KC_ATTENTION, s, ok = AttnDispatch<T>::run(aa, d, nq / nkv, 148 * 4, s, h->use_pdl));
+      Pair<AttnArgs<T>> aa;
+      for (int m = 0; m < 2; ++m) {
+        const StepTab& tb = h->tab[m];
+        T* kpool = (T*)h->ws[m].kv + (size_t)l * layer_kv;
+        aa.m[m] = AttnArgs<T>{tb.counts, tb.item_row0, tb.item_ntok, tb.item_kv0, tb.item_kv1, tb.item_part, tb.row_slot, tb.row_pos, h->pt[m].bt, h->max_pages,
+                              (const float*)h->ws[m].q, kpool, kpool + half_kv, (T*)h->ws[m].attn_out, h->ws[m].part_acc, h->ws[m].part_ml, nq, nkv, 1.0f / sqrtf((float)d)};
+      }
+      KL(h, TANDEM_KC_ATTENTION, s, ok = AttnDispatch<T>::run(aa, d, nq / nkv, 148 * 2, s, pdl));
     }
     if (!ok) return fail(h, TANDEM_EINVAL, "unsupported (head_dim, group) for attention");
-    CombineArgs<T> ca{tb.counts, tb.comb_row, tb.comb_part0, tb.comb_n, tb.comb_stride, ws.part_acc, ws.part_ml, (T*)ws.attn_out, nq, d};
-    KL(h, TANDEM_KC_ATTN_COMBINE, s, launch_ex(attn_combine_kernel<T>, dim3(148), dim3(256), 0, s, h->use_pdl, ca));
+    {
+      Pair<CombineArgs<T>> ca;
+      for (int m = 0; m < 2; ++m) {
+        const StepTab& tb = h->tab[m];
+        ca.m[m] = CombineArgs<T>{tb.counts, tb.comb_row, tb.comb_part0, tb.comb_n, tb.comb_stride, h->ws[m].part_acc, h->ws[m].part_ml, (T*)h->ws[m].attn_out, nq, d};
+      }
+      KL(h, TANDEM_KC_ATTN_COMBINE, s, launch_ex(attn_combine_kernel<T>, dim3(148, 2), dim3(256), 0, s, pdl, ca));
+    }
     // S6 O projection + residual + RMSNorm(mlp)
-    if ((rc = launch_gemm<T>(h, m, 1, l, ws.attn_out, w.wo[l], H, nq * d, ws.gemm_out, tb.counts + C_ROWS, h->row_cap, &ns, &ss, s))) return rc;
-    launch_residual_norm<T>(h, s, row_grid, tb.counts, ws.gemm_out, ns, ss, ws.x, (const T*)w.mlp_norm[l], (T*)ws.act, nullptr, H, c.rms_eps);
+    for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].attn_out, h->w[m].wo[l], h->ws[m].gemm_out, h->tab[m].counts + C_ROWS);
+    if ((rc = launch_gemm<T>(h, 1, A, W, H, nq * d, O, RP, h->row_cap, &ns, &ss, s))) return rc;
+    {
+      Pair<ResNormArgs<T>> na;
+      for (int m = 0; m < 2; ++m) na.m[m] = ResNormArgs<T>{h->tab[m].counts, h->ws[m].gemm_out, ns, ss, h->ws[m].x, (const T*)h->w[m].mlp_norm[l], (T*)h->ws[m].act, nullptr, H, c.rms_eps};
+      launch_residual_norm<T>(h, s, row_grid, na);
+    }
     // S7 gate/up + SwiGLU, down + residual + RMSNorm(next layer | final)
     if (h->gemm_impl == TANDEM_GEMM_TCGEN05) {   // SwiGLU in the GEMM epilogue (gate/up rows interleaved at load time)
-      if ((rc = launch_gemm<T>(h, m, 2, l, ws.act, w.wgu[l], 2 * I, H, (float*)ws.mlp_act, tb.counts + C_ROWS, h->row_cap, &ns, &ss, s, kTcEpiSwiGLU))) return rc;
+      for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].act, h->w[m].wgu[l], (float*)h->ws[m].mlp_act, h->tab[m].counts + C_ROWS);
+      if ((rc = launch_gemm<T>(h, 2, A, W, 2 * I, H, O, RP, h->row_cap, &ns, &ss, s, kTcEpiSwiGLU))) return rc;
     } else {
-      if ((rc = launch_gemm<T>(h, m, 2, l, ws.act, w.wgu[l], 2 * I, H, ws.gemm_out, tb.counts + C_ROWS, h->row_cap, &ns, &ss, s))) return rc;
-      KL(h, TANDEM_KC_SWIGLU, s, launch_ex(swiglu_kernel<T, 256>, dim3(row_grid), dim3(256), 0, s, h->use_pdl, tb.counts, ws.gemm_out, ns, ss, (T*)ws.mlp_act, I));
+      for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].act, h->w[m].wgu[l], h->ws[m].gemm_out, h->tab[m].counts + C_ROWS);
+      if ((rc = launch_gemm<T>(h, 2, A, W, 2 * I, H, O, RP, h->row_cap, &ns, &ss, s))) return rc;
+      Pair<SwigluArgs<T>> sg;
+      for (int m = 0; m < 2; ++m) sg.m[m] = SwigluArgs<T>{h->tab[m].counts, h->ws[m].gemm_out, ns, ss, (T*)h->ws[m].mlp_act, I};
+      KL(h, TANDEM_KC_SWIGLU, s, launch_ex(swiglu_kernel<T, 256>, dim3(row_grid, 2), dim3(256), 0, s, pdl, sg));
     }
-    if ((rc = launch_gemm<T>(h, m, 3, l, ws.mlp_act, w.wdown[l], H, I, ws.gemm_out, tb.counts + C_ROWS, h->row_cap, &ns, &ss, s))) return rc;
+    for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].mlp_act, h->w[m].wdown[l], h->ws[m].gemm_out, h->tab[m].counts + C_ROWS);
+    if ((rc = launch_gemm<T>(h, 3, A, W, H, I, O, RP, h->row_cap, &ns, &ss, s))) return rc;
     const bool last = l == c.n_layers - 1;
-    launch_residual_norm<T>(h, s, row_grid, tb.counts, ws.gemm_out, ns, ss, ws.x, (const T*)(last ? w.final_norm : w.attn_norm[l + 1]),
-                            (T*)(last ? ws.lm_in : ws.act), last ? tb.row_emit : nullptr, H, c.rms_eps);
+    {
+      Pair<ResNormArgs<T>> na;
+      for (int m = 0; m < 2; ++m)
+        na.m[m] = ResNormArgs<T>{h->tab[m].counts, h->ws[m].gemm_out, ns, ss, h->ws[m].x, (const T*)(last ? h->w[m].final_norm : h->w[m].attn_norm[l + 1]),
+                                 (T*)(last ? h->ws[m].lm_in : h->ws[m].act), last ? h->tab[m].row_emit : nullptr, H, c.rms_eps};
+      launch_residual_norm<T>(h, s, row_grid, na);
+    }
   }
   // S8 LM head on the emitting rows only, then sample + switch + emit
-  if ((rc = launch_gemm<T>(h, m, 4, 0, ws.lm_in, w.lm_head, V, H, ws.logits, tb.counts + C_EMIT, c.max_seqs, &ns, &ss, s))) return rc;
-  SampleArgs sa{h->st, tb, io, rp, ws.logits, h->word_start_dev, h->tokens, h->out_owner, h->out_logp, V, c.max_seq_len, m};
-  KL(h, TANDEM_KC_SAMPLE, s, launch_ex(sample_switch_emit_kernel<256>, dim3(c.max_seqs), dim3(256), 0, s, h->use_pdl, sa));
+  for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].lm_in, h->w[m].lm_head, h->ws[m].logits, h->tab[m].counts + C_EMIT);
+  if ((rc = launch_gemm<T>(h, 4, A, W, V, H, O, RP, c.max_seqs, &ns, &ss, s))) return rc;
+  Pair<SampleArgs> sa;
+  for (int m = 0; m < 2; ++m) sa.m[m] = SampleArgs{h->st, h->tab[m], io, rp, h->ws[m].logits, h->word_start_dev, h->tokens, h->out_owner, h->out_logp, V, c.max_seq_len, m};
+  KL(h, TANDEM_KC_SAMPLE, s, launch_ex(sample_switch_emit_kernel<256>, dim3(c.max_seqs, 2), dim3(256), 0, s, pdl, sa));
   return TANDEM_OK;
 }
 
@@ -274,25 +328,10 @@ int launch_step(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaSt
   sa.st = h->st; sa.pt[0] = h->pt[0]; sa.pt[1] = h->pt[1]; sa.tab[0] = h->tab[0]; sa.tab[1] = h->tab[1];
   sa.io = io; sa.stats = h->stats; sa.tokens = h->tokens; sa.max_seqs = c.max_seqs; sa.max_seq_len = c.max_seq_len;
   sa.max_pages = h->max_pages; sa.row_cap = h->row_cap; sa.tile_tok = h->tile_tok;
-  sa.work_ctr = h->work_ctr; sa.n_work_ctr = 2 * c.n_layers;
+  sa.work_ctr = h->work_ctr; sa.n_work_ctr = c.n_layers;
   KL(h, TANDEM_KC_SCHED, s, (sched_kernel<<<1, 1024, 0, s>>>(sa)));
-  if (h->profile) {   // one stream, one kernel at a time: each kernel's duration is its own
-    for (int m = 0; m < 2; ++m) {
-      const int rc = (c.dtype == TANDEM_F32) ? model_forward<float>(h, m, io, rp, s) : model_forward<bf16>(h, m, io, rp, s);
-      if (rc) return rc;
-    }
-    FinalArgs fa{h->st, {h->pt[0], h->pt[1]}, io, h->stats, h->n_active, c.max_seqs, h->max_pages, h->pool_pages};
-    KL(h, TANDEM_KC_FINALIZE, s, (finalize_kernel<<<1, 1024, 0, s>>>(fa)));
-    return TANDEM_OK;
-  }
-  CU(h, cudaEventRecord(h->ev_fork, s));
-  for (int m = 0; m < 2; ++m) {
-    CU(h, cudaStreamWaitEvent(h->ms[m], h->ev_fork, 0));
-    const int rc = (c.dtype == TANDEM_F32) ? model_forward<float>(h, m, io, rp, h->ms[m]) : model_forward<bf16>(h, m, io, rp, h->ms[m]);
-    if (rc) return rc;
-    CU(h, cudaEventRecord(h->ev_join[m], h->ms[m]));
-    CU(h, cudaStreamWaitEvent(s, h->ev_join[m], 0));
-  }
+  const int rc = (c.dtype == TANDEM_F32) ? forward_pair<float>(h, io, rp, s) : forward_pair<bf16>(h, io, rp, s);
+  if (rc) return rc;
   FinalArgs fa{h->st, {h->pt[0], h->pt[1]}, io, h->stats, h->n_active, c.max_seqs, h->max_pages, h->pool_pages};
   KL(h, TANDEM_KC_FINALIZE, s, (finalize_kernel<<<1, 1024, 0, s>>>(fa)));
   return TANDEM_OK;
@@ -624,8 +663,8 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
       h->kv_map_store[m] = *mp;
       h->kv_map[m] = &h->kv_map_store[m];
     }
-    AttnMmaArgs dummy{};
-    if (!run_attn_mma(h->kv_map_store[0], dummy, d, nq / nkv, 1, 0, true)) {
+    Pair<AttnMmaArgs> dummy{}; Pair<CUtensorMap> dmaps{};
+    if (!run_attn_mma(dmaps, dummy, d, nq / nkv, 1, 0, true)) {
       cudaGetLastError();
       h->err = "tensor-core attention: unsupported (head_dim, group) or shared-memory limit"; fprintf(stderr, "tandem_init: %s\n", h->err.c_str());
       tandem_free(h); return TANDEM_EINVAL;
@@ -882,8 +921,13 @@ int tandem_test_gemm(int32_t dtype, int32_t impl, int32_t rows, int32_t N, int32
     return tc_gemm_test(rows, N, K, A_dev, W_dev, out_dev, impl == 3 ? kTcEpiSwiGLU : kTcEpiPartial);
   }
   dim3 grid((N + kSimtTile - 1) / kSimtTile, std::max(1, std::min((rows + kSimtTile - 1) / kSimtTile, 64)));
-  if (dtype == TANDEM_F32) gemm_simt_kernel<float><<<grid, 256>>>(nullptr, rows, (const float*)A_dev, (const float*)W_dev, out_dev, N, K);
-  else gemm_simt_kernel<bf16><<<grid, 256>>>(nullptr, rows, (const bf16*)A_dev, (const bf16*)W_dev, out_dev, N, K);
+  if (dtype == TANDEM_F32) {
+    Pair<SimtGemmArgs<float>> g; g.m[0] = g.m[1] = SimtGemmArgs<float>{nullptr, rows, (const float*)A_dev, (const float*)W_dev, out_dev, N, K};
+    gemm_simt_kernel<float><<<grid, 256>>>(g);
+  } else {
+    Pair<SimtGemmArgs<bf16>> g; g.m[0] = g.m[1] = SimtGemmArgs<bf16>{nullptr, rows, (const bf16*)A_dev, (const bf16*)W_dev, out_dev, N, K};
+    gemm_simt_kernel<bf16><<<grid, 256>>>(g);
+  }
   return cudaDeviceSynchronize() == cudaSuccess ? TANDEM_OK : TANDEM_ECUDA;
 }
 
