@@ -10,7 +10,7 @@ namespace tandem {
 
 constexpr int kPageTokens = 16;      // KV page size (BASELINE.json configs[2]: "paged KV with 16-token blocks")
 constexpr int kAttnMinChunk = 256;   // smallest KV split of an attention item
-constexpr int kAttnMaxSplits = 8;    // an item is split along KV into at most this many chunks
+constexpr int kAttnMaxSplits = 4;    // an item is split along KV into at most this many chunks
 constexpr int kAttnTileRows = 64;    // (query token, q-head of the group) rows per attention item = 4 MMA m-tiles
 constexpr int kAttnSplitTiles = 4;   // sequences with at most this many q-tiles this step are also split along KV
 // KV positions per split for a context of kv_len positions: a function of kv_len only, so the reduction order of a row
