@@ -129,6 +129,18 @@ def build_inputs(wl, fast_forward, rank):
     return prompts, table, seq_ids
 
 
+def reduce_over_ranks(dist, seconds_or_ms, tokens, device):
+    """Whole-job aggregation of one timed region: (max over ranks of the time, sum over ranks of the units). Works on any
+    backend (nccl on the GPUs, gloo in the CPU test); without a process group it is the identity."""
+    if dist is None:
+        return float(seconds_or_ms), float(tokens)
+    import torch
+    t = torch.tensor([float(seconds_or_ms), float(tokens)], dtype=torch.float64, device=device)
+    tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
+    return float(tmax[0]), float(tsum[1])
+
+
 def weight_bytes_per_model(shape):
     return shape.params_read_per_step * (4 if shape.dtype == "f32" else 2)
 
@@ -257,13 +269,7 @@ def run_ours(args):
     d = {k: s1[k] - s0[k] for k in ("steps", "tokens_emitted", "rows_senior", "rows_junior", "catchup_rows", "kv_bytes_read",
                                     "weight_bytes_read", "kernel_launches")}
     tokens = d["tokens_emitted"]
-    if dist:
-        t = torch.tensor([ms, float(tokens)], dtype=torch.float64, device="cuda")
-        tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
-        ms_all, tokens_all = float(tmax[0]), float(tsum[1])
-    else:
-        ms_all, tokens_all = ms, float(tokens)
+    ms_all, tokens_all = reduce_over_ranks(dist, ms, tokens, "cuda")
     pk = peaks()
     step_bytes = (d["weight_bytes_read"] + d["kv_bytes_read"]) / max(1, K)
     step_gbs = step_bytes / (ms / K * 1e-3) / 1e9
@@ -329,12 +335,7 @@ def run_ours(args):
             g = eng.generate(prm, e_prompts, [new] * B, seq_ids=seq_ids, stream=stream)
             torch.cuda.synchronize()
             dt = time.perf_counter() - t0
-        tok = float(g["len"].sum())
-        if dist:
-            t = torch.tensor([dt, tok], dtype=torch.float64, device="cuda")
-            tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-            tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
-            dt, tok = float(tmax[0]), float(tsum[1])
+        dt, tok = reduce_over_ranks(dist, dt, float(g["len"].sum()), "cuda")
         steps_e = max(1, g["stats"]["steps"])
         h2d = e_rows * 4 + (B + 1) * 8 + 3 * B * 4 + shape.vocab
         d2h = B * new * (4 + 1 + 4) + B * 4
