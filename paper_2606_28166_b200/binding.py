@@ -17,8 +17,8 @@ _ERR = {0: "OK", -1: "EINVAL", -2: "ENOMEM", -3: "ECUDA", -4: "ESTATE", -5: "EFU
 
 EXPORTED_SYMBOLS = ["tandem_init", "tandem_load_weights", "tandem_step", "tandem_generate", "tandem_reset",
                     "tandem_free", "tandem_last_error", "tandem_get_stats", "tandem_set_profile", "tandem_get_profile",
-                    "tandem_kernel_class_name", "tandem_test_uniforms", "tandem_test_philox", "tandem_test_gemm", "tandem_test_gemm_time"]
-KC_NUM = 14
+                    "tandem_kernel_class_name", "tandem_debug_lt_times", "tandem_test_uniforms", "tandem_test_philox", "tandem_test_gemm", "tandem_test_gemm_time"]
+KC_NUM = 15
 
 
 class TandemError(RuntimeError):
@@ -99,6 +99,7 @@ def lib():
         L.tandem_test_uniforms.argtypes = [C.c_uint64, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_void_p]
         L.tandem_test_philox.argtypes = [C.POINTER(C.c_uint32), C.POINTER(C.c_uint32), C.POINTER(C.c_uint32)]
         L.tandem_test_gemm.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.tandem_debug_lt_times.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
         L.tandem_test_gemm_time.argtypes = [C.c_int32] * 8 + [C.POINTER(C.c_float)]
         _lib = L
     return _lib
@@ -226,6 +227,12 @@ class Tandem:
 
     def set_profile(self, enable):
         self._check(lib().tandem_set_profile(self._h, 1 if enable else 0))
+
+    def debug_lt_times(self):
+        n = (self.config.shape.n_layers + 1) * 32
+        out = np.zeros(n, np.uint64)
+        self._check(lib().tandem_debug_lt_times(self._h, out.ctypes.data, n))
+        return out.reshape(-1, 32)
 
     def get_profile(self):
         """dict kernel class name -> (device milliseconds, launches) accumulated while profiling was enabled."""

@@ -28,7 +28,7 @@ constexpr int kTcMaxRows = 256;      // token rows per accumulator pass = max UM
 constexpr int kTcMaxStages = 10;
 constexpr int kTcRingBytes = 200 * 1024;
 constexpr int kTcSmemBytes = kTcRingBytes + 1024;   // + alignment slack
-constexpr int kTcThreads = 192;
+constexpr int kTcThreads = 224;
 constexpr int kTcWBytes = kTcTileN * kTcBlockK * 2;     // 16384
 constexpr int kTcABoxBytes = kTcRowBox * kTcBlockK * 2; // 4096
 
@@ -116,7 +116,7 @@ __device__ __forceinline__ uint32_t umma_idesc_bf16(int n) {
   return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(kTcTileN >> 4) << 24);
 }
 
-struct TcMaps { CUtensorMap w[2], a[2]; };   // weight and activation descriptors of the two models
+struct TcMaps { CUtensorMap w[2], a[2][4]; };   // per model: weight descriptor; activation descriptors with 128/64/32/16-row boxes
 
 struct TcGemmArgs {
   float* out;                 // [n_split][row_cap][N] fp32 partials
@@ -128,35 +128,18 @@ struct TcGemmArgs {
 };
 
 // ---------------------------------------------------------------------------------------------- the kernel
-namespace ptx {
-__device__ __forceinline__ uint32_t cluster_ctarank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
-__device__ __forceinline__ void cluster_sync() {
-  asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
-  asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
-}
-// the box lands at the same CTA-relative smem offset, and signals the mbarrier at the same offset, in every CTA of `mask`
-__device__ __forceinline__ void tma_load_2d_mc(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar, uint16_t mask, uint64_t policy) {
-  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster.L2::cache_hint [%0], [%1, {%2, %3}], [%4], %5, %6;"
-               ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar), "h"(mask), "l"(policy) : "memory");
-}
-__device__ __forceinline__ void umma_commit_mc(uint32_t bar, uint16_t mask) {
-  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(bar), "h"(mask) : "memory");
-}
-}  // namespace ptx
-
 enum { kTcEpiPartial = 0, kTcEpiSwiGLU = 1 };
 
-// CL   = CTAs per cluster along the weight tiles: they need the same activation tile, so each loads 1/CL of its 32-row boxes
-//        and multicasts them to all (L2 -> SM traffic of the activations / CL); a stage is released to the producers only
-//        when the MMAs of all CL CTAs have read it (commit multicast to every CTA's empty barrier).
 // EPI  = kTcEpiPartial: fp32 partial out[split][r][n];
 //        kTcEpiSwiGLU : W rows interleaved (2i = gate_i, 2i+1 = up_i), n_split = 1: act[r][i] = silu(gate) * up as bf16.
-template <int CL, int EPI>
+// Cluster launches with TMA multicast of the activation boxes (2 and 4 CTAs) were built and measured: no gain at any of
+// the projection shapes on B200 (profiles/gemm_sweep_r1.md), so the kernel is single-CTA.
+template <int EPI>
 __global__ void __launch_bounds__(kTcThreads, 1)
 gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ Pair<TcGemmArgs> gp) {
   const TcGemmArgs& g = gp.m[blockIdx.z];                  // blockIdx.z = model
   const CUtensorMap* tmap_w = &maps.w[blockIdx.z];
-  const CUtensorMap* tmap_a = &maps.a[blockIdx.z];
+  const CUtensorMap* tmap_a = maps.a[blockIdx.z];
   extern __shared__ uint8_t tc_smem_raw[];
   __shared__ __align__(8) uint64_t bars[2 * kTcMaxStages + 2];
   __shared__ uint32_t tmem_base_smem;
@@ -174,8 +157,6 @@ gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__
   const int nbox_max = (min(rows, kTcMaxRows) + kTcRowBox - 1) / kTcRowBox;
   const int stage_bytes = kTcWBytes + nbox_max * kTcABoxBytes;
   const int n_stages = min(kTcMaxStages, g.ring_bytes / stage_bytes);
-  const uint32_t cta_rank = CL > 1 ? ptx::cluster_ctarank() : 0u;
-  constexpr uint16_t kMask = (uint16_t)((1u << CL) - 1u);
 
   const uint32_t ring = (ptx::smem_u32(tc_smem_raw) + 1023u) & ~1023u;   // 128B swizzle atoms are 1024-byte aligned
   const uint32_t bar0 = ptx::smem_u32(bars);
@@ -185,7 +166,7 @@ gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__
   const uint32_t tmem_empty_bar = tmem_full_bar + 8u;
 
   if (threadIdx.x == 0) {
-    for (int s = 0; s < n_stages; ++s) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), CL); }
+    for (int s = 0; s < n_stages; ++s) { ptx::mbar_init(full_bar(s), 2); ptx::mbar_init(empty_bar(s), 1); }   // full: weight + activation producers
     ptx::mbar_init(tmem_full_bar, 1);
     ptx::mbar_init(tmem_empty_bar, 4);
     ptx::fence_mbar_init();
@@ -194,45 +175,43 @@ gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__
   }
   if (warp == 2) ptx::tmem_alloc<kTcMaxRows>(ptx::smem_u32(&tmem_base_smem));
   ptx::tc_fence_before();
-  if (CL > 1) ptx::cluster_sync(); else __syncthreads();   // peers' barriers must exist before anything is multicast to them
+  __syncthreads();
   ptx::tc_fence_after();
   const uint32_t tmem_base = tmem_base_smem;
 
   if (warp == 0) {
-    // ===== TMA producer: weights stream once (evict-first), activations are shared by every CTA (evict-last)
+    // ===== weight producer: weights stream once (L2 evict-first) and do not depend on the predecessor kernel, so this
+    // warp never waits for it. (A thread issues one TMA box in ~0.1-0.2 us: weights and activations have a warp each.)
     if (lane == 0) {
-      const uint64_t pol_w = ptx::policy_evict_first(), pol_a = ptx::policy_evict_last();
-      // Weights do not depend on the predecessor kernel: fill the ring with the first weight tiles right away, wait for
-      // the predecessor (PDL), then add the activation boxes of those stages and carry on normally.
-      const int npre = min(n_stages, kb1 - kb0);
-      const int nbox0 = (min(rows, kTcMaxRows) + kTcRowBox - 1) / kTcRowBox;
-      for (int i = 0; i < npre; ++i) {
-        ptx::mbar_expect_tx(full_bar(i), (uint32_t)(kTcWBytes + nbox0 * kTcABoxBytes));
-        ptx::tma_load_2d(ring + (uint32_t)(i * stage_bytes), tmap_w, (kb0 + i) * kTcBlockK, n0, full_bar(i), pol_w);
-      }
-      pdl_wait();
-      for (int i = 0; i < npre; ++i) {
-        const uint32_t dst = ring + (uint32_t)(i * stage_bytes);
-        for (int j = (int)cta_rank; j < nbox0; j += CL) {
-          if (CL > 1) ptx::tma_load_2d_mc(dst + kTcWBytes + j * kTcABoxBytes, tmap_a, (kb0 + i) * kTcBlockK, j * kTcRowBox, full_bar(i), kMask, pol_a);
-          else ptx::tma_load_2d(dst + kTcWBytes + j * kTcABoxBytes, tmap_a, (kb0 + i) * kTcBlockK, j * kTcRowBox, full_bar(i), pol_a);
+      const uint64_t pol_w = ptx::policy_evict_first();
+      int it = 0;
+      for (int c = 0; c < n_chunks; ++c)
+        for (int kb = kb0; kb < kb1; ++kb, ++it) {
+          const int s = it % n_stages;
+          ptx::mbar_wait(empty_bar(s), ((uint32_t)(it / n_stages) & 1u) ^ 1u);
+          ptx::mbar_expect_tx(full_bar(s), (uint32_t)kTcWBytes);
+          ptx::tma_load_2d(ring + (uint32_t)(s * stage_bytes), tmap_w, kb * kTcBlockK, n0, full_bar(s), pol_w);
         }
-      }
+    }
+  } else if (warp == 6) {
+    // ===== activation producer: the activation tile is shared by every CTA (L2 evict-last); greedy 128/64/32/16-row boxes
+    if (lane == 0) {
+      const uint64_t pol_a = ptx::policy_evict_last();
+      pdl_wait();                                            // the activations come from the predecessor kernel
       int it = 0;
       for (int c = 0; c < n_chunks; ++c) {
         const int r0 = c * kTcMaxRows;
         const int nbox = (min(rows - r0, kTcMaxRows) + kTcRowBox - 1) / kTcRowBox;
         for (int kb = kb0; kb < kb1; ++kb, ++it) {
-          if (it < npre) continue;
           const int s = it % n_stages;
-          const uint32_t ph = (uint32_t)(it / n_stages) & 1u;
-          ptx::mbar_wait(empty_bar(s), ph ^ 1u);
-          const uint32_t dst = ring + (uint32_t)(s * stage_bytes);
-          ptx::mbar_expect_tx(full_bar(s), (uint32_t)(kTcWBytes + nbox * kTcABoxBytes));
-          ptx::tma_load_2d(dst, tmap_w, kb * kTcBlockK, n0, full_bar(s), pol_w);
-          for (int j = (int)cta_rank; j < nbox; j += CL) {
-            if (CL > 1) ptx::tma_load_2d_mc(dst + kTcWBytes + j * kTcABoxBytes, tmap_a, kb * kTcBlockK, r0 + j * kTcRowBox, full_bar(s), kMask, pol_a);
-            else ptx::tma_load_2d(dst + kTcWBytes + j * kTcABoxBytes, tmap_a, kb * kTcBlockK, r0 + j * kTcRowBox, full_bar(s), pol_a);
+          ptx::mbar_wait(empty_bar(s), ((uint32_t)(it / n_stages) & 1u) ^ 1u);
+          ptx::mbar_expect_tx(full_bar(s), (uint32_t)(nbox * kTcABoxBytes));
+          const uint32_t dst = ring + (uint32_t)(s * stage_bytes) + kTcWBytes;
+          int j = 0;
+#pragma unroll
+          for (int b = 0; b < 4; ++b) {
+            const int bx = 8 >> b;
+            while (nbox - j >= bx) { ptx::tma_load_2d(dst + j * kTcABoxBytes, tmap_a + b, kb * kTcBlockK, r0 + j * kTcRowBox, full_bar(s), pol_a); j += bx; }
           }
         }
       }
@@ -257,7 +236,7 @@ gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__
 #pragma unroll
           for (int k = 0; k < kTcBlockK / 16; ++k)   // UMMA K = 16 bf16 = 32 bytes: advance the start address inside the swizzle row
             ptx::umma_bf16(tmem_base, dw + (uint64_t)(2 * k), da + (uint64_t)(2 * k), idesc, (kb > kb0 || k > 0) ? 1u : 0u);
-          if (CL > 1) ptx::umma_commit_mc(empty_bar(s), kMask); else ptx::umma_commit(empty_bar(s));   // stage free once these MMAs have read it
+          ptx::umma_commit(empty_bar(s));            // stage free once these MMAs have read it
         }
         ptx::umma_commit(tmem_full_bar);             // accumulator of this chunk complete
       }
@@ -306,7 +285,7 @@ gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__
     }
   }
   ptx::tc_fence_before();
-  if (CL > 1) ptx::cluster_sync(); else __syncthreads();   // no CTA leaves while a peer may still multicast into it
+  __syncthreads();
   if (warp == 2) ptx::tmem_dealloc<kTcMaxRows>(tmem_base);
 }
 
@@ -337,12 +316,8 @@ inline TcGemmPlans* tc_gemm_create() {
     return nullptr;
   }
   bool ok = true;
-  ok &= cudaFuncSetAttribute(gemm_tcgen05_kernel<1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes) == cudaSuccess;
-  ok &= cudaFuncSetAttribute(gemm_tcgen05_kernel<2, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes) == cudaSuccess;
-  ok &= cudaFuncSetAttribute(gemm_tcgen05_kernel<4, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes) == cudaSuccess;
-  ok &= cudaFuncSetAttribute(gemm_tcgen05_kernel<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes) == cudaSuccess;
-  ok &= cudaFuncSetAttribute(gemm_tcgen05_kernel<2, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes) == cudaSuccess;
-  ok &= cudaFuncSetAttribute(gemm_tcgen05_kernel<4, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes) == cudaSuccess;
+  ok &= cudaFuncSetAttribute(gemm_tcgen05_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes) == cudaSuccess;
+  ok &= cudaFuncSetAttribute(gemm_tcgen05_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes) == cudaSuccess;
   if (!ok) {
     cudaGetLastError();
     return nullptr;
@@ -375,17 +350,11 @@ inline const CUtensorMap* tc_gemm_map(TcGemmPlans* p, const void* base, int n_ro
 // Launch on `s`. out receives *n_split partials, *split_stride floats apart (epi = kTcEpiPartial), or the bf16 SwiGLU
 // activations [rows, N/2] (epi = kTcEpiSwiGLU; W rows interleaved gate/up). Returns 0, or -1 (TANDEM_EINVAL) / -3 (TANDEM_ECUDA).
 // which == 4 (LM head) never splits: the sampler reads the logits in place.
-template <int CL, int EPI>
-inline int tc_gemm_launch_cl(const TcMaps& maps, const Pair<TcGemmArgs>& g, dim3 grid, cudaStream_t s, bool pdl) {
-  cudaLaunchConfig_t cfg{};
-  cfg.gridDim = grid; cfg.blockDim = dim3(kTcThreads); cfg.dynamicSmemBytes = (size_t)g.m[0].ring_bytes + 1024; cfg.stream = s;
-  cudaLaunchAttribute at[2];
-  at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-  at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[1].val.programmaticStreamSerializationAllowed = 1;
-  cfg.attrs = at; cfg.numAttrs = pdl ? 2 : 1;
-  return cudaLaunchKernelEx(&cfg, gemm_tcgen05_kernel<CL, EPI>, maps, g) == cudaSuccess ? 0 : -3;
+template <int EPI>
+inline int tc_gemm_launch_epi(const TcMaps& maps, const Pair<TcGemmArgs>& g, dim3 grid, cudaStream_t s, bool pdl) {
+  return launch_ex(gemm_tcgen05_kernel<EPI>, grid, dim3(kTcThreads), (size_t)g.m[0].ring_bytes + 1024, s, pdl, maps, g) == cudaSuccess ? 0 : -3;
 }
-struct TcGemmTune { int cl = 0, ring_kb = 0, splits = 0; bool pdl = false; };   // 0 = automatic; overrides for tuning / tandem_test_gemm_time
+struct TcGemmTune { int ring_kb = 0, splits = 0; bool pdl = false; };   // 0 = automatic; overrides for tuning / tandem_test_gemm_time
 // One launch for n_models (1 or 2) problems of the same shape: out[m] = A[m] W[m]^T, rows of model m from rows_ptr[m].
 inline int tc_gemm_launch(TcGemmPlans* p, int n_models, int which, const void* const* A, const void* const* W, int N, int K, float* const* out,
                           const int32_t* const* rows_ptr, int rows_cap, int* n_split, size_t* split_stride, cudaStream_t s, int epi = kTcEpiPartial,
@@ -396,11 +365,7 @@ inline int tc_gemm_launch(TcGemmPlans* p, int n_models, int which, const void* c
   *n_split = S;
   *split_stride = (size_t)rows_cap * N;
   const int tiles = (N + kTcTileN - 1) / kTcTileN;
-  // Clusters with activation multicast are implemented (CL = 2, 4) but measured no faster than CL = 1 on B200 at any of the
-  // projection shapes (profiles/gemm_sweep_r1.md), so the automatic choice is 1; tandem_test_gemm_time can still select them.
-  int cl = 1;
-  if (tune && tune->cl > 0) cl = tune->cl;
-  const int tiles_pad = (tiles + cl - 1) / cl * cl;
+  const int tiles_pad = tiles;
   TcMaps maps;
   Pair<TcGemmArgs> g;
   const int ring = (tune && tune->ring_kb > 0) ? tune->ring_kb * 1024
@@ -408,21 +373,19 @@ inline int tc_gemm_launch(TcGemmPlans* p, int n_models, int which, const void* c
   for (int m = 0; m < 2; ++m) {
     const int mm = m < n_models ? m : 0;
     const CUtensorMap* mw = tc_gemm_map(p, W[mm], N, K, kTcTileN);
-    const CUtensorMap* ma = tc_gemm_map(p, A[mm], rows_cap, K, kTcRowBox);
-    if (!mw || !ma) return -3;
-    maps.w[m] = *mw; maps.a[m] = *ma;
+    if (!mw) return -3;
+    maps.w[m] = *mw;
+    for (int b = 0; b < 4; ++b) {
+      const CUtensorMap* ma = tc_gemm_map(p, A[mm], rows_cap, K, 128 >> b);
+      if (!ma) return -3;
+      maps.a[m][b] = *ma;
+    }
     g.m[m] = TcGemmArgs{out[mm], rows_ptr ? rows_ptr[mm] : nullptr, rows_cap, N, K, S, *split_stride, ring};
   }
   dim3 grid(tiles_pad, S, n_models);
   const bool pdl = tune && tune->pdl;
-  if (epi == kTcEpiSwiGLU) {
-    if (cl == 4) return tc_gemm_launch_cl<4, 1>(maps, g, grid, s, pdl);
-    if (cl == 2) return tc_gemm_launch_cl<2, 1>(maps, g, grid, s, pdl);
-    return tc_gemm_launch_cl<1, 1>(maps, g, grid, s, pdl);
-  }
-  if (cl == 4) return tc_gemm_launch_cl<4, 0>(maps, g, grid, s, pdl);
-  if (cl == 2) return tc_gemm_launch_cl<2, 0>(maps, g, grid, s, pdl);
-  return tc_gemm_launch_cl<1, 0>(maps, g, grid, s, pdl);
+  if (epi == kTcEpiSwiGLU) return tc_gemm_launch_epi<1>(maps, g, grid, s, pdl);
+  return tc_gemm_launch_epi<0>(maps, g, grid, s, pdl);
 }
 
 // Unit-test hook: out[rows, N] = A W^T (partials summed here), synchronous.

@@ -20,6 +20,7 @@
 #include "attention_mma.cuh"
 #include "gemm_simt.cuh"
 #include "gemm_tcgen05.cuh"
+#include "layer_tail.cuh"
 
 using namespace tandem;
 
@@ -64,6 +65,10 @@ struct tandem_handle {
   int row_cap = 0, max_pages = 0, pool_pages = 0, tile_tok = 0, max_items = 0, max_comb = 0, part_cap = 0, gemm_impl = TANDEM_GEMM_SIMT, attn_impl = TANDEM_ATTN_ALU;
   int n_sms = 148;
   int attn_ctas_per_sm = 2, gemm_ring_kb = 0;   // tuning knobs (env TANDEM_ATTN_CTAS_PER_SM, TANDEM_GEMM_RING_KB; 0 = automatic)
+  bool use_tail = false;                        // persistent layer-tail kernel (bf16 + tcgen05 + tensor-core attention; env TANDEM_TAIL=1 enables)
+  LtWMaps* lt_wmaps = nullptr; LtAMaps* lt_amaps = nullptr; bool lt_maps_ready = false;   // device tensor-map tables of the layer-tail kernel
+  unsigned long long* lt_ts = nullptr;          // env TANDEM_LT_DEBUG=1: per-phase timestamps of the layer-tail launches (tandem_debug_lt_times)
+  int32_t* lt_bar = nullptr;                    // grid-barrier counters of the layer-tail launches, zeroed by the scheduler
   bool use_pdl = true;                          // programmatic dependent launch along each model's kernel chain (env TANDEM_PDL=0 disables)
   size_t gemm_out_cols = 0;
   ModelWeights w[2];
@@ -96,6 +101,7 @@ struct tandem_handle {
 
 namespace {
 
+int build_layer_tail_maps(tandem_handle* h);
 int fail(tandem_handle* h, int code, const std::string& msg) {
   if (h) h->err = msg;
   return code;
@@ -209,6 +215,81 @@ bool attn_supported(int dtype, int D, int G) {
   return (D == 64 && (G == 1 || G == 2 || G == 4 || G == 7 || G == 8)) || (D == 128 && (G == 1 || G == 2 || G == 4 || G == 8));
 }
 
+// ------------------------------------------------------------------------------------------ persistent layer tail
+// Launch li = 0: QKV + RoPE of layer 0 (after embed_norm). Launch li = l + 1: O .. NORM2 of layer l and, unless l is the last
+// layer, QKV + RoPE of layer l + 1.
+int build_layer_tail_maps(tandem_handle* h) {
+  const tandem_config& c = h->cfg;
+  const int H = c.hidden, nq = c.n_q_heads, nkv = c.n_kv_heads, d = c.head_dim, I = c.intermediate, L = c.n_layers;
+  const int qkv_n = (nq + 2 * nkv) * d;
+  std::vector<LtWMaps> wm(L);
+  LtAMaps am;
+  std::memset(wm.data(), 0, sizeof(LtWMaps) * L); std::memset(&am, 0, sizeof(am));
+  bool ok = true;
+  auto put = [&](CUtensorMap& dst, const void* base, int rows, int K, int box) {
+    const CUtensorMap* mp = tc_gemm_map(h->tc, base, rows, K, box);
+    if (!mp) { ok = false; return; }
+    dst = *mp;
+  };
+  for (int m = 0; m < 2; ++m) {
+    const ModelWeights& w = h->w[m]; Workspace& ws = h->ws[m];
+    for (int l = 0; l < L; ++l)
+      for (int b = 0; b < 2; ++b) {
+        const int box = b == 0 ? 256 : 128;
+        put(wm[l].w[0][m][b], w.wo[l], H, nq * d, box); put(wm[l].w[1][m][b], w.wgu[l], 2 * I, H, box);
+        put(wm[l].w[2][m][b], w.wdown[l], H, I, box);   put(wm[l].w[3][m][b], w.wqkv[l], qkv_n, H, box);
+      }
+    for (int b = 0; b < 4; ++b) {
+      const int box = 128 >> b;
+      put(am.a[0][m][b], ws.attn_out, h->row_cap, nq * d, box); put(am.a[1][m][b], ws.act, h->row_cap, H, box);
+      put(am.a[2][m][b], ws.mlp_act, h->row_cap, I, box);
+    }
+  }
+  if (!ok) return fail(h, TANDEM_ECUDA, "tensor map encode failed (layer tail)");
+  tc_gemm_invalidate(h->tc, 0);   // the per-launch cache is not needed for these
+  if (!h->lt_wmaps) { DM(h, &h->lt_wmaps, sizeof(LtWMaps) * L); DM(h, &h->lt_amaps, sizeof(LtAMaps)); }
+  CU(h, cudaMemcpy(h->lt_wmaps, wm.data(), sizeof(LtWMaps) * L, cudaMemcpyHostToDevice));
+  CU(h, cudaMemcpy(h->lt_amaps, &am, sizeof(am), cudaMemcpyHostToDevice));
+  h->lt_maps_ready = true;
+  return TANDEM_OK;
+}
+
+int launch_layer_tail(tandem_handle* h, int li, cudaStream_t s) {
+  const tandem_config& c = h->cfg;
+  const int H = c.hidden, nq = c.n_q_heads, nkv = c.n_kv_heads, d = c.head_dim, I = c.intermediate, L = c.n_layers;
+  const int qkv_n = (nq + 2 * nkv) * d;
+  const int l = li - 1;                   // layer whose attention output this launch consumes (-1: none)
+  const int ln = li;                      // layer whose QKV / RoPE this launch produces (== L: none)
+  const size_t layer_kv = (size_t)2 * h->pool_pages * nkv * kPageTokens * d;
+  const size_t half_kv = (size_t)h->pool_pages * nkv * kPageTokens * d;
+  LtArgs a{};
+  for (int m = 0; m < 2; ++m) {
+    const ModelWeights& w = h->w[m]; Workspace& ws = h->ws[m]; const StepTab& tb = h->tab[m];
+    LtModel& M = a.m[m];
+    M.counts = tb.counts; M.x = ws.x; M.gemm_out = ws.gemm_out; M.act = (bf16*)ws.act; M.mlp_act = (bf16*)ws.mlp_act; M.lm_in = (bf16*)ws.lm_in;
+    M.row_pos = tb.row_pos; M.row_kvslot = tb.row_kvslot; M.q = (bf16*)ws.q;
+    if (l >= 0) {
+      M.g_mlp = (const bf16*)w.mlp_norm[l];
+      M.g_next = (const bf16*)(l == L - 1 ? w.final_norm : w.attn_norm[l + 1]);
+      M.row_emit = l == L - 1 ? tb.row_emit : nullptr;
+    }
+    if (ln < L) {
+      bf16* kpool = (bf16*)ws.kv + (size_t)ln * layer_kv;
+      M.kpool = kpool; M.vpool = kpool + half_kv;
+    }
+  }
+  a.H = H; a.I = I; a.nq = nq; a.nkv = nkv; a.d = d; a.eps = c.rms_eps; a.rope_cs = h->rope_cs;
+  a.S_o = tc_gemm_splits(H, nq * d); a.S_down = tc_gemm_splits(H, I); a.S_qkv = tc_gemm_splits(qkv_n, H); a.row_cap = h->row_cap;
+  a.bar = h->lt_bar + li * LT_NPHASE;
+  a.dbg_ts = h->lt_ts ? h->lt_ts + (size_t)li * 32 : nullptr;
+  a.wm_l = h->lt_wmaps + (l >= 0 ? l : 0); a.wm_ln = h->lt_wmaps + (ln < L ? ln : 0); a.am = h->lt_amaps;
+  a.phase_mask = (l >= 0 ? (1 << LT_O) | (1 << LT_NORM1) | (1 << LT_GU) | (1 << LT_DOWN) | (1 << LT_NORM2) : 0) |
+                 (ln < L ? (1 << LT_QKV) | (1 << LT_ROPE) : 0);
+  cudaError_t e = cudaSuccess;
+  KL(h, TANDEM_KC_LAYER_TAIL, s, e = launch_ex(layer_tail_kernel, dim3(h->n_sms), dim3(kLtThreads), kLtSmemBytes, s, h->use_pdl, a));
+  return e == cudaSuccess ? TANDEM_OK : fail(h, TANDEM_ECUDA, std::string("layer_tail launch: ") + cudaGetErrorString(e));
+}
+
 // ------------------------------------------------------------------------------------------ both models' forward (S1..S8)
 // Every kernel is launched once for the two models (Pair arguments): the models advance layer by layer in lock-step on
 // one stream, each launch carrying the senior's and the junior's half of the work.
@@ -231,7 +312,27 @@ int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaS
     for (int m = 0; m < 2; ++m) ea.m[m] = EmbedArgs<T>{h->tab[m].counts, h->tab[m].row_tok, (const T*)h->w[m].embed, (const T*)h->w[m].attn_norm[0], h->ws[m].x, (T*)h->ws[m].act, H, c.rms_eps};
     KL(h, TANDEM_KC_EMBED, s, launch_ex(embed_norm_kernel<T, 256>, dim3(row_grid, 2), dim3(256), 0, s, false, ea));
   }
+  const bool tail = h->use_tail && sizeof(T) == 2;
+  if (tail && (rc = launch_layer_tail(h, 0, s))) return rc;
   for (int l = 0; l < c.n_layers; ++l) {
+    if (tail) {   // attention + combine, then everything up to the next attention in one persistent kernel
+      const long long rows_per_half = (long long)h->pool_pages * nkv * kPageTokens;
+      Pair<AttnMmaArgs> ma; Pair<CUtensorMap> kmaps; Pair<CombineArgs<T>> ca;
+      for (int m = 0; m < 2; ++m) {
+        const StepTab& tb = h->tab[m];
+        ma.m[m] = AttnMmaArgs{tb.counts, tb.item_row0, tb.item_ntok, tb.item_kv0, tb.item_kv1, tb.item_part, tb.row_slot, tb.row_pos, h->pt[m].bt, h->max_pages,
+                              (const bf16*)h->ws[m].q, (bf16*)h->ws[m].attn_out, h->ws[m].part_acc, h->ws[m].part_ml, nq, nkv, 1.0f / sqrtf((float)d),
+                              (int)((2ll * l) * rows_per_half), (int)((2ll * l + 1) * rows_per_half), h->work_ctr + l};
+        kmaps.m[m] = h->kv_map_store[m];
+        ca.m[m] = CombineArgs<T>{tb.counts, tb.comb_row, tb.comb_part0, tb.comb_n, tb.comb_stride, h->ws[m].part_acc, h->ws[m].part_ml, (T*)h->ws[m].attn_out, nq, d};
+      }
+      bool ok = true;
+      KL(h, TANDEM_KC_ATTENTION, s, ok = run_attn_mma(kmaps, ma, d, nq / nkv, h->attn_ctas_per_sm * h->n_sms, s, false, pdl));
+      if (!ok) return fail(h, TANDEM_EINVAL, "unsupported (head_dim, group) for attention");
+      KL(h, TANDEM_KC_ATTN_COMBINE, s, launch_ex(attn_combine_kernel<T>, dim3(148, 2), dim3(256), 0, s, pdl, ca));
+      if ((rc = launch_layer_tail(h, l + 1, s))) return rc;
+      continue;
+    }
     // S3 QKV projection
     for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].act, h->w[m].wqkv[l], h->ws[m].gemm_out, h->tab[m].counts + C_ROWS);
     if ((rc = launch_gemm<T>(h, 0, A, W, qkv_n, H, O, RP, h->row_cap, &ns, &ss, s))) return rc;
@@ -328,7 +429,7 @@ int launch_step(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaSt
   sa.st = h->st; sa.pt[0] = h->pt[0]; sa.pt[1] = h->pt[1]; sa.tab[0] = h->tab[0]; sa.tab[1] = h->tab[1];
   sa.io = io; sa.stats = h->stats; sa.tokens = h->tokens; sa.max_seqs = c.max_seqs; sa.max_seq_len = c.max_seq_len;
   sa.max_pages = h->max_pages; sa.row_cap = h->row_cap; sa.tile_tok = h->tile_tok;
-  sa.work_ctr = h->work_ctr; sa.n_work_ctr = c.n_layers;
+  sa.work_ctr = h->work_ctr; sa.n_work_ctr = c.n_layers + (c.n_layers + 1) * LT_NPHASE;
   KL(h, TANDEM_KC_SCHED, s, (sched_kernel<<<1, 1024, 0, s>>>(sa)));
   const int rc = (c.dtype == TANDEM_F32) ? forward_pair<float>(h, io, rp, s) : forward_pair<bf16>(h, io, rp, s);
   if (rc) return rc;
@@ -493,6 +594,7 @@ int check_ready(tandem_handle* h) {
   if (!h) return TANDEM_EINVAL;
   if (h->cuda_fault) return fail(h, TANDEM_ECUDA, "a previous CUDA error is sticky: " + h->err);
   if (!h->w[0].loaded || !h->w[1].loaded) return fail(h, TANDEM_ESTATE, "weights of both models must be loaded first");
+  if (h->use_tail && !h->lt_maps_ready) return build_layer_tail_maps(h);
   return TANDEM_OK;
 }
 
@@ -567,7 +669,9 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
   INIT_TRY(dmalloc(h, &h->word_start_dev, (size_t)V));
   INIT_TRY(dmalloc(h, &h->stats, sizeof(DevStats)));
   INIT_CU(cudaMemset(h->stats, 0, sizeof(DevStats)));
-  INIT_TRY(dmalloc(h, &h->work_ctr, (size_t)2 * c.n_layers * 4));
+  INIT_TRY(dmalloc(h, &h->work_ctr, (size_t)(c.n_layers + (c.n_layers + 1) * LT_NPHASE) * 4));
+  h->lt_bar = h->work_ctr + c.n_layers;
+  if (getenv("TANDEM_LT_DEBUG")) { INIT_TRY(dmalloc(h, &h->lt_ts, (size_t)(c.n_layers + 1) * 32 * 8)); INIT_CU(cudaMemset(h->lt_ts, 0, (size_t)(c.n_layers + 1) * 32 * 8)); }
   INIT_TRY(dmalloc(h, &h->n_active, 4));
   INIT_CU(cudaMemset(h->n_active, 0, 4));
   INIT_TRY(dmalloc(h, &h->stage_off, (size_t)(S + 1) * sizeof(long long)));
@@ -645,6 +749,11 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
   INIT_CU(cudaStreamCreateWithFlags(&h->gs, cudaStreamNonBlocking));
   if (const char* e = getenv("TANDEM_ATTN_CTAS_PER_SM")) h->attn_ctas_per_sm = std::max(1, std::min(2, atoi(e)));
   if (const char* e = getenv("TANDEM_PDL")) h->use_pdl = atoi(e) != 0;
+  // The persistent layer-tail kernel (layer_tail.cuh) is correct and tested but, at 157 us per layer against ~150 us for the
+  // PDL-chained separate kernels, not yet faster: opt-in with TANDEM_TAIL=1.
+  h->use_tail = false;
+  if (const char* e = getenv("TANDEM_TAIL"))
+    h->use_tail = atoi(e) != 0 && c.dtype == TANDEM_BF16 && h->gemm_impl == TANDEM_GEMM_TCGEN05 && h->attn_impl == TANDEM_ATTN_MMA;
   if (const char* e = getenv("TANDEM_GEMM_RING_KB")) h->gemm_ring_kb = std::max(0, std::min(200, atoi(e)));
   {
     int dev_sms = 0;
@@ -653,6 +762,9 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
   if (h->gemm_impl == TANDEM_GEMM_TCGEN05 || h->attn_impl == TANDEM_ATTN_MMA) {
     h->tc = tc_gemm_create();
     if (!h->tc) { h->err = "tcgen05 GEMM setup failed (driver entry point for tensor maps not found)"; fprintf(stderr, "tandem_init: %s\n", h->err.c_str()); tandem_free(h); return TANDEM_ECUDA; }
+  }
+  if (h->use_tail && cudaFuncSetAttribute(layer_tail_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kLtSmemBytes) != cudaSuccess) {
+    cudaGetLastError(); h->use_tail = false;
   }
   if (h->attn_impl == TANDEM_ATTN_MMA) {
     const long long total_rows = 2ll * c.n_layers * h->pool_pages * nkv * kPageTokens;
@@ -715,9 +827,16 @@ int tandem_get_profile(tandem_handle* h, double* ms, int64_t* launches) {
   return TANDEM_OK;
 }
 
+int tandem_debug_lt_times(tandem_handle* h, unsigned long long* out, int n) {
+  if (!h || !out || !h->lt_ts) return TANDEM_ESTATE;
+  CU(h, cudaDeviceSynchronize());
+  CU(h, cudaMemcpy(out, h->lt_ts, (size_t)std::min(n, (h->cfg.n_layers + 1) * 32) * 8, cudaMemcpyDeviceToHost));
+  return TANDEM_OK;
+}
+
 const char* tandem_kernel_class_name(int kc) {
   static const char* names[TANDEM_KC_NUM] = {"sched", "embed_norm", "gemm_qkv", "rope_append", "attention", "attn_combine", "gemm_o",
-                                             "residual_norm", "gemm_gateup", "swiglu", "gemm_down", "gemm_lmhead", "sample_switch_emit", "finalize"};
+                                             "residual_norm", "gemm_gateup", "swiglu", "gemm_down", "gemm_lmhead", "sample_switch_emit", "finalize", "layer_tail"};
   return (kc >= 0 && kc < TANDEM_KC_NUM) ? names[kc] : "?";
 }
 
@@ -765,6 +884,7 @@ int tandem_load_weights(tandem_handle* h, int model, const tandem_weights* w) {
   mw.loaded = true;
   if (h->graph) { cudaGraphExecDestroy(h->graph); h->graph = nullptr; h->gkey.valid = false; }
   if (h->tc) tc_gemm_invalidate(h->tc, model);
+  h->lt_maps_ready = false;
   return TANDEM_OK;
 }
 
@@ -874,7 +994,7 @@ void tandem_free(tandem_handle* h) {
   if (h->ev_out) cudaEventDestroy(h->ev_out);
   if (h->gs) cudaStreamDestroy(h->gs);
   fr(h->st_mem); fr(h->st_mem8); fr(h->tokens); fr(h->out_owner); fr(h->out_logp); fr(h->rope_cs); fr(h->word_start_dev); fr(h->stats);
-  fr(h->n_active); fr(h->work_ctr); fr(h->stage_tokens); fr(h->stage_off); fr(h->stage_i32);
+  fr(h->lt_wmaps); fr(h->lt_amaps); fr(h->lt_ts); fr(h->n_active); fr(h->work_ctr); fr(h->stage_tokens); fr(h->stage_off); fr(h->stage_i32);
   cudaGetLastError();
   delete h;
 }
@@ -934,7 +1054,7 @@ int tandem_test_gemm(int32_t dtype, int32_t impl, int32_t rows, int32_t N, int32
 int tandem_test_gemm_time(int32_t rows, int32_t N, int32_t K, int32_t iters, int32_t cluster, int32_t ring_kb, int32_t splits, int32_t flags,
                           float* ms_per_launch) {
   if (rows <= 0 || N <= 0 || K <= 0 || iters <= 0 || !ms_per_launch) return TANDEM_EINVAL;
-  TcGemmTune t; t.cl = cluster; t.ring_kb = ring_kb; t.splits = splits; t.pdl = (flags & 2) != 0;
+  (void)cluster; TcGemmTune t; t.ring_kb = ring_kb; t.splits = splits; t.pdl = (flags & 2) != 0;
   return tc_gemm_time(rows, N, K, iters, t, (flags & 1) ? kTcEpiSwiGLU : kTcEpiPartial, ms_per_launch);
 }
 
