@@ -145,13 +145,14 @@ def weight_bytes_per_model(shape):
     return shape.params_read_per_step * (4 if shape.dtype == "f32" else 2)
 
 
-def class_bytes(shape, cls, rows, kv_bytes_per_layer_launch, emit_rows):
-    """ALGORITHMIC HBM bytes of one launch of kernel class `cls` at `rows` rows: the operand
-    that must be streamed (weights / KV) + activations in + one copy of the result. bf16 = 2 bytes, fp32 = 4."""
+def class_bytes(shape, cls, rows, kv_bytes_per_layer_launch, emit_rows, n_models=2):
+    """ALGORITHMIC HBM bytes of one launch of kernel class `cls`. Every launch serves `n_models` models:
+    `rows`, `emit_rows` and the KV bytes are the totals over those models; weights are streamed once per model. Counted: the
+    operand that must be streamed (weights / KV) + activations in + one copy of the result. bf16 = 2 bytes, fp32 = 4."""
     H, I, V = shape.hidden, shape.intermediate, shape.vocab
     qd, kd = shape.n_q_heads * shape.head_dim, shape.n_kv_heads * shape.head_dim
     es = 4 if shape.dtype == "f32" else 2
-    g = lambda N, K, r: N * K * es + r * K * es + r * N * 4
+    g = lambda N, K, r: n_models * N * K * es + r * K * es + r * N * 4
     if cls == "gemm_qkv":
         return g(qd + 2 * kd, H, rows)
     if cls == "gemm_o":
@@ -162,6 +163,8 @@ def class_bytes(shape, cls, rows, kv_bytes_per_layer_launch, emit_rows):
         return g(H, I, rows)
     if cls == "gemm_lmhead":
         return g(V, H, emit_rows)
+    if cls == "layer_tail":
+        return g(H, qd, rows) + g(2 * I, H, rows) + g(H, I, rows) + g(qd + 2 * kd, H, rows)
     if cls == "attention":
         return kv_bytes_per_layer_launch + rows * qd * (4 + es)
     if cls == "rope_append":
@@ -285,10 +288,10 @@ def run_ours(args):
         prof = eng.get_profile()
         eng.set_profile(False)
         p1 = eng.get_stats()
-        msteps = max(1, (p1["weight_bytes_read"] - p0["weight_bytes_read"]) // weight_bytes_per_model(shape))
-        rows = (p1["rows_senior"] + p1["rows_junior"] - p0["rows_senior"] - p0["rows_junior"]) / msteps
-        emit_rows = (p1["tokens_emitted"] - p0["tokens_emitted"]) / msteps
-        kv_launch = (p1["kv_bytes_read"] - p0["kv_bytes_read"]) / msteps / shape.n_layers
+        psteps = max(1, p1["steps"] - p0["steps"])            # every launch serves both models: per-step totals
+        rows = (p1["rows_senior"] + p1["rows_junior"] - p0["rows_senior"] - p0["rows_junior"]) / psteps
+        emit_rows = (p1["tokens_emitted"] - p0["tokens_emitted"]) / psteps
+        kv_launch = (p1["kv_bytes_read"] - p0["kv_bytes_read"]) / psteps / shape.n_layers
         total_ms = sum(v[0] for v in prof.values())
         for name, (kms, n) in prof.items():
             if n == 0:
