@@ -98,6 +98,14 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
       : "r"(taddr));
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+// One lane of a converged warp. The TMA / MMA warps run their loops with all 32 lanes and issue under elect_one(): the operands
+// (descriptors, addresses) are then provably warp-uniform and stay in uniform registers. Issued from a single divergent thread
+// (`if (lane == 0)`), every tcgen05.mma cost 151 cycles (R2UR moves) instead of 99 / 128 at N <= 128 / N = 256 (measured, B200).
+__device__ __forceinline__ bool elect_one() {
+  uint32_t p;
+  asm volatile("{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.u32 %0, 1, 0, P;\n\t}" : "=r"(p));
+  return p != 0;
+}
 }  // namespace ptx
 
 // Shared-memory matrix descriptor of a K-major bf16 tile whose rows are 128 bytes (64 elements) with the 128-byte
@@ -182,20 +190,23 @@ gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__
   if (warp == 0) {
     // ===== weight producer: weights stream once (L2 evict-first) and do not depend on the predecessor kernel, so this
     // warp never waits for it. (A thread issues one TMA box in ~0.1-0.2 us: weights and activations have a warp each.)
-    if (lane == 0) {
+    {
       const uint64_t pol_w = ptx::policy_evict_first();
       int it = 0;
       for (int c = 0; c < n_chunks; ++c)
         for (int kb = kb0; kb < kb1; ++kb, ++it) {
           const int s = it % n_stages;
           ptx::mbar_wait(empty_bar(s), ((uint32_t)(it / n_stages) & 1u) ^ 1u);
-          ptx::mbar_expect_tx(full_bar(s), (uint32_t)kTcWBytes);
-          ptx::tma_load_2d(ring + (uint32_t)(s * stage_bytes), tmap_w, kb * kTcBlockK, n0, full_bar(s), pol_w);
+          if (ptx::elect_one()) {
+            ptx::mbar_expect_tx(full_bar(s), (uint32_t)kTcWBytes);
+            ptx::tma_load_2d(ring + (uint32_t)(s * stage_bytes), tmap_w, kb * kTcBlockK, n0, full_bar(s), pol_w);
+          }
+          __syncwarp();
         }
     }
   } else if (warp == 6) {
     // ===== activation producer: the activation tile is shared by every CTA (L2 evict-last); greedy 128/64/32/16-row boxes
-    if (lane == 0) {
+    {
       const uint64_t pol_a = ptx::policy_evict_last();
       pdl_wait();                                            // the activations come from the predecessor kernel
       int it = 0;
@@ -205,20 +216,23 @@ gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__
         for (int kb = kb0; kb < kb1; ++kb, ++it) {
           const int s = it % n_stages;
           ptx::mbar_wait(empty_bar(s), ((uint32_t)(it / n_stages) & 1u) ^ 1u);
-          ptx::mbar_expect_tx(full_bar(s), (uint32_t)(nbox * kTcABoxBytes));
-          const uint32_t dst = ring + (uint32_t)(s * stage_bytes) + kTcWBytes;
-          int j = 0;
+          if (ptx::elect_one()) {
+            ptx::mbar_expect_tx(full_bar(s), (uint32_t)(nbox * kTcABoxBytes));
+            const uint32_t dst = ring + (uint32_t)(s * stage_bytes) + kTcWBytes;
+            int j = 0;
 #pragma unroll
-          for (int b = 0; b < 4; ++b) {
-            const int bx = 8 >> b;
-            while (nbox - j >= bx) { ptx::tma_load_2d(dst + j * kTcABoxBytes, tmap_a + b, kb * kTcBlockK, r0 + j * kTcRowBox, full_bar(s), pol_a); j += bx; }
+            for (int b = 0; b < 4; ++b) {
+              const int bx = 8 >> b;
+              while (nbox - j >= bx) { ptx::tma_load_2d(dst + j * kTcABoxBytes, tmap_a + b, kb * kTcBlockK, r0 + j * kTcRowBox, full_bar(s), pol_a); j += bx; }
+            }
           }
+          __syncwarp();
         }
       }
     }
   } else if (warp == 1) {
-    // ===== MMA issuer: one thread drives the tensor core for the whole CTA
-    if (lane == 0) {
+    // ===== MMA issuer: one elected lane drives the tensor core for the whole CTA
+    {
       int it = 0;
       for (int c = 0; c < n_chunks; ++c) {
         const int r0 = c * kTcMaxRows;
@@ -233,12 +247,16 @@ gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__
           ptx::tc_fence_after();
           const uint32_t sw = ring + (uint32_t)(s * stage_bytes);
           const uint64_t dw = umma_desc_sw128(sw), da = umma_desc_sw128(sw + kTcWBytes);
+          if (ptx::elect_one()) {
 #pragma unroll
-          for (int k = 0; k < kTcBlockK / 16; ++k)   // UMMA K = 16 bf16 = 32 bytes: advance the start address inside the swizzle row
-            ptx::umma_bf16(tmem_base, dw + (uint64_t)(2 * k), da + (uint64_t)(2 * k), idesc, (kb > kb0 || k > 0) ? 1u : 0u);
-          ptx::umma_commit(empty_bar(s));            // stage free once these MMAs have read it
+            for (int k = 0; k < kTcBlockK / 16; ++k)   // UMMA K = 16 bf16 = 32 bytes: advance the start address inside the swizzle row
+              ptx::umma_bf16(tmem_base, dw + (uint64_t)(2 * k), da + (uint64_t)(2 * k), idesc, (kb > kb0 || k > 0) ? 1u : 0u);
+            ptx::umma_commit(empty_bar(s));            // stage free once these MMAs have read it
+          }
+          __syncwarp();
         }
-        ptx::umma_commit(tmem_full_bar);             // accumulator of this chunk complete
+        if (ptx::elect_one()) ptx::umma_commit(tmem_full_bar);   // accumulator of this chunk complete
+        __syncwarp();
       }
     }
   } else {

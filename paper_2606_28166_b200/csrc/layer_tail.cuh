@@ -11,7 +11,7 @@
 // activations, and it streams the next phase's weight tiles into the shared-memory ring while the other warps finish the
 // epilogue, wait at the barrier and run the element-wise phase. Only the activation boxes of a stage wait for the barrier.
 // This removes the per-kernel fixed costs (launch, prologue, first TMA round trip, drain) that made the seven separate
-// kernels take 190 us per layer for 62 us of weight streaming (profiles/launches_r1b.md).
+// kernels take 190 us per layer for 62 us of weight streaming (profiles/launches_r1c.md).
 //   warp 0    : weight TMA producer (never waits for a grid barrier: runs ahead as far as the ring allows)
 //   warp 10   : activation TMA producer (same stage sequence, gated by the barrier of the producing phase)
 //   warp 1    : MMA issuer (tcgen05.mma, one thread)
@@ -270,7 +270,7 @@ __global__ void __launch_bounds__(kLtThreads, 1) layer_tail_kernel(const __grid_
   if (warp == 0) {
     // ===== weight producer: runs ahead of the activations across phase boundaries, bounded only by free ring slots.
     // (One thread issues a TMA box in ~0.1-0.2 us, so weights and activations are issued by different warps.)
-    if (lane == 0) {
+    {
       const uint64_t pol_w = ptx::policy_evict_first();
       LtWalker ww; ww.start(cta);
       LtUC uw;
@@ -281,14 +281,17 @@ __global__ void __launch_bounds__(kLtThreads, 1) layer_tail_kernel(const __grid_
         for (int kb = uw.kb0; kb < uw.kb1; ++kb, ++nw) {
           const int s = nw % n_stages;
           ptx::mbar_wait(empty_bar(s), ((uint32_t)(nw / n_stages) & 1u) ^ 1u);
-          ptx::mbar_expect_tx(full_bar(s), (uint32_t)(uw.box256 ? kLtW2Bytes : kTcWBytes));
-          ptx::tma_load_2d(ring + (uint32_t)(s * stage_bytes), mw, kb * kTcBlockK, uw.n0, full_bar(s), pol_w);
+          if (ptx::elect_one()) {
+            ptx::mbar_expect_tx(full_bar(s), (uint32_t)(uw.box256 ? kLtW2Bytes : kTcWBytes));
+            ptx::tma_load_2d(ring + (uint32_t)(s * stage_bytes), mw, kb * kTcBlockK, uw.n0, full_bar(s), pol_w);
+          }
+          __syncwarp();
         }
       }
     }
   } else if (warp == 10) {
     // ===== activation producer: same stage sequence, gated by the grid barrier of the phase that produces the operand
-    if (lane == 0) {
+    {
       const uint64_t pol_a = ptx::policy_evict_last();
       LtWalker wa; wa.start(cta);
       LtUC ua;
@@ -307,20 +310,23 @@ __global__ void __launch_bounds__(kLtThreads, 1) layer_tail_kernel(const __grid_
         for (int kb = ua.kb0; kb < ua.kb1; ++kb, ++na) {
           const int s = na % n_stages;
           ptx::mbar_wait(empty_bar(s), ((uint32_t)(na / n_stages) & 1u) ^ 1u);
-          ptx::mbar_expect_tx(full_bar(s), (uint32_t)(nbox * kTcABoxBytes));
-          const uint32_t dst = ring + (uint32_t)(s * stage_bytes) + kLtW2Bytes;
-          int j = 0;                                     // rows issued so far, in 16-row units: greedy 128 / 64 / 32 / 16-row boxes
+          if (ptx::elect_one()) {
+            ptx::mbar_expect_tx(full_bar(s), (uint32_t)(nbox * kTcABoxBytes));
+            const uint32_t dst = ring + (uint32_t)(s * stage_bytes) + kLtW2Bytes;
+            int j = 0;                                     // rows issued so far, in 16-row units: greedy 128 / 64 / 32 / 16-row boxes
 #pragma unroll
-          for (int b = 0; b < 4; ++b) {
-            const int bx = 8 >> b;
-            while (nbox - j >= bx) { ptx::tma_load_2d(dst + j * kTcABoxBytes, ma + b, kb * kTcBlockK, ua.r0 + j * kTcRowBox, full_bar(s), pol_a); j += bx; }
+            for (int b = 0; b < 4; ++b) {
+              const int bx = 8 >> b;
+              while (nbox - j >= bx) { ptx::tma_load_2d(dst + j * kTcABoxBytes, ma + b, kb * kTcBlockK, ua.r0 + j * kTcRowBox, full_bar(s), pol_a); j += bx; }
+            }
           }
+          __syncwarp();
         }
       }
     }
   } else if (warp == 1) {
-    // ===== MMA issuer
-    if (lane == 0) {
+    // ===== MMA issuer (all lanes run the loop, one elected lane issues: see ptx::elect_one)
+    {
       LtWalker w; w.start(cta);
       LtUC u;
       int it = 0, acc_it = 0;
@@ -337,22 +343,26 @@ __global__ void __launch_bounds__(kLtThreads, 1) layer_tail_kernel(const __grid_
           t0 = clock64();
           ptx::mbar_wait(full_bar(s), (uint32_t)(it / n_stages) & 1u);
           dbg_full += clock64() - t0;
-          if (a.dbg_ts && cta == 0 && u.phase == LT_GU && kb - u.kb0 < 8 && acc_it < 2) a.dbg_ts[20 + (kb - u.kb0)] = lt_now();
+          if (a.dbg_ts && cta == 0 && lane == 0 && u.phase == LT_GU && kb - u.kb0 < 8 && acc_it < 2) a.dbg_ts[20 + (kb - u.kb0)] = lt_now();
           ptx::tc_fence_after();
           const uint32_t sw = ring + (uint32_t)(s * stage_bytes);
           const uint64_t da = umma_desc_sw128(sw + kLtW2Bytes);
-          for (int j = 0; j < u.ntile; ++j) {
-            const uint64_t dw = umma_desc_sw128(sw + j * kTcWBytes);
+          if (ptx::elect_one()) {
+            for (int j = 0; j < u.ntile; ++j) {
+              const uint64_t dw = umma_desc_sw128(sw + j * kTcWBytes);
 #pragma unroll
-            for (int k = 0; k < kTcBlockK / 16; ++k)
-              ptx::umma_bf16(tmem_base + (uint32_t)(j * kTcMaxRows), dw + (uint64_t)(2 * k), da + (uint64_t)(2 * k), idesc, (kb > u.kb0 || k > 0) ? 1u : 0u);
+              for (int k = 0; k < kTcBlockK / 16; ++k)
+                ptx::umma_bf16(tmem_base + (uint32_t)(j * kTcMaxRows), dw + (uint64_t)(2 * k), da + (uint64_t)(2 * k), idesc, (kb > u.kb0 || k > 0) ? 1u : 0u);
+            }
+            ptx::umma_commit(empty_bar(s));
           }
-          ptx::umma_commit(empty_bar(s));
+          __syncwarp();
         }
-        ptx::umma_commit(tmem_full_bar);
+        if (ptx::elect_one()) ptx::umma_commit(tmem_full_bar);
+        __syncwarp();
         ++acc_it;
       }
-      if (a.dbg_ts && cta == 0) { a.dbg_ts[16] = (unsigned long long)dbg_full; a.dbg_ts[17] = (unsigned long long)dbg_empty; a.dbg_ts[18] = (unsigned long long)it; a.dbg_ts[19] = (unsigned long long)n_stages; }
+      if (a.dbg_ts && cta == 0 && lane == 0) { a.dbg_ts[16] = (unsigned long long)dbg_full; a.dbg_ts[17] = (unsigned long long)dbg_empty; a.dbg_ts[18] = (unsigned long long)it; a.dbg_ts[19] = (unsigned long long)n_stages; }
     }
   } else {
     // ===== epilogue warps (TMEM quarter q = warp % 4) + element-wise phases
