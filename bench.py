@@ -44,6 +44,8 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=8)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg3_4b_bf16")
+    ap.add_argument("--p", type=float, default=None, help="override the workload's switch probability (cfg5 sweep)")
+    ap.add_argument("--word-start-frac", type=float, default=None, help="override the word-start table density (cfg5 sweep)")
     ap.add_argument("--fast-forward", type=int, default=-1,
                     help="tokens already generated per sequence before the timed window (ingested as context by prefill); "
                          "-1 = half of the workload's max_new: step time is affine in the context length, so a step at the "
@@ -195,6 +197,10 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     T.build()
     wl = get_workload(args.workload)
+    if args.p is not None:
+        wl = wl.with_(p=args.p)
+    if args.word_start_frac is not None:
+        wl = wl.with_(word_start_frac=args.word_start_frac)
     shape, B = wl.shape, wl.batch
     W, K = max(3, args.warmup), args.steps
     if args.fast_forward < 0:
@@ -204,7 +210,7 @@ def run_ours(args):
     prefill_rows = sum(len(p) for p in prompts)
     row_cap = 4096
     prefill_steps = (prefill_rows + row_cap - 1) // row_cap + 2
-    gen_budget = prefill_steps + args.ramp + args.max_drain + W + K + args.profile_steps + 64
+    gen_budget = prefill_steps + max(args.ramp, int(4.0 / max(wl.p * wl.word_start_frac, 1e-3))) + args.max_drain + W + K + args.profile_steps + 64
     max_seq_len = ((max_prompt + max(gen_budget, args.e2e_new) + 15) // 16) * 16
     eng = T.Tandem(T.TandemConfig(shape, max_seqs=B, max_seq_len=max_seq_len, device=local, max_rows_per_step=row_cap, use_graph=1))
     w_cpu = []
@@ -230,7 +236,9 @@ def run_ours(args):
         if st["tokens_emitted"] >= B or n_setup > 4 * prefill_steps + 16:
             break
         eng.step(prm, out=out, stream=stream); n_setup += 1
-    for _ in range(args.ramp):
+    # every sequence should have changed hands a few times before timing: ~4 expected switches per sequence (rate p * f per token)
+    ramp = max(args.ramp, int(4.0 / (wl.p * wl.word_start_frac)) if wl.p * wl.word_start_frac > 0 else 0)
+    for _ in range(ramp):
         eng.step(prm, out=out, stream=stream)
     # keep stepping until the partner's first catch-up over the (fast-forwarded) context has drained: steady state is
     # ~2 rows per sequence per step; the budget above reserves room for these steps
@@ -319,7 +327,7 @@ def run_ours(args):
                       "ctx_mean_timed": ctx_mean, "p": wl.p, "word_start_frac": wl.word_start_frac, "temperature": wl.temperature,
                       "page_tokens": 16, "parallelism": "dp%d (independent sequences, replicated weights, no collective)" % world,
                       "l2": "inputs larger than L2 (16.1 GB of weights + KV streamed per step vs 126 MB L2)",
-                      "setup_steps": n_setup + args.ramp + n_drain, "setup_seconds": setup_s, "cuda_graph": True},
+                      "setup_steps": n_setup + ramp + n_drain, "setup_seconds": setup_s, "cuda_graph": True},
            "clocks": clk, "gpu_launches": int(d["kernel_launches"]),
            "step_roofline": {"bound": "hbm", "alg_bytes_per_step": step_bytes, "weights_bytes_per_step": d["weight_bytes_read"] / K,
                              "kv_bytes_per_step": d["kv_bytes_read"] / K, "achieved": step_gbs, "unit": "GB/s",

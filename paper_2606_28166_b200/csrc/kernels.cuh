@@ -413,12 +413,15 @@ __global__ void __launch_bounds__(NT) swiglu_kernel(const __grid_constant__ Pair
 }
 
 // ============================================================================================ S8: sample + switch + emit
-// One CTA per emitting sequence of model M. logits row j (fp32, [n_emit, V]) -> token (forced | greedy argmax |
+// n_chunk CTAs per emitting sequence of model M (slices of the vocabulary; the last to finish merges). logits row j (fp32, [n_emit, V]) -> token (forced | greedy argmax |
 // Gumbel-max on position-addressed uniforms), log-prob under softmax(z/T'), authorship flag; then the rule of
 // PAPER.md L61 / Alg. 1 lines 9-15 / L271: EOS or length => done; boundary = word_start[y]; cap counter; coin.
 struct SampleArgs {
   SeqState st; StepTab tab; StepIO io; RuleParams rp; const float* logits; const uint8_t* word_start;
   int32_t* tokens; uint8_t* out_owner; float* out_logp; int vocab, max_seq_len, model;
+  float* chunk_part;   // [max_seqs][n_chunk][6]: (max, sum, raw best value, raw best id, Gumbel best value, Gumbel best id) per vocabulary chunk
+  int32_t* chunk_ctr;  // [max_seqs] arrival counters, zero between steps (the last arriver resets its own)
+  int n_chunk;         // CTAs per row = gridDim.y
 };
 
 struct ArgBest { float v; int i; };
@@ -429,11 +432,15 @@ __device__ __forceinline__ ArgBest better(ArgBest a, ArgBest b) {  // larger val
 template <int NT>
 __global__ void __launch_bounds__(NT) sample_switch_emit_kernel(const __grid_constant__ Pair<SampleArgs> pp) {
   pdl_trigger(); pdl_wait();
-  const SampleArgs& a = pp.m[blockIdx.y];
+  const SampleArgs& a = pp.m[blockIdx.z];
   __shared__ float s_m[NT / 32], s_s[NT / 32], s_bv[NT / 32], s_gv[NT / 32];
   __shared__ int s_bi[NT / 32], s_gi[NT / 32];
   const int j = blockIdx.x;
   if (j >= a.tab.counts[C_EMIT]) return;
+  // the vocabulary is cut into n_chunk slices (multiples of 4 ids = whole Philox blocks), one CTA each
+  const int n_chunk = a.n_chunk, ch = blockIdx.y;
+  const int per = (((a.vocab + 3) / 4 + n_chunk - 1) / n_chunk) * 4;
+  const int v_lo = ch * per, v_hi = min(a.vocab, v_lo + per);
   const int s = a.tab.emit_slot[j];
   const int V = a.vocab;
   const float* z = a.logits + (size_t)j * V;
@@ -445,13 +452,13 @@ __global__ void __launch_bounds__(NT) sample_switch_emit_kernel(const __grid_con
 
   if (a.io.dbg_logits) {  // debug: the owner's logits for this position
     float* dst = a.io.dbg_logits + (size_t)s * V;
-    for (int v = threadIdx.x; v < V; v += NT) dst[v] = z[v];
+    for (int v = v_lo + threadIdx.x; v < v_hi; v += NT) dst[v] = z[v];
   }
   // one pass: running (max, sum exp) of z*invT for the log-softmax, raw argmax, Gumbel-perturbed argmax
   float m = -INFINITY, sum = 0.f;
   ArgBest raw = {-INFINITY, 0x7fffffff}, gum = {-INFINITY, 0x7fffffff};
   const uint32_t k0 = (uint32_t)a.rp.seed, k1 = (uint32_t)(a.rp.seed >> 32);
-  for (int b4 = threadIdx.x; b4 * 4 < V; b4 += NT) {
+  for (int b4 = v_lo / 4 + threadIdx.x; b4 * 4 < v_hi; b4 += NT) {
     uint32_t c[4] = {(uint32_t)b4, (uint32_t)t, (uint32_t)sid, 0u};
     if (!greedy && !u_row) philox4x32_10(c, k0, k1);
 #pragma unroll
@@ -490,6 +497,25 @@ __global__ void __launch_bounds__(NT) sample_switch_emit_kernel(const __grid_con
     m = mn;
     raw = better(raw, ArgBest{s_bv[k], s_bi[k]});
     gum = better(gum, ArgBest{s_gv[k], s_gi[k]});
+  }
+  if (n_chunk > 1) {
+    // publish this slice; the CTA that arrives last merges all slices in slice order (deterministic) and applies the rule
+    float* cp = a.chunk_part + ((size_t)j * n_chunk + ch) * 6;
+    cp[0] = m; cp[1] = sum; cp[2] = raw.v; cp[3] = __int_as_float(raw.i); cp[4] = gum.v; cp[5] = __int_as_float(gum.i);
+    __threadfence();
+    if (atomicAdd(a.chunk_ctr + j, 1) != n_chunk - 1) return;
+    a.chunk_ctr[j] = 0;
+    __threadfence();
+    m = -INFINITY; sum = 0.f; raw = ArgBest{-INFINITY, 0x7fffffff}; gum = raw;
+    for (int k = 0; k < n_chunk; ++k) {
+      const float* q = a.chunk_part + ((size_t)j * n_chunk + k) * 6;
+      const float mk = __ldcg(q), sk = __ldcg(q + 1);
+      const float mn = fmaxf(m, mk);
+      sum = (m == -INFINITY ? 0.f : sum * expf(m - mn)) + (mk == -INFINITY ? 0.f : sk * expf(mk - mn));
+      m = mn;
+      raw = better(raw, ArgBest{__ldcg(q + 2), __float_as_int(__ldcg(q + 3))});
+      gum = better(gum, ArgBest{__ldcg(q + 4), __float_as_int(__ldcg(q + 5))});
+    }
   }
   int y = greedy ? raw.i : gum.i;
   if (a.io.forced_tokens) {

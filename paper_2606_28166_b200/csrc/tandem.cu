@@ -23,6 +23,7 @@
 #include "layer_tail.cuh"
 
 using namespace tandem;
+constexpr int kSampleMaxChunks = 32;
 
 namespace {
 
@@ -41,6 +42,7 @@ struct Workspace {  // per model, sized for row_cap rows
   void* lm_in = nullptr;       // final-normed last rows [max_seqs, H]
   float* gemm_out = nullptr;   // split-K partial outputs [S][R][N], S*N <= gemm_out_cols
   float* logits = nullptr;     // [max_seqs, V]
+  float* chunk_part = nullptr; int32_t* chunk_ctr = nullptr;   // sampler: per-slice partials and arrival counters
   float* part_acc = nullptr; float2* part_ml = nullptr;
   void* kv = nullptr;          // page pool: [layer][K|V][page][nkv][16][d]
   int32_t* tab_mem = nullptr;  // backing store of the StepTab arrays
@@ -418,8 +420,11 @@ int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaS
   for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].lm_in, h->w[m].lm_head, h->ws[m].logits, h->tab[m].counts + C_EMIT);
   if ((rc = launch_gemm<T>(h, 4, A, W, V, H, O, RP, c.max_seqs, &ns, &ss, s))) return rc;
   Pair<SampleArgs> sa;
-  for (int m = 0; m < 2; ++m) sa.m[m] = SampleArgs{h->st, h->tab[m], io, rp, h->ws[m].logits, h->word_start_dev, h->tokens, h->out_owner, h->out_logp, V, c.max_seq_len, m};
-  KL(h, TANDEM_KC_SAMPLE, s, launch_ex(sample_switch_emit_kernel<256>, dim3(c.max_seqs, 2), dim3(256), 0, s, pdl, sa));
+  const int n_chunk = std::max(1, std::min(kSampleMaxChunks, V / 8192));   // ~8k ids per CTA: 18 slices at V = 151,936
+  for (int m = 0; m < 2; ++m)
+    sa.m[m] = SampleArgs{h->st, h->tab[m], io, rp, h->ws[m].logits, h->word_start_dev, h->tokens, h->out_owner, h->out_logp, V, c.max_seq_len, m,
+                         h->ws[m].chunk_part, h->ws[m].chunk_ctr, n_chunk};
+  KL(h, TANDEM_KC_SAMPLE, s, launch_ex(sample_switch_emit_kernel<256>, dim3(c.max_seqs, n_chunk, 2), dim3(256), 0, s, pdl, sa));
   return TANDEM_OK;
 }
 
@@ -713,6 +718,9 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
     INIT_TRY(dmalloc(h, &w.lm_in, (size_t)std::max(S, 256) * H * h->esize));
     INIT_TRY(dmalloc(h, &w.gemm_out, (size_t)R * cols * 4));
     INIT_TRY(dmalloc(h, &w.logits, (size_t)S * V * 4));
+    INIT_TRY(dmalloc(h, &w.chunk_part, (size_t)S * kSampleMaxChunks * 6 * 4));
+    INIT_TRY(dmalloc(h, &w.chunk_ctr, (size_t)S * 4));
+    INIT_CU(cudaMemset(w.chunk_ctr, 0, (size_t)S * 4));
     INIT_TRY(dmalloc(h, &w.part_acc, (size_t)h->part_cap * nq * d * 4));
     INIT_TRY(dmalloc(h, &w.part_ml, (size_t)h->part_cap * nq * sizeof(float2)));
     INIT_TRY(dmalloc(h, &w.kv, (size_t)h->pool_pages * page_bytes));
@@ -801,6 +809,7 @@ int tandem_reset(tandem_handle* h) {
     CU(h, cudaMemcpy(h->ws[m].free_pages, fp.data(), (size_t)h->pool_pages * 4, cudaMemcpyHostToDevice));
     CU(h, cudaMemcpy(h->ws[m].free_top, &top, 4, cudaMemcpyHostToDevice));
     CU(h, cudaMemset(h->ws[m].npages, 0, (size_t)S * 4));
+    CU(h, cudaMemset(h->ws[m].chunk_ctr, 0, (size_t)S * 4));
   }
   std::fill(h->slot_busy.begin(), h->slot_busy.end(), 0);
   h->launches = 0;
@@ -980,7 +989,7 @@ void tandem_free(tandem_handle* h) {
   auto fr = [](void* p) { if (p) cudaFree(p); };
   for (int m = 0; m < 2; ++m) {
     Workspace& w = h->ws[m];
-    fr(w.x); fr(w.act); fr(w.q); fr(w.attn_out); fr(w.mlp_act); fr(w.lm_in); fr(w.gemm_out); fr(w.logits); fr(w.part_acc); fr(w.part_ml); fr(w.kv);
+    fr(w.chunk_part); fr(w.chunk_ctr); fr(w.x); fr(w.act); fr(w.q); fr(w.attn_out); fr(w.mlp_act); fr(w.lm_in); fr(w.gemm_out); fr(w.logits); fr(w.part_acc); fr(w.part_ml); fr(w.kv);
     fr(w.tab_mem); fr(w.bt); fr(w.npages); fr(w.free_pages); fr(w.free_top);
     ModelWeights& mw = h->w[m];
     fr(mw.embed); fr(mw.lm_head); fr(mw.final_norm);
