@@ -936,6 +936,13 @@ int tandem_generate(tandem_handle* h, const tandem_params* params, int32_t B, co
   const RuleParams rp = make_rule(params);
   std::vector<int> slot_seq(c.max_seqs, -1);
   std::vector<int32_t> ids(c.max_seqs), nemit(c.max_seqs), plen(c.max_seqs);
+  // Admission by reservation: a sequence is admitted only if each model's page pool can hold its whole context
+  // (prompt + max_new), so a rollout never runs out of pages half-way; the rest waits in the queue (order preserved).
+  std::vector<int> slot_pages(c.max_seqs, 0);
+  auto pages_of = [&](int b) { return (int)((prompt_offsets[b + 1] - prompt_offsets[b] + max_new[b] + kPageTokens - 1) / kPageTokens); };
+  int pages_reserved = 0;
+  const int pages_avail = h->pool_pages - 1;
+  for (int b = 0; b < B; ++b) if (pages_of(b) > pages_avail) return fail(h, TANDEM_ENOMEM, "a single sequence needs more KV pages than the pool holds");
   int next = 0, finished = 0;
   const int poll = 16;
   int64_t budget = 0;   // generous bound on the number of steps: guards against a stuck sequence
@@ -945,12 +952,14 @@ int tandem_generate(tandem_handle* h, const tandem_params* params, int32_t B, co
     if ((budget -= poll) < 0) return fail(h, TANDEM_ESTATE, "generation made no progress (internal error)");
     int nfree = 0;
     for (int i = 0; i < c.max_seqs; ++i) nfree += !h->slot_busy[i];
-    const int n = std::min(nfree, B - next);
+    int n = 0, add = 0;
+    while (n < std::min(nfree, B - next) && pages_reserved + add + pages_of(next + n) <= pages_avail) { add += pages_of(next + n); ++n; }
     if (n > 0) {
       std::vector<int32_t> slots(n);
       for (int i = 0; i < n; ++i) ids[i] = seq_ids ? seq_ids[next + i] : next + i;
       if ((rc = admit(h, params, ovr, n, prompt_tokens, prompt_offsets + next, ids.data(), max_new + next, slots.data(), s))) return rc;
-      for (int i = 0; i < n; ++i) slot_seq[slots[i]] = next + i;
+      for (int i = 0; i < n; ++i) { slot_seq[slots[i]] = next + i; slot_pages[slots[i]] = pages_of(next + i); }
+      pages_reserved += add;
       next += n;
     }
     for (int k = 0; k < poll; ++k) if ((rc = run_step(h, io, rp, s))) return rc;
@@ -965,6 +974,7 @@ int tandem_generate(tandem_handle* h, const tandem_params* params, int32_t B, co
       if (out_owner) CU(h, cudaMemcpy(out_owner + (size_t)b * out_stride, h->out_owner + (size_t)i * c.max_seq_len, (size_t)len, cudaMemcpyDeviceToHost));
       if (out_sen_logp) CU(h, cudaMemcpy(out_sen_logp + (size_t)b * out_stride, h->out_logp + (size_t)i * c.max_seq_len, (size_t)len * 4, cudaMemcpyDeviceToHost));
       slot_seq[i] = -1;
+      pages_reserved -= slot_pages[i]; slot_pages[i] = 0;
       ++finished;
     }
   }

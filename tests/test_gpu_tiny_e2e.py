@@ -118,3 +118,31 @@ def test_explicit_sample_uniforms_and_forced_tokens():
     _compare(out, ref, B, logp_tol=2e-5)
     assert out["len"][2] <= 9
     eng.free()
+
+
+def test_generate_queues_when_the_kv_pool_is_short():
+    """A page pool that holds about two rollouts at a time: tandem_generate admits by reservation (whole context of a sequence
+    must fit in each model's pool), the rest waits; results still equal the oracle's and no page runs out mid-rollout. A
+    sequence that can never fit is refused with TANDEM_ENOMEM up front."""
+    shape = get_workload("cfg1_tiny_f32").shape
+    ws = make_word_start(shape.vocab, 0.3, 11)
+    rng = np.random.default_rng(8)
+    B = 6
+    prompts = [rng.integers(0, shape.vocab, size=int(n)).astype(np.int32) for n in (20, 33, 7, 48, 16, 30)]
+    max_new = np.array([30, 12, 40, 16, 25, 31], dtype=np.int32)
+    page_bytes = 2 * shape.n_layers * shape.n_kv_heads * 16 * shape.head_dim * 4
+    eng, orc, _ = make_pair(shape, (1, 2), max_seqs=6, max_seq_len=96, kv_bytes_per_model=9 * page_bytes)   # 8 usable pages = 128 positions
+    op = OParams(p=0.5, temperature=1.0, seed=77)
+    ref = tandem_generate(orc, op, prompts, max_new, ws, uni=Uniforms(seed=77))
+    out = eng.generate(T.TandemParams(ws, p=0.5, temperature=1.0, seed=77), prompts, max_new)
+    _compare(out, ref, B, logp_tol=2e-5)
+    assert out["stats"]["peak_resident"] < B and max(out["stats"]["peak_pages_senior"], out["stats"]["peak_pages_junior"]) <= 8
+    with pytest.raises(T.TandemError) as e:
+        eng.generate(T.TandemParams(ws, p=0.5, temperature=1.0, seed=77), [np.zeros(90, np.int32)], [60])
+    assert e.value.code == -1 or e.value.code == -2      # prompt + max_new > max_seq_len (EINVAL) or > pool (ENOMEM)
+    eng.free()
+    eng2, _, _ = make_pair(shape, (1, 2), max_seqs=2, max_seq_len=96, kv_bytes_per_model=4 * page_bytes)   # 3 usable pages = 48 positions
+    with pytest.raises(T.TandemError) as e:
+        eng2.generate(T.TandemParams(ws, p=0.5, temperature=1.0, seed=77), [np.zeros(40, np.int32)], [16])   # 56 positions = 4 pages
+    assert e.value.code == -2
+    eng2.free()
