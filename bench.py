@@ -56,6 +56,9 @@ def parse_args():
     ap.add_argument("--e2e-new", type=int, default=64, help="new tokens per sequence in the end-to-end tandem_generate leg")
     ap.add_argument("--profiler-range", action="store_true",
                     help="cudaProfilerStart/Stop around the timed region (for `ncu --profile-from-start off`)")
+    ap.add_argument("--full-rollout", type=float, default=0.0, metavar="SCALE",
+                    help="instead of timed steps: run the WHOLE workload through tandem_generate (host buffers, admission queue) with "
+                         "every max_new multiplied by SCALE (1.0 = the workload as specified) and report tokens/s of the call")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-new", type=int, default=8, help="new tokens of the oracle's bounded sample")
@@ -180,6 +183,67 @@ def class_bytes(shape, cls, rows, kv_bytes_per_layer_launch, emit_rows, n_models
     if cls == "sample_switch_emit":
         return emit_rows * V * 4
     return 0
+
+
+def run_full_rollout(args):
+    """The whole workload through one tandem_generate call: prompts in, tokens / owner flags / senior log-probs out, sequences
+    admitted as KV pages allow (cfg 4 does not fit at once). Ownership of a few sequences is re-derived with the oracle's
+    integer rule from the returned tokens as a sanity check."""
+    import torch
+    import paper_2606_28166_b200 as T
+    from workloads import get_workload, make_weights, make_word_start, make_prompts, make_max_new
+    from oracle import TandemParams as OParams, owners_from_tokens
+    from oracle.rule import Uniforms
+    torch.cuda.set_device(0)
+    T.build()
+    wl = get_workload(args.workload)
+    shape = wl.shape
+    prompts = make_prompts(wl)
+    max_new = np.maximum(1, (make_max_new(wl) * args.full_rollout).astype(np.int32))
+    B = len(prompts)
+    table = make_word_start(shape.vocab, wl.word_start_frac, wl.seeds["table"])
+    # weights are drawn on the GPU, parked on the host and loaded from there, so that no staging copy competes with the KV pools
+    to_cpu = lambda w: dict(embed=w["embed"].cpu(), lm_head=w["lm_head"].cpu(), final_norm=w["final_norm"].cpu(),
+                            layers=[{k: v.cpu() for k, v in l.items()} for l in w["layers"]])
+    w_host = []
+    for seed in (wl.seeds["senior"], wl.seeds["junior"]):
+        w = make_weights(shape, seed, device="cuda"); w_host.append(to_cpu(w)); del w; torch.cuda.empty_cache()
+    free, _ = torch.cuda.mem_get_info()
+    wbytes = 2 * (shape.params_read_per_step + shape.vocab * shape.hidden) * 2      # both models, embedding included
+    need = sum((len(p) + int(n) + 15) // 16 + 1 for p, n in zip(prompts, max_new)) * shape.kv_elems_per_token * 2 * 16
+    kv_per_model = int(min((free - wbytes - 4.5e9) / 2, need + (64 << 20)))            # workspaces and the CUDA context stay free
+    max_seqs = min(B, 256)
+    eng = T.Tandem(T.TandemConfig(shape, max_seqs=max_seqs, max_seq_len=(max(len(p) for p in prompts) + int(max_new.max()) + 31) // 16 * 16,
+                                  kv_bytes_per_model=kv_per_model, max_rows_per_step=4096, use_graph=1))
+    for m in range(2):
+        eng.load_weights(m, w_host[m])
+    del w_host
+    seed = 20260628
+    prm = T.TandemParams(table, p=wl.p, temperature=wl.temperature, top_p=wl.top_p, seed=seed)
+    t0 = time.perf_counter()
+    g = eng.generate(prm, prompts, max_new)
+    dt = time.perf_counter() - t0
+    assert (g["len"] == max_new).all()
+    for b in sorted(set([0, B // 3, B - 1])):
+        o = owners_from_tokens(g["tokens"][b, :g["len"][b]], table, OParams(p=wl.p, seed=seed), Uniforms(seed=seed), b=b)
+        assert np.array_equal(o, g["owner"][b, :g["len"][b]]), "owner flags differ from the rule replayed on the returned tokens"
+    st = g["stats"]
+    tok = int(g["len"].sum())
+    pk = peaks()
+    gbs = (st["kv_bytes_read"] + st["weight_bytes_read"]) / dt / 1e9
+    print(json.dumps({"metric": METRIC, "value": tok / dt, "unit": "tokens/s", "n_gpus": 1, "steps": int(st["steps"]), "warmup": 0,
+                      "ms_per_step": dt / max(1, st["steps"]) * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+                      "data": "synthetic",
+                      "config": {"workload": wl.name, "mode": "full rollout through tandem_generate (prefill, admission queue, host buffers)",
+                                 "sequences": B, "max_new_scale": args.full_rollout, "mean_new": float(max_new.mean()), "tokens": tok, "seconds": dt,
+                                 "max_seqs": max_seqs, "peak_resident": int(st["peak_resident"]), "kv_gb_per_model": kv_per_model / 1e9,
+                                 "peak_pages": [int(st["peak_pages_senior"]), int(st["peak_pages_junior"])],
+                                 "senior_share": float(g["mask"].sum() / max(1, tok))},
+                      "gpu_launches": int(st["kernel_launches"]),
+                      "step_roofline": {"bound": "hbm", "achieved": gbs, "unit": "GB/s", "frac_of_measured": gbs / pk["hbm_gbs"], "frac_of_8TBs": gbs / NOMINAL_HBM_GBS},
+                      "e2e": {"value": tok / dt, "unit": "tokens/s", "h2d_bytes_per_step": sum(len(p) for p in prompts) * 4 / max(1, st["steps"]),
+                              "d2h_bytes_per_step": tok * 9 / max(1, st["steps"])}}))
+    eng.free()
 
 
 def run_ours(args):
@@ -441,5 +505,7 @@ if __name__ == "__main__":
     a = parse_args()
     if a.impl == "reference":
         run_reference(a)
+    elif a.full_rollout > 0:
+        run_full_rollout(a)
     else:
         run_ours(a)

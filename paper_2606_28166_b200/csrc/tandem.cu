@@ -1,5 +1,5 @@
 // tandem.cu - host side of the C ABI declared in include/tandem.h: handle, weights, admission, the step
-// (S0 scheduler -> per model S1..S8 -> finalize) and whole-rollout generation. All arithmetic of the path
+// (S0 scheduler -> S1..S8 for both models, every kernel launched once for the pair -> finalize) and whole-rollout generation. All arithmetic of the path
 // runs in the kernels of this directory; there is no CPU fallback.
 #include "../../include/tandem.h"
 
@@ -83,7 +83,7 @@ struct tandem_handle {
   float2* rope_cs = nullptr;
   uint8_t* word_start_dev = nullptr; std::vector<uint8_t> word_start_host;
   DevStats* stats = nullptr; int32_t* n_active = nullptr; int32_t* work_ctr = nullptr;
-  cudaStream_t ms[2]{}; cudaStream_t gs{}; cudaEvent_t ev_fork{}, ev_join[2]{}, ev_in{}, ev_out{};
+  cudaStream_t gs{}; cudaEvent_t ev_in{}, ev_out{};   // internal stream of the captured step graph and its fork / join events
   std::vector<uint8_t> slot_busy;           // host view of the slots
   // admission staging
   int32_t* stage_tokens = nullptr; size_t stage_cap = 0; long long* stage_off = nullptr; int32_t* stage_i32 = nullptr;
@@ -748,10 +748,7 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
     INIT_TRY(dmalloc(h, &w.free_top, 4));
     INIT_CU(cudaMemset(w.bt, 0, (size_t)S * h->max_pages * 4));
     h->pt[m].bt = w.bt; h->pt[m].npages = w.npages; h->pt[m].free_pages = w.free_pages; h->pt[m].free_top = w.free_top;
-    INIT_CU(cudaStreamCreateWithFlags(&h->ms[m], cudaStreamNonBlocking));
-    INIT_CU(cudaEventCreateWithFlags(&h->ev_join[m], cudaEventDisableTiming));
   }
-  INIT_CU(cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));
   INIT_CU(cudaEventCreateWithFlags(&h->ev_in, cudaEventDisableTiming));
   INIT_CU(cudaEventCreateWithFlags(&h->ev_out, cudaEventDisableTiming));
   INIT_CU(cudaStreamCreateWithFlags(&h->gs, cudaStreamNonBlocking));
@@ -1004,11 +1001,8 @@ void tandem_free(tandem_handle* h) {
     ModelWeights& mw = h->w[m];
     fr(mw.embed); fr(mw.lm_head); fr(mw.final_norm);
     for (auto* v : {&mw.attn_norm, &mw.wqkv, &mw.wo, &mw.mlp_norm, &mw.wgu, &mw.wdown}) for (void* p : *v) fr(p);
-    if (h->ms[m]) cudaStreamDestroy(h->ms[m]);
-    if (h->ev_join[m]) cudaEventDestroy(h->ev_join[m]);
   }
   for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
-  if (h->ev_fork) cudaEventDestroy(h->ev_fork);
   if (h->ev_in) cudaEventDestroy(h->ev_in);
   if (h->ev_out) cudaEventDestroy(h->ev_out);
   if (h->gs) cudaStreamDestroy(h->gs);
