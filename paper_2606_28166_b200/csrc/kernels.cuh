@@ -350,12 +350,14 @@ __global__ void __launch_bounds__(NT) rope_append_kernel(const __grid_constant__
   const int half = d >> 1, hq = half >> 2;                 // hq: groups of 4 pairs per head
   const int ld = (nq + 2 * nkv) * d;
   const int n_rot = (nq + nkv) * hq, n_v = nkv * (d >> 2);
-  for (int r = blockIdx.x; r < n_rows; r += gridDim.x) {
+  // four CTAs per row (blockIdx.x = 4 * row-lane + quarter): one item per thread at the 4B shape, so a row costs one memory latency
+  const int quarter = blockIdx.x & 3;
+  for (int r = blockIdx.x >> 2; r < n_rows; r += gridDim.x >> 2) {
     const int pos = row_pos[r];
     const int kvslot = row_kvslot[r];
     const int page = kvslot / kPageTokens, off = kvslot % kPageTokens;
     const float* src = part + (size_t)r * ld;
-    for (int i = threadIdx.x; i < n_rot + n_v; i += NT) {
+    for (int i = quarter * NT + threadIdx.x; i < n_rot + n_v; i += 4 * NT) {
       if (i < n_rot) {
         const int head = i / hq, j = (i - head * hq) << 2;
         float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a;

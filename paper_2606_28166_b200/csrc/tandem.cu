@@ -331,7 +331,7 @@ int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaS
       bool ok = true;
       KL(h, TANDEM_KC_ATTENTION, s, ok = run_attn_mma(kmaps, ma, d, nq / nkv, h->attn_ctas_per_sm * h->n_sms, s, false, pdl));
       if (!ok) return fail(h, TANDEM_EINVAL, "unsupported (head_dim, group) for attention");
-      KL(h, TANDEM_KC_ATTN_COMBINE, s, launch_ex(attn_combine_kernel<T>, dim3(148, 2), dim3(256), 0, s, pdl, ca));
+      KL(h, TANDEM_KC_ATTN_COMBINE, s, launch_ex(attn_combine_kernel<T>, dim3(148 * 4, 2), dim3(256), 0, s, pdl, ca));
       if ((rc = launch_layer_tail(h, l + 1, s))) return rc;
       continue;
     }
@@ -345,14 +345,14 @@ int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaS
         T* kpool = (T*)h->ws[m].kv + (size_t)l * layer_kv;
         ra.m[m] = RopeArgs<T, bf16>{h->tab[m].counts, h->tab[m].row_pos, h->tab[m].row_kvslot, h->ws[m].gemm_out, ns, ss, h->rope_cs, (bf16*)h->ws[m].q, kpool, kpool + half_kv, nq, nkv, d};
       }
-      KL(h, TANDEM_KC_ROPE_APPEND, s, launch_ex(rope_append_kernel<T, bf16, 256>, dim3(row_grid, 2), dim3(256), 0, s, pdl, ra));
+      KL(h, TANDEM_KC_ROPE_APPEND, s, launch_ex(rope_append_kernel<T, bf16, 256>, dim3(row_grid * 4, 2), dim3(256), 0, s, pdl, ra));
     } else {
       Pair<RopeArgs<T, float>> ra;
       for (int m = 0; m < 2; ++m) {
         T* kpool = (T*)h->ws[m].kv + (size_t)l * layer_kv;
         ra.m[m] = RopeArgs<T, float>{h->tab[m].counts, h->tab[m].row_pos, h->tab[m].row_kvslot, h->ws[m].gemm_out, ns, ss, h->rope_cs, (float*)h->ws[m].q, kpool, kpool + half_kv, nq, nkv, d};
       }
-      KL(h, TANDEM_KC_ROPE_APPEND, s, launch_ex(rope_append_kernel<T, float, 256>, dim3(row_grid, 2), dim3(256), 0, s, pdl, ra));
+      KL(h, TANDEM_KC_ROPE_APPEND, s, launch_ex(rope_append_kernel<T, float, 256>, dim3(row_grid * 4, 2), dim3(256), 0, s, pdl, ra));
     }
     // S5 attention (decode splits + catch-up rows), then combine
     bool ok = true;
@@ -384,7 +384,7 @@ int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaS
         const StepTab& tb = h->tab[m];
         ca.m[m] = CombineArgs<T>{tb.counts, tb.comb_row, tb.comb_part0, tb.comb_n, tb.comb_stride, h->ws[m].part_acc, h->ws[m].part_ml, (T*)h->ws[m].attn_out, nq, d};
       }
-      KL(h, TANDEM_KC_ATTN_COMBINE, s, launch_ex(attn_combine_kernel<T>, dim3(148, 2), dim3(256), 0, s, pdl, ca));
+      KL(h, TANDEM_KC_ATTN_COMBINE, s, launch_ex(attn_combine_kernel<T>, dim3(148 * 4, 2), dim3(256), 0, s, pdl, ca));
     }
     // S6 O projection + residual + RMSNorm(mlp)
     for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].attn_out, h->w[m].wo[l], h->ws[m].gemm_out, h->tab[m].counts + C_ROWS);
