@@ -11,7 +11,7 @@
 // activations, and it streams the next phase's weight tiles into the shared-memory ring while the other warps finish the
 // epilogue, wait at the barrier and run the element-wise phase. Only the activation boxes of a stage wait for the barrier.
 // This removes the per-kernel fixed costs (launch, prologue, first TMA round trip, drain) that made the seven separate
-// kernels take 190 us per layer for 62 us of weight streaming (profiles/launches_r1c.md).
+// kernels take 190 us per layer for 62 us of weight streaming (profiles/launches_r1d.md).
 //   warp 0    : weight TMA producer (never waits for a grid barrier: runs ahead as far as the ring allows)
 //   warp 10   : activation TMA producer (same stage sequence, gated by the barrier of the producing phase)
 //   warp 1    : MMA issuer (tcgen05.mma, one thread)
