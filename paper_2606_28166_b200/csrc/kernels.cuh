@@ -286,7 +286,7 @@ template <typename T> struct ResNormArgs {
 };
 template <typename T, int NT, int VPT>
 __global__ void __launch_bounds__(NT) residual_norm_kernel(const __grid_constant__ Pair<ResNormArgs<T>> pp) {
-  pdl_trigger(); pdl_wait();
+  pdl_trigger();
   const ResNormArgs<T>& a = pp.m[blockIdx.y];
   const int32_t* __restrict__ counts = a.counts; const float* __restrict__ part = a.part; const int n_split = a.n_split;
   const size_t split_stride = a.split_stride; float* __restrict__ x = a.x; const T* __restrict__ gain = a.gain; T* __restrict__ act = a.act;
@@ -294,6 +294,15 @@ __global__ void __launch_bounds__(NT) residual_norm_kernel(const __grid_constant
   __shared__ float red[32];
   const int n_rows = counts[C_ROWS];
   const int H4 = H >> 2;
+  // constants first (gains, scheduler tables): they do not depend on the predecessor kernel, so they load while it drains
+  float4 gn[VPT];
+#pragma unroll
+  for (int i = 0; i < VPT; ++i) {
+    const int j4 = threadIdx.x + i * NT;
+    gn[i] = j4 < H4 ? ld4(gain + 4 * j4) : make_float4(0.f, 0.f, 0.f, 0.f);
+  }
+  const int orow0 = (int)blockIdx.x < n_rows ? (out_map ? out_map[blockIdx.x] : (int)blockIdx.x) : -1;
+  pdl_wait();
   for (int r = blockIdx.x; r < n_rows; r += gridDim.x) {
     float4 v[VPT];
 #pragma unroll
@@ -301,7 +310,7 @@ __global__ void __launch_bounds__(NT) residual_norm_kernel(const __grid_constant
       const int j4 = threadIdx.x + i * NT;
       v[i] = j4 < H4 ? ld4(x + (size_t)r * H + 4 * j4) : make_float4(0.f, 0.f, 0.f, 0.f);
     }
-#pragma unroll 4
+#pragma unroll 8
     for (int s = 0; s < n_split; ++s) {
 #pragma unroll
       for (int i = 0; i < VPT; ++i) {
@@ -316,16 +325,13 @@ __global__ void __launch_bounds__(NT) residual_norm_kernel(const __grid_constant
       if (j4 < H4) st4(x + (size_t)r * H + 4 * j4, v[i]);
       ss += v[i].x * v[i].x + v[i].y * v[i].y + v[i].z * v[i].z + v[i].w * v[i].w;
     }
-    const int orow = out_map ? out_map[r] : r;
+    const int orow = r == (int)blockIdx.x ? orow0 : (out_map ? out_map[r] : r);
     const float inv = rsqrtf(block_sum<NT>(ss, red) / (float)H + eps);
     if (orow < 0) continue;
 #pragma unroll
     for (int i = 0; i < VPT; ++i) {
       const int j4 = threadIdx.x + i * NT;
-      if (j4 < H4) {
-        const float4 g = ld4(gain + 4 * j4);
-        st4(act + (size_t)orow * H + 4 * j4, make_float4(v[i].x * g.x * inv, v[i].y * g.y * inv, v[i].z * g.z * inv, v[i].w * g.w * inv));
-      }
+      if (j4 < H4) st4(act + (size_t)orow * H + 4 * j4, make_float4(v[i].x * gn[i].x * inv, v[i].y * gn[i].y * inv, v[i].z * gn[i].z * inv, v[i].w * gn[i].w * inv));
     }
   }
 }
