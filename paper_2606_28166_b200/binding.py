@@ -17,7 +17,7 @@ _ERR = {0: "OK", -1: "EINVAL", -2: "ENOMEM", -3: "ECUDA", -4: "ESTATE", -5: "EFU
 
 EXPORTED_SYMBOLS = ["tandem_init", "tandem_load_weights", "tandem_step", "tandem_generate", "tandem_reset",
                     "tandem_free", "tandem_last_error", "tandem_get_stats", "tandem_set_profile", "tandem_get_profile",
-                    "tandem_kernel_class_name", "tandem_debug_lt_times", "tandem_test_uniforms", "tandem_test_philox", "tandem_test_gemm", "tandem_test_gemm_time"]
+                    "tandem_kernel_class_name", "tandem_debug_lt_times", "tandem_test_uniforms", "tandem_test_nucleus", "tandem_test_philox", "tandem_test_gemm", "tandem_test_gemm_time"]
 KC_NUM = 15
 
 
@@ -97,6 +97,7 @@ def lib():
         L.tandem_last_error.argtypes = [C.c_void_p]
         L.tandem_last_error.restype = C.c_char_p
         L.tandem_test_uniforms.argtypes = [C.c_uint64, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_void_p]
+        L.tandem_test_nucleus.argtypes = [C.c_int32, C.c_float, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.tandem_test_philox.argtypes = [C.POINTER(C.c_uint32), C.POINTER(C.c_uint32), C.POINTER(C.c_uint32)]
         L.tandem_test_gemm.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
         L.tandem_debug_lt_times.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
@@ -254,6 +255,12 @@ class Tandem:
 
 def tandem_test_uniforms(seed, seq_id, t, stream, n, out_dev):
     rc = lib().tandem_test_uniforms(seed, seq_id, t, stream, n, out_dev.data_ptr())
+    if rc:
+        raise TandemError(rc)
+
+
+def tandem_test_nucleus(logits, temperature, top_p, u, token_out, keep_out):
+    rc = lib().tandem_test_nucleus(logits.numel(), temperature, top_p, logits.data_ptr(), u.data_ptr(), token_out.data_ptr(), keep_out.data_ptr())
     if rc:
         raise TandemError(rc)
 

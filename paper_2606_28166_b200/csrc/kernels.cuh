@@ -437,6 +437,109 @@ __device__ __forceinline__ ArgBest better(ArgBest a, ArgBest b) {  // larger val
   return (b.v > a.v || (b.v == a.v && b.i < a.i)) ? b : a;
 }
 
+// Nucleus (top-p) filtering, then the Gumbel argmax over the kept set (reading R10; off the fast path). The whole CTA
+// scans the row (L2-resident): x_v = z_v * invT maps to an order-preserving 32-bit key; a bitwise search finds the
+// largest key k with  sum_{key_v >= k} p_v >= top_p, i.e. the probability of the last kept id; ids above it are kept,
+// ids equal to it by ascending id until the mass reaches top_p. m, sum: the row's max and sum exp(x - m).
+__device__ __forceinline__ uint32_t order_key(float x) {
+  const uint32_t u = __float_as_uint(x);
+  return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ __forceinline__ float key_value(uint32_t k) {
+  return __uint_as_float((k & 0x80000000u) ? (k & 0x7fffffffu) : ~k);
+}
+template <int NT>
+__device__ int nucleus_gumbel_argmax(const float* __restrict__ z, int V, float invT, float m, float sum, float top_p,
+                                     const float* __restrict__ u_row, uint32_t k0, uint32_t k1, int t, int sid,
+                                     float* s_red, int* s_redi, uint8_t* keep_out = nullptr) {
+  const float target = top_p * sum;   // in units of exp(x - m)
+  uint32_t key = 0u;
+  for (int bit = 31; bit >= 0; --bit) {
+    const uint32_t cand = key | (1u << bit);
+    float f = 0.f;
+    for (int v = threadIdx.x; v < V; v += NT) {
+      const float x = z[v] * invT;
+      if (order_key(x) >= cand) f += expf(x - m);
+    }
+    if (block_sum<NT>(f, s_red) >= target) key = cand;
+  }
+  // mass strictly above the threshold probability, and the number of ids at it
+  float above = 0.f, ties = 0.f;
+  for (int v = threadIdx.x; v < V; v += NT) {
+    const float x = z[v] * invT;
+    const uint32_t kx = order_key(x);
+    if (kx > key) above += expf(x - m);
+    ties += (kx == key) ? 1.f : 0.f;
+  }
+  above = block_sum<NT>(above, s_red);
+  const int n_ties = (int)block_sum<NT>(ties, s_red);
+  int id_cut = V;   // ids at the threshold are kept while id <= id_cut
+  if (n_ties > 1) {
+    const float e = expf(key_value(key) - m);
+    int c = (int)ceilf((target - above) / e);
+    c = max(1, min(c, n_ties));
+    if (c < n_ties) {   // the c-th smallest id among the ties
+      int lo = 0, hi = V - 1;
+      while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        float cnt = 0.f;
+        for (int v = threadIdx.x; v <= mid; v += NT) cnt += (order_key(z[v] * invT) == key) ? 1.f : 0.f;
+        if ((int)block_sum<NT>(cnt, s_red) >= c) hi = mid; else lo = mid + 1;
+      }
+      id_cut = lo;
+    }
+  }
+  ArgBest best = {-INFINITY, 0x7fffffff};
+  for (int b4 = threadIdx.x; b4 * 4 < V; b4 += NT) {
+    uint32_t c[4] = {(uint32_t)b4, (uint32_t)t, (uint32_t)sid, 0u};
+    if (!u_row) philox4x32_10(c, k0, k1);
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+      const int v = b4 * 4 + w;
+      if (v >= V) break;
+      const float x = z[v] * invT;
+      const uint32_t kx = order_key(x);
+      const bool keep = kx > key || (kx == key && v <= id_cut);
+      if (keep_out) keep_out[v] = keep;
+      if (keep) {
+        const float u = u_row ? u_row[v] : uniform_from_bits(c[w]);
+        best = better(best, ArgBest{x + gumbel_from_uniform(u), v});
+      }
+    }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    ArgBest o2 = {__shfl_xor_sync(0xffffffffu, best.v, o), __shfl_xor_sync(0xffffffffu, best.i, o)};
+    best = better(best, o2);
+  }
+  __syncthreads();
+  if ((threadIdx.x & 31) == 0) { s_red[threadIdx.x >> 5] = best.v; s_redi[threadIdx.x >> 5] = best.i; }
+  __syncthreads();
+  best = ArgBest{s_red[0], s_redi[0]};
+  for (int k = 1; k < NT / 32; ++k) best = better(best, ArgBest{s_red[k], s_redi[k]});
+  return best.i;
+}
+
+// test hook: one row of logits through the nucleus search exactly as the sampler runs it (explicit uniforms)
+template <int NT>
+__global__ void __launch_bounds__(NT) test_nucleus_kernel(const float* z, int V, float temperature, float top_p, const float* u, int32_t* token,
+                                                          uint8_t* keep) {
+  __shared__ float s_red[NT / 32];
+  __shared__ int s_redi[NT / 32];
+  const float invT = 1.f / temperature;
+  float m = -INFINITY;
+  for (int v = threadIdx.x; v < V; v += NT) m = fmaxf(m, z[v] * invT);
+  for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if ((threadIdx.x & 31) == 0) s_red[threadIdx.x >> 5] = m;
+  __syncthreads();
+  for (int k = 0; k < NT / 32; ++k) m = fmaxf(m, s_red[k]);
+  float sum = 0.f;
+  for (int v = threadIdx.x; v < V; v += NT) sum += expf(z[v] * invT - m);
+  sum = block_sum<NT>(sum, s_red);
+  const int y = nucleus_gumbel_argmax<NT>(z, V, invT, m, sum, top_p, u, 0u, 0u, 1, 0, s_red, s_redi, keep);
+  if (threadIdx.x == 0) *token = y;
+}
+
 template <int NT>
 __global__ void __launch_bounds__(NT) sample_switch_emit_kernel(const __grid_constant__ Pair<SampleArgs> pp) {
   pdl_trigger(); pdl_wait();
@@ -498,32 +601,50 @@ __global__ void __launch_bounds__(NT) sample_switch_emit_kernel(const __grid_con
   const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
   if (l == 0) { s_m[w] = m; s_s[w] = sum; s_bv[w] = raw.v; s_bi[w] = raw.i; s_gv[w] = gum.v; s_gi[w] = gum.i; }
   __syncthreads();
-  if (threadIdx.x != 0) return;
-  for (int k = 1; k < NT / 32; ++k) {
-    const float mn = fmaxf(m, s_m[k]);
-    sum = (m == -INFINITY ? 0.f : sum * expf(m - mn)) + (s_m[k] == -INFINITY ? 0.f : s_s[k] * expf(s_m[k] - mn));
-    m = mn;
-    raw = better(raw, ArgBest{s_bv[k], s_bi[k]});
-    gum = better(gum, ArgBest{s_gv[k], s_gi[k]});
-  }
-  if (n_chunk > 1) {
-    // publish this slice; the CTA that arrives last merges all slices in slice order (deterministic) and applies the rule
-    float* cp = a.chunk_part + ((size_t)j * n_chunk + ch) * 6;
-    cp[0] = m; cp[1] = sum; cp[2] = raw.v; cp[3] = __int_as_float(raw.i); cp[4] = gum.v; cp[5] = __int_as_float(gum.i);
-    __threadfence();
-    if (atomicAdd(a.chunk_ctr + j, 1) != n_chunk - 1) return;
-    a.chunk_ctr[j] = 0;
-    __threadfence();
-    m = -INFINITY; sum = 0.f; raw = ArgBest{-INFINITY, 0x7fffffff}; gum = raw;
-    for (int k = 0; k < n_chunk; ++k) {
-      const float* q = a.chunk_part + ((size_t)j * n_chunk + k) * 6;
-      const float mk = __ldcg(q), sk = __ldcg(q + 1);
-      const float mn = fmaxf(m, mk);
-      sum = (m == -INFINITY ? 0.f : sum * expf(m - mn)) + (mk == -INFINITY ? 0.f : sk * expf(mk - mn));
+  const bool nucleus = !greedy && a.rp.top_p < 1.f;   // the whole CTA stays for the nucleus search, else thread 0 alone
+  if (!nucleus && threadIdx.x != 0) return;
+  bool last = true;
+  if (threadIdx.x == 0) {
+    for (int k = 1; k < NT / 32; ++k) {
+      const float mn = fmaxf(m, s_m[k]);
+      sum = (m == -INFINITY ? 0.f : sum * expf(m - mn)) + (s_m[k] == -INFINITY ? 0.f : s_s[k] * expf(s_m[k] - mn));
       m = mn;
-      raw = better(raw, ArgBest{__ldcg(q + 2), __float_as_int(__ldcg(q + 3))});
-      gum = better(gum, ArgBest{__ldcg(q + 4), __float_as_int(__ldcg(q + 5))});
+      raw = better(raw, ArgBest{s_bv[k], s_bi[k]});
+      gum = better(gum, ArgBest{s_gv[k], s_gi[k]});
     }
+    if (n_chunk > 1) {
+      // publish this slice; the CTA that arrives last merges all slices in slice order (deterministic) and applies the rule
+      float* cp = a.chunk_part + ((size_t)j * n_chunk + ch) * 6;
+      cp[0] = m; cp[1] = sum; cp[2] = raw.v; cp[3] = __int_as_float(raw.i); cp[4] = gum.v; cp[5] = __int_as_float(gum.i);
+      __threadfence();
+      last = atomicAdd(a.chunk_ctr + j, 1) == n_chunk - 1;
+      if (last) {
+        a.chunk_ctr[j] = 0;
+        __threadfence();
+        m = -INFINITY; sum = 0.f; raw = ArgBest{-INFINITY, 0x7fffffff}; gum = raw;
+        for (int k = 0; k < n_chunk; ++k) {
+          const float* q = a.chunk_part + ((size_t)j * n_chunk + k) * 6;
+          const float mk = __ldcg(q), sk = __ldcg(q + 1);
+          const float mn = fmaxf(m, mk);
+          sum = (m == -INFINITY ? 0.f : sum * expf(m - mn)) + (mk == -INFINITY ? 0.f : sk * expf(mk - mn));
+          m = mn;
+          raw = better(raw, ArgBest{__ldcg(q + 2), __float_as_int(__ldcg(q + 3))});
+          gum = better(gum, ArgBest{__ldcg(q + 4), __float_as_int(__ldcg(q + 5))});
+        }
+      }
+    }
+  }
+  if (nucleus) {
+    __shared__ float s_fin[2];
+    __shared__ int s_last;
+    if (threadIdx.x == 0) { s_last = last; s_fin[0] = m; s_fin[1] = sum; }
+    __syncthreads();
+    if (!s_last) return;
+    const int yn = nucleus_gumbel_argmax<NT>(z, V, invT, s_fin[0], s_fin[1], a.rp.top_p, u_row, k0, k1, t, sid, s_s, s_bi);
+    if (threadIdx.x != 0) return;
+    gum.i = yn;
+  } else if (!last) {
+    return;
   }
   int y = greedy ? raw.i : gum.i;
   if (a.io.forced_tokens) {

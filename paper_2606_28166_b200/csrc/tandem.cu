@@ -53,7 +53,7 @@ struct GraphKey {
   StepIO io; RuleParams rp; bool valid = false;
   bool same(const StepIO& i, const RuleParams& r) const {
     return valid && std::memcmp(&io, &i, sizeof(StepIO)) == 0 && rp.p == r.p && rp.switch_mode == r.switch_mode && rp.cap_k == r.cap_k &&
-           rp.temperature == r.temperature && rp.eos_id == r.eos_id && rp.seed == r.seed;
+           rp.temperature == r.temperature && rp.eos_id == r.eos_id && rp.seed == r.seed && rp.top_p == r.top_p;
   }
 };
 
@@ -496,7 +496,7 @@ int check_params(tandem_handle* h, const tandem_params* p) {
   if (p->start_owner < 0 || p->start_owner > 2) return fail(h, TANDEM_EINVAL, "bad start_owner");
   if (p->cap_k < 0) return fail(h, TANDEM_EINVAL, "cap_k must be >= 0");
   if (!(p->temperature >= 0.f)) return fail(h, TANDEM_EINVAL, "temperature must be >= 0");
-  if (p->top_p != 1.0f) return fail(h, TANDEM_EINVAL, "top_p < 1 is not implemented in this version");
+  if (!(p->top_p > 0.f && p->top_p <= 1.0f)) return fail(h, TANDEM_EINVAL, "top_p must be in (0, 1]");
   if (p->eos_id >= h->cfg.vocab) return fail(h, TANDEM_EINVAL, "eos_id >= vocab");
   if (!p->word_start) return fail(h, TANDEM_EINVAL, "word_start is NULL");
   return TANDEM_OK;
@@ -523,7 +523,7 @@ StepIO make_io(const tandem_step_out* out, const tandem_overrides* ovr) {
   return io;
 }
 RuleParams make_rule(const tandem_params* p) {
-  RuleParams r{}; r.p = p->p; r.switch_mode = p->switch_mode; r.cap_k = p->cap_k; r.temperature = p->temperature; r.eos_id = p->eos_id; r.seed = p->seed;
+  RuleParams r{}; r.p = p->p; r.switch_mode = p->switch_mode; r.cap_k = p->cap_k; r.temperature = p->temperature; r.eos_id = p->eos_id; r.seed = p->seed; r.top_p = p->top_p;
   return r;
 }
 
@@ -1032,6 +1032,13 @@ __global__ void test_philox_kernel(uint32_t* io) {
 int tandem_test_uniforms(uint64_t seed, int32_t seq_id, int32_t t, int32_t stream, int32_t n, float* out_dev) {
   if (n <= 0 || !out_dev) return TANDEM_EINVAL;
   test_uniforms_kernel<<<(n + 255) / 256, 256>>>(seed, seq_id, t, stream, n, out_dev);
+  return cudaDeviceSynchronize() == cudaSuccess ? TANDEM_OK : TANDEM_ECUDA;
+}
+
+int tandem_test_nucleus(int32_t vocab, float temperature, float top_p, const float* logits_dev, const float* u_dev, int32_t* token_dev,
+                        uint8_t* keep_dev) {
+  if (vocab <= 0 || !(temperature > 0.f) || !(top_p > 0.f && top_p < 1.f) || !logits_dev || !u_dev || !token_dev || !keep_dev) return TANDEM_EINVAL;
+  test_nucleus_kernel<256><<<1, 256>>>(logits_dev, vocab, temperature, top_p, u_dev, token_dev, keep_dev);
   return cudaDeviceSynchronize() == cudaSuccess ? TANDEM_OK : TANDEM_ECUDA;
 }
 

@@ -64,7 +64,7 @@ def test_api_errors():
     assert e.value.code == -4                                   # ESTATE: no weights yet
     eng.free()
     eng, _, _ = make_pair(SHAPE, max_seqs=2, max_seq_len=32)
-    for bad in (dict(p=1.5), dict(top_p=0.9), dict(temperature=-1.0), dict(cap_k=-1), dict(eos_id=SHAPE.vocab)):
+    for bad in (dict(p=1.5), dict(top_p=0.0), dict(top_p=1.5), dict(temperature=-1.0), dict(cap_k=-1), dict(eos_id=SHAPE.vocab)):
         with pytest.raises(T.TandemError) as e:
             eng.generate(T.TandemParams(ws, **bad), [np.arange(4, dtype=np.int32)], [4])
         assert e.value.code == -1

@@ -98,3 +98,54 @@ def test_tcgen05_gemm_swiglu_epilogue(rows, I, K):
     ref = gate / (1 + torch.exp(-gate)) * up
     err = torch.max(torch.abs(out.double() - ref)).item()
     assert err <= 2 ** -8 * max(1e-3, ref.abs().max().item()) + 1e-6, (err, ref.abs().max().item())   # one bf16 rounding of the result
+
+
+def _nucleus(z, temperature, top_p, u):
+    zt = torch.tensor(z, dtype=torch.float32, device="cuda")
+    ut = torch.tensor(u, dtype=torch.float32, device="cuda")
+    tok = torch.zeros(1, dtype=torch.int32, device="cuda")
+    keep = torch.zeros(len(z), dtype=torch.uint8, device="cuda")
+    T.tandem_test_nucleus(zt, temperature, top_p, ut, tok, keep)
+    return int(tok.item()), keep.cpu().numpy().astype(bool)
+
+
+def test_nucleus_hand_examples_and_ties():
+    """The kept set of reading R10 on the hand example of tests/test_oracle_sampler.py, on exact ties (lower id first) and on a
+    one-hot row; the expected masks come from oracle.sampler.kept_set_top_p."""
+    from oracle.sampler import kept_set_top_p
+    z = np.log(np.array([0.3, 0.05, 0.5, 0.15]))
+    u = np.full(4, 0.5, dtype=np.float32)
+    for top_p in (0.45, 0.51, 0.79, 0.81, 0.96, 1e-6):
+        _, keep = _nucleus(z, 1.0, top_p, u)
+        assert keep.tolist() == kept_set_top_p(z.astype(np.float32), 1.0, top_p).tolist(), top_p
+    for V, top_p in ((4, 0.3), (4, 0.55), (7, 0.5), (1000, 0.25), (1000, 0.999)):      # all ids tie: a prefix by id
+        _, keep = _nucleus(np.zeros(V), 1.0, top_p, np.full(V, 0.5, np.float32))
+        want = kept_set_top_p(np.zeros(V, np.float32), 1.0, top_p)
+        assert abs(int(keep.sum()) - int(want.sum())) <= (1 if abs(V * top_p - round(V * top_p)) < 1e-6 else 0) and keep[:keep.sum()].all()
+    z = np.array([0., 2., 2., -1., 2., 2., 0.5]); u = np.full(7, 0.5, np.float32)        # four-way tie at the top
+    for top_p in (0.1, 0.3, 0.5, 0.7):
+        _, keep = _nucleus(z, 1.0, top_p, u)
+        assert keep.tolist() == kept_set_top_p(z.astype(np.float32), 1.0, top_p).tolist(), top_p
+    z = np.full(300, -30.0); z[123] = 10.0
+    tok, keep = _nucleus(z, 0.7, 0.9, np.full(300, 0.5, np.float32))
+    assert tok == 123 and keep.sum() == 1 and keep[123]
+
+
+@pytest.mark.parametrize("V,temperature,top_p,seed", [(512, 0.7, 0.8, 0), (1000, 1.0, 0.5, 1), (4099, 0.6, 0.95, 2), (151936, 0.7, 0.8, 3),
+                                                       (151936, 1.0, 0.2, 4)])
+def test_nucleus_random_rows_match_oracle(V, temperature, top_p, seed):
+    """Random rows (no exact ties): kept set identical to the oracle's float64 sort-and-cumsum except possibly the one id whose
+    cumulative mass lands within fp32 rounding of top_p; sampled token identical."""
+    from oracle.sampler import kept_set_top_p, sample_token
+    rng = np.random.default_rng(seed)
+    for rep in range(3):
+        z = (rng.standard_normal(V) * 3.0).astype(np.float32)
+        u = np.minimum((rng.integers(0, 1 << 32, size=V, dtype=np.uint64).astype(np.float32) + 0.5) * np.float32(2.0 ** -32),
+                       np.float32(1 - 2.0 ** -24)).astype(np.float32)
+        tok, keep = _nucleus(z, temperature, top_p, u)
+        want = kept_set_top_p(z, temperature, top_p)
+        assert int(np.sum(keep != want)) <= 1
+        p = np.exp(z.astype(np.float64) / temperature); p /= p.sum()
+        assert p[keep].sum() >= top_p - 1e-5 and (keep.sum() == 1 or p[keep].sum() - p[keep].min() < top_p + 1e-5)   # reaches top_p, minimal
+        if np.array_equal(keep, want):
+            assert tok == sample_token(z, temperature, top_p, u)
