@@ -45,6 +45,7 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg3_4b_bf16")
     ap.add_argument("--p", type=float, default=None, help="override the workload's switch probability (cfg5 sweep)")
+    ap.add_argument("--top-p", type=float, default=None, help="override the workload's top-p (the paper trains at 1.0, evaluates at 0.8)")
     ap.add_argument("--word-start-frac", type=float, default=None, help="override the word-start table density (cfg5 sweep)")
     ap.add_argument("--fast-forward", type=int, default=-1,
                     help="tokens already generated per sequence before the timed window (ingested as context by prefill); "
@@ -265,6 +266,8 @@ def run_ours(args):
         wl = wl.with_(p=args.p)
     if args.word_start_frac is not None:
         wl = wl.with_(word_start_frac=args.word_start_frac)
+    if args.top_p is not None:
+        wl = wl.with_(top_p=args.top_p)
     shape, B = wl.shape, wl.batch
     W, K = max(3, args.warmup), args.steps
     if args.fast_forward < 0:
@@ -388,7 +391,7 @@ def run_ours(args):
     res = {"metric": METRIC, "value": tokens_all / (ms_all * 1e-3), "unit": "tokens/s", "n_gpus": world, "steps": K, "warmup": W,
            "ms_per_step": ms_all / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
            "config": {"workload": wl.name, "batch_per_gpu": B, "prompt_len": list(wl.prompt_len), "fast_forward": args.fast_forward,
-                      "ctx_mean_timed": ctx_mean, "p": wl.p, "word_start_frac": wl.word_start_frac, "temperature": wl.temperature,
+                      "ctx_mean_timed": ctx_mean, "p": wl.p, "word_start_frac": wl.word_start_frac, "temperature": wl.temperature, "top_p": wl.top_p,
                       "page_tokens": 16, "parallelism": "dp%d (independent sequences, replicated weights, no collective)" % world,
                       "l2": "inputs larger than L2 (16.1 GB of weights + KV streamed per step vs 126 MB L2)",
                       "setup_steps": n_setup + ramp + n_drain, "setup_seconds": setup_s, "cuda_graph": True},

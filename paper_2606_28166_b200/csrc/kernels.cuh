@@ -437,10 +437,28 @@ __device__ __forceinline__ ArgBest better(ArgBest a, ArgBest b) {  // larger val
   return (b.v > a.v || (b.v == a.v && b.i < a.i)) ? b : a;
 }
 
-// Nucleus (top-p) filtering, then the Gumbel argmax over the kept set (reading R10; off the fast path). The whole CTA
-// scans the row (L2-resident): x_v = z_v * invT maps to an order-preserving 32-bit key; a bitwise search finds the
-// largest key k with  sum_{key_v >= k} p_v >= top_p, i.e. the probability of the last kept id; ids above it are kept,
-// ids equal to it by ascending id until the mass reaches top_p. m, sum: the row's max and sum exp(x - m).
+// Nucleus (top-p) filtering, then the Gumbel argmax over the kept set (reading R10; off the fast path: a few passes over the
+// L2-resident row by the CTA that merges it). Masses are fixed-point integers (exp(x - m) * 2^40), so every sum is exact and
+// independent of the order of accumulation. Each id has a 24-bit depth T = floor(2^18 * min(log2e * (m - x), 64)), monotone in
+// x. Level passes histogram the ids under the current prefix of T on its next 4 bits (16 bins of mass in registers, no atomics)
+// and descend into the bin where the cumulative mass crosses top_p * total; from the second level on the same pass also
+// gathers those ids into shared memory (an order-preserving 32-bit key of x, mass, id) and the descent stops once they fit.
+// A bitwise search over the list finds the largest key k with mass{key >= k} >= target, i.e. the last kept probability. Ids
+// above it are kept, ids equal to it by ascending id until the mass is reached. If the ids still do not fit after all 24 bits
+// (a row of equal logits), the same search scans the row instead of the list. Last pass: the Gumbel argmax over the kept ids.
+constexpr int kNucleusCap = 2048;
+constexpr int kNucleusBins = 16;
+template <int NT> struct NucleusSmem {
+  unsigned long long ph[kNucleusBins][NT];   // a private histogram per thread: no atomics, no bank conflicts
+  unsigned long long hist[kNucleusBins];
+  unsigned long long cq[kNucleusCap];
+  unsigned long long red[NT / 32];
+  uint32_t ck[kNucleusCap];
+  int cid[kNucleusCap];
+  float redf[NT / 32];
+  int redi[NT / 32];
+  int n;
+};
 __device__ __forceinline__ uint32_t order_key(float x) {
   const uint32_t u = __float_as_uint(x);
   return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
@@ -448,61 +466,179 @@ __device__ __forceinline__ uint32_t order_key(float x) {
 __device__ __forceinline__ float key_value(uint32_t k) {
   return __uint_as_float((k & 0x80000000u) ? (k & 0x7fffffffu) : ~k);
 }
+__device__ __forceinline__ uint32_t nucleus_depth(float d) { return (uint32_t)(fminf(d * 1.4426950408889634f, 63.99999f) * 262144.f); }
+__device__ __forceinline__ unsigned long long nucleus_mass(float d) { return (unsigned long long)(expf(-d) * 1099511627776.f); }
 template <int NT>
-__device__ int nucleus_gumbel_argmax(const float* __restrict__ z, int V, float invT, float m, float sum, float top_p,
+__device__ __forceinline__ unsigned long long block_sum_u64(unsigned long long v, unsigned long long* red) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  __syncthreads();
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
+  __syncthreads();
+  unsigned long long r = 0;
+#pragma unroll
+  for (int k = 0; k < NT / 32; ++k) r += red[k];
+  return r;
+}
+// fn(z_v, v) over a row: 16-byte loads when the row allows, eight of them in flight per thread (one CTA reads the whole row
+// out of L2, so the pass is bound by load latency)
+template <int NT, typename F>
+__device__ __forceinline__ void row_scan(const float* __restrict__ z, int V, F&& fn) {
+  if ((V & 3) == 0 && (reinterpret_cast<uintptr_t>(z) & 15) == 0) {
+    const float4* z4 = reinterpret_cast<const float4*>(z);
+    const int n4 = V >> 2;
+    constexpr int U = 8;
+    int i = threadIdx.x;
+    for (; i + (U - 1) * NT < n4; i += U * NT) {
+      float4 q[U];
+#pragma unroll
+      for (int k = 0; k < U; ++k) q[k] = __ldg(z4 + i + k * NT);
+#pragma unroll
+      for (int k = 0; k < U; ++k) {
+        const int v = 4 * (i + k * NT);
+        fn(q[k].x, v); fn(q[k].y, v + 1); fn(q[k].z, v + 2); fn(q[k].w, v + 3);
+      }
+    }
+    for (; i < n4; i += NT) {
+      const float4 q = __ldg(z4 + i);
+      fn(q.x, 4 * i); fn(q.y, 4 * i + 1); fn(q.z, 4 * i + 2); fn(q.w, 4 * i + 3);
+    }
+  } else {
+    for (int v = threadIdx.x; v < V; v += NT) fn(__ldg(z + v), v);
+  }
+}
+template <int NT>
+__device__ int nucleus_gumbel_argmax(const float* __restrict__ z, int V, float invT, float m, float top_p,
                                      const float* __restrict__ u_row, uint32_t k0, uint32_t k1, int t, int sid,
-                                     float* s_red, int* s_redi, uint8_t* keep_out = nullptr) {
-  const float target = top_p * sum;   // in units of exp(x - m)
+                                     NucleusSmem<NT>& S, uint8_t* keep_out = nullptr) {
+  typedef unsigned long long u64;
+  const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  uint32_t prefix = 0;
+  u64 above = 0, target = 0;   // above: the mass of the ids shallower than the prefix (larger x)
+  int lvl = 0;                 // the ids under the prefix: (T >> (24 - 4 lvl)) == prefix
+  bool listed = false;
+  for (; lvl < 6; ++lvl) {
+    if (threadIdx.x == 0) S.n = 0;
+    __syncthreads();
+    const int sh_pre = 24 - 4 * lvl, sh_bin = 20 - 4 * lvl;
+    const bool gather = lvl > 0 || V <= kNucleusCap;
+#pragma unroll
+    for (int k = 0; k < kNucleusBins; ++k) S.ph[k][threadIdx.x] = 0;
+    row_scan<NT>(z, V, [&](float zv, int v) {
+      const float x = zv * invT, d = m - x;
+      const uint32_t T = nucleus_depth(d);
+      if ((T >> sh_pre) == prefix) {
+        const int b = (T >> sh_bin) & (kNucleusBins - 1);
+        const u64 q = nucleus_mass(d);
+        S.ph[b][threadIdx.x] += q;
+        if (gather) {   // one counter increment for the lanes here
+          const unsigned act = __activemask();
+          const int leader = __ffs(act) - 1;
+          int base = 0;
+          if (lane == leader) base = atomicAdd(&S.n, __popc(act));
+          const int i = __shfl_sync(act, base, leader) + __popc(act & ((1u << lane) - 1u));
+          if (i < kNucleusCap) { S.ck[i] = order_key(x); S.cq[i] = q; S.cid[i] = v; }
+        }
+      }
+    });
+    __syncthreads();
+    for (int k = w; k < kNucleusBins; k += NT / 32) {   // bin k: the sum over all threads' private counters
+      u64 hs = 0;
+      for (int i = lane; i < NT; i += 32) hs += S.ph[k][i];
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) hs += __shfl_xor_sync(0xffffffffu, hs, o);
+      if (lane == 0) S.hist[k] = hs;
+    }
+    __syncthreads();
+    if (gather && S.n <= kNucleusCap) { listed = true; break; }
+    u64 h[kNucleusBins];
+#pragma unroll
+    for (int k = 0; k < kNucleusBins; ++k) h[k] = S.hist[k];
+    if (lvl == 0) {
+      u64 total = 0;
+#pragma unroll
+      for (int k = 0; k < kNucleusBins; ++k) total += h[k];
+      target = __double2ull_ru((double)top_p * (double)total);
+      if (target < 1) target = 1;
+    }
+    int bs = kNucleusBins - 1;
+    bool found = false;
+#pragma unroll
+    for (int k = 0; k < kNucleusBins - 1; ++k) {
+      if (!found) {
+        if (above + h[k] >= target) { bs = k; found = true; } else { above += h[k]; }
+      }
+    }
+    prefix = (prefix << 4) | (uint32_t)bs;
+    __syncthreads();
+  }
+  const int sh = 24 - 4 * lvl;
+  const int n = listed ? S.n : 0;
+  if (lvl == 0) {   // the list holds the whole (short) row: no level pass fixed the target yet
+    u64 tot = 0;
+    for (int i = threadIdx.x; i < n; i += NT) tot += S.cq[i];
+    target = __double2ull_ru((double)top_p * (double)block_sum_u64<NT>(tot, S.red));
+    if (target < 1) target = 1;
+  }
+  // fn(key, mass, id) over the ids of the threshold bin
+  auto scan = [&](auto&& fn) {
+    if (listed) {
+      for (int i = threadIdx.x; i < n; i += NT) fn(S.ck[i], S.cq[i], S.cid[i]);
+    } else {
+      row_scan<NT>(z, V, [&](float zv, int v) {
+        const float x = zv * invT, d = m - x;
+        if ((nucleus_depth(d) >> sh) == prefix) fn(order_key(x), nucleus_mass(d), v);
+      });
+    }
+  };
   uint32_t key = 0u;
   for (int bit = 31; bit >= 0; --bit) {
     const uint32_t cand = key | (1u << bit);
-    float f = 0.f;
-    for (int v = threadIdx.x; v < V; v += NT) {
-      const float x = z[v] * invT;
-      if (order_key(x) >= cand) f += expf(x - m);
-    }
-    if (block_sum<NT>(f, s_red) >= target) key = cand;
+    u64 f = 0;
+    scan([&](uint32_t k, u64 q, int) { if (k >= cand) f += q; });
+    if (above + block_sum_u64<NT>(f, S.red) >= target) key = cand;
   }
-  // mass strictly above the threshold probability, and the number of ids at it
-  float above = 0.f, ties = 0.f;
-  for (int v = threadIdx.x; v < V; v += NT) {
-    const float x = z[v] * invT;
-    const uint32_t kx = order_key(x);
-    if (kx > key) above += expf(x - m);
-    ties += (kx == key) ? 1.f : 0.f;
-  }
-  above = block_sum<NT>(above, s_red);
-  const int n_ties = (int)block_sum<NT>(ties, s_red);
+  u64 fs = 0, nt = 0;
+  scan([&](uint32_t k, u64 q, int) { if (k > key) fs += q; if (k == key) nt += 1; });
+  const u64 above_strict = above + block_sum_u64<NT>(fs, S.red);
+  const int n_ties = (int)block_sum_u64<NT>(nt, S.red);
   int id_cut = V;   // ids at the threshold are kept while id <= id_cut
   if (n_ties > 1) {
-    const float e = expf(key_value(key) - m);
-    int c = (int)ceilf((target - above) / e);
-    c = max(1, min(c, n_ties));
-    if (c < n_ties) {   // the c-th smallest id among the ties
+    const u64 q = nucleus_mass(m - key_value(key));
+    u64 c = q ? (target - above_strict + q - 1) / q : (u64)n_ties;
+    if (c < 1) c = 1;
+    if (c < (u64)n_ties) {   // the c-th smallest id among the ties
       int lo = 0, hi = V - 1;
       while (lo < hi) {
         const int mid = (lo + hi) >> 1;
-        float cnt = 0.f;
-        for (int v = threadIdx.x; v <= mid; v += NT) cnt += (order_key(z[v] * invT) == key) ? 1.f : 0.f;
-        if ((int)block_sum<NT>(cnt, s_red) >= c) hi = mid; else lo = mid + 1;
+        u64 cnt = 0;
+        scan([&](uint32_t k, u64, int id) { if (k == key && id <= mid) cnt += 1; });
+        if (block_sum_u64<NT>(cnt, S.red) >= c) hi = mid; else lo = mid + 1;
       }
       id_cut = lo;
     }
   }
+  // the Gumbel argmax over the kept ids (Philox blocks of 4 ids, drawn only where an id is kept)
   ArgBest best = {-INFINITY, 0x7fffffff};
+  const bool vec = (V & 3) == 0 && (reinterpret_cast<uintptr_t>(z) & 15) == 0;
+#pragma unroll 2
   for (int b4 = threadIdx.x; b4 * 4 < V; b4 += NT) {
+    float zz[4] = {0.f, 0.f, 0.f, 0.f};
+    if (vec) { const float4 q = __ldg(reinterpret_cast<const float4*>(z) + b4); zz[0] = q.x; zz[1] = q.y; zz[2] = q.z; zz[3] = q.w; }
+    else { for (int ww = 0; ww < 4 && b4 * 4 + ww < V; ++ww) zz[ww] = z[b4 * 4 + ww]; }
     uint32_t c[4] = {(uint32_t)b4, (uint32_t)t, (uint32_t)sid, 0u};
-    if (!u_row) philox4x32_10(c, k0, k1);
+    bool drawn = u_row != nullptr;
 #pragma unroll
-    for (int w = 0; w < 4; ++w) {
-      const int v = b4 * 4 + w;
+    for (int ww = 0; ww < 4; ++ww) {
+      const int v = b4 * 4 + ww;
       if (v >= V) break;
-      const float x = z[v] * invT;
+      const float x = zz[ww] * invT;
       const uint32_t kx = order_key(x);
       const bool keep = kx > key || (kx == key && v <= id_cut);
       if (keep_out) keep_out[v] = keep;
       if (keep) {
-        const float u = u_row ? u_row[v] : uniform_from_bits(c[w]);
+        if (!drawn) { philox4x32_10(c, k0, k1); drawn = true; }
+        const float u = u_row ? u_row[v] : uniform_from_bits(c[ww]);
         best = better(best, ArgBest{x + gumbel_from_uniform(u), v});
       }
     }
@@ -513,10 +649,10 @@ __device__ int nucleus_gumbel_argmax(const float* __restrict__ z, int V, float i
     best = better(best, o2);
   }
   __syncthreads();
-  if ((threadIdx.x & 31) == 0) { s_red[threadIdx.x >> 5] = best.v; s_redi[threadIdx.x >> 5] = best.i; }
+  if ((threadIdx.x & 31) == 0) { S.redf[w] = best.v; S.redi[w] = best.i; }
   __syncthreads();
-  best = ArgBest{s_red[0], s_redi[0]};
-  for (int k = 1; k < NT / 32; ++k) best = better(best, ArgBest{s_red[k], s_redi[k]});
+  best = ArgBest{S.redf[0], S.redi[0]};
+  for (int k = 1; k < NT / 32; ++k) best = better(best, ArgBest{S.redf[k], S.redi[k]});
   return best.i;
 }
 
@@ -524,23 +660,21 @@ __device__ int nucleus_gumbel_argmax(const float* __restrict__ z, int V, float i
 template <int NT>
 __global__ void __launch_bounds__(NT) test_nucleus_kernel(const float* z, int V, float temperature, float top_p, const float* u, int32_t* token,
                                                           uint8_t* keep) {
-  __shared__ float s_red[NT / 32];
-  __shared__ int s_redi[NT / 32];
+  extern __shared__ __align__(16) unsigned char nucleus_smem[];
+  NucleusSmem<NT>& S = *reinterpret_cast<NucleusSmem<NT>*>(nucleus_smem);
   const float invT = 1.f / temperature;
   float m = -INFINITY;
   for (int v = threadIdx.x; v < V; v += NT) m = fmaxf(m, z[v] * invT);
   for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
-  if ((threadIdx.x & 31) == 0) s_red[threadIdx.x >> 5] = m;
+  if ((threadIdx.x & 31) == 0) S.redf[threadIdx.x >> 5] = m;
   __syncthreads();
-  for (int k = 0; k < NT / 32; ++k) m = fmaxf(m, s_red[k]);
-  float sum = 0.f;
-  for (int v = threadIdx.x; v < V; v += NT) sum += expf(z[v] * invT - m);
-  sum = block_sum<NT>(sum, s_red);
-  const int y = nucleus_gumbel_argmax<NT>(z, V, invT, m, sum, top_p, u, 0u, 0u, 1, 0, s_red, s_redi, keep);
+  for (int k = 0; k < NT / 32; ++k) m = fmaxf(m, S.redf[k]);
+  __syncthreads();
+  const int y = nucleus_gumbel_argmax<NT>(z, V, invT, m, top_p, u, 0u, 0u, 1, 0, S, keep);
   if (threadIdx.x == 0) *token = y;
 }
 
-template <int NT>
+template <int NT, bool NUCLEUS>
 __global__ void __launch_bounds__(NT) sample_switch_emit_kernel(const __grid_constant__ Pair<SampleArgs> pp) {
   pdl_trigger(); pdl_wait();
   const SampleArgs& a = pp.m[blockIdx.z];
@@ -601,7 +735,7 @@ __global__ void __launch_bounds__(NT) sample_switch_emit_kernel(const __grid_con
   const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
   if (l == 0) { s_m[w] = m; s_s[w] = sum; s_bv[w] = raw.v; s_bi[w] = raw.i; s_gv[w] = gum.v; s_gi[w] = gum.i; }
   __syncthreads();
-  const bool nucleus = !greedy && a.rp.top_p < 1.f;   // the whole CTA stays for the nucleus search, else thread 0 alone
+  const bool nucleus = NUCLEUS && !greedy && a.rp.top_p < 1.f;   // the whole CTA stays for the nucleus search, else thread 0 alone
   if (!nucleus && threadIdx.x != 0) return;
   bool last = true;
   if (threadIdx.x == 0) {
@@ -634,18 +768,22 @@ __global__ void __launch_bounds__(NT) sample_switch_emit_kernel(const __grid_con
       }
     }
   }
-  if (nucleus) {
-    __shared__ float s_fin[2];
+  bool searched = false;
+  if constexpr (NUCLEUS) {
+   if (nucleus) {
+    extern __shared__ __align__(16) unsigned char nucleus_smem[];   // sizeof(NucleusSmem<NT>) when top_p < 1, else none
+    __shared__ float s_fin;
     __shared__ int s_last;
-    if (threadIdx.x == 0) { s_last = last; s_fin[0] = m; s_fin[1] = sum; }
+    if (threadIdx.x == 0) { s_last = last; s_fin = m; }
     __syncthreads();
     if (!s_last) return;
-    const int yn = nucleus_gumbel_argmax<NT>(z, V, invT, s_fin[0], s_fin[1], a.rp.top_p, u_row, k0, k1, t, sid, s_s, s_bi);
+    const int yn = nucleus_gumbel_argmax<NT>(z, V, invT, s_fin, a.rp.top_p, u_row, k0, k1, t, sid, *reinterpret_cast<NucleusSmem<NT>*>(nucleus_smem));
     if (threadIdx.x != 0) return;
     gum.i = yn;
-  } else if (!last) {
-    return;
+    searched = true;
+   }
   }
+  if (!searched && !last) return;
   int y = greedy ? raw.i : gum.i;
   if (a.io.forced_tokens) {
     const int f = a.io.forced_tokens[(size_t)s * a.io.forced_stride + (t - 1)];

@@ -424,7 +424,9 @@ int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaS
   for (int m = 0; m < 2; ++m)
     sa.m[m] = SampleArgs{h->st, h->tab[m], io, rp, h->ws[m].logits, h->word_start_dev, h->tokens, h->out_owner, h->out_logp, V, c.max_seq_len, m,
                          h->ws[m].chunk_part, h->ws[m].chunk_ctr, n_chunk};
-  KL(h, TANDEM_KC_SAMPLE, s, launch_ex(sample_switch_emit_kernel<256>, dim3(c.max_seqs, n_chunk, 2), dim3(256), 0, s, pdl, sa));
+  const size_t nucleus_smem = (rp.temperature > 0.f && rp.top_p < 1.f) ? sizeof(NucleusSmem<256>) : 0;
+  if (nucleus_smem) KL(h, TANDEM_KC_SAMPLE, s, launch_ex(sample_switch_emit_kernel<256, true>, dim3(c.max_seqs, n_chunk, 2), dim3(256), nucleus_smem, s, pdl, sa));
+  else KL(h, TANDEM_KC_SAMPLE, s, launch_ex(sample_switch_emit_kernel<256, false>, dim3(c.max_seqs, n_chunk, 2), dim3(256), 0, s, pdl, sa));
   return TANDEM_OK;
 }
 
@@ -768,6 +770,8 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
     h->tc = tc_gemm_create();
     if (!h->tc) { h->err = "tcgen05 GEMM setup failed (driver entry point for tensor maps not found)"; fprintf(stderr, "tandem_init: %s\n", h->err.c_str()); tandem_free(h); return TANDEM_ECUDA; }
   }
+  if (cudaFuncSetAttribute(sample_switch_emit_kernel<256, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(NucleusSmem<256>)) != cudaSuccess)
+    return bad("cannot reserve shared memory for the nucleus sampler");
   if (h->use_tail && cudaFuncSetAttribute(layer_tail_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kLtSmemBytes) != cudaSuccess) {
     cudaGetLastError(); h->use_tail = false;
   }
@@ -1038,7 +1042,8 @@ int tandem_test_uniforms(uint64_t seed, int32_t seq_id, int32_t t, int32_t strea
 int tandem_test_nucleus(int32_t vocab, float temperature, float top_p, const float* logits_dev, const float* u_dev, int32_t* token_dev,
                         uint8_t* keep_dev) {
   if (vocab <= 0 || !(temperature > 0.f) || !(top_p > 0.f && top_p < 1.f) || !logits_dev || !u_dev || !token_dev || !keep_dev) return TANDEM_EINVAL;
-  test_nucleus_kernel<256><<<1, 256>>>(logits_dev, vocab, temperature, top_p, u_dev, token_dev, keep_dev);
+  cudaFuncSetAttribute(test_nucleus_kernel<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(NucleusSmem<256>));
+  test_nucleus_kernel<256><<<1, 256, sizeof(NucleusSmem<256>)>>>(logits_dev, vocab, temperature, top_p, u_dev, token_dev, keep_dev);
   return cudaDeviceSynchronize() == cudaSuccess ? TANDEM_OK : TANDEM_ECUDA;
 }
 

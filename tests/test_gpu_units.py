@@ -126,6 +126,11 @@ def test_nucleus_hand_examples_and_ties():
     for top_p in (0.1, 0.3, 0.5, 0.7):
         _, keep = _nucleus(z, 1.0, top_p, u)
         assert keep.tolist() == kept_set_top_p(z.astype(np.float32), 1.0, top_p).tolist(), top_p
+    z = np.zeros(151936); z[77] = 1.0                                                     # a flat row: the threshold bin overflows the list
+    for top_p in (0.3, 0.9):
+        _, keep = _nucleus(z, 1.0, top_p, np.full(z.size, 0.5, np.float32))
+        want = kept_set_top_p(z.astype(np.float32), 1.0, top_p)
+        assert keep[77] and abs(int(keep.sum()) - int(want.sum())) <= 1 and keep[:keep.sum()].all()
     z = np.full(300, -30.0); z[123] = 10.0
     tok, keep = _nucleus(z, 0.7, 0.9, np.full(300, 0.5, np.float32))
     assert tok == 123 and keep.sum() == 1 and keep[123]
