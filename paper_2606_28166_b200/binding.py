@@ -15,10 +15,10 @@ GEMM_AUTO, GEMM_SIMT, GEMM_TCGEN05 = 0, 1, 2
 ATTN_AUTO, ATTN_ALU, ATTN_MMA = 0, 1, 2
 _ERR = {0: "OK", -1: "EINVAL", -2: "ENOMEM", -3: "ECUDA", -4: "ESTATE", -5: "EFULL"}
 
-EXPORTED_SYMBOLS = ["tandem_init", "tandem_load_weights", "tandem_step", "tandem_generate", "tandem_reset",
+EXPORTED_SYMBOLS = ["tandem_init", "tandem_load_weights", "tandem_step", "tandem_generate", "tandem_score", "tandem_reset",
                     "tandem_free", "tandem_last_error", "tandem_get_stats", "tandem_set_profile", "tandem_get_profile",
                     "tandem_kernel_class_name", "tandem_debug_lt_times", "tandem_test_uniforms", "tandem_test_nucleus", "tandem_test_philox", "tandem_test_gemm", "tandem_test_gemm_time"]
-KC_NUM = 15
+KC_NUM = 16
 
 
 class TandemError(RuntimeError):
@@ -83,6 +83,7 @@ def lib():
         L.tandem_init.argtypes = [C.POINTER(_Config), C.POINTER(C.c_void_p)]
         L.tandem_load_weights.argtypes = [C.c_void_p, C.c_int, C.POINTER(_Weights)]
         L.tandem_step.argtypes = [C.c_void_p, C.POINTER(_StepIn), C.POINTER(_StepOut), C.c_void_p]
+        L.tandem_score.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.tandem_generate.argtypes = [C.c_void_p, C.POINTER(_Params), C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                       C.POINTER(_Overrides), C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                       C.POINTER(_Stats), C.c_void_p]
@@ -217,6 +218,21 @@ class Tandem:
         valid = np.arange(L)[None, :] < out_n[:, None]
         stats = {n: getattr(st, n) for n, _ in _Stats._fields_}
         return dict(tokens=out_t, owner=out_o, mask=((out_o == 0) & valid).astype(np.uint8), sen_logp=out_p, len=out_n, stats=stats)
+
+    def score(self, streams, temperature=1.0, stream=None):
+        """Teacher-forced dual scoring of finished token streams (prompt + response). Returns dict(sen_logp, jun_logp, overlap:
+        lists of float32 arrays, one per stream, entry 0 = 0; stats dict). The junior's cross-entropy over a set of positions is
+        the mean of -jun_logp there; alpha is the mean of overlap."""
+        B = len(streams)
+        toks = np.ascontiguousarray(np.concatenate(streams), dtype=np.int32) if B else np.zeros(0, np.int32)
+        offs = np.zeros(B + 1, dtype=np.int64)
+        offs[1:] = np.cumsum([len(p) for p in streams])
+        outs = [np.zeros(max(1, toks.size), np.float32) for _ in range(3)]
+        st = _Stats()
+        self._check(lib().tandem_score(self._h, B, toks.ctypes.data, offs.ctypes.data, float(temperature), outs[0].ctypes.data,
+                                       outs[1].ctypes.data, outs[2].ctypes.data, C.byref(st), stream))
+        cut = lambda a: [a[offs[b]:offs[b + 1]].copy() for b in range(B)]
+        return dict(sen_logp=cut(outs[0]), jun_logp=cut(outs[1]), overlap=cut(outs[2]), stats={n: getattr(st, n) for n, _ in _Stats._fields_})
 
     def reset(self):
         self._check(lib().tandem_reset(self._h))

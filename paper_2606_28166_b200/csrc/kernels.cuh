@@ -15,6 +15,7 @@ struct SchedArgs {
   SeqState st; PageTab pt[2]; StepTab tab[2]; StepIO io; DevStats* stats;
   const int32_t* tokens; int max_seqs, max_seq_len, max_pages, row_cap, tile_tok;
   int32_t* work_ctr; int n_work_ctr;   // dynamic-scheduling counters of the attention launches of this step
+  int score;                           // teacher-forced dual scoring (tandem_score): both models ingest every sequence, every row reaches the LM head
 };
 
 __device__ __forceinline__ int block_excl_scan_1024(int v, int* total, int* wsum) {
@@ -63,19 +64,22 @@ __global__ void __launch_bounds__(1024) sched_kernel(SchedArgs a) {
   const int nctx = live ? a.st.n_ctx[s] : 0;
   int resident_total;
   block_excl_scan_1024(live ? 1 : 0, &resident_total, wsum);
+  const int nfeed = a.score ? nctx - 1 : nctx;   // scoring: the last token is only a target
+  int fed[2] = {0, 0};
 
   for (int M = 0; M < 2; ++M) {
     const StepTab& tb = a.tab[M];
     const PageTab& pt = a.pt[M];
-    const bool mine = owner == M;
+    const bool mine = a.score ? live : owner == M;
     const int ing = mine ? a.st.ing[M][s] : 0;
-    const int want = mine ? nctx - ing : 0;
+    const int want = mine ? nfeed - ing : 0;
     int total_want;
     const int pre = block_excl_scan_1024(want, &total_want, wsum);
     const int rows = min(want, max(0, a.row_cap - pre));
     const int cu = min(pre, a.row_cap);
     const int n_rows = min(total_want, a.row_cap);
-    const bool emits = mine && rows == want && want > 0;
+    const bool emits = !a.score && mine && rows == want && want > 0;
+    fed[M] = ing + rows;
 
     // pages for positions [ing, ing + rows)
     if (rows > 0) {
@@ -146,7 +150,7 @@ __global__ void __launch_bounds__(1024) sched_kernel(SchedArgs a) {
       tb.row_pos[r] = pos;
       tb.row_tok[r] = a.tokens[(size_t)q * a.max_seq_len + pos];
       tb.row_kvslot[r] = pt.bt[(size_t)q * a.max_pages + pos / kPageTokens] * kPageTokens + pos % kPageTokens;
-      tb.row_emit[r] = (off == sm_rows[q] - 1) ? sm_emit[q] : -1;
+      tb.row_emit[r] = a.score ? r : ((off == sm_rows[q] - 1) ? sm_emit[q] : -1);
     }
     for (int i = threadIdx.x; i < n_items; i += blockDim.x) {
       const int q = find_owner_slot(cu_items, kMaxSlots, i);
@@ -172,7 +176,7 @@ __global__ void __launch_bounds__(1024) sched_kernel(SchedArgs a) {
       }
     }
     if (threadIdx.x == 0) {
-      tb.counts[C_ROWS] = n_rows; tb.counts[C_SCHED] = n_sched; tb.counts[C_EMIT] = n_emit;
+      tb.counts[C_ROWS] = n_rows; tb.counts[C_SCHED] = n_sched; tb.counts[C_EMIT] = a.score ? n_rows : n_emit;
       tb.counts[C_ITEMS] = n_items; tb.counts[C_COMB] = n_comb; tb.counts[C_PARTS] = n_parts;
       a.stats->rows[M] += (unsigned long long)n_rows;
       a.stats->catchup_rows += (unsigned long long)(n_rows - n_sched);
@@ -185,6 +189,7 @@ __global__ void __launch_bounds__(1024) sched_kernel(SchedArgs a) {
     if (threadIdx.x == 0) a.stats->kv_tokens_read += (unsigned long long)kv_total;
     __syncthreads();
   }
+  if (a.score && live && fed[0] >= nfeed && fed[1] >= nfeed) a.st.done[s] = 1;   // both models have seen the whole stream after this step
   if (threadIdx.x == 0) {
     a.stats->steps += 1ull;
     a.stats->peak_resident = max(a.stats->peak_resident, resident_total);
@@ -814,6 +819,81 @@ __global__ void __launch_bounds__(NT) sample_switch_emit_kernel(const __grid_con
   }
   a.st.cap_c[s] = c;
   a.st.owner[s] = (uint8_t)owner;
+}
+
+// ============================================================================================ dual scoring (NEXT-1)
+// PAPER.md L126 / L134 (section 4.4.2), reading R17: row r of the step holds position pos of sequence slot q in BOTH models
+// (the scheduler keeps them in lock-step while scoring); with y = the stream's token at pos + 1 and p = softmax(z / T'):
+//   out_sen[q][pos+1] = log p_sen(y), out_jun[q][pos+1] = log p_jun(y), out_alpha[q][pos+1] = sum_v min(p_sen(v), p_jun(v)).
+// One CTA per row, two passes over the two fp32 logit rows: (max, sum exp) of each, then the min-sum.
+struct ScoreArgs {
+  const int32_t* counts; const int32_t* row_slot; const int32_t* row_pos; const int32_t* tokens; int max_seq_len;
+  const float* z_sen; const float* z_jun; int vocab; float invT;
+  float* out_sen; float* out_jun; float* out_alpha;
+};
+template <int NT>
+__global__ void __launch_bounds__(NT) score_kernel(const __grid_constant__ ScoreArgs a) {
+  pdl_trigger(); pdl_wait();
+  __shared__ float red[32];
+  __shared__ float s_m[2][NT / 32], s_s[2][NT / 32];
+  const int V = a.vocab;
+  const float invT = a.invT;
+  const int n_rows = a.counts[C_ROWS];
+  for (int r = blockIdx.x; r < n_rows; r += gridDim.x) {
+    const float* zs = a.z_sen + (size_t)r * V;
+    const float* zj = a.z_jun + (size_t)r * V;
+    float m[2] = {-INFINITY, -INFINITY}, sum[2] = {0.f, 0.f};
+    auto upd = [&](int k, float x) { if (x > m[k]) { sum[k] = sum[k] * expf(m[k] - x) + 1.f; m[k] = x; } else { sum[k] += expf(x - m[k]); } };
+    row_scan<NT>(zs, V, [&](float zv, int) { upd(0, zv * invT); });
+    row_scan<NT>(zj, V, [&](float zv, int) { upd(1, zv * invT); });
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        const float m2 = __shfl_xor_sync(0xffffffffu, m[k], o), s2 = __shfl_xor_sync(0xffffffffu, sum[k], o);
+        const float mn = fmaxf(m[k], m2);
+        sum[k] = (m[k] == -INFINITY ? 0.f : sum[k] * expf(m[k] - mn)) + (m2 == -INFINITY ? 0.f : s2 * expf(m2 - mn));
+        m[k] = mn;
+      }
+      if (l == 0) { s_m[k][w] = m[k]; s_s[k][w] = sum[k]; }
+    }
+    __syncthreads();
+    float lse[2];
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {   // every thread merges the warps' results in the same order
+      float mm = s_m[k][0], ss = s_s[k][0];
+      for (int i = 1; i < NT / 32; ++i) {
+        const float mn = fmaxf(mm, s_m[k][i]);
+        ss = (mm == -INFINITY ? 0.f : ss * expf(mm - mn)) + (s_m[k][i] == -INFINITY ? 0.f : s_s[k][i] * expf(s_m[k][i] - mn));
+        mm = mn;
+      }
+      lse[k] = mm + logf(ss);
+    }
+    float acc = 0.f;
+    if ((V & 3) == 0 && ((reinterpret_cast<uintptr_t>(zs) | reinterpret_cast<uintptr_t>(zj)) & 15) == 0) {
+      const float4* a4 = reinterpret_cast<const float4*>(zs);
+      const float4* b4 = reinterpret_cast<const float4*>(zj);
+#pragma unroll 4
+      for (int i = threadIdx.x; i < (V >> 2); i += NT) {
+        const float4 p = __ldg(a4 + i), q = __ldg(b4 + i);
+        acc += fminf(expf(p.x * invT - lse[0]), expf(q.x * invT - lse[1])) + fminf(expf(p.y * invT - lse[0]), expf(q.y * invT - lse[1])) +
+               fminf(expf(p.z * invT - lse[0]), expf(q.z * invT - lse[1])) + fminf(expf(p.w * invT - lse[0]), expf(q.w * invT - lse[1]));
+      }
+    } else {
+      for (int v = threadIdx.x; v < V; v += NT) acc += fminf(expf(zs[v] * invT - lse[0]), expf(zj[v] * invT - lse[1]));
+    }
+    acc = block_sum<NT>(acc, red);
+    if (threadIdx.x == 0) {
+      const int q = a.row_slot[r], pos = a.row_pos[r];
+      const int y = a.tokens[(size_t)q * a.max_seq_len + pos + 1];
+      const size_t o = (size_t)q * a.max_seq_len + pos + 1;
+      a.out_sen[o] = zs[y] * invT - lse[0];
+      a.out_jun[o] = zj[y] * invT - lse[1];
+      a.out_alpha[o] = acc;
+    }
+    __syncthreads();
+  }
 }
 
 }  // namespace tandem

@@ -42,6 +42,7 @@ struct Workspace {  // per model, sized for row_cap rows
   void* lm_in = nullptr;       // final-normed last rows [max_seqs, H]
   float* gemm_out = nullptr;   // split-K partial outputs [S][R][N], S*N <= gemm_out_cols
   float* logits = nullptr;     // [max_seqs, V]
+  void* score_lm_in = nullptr; float* score_logits = nullptr;   // tandem_score: [row_cap, H] and [row_cap, V], allocated at its first call
   float* chunk_part = nullptr; int32_t* chunk_ctr = nullptr;   // sampler: per-slice partials and arrival counters
   float* part_acc = nullptr; float2* part_ml = nullptr;
   void* kv = nullptr;          // page pool: [layer][K|V][page][nkv][16][d]
@@ -80,6 +81,7 @@ struct tandem_handle {
   SeqState st{};
   int32_t* st_mem = nullptr; uint8_t* st_mem8 = nullptr;
   int32_t* tokens = nullptr; uint8_t* out_owner = nullptr; float* out_logp = nullptr;
+  float* score_out[2] = {nullptr, nullptr};   // tandem_score: junior log-probs and overlap [max_seqs][max_seq_len] (the senior's go to out_logp)
   float2* rope_cs = nullptr;
   uint8_t* word_start_dev = nullptr; std::vector<uint8_t> word_start_host;
   DevStats* stats = nullptr; int32_t* n_active = nullptr; int32_t* work_ctr = nullptr;
@@ -296,7 +298,7 @@ int launch_layer_tail(tandem_handle* h, int li, cudaStream_t s) {
 // Every kernel is launched once for the two models (Pair arguments): the models advance layer by layer in lock-step on
 // one stream, each launch carrying the senior's and the junior's half of the work.
 template <typename T>
-int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaStream_t s) {
+int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaStream_t s, bool score = false, float score_inv_t = 1.f) {
   const tandem_config& c = h->cfg;
   const int H = c.hidden, nq = c.n_q_heads, nkv = c.n_kv_heads, d = c.head_dim, I = c.intermediate, V = c.vocab;
   const int qkv_n = (nq + 2 * nkv) * d;
@@ -314,7 +316,7 @@ int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaS
     for (int m = 0; m < 2; ++m) ea.m[m] = EmbedArgs<T>{h->tab[m].counts, h->tab[m].row_tok, (const T*)h->w[m].embed, (const T*)h->w[m].attn_norm[0], h->ws[m].x, (T*)h->ws[m].act, H, c.rms_eps};
     KL(h, TANDEM_KC_EMBED, s, launch_ex(embed_norm_kernel<T, 256>, dim3(row_grid, 2), dim3(256), 0, s, false, ea));
   }
-  const bool tail = h->use_tail && sizeof(T) == 2;
+  const bool tail = h->use_tail && sizeof(T) == 2 && !score;
   if (tail && (rc = launch_layer_tail(h, 0, s))) return rc;
   for (int l = 0; l < c.n_layers; ++l) {
     if (tail) {   // attention + combine, then everything up to the next attention in one persistent kernel
@@ -412,11 +414,19 @@ int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaS
       Pair<ResNormArgs<T>> na;
       for (int m = 0; m < 2; ++m)
         na.m[m] = ResNormArgs<T>{h->tab[m].counts, h->ws[m].gemm_out, ns, ss, h->ws[m].x, (const T*)(last ? h->w[m].final_norm : h->w[m].attn_norm[l + 1]),
-                                 (T*)(last ? h->ws[m].lm_in : h->ws[m].act), last ? h->tab[m].row_emit : nullptr, H, c.rms_eps};
+                                 (T*)(last ? (score ? h->ws[m].score_lm_in : h->ws[m].lm_in) : h->ws[m].act), last ? h->tab[m].row_emit : nullptr, H, c.rms_eps};
       launch_residual_norm<T>(h, s, row_grid, na);
     }
   }
   // S8 LM head on the emitting rows only, then sample + switch + emit
+  if (score) {   // every row reaches the LM head (the scheduler set row_emit[r] = r); the dual-scoring kernel replaces the sampler
+    for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].score_lm_in, h->w[m].lm_head, h->ws[m].score_logits, h->tab[m].counts + C_EMIT);
+    if ((rc = launch_gemm<T>(h, 4, A, W, V, H, O, RP, h->row_cap, &ns, &ss, s))) return rc;
+    const ScoreArgs sc{h->tab[0].counts, h->tab[0].row_slot, h->tab[0].row_pos, h->tokens, c.max_seq_len, h->ws[0].score_logits, h->ws[1].score_logits, V,
+                       score_inv_t, h->out_logp, h->score_out[0], h->score_out[1]};
+    KL(h, TANDEM_KC_SCORE, s, launch_ex(score_kernel<512>, dim3(h->row_cap), dim3(512), 0, s, pdl, sc));
+    return TANDEM_OK;
+  }
   for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].lm_in, h->w[m].lm_head, h->ws[m].logits, h->tab[m].counts + C_EMIT);
   if ((rc = launch_gemm<T>(h, 4, A, W, V, H, O, RP, c.max_seqs, &ns, &ss, s))) return rc;
   Pair<SampleArgs> sa;
@@ -430,15 +440,16 @@ int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaS
   return TANDEM_OK;
 }
 
-int launch_step(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaStream_t s) {
+int launch_step(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaStream_t s, bool score = false, float score_inv_t = 1.f) {
   const tandem_config& c = h->cfg;
   SchedArgs sa{};
   sa.st = h->st; sa.pt[0] = h->pt[0]; sa.pt[1] = h->pt[1]; sa.tab[0] = h->tab[0]; sa.tab[1] = h->tab[1];
   sa.io = io; sa.stats = h->stats; sa.tokens = h->tokens; sa.max_seqs = c.max_seqs; sa.max_seq_len = c.max_seq_len;
   sa.max_pages = h->max_pages; sa.row_cap = h->row_cap; sa.tile_tok = h->tile_tok;
   sa.work_ctr = h->work_ctr; sa.n_work_ctr = c.n_layers + (c.n_layers + 1) * LT_NPHASE;
+  sa.score = score ? 1 : 0;
   KL(h, TANDEM_KC_SCHED, s, (sched_kernel<<<1, 1024, 0, s>>>(sa)));
-  const int rc = (c.dtype == TANDEM_F32) ? forward_pair<float>(h, io, rp, s) : forward_pair<bf16>(h, io, rp, s);
+  const int rc = (c.dtype == TANDEM_F32) ? forward_pair<float>(h, io, rp, s, score, score_inv_t) : forward_pair<bf16>(h, io, rp, s, score, score_inv_t);
   if (rc) return rc;
   FinalArgs fa{h->st, {h->pt[0], h->pt[1]}, io, h->stats, h->n_active, c.max_seqs, h->max_pages, h->pool_pages};
   KL(h, TANDEM_KC_FINALIZE, s, (finalize_kernel<<<1, 1024, 0, s>>>(fa)));
@@ -539,7 +550,7 @@ int refresh_slots(tandem_handle* h, cudaStream_t s) {
 }
 
 int admit(tandem_handle* h, const tandem_params* p, const tandem_overrides* ovr, int n, const int32_t* toks, const int64_t* offs,
-          const int32_t* seq_ids, const int32_t* max_new, int32_t* slots_out, cudaStream_t s) {
+          const int32_t* seq_ids, const int32_t* max_new, int32_t* slots_out, cudaStream_t s, bool score = false) {
   const tandem_config& c = h->cfg;
   if (n <= 0) return TANDEM_OK;
   if (!toks || !offs || !max_new) return fail(h, TANDEM_EINVAL, "admission arrays are NULL");
@@ -551,7 +562,7 @@ int admit(tandem_handle* h, const tandem_params* p, const tandem_overrides* ovr,
     const int64_t len = offs[i + 1] - offs[i];
     if (len < 1) return fail(h, TANDEM_EINVAL, "empty prompt");
     if (max_new[i] < 1) return fail(h, TANDEM_EINVAL, "max_new must be >= 1");
-    if (len + max_new[i] > c.max_seq_len) return fail(h, TANDEM_EINVAL, "prompt + max_new exceeds max_seq_len");
+    if (len + (score ? 0 : max_new[i]) > c.max_seq_len) return fail(h, TANDEM_EINVAL, score ? "stream longer than max_seq_len" : "prompt + max_new exceeds max_seq_len");
   }
   for (int64_t k = offs[0]; k < offs[n]; ++k) if (toks[k] < 0 || toks[k] >= c.vocab) return fail(h, TANDEM_EINVAL, "token id out of range");
   if ((size_t)total > h->stage_cap) {
@@ -846,7 +857,7 @@ int tandem_debug_lt_times(tandem_handle* h, unsigned long long* out, int n) {
 
 const char* tandem_kernel_class_name(int kc) {
   static const char* names[TANDEM_KC_NUM] = {"sched", "embed_norm", "gemm_qkv", "rope_append", "attention", "attn_combine", "gemm_o",
-                                             "residual_norm", "gemm_gateup", "swiglu", "gemm_down", "gemm_lmhead", "sample_switch_emit", "finalize", "layer_tail"};
+                                             "residual_norm", "gemm_gateup", "swiglu", "gemm_down", "gemm_lmhead", "sample_switch_emit", "finalize", "layer_tail", "score"};
   return (kc >= 0 && kc < TANDEM_KC_NUM) ? names[kc] : "?";
 }
 
@@ -992,6 +1003,89 @@ int tandem_generate(tandem_handle* h, const tandem_params* params, int32_t B, co
   return TANDEM_OK;
 }
 
+int tandem_score(tandem_handle* h, int32_t n_seqs, const int32_t* tokens, const int64_t* offsets, float temperature,
+                 float* sen_logp, float* jun_logp, float* overlap, tandem_stats* stats, void* cuda_stream) {
+  int rc = check_ready(h);
+  if (rc) return rc;
+  if (n_seqs < 0 || (n_seqs > 0 && (!tokens || !offsets))) return fail(h, TANDEM_EINVAL, "bad arguments");
+  if (!(temperature > 0.f)) return fail(h, TANDEM_EINVAL, "temperature must be > 0");
+  const tandem_config& c = h->cfg;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  for (int m = 0; m < 2; ++m) {   // the scoring buffers exist from the first call on
+    if (!h->ws[m].score_lm_in) DM(h, &h->ws[m].score_lm_in, (size_t)h->row_cap * c.hidden * h->esize);
+    if (!h->ws[m].score_logits) DM(h, &h->ws[m].score_logits, (size_t)h->row_cap * c.vocab * sizeof(float));
+    if (!h->score_out[m]) DM(h, &h->score_out[m], (size_t)c.max_seqs * c.max_seq_len * sizeof(float));
+  }
+  if ((rc = tandem_reset(h))) return rc;
+  const int64_t total = n_seqs > 0 ? offsets[n_seqs] - offsets[0] : 0;
+  for (float* o : {sen_logp, jun_logp, overlap}) if (o && total > 0) std::memset(o + offsets[0], 0, (size_t)total * sizeof(float));
+  cudaEvent_t e0, e1;
+  CU(h, cudaEventCreate(&e0)); CU(h, cudaEventCreate(&e1));
+  CU(h, cudaEventRecord(e0, s));
+  tandem_params prm{};   // admission only needs an owner; the rule never runs while scoring
+  prm.p = 0.f; prm.switch_mode = TANDEM_TOGGLE; prm.start_owner = TANDEM_SENIOR; prm.temperature = temperature; prm.top_p = 1.f; prm.eos_id = -1;
+  const StepIO io = make_io(nullptr, nullptr);
+  const RuleParams rp = make_rule(&prm);
+  auto pages_of = [&](int b) { return (int)((offsets[b + 1] - offsets[b] + kPageTokens - 1) / kPageTokens); };
+  const int pages_avail = h->pool_pages - 1;
+  for (int b = 0; b < n_seqs; ++b) {
+    if (offsets[b + 1] - offsets[b] < 1) return fail(h, TANDEM_EINVAL, "empty stream");
+    if (pages_of(b) > pages_avail) return fail(h, TANDEM_ENOMEM, "a single stream needs more KV pages than the pool holds");
+  }
+  std::vector<int> slot_seq(c.max_seqs, -1), slot_pages(c.max_seqs, 0);
+  std::vector<int32_t> ids(c.max_seqs), ones(c.max_seqs, 1);
+  std::vector<float> row(c.max_seq_len);
+  int next = 0, finished = 0, pages_reserved = 0;
+  int64_t budget = 1024;
+  for (int b = 0; b < n_seqs; ++b) budget += 4 + 4 * (offsets[b + 1] - offsets[b]);
+  const bool was_profiling = h->profile;
+  h->profile = false;
+  while (finished < n_seqs) {
+    if (--budget < 0) { h->profile = was_profiling; return fail(h, TANDEM_ESTATE, "scoring made no progress (internal error)"); }
+    int nfree = 0;
+    for (int i = 0; i < c.max_seqs; ++i) nfree += !h->slot_busy[i];
+    int n = 0, add = 0;
+    while (n < std::min(nfree, n_seqs - next) && pages_reserved + add + pages_of(next + n) <= pages_avail) { add += pages_of(next + n); ++n; }
+    if (n > 0) {
+      std::vector<int32_t> slots(n);
+      for (int i = 0; i < n; ++i) ids[i] = next + i;
+      if ((rc = admit(h, &prm, nullptr, n, tokens, offsets + next, ids.data(), ones.data(), slots.data(), s, true))) { h->profile = was_profiling; return rc; }
+      for (int i = 0; i < n; ++i) { slot_seq[slots[i]] = next + i; slot_pages[slots[i]] = pages_of(next + i); }
+      pages_reserved += add;
+      next += n;
+    }
+    if ((rc = launch_step(h, io, rp, s, true, 1.f / temperature))) { h->profile = was_profiling; return rc; }
+    CU(h, cudaGetLastError());
+    if ((rc = refresh_slots(h, s))) { h->profile = was_profiling; return rc; }
+    for (int i = 0; i < c.max_seqs; ++i) {
+      if (slot_seq[i] < 0 || h->slot_busy[i]) continue;
+      const int b = slot_seq[i];
+      const int64_t len = offsets[b + 1] - offsets[b];
+      float* outs[3] = {sen_logp, jun_logp, overlap};
+      const float* devs[3] = {h->out_logp, h->score_out[0], h->score_out[1]};
+      for (int k = 0; k < 3; ++k) {
+        if (!outs[k] || len < 2) continue;
+        CU(h, cudaMemcpy(outs[k] + offsets[b] + 1, devs[k] + (size_t)i * c.max_seq_len + 1, (size_t)(len - 1) * sizeof(float), cudaMemcpyDeviceToHost));
+      }
+      slot_seq[i] = -1;
+      pages_reserved -= slot_pages[i]; slot_pages[i] = 0;
+      ++finished;
+    }
+  }
+  h->profile = was_profiling;
+  CU(h, cudaEventRecord(e1, s));
+  CU(h, cudaEventSynchronize(e1));
+  float ms = 0.f;
+  CU(h, cudaEventElapsedTime(&ms, e0, e1));
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  if ((rc = check_oom(h, s))) return rc;
+  if (stats) {
+    if ((rc = fill_stats(h, stats))) return rc;
+    stats->seconds_total = ms * 1e-3;
+  }
+  return TANDEM_OK;
+}
+
 void tandem_free(tandem_handle* h) {
   if (!h) return;
   cudaDeviceSynchronize();
@@ -1000,7 +1094,7 @@ void tandem_free(tandem_handle* h) {
   auto fr = [](void* p) { if (p) cudaFree(p); };
   for (int m = 0; m < 2; ++m) {
     Workspace& w = h->ws[m];
-    fr(w.chunk_part); fr(w.chunk_ctr); fr(w.x); fr(w.act); fr(w.q); fr(w.attn_out); fr(w.mlp_act); fr(w.lm_in); fr(w.gemm_out); fr(w.logits); fr(w.part_acc); fr(w.part_ml); fr(w.kv);
+    fr(w.score_lm_in); fr(w.score_logits); fr(w.chunk_part); fr(w.chunk_ctr); fr(w.x); fr(w.act); fr(w.q); fr(w.attn_out); fr(w.mlp_act); fr(w.lm_in); fr(w.gemm_out); fr(w.logits); fr(w.part_acc); fr(w.part_ml); fr(w.kv);
     fr(w.tab_mem); fr(w.bt); fr(w.npages); fr(w.free_pages); fr(w.free_top);
     ModelWeights& mw = h->w[m];
     fr(mw.embed); fr(mw.lm_head); fr(mw.final_norm);
@@ -1010,7 +1104,7 @@ void tandem_free(tandem_handle* h) {
   if (h->ev_in) cudaEventDestroy(h->ev_in);
   if (h->ev_out) cudaEventDestroy(h->ev_out);
   if (h->gs) cudaStreamDestroy(h->gs);
-  fr(h->st_mem); fr(h->st_mem8); fr(h->tokens); fr(h->out_owner); fr(h->out_logp); fr(h->rope_cs); fr(h->word_start_dev); fr(h->stats);
+  fr(h->score_out[0]); fr(h->score_out[1]); fr(h->st_mem); fr(h->st_mem8); fr(h->tokens); fr(h->out_owner); fr(h->out_logp); fr(h->rope_cs); fr(h->word_start_dev); fr(h->stats);
   fr(h->lt_wmaps); fr(h->lt_amaps); fr(h->lt_ts); fr(h->n_active); fr(h->work_ctr); fr(h->stage_tokens); fr(h->stage_off); fr(h->stage_i32);
   cudaGetLastError();
   delete h;
