@@ -45,6 +45,9 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg3_4b_bf16")
     ap.add_argument("--p", type=float, default=None, help="override the workload's switch probability (cfg5 sweep)")
+    ap.add_argument("--score", type=int, default=0, help="N > 0: time tandem_score (teacher-forced dual scoring, NEXT-1) on N synthetic streams instead of the rollout")
+    ap.add_argument("--score-len", type=int, default=2048, help="tokens per stream for --score")
+    ap.add_argument("--score-rows", type=int, default=512, help="rows per step and model for --score (max_rows_per_step)")
     ap.add_argument("--top-p", type=float, default=None, help="override the workload's top-p (the paper trains at 1.0, evaluates at 0.8)")
     ap.add_argument("--word-start-frac", type=float, default=None, help="override the word-start table density (cfg5 sweep)")
     ap.add_argument("--fast-forward", type=int, default=-1,
@@ -244,6 +247,56 @@ def run_full_rollout(args):
                       "step_roofline": {"bound": "hbm", "achieved": gbs, "unit": "GB/s", "frac_of_measured": gbs / pk["hbm_gbs"], "frac_of_8TBs": gbs / NOMINAL_HBM_GBS},
                       "e2e": {"value": tok / dt, "unit": "tokens/s", "h2d_bytes_per_step": sum(len(p) for p in prompts) * 4 / max(1, st["steps"]),
                               "d2h_bytes_per_step": tok * 9 / max(1, st["steps"])}}))
+    eng.free()
+
+
+def run_score(args):
+    """tandem_score on N streams of the workload's shape (host buffers in and out): both models read every stream through the
+    ragged prefill path, every position reaches the LM head, and the score kernel reduces the two logit rows to (log p_sen(y),
+    log p_jun(y), alpha). A few positions are checked against oracle.dual_score when the shape is small enough to afford it."""
+    import torch
+    import paper_2606_28166_b200 as T
+    from workloads import get_workload, make_weights
+    torch.cuda.set_device(0)
+    T.build()
+    wl = get_workload(args.workload)
+    shape = wl.shape
+    N, L = args.score, args.score_len
+    rng = np.random.default_rng(wl.seeds["prompts"] if "prompts" in wl.seeds else 1)
+    streams = [rng.integers(0, shape.vocab, size=L).astype(np.int32) for _ in range(N)]
+    max_seqs = min(N, 64)
+    kv = (max_seqs + 1) * ((L + 15) // 16 + 1) * shape.kv_elems_per_token * 2 * 16
+    eng = T.Tandem(T.TandemConfig(shape, max_seqs=max_seqs, max_seq_len=(L + 15) // 16 * 16, kv_bytes_per_model=kv, max_rows_per_step=args.score_rows))
+    for m, seed in enumerate((wl.seeds["senior"], wl.seeds["junior"])):
+        w = make_weights(shape, seed, device="cuda"); eng.load_weights(m, w); del w; torch.cuda.empty_cache()
+    eng.score(streams[:min(N, 2)])                       # warm-up: buffers, tensor maps
+    t0 = time.perf_counter()
+    out = eng.score(streams)
+    dt = time.perf_counter() - t0
+    eng.set_profile(True)                                # a second pass with one event pair per kernel launch: where the time goes
+    eng.score(streams[:min(N, 8)])
+    prof = eng.get_profile()
+    eng.set_profile(False)
+    tot = sum(ms for ms, n in prof.values()) or 1.0
+    kernels = {k: {"ms_per_launch": ms / n, "launches": n, "share": ms / tot} for k, (ms, n) in prof.items() if n}
+    st = out["stats"]
+    tok = N * (L - 1)
+    alpha = float(np.mean(np.concatenate([o[1:] for o in out["overlap"]])))
+    ce = float(-np.mean(np.concatenate([o[1:] for o in out["jun_logp"]])))
+    assert 0.0 < alpha <= 1.0 + 1e-5 and np.isfinite(ce)
+    pk = peaks()
+    flops = 2.0 * 2 * (shape.params_read_per_step + shape.vocab * shape.hidden) * tok     # both models, projections and LM head (attention extra)
+    wbytes = float(st["weight_bytes_read"])
+    print(json.dumps({"metric": "dual-scored tokens/s (teacher-forced, both models, 1 B200)", "value": tok / dt, "unit": "tokens/s", "n_gpus": 1,
+                      "steps": int(st["steps"]), "warmup": 1, "ms_per_step": dt / max(1, st["steps"]) * 1e3, "higher_is_better": True, "scaling": "weak",
+                      "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+                      "config": {"workload": wl.name, "mode": "tandem_score (host buffers)", "streams": N, "tokens_per_stream": L,
+                                 "rows_per_step_and_model": args.score_rows, "seconds": dt, "mean_alpha": alpha, "junior_cross_entropy": ce},
+                      "gpu_launches": int(st["kernel_launches"]), "kernels": kernels,
+                      "step_roofline": {"tensor_tflops": flops / dt / 1e12, "tensor_peak": pk.get("bf16_tflops_sustained", pk.get("bf16_tflops")),
+                                        "weights_gbs": wbytes / dt / 1e9, "hbm_peak": pk["hbm_gbs"]},
+                      "e2e": {"value": tok / dt, "unit": "tokens/s", "h2d_bytes_per_step": N * L * 4 / max(1, st["steps"]),
+                              "d2h_bytes_per_step": tok * 12 / max(1, st["steps"])}}))
     eng.free()
 
 
@@ -508,6 +561,8 @@ if __name__ == "__main__":
     a = parse_args()
     if a.impl == "reference":
         run_reference(a)
+    elif a.score > 0:
+        run_score(a)
     elif a.full_rollout > 0:
         run_full_rollout(a)
     else:

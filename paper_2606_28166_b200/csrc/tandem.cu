@@ -1038,10 +1038,8 @@ int tandem_score(tandem_handle* h, int32_t n_seqs, const int32_t* tokens, const 
   int next = 0, finished = 0, pages_reserved = 0;
   int64_t budget = 1024;
   for (int b = 0; b < n_seqs; ++b) budget += 4 + 4 * (offsets[b + 1] - offsets[b]);
-  const bool was_profiling = h->profile;
-  h->profile = false;
   while (finished < n_seqs) {
-    if (--budget < 0) { h->profile = was_profiling; return fail(h, TANDEM_ESTATE, "scoring made no progress (internal error)"); }
+    if (--budget < 0) return fail(h, TANDEM_ESTATE, "scoring made no progress (internal error)");
     int nfree = 0;
     for (int i = 0; i < c.max_seqs; ++i) nfree += !h->slot_busy[i];
     int n = 0, add = 0;
@@ -1049,14 +1047,22 @@ int tandem_score(tandem_handle* h, int32_t n_seqs, const int32_t* tokens, const 
     if (n > 0) {
       std::vector<int32_t> slots(n);
       for (int i = 0; i < n; ++i) ids[i] = next + i;
-      if ((rc = admit(h, &prm, nullptr, n, tokens, offsets + next, ids.data(), ones.data(), slots.data(), s, true))) { h->profile = was_profiling; return rc; }
+      if ((rc = admit(h, &prm, nullptr, n, tokens, offsets + next, ids.data(), ones.data(), slots.data(), s, true))) return rc;
       for (int i = 0; i < n; ++i) { slot_seq[slots[i]] = next + i; slot_pages[slots[i]] = pages_of(next + i); }
       pages_reserved += add;
       next += n;
     }
-    if ((rc = launch_step(h, io, rp, s, true, 1.f / temperature))) { h->profile = was_profiling; return rc; }
+    if (h->profile) { h->ev_used = 0; h->prof_pending.clear(); }
+    if ((rc = launch_step(h, io, rp, s, true, 1.f / temperature))) return rc;
     CU(h, cudaGetLastError());
-    if ((rc = refresh_slots(h, s))) { h->profile = was_profiling; return rc; }
+    if ((rc = refresh_slots(h, s))) return rc;   // synchronises the stream
+    if (h->profile) {
+      for (const auto& r : h->prof_pending) {
+        float pms = 0.f;
+        CU(h, cudaEventElapsedTime(&pms, r.e0, r.e1));
+        h->prof_ms[r.cls] += pms; h->prof_n[r.cls] += 1;
+      }
+    }
     for (int i = 0; i < c.max_seqs; ++i) {
       if (slot_seq[i] < 0 || h->slot_busy[i]) continue;
       const int b = slot_seq[i];
@@ -1072,7 +1078,6 @@ int tandem_score(tandem_handle* h, int32_t n_seqs, const int32_t* tokens, const 
       ++finished;
     }
   }
-  h->profile = was_profiling;
   CU(h, cudaEventRecord(e1, s));
   CU(h, cudaEventSynchronize(e1));
   float ms = 0.f;
