@@ -10,8 +10,12 @@ top-k 20 - PAPER.md L295-301, Table 3). BASELINE.json north_star (g) fixes the m
                     kept set = all ids if top_p >= 1, else the shortest prefix of ids sorted by
                     descending softmax(z/T) (ties: lower id first) whose cumulative probability
                     reaches top_p (never empty).
+  top-k (R18):      PAPER.md Table 3 (L299-301) evaluates with top-k 20 next to top-p 0.8 and trains with top-k -1. The
+                    paper does not say how the two filters compose; reading R18 takes the usual order of its
+                    generation engine: top-k first (the k ids of largest z / T, ties: lower id first; k <= 0 or
+                    k >= V: no filter), then top-p on the distribution renormalised over those k ids.
   log-prob:         log softmax(z / T')[y], T' = T (1 if greedy) - the distribution actually sampled
-                    from, before any top-p truncation (R11).
+                    from, before any top-p / top-k truncation (R11).
 """
 import numpy as np
 
@@ -47,13 +51,27 @@ def kept_set_top_p(z, temperature, top_p):
     return keep
 
 
-def sample_token(z, temperature, top_p, u):
+def kept_set(z, temperature, top_p=1.0, top_k=0):
+    """Boolean mask of the ids the Gumbel argmax runs over: top-k first, then top-p on the renormalised rest (R18)."""
+    z = np.asarray(z, dtype=np.float64)
+    V = z.shape[0]
+    keep = np.ones(V, dtype=bool)
+    if 0 < top_k < V:
+        order = np.lexsort((np.arange(V), -z))        # descending z (the order of z / T for T > 0), ties: lower id first
+        keep = np.zeros(V, dtype=bool)
+        keep[order[:top_k]] = True
+    if top_p < 1.0:
+        zz = np.where(keep, z, -np.inf)               # softmax over the kept ids only
+        keep = keep & kept_set_top_p(zz, temperature, top_p)
+    return keep
+
+
+def sample_token(z, temperature, top_p, u, top_k=0):
     """One token from logits z. `u`: float32 uniforms [V] (ignored when greedy)."""
     z = np.asarray(z, dtype=np.float64)
     if temperature <= 0:
         return int(np.argmax(z))                    # np.argmax returns the lowest index among ties
     score = z / float(temperature) + gumbel_from_uniform(u)
-    if top_p < 1.0:
-        keep = kept_set_top_p(z, temperature, top_p)
-        score = np.where(keep, score, -np.inf)
+    if top_p < 1.0 or top_k > 0:
+        score = np.where(kept_set(z, temperature, top_p, top_k), score, -np.inf)
     return int(np.argmax(score))
