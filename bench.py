@@ -48,6 +48,8 @@ def parse_args():
     ap.add_argument("--score", type=int, default=0, help="N > 0: time tandem_score (teacher-forced dual scoring, NEXT-1) on N synthetic streams instead of the rollout")
     ap.add_argument("--score-len", type=int, default=2048, help="tokens per stream for --score")
     ap.add_argument("--score-rows", type=int, default=512, help="rows per step and model for --score (max_rows_per_step)")
+    ap.add_argument("--top-k", type=int, default=0, help="top-k filter of the sampler (0 = off; the paper evaluates with 20)")
+    ap.add_argument("--temperature", type=float, default=None, help="override the workload's sampling temperature")
     ap.add_argument("--top-p", type=float, default=None, help="override the workload's top-p (the paper trains at 1.0, evaluates at 0.8)")
     ap.add_argument("--word-start-frac", type=float, default=None, help="override the word-start table density (cfg5 sweep)")
     ap.add_argument("--fast-forward", type=int, default=-1,
@@ -223,7 +225,7 @@ def run_full_rollout(args):
         eng.load_weights(m, w_host[m])
     del w_host
     seed = 20260628
-    prm = T.TandemParams(table, p=wl.p, temperature=wl.temperature, top_p=wl.top_p, seed=seed)
+    prm = T.TandemParams(table, p=wl.p, temperature=wl.temperature, top_p=wl.top_p, top_k=args.top_k, seed=seed)
     t0 = time.perf_counter()
     g = eng.generate(prm, prompts, max_new)
     dt = time.perf_counter() - t0
@@ -321,6 +323,8 @@ def run_ours(args):
         wl = wl.with_(word_start_frac=args.word_start_frac)
     if args.top_p is not None:
         wl = wl.with_(top_p=args.top_p)
+    if args.temperature is not None:
+        wl = wl.with_(temperature=args.temperature)
     shape, B = wl.shape, wl.batch
     W, K = max(3, args.warmup), args.steps
     if args.fast_forward < 0:
@@ -342,7 +346,7 @@ def run_ours(args):
                               layers=[{k: v.cpu() for k, v in l.items()} for l in w["layers"]]))
         del w
         torch.cuda.empty_cache()
-    prm = T.TandemParams(table, p=wl.p, temperature=wl.temperature, top_p=wl.top_p, seed=20260628)
+    prm = T.TandemParams(table, p=wl.p, temperature=wl.temperature, top_p=wl.top_p, top_k=args.top_k, seed=20260628)
     out = dict(token=torch.zeros(B, dtype=torch.int32, device="cuda"), owner=torch.zeros(B, dtype=torch.uint8, device="cuda"),
                sen_logp=torch.zeros(B, device="cuda"), done=torch.zeros(B, dtype=torch.uint8, device="cuda"))
     stream = torch.cuda.current_stream().cuda_stream
@@ -444,7 +448,7 @@ def run_ours(args):
     res = {"metric": METRIC, "value": tokens_all / (ms_all * 1e-3), "unit": "tokens/s", "n_gpus": world, "steps": K, "warmup": W,
            "ms_per_step": ms_all / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
            "config": {"workload": wl.name, "batch_per_gpu": B, "prompt_len": list(wl.prompt_len), "fast_forward": args.fast_forward,
-                      "ctx_mean_timed": ctx_mean, "p": wl.p, "word_start_frac": wl.word_start_frac, "temperature": wl.temperature, "top_p": wl.top_p,
+                      "ctx_mean_timed": ctx_mean, "p": wl.p, "word_start_frac": wl.word_start_frac, "temperature": wl.temperature, "top_p": wl.top_p, "top_k": args.top_k,
                       "page_tokens": 16, "parallelism": "dp%d (independent sequences, replicated weights, no collective)" % world,
                       "l2": "inputs larger than L2 (16.1 GB of weights + KV streamed per step vs 126 MB L2)",
                       "setup_steps": n_setup + ramp + n_drain, "setup_seconds": setup_s, "cuda_graph": True},

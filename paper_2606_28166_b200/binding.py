@@ -45,7 +45,7 @@ class _Weights(C.Structure):
 
 class _Params(C.Structure):
     _fields_ = [("p", C.c_float), ("switch_mode", C.c_int32), ("start_owner", C.c_int32), ("cap_k", C.c_int32),
-                ("temperature", C.c_float), ("top_p", C.c_float), ("eos_id", C.c_int32), ("seed", C.c_uint64),
+                ("temperature", C.c_float), ("top_p", C.c_float), ("top_k", C.c_int32), ("eos_id", C.c_int32), ("seed", C.c_uint64),
                 ("word_start", C.c_void_p)]
 
 
@@ -98,7 +98,7 @@ def lib():
         L.tandem_last_error.argtypes = [C.c_void_p]
         L.tandem_last_error.restype = C.c_char_p
         L.tandem_test_uniforms.argtypes = [C.c_uint64, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_void_p]
-        L.tandem_test_nucleus.argtypes = [C.c_int32, C.c_float, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.tandem_test_nucleus.argtypes = [C.c_int32, C.c_float, C.c_float, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.tandem_test_philox.argtypes = [C.POINTER(C.c_uint32), C.POINTER(C.c_uint32), C.POINTER(C.c_uint32)]
         L.tandem_test_gemm.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
         L.tandem_debug_lt_times.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
@@ -122,9 +122,9 @@ class TandemParams:
     """Mirror of tandem_params; `word_start` is a uint8 NumPy array [vocab] (host)."""
 
     def __init__(self, word_start, p=0.5, switch_mode=TOGGLE, start_owner=SENIOR, cap_k=0, temperature=1.0, top_p=1.0,
-                 eos_id=-1, seed=0):
+                 eos_id=-1, seed=0, top_k=0):
         self.word_start = np.ascontiguousarray(word_start, dtype=np.uint8)
-        self.c = _Params(p, switch_mode, start_owner, cap_k, temperature, top_p, eos_id, seed, self.word_start.ctypes.data)
+        self.c = _Params(p, switch_mode, start_owner, cap_k, temperature, top_p, top_k, eos_id, seed, self.word_start.ctypes.data)
 
 
 def _ptr(t):
@@ -275,8 +275,8 @@ def tandem_test_uniforms(seed, seq_id, t, stream, n, out_dev):
         raise TandemError(rc)
 
 
-def tandem_test_nucleus(logits, temperature, top_p, u, token_out, keep_out):
-    rc = lib().tandem_test_nucleus(logits.numel(), temperature, top_p, logits.data_ptr(), u.data_ptr(), token_out.data_ptr(), keep_out.data_ptr())
+def tandem_test_nucleus(logits, temperature, top_p, u, token_out, keep_out, top_k=0):
+    rc = lib().tandem_test_nucleus(logits.numel(), temperature, top_p, top_k, logits.data_ptr(), u.data_ptr(), token_out.data_ptr(), keep_out.data_ptr())
     if rc:
         raise TandemError(rc)
 

@@ -103,7 +103,7 @@ struct StepIO {         // per-step optional outputs / overrides (device pointer
 };
 
 struct RuleParams {
-  float p; int switch_mode; int cap_k; float temperature; int eos_id; unsigned long long seed; float top_p;
+  float p; int switch_mode; int cap_k; float temperature; int eos_id; unsigned long long seed; float top_p; int top_k;
 };
 
 // ------------------------------------------------------------------------------------------------------------

@@ -513,114 +513,193 @@ __device__ __forceinline__ void row_scan(const float* __restrict__ z, int V, F&&
   }
 }
 template <int NT>
-__device__ int nucleus_gumbel_argmax(const float* __restrict__ z, int V, float invT, float m, float top_p,
+__device__ int nucleus_gumbel_argmax(const float* __restrict__ z, int V, float invT, float m, float top_p, int top_k,
                                      const float* __restrict__ u_row, uint32_t k0, uint32_t k1, int t, int sid,
                                      NucleusSmem<NT>& S, uint8_t* keep_out = nullptr) {
   typedef unsigned long long u64;
   const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const bool use_k = top_k > 0 && top_k < V, use_p = top_p < 1.f;
   uint32_t prefix = 0;
   u64 above = 0, target = 0;   // above: the mass of the ids shallower than the prefix (larger x)
   int lvl = 0;                 // the ids under the prefix: (T >> (24 - 4 lvl)) == prefix
   bool listed = false;
-  for (; lvl < 6; ++lvl) {
-    if (threadIdx.x == 0) S.n = 0;
-    __syncthreads();
-    const int sh_pre = 24 - 4 * lvl, sh_bin = 20 - 4 * lvl;
-    const bool gather = lvl > 0 || V <= kNucleusCap;
+  // a filter keeps id v with key kx iff kx > key || (kx == key && v <= cut)
+  uint32_t keyK = 0u, keyP = 0u;
+  int cutK = V, cutP = V;
+  auto append = [&](uint32_t k, u64 q, int v) {   // one counter increment for the lanes here
+    const unsigned act = __activemask();
+    const int leader = __ffs(act) - 1;
+    int base = 0;
+    if (lane == leader) base = atomicAdd(&S.n, __popc(act));
+    const int i = __shfl_sync(act, base, leader) + __popc(act & ((1u << lane) - 1u));
+    if (i < kNucleusCap) { S.ck[i] = k; S.cq[i] = q; S.cid[i] = v; }
+  };
+  // c-th smallest id among the entries of `scan` with key == key
+  auto tie_cut = [&](auto&& scan, uint32_t key, u64 c) {
+    int lo = 0, hi = V - 1;
+    while (lo < hi) {
+      const int mid = (lo + hi) >> 1;
+      u64 cnt = 0;
+      scan([&](uint32_t k, u64, int id) { if (k == key && id <= mid) cnt += 1; });
+      if (block_sum_u64<NT>(cnt, S.red) >= c) hi = mid; else lo = mid + 1;
+    }
+    return lo;
+  };
+  if (use_k) {
+    // top-k (reading R18): the same descent on counts until the ids down to and including the bin of the k-th largest fit the list
+    u64 cabove = 0;
+    bool fits = false;
+    while (lvl < 6 && !fits) {
+      const int sh_pre = 24 - 4 * lvl, sh_bin = 20 - 4 * lvl;
 #pragma unroll
-    for (int k = 0; k < kNucleusBins; ++k) S.ph[k][threadIdx.x] = 0;
-    row_scan<NT>(z, V, [&](float zv, int v) {
-      const float x = zv * invT, d = m - x;
-      const uint32_t T = nucleus_depth(d);
-      if ((T >> sh_pre) == prefix) {
-        const int b = (T >> sh_bin) & (kNucleusBins - 1);
-        const u64 q = nucleus_mass(d);
-        S.ph[b][threadIdx.x] += q;
-        if (gather) {   // one counter increment for the lanes here
-          const unsigned act = __activemask();
-          const int leader = __ffs(act) - 1;
-          int base = 0;
-          if (lane == leader) base = atomicAdd(&S.n, __popc(act));
-          const int i = __shfl_sync(act, base, leader) + __popc(act & ((1u << lane) - 1u));
-          if (i < kNucleusCap) { S.ck[i] = order_key(x); S.cq[i] = q; S.cid[i] = v; }
+      for (int k = 0; k < kNucleusBins; ++k) S.ph[k][threadIdx.x] = 0;
+      row_scan<NT>(z, V, [&](float zv, int) {
+        const uint32_t T = nucleus_depth(m - zv * invT);
+        if ((T >> sh_pre) == prefix) S.ph[(T >> sh_bin) & (kNucleusBins - 1)][threadIdx.x] += 1;
+      });
+      __syncthreads();
+      for (int k = w; k < kNucleusBins; k += NT / 32) {
+        u64 hs = 0;
+        for (int i = lane; i < NT; i += 32) hs += S.ph[k][i];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) hs += __shfl_xor_sync(0xffffffffu, hs, o);
+        if (lane == 0) S.hist[k] = hs;
+      }
+      __syncthreads();
+      int bs = kNucleusBins - 1;
+      bool found = false;
+      for (int k = 0; k < kNucleusBins - 1; ++k) {
+        if (!found) {
+          if (cabove + S.hist[k] >= (u64)top_k) { bs = k; found = true; } else { cabove += S.hist[k]; }
         }
       }
-    });
-    __syncthreads();
-    for (int k = w; k < kNucleusBins; k += NT / 32) {   // bin k: the sum over all threads' private counters
-      u64 hs = 0;
-      for (int i = lane; i < NT; i += 32) hs += S.ph[k][i];
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) hs += __shfl_xor_sync(0xffffffffu, hs, o);
-      if (lane == 0) S.hist[k] = hs;
+      fits = cabove + S.hist[bs] <= (u64)kNucleusCap;
+      prefix = (prefix << 4) | (uint32_t)bs;
+      ++lvl;
+      __syncthreads();
     }
+    const int shk = 24 - 4 * lvl;
+    if (threadIdx.x == 0) S.n = 0;
     __syncthreads();
-    if (gather && S.n <= kNucleusCap) { listed = true; break; }
-    u64 h[kNucleusBins];
-#pragma unroll
-    for (int k = 0; k < kNucleusBins; ++k) h[k] = S.hist[k];
-    if (lvl == 0) {
-      u64 total = 0;
-#pragma unroll
-      for (int k = 0; k < kNucleusBins; ++k) total += h[k];
-      target = __double2ull_ru((double)top_p * (double)total);
-      if (target < 1) target = 1;
-    }
-    int bs = kNucleusBins - 1;
-    bool found = false;
-#pragma unroll
-    for (int k = 0; k < kNucleusBins - 1; ++k) {
-      if (!found) {
-        if (above + h[k] >= target) { bs = k; found = true; } else { above += h[k]; }
-      }
-    }
-    prefix = (prefix << 4) | (uint32_t)bs;
-    __syncthreads();
-  }
-  const int sh = 24 - 4 * lvl;
-  const int n = listed ? S.n : 0;
-  if (lvl == 0) {   // the list holds the whole (short) row: no level pass fixed the target yet
-    u64 tot = 0;
-    for (int i = threadIdx.x; i < n; i += NT) tot += S.cq[i];
-    target = __double2ull_ru((double)top_p * (double)block_sum_u64<NT>(tot, S.red));
-    if (target < 1) target = 1;
-  }
-  // fn(key, mass, id) over the ids of the threshold bin
-  auto scan = [&](auto&& fn) {
-    if (listed) {
-      for (int i = threadIdx.x; i < n; i += NT) fn(S.ck[i], S.cq[i], S.cid[i]);
-    } else {
+    if (fits) {
       row_scan<NT>(z, V, [&](float zv, int v) {
         const float x = zv * invT, d = m - x;
-        if ((nucleus_depth(d) >> sh) == prefix) fn(order_key(x), nucleus_mass(d), v);
+        if ((nucleus_depth(d) >> shk) <= prefix) append(order_key(x), nucleus_mass(d), v);
       });
+      __syncthreads();
+      listed = true;
     }
-  };
-  uint32_t key = 0u;
-  for (int bit = 31; bit >= 0; --bit) {
-    const uint32_t cand = key | (1u << bit);
-    u64 f = 0;
-    scan([&](uint32_t k, u64 q, int) { if (k >= cand) f += q; });
-    if (above + block_sum_u64<NT>(f, S.red) >= target) key = cand;
-  }
-  u64 fs = 0, nt = 0;
-  scan([&](uint32_t k, u64 q, int) { if (k > key) fs += q; if (k == key) nt += 1; });
-  const u64 above_strict = above + block_sum_u64<NT>(fs, S.red);
-  const int n_ties = (int)block_sum_u64<NT>(nt, S.red);
-  int id_cut = V;   // ids at the threshold are kept while id <= id_cut
-  if (n_ties > 1) {
-    const u64 q = nucleus_mass(m - key_value(key));
-    u64 c = q ? (target - above_strict + q - 1) / q : (u64)n_ties;
-    if (c < 1) c = 1;
-    if (c < (u64)n_ties) {   // the c-th smallest id among the ties
-      int lo = 0, hi = V - 1;
-      while (lo < hi) {
-        const int mid = (lo + hi) >> 1;
-        u64 cnt = 0;
-        scan([&](uint32_t k, u64, int id) { if (k == key && id <= mid) cnt += 1; });
-        if (block_sum_u64<NT>(cnt, S.red) >= c) hi = mid; else lo = mid + 1;
+    const int nk = listed ? S.n : 0;
+    auto scan_k = [&](auto&& fn) {   // the list, or the whole row when even the deepest bin does not fit (a row of equal logits)
+      if (listed) {
+        for (int i = threadIdx.x; i < nk; i += NT) fn(S.ck[i], S.cq[i], S.cid[i]);
+      } else {
+        row_scan<NT>(z, V, [&](float zv, int v) { const float x = zv * invT; fn(order_key(x), nucleus_mass(m - x), v); });
       }
-      id_cut = lo;
+    };
+    for (int bit = 31; bit >= 0; --bit) {   // the k-th largest key
+      const uint32_t cand = keyK | (1u << bit);
+      u64 c = 0;
+      scan_k([&](uint32_t k, u64, int) { if (k >= cand) c += 1; });
+      if (block_sum_u64<NT>(c, S.red) >= (u64)top_k) keyK = cand;
+    }
+    u64 gt = 0, eq = 0;
+    scan_k([&](uint32_t k, u64, int) { if (k > keyK) gt += 1; if (k == keyK) eq += 1; });
+    gt = block_sum_u64<NT>(gt, S.red);
+    eq = block_sum_u64<NT>(eq, S.red);
+    const u64 need = (u64)top_k - gt;
+    if (need < eq) cutK = tie_cut(scan_k, keyK, need);
+  }
+  if (use_p && !use_k) {
+    for (; lvl < 6; ++lvl) {
+      if (threadIdx.x == 0) S.n = 0;
+      __syncthreads();
+      const int sh_pre = 24 - 4 * lvl, sh_bin = 20 - 4 * lvl;
+      const bool gather = lvl > 0 || V <= kNucleusCap;
+#pragma unroll
+      for (int k = 0; k < kNucleusBins; ++k) S.ph[k][threadIdx.x] = 0;
+      row_scan<NT>(z, V, [&](float zv, int v) {
+        const float x = zv * invT, d = m - x;
+        const uint32_t T = nucleus_depth(d);
+        if ((T >> sh_pre) == prefix) {
+          const int b = (T >> sh_bin) & (kNucleusBins - 1);
+          const u64 q = nucleus_mass(d);
+          S.ph[b][threadIdx.x] += q;
+          if (gather) append(order_key(x), q, v);
+        }
+      });
+      __syncthreads();
+      for (int k = w; k < kNucleusBins; k += NT / 32) {   // bin k: the sum over all threads' private counters
+        u64 hs = 0;
+        for (int i = lane; i < NT; i += 32) hs += S.ph[k][i];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) hs += __shfl_xor_sync(0xffffffffu, hs, o);
+        if (lane == 0) S.hist[k] = hs;
+      }
+      __syncthreads();
+      if (gather && S.n <= kNucleusCap) { listed = true; break; }
+      u64 h[kNucleusBins];
+#pragma unroll
+      for (int k = 0; k < kNucleusBins; ++k) h[k] = S.hist[k];
+      if (lvl == 0) {
+        u64 total = 0;
+#pragma unroll
+        for (int k = 0; k < kNucleusBins; ++k) total += h[k];
+        target = __double2ull_ru((double)top_p * (double)total);
+        if (target < 1) target = 1;
+      }
+      int bs = kNucleusBins - 1;
+      bool found = false;
+#pragma unroll
+      for (int k = 0; k < kNucleusBins - 1; ++k) {
+        if (!found) {
+          if (above + h[k] >= target) { bs = k; found = true; } else { above += h[k]; }
+        }
+      }
+      prefix = (prefix << 4) | (uint32_t)bs;
+      __syncthreads();
+    }
+  }
+  if (use_p) {
+    const int sh = 24 - 4 * lvl;
+    const int n = listed ? S.n : 0;
+    // fn(key, mass, id) over the candidates: the survivors of top-k, else the ids of the threshold bin
+    auto scan = [&](auto&& fn) {
+      if (listed) {
+        for (int i = threadIdx.x; i < n; i += NT) {
+          const uint32_t k = S.ck[i]; const int id = S.cid[i];
+          if (!use_k || k > keyK || (k == keyK && id <= cutK)) fn(k, S.cq[i], id);
+        }
+      } else {
+        row_scan<NT>(z, V, [&](float zv, int v) {
+          const float x = zv * invT, d = m - x;
+          const uint32_t k = order_key(x);
+          if (use_k ? (k > keyK || (k == keyK && v <= cutK)) : ((nucleus_depth(d) >> sh) == prefix)) fn(k, nucleus_mass(d), v);
+        });
+      }
+    };
+    if (use_k || lvl == 0) {   // no level pass fixed the target: top-p renormalises over the top-k survivors / a short row sits in the list
+      u64 tot = 0;
+      scan([&](uint32_t, u64 q, int) { tot += q; });
+      target = __double2ull_ru((double)top_p * (double)block_sum_u64<NT>(tot, S.red));
+      if (target < 1) target = 1;
+      above = 0;
+    }
+    for (int bit = 31; bit >= 0; --bit) {
+      const uint32_t cand = keyP | (1u << bit);
+      u64 f = 0;
+      scan([&](uint32_t k, u64 q, int) { if (k >= cand) f += q; });
+      if (above + block_sum_u64<NT>(f, S.red) >= target) keyP = cand;
+    }
+    u64 fs = 0, nt = 0;
+    scan([&](uint32_t k, u64 q, int) { if (k > keyP) fs += q; if (k == keyP) nt += 1; });
+    const u64 above_strict = above + block_sum_u64<NT>(fs, S.red);
+    const u64 n_ties = block_sum_u64<NT>(nt, S.red);
+    if (n_ties > 1) {
+      const u64 q = nucleus_mass(m - key_value(keyP));
+      u64 c = q ? (target - above_strict + q - 1) / q : n_ties;
+      if (c < 1) c = 1;
+      if (c < n_ties) cutP = tie_cut(scan, keyP, c);
     }
   }
   // the Gumbel argmax over the kept ids (Philox blocks of 4 ids, drawn only where an id is kept)
@@ -639,7 +718,7 @@ __device__ int nucleus_gumbel_argmax(const float* __restrict__ z, int V, float i
       if (v >= V) break;
       const float x = zz[ww] * invT;
       const uint32_t kx = order_key(x);
-      const bool keep = kx > key || (kx == key && v <= id_cut);
+      const bool keep = (kx > keyK || (kx == keyK && v <= cutK)) && (kx > keyP || (kx == keyP && v <= cutP));
       if (keep_out) keep_out[v] = keep;
       if (keep) {
         if (!drawn) { philox4x32_10(c, k0, k1); drawn = true; }
@@ -663,7 +742,7 @@ __device__ int nucleus_gumbel_argmax(const float* __restrict__ z, int V, float i
 
 // test hook: one row of logits through the nucleus search exactly as the sampler runs it (explicit uniforms)
 template <int NT>
-__global__ void __launch_bounds__(NT) test_nucleus_kernel(const float* z, int V, float temperature, float top_p, const float* u, int32_t* token,
+__global__ void __launch_bounds__(NT) test_nucleus_kernel(const float* z, int V, float temperature, float top_p, int top_k, const float* u, int32_t* token,
                                                           uint8_t* keep) {
   extern __shared__ __align__(16) unsigned char nucleus_smem[];
   NucleusSmem<NT>& S = *reinterpret_cast<NucleusSmem<NT>*>(nucleus_smem);
@@ -675,7 +754,7 @@ __global__ void __launch_bounds__(NT) test_nucleus_kernel(const float* z, int V,
   __syncthreads();
   for (int k = 0; k < NT / 32; ++k) m = fmaxf(m, S.redf[k]);
   __syncthreads();
-  const int y = nucleus_gumbel_argmax<NT>(z, V, invT, m, top_p, u, 0u, 0u, 1, 0, S, keep);
+  const int y = nucleus_gumbel_argmax<NT>(z, V, invT, m, top_p, top_k, u, 0u, 0u, 1, 0, S, keep);
   if (threadIdx.x == 0) *token = y;
 }
 
@@ -740,7 +819,7 @@ __global__ void __launch_bounds__(NT) sample_switch_emit_kernel(const __grid_con
   const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
   if (l == 0) { s_m[w] = m; s_s[w] = sum; s_bv[w] = raw.v; s_bi[w] = raw.i; s_gv[w] = gum.v; s_gi[w] = gum.i; }
   __syncthreads();
-  const bool nucleus = NUCLEUS && !greedy && a.rp.top_p < 1.f;   // the whole CTA stays for the nucleus search, else thread 0 alone
+  const bool nucleus = NUCLEUS && !greedy && (a.rp.top_p < 1.f || (a.rp.top_k > 0 && a.rp.top_k < a.vocab));   // the whole CTA stays for the nucleus search, else thread 0 alone
   if (!nucleus && threadIdx.x != 0) return;
   bool last = true;
   if (threadIdx.x == 0) {
@@ -782,7 +861,7 @@ __global__ void __launch_bounds__(NT) sample_switch_emit_kernel(const __grid_con
     if (threadIdx.x == 0) { s_last = last; s_fin = m; }
     __syncthreads();
     if (!s_last) return;
-    const int yn = nucleus_gumbel_argmax<NT>(z, V, invT, s_fin, a.rp.top_p, u_row, k0, k1, t, sid, *reinterpret_cast<NucleusSmem<NT>*>(nucleus_smem));
+    const int yn = nucleus_gumbel_argmax<NT>(z, V, invT, s_fin, a.rp.top_p, a.rp.top_k, u_row, k0, k1, t, sid, *reinterpret_cast<NucleusSmem<NT>*>(nucleus_smem));
     if (threadIdx.x != 0) return;
     gum.i = yn;
     searched = true;

@@ -54,7 +54,7 @@ struct GraphKey {
   StepIO io; RuleParams rp; bool valid = false;
   bool same(const StepIO& i, const RuleParams& r) const {
     return valid && std::memcmp(&io, &i, sizeof(StepIO)) == 0 && rp.p == r.p && rp.switch_mode == r.switch_mode && rp.cap_k == r.cap_k &&
-           rp.temperature == r.temperature && rp.eos_id == r.eos_id && rp.seed == r.seed && rp.top_p == r.top_p;
+           rp.temperature == r.temperature && rp.eos_id == r.eos_id && rp.seed == r.seed && rp.top_p == r.top_p && rp.top_k == r.top_k;
   }
 };
 
@@ -434,7 +434,7 @@ int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaS
   for (int m = 0; m < 2; ++m)
     sa.m[m] = SampleArgs{h->st, h->tab[m], io, rp, h->ws[m].logits, h->word_start_dev, h->tokens, h->out_owner, h->out_logp, V, c.max_seq_len, m,
                          h->ws[m].chunk_part, h->ws[m].chunk_ctr, n_chunk};
-  const size_t nucleus_smem = (rp.temperature > 0.f && rp.top_p < 1.f) ? sizeof(NucleusSmem<256>) : 0;
+  const size_t nucleus_smem = (rp.temperature > 0.f && (rp.top_p < 1.f || (rp.top_k > 0 && rp.top_k < V))) ? sizeof(NucleusSmem<256>) : 0;
   if (nucleus_smem) KL(h, TANDEM_KC_SAMPLE, s, launch_ex(sample_switch_emit_kernel<256, true>, dim3(c.max_seqs, n_chunk, 2), dim3(256), nucleus_smem, s, pdl, sa));
   else KL(h, TANDEM_KC_SAMPLE, s, launch_ex(sample_switch_emit_kernel<256, false>, dim3(c.max_seqs, n_chunk, 2), dim3(256), 0, s, pdl, sa));
   return TANDEM_OK;
@@ -510,6 +510,7 @@ int check_params(tandem_handle* h, const tandem_params* p) {
   if (p->cap_k < 0) return fail(h, TANDEM_EINVAL, "cap_k must be >= 0");
   if (!(p->temperature >= 0.f)) return fail(h, TANDEM_EINVAL, "temperature must be >= 0");
   if (!(p->top_p > 0.f && p->top_p <= 1.0f)) return fail(h, TANDEM_EINVAL, "top_p must be in (0, 1]");
+  if (p->top_k > kNucleusCap && p->top_k < h->cfg.vocab) return fail(h, TANDEM_EINVAL, "top_k above 2048 (and below vocab) is not supported");
   if (p->eos_id >= h->cfg.vocab) return fail(h, TANDEM_EINVAL, "eos_id >= vocab");
   if (!p->word_start) return fail(h, TANDEM_EINVAL, "word_start is NULL");
   return TANDEM_OK;
@@ -536,7 +537,7 @@ StepIO make_io(const tandem_step_out* out, const tandem_overrides* ovr) {
   return io;
 }
 RuleParams make_rule(const tandem_params* p) {
-  RuleParams r{}; r.p = p->p; r.switch_mode = p->switch_mode; r.cap_k = p->cap_k; r.temperature = p->temperature; r.eos_id = p->eos_id; r.seed = p->seed; r.top_p = p->top_p;
+  RuleParams r{}; r.p = p->p; r.switch_mode = p->switch_mode; r.cap_k = p->cap_k; r.temperature = p->temperature; r.eos_id = p->eos_id; r.seed = p->seed; r.top_p = p->top_p; r.top_k = p->top_k;
   return r;
 }
 
@@ -1023,7 +1024,7 @@ int tandem_score(tandem_handle* h, int32_t n_seqs, const int32_t* tokens, const 
   CU(h, cudaEventCreate(&e0)); CU(h, cudaEventCreate(&e1));
   CU(h, cudaEventRecord(e0, s));
   tandem_params prm{};   // admission only needs an owner; the rule never runs while scoring
-  prm.p = 0.f; prm.switch_mode = TANDEM_TOGGLE; prm.start_owner = TANDEM_SENIOR; prm.temperature = temperature; prm.top_p = 1.f; prm.eos_id = -1;
+  prm.p = 0.f; prm.switch_mode = TANDEM_TOGGLE; prm.start_owner = TANDEM_SENIOR; prm.temperature = temperature; prm.top_p = 1.f; prm.top_k = 0; prm.eos_id = -1;
   const StepIO io = make_io(nullptr, nullptr);
   const RuleParams rp = make_rule(&prm);
   auto pages_of = [&](int b) { return (int)((offsets[b + 1] - offsets[b] + kPageTokens - 1) / kPageTokens); };
@@ -1138,11 +1139,11 @@ int tandem_test_uniforms(uint64_t seed, int32_t seq_id, int32_t t, int32_t strea
   return cudaDeviceSynchronize() == cudaSuccess ? TANDEM_OK : TANDEM_ECUDA;
 }
 
-int tandem_test_nucleus(int32_t vocab, float temperature, float top_p, const float* logits_dev, const float* u_dev, int32_t* token_dev,
+int tandem_test_nucleus(int32_t vocab, float temperature, float top_p, int32_t top_k, const float* logits_dev, const float* u_dev, int32_t* token_dev,
                         uint8_t* keep_dev) {
-  if (vocab <= 0 || !(temperature > 0.f) || !(top_p > 0.f && top_p < 1.f) || !logits_dev || !u_dev || !token_dev || !keep_dev) return TANDEM_EINVAL;
+  if (vocab <= 0 || !(temperature > 0.f) || !(top_p > 0.f && top_p <= 1.f) || top_k > kNucleusCap || !logits_dev || !u_dev || !token_dev || !keep_dev) return TANDEM_EINVAL;
   cudaFuncSetAttribute(test_nucleus_kernel<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(NucleusSmem<256>));
-  test_nucleus_kernel<256><<<1, 256, sizeof(NucleusSmem<256>)>>>(logits_dev, vocab, temperature, top_p, u_dev, token_dev, keep_dev);
+  test_nucleus_kernel<256><<<1, 256, sizeof(NucleusSmem<256>)>>>(logits_dev, vocab, temperature, top_p, top_k, u_dev, token_dev, keep_dev);
   return cudaDeviceSynchronize() == cudaSuccess ? TANDEM_OK : TANDEM_ECUDA;
 }
 

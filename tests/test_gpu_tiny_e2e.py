@@ -100,10 +100,10 @@ def test_sampled_rollouts_match_oracle_counter_rng(mode, start, p, cap):
     eng.free()
 
 
-@pytest.mark.parametrize("temperature,top_p", [(0.7, 0.8), (1.0, 0.3), (0.6, 0.95)])
-def test_nucleus_rollouts_match_oracle(temperature, top_p):
-    """top-p < 1 (the evaluation setting T = 0.7, top-p 0.8 of Table 3 among them): tokens, owners, mask as the oracle's; the
-    log-prob is that of the untruncated softmax(z/T) (R11)."""
+@pytest.mark.parametrize("temperature,top_p,top_k", [(0.7, 0.8, 0), (1.0, 0.3, 0), (0.6, 0.95, 0), (0.7, 0.8, 20), (1.0, 1.0, 5), (0.9, 1.0, 1)])
+def test_nucleus_rollouts_match_oracle(temperature, top_p, top_k):
+    """top-p < 1 and top-k (the evaluation setting T = 0.7, top-p 0.8, top-k 20 of Table 3 among them; top-k 1 = greedy): tokens,
+    owners, mask as the oracle's; the log-prob is that of the untruncated softmax(z/T) (R11)."""
     shape = get_workload("cfg1_tiny_f32").shape
     ws = make_word_start(shape.vocab, 0.3, 11)
     rng = np.random.default_rng(8)
@@ -111,9 +111,9 @@ def test_nucleus_rollouts_match_oracle(temperature, top_p):
     prompts = [rng.integers(0, shape.vocab, size=int(n)).astype(np.int32) for n in (3, 16, 21, 9, 30)]
     max_new = np.array([30, 24, 17, 32, 8], dtype=np.int32)
     eng, orc, _ = make_pair(shape, (1, 2), max_seqs=3, max_seq_len=64, gain_jitter=0.1)
-    op = OParams(p=0.5, temperature=temperature, top_p=top_p, eos_id=3, seed=77)
+    op = OParams(p=0.5, temperature=temperature, top_p=top_p, top_k=top_k, eos_id=3, seed=77)
     ref = tandem_generate(orc, op, prompts, max_new, ws, uni=Uniforms(seed=77, seq_ids=np.arange(B, dtype=np.int32)))
-    out = eng.generate(T.TandemParams(ws, p=0.5, temperature=temperature, top_p=top_p, eos_id=3, seed=77), prompts, max_new)
+    out = eng.generate(T.TandemParams(ws, p=0.5, temperature=temperature, top_p=top_p, top_k=top_k, eos_id=3, seed=77), prompts, max_new)
     _compare(out, ref, B, logp_tol=2e-5)
     solo = eng.generate(T.TandemParams(ws, p=0.5, temperature=temperature, top_p=1.0, eos_id=3, seed=77), prompts, max_new)
     assert any(not np.array_equal(solo["tokens"][b, :out["len"][b]], out["tokens"][b, :out["len"][b]]) for b in range(B))  # the filter bites

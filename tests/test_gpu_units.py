@@ -100,12 +100,12 @@ def test_tcgen05_gemm_swiglu_epilogue(rows, I, K):
     assert err <= 2 ** -8 * max(1e-3, ref.abs().max().item()) + 1e-6, (err, ref.abs().max().item())   # one bf16 rounding of the result
 
 
-def _nucleus(z, temperature, top_p, u):
+def _nucleus(z, temperature, top_p, u, top_k=0):
     zt = torch.tensor(z, dtype=torch.float32, device="cuda")
     ut = torch.tensor(u, dtype=torch.float32, device="cuda")
     tok = torch.zeros(1, dtype=torch.int32, device="cuda")
     keep = torch.zeros(len(z), dtype=torch.uint8, device="cuda")
-    T.tandem_test_nucleus(zt, temperature, top_p, ut, tok, keep)
+    T.tandem_test_nucleus(zt, temperature, top_p, ut, tok, keep, top_k=top_k)
     return int(tok.item()), keep.cpu().numpy().astype(bool)
 
 
@@ -154,3 +154,48 @@ def test_nucleus_random_rows_match_oracle(V, temperature, top_p, seed):
         assert p[keep].sum() >= top_p - 1e-5 and (keep.sum() == 1 or p[keep].sum() - p[keep].min() < top_p + 1e-5)   # reaches top_p, minimal
         if np.array_equal(keep, want):
             assert tok == sample_token(z, temperature, top_p, u)
+
+
+def test_top_k_hand_examples_ties_and_composition():
+    """Reading R18 on the oracle's hand example, exact ties (lower id first), flat rows (the k-th largest sits in a bin that
+    overflows the list), k = 1 = greedy, and top-k composed with top-p; masks from oracle.sampler.kept_set."""
+    from oracle.sampler import kept_set
+    z = np.log(np.array([0.3, 0.05, 0.5, 0.15]))
+    u = np.full(4, 0.5, dtype=np.float32)
+    for top_p, top_k in ((1.0, 1), (1.0, 2), (1.0, 3), (0.7, 3), (0.81, 2), (0.6, 2), (0.63, 2)):
+        tok, keep = _nucleus(z, 1.0, top_p, u, top_k)
+        assert keep.tolist() == kept_set(z.astype(np.float32), 1.0, top_p, top_k).tolist(), (top_p, top_k)
+        if top_k == 1:
+            assert tok == 2
+    z = np.array([0., 2., 2., -1., 2., 2., 0.5]); u = np.full(7, 0.5, np.float32)
+    for top_k in (1, 2, 3, 4, 5, 6):
+        _, keep = _nucleus(z, 0.7, 1.0, u, top_k)
+        assert keep.tolist() == kept_set(z.astype(np.float32), 0.7, 1.0, top_k).tolist(), top_k
+    for V, top_k in ((1000, 20), (151936, 20), (151936, 2048), (5000, 1)):             # all ids tie: the first k ids
+        _, keep = _nucleus(np.zeros(V), 1.0, 1.0, np.full(V, 0.5, np.float32), top_k)
+        assert int(keep.sum()) == top_k and keep[:top_k].all()
+    with pytest.raises(T.TandemError):                                                  # the list holds 2048 ids
+        _nucleus(np.zeros(5000), 1.0, 1.0, np.full(5000, 0.5, np.float32), 3000)
+    z = np.zeros(151936); z[[5, 100000, 77]] = [3.0, 2.0, 1.0]                          # three spikes on a flat row
+    _, keep = _nucleus(z, 1.0, 1.0, np.full(z.size, 0.5, np.float32), 5)
+    assert np.flatnonzero(keep).tolist() == [0, 1, 5, 77, 100000]
+
+
+@pytest.mark.parametrize("V,temperature,top_p,top_k,seed", [(512, 0.7, 0.8, 20, 0), (1000, 1.0, 1.0, 50, 1), (4099, 0.6, 0.95, 7, 2),
+                                                             (151936, 0.7, 0.8, 20, 3), (151936, 1.0, 1.0, 2048, 4), (151936, 0.7, 0.5, 1000, 5)])
+def test_top_k_random_rows_match_oracle(V, temperature, top_p, top_k, seed):
+    """Random rows: top-k is index work (bit-exact); with top-p on top the one id at the fp32 rounding boundary may differ."""
+    from oracle.sampler import kept_set, sample_token
+    rng = np.random.default_rng(seed)
+    for rep in range(3):
+        z = (rng.standard_normal(V) * 3.0).astype(np.float32)
+        u = np.minimum((rng.integers(0, 1 << 32, size=V, dtype=np.uint64).astype(np.float32) + 0.5) * np.float32(2.0 ** -32),
+                       np.float32(1 - 2.0 ** -24)).astype(np.float32)
+        tok, keep = _nucleus(z, temperature, top_p, u, top_k)
+        want = kept_set(z, temperature, top_p, top_k)
+        if top_p >= 1.0:
+            assert np.array_equal(keep, want) and int(keep.sum()) == top_k
+        else:
+            assert int(np.sum(keep != want)) <= 1 and not (keep & ~kept_set(z, temperature, 1.0, top_k)).any()
+        if np.array_equal(keep, want):
+            assert tok == sample_token(z, temperature, top_p, u, top_k)
