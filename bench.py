@@ -225,13 +225,13 @@ def run_full_rollout(args):
         eng.load_weights(m, w_host[m])
     del w_host
     seed = 20260628
-    prm = T.TandemParams(table, p=wl.p, temperature=wl.temperature, top_p=wl.top_p, top_k=args.top_k, seed=seed)
+    prm = T.TandemParams(table, p=wl.p, switch_mode=wl.switch_mode, temperature=wl.temperature, top_p=wl.top_p, top_k=args.top_k or wl.top_k, seed=seed)
     t0 = time.perf_counter()
     g = eng.generate(prm, prompts, max_new)
     dt = time.perf_counter() - t0
     assert (g["len"] == max_new).all()
     for b in sorted(set([0, B // 3, B - 1])):
-        o = owners_from_tokens(g["tokens"][b, :g["len"][b]], table, OParams(p=wl.p, seed=seed), Uniforms(seed=seed), b=b)
+        o = owners_from_tokens(g["tokens"][b, :g["len"][b]], table, OParams(p=wl.p, switch_mode=wl.switch_mode, seed=seed), Uniforms(seed=seed), b=b)
         assert np.array_equal(o, g["owner"][b, :g["len"][b]]), "owner flags differ from the rule replayed on the returned tokens"
     st = g["stats"]
     tok = int(g["len"].sum())
@@ -334,7 +334,7 @@ def run_ours(args):
     prefill_rows = sum(len(p) for p in prompts)
     row_cap = 4096
     prefill_steps = (prefill_rows + row_cap - 1) // row_cap + 2
-    gen_budget = prefill_steps + max(args.ramp, int(4.0 / max(wl.p * wl.word_start_frac, 1e-3))) + args.max_drain + W + K + args.profile_steps + 64
+    gen_budget = prefill_steps + max(args.ramp, int(8.0 / max(wl.p * wl.word_start_frac, 1e-3))) + args.max_drain + W + K + args.profile_steps + 64
     max_seq_len = ((max_prompt + max(gen_budget, args.e2e_new) + 15) // 16) * 16
     eng = T.Tandem(T.TandemConfig(shape, max_seqs=B, max_seq_len=max_seq_len, device=local, max_rows_per_step=row_cap, use_graph=1))
     w_cpu = []
@@ -346,7 +346,7 @@ def run_ours(args):
                               layers=[{k: v.cpu() for k, v in l.items()} for l in w["layers"]]))
         del w
         torch.cuda.empty_cache()
-    prm = T.TandemParams(table, p=wl.p, temperature=wl.temperature, top_p=wl.top_p, top_k=args.top_k, seed=20260628)
+    prm = T.TandemParams(table, p=wl.p, switch_mode=wl.switch_mode, temperature=wl.temperature, top_p=wl.top_p, top_k=args.top_k or wl.top_k, seed=20260628)
     out = dict(token=torch.zeros(B, dtype=torch.int32, device="cuda"), owner=torch.zeros(B, dtype=torch.uint8, device="cuda"),
                sen_logp=torch.zeros(B, device="cuda"), done=torch.zeros(B, dtype=torch.uint8, device="cuda"))
     stream = torch.cuda.current_stream().cuda_stream
@@ -360,8 +360,8 @@ def run_ours(args):
         if st["tokens_emitted"] >= B or n_setup > 4 * prefill_steps + 16:
             break
         eng.step(prm, out=out, stream=stream); n_setup += 1
-    # every sequence should have changed hands a few times before timing: ~4 expected switches per sequence (rate p * f per token)
-    ramp = max(args.ramp, int(4.0 / (wl.p * wl.word_start_frac)) if wl.p * wl.word_start_frac > 0 else 0)
+    # every sequence should have changed hands a few times before timing: ~8 expected switches per sequence (e^-8 of them none) (rate p * f per token)
+    ramp = max(args.ramp, int(8.0 / (wl.p * wl.word_start_frac)) if wl.p * wl.word_start_frac > 0 else 0)
     for _ in range(ramp):
         eng.step(prm, out=out, stream=stream)
     # keep stepping until the partner's first catch-up over the (fast-forwarded) context has drained: steady state is
@@ -448,7 +448,7 @@ def run_ours(args):
     res = {"metric": METRIC, "value": tokens_all / (ms_all * 1e-3), "unit": "tokens/s", "n_gpus": world, "steps": K, "warmup": W,
            "ms_per_step": ms_all / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
            "config": {"workload": wl.name, "batch_per_gpu": B, "prompt_len": list(wl.prompt_len), "fast_forward": args.fast_forward,
-                      "ctx_mean_timed": ctx_mean, "p": wl.p, "word_start_frac": wl.word_start_frac, "temperature": wl.temperature, "top_p": wl.top_p, "top_k": args.top_k,
+                      "ctx_mean_timed": ctx_mean, "p": wl.p, "word_start_frac": wl.word_start_frac, "temperature": wl.temperature, "top_p": wl.top_p, "top_k": args.top_k or wl.top_k, "switch_mode": "REDRAW" if wl.switch_mode else "TOGGLE",
                       "page_tokens": 16, "parallelism": "dp%d (independent sequences, replicated weights, no collective)" % world,
                       "l2": "inputs larger than L2 (16.1 GB of weights + KV streamed per step vs 126 MB L2)",
                       "setup_steps": n_setup + ramp + n_drain, "setup_seconds": setup_s, "cuda_graph": True},
@@ -510,7 +510,7 @@ def oracle_rollout(wl, w_cpu, prompt, table, seq_id, n_new, prm_seed, models=Non
         except Exception:
             roomy = False
         models = (OracleModel(wl.shape, w_cpu[0], cache=roomy), OracleModel(wl.shape, w_cpu[1], cache=roomy))
-    op = OParams(p=wl.p, temperature=wl.temperature, top_p=wl.top_p, seed=prm_seed)
+    op = OParams(p=wl.p, switch_mode=wl.switch_mode, temperature=wl.temperature, top_p=wl.top_p, top_k=wl.top_k, seed=prm_seed)
     t0 = time.perf_counter()
     r = tandem_generate(models, op, [prompt], [n_new], table, uni=Uniforms(seed=prm_seed, seq_ids=[int(seq_id)]))
     dt = time.perf_counter() - t0

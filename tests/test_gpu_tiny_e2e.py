@@ -120,6 +120,38 @@ def test_nucleus_rollouts_match_oracle(temperature, top_p, top_k):
     eng.free()
 
 
+@pytest.mark.parametrize("mode,p", [(T.TOGGLE, 1.0), (T.REDRAW, 0.5)])
+def test_reasoning_step_handoff_protocol(mode, p):
+    """The paper's evaluation protocol (L99 section 4.3: strict alternation at every boundary token; L480 App. C.5: Bernoulli(0.5)
+    draw of the next contributor) with the evaluation sampler (T 0.7, top-p 0.8, top-k 20): a sparse boundary table, TOGGLE p = 1
+    or REDRAW p = 0.5. Tokens / owners / mask as the oracle's; under strict alternation the owner changes exactly after each
+    boundary token and never elsewhere."""
+    shape = get_workload("cfg1_tiny_f32").shape
+    ws = make_word_start(shape.vocab, 0.08, 13)
+    rng = np.random.default_rng(9)
+    B = 4
+    prompts = [rng.integers(0, shape.vocab, size=int(n)).astype(np.int32) for n in (5, 18, 31, 12)]
+    max_new = np.array([48, 40, 33, 48], dtype=np.int32)
+    eng, orc, _ = make_pair(shape, (1, 2), max_seqs=4, max_seq_len=96, gain_jitter=0.1)
+    kw = dict(p=p, switch_mode=mode, temperature=0.7, top_p=0.8, top_k=20, seed=31)
+    ref = tandem_generate(orc, OParams(**kw), prompts, max_new, ws, uni=Uniforms(seed=31, seq_ids=np.arange(B, dtype=np.int32)))
+    out = eng.generate(T.TandemParams(ws, **kw), prompts, max_new)
+    _compare(out, ref, B, logp_tol=2e-5)
+    switches = 0
+    for b in range(B):
+        n = out["len"][b]
+        tok, own = out["tokens"][b, :n], out["owner"][b, :n]
+        flips = own[1:] != own[:-1]
+        boundary = ws[tok[:-1]].astype(bool)
+        if mode == T.TOGGLE:
+            assert np.array_equal(flips, boundary)
+        else:
+            assert not flips[~boundary].any()
+        switches += int(flips.sum())
+    assert switches >= 3
+    eng.free()
+
+
 def test_explicit_sample_uniforms_and_forced_tokens():
     shape = get_workload("cfg1_tiny_f32").shape
     ws = make_word_start(shape.vocab, 0.3, 11)

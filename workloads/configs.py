@@ -45,7 +45,9 @@ class Workload:
     geom_mean: float = 0.0         # > 0: max_new[b] = min(Geometric(1/geom_mean), max_new)   (R8)
     temperature: float = 1.0       # 0 => greedy
     top_p: float = 1.0
+    top_k: int = 0                 # 0 = off (Table 3: training -1, evaluation 20)
     p: float = 0.5
+    switch_mode: int = 0           # 0 TOGGLE, 1 REDRAW (the values of tandem.h / oracle.rule)
     word_start_frac: float = 0.30
     explicit_uniforms: bool = False
     page_tokens: int = 16
@@ -73,6 +75,14 @@ WORKLOADS = {
     "cfg4_4b_long": Workload("cfg4_4b_long", FOURB, 64, 8, (64, 512), 8192, geom_mean=3000.0),
     # configs[4]: switch-rate sweep base point (p and word_start_frac are swept by the caller)
     "cfg5_sweep": Workload("cfg5_sweep", FOURB, 16, 8, (256, 256), 2048),
+    # Reasoning-step handoff, the paper's evaluation protocol (section 4.3: the two models "alternate at every
+    # \\n\\n-boundary token, each producing one reasoning step"; L480-482 App. C.5: an independent Bernoulli(0.5) draw at every
+    # boundary instead), with the evaluation sampler of Table 3 (T 0.7, top-p 0.8, top-k 20). The table marks the boundary ids;
+    # the stand-in marks 2% of the vocabulary, i.e. a reasoning step of about 50 tokens (the paper gives no step length).
+    "handoff_strict_4b": Workload("handoff_strict_4b", FOURB, 16, 8, (64, 512), 4096, temperature=0.7, top_p=0.8, top_k=20, p=1.0,
+                                  switch_mode=0, word_start_frac=0.02),
+    "handoff_bernoulli_4b": Workload("handoff_bernoulli_4b", FOURB, 16, 8, (64, 512), 4096, temperature=0.7, top_p=0.8, top_k=20, p=0.5,
+                                     switch_mode=1, word_start_frac=0.02),
 }
 
 
