@@ -34,11 +34,12 @@ from .sampler import sample_token, log_prob, kept_set_top_p, kept_set
 from .rule import (SENIOR, JUNIOR, DRAW, TOGGLE, REDRAW, TandemParams,
                    owners_from_tokens, tandem_generate, solo_generate)
 from .score import teacher_forced_logits, replay_owner_logits, overlap_from_logits, dual_score
+from .grpo import group_advantages, grpo_objective
 
 __all__ = [
     "philox4x32_10", "uniform_from_bits", "uniforms_sample", "uniforms_switch", "gumbel_from_uniform",
     "OracleModel", "KVState", "sample_token", "log_prob", "kept_set_top_p", "kept_set",
     "SENIOR", "JUNIOR", "DRAW", "TOGGLE", "REDRAW", "TandemParams",
     "owners_from_tokens", "tandem_generate", "solo_generate",
-    "teacher_forced_logits", "replay_owner_logits", "overlap_from_logits", "dual_score",
+    "teacher_forced_logits", "replay_owner_logits", "overlap_from_logits", "dual_score", "group_advantages", "grpo_objective",
 ]
