@@ -45,6 +45,7 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg3_4b_bf16")
     ap.add_argument("--p", type=float, default=None, help="override the workload's switch probability (cfg5 sweep)")
+    ap.add_argument("--grpo", action="store_true", help="time tandem_grpo_objective (senior-masked GRPO forward, NEXT-3) on the workload's batch x max_new")
     ap.add_argument("--score", type=int, default=0, help="N > 0: time tandem_score (teacher-forced dual scoring, NEXT-1) on N synthetic streams instead of the rollout")
     ap.add_argument("--score-len", type=int, default=2048, help="tokens per stream for --score")
     ap.add_argument("--score-rows", type=int, default=512, help="rows per step and model for --score (max_rows_per_step)")
@@ -250,6 +251,56 @@ def run_full_rollout(args):
                       "e2e": {"value": tok / dt, "unit": "tokens/s", "h2d_bytes_per_step": sum(len(p) for p in prompts) * 4 / max(1, st["steps"]),
                               "d2h_bytes_per_step": tok * 9 / max(1, st["steps"])}}))
     eng.free()
+
+
+def run_grpo(args):
+    """tandem_grpo_objective on device buffers of the workload's rollout shape (B = prompts x G rollouts, L = max_new): advantages,
+    clipped senior-masked surrogate, loss. HBM-bound element-wise work: bytes = B L (owner 1 + two log-probs 8 [+ 4 token output])."""
+    import torch
+    import paper_2606_28166_b200 as T
+    from workloads import get_workload
+    torch.cuda.set_device(0)
+    T.build()
+    wl = get_workload(args.workload)
+    B, L, G = wl.batch, wl.max_new, wl.group
+    g = torch.Generator(device="cuda"); g.manual_seed(1)
+    rewards = (torch.rand(B, device="cuda", generator=g) < 0.4).float()
+    lengths = torch.randint(L // 2, L + 1, (B,), device="cuda", generator=g, dtype=torch.int32)
+    owner = (torch.rand(B, L, device="cuda", generator=g) < 0.5).to(torch.uint8)
+    old = -3 * torch.rand(B, L, device="cuda", generator=g)
+    new = old + 0.1 * torch.randn(B, L, device="cuda", generator=g)
+    out = {}
+    for want_tokens in (False, True):
+        for _ in range(5):
+            r = T.grpo_objective(rewards, G, lengths, owner, new, old, want_tokens=want_tokens)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        n = max(20, args.steps)
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+        res = torch.empty(8, device="cuda")
+        tot = 0.0
+        for _ in range(n):
+            flush.zero_()                                # inputs (4.7 MB) would otherwise sit in L2
+            e0.record()
+            lib_rc = T.binding.lib().tandem_grpo_objective(B // G, G, L, rewards.data_ptr(), lengths.data_ptr(), owner.data_ptr(), new.data_ptr(),
+                                                           old.data_ptr(), None, 0.2, 0.0, 1e-6, r["advantages"].data_ptr(),
+                                                           r["token_obj"].data_ptr() if want_tokens else None, r["seq_obj"].data_ptr(),
+                                                           res.data_ptr(), None)
+            e1.record(); torch.cuda.synchronize()
+            assert lib_rc == 0
+            tot += e0.elapsed_time(e1)
+        us = tot / n * 1e3
+        byt = B * L * (9 + (4 if want_tokens else 0))
+        out["with_token_obj" if want_tokens else "scalars_only"] = {"us_per_call": us, "alg_bytes": byt, "gbs": byt / us / 1e3}
+    pk = peaks()
+    best = out["scalars_only"]
+    print(json.dumps({"metric": "senior-masked GRPO objective, forward (rollout tokens/s consumed)", "value": B * L / (best["us_per_call"] * 1e-6),
+                      "unit": "tokens/s", "n_gpus": 1, "steps": max(20, args.steps), "warmup": 5, "ms_per_step": best["us_per_call"] * 1e-3,
+                      "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                      "config": {"workload": wl.name, "mode": "tandem_grpo_objective", "rollouts": B, "group": G, "stride": L, "l2": "flushed between calls"},
+                      "gpu_launches": 1, "variants": out,
+                      "roofline": {"bound": "hbm", "achieved": best["gbs"], "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": best["gbs"] / pk["hbm_gbs"],
+                                   "traffic": None, "note": "one memset and one kernel of a few microseconds: launch latency and the tail of 128 CTAs, not bandwidth, set the time at this size"},
+                      "loss": r["loss"], "clip_frac": r["clip_frac"]}))
 
 
 def run_score(args):
@@ -565,6 +616,8 @@ if __name__ == "__main__":
     a = parse_args()
     if a.impl == "reference":
         run_reference(a)
+    elif a.grpo:
+        run_grpo(a)
     elif a.score > 0:
         run_score(a)
     elif a.full_rollout > 0:

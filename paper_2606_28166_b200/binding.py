@@ -15,7 +15,7 @@ GEMM_AUTO, GEMM_SIMT, GEMM_TCGEN05 = 0, 1, 2
 ATTN_AUTO, ATTN_ALU, ATTN_MMA = 0, 1, 2
 _ERR = {0: "OK", -1: "EINVAL", -2: "ENOMEM", -3: "ECUDA", -4: "ESTATE", -5: "EFULL"}
 
-EXPORTED_SYMBOLS = ["tandem_init", "tandem_load_weights", "tandem_step", "tandem_generate", "tandem_score", "tandem_reset",
+EXPORTED_SYMBOLS = ["tandem_init", "tandem_load_weights", "tandem_step", "tandem_generate", "tandem_score", "tandem_grpo_objective", "tandem_reset",
                     "tandem_free", "tandem_last_error", "tandem_get_stats", "tandem_set_profile", "tandem_get_profile",
                     "tandem_kernel_class_name", "tandem_debug_lt_times", "tandem_test_uniforms", "tandem_test_nucleus", "tandem_test_philox", "tandem_test_gemm", "tandem_test_gemm_time"]
 KC_NUM = 16
@@ -84,6 +84,7 @@ def lib():
         L.tandem_load_weights.argtypes = [C.c_void_p, C.c_int, C.POINTER(_Weights)]
         L.tandem_step.argtypes = [C.c_void_p, C.POINTER(_StepIn), C.POINTER(_StepOut), C.c_void_p]
         L.tandem_score.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.tandem_grpo_objective.argtypes = [C.c_int32, C.c_int32, C.c_int32] + [C.c_void_p] * 6 + [C.c_float] * 3 + [C.c_void_p] * 5
         L.tandem_generate.argtypes = [C.c_void_p, C.POINTER(_Params), C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                       C.POINTER(_Overrides), C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                       C.POINTER(_Stats), C.c_void_p]
@@ -267,6 +268,28 @@ class Tandem:
             self.free()
         except Exception:
             pass
+
+
+def grpo_objective(rewards, group, lengths, owner, logp_new, logp_old, logp_ref=None, clip_eps=0.2, kl_beta=0.0, adv_eps=1e-6,
+                   want_tokens=True, stream=None):
+    """Senior-masked GRPO objective on device tensors (torch, CUDA): rewards [B] f32, lengths [B] i32, owner [B, L] u8, logp_* [B, L]
+    f32. Returns dict(advantages [B], token_obj [B, L] | None, seq_obj [B], loss, clip_frac, n_senior, n_live) - the scalars after a
+    synchronising copy."""
+    import torch
+    B, L = owner.shape
+    assert B % group == 0 and rewards.numel() == B and lengths.numel() == B
+    for t_ in (rewards, lengths, owner, logp_new, logp_old) + ((logp_ref,) if logp_ref is not None else ()):
+        assert t_.is_cuda and t_.is_contiguous()
+    adv = torch.empty(B, dtype=torch.float32, device=owner.device); seq = torch.empty_like(adv)
+    tok = torch.empty(B, L, dtype=torch.float32, device=owner.device) if want_tokens else None
+    res = torch.empty(8, dtype=torch.float32, device=owner.device)
+    rc = lib().tandem_grpo_objective(B // group, group, L, rewards.data_ptr(), lengths.data_ptr(), owner.data_ptr(), logp_new.data_ptr(),
+                                     logp_old.data_ptr(), _ptr(logp_ref), clip_eps, kl_beta, adv_eps, adv.data_ptr(), _ptr(tok), seq.data_ptr(),
+                                     res.data_ptr(), stream)
+    if rc:
+        raise TandemError(rc)
+    r = res.cpu().numpy()
+    return dict(advantages=adv, token_obj=tok, seq_obj=seq, loss=float(r[0]), clip_frac=float(r[1]), n_senior=int(r[2]), n_live=int(r[3]))
 
 
 def tandem_test_uniforms(seed, seq_id, t, stream, n, out_dev):

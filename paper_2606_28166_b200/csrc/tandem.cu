@@ -21,6 +21,7 @@
 #include "gemm_simt.cuh"
 #include "gemm_tcgen05.cuh"
 #include "layer_tail.cuh"
+#include "grpo.cuh"
 
 using namespace tandem;
 constexpr int kSampleMaxChunks = 32;
@@ -1090,6 +1091,21 @@ int tandem_score(tandem_handle* h, int32_t n_seqs, const int32_t* tokens, const 
     stats->seconds_total = ms * 1e-3;
   }
   return TANDEM_OK;
+}
+
+int tandem_grpo_objective(int32_t n_groups, int32_t group, int32_t stride, const float* rewards, const int32_t* len, const uint8_t* owner,
+                          const float* logp_new, const float* logp_old, const float* logp_ref, float clip_eps, float kl_beta, float adv_eps,
+                          float* advantages, float* token_obj, float* seq_obj, float* result, void* cuda_stream) {
+  if (n_groups < 0 || group < 1 || stride < 1 || !(clip_eps >= 0.f) || !(adv_eps >= 0.f)) return TANDEM_EINVAL;
+  if (!rewards || !len || !owner || !logp_new || !logp_old || !advantages || !seq_obj || !result) return TANDEM_EINVAL;
+  if (kl_beta != 0.f && !logp_ref) return TANDEM_EINVAL;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  const int B = n_groups * group;
+  if (cudaMemsetAsync(result, 0, 8 * sizeof(float), s) != cudaSuccess) { cudaGetLastError(); return TANDEM_ECUDA; }
+  if (B == 0) return TANDEM_OK;
+  const GrpoArgs a{B, group, stride, rewards, len, owner, logp_new, logp_old, logp_ref, clip_eps, kl_beta, adv_eps, advantages, token_obj, seq_obj, result};
+  grpo_seq_kernel<256><<<B, 256, 0, s>>>(a);
+  return cudaGetLastError() == cudaSuccess ? TANDEM_OK : TANDEM_ECUDA;
 }
 
 void tandem_free(tandem_handle* h) {
