@@ -97,6 +97,44 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
         "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
       : "r"(taddr));
 }
+// ---- CTA pair (cta_group::2): two CTAs of a cluster on the two SMs of a TPC drive one M = 256 MMA; each holds its own 128
+// weight rows (A) and HALF of the token rows (B), so the activation bytes an SM has to pull out of L2 halve.
+__device__ __forceinline__ uint32_t cluster_ctarank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ void cluster_sync_all() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ uint32_t mapa_rank(uint32_t addr, uint32_t rank) {   // the same shared-memory offset in CTA `rank` of the cluster
+  uint32_t r; asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank)); return r;
+}
+__device__ __forceinline__ void mbar_expect_tx_cluster(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.release.cluster.shared::cluster.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar) {
+  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+// TMA load into this CTA's shared memory that signals a barrier which may live in the peer CTA of the pair
+__device__ __forceinline__ void tma_load_2d_pair(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar_cluster, uint64_t policy) {
+  asm volatile("cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3}], [%4], %5;"
+               ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar_cluster), "l"(policy) : "memory");
+}
+template <int COLS> __device__ __forceinline__ void tmem_alloc_pair(uint32_t smem_dst) {
+  asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "n"(COLS) : "memory");
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+}
+template <int COLS> __device__ __forceinline__ void tmem_dealloc_pair(uint32_t taddr) {
+  asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(taddr), "n"(COLS) : "memory");
+}
+__device__ __forceinline__ void umma_bf16_pair(uint32_t d_tmem, uint64_t desc_a, uint64_t desc_b, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem), "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+// arrives on the barrier at this shared-memory offset in BOTH CTAs of the pair once the MMAs issued so far have completed
+__device__ __forceinline__ void umma_commit_pair(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(bar), "h"((uint16_t)3) : "memory");
+}
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 // One lane of a converged warp. The TMA / MMA warps run their loops with all 32 lanes and issue under elect_one(): the operands
 // (descriptors, addresses) are then provably warp-uniform and stay in uniform registers. Issued from a single divergent thread
@@ -120,8 +158,8 @@ __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t smem_addr) {
   return d;
 }
 // Instruction descriptor, kind::f16: D fp32, A and B bf16, both K-major, M = 128, N = n (multiple of 16, <= 256).
-__device__ __forceinline__ uint32_t umma_idesc_bf16(int n) {
-  return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(kTcTileN >> 4) << 24);
+__device__ __forceinline__ uint32_t umma_idesc_bf16(int n, int m = kTcTileN) {
+  return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(m >> 4) << 24);
 }
 
 struct TcMaps { CUtensorMap w[2], a[2][4]; };   // per model: weight descriptor; activation descriptors with 128/64/32/16-row boxes
@@ -141,8 +179,13 @@ enum { kTcEpiPartial = 0, kTcEpiSwiGLU = 1 };
 // EPI  = kTcEpiPartial: fp32 partial out[split][r][n];
 //        kTcEpiSwiGLU : W rows interleaved (2i = gate_i, 2i+1 = up_i), n_split = 1: act[r][i] = silu(gate) * up as bf16.
 // Cluster launches with TMA multicast of the activation boxes (2 and 4 CTAs) were built and measured: no gain at any of
-// the projection shapes on B200 (profiles/gemm_sweep_r1.md), so the kernel is single-CTA.
-template <int EPI>
+// the projection shapes on B200 (profiles/gemm_sweep_r1.md): multicast does not lower what each SM has to ingest. The CTA pair does.
+// PAIR = true: launched in clusters of two CTAs along x (adjacent weight tiles). The pair runs one cta_group::2 MMA with M = 256:
+//        each CTA streams its own 128 weight rows and HALF of the token rows, both signal the leader's (rank 0) full barrier,
+//        the leader's MMA warp issues for both and its commits arrive on the empty / accumulator barriers of both CTAs; each CTA
+//        drains its own 128 TMEM lanes. The activation bytes an SM pulls out of L2 halve (profiles/gemm_sweep_r1.md: the
+//        projections are bound by SM ingest, not HBM, above ~64 token rows).
+template <int EPI, bool PAIR>
 __global__ void __launch_bounds__(kTcThreads, 1)
 gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ Pair<TcGemmArgs> gp) {
   const TcGemmArgs& g = gp.m[blockIdx.z];                  // blockIdx.z = model
@@ -156,13 +199,18 @@ gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__
   const int rows = g.rows_ptr ? *g.rows_ptr : g.rows_fixed;   // scheduler output: complete before any kernel of the chain starts
   if (rows <= 0) { pdl_wait(); return; }                   // uniform over the grid: nothing was scheduled for this model
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = PAIR ? ptx::cluster_ctarank() : 0u;
+  const bool leader = rank == 0;
   const int n0 = blockIdx.x * kTcTileN;
   const int split = blockIdx.y;
   const int kb_total = (g.K + kTcBlockK - 1) / kTcBlockK;
   const int kb0 = (int)((long long)kb_total * split / g.n_split);
   const int kb1 = (int)((long long)kb_total * (split + 1) / g.n_split);
   const int n_chunks = (rows + kTcMaxRows - 1) / kTcMaxRows;
-  const int nbox_max = (min(rows, kTcMaxRows) + kTcRowBox - 1) / kTcRowBox;
+  // token rows of a chunk are padded to the box granularity; a pair splits them in two halves of whole boxes
+  constexpr int kPad = PAIR ? 2 * kTcRowBox : kTcRowBox;
+  auto chunk_cols = [&](int r0) { return ((min(rows - r0, kTcMaxRows) + kPad - 1) / kPad) * kPad; };
+  const int nbox_max = chunk_cols(0) / kTcRowBox / (PAIR ? 2 : 1);   // boxes this CTA loads per stage
   const int stage_bytes = kTcWBytes + nbox_max * kTcABoxBytes;
   const int n_stages = min(kTcMaxStages, g.ring_bytes / stage_bytes);
 
@@ -174,16 +222,17 @@ gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__
   const uint32_t tmem_empty_bar = tmem_full_bar + 8u;
 
   if (threadIdx.x == 0) {
-    for (int s = 0; s < n_stages; ++s) { ptx::mbar_init(full_bar(s), 2); ptx::mbar_init(empty_bar(s), 1); }   // full: weight + activation producers
+    // full: weight + activation producers (a pair: the leader's two, which also post the peer's bytes); empty / accumulator-full: one commit
+    for (int s = 0; s < n_stages; ++s) { ptx::mbar_init(full_bar(s), 2); ptx::mbar_init(empty_bar(s), 1); }
     ptx::mbar_init(tmem_full_bar, 1);
-    ptx::mbar_init(tmem_empty_bar, 4);
+    ptx::mbar_init(tmem_empty_bar, PAIR ? 8 : 4);          // the epilogue warps (of both CTAs; only the leader's is used)
     ptx::fence_mbar_init();
     ptx::prefetch_tmap(tmap_w);
     ptx::prefetch_tmap(tmap_a);
   }
-  if (warp == 2) ptx::tmem_alloc<kTcMaxRows>(ptx::smem_u32(&tmem_base_smem));
+  if (warp == 2) { if (PAIR) ptx::tmem_alloc_pair<kTcMaxRows>(ptx::smem_u32(&tmem_base_smem)); else ptx::tmem_alloc<kTcMaxRows>(ptx::smem_u32(&tmem_base_smem)); }
   ptx::tc_fence_before();
-  __syncthreads();
+  if (PAIR) ptx::cluster_sync_all(); else __syncthreads();   // barriers of both CTAs are initialised before anyone signals them
   ptx::tc_fence_after();
   const uint32_t tmem_base = tmem_base_smem;
 
@@ -198,8 +247,13 @@ gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__
           const int s = it % n_stages;
           ptx::mbar_wait(empty_bar(s), ((uint32_t)(it / n_stages) & 1u) ^ 1u);
           if (ptx::elect_one()) {
-            ptx::mbar_expect_tx(full_bar(s), (uint32_t)kTcWBytes);
-            ptx::tma_load_2d(ring + (uint32_t)(s * stage_bytes), tmap_w, kb * kTcBlockK, n0, full_bar(s), pol_w);
+            if (PAIR) {   // the leader posts the bytes of both CTAs' loads (a remote arrive per stage would stall the peer's producer)
+              if (leader) ptx::mbar_expect_tx(full_bar(s), 2u * (uint32_t)kTcWBytes);
+              ptx::tma_load_2d_pair(ring + (uint32_t)(s * stage_bytes), tmap_w, kb * kTcBlockK, n0, ptx::mapa_rank(full_bar(s), 0), pol_w);
+            } else {
+              ptx::mbar_expect_tx(full_bar(s), (uint32_t)kTcWBytes);
+              ptx::tma_load_2d(ring + (uint32_t)(s * stage_bytes), tmap_w, kb * kTcBlockK, n0, full_bar(s), pol_w);
+            }
           }
           __syncwarp();
         }
@@ -211,19 +265,26 @@ gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__
       pdl_wait();                                            // the activations come from the predecessor kernel
       int it = 0;
       for (int c = 0; c < n_chunks; ++c) {
-        const int r0 = c * kTcMaxRows;
-        const int nbox = (min(rows - r0, kTcMaxRows) + kTcRowBox - 1) / kTcRowBox;
+        const int cols = chunk_cols(c * kTcMaxRows);
+        const int nbox = cols / kTcRowBox / (PAIR ? 2 : 1);
+        const int r0 = c * kTcMaxRows + (PAIR ? (int)rank * (cols / 2) : 0);   // a pair: this CTA's half of the token rows
         for (int kb = kb0; kb < kb1; ++kb, ++it) {
           const int s = it % n_stages;
           ptx::mbar_wait(empty_bar(s), ((uint32_t)(it / n_stages) & 1u) ^ 1u);
           if (ptx::elect_one()) {
-            ptx::mbar_expect_tx(full_bar(s), (uint32_t)(nbox * kTcABoxBytes));
+            const uint32_t fb = PAIR ? ptx::mapa_rank(full_bar(s), 0) : full_bar(s);
+            if (!PAIR) ptx::mbar_expect_tx(fb, (uint32_t)(nbox * kTcABoxBytes));
+            else if (leader) ptx::mbar_expect_tx(full_bar(s), 2u * (uint32_t)(nbox * kTcABoxBytes));
             const uint32_t dst = ring + (uint32_t)(s * stage_bytes) + kTcWBytes;
             int j = 0;
 #pragma unroll
             for (int b = 0; b < 4; ++b) {
               const int bx = 8 >> b;
-              while (nbox - j >= bx) { ptx::tma_load_2d(dst + j * kTcABoxBytes, tmap_a + b, kb * kTcBlockK, r0 + j * kTcRowBox, full_bar(s), pol_a); j += bx; }
+              while (nbox - j >= bx) {
+                if (PAIR) ptx::tma_load_2d_pair(dst + j * kTcABoxBytes, tmap_a + b, kb * kTcBlockK, r0 + j * kTcRowBox, fb, pol_a);
+                else ptx::tma_load_2d(dst + j * kTcABoxBytes, tmap_a + b, kb * kTcBlockK, r0 + j * kTcRowBox, fb, pol_a);
+                j += bx;
+              }
             }
           }
           __syncwarp();
@@ -231,13 +292,12 @@ gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__
       }
     }
   } else if (warp == 1) {
-    // ===== MMA issuer: one elected lane drives the tensor core for the whole CTA
-    {
+    // ===== MMA issuer: one elected lane drives the tensor core for the whole CTA (for both CTAs of a pair: the leader's)
+    if (leader) {
       int it = 0;
       for (int c = 0; c < n_chunks; ++c) {
-        const int r0 = c * kTcMaxRows;
-        const int ncols = ((min(rows - r0, kTcMaxRows) + kTcRowBox - 1) / kTcRowBox) * kTcRowBox;
-        const uint32_t idesc = umma_idesc_bf16(ncols);
+        const int ncols = chunk_cols(c * kTcMaxRows);
+        const uint32_t idesc = umma_idesc_bf16(ncols, PAIR ? 2 * kTcTileN : kTcTileN);
         ptx::mbar_wait(tmem_empty_bar, ((uint32_t)c & 1u) ^ 1u);
         ptx::tc_fence_after();
         for (int kb = kb0; kb < kb1; ++kb, ++it) {
@@ -249,13 +309,15 @@ gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__
           const uint64_t dw = umma_desc_sw128(sw), da = umma_desc_sw128(sw + kTcWBytes);
           if (ptx::elect_one()) {
 #pragma unroll
-            for (int k = 0; k < kTcBlockK / 16; ++k)   // UMMA K = 16 bf16 = 32 bytes: advance the start address inside the swizzle row
-              ptx::umma_bf16(tmem_base, dw + (uint64_t)(2 * k), da + (uint64_t)(2 * k), idesc, (kb > kb0 || k > 0) ? 1u : 0u);
-            ptx::umma_commit(empty_bar(s));            // stage free once these MMAs have read it
+            for (int k = 0; k < kTcBlockK / 16; ++k) {   // UMMA K = 16 bf16 = 32 bytes: advance the start address inside the swizzle row
+              if (PAIR) ptx::umma_bf16_pair(tmem_base, dw + (uint64_t)(2 * k), da + (uint64_t)(2 * k), idesc, (kb > kb0 || k > 0) ? 1u : 0u);
+              else ptx::umma_bf16(tmem_base, dw + (uint64_t)(2 * k), da + (uint64_t)(2 * k), idesc, (kb > kb0 || k > 0) ? 1u : 0u);
+            }
+            if (PAIR) ptx::umma_commit_pair(empty_bar(s)); else ptx::umma_commit(empty_bar(s));   // stage free once these MMAs have read it
           }
           __syncwarp();
         }
-        if (ptx::elect_one()) ptx::umma_commit(tmem_full_bar);   // accumulator of this chunk complete
+        if (ptx::elect_one()) { if (PAIR) ptx::umma_commit_pair(tmem_full_bar); else ptx::umma_commit(tmem_full_bar); }   // accumulator of this chunk complete
         __syncwarp();
       }
     }
@@ -264,6 +326,7 @@ gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__
     const int q = warp & 3;
     const int n = n0 + q * 32 + lane;
     float* outp = g.out + (size_t)split * g.split_stride;
+    const uint32_t te_bar = PAIR ? ptx::mapa_rank(tmem_empty_bar, 0) : tmem_empty_bar;
     pdl_wait();                                            // the predecessor may still be reading the buffer this kernel writes
     for (int c = 0; c < n_chunks; ++c) {
       const int r0 = c * kTcMaxRows;
@@ -299,12 +362,12 @@ gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__
       }
       ptx::tc_fence_before();
       __syncwarp();
-      if (lane == 0) ptx::mbar_arrive(tmem_empty_bar);
+      if (lane == 0) { if (PAIR) ptx::mbar_arrive_cluster(te_bar); else ptx::mbar_arrive(te_bar); }
     }
   }
   ptx::tc_fence_before();
-  __syncthreads();
-  if (warp == 2) ptx::tmem_dealloc<kTcMaxRows>(tmem_base);
+  if (PAIR) ptx::cluster_sync_all(); else __syncthreads();   // a pair: neither CTA leaves while the other may still read its shared memory / signal it
+  if (warp == 2) { if (PAIR) ptx::tmem_dealloc_pair<kTcMaxRows>(tmem_base); else ptx::tmem_dealloc<kTcMaxRows>(tmem_base); }
 }
 
 // ---------------------------------------------------------------------------------------------- host side
@@ -334,8 +397,10 @@ inline TcGemmPlans* tc_gemm_create() {
     return nullptr;
   }
   bool ok = true;
-  ok &= cudaFuncSetAttribute(gemm_tcgen05_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes) == cudaSuccess;
-  ok &= cudaFuncSetAttribute(gemm_tcgen05_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes) == cudaSuccess;
+  ok &= cudaFuncSetAttribute(gemm_tcgen05_kernel<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes) == cudaSuccess;
+  ok &= cudaFuncSetAttribute(gemm_tcgen05_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes) == cudaSuccess;
+  ok &= cudaFuncSetAttribute(gemm_tcgen05_kernel<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes) == cudaSuccess;
+  ok &= cudaFuncSetAttribute(gemm_tcgen05_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes) == cudaSuccess;
   if (!ok) {
     cudaGetLastError();
     return nullptr;
@@ -369,10 +434,12 @@ inline const CUtensorMap* tc_gemm_map(TcGemmPlans* p, const void* base, int n_ro
 // activations [rows, N/2] (epi = kTcEpiSwiGLU; W rows interleaved gate/up). Returns 0, or -1 (TANDEM_EINVAL) / -3 (TANDEM_ECUDA).
 // which == 4 (LM head) never splits: the sampler reads the logits in place.
 template <int EPI>
-inline int tc_gemm_launch_epi(const TcMaps& maps, const Pair<TcGemmArgs>& g, dim3 grid, cudaStream_t s, bool pdl) {
-  return launch_ex(gemm_tcgen05_kernel<EPI>, grid, dim3(kTcThreads), (size_t)g.m[0].ring_bytes + 1024, s, pdl, maps, g) == cudaSuccess ? 0 : -3;
+inline int tc_gemm_launch_epi(const TcMaps& maps, const Pair<TcGemmArgs>& g, dim3 grid, cudaStream_t s, bool pdl, bool pair) {
+  const size_t smem = (size_t)g.m[0].ring_bytes + 1024;
+  if (pair) return launch_ex_cluster(gemm_tcgen05_kernel<EPI, true>, grid, dim3(kTcThreads), smem, s, pdl, 2, maps, g) == cudaSuccess ? 0 : -3;
+  return launch_ex(gemm_tcgen05_kernel<EPI, false>, grid, dim3(kTcThreads), smem, s, pdl, maps, g) == cudaSuccess ? 0 : -3;
 }
-struct TcGemmTune { int ring_kb = 0, splits = 0; bool pdl = false; };   // 0 = automatic; overrides for tuning / tandem_test_gemm_time
+struct TcGemmTune { int ring_kb = 0, splits = 0; bool pdl = false; int pair = 0; };   // pair: 1 = CTA pairs (cta_group::2), 0 = single CTAs   // 0 = automatic; overrides for tuning / tandem_test_gemm_time
 // One launch for n_models (1 or 2) problems of the same shape: out[m] = A[m] W[m]^T, rows of model m from rows_ptr[m].
 inline int tc_gemm_launch(TcGemmPlans* p, int n_models, int which, const void* const* A, const void* const* W, int N, int K, float* const* out,
                           const int32_t* const* rows_ptr, int rows_cap, int* n_split, size_t* split_stride, cudaStream_t s, int epi = kTcEpiPartial,
@@ -383,7 +450,8 @@ inline int tc_gemm_launch(TcGemmPlans* p, int n_models, int which, const void* c
   *n_split = S;
   *split_stride = (size_t)rows_cap * N;
   const int tiles = (N + kTcTileN - 1) / kTcTileN;
-  const int tiles_pad = tiles;
+  const bool pair = tune && tune->pair > 0;
+  const int tiles_pad = pair ? (tiles + 1) & ~1 : tiles;   // a pair takes two adjacent weight tiles (a tile past N reads zeros and writes nothing)
   TcMaps maps;
   Pair<TcGemmArgs> g;
   const int ring = (tune && tune->ring_kb > 0) ? tune->ring_kb * 1024
@@ -402,8 +470,8 @@ inline int tc_gemm_launch(TcGemmPlans* p, int n_models, int which, const void* c
   }
   dim3 grid(tiles_pad, S, n_models);
   const bool pdl = tune && tune->pdl;
-  if (epi == kTcEpiSwiGLU) return tc_gemm_launch_epi<1>(maps, g, grid, s, pdl);
-  return tc_gemm_launch_epi<0>(maps, g, grid, s, pdl);
+  if (epi == kTcEpiSwiGLU) return tc_gemm_launch_epi<1>(maps, g, grid, s, pdl, pair);
+  return tc_gemm_launch_epi<0>(maps, g, grid, s, pdl, pair);
 }
 
 // Unit-test hook: out[rows, N] = A W^T (partials summed here), synchronous.
@@ -414,13 +482,14 @@ __global__ void tc_sum_partials_kernel(const float* __restrict__ part, int n_spl
     out[i] = v;
   }
 }
-inline int tc_gemm_test(int rows, int N, int K, const void* A, const void* W, float* out, int epi = kTcEpiPartial) {
+inline int tc_gemm_test(int rows, int N, int K, const void* A, const void* W, float* out, int epi = kTcEpiPartial, bool pair = false) {
+  TcGemmTune tune; tune.pair = pair ? 1 : 0;
   if (rows == 0) return 0;
   TcGemmPlans* p = tc_gemm_create();
   if (!p) return -3;
   if (epi == kTcEpiSwiGLU) {   // W rows interleaved gate/up; out is bf16 [rows, N/2]
     int ns; size_t ss;
-    int rc = tc_gemm_launch(p, 1, 2, &A, &W, N, K, &out, nullptr, rows, &ns, &ss, 0, epi);
+    int rc = tc_gemm_launch(p, 1, 2, &A, &W, N, K, &out, nullptr, rows, &ns, &ss, 0, epi, &tune);
     if (rc == 0) rc = cudaDeviceSynchronize() == cudaSuccess ? 0 : -3;
     tc_gemm_destroy(p);
     return rc;
@@ -429,7 +498,7 @@ inline int tc_gemm_test(int rows, int N, int K, const void* A, const void* W, fl
   float* part = nullptr;
   if (cudaMalloc(&part, (size_t)S * rows * N * sizeof(float)) != cudaSuccess) { tc_gemm_destroy(p); return -2; }
   int ns; size_t ss;
-  int rc = tc_gemm_launch(p, 1, 0, &A, &W, N, K, &part, nullptr, rows, &ns, &ss, 0);
+  int rc = tc_gemm_launch(p, 1, 0, &A, &W, N, K, &part, nullptr, rows, &ns, &ss, 0, kTcEpiPartial, &tune);
   if (rc == 0) {
     tc_sum_partials_kernel<<<296, 256>>>(part, ns, ss, out, (size_t)rows * N);
     rc = cudaDeviceSynchronize() == cudaSuccess ? 0 : -3;

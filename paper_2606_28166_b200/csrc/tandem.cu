@@ -69,6 +69,9 @@ struct tandem_handle {
   int row_cap = 0, max_pages = 0, pool_pages = 0, tile_tok = 0, max_items = 0, max_comb = 0, part_cap = 0, gemm_impl = TANDEM_GEMM_SIMT, attn_impl = TANDEM_ATTN_ALU;
   int n_sms = 148;
   int attn_ctas_per_sm = 2, gemm_ring_kb = 0;   // tuning knobs (env TANDEM_ATTN_CTAS_PER_SM, TANDEM_GEMM_RING_KB; 0 = automatic)
+  int gemm_pair = -1;                            // tcgen05 projections as CTA pairs (cta_group::2): -1 = automatic (while scoring: hundreds of
+                                                 // rows per launch, +5%; no gain at the rollout's ~128 rows), 0 / 1 = env TANDEM_GEMM_PAIR
+  bool scoring = false;
   bool use_tail = false;                        // persistent layer-tail kernel (bf16 + tcgen05 + tensor-core attention; env TANDEM_TAIL=1 enables)
   LtWMaps* lt_wmaps = nullptr; LtAMaps* lt_amaps = nullptr; bool lt_maps_ready = false;   // device tensor-map tables of the layer-tail kernel
   unsigned long long* lt_ts = nullptr;          // env TANDEM_LT_DEBUG=1: per-phase timestamps of the layer-tail launches (tandem_debug_lt_times)
@@ -158,7 +161,7 @@ int launch_gemm(tandem_handle* h, int which, const void* const* A, const void* c
   static const int cls_of[5] = {TANDEM_KC_GEMM_QKV, TANDEM_KC_GEMM_O, TANDEM_KC_GEMM_GATEUP, TANDEM_KC_GEMM_DOWN, TANDEM_KC_GEMM_LMHEAD};
   if (h->gemm_impl == TANDEM_GEMM_TCGEN05 && sizeof(T) == 2) {
     int rc = 0;
-    TcGemmTune tune; tune.ring_kb = h->gemm_ring_kb; tune.pdl = h->use_pdl;
+    TcGemmTune tune; tune.ring_kb = h->gemm_ring_kb; tune.pdl = h->use_pdl; tune.pair = h->gemm_pair >= 0 ? h->gemm_pair : (h->scoring ? 1 : 0);
     KL(h, cls_of[which], s, rc = tc_gemm_launch(h->tc, 2, which, A, W, N, K, out, rows_ptr, rows_cap, n_split, split_stride, s, epi, &tune));
     return rc == 0 ? TANDEM_OK : fail(h, rc, "tcgen05 GEMM launch failed (tensor map encode or K % 8 != 0)");
   }
@@ -637,7 +640,7 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
   tandem_handle* h = new tandem_handle();
   h->cfg = *cfg;
   const tandem_config& c = h->cfg;
-  auto bad = [&](const char* m) { int rc = fail(h, TANDEM_EINVAL, m); fprintf(stderr, "tandem_init: %s\n", m); delete h; return rc; };
+  auto bad = [&](const char* m) { int rc = fail(h, TANDEM_EINVAL, m); fprintf(stderr, "tandem_init: %s\n", m); tandem_free(h); return rc; };   // frees whatever was allocated so far
   if (c.n_layers < 1 || c.hidden < 8 || c.n_q_heads < 1 || c.n_kv_heads < 1 || c.head_dim < 8 || c.intermediate < 8 || c.vocab < 2) return bad("bad model dimensions");
   if (c.n_q_heads % c.n_kv_heads) return bad("n_q_heads must be a multiple of n_kv_heads");
   if ((c.hidden % 8) || (c.intermediate % 8) || (c.head_dim % 8) || c.hidden > 8192) return bad("hidden, intermediate, head_dim must be multiples of 8; hidden <= 8192");
@@ -775,6 +778,7 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
   if (const char* e = getenv("TANDEM_TAIL"))
     h->use_tail = atoi(e) != 0 && c.dtype == TANDEM_BF16 && h->gemm_impl == TANDEM_GEMM_TCGEN05 && h->attn_impl == TANDEM_ATTN_MMA;
   if (const char* e = getenv("TANDEM_GEMM_RING_KB")) h->gemm_ring_kb = std::max(0, std::min(200, atoi(e)));
+  if (const char* e = getenv("TANDEM_GEMM_PAIR")) h->gemm_pair = atoi(e) != 0 ? 1 : 0;
   {
     int dev_sms = 0;
     if (cudaDeviceGetAttribute(&dev_sms, cudaDevAttrMultiProcessorCount, c.device) == cudaSuccess && dev_sms > 0) h->n_sms = dev_sms;
@@ -1055,7 +1059,10 @@ int tandem_score(tandem_handle* h, int32_t n_seqs, const int32_t* tokens, const 
       next += n;
     }
     if (h->profile) { h->ev_used = 0; h->prof_pending.clear(); }
-    if ((rc = launch_step(h, io, rp, s, true, 1.f / temperature))) return rc;
+    h->scoring = true;
+    rc = launch_step(h, io, rp, s, true, 1.f / temperature);
+    h->scoring = false;
+    if (rc) return rc;
     CU(h, cudaGetLastError());
     if ((rc = refresh_slots(h, s))) return rc;   // synchronises the stream
     if (h->profile) {
@@ -1177,9 +1184,9 @@ int tandem_test_philox(const uint32_t ctr[4], const uint32_t key[2], uint32_t ou
 
 int tandem_test_gemm(int32_t dtype, int32_t impl, int32_t rows, int32_t N, int32_t K, const void* A_dev, const void* W_dev, float* out_dev) {
   if (rows < 0 || N <= 0 || K <= 0 || !A_dev || !W_dev || !out_dev) return TANDEM_EINVAL;
-  if (impl == TANDEM_GEMM_TCGEN05 || impl == 3) {
+  if (impl == TANDEM_GEMM_TCGEN05 || (impl >= 3 && impl <= 5)) {   // 3: SwiGLU epilogue; 4, 5: the same two as CTA pairs (cta_group::2)
     if (dtype != TANDEM_BF16) return TANDEM_EINVAL;
-    return tc_gemm_test(rows, N, K, A_dev, W_dev, out_dev, impl == 3 ? kTcEpiSwiGLU : kTcEpiPartial);
+    return tc_gemm_test(rows, N, K, A_dev, W_dev, out_dev, (impl == 3 || impl == 5) ? kTcEpiSwiGLU : kTcEpiPartial, impl >= 4);
   }
   dim3 grid((N + kSimtTile - 1) / kSimtTile, std::max(1, std::min((rows + kSimtTile - 1) / kSimtTile, 64)));
   if (dtype == TANDEM_F32) {
@@ -1195,7 +1202,7 @@ int tandem_test_gemm(int32_t dtype, int32_t impl, int32_t rows, int32_t N, int32
 int tandem_test_gemm_time(int32_t rows, int32_t N, int32_t K, int32_t iters, int32_t cluster, int32_t ring_kb, int32_t splits, int32_t flags,
                           float* ms_per_launch) {
   if (rows <= 0 || N <= 0 || K <= 0 || iters <= 0 || !ms_per_launch) return TANDEM_EINVAL;
-  (void)cluster; TcGemmTune t; t.ring_kb = ring_kb; t.splits = splits; t.pdl = (flags & 2) != 0;
+  TcGemmTune t; t.ring_kb = ring_kb; t.splits = splits; t.pdl = (flags & 2) != 0; t.pair = cluster == 2 ? 1 : 0;
   return tc_gemm_time(rows, N, K, iters, t, (flags & 1) ? kTcEpiSwiGLU : kTcEpiPartial, ms_per_launch);
 }
 

@@ -71,7 +71,8 @@ def test_simt_gemm_bf16(rows, N, K):
                                       (5, 200, 72), (1000, 640, 1024)])
 def test_tcgen05_gemm_bf16(rows, N, K):
     """tcgen05/TMEM/TMA GEMM (swap-AB, split-K) against a float64 matmul of the same bf16 values: the seven projection
-    shapes of the configs plus ragged rows (1, 33, 257, 1000), N not a multiple of the 128-row tile and K not a multiple of 64."""
+    shapes of the configs plus ragged rows (1, 33, 257, 1000), N not a multiple of the 128-row tile and K not a multiple of 64.
+    Also as CTA pairs (cta_group::2, impl 4): same accumulation order per output, so bit-identical to the single-CTA kernel."""
     g = torch.Generator().manual_seed(rows * 7919 + N + K)
     A = torch.randn(rows, K, generator=g).to(torch.bfloat16).cuda()
     W = (torch.randn(N, K, generator=g) * 0.05).to(torch.bfloat16).cuda()
@@ -81,6 +82,9 @@ def test_tcgen05_gemm_bf16(rows, N, K):
     err = torch.max(torch.abs(out.double() - ref)).item()
     assert np.isfinite(err)
     assert err <= 2e-6 * max(1.0, ref.abs().max().item()) * (K ** 0.5), (err, ref.abs().max().item())
+    pair = torch.full((rows, N), float("nan"), device="cuda")
+    T.tandem_test_gemm(T.BF16, 4, A, W, pair)
+    assert torch.equal(pair, out)
 
 
 @pytest.mark.parametrize("rows,I,K", [(1, 64, 64), (37, 192, 128), (140, 9728, 2560), (300, 512, 256), (64, 4864, 896)])
@@ -98,6 +102,9 @@ def test_tcgen05_gemm_swiglu_epilogue(rows, I, K):
     ref = gate / (1 + torch.exp(-gate)) * up
     err = torch.max(torch.abs(out.double() - ref)).item()
     assert err <= 2 ** -8 * max(1e-3, ref.abs().max().item()) + 1e-6, (err, ref.abs().max().item())   # one bf16 rounding of the result
+    pair = torch.zeros(rows, I, dtype=torch.bfloat16, device="cuda")
+    T.tandem_test_gemm(T.BF16, 5, A, W, pair)                                                          # the CTA-pair launch of the same kernel
+    assert torch.equal(pair, out)
 
 
 def _nucleus(z, temperature, top_p, u, top_k=0):
