@@ -8,7 +8,8 @@
 // weight streamer: every weight byte crosses HBM once (TMA, L2 evict-first), the activation tile is re-read from L2.
 //   grid = (N/128 weight tiles, S K-splits); each CTA accumulates its K-slice for all rows in TMEM and writes an
 //   fp32 partial out[s][r][n]; the consumer kernel sums the S partials in a fixed order (deterministic, no atomics).
-//   warp 0: TMA producer   warp 1: MMA issuer   warps 2-5: epilogue (tcgen05.ld -> coalesced global stores)
+//   warp 0: weight TMA   warp 6: activation TMA   warp 1: MMA issuer   warps 2-5, 7-10: epilogue (tcgen05.ld -> coalesced global
+//   stores; two warps per TMEM lane quarter: the epilogue is an exposed tail, every CTA owns a single tile)
 //   smem ring: stage = 16 KB of W (128 x 64 bf16, 128B swizzle) + nbox x 4 KB of A (32-row boxes), as many stages
 //   as fit in 200 KB (4 at 256 rows, 6 at 128 rows, 9 at 32 rows).
 #pragma once
@@ -28,7 +29,7 @@ constexpr int kTcMaxRows = 256;      // token rows per accumulator pass = max UM
 constexpr int kTcMaxStages = 10;
 constexpr int kTcRingBytes = 200 * 1024;
 constexpr int kTcSmemBytes = kTcRingBytes + 1024;   // + alignment slack
-constexpr int kTcThreads = 224;
+constexpr int kTcThreads = 352;        // warps: 0 weight TMA, 1 MMA, 2-5 and 7-10 epilogue (two per TMEM lane quarter), 6 activation TMA
 constexpr int kTcWBytes = kTcTileN * kTcBlockK * 2;     // 16384
 constexpr int kTcABoxBytes = kTcRowBox * kTcBlockK * 2; // 4096
 
@@ -186,7 +187,7 @@ enum { kTcEpiPartial = 0, kTcEpiSwiGLU = 1 };
 //        drains its own 128 TMEM lanes. The activation bytes an SM pulls out of L2 halve (profiles/gemm_sweep_r1.md: the
 //        projections are bound by SM ingest, not HBM, above ~64 token rows).
 template <int EPI, bool PAIR>
-__global__ void __launch_bounds__(kTcThreads, 1)
+__global__ void __launch_bounds__(kTcThreads, 2)   // two CTAs per SM whenever the ring allows: <= 93 registers per thread
 gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ Pair<TcGemmArgs> gp) {
   const TcGemmArgs& g = gp.m[blockIdx.z];                  // blockIdx.z = model
   const CUtensorMap* tmap_w = &maps.w[blockIdx.z];
@@ -225,7 +226,7 @@ gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__
     // full: weight + activation producers (a pair: the leader's two, which also post the peer's bytes); empty / accumulator-full: one commit
     for (int s = 0; s < n_stages; ++s) { ptx::mbar_init(full_bar(s), 2); ptx::mbar_init(empty_bar(s), 1); }
     ptx::mbar_init(tmem_full_bar, 1);
-    ptx::mbar_init(tmem_empty_bar, PAIR ? 8 : 4);          // the epilogue warps (of both CTAs; only the leader's is used)
+    ptx::mbar_init(tmem_empty_bar, PAIR ? 16 : 8);         // the epilogue warps (of both CTAs; only the leader's is used)
     ptx::fence_mbar_init();
     ptx::prefetch_tmap(tmap_w);
     ptx::prefetch_tmap(tmap_a);
@@ -322,8 +323,10 @@ gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__
       }
     }
   } else {
-    // ===== epilogue: warp w may touch TMEM lanes 32*(w%4)..+31; lane = weight row n, column = token row r
+    // ===== epilogue: warp w may touch TMEM lanes 32*(w%4)..+31; lane = weight row n, column = token row r. Each lane quarter
+    // has two warps (2-5 and 7-10) that take alternate groups of 32 columns.
     const int q = warp & 3;
+    const int half = warp >= 7 ? 1 : 0;
     const int n = n0 + q * 32 + lane;
     float* outp = g.out + (size_t)split * g.split_stride;
     const uint32_t te_bar = PAIR ? ptx::mapa_rank(tmem_empty_bar, 0) : tmem_empty_bar;
@@ -333,7 +336,7 @@ gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__
       const int crow = min(rows - r0, kTcMaxRows);
       ptx::mbar_wait(tmem_full_bar, (uint32_t)c & 1u);
       ptx::tc_fence_after();
-      for (int c0 = 0; c0 < crow; c0 += 32) {
+      for (int c0 = 32 * half; c0 < crow; c0 += 64) {
         uint32_t v[32];
         ptx::tmem_ld32(tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)c0, v);
         ptx::tmem_ld_wait();
