@@ -359,7 +359,7 @@ gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__
             const float recv = __shfl_xor_sync(0xffffffffu, send, 1);
             const float gate = odd ? recv : mine, up = odd ? mine : recv;
             const int r = c0 + (odd ? 16 : 0) + j;
-            if (r < crow && n < g.N) act[(size_t)(r0 + r) * I + i] = __float2bfloat16_rn(gate / (1.f + expf(-gate)) * up);
+            if (r < crow && n < g.N) act[(size_t)(r0 + r) * I + i] = __float2bfloat16_rn(__fdividef(gate, 1.f + __expf(-gate)) * up);   // bf16 result: fast exp / divide are exact enough
           }
         }
       }
