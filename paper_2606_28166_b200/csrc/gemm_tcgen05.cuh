@@ -374,10 +374,13 @@ gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__
 }
 
 // ---------------------------------------------------------------------------------------------- host side
-// K-splits: enough CTAs to put one on (almost) every SM, never more than one wave of 148, each slice >= 4 k-blocks.
-// A function of the shape only, so the reduction order (and every logit) is independent of the batch.
-inline int tc_gemm_splits(int N, int K) {
-  const int tiles = (N + kTcTileN - 1) / kTcTileN, kb = (K + kTcBlockK - 1) / kTcBlockK;
+// K-splits: as many as keep the whole launch (all tiles of all models in it) within one CTA per SM, each slice >= 4 k-blocks.
+// One CTA per SM with the deep 200 KB ring beats two per SM with an uneven second layer (measured on the 4B shape, both models
+// per launch: O and down 3 splits = 120 CTAs: 12.98 ms per step; 4 splits = 160 CTAs: 13.13; 7 splits = 280 CTAs: 13.15), and
+// the consumer kernel has fewer partials to sum. A function of the shape and of the number of models per launch only, so the
+// reduction order (and every logit) is independent of the batch.
+inline int tc_gemm_splits(int N, int K, int n_models = 1) {
+  const int tiles = n_models * ((N + kTcTileN - 1) / kTcTileN), kb = (K + kTcBlockK - 1) / kTcBlockK;
   int s = 1;
   while (tiles * (s + 1) <= 148 && (s + 1) * 4 <= kb && s < 16) ++s;
   return s;
@@ -448,7 +451,7 @@ inline int tc_gemm_launch(TcGemmPlans* p, int n_models, int which, const void* c
                           const int32_t* const* rows_ptr, int rows_cap, int* n_split, size_t* split_stride, cudaStream_t s, int epi = kTcEpiPartial,
                           const TcGemmTune* tune = nullptr) {
   if (!p || (K % 8) != 0) return -1;                       // TMA needs 16-byte row strides
-  int S = (which == 4 || epi == kTcEpiSwiGLU) ? 1 : tc_gemm_splits(N, K);
+  int S = (which == 4 || epi == kTcEpiSwiGLU) ? 1 : tc_gemm_splits(N, K, n_models);
   if (tune && tune->splits > 0) S = tune->splits;
   *n_split = S;
   *split_stride = (size_t)rows_cap * N;

@@ -161,7 +161,8 @@ int launch_gemm(tandem_handle* h, int which, const void* const* A, const void* c
   static const int cls_of[5] = {TANDEM_KC_GEMM_QKV, TANDEM_KC_GEMM_O, TANDEM_KC_GEMM_GATEUP, TANDEM_KC_GEMM_DOWN, TANDEM_KC_GEMM_LMHEAD};
   if (h->gemm_impl == TANDEM_GEMM_TCGEN05 && sizeof(T) == 2) {
     int rc = 0;
-    TcGemmTune tune; tune.ring_kb = h->gemm_ring_kb; tune.pdl = h->use_pdl; tune.pair = h->gemm_pair >= 0 ? h->gemm_pair : (h->scoring ? 1 : 0);
+    TcGemmTune tune; tune.ring_kb = h->gemm_ring_kb; tune.pdl = h->use_pdl;
+ tune.pair = h->gemm_pair >= 0 ? h->gemm_pair : (h->scoring ? 1 : 0);
     KL(h, cls_of[which], s, rc = tc_gemm_launch(h->tc, 2, which, A, W, N, K, out, rows_ptr, rows_cap, n_split, split_stride, s, epi, &tune));
     return rc == 0 ? TANDEM_OK : fail(h, rc, "tcgen05 GEMM launch failed (tensor map encode or K % 8 != 0)");
   }
@@ -287,7 +288,7 @@ int launch_layer_tail(tandem_handle* h, int li, cudaStream_t s) {
     }
   }
   a.H = H; a.I = I; a.nq = nq; a.nkv = nkv; a.d = d; a.eps = c.rms_eps; a.rope_cs = h->rope_cs;
-  a.S_o = tc_gemm_splits(H, nq * d); a.S_down = tc_gemm_splits(H, I); a.S_qkv = tc_gemm_splits(qkv_n, H); a.row_cap = h->row_cap;
+  a.S_o = tc_gemm_splits(H, nq * d, 2); a.S_down = tc_gemm_splits(H, I, 2); a.S_qkv = tc_gemm_splits(qkv_n, H, 2); a.row_cap = h->row_cap;
   a.bar = h->lt_bar + li * LT_NPHASE;
   a.dbg_ts = h->lt_ts ? h->lt_ts + (size_t)li * 32 : nullptr;
   a.wm_l = h->lt_wmaps + (l >= 0 ? l : 0); a.wm_ln = h->lt_wmaps + (ln < L ? ln : 0); a.am = h->lt_amaps;
