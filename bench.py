@@ -194,13 +194,11 @@ def class_bytes(shape, cls, rows, kv_bytes_per_layer_launch, emit_rows, n_models
 
 def run_full_rollout(args):
     """The whole workload through one tandem_generate call: prompts in, tokens / owner flags / senior log-probs out, sequences
-    admitted as KV pages allow (cfg 4 does not fit at once). Ownership of a few sequences is re-derived with the oracle's
-    integer rule from the returned tokens as a sanity check."""
+    admitted as KV pages allow (cfg 4 does not fit at once). Sanity checks here use no oracle code (the parity tests do that): every
+    sequence reaches its length and an owner change only ever follows a word-start token."""
     import torch
     import paper_2606_28166_b200 as T
     from workloads import get_workload, make_weights, make_word_start, make_prompts, make_max_new
-    from oracle import TandemParams as OParams, owners_from_tokens
-    from oracle.rule import Uniforms
     torch.cuda.set_device(0)
     T.build()
     wl = get_workload(args.workload)
@@ -231,9 +229,10 @@ def run_full_rollout(args):
     g = eng.generate(prm, prompts, max_new)
     dt = time.perf_counter() - t0
     assert (g["len"] == max_new).all()
-    for b in sorted(set([0, B // 3, B - 1])):
-        o = owners_from_tokens(g["tokens"][b, :g["len"][b]], table, OParams(p=wl.p, switch_mode=wl.switch_mode, seed=seed), Uniforms(seed=seed), b=b)
-        assert np.array_equal(o, g["owner"][b, :g["len"][b]]), "owner flags differ from the rule replayed on the returned tokens"
+    for b in range(B):                                   # TOGGLE / REDRAW without cap: the author changes only after a word-start token
+        n = int(g["len"][b])
+        flips = g["owner"][b, 1:n] != g["owner"][b, :n - 1]
+        assert not flips[table[g["tokens"][b, :n - 1]] == 0].any(), "an owner change follows a token that starts no word"
     st = g["stats"]
     tok = int(g["len"].sum())
     pk = peaks()
@@ -306,7 +305,7 @@ def run_grpo(args):
 def run_score(args):
     """tandem_score on N streams of the workload's shape (host buffers in and out): both models read every stream through the
     ragged prefill path, every position reaches the LM head, and the score kernel reduces the two logit rows to (log p_sen(y),
-    log p_jun(y), alpha). A few positions are checked against oracle.dual_score when the shape is small enough to afford it."""
+    log p_jun(y), alpha). Parity with oracle.dual_score is the job of tests/test_gpu_score.py; here only ranges are checked."""
     import torch
     import paper_2606_28166_b200 as T
     from workloads import get_workload, make_weights
