@@ -24,7 +24,11 @@ forms for RoPE/RMSNorm/softmax/SwiGLU, library-routine cross-check of the forwar
 (torch float64 sdpa/rms_norm/silu), incremental-KV == full recompute, p=0 == solo,
 p=1 closed form, brute-force coin enumeration against a table-driven transcription
 of section 3.3, role-swap symmetry, same-weights schedule independence, Gumbel-max
-frequencies vs softmax (chi-square), top-p hand example, senior share / run-length laws.
+frequencies vs softmax (chi-square), top-p hand example, senior share / run-length laws; top-k hand
+examples, top-k 1 = greedy, frequencies under the renormalised distribution (sampler.kept_set, R18); overlap alpha on
+hand-worked distributions and as 1 - total variation, junior cross-entropy against torch's cross_entropy, role swap,
+agreement with the rollout's recorded senior log-probs (score.dual_score, R17); binary-reward advantages in closed
+form, a hand-worked clipped surrogate, a torch re-composition, on-policy special cases (grpo.grpo_objective, R19).
 Parity that stays unpinned: any comparison with the paper's own rollouts, rewards or
 accuracy numbers (its weights, tokenizer and datasets are not available).
 """
