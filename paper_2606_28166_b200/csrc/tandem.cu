@@ -90,6 +90,12 @@ struct tandem_handle {
   uint8_t* word_start_dev = nullptr; std::vector<uint8_t> word_start_host;
   DevStats* stats = nullptr; int32_t* n_active = nullptr; int32_t* work_ctr = nullptr;
   cudaStream_t gs{}; cudaEvent_t ev_in{}, ev_out{};   // internal stream of the captured step graph and its fork / join events
+  // staggered two-stream mode (forward_pair): the junior's chain runs on gs2, half a layer behind the senior's
+  bool use_stagger = false;
+  cudaStream_t gs2{}; cudaEvent_t ev_fork{}, ev_join{};
+  std::vector<cudaEvent_t> stagger_ev;          // [2 * layer + model]: that model's attention launch of that layer has been issued and is complete
+  int stagger_attn_ctas_per_sm = 1, stagger_ring_kb = 98; bool stagger_events = true, stagger_deep = true;
+  int32_t* zero_counts = nullptr;               // C_NUM zeros: the absent second model of a one-model attention launch
   std::vector<uint8_t> slot_busy;           // host view of the slots
   // admission staging
   int32_t* stage_tokens = nullptr; size_t stage_cap = 0; long long* stage_off = nullptr; int32_t* stage_i32 = nullptr;
@@ -155,7 +161,7 @@ cudaEvent_t prof_event(tandem_handle* h) {
 // read from rows_ptr[m] on the device.
 template <typename T>
 int launch_gemm(tandem_handle* h, int which, const void* const* A, const void* const* W, int N, int K, float* const* out,
-                const int32_t* const* rows_ptr, int rows_cap, int* n_split, size_t* split_stride, cudaStream_t s, int epi = kTcEpiPartial) {
+                const int32_t* const* rows_ptr, int rows_cap, int* n_split, size_t* split_stride, cudaStream_t s, int epi = kTcEpiPartial, int nm = 2) {
   *n_split = 1;
   *split_stride = (size_t)rows_cap * N;
   static const int cls_of[5] = {TANDEM_KC_GEMM_QKV, TANDEM_KC_GEMM_O, TANDEM_KC_GEMM_GATEUP, TANDEM_KC_GEMM_DOWN, TANDEM_KC_GEMM_LMHEAD};
@@ -163,20 +169,25 @@ int launch_gemm(tandem_handle* h, int which, const void* const* A, const void* c
     int rc = 0;
     TcGemmTune tune; tune.ring_kb = h->gemm_ring_kb; tune.pdl = h->use_pdl;
  tune.pair = h->gemm_pair >= 0 ? h->gemm_pair : (h->scoring ? 1 : 0);
-    KL(h, cls_of[which], s, rc = tc_gemm_launch(h->tc, 2, which, A, W, N, K, out, rows_ptr, rows_cap, n_split, split_stride, s, epi, &tune));
+    if (nm == 1) {   // staggered mode: the K-splits of the paired launch (same reduction order, bit-identical results) and a ring that leaves
+                     // room for the other model's attention CTA on the same SM
+      if (which != 4 && epi != kTcEpiSwiGLU) tune.splits = tc_gemm_splits(N, K, 2);
+      if (tune.ring_kb == 0) tune.ring_kb = h->stagger_ring_kb;
+    }
+    KL(h, cls_of[which], s, rc = tc_gemm_launch(h->tc, nm, which, A, W, N, K, out, rows_ptr, rows_cap, n_split, split_stride, s, epi, &tune));
     return rc == 0 ? TANDEM_OK : fail(h, rc, "tcgen05 GEMM launch failed (tensor map encode or K % 8 != 0)");
   }
-  dim3 grid((N + kSimtTile - 1) / kSimtTile, std::min((rows_cap + kSimtTile - 1) / kSimtTile, 16), 2);
+  dim3 grid((N + kSimtTile - 1) / kSimtTile, std::min((rows_cap + kSimtTile - 1) / kSimtTile, 16), nm);
   Pair<SimtGemmArgs<T>> g;
-  for (int m = 0; m < 2; ++m) g.m[m] = SimtGemmArgs<T>{rows_ptr[m], 0, (const T*)A[m], (const T*)W[m], out[m], N, K};
+  for (int m = 0; m < 2; ++m) { const int mm = m < nm ? m : 0; g.m[m] = SimtGemmArgs<T>{rows_ptr[mm], 0, (const T*)A[mm], (const T*)W[mm], out[mm], N, K}; }
   KL(h, cls_of[which], s, launch_ex(gemm_simt_kernel<T>, grid, dim3(256), 0, s, h->use_pdl, g));
   return TANDEM_OK;
 }
 
 template <typename T>
-void launch_residual_norm(tandem_handle* h, cudaStream_t s, int grid_x, const Pair<ResNormArgs<T>>& a) {
+void launch_residual_norm(tandem_handle* h, cudaStream_t s, int grid_x, const Pair<ResNormArgs<T>>& a, int nm = 2) {
   const int v = (a.m[0].H / 4 + 255) / 256;   // float4 per thread; tandem_init guarantees H % 8 == 0 and H <= 8192
-  const dim3 grid(grid_x, 2);
+  const dim3 grid(grid_x, nm);
   if (v <= 1) KL(h, TANDEM_KC_RESIDUAL_NORM, s, launch_ex(residual_norm_kernel<T, 256, 1>, grid, dim3(256), 0, s, h->use_pdl, a));
   else if (v <= 2) KL(h, TANDEM_KC_RESIDUAL_NORM, s, launch_ex(residual_norm_kernel<T, 256, 2>, grid, dim3(256), 0, s, h->use_pdl, a));
   else if (v <= 4) KL(h, TANDEM_KC_RESIDUAL_NORM, s, launch_ex(residual_norm_kernel<T, 256, 4>, grid, dim3(256), 0, s, h->use_pdl, a));
@@ -184,21 +195,21 @@ void launch_residual_norm(tandem_handle* h, cudaStream_t s, int grid_x, const Pa
 }
 
 template <typename T, int D, int G>
-void launch_attn_dg(const Pair<AttnArgs<T>>& a, int grid, cudaStream_t s, bool pdl) {
-  launch_ex(paged_attention_kernel<T, D, G>, dim3(grid, 2), dim3(kAttnThreads), 0, s, pdl, a);
+void launch_attn_dg(const Pair<AttnArgs<T>>& a, int grid, cudaStream_t s, bool pdl, int nm) {
+  launch_ex(paged_attention_kernel<T, D, G>, dim3(grid, nm), dim3(kAttnThreads), 0, s, pdl, a);
 }
 template <typename T> struct AttnDispatch;
 template <> struct AttnDispatch<float> {
-  static bool run(const Pair<AttnArgs<float>>& a, int D, int G, int grid, cudaStream_t s, bool pdl) {
-#define TD_CASE(d, g) if (D == d && G == g) { launch_attn_dg<float, d, g>(a, grid, s, pdl); return true; }
+  static bool run(const Pair<AttnArgs<float>>& a, int D, int G, int grid, cudaStream_t s, bool pdl, int nm = 2) {
+#define TD_CASE(d, g) if (D == d && G == g) { launch_attn_dg<float, d, g>(a, grid, s, pdl, nm); return true; }
     TD_CASE(32, 1) TD_CASE(32, 2) TD_CASE(32, 4) TD_CASE(64, 1) TD_CASE(64, 2) TD_CASE(64, 4) TD_CASE(128, 1) TD_CASE(128, 2) TD_CASE(128, 4)
 #undef TD_CASE
     return false;
   }
 };
 template <> struct AttnDispatch<bf16> {
-  static bool run(const Pair<AttnArgs<bf16>>& a, int D, int G, int grid, cudaStream_t s, bool pdl) {
-#define TD_CASE(d, g) if (D == d && G == g) { launch_attn_dg<bf16, d, g>(a, grid, s, pdl); return true; }
+  static bool run(const Pair<AttnArgs<bf16>>& a, int D, int G, int grid, cudaStream_t s, bool pdl, int nm = 2) {
+#define TD_CASE(d, g) if (D == d && G == g) { launch_attn_dg<bf16, d, g>(a, grid, s, pdl, nm); return true; }
     TD_CASE(64, 1) TD_CASE(64, 2) TD_CASE(64, 4) TD_CASE(64, 7) TD_CASE(64, 8) TD_CASE(128, 1) TD_CASE(128, 2) TD_CASE(128, 4) TD_CASE(128, 8)
 #undef TD_CASE
     return false;
@@ -206,15 +217,20 @@ template <> struct AttnDispatch<bf16> {
 };
 template <int D, int G> struct AmStages { static constexpr int value = D == 128 ? 2 : 4; };
 template <int D, int G>
-bool launch_attn_mma_dg(const Pair<CUtensorMap>& map, const Pair<AttnMmaArgs>& a, int grid, cudaStream_t s, bool set_attr, bool pdl) {
+bool launch_attn_mma_dg(const Pair<CUtensorMap>& map, const Pair<AttnMmaArgs>& a, int grid, cudaStream_t s, bool set_attr, bool pdl, bool deep) {
   constexpr int ST = AmStages<D, G>::value;
   constexpr int smem = attn_mma_smem_bytes<D, ST>();
-  if (set_attr) return cudaFuncSetAttribute(paged_attention_mma_kernel<D, G, ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) == cudaSuccess;
+  // deep = the staggered mode's one-CTA-per-SM launch: a ring of 1.5x the stages (the second CTA slot of the SM belongs to a GEMM CTA)
+  constexpr int STD = ST + ST / 2;
+  constexpr int smem_deep = attn_mma_smem_bytes<D, STD>();
+  if (set_attr) return cudaFuncSetAttribute(paged_attention_mma_kernel<D, G, ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) == cudaSuccess &&
+                       cudaFuncSetAttribute(paged_attention_mma_kernel<D, G, STD>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_deep) == cudaSuccess;
+  if (deep) return launch_ex(paged_attention_mma_kernel<D, G, STD>, dim3(grid), dim3(kAmThreads), smem_deep, s, pdl, map, a) == cudaSuccess;
   return launch_ex(paged_attention_mma_kernel<D, G, ST>, dim3(grid), dim3(kAmThreads), smem, s, pdl, map, a) == cudaSuccess;
 }
 // set_attr = true: only raise the kernel's dynamic shared memory limit (called once from tandem_init)
-bool run_attn_mma(const Pair<CUtensorMap>& map, const Pair<AttnMmaArgs>& a, int D, int G, int grid, cudaStream_t s, bool set_attr, bool pdl = false) {
-#define TD_CASE(d, g) if (D == d && G == g) return launch_attn_mma_dg<d, g>(map, a, grid, s, set_attr, pdl);
+bool run_attn_mma(const Pair<CUtensorMap>& map, const Pair<AttnMmaArgs>& a, int D, int G, int grid, cudaStream_t s, bool set_attr, bool pdl = false, bool deep = false) {
+#define TD_CASE(d, g) if (D == d && G == g) return launch_attn_mma_dg<d, g>(map, a, grid, s, set_attr, pdl, deep);
   TD_CASE(64, 1) TD_CASE(64, 2) TD_CASE(64, 4) TD_CASE(64, 7) TD_CASE(64, 8) TD_CASE(128, 1) TD_CASE(128, 2) TD_CASE(128, 4) TD_CASE(128, 8)
 #undef TD_CASE
   return false;
@@ -303,7 +319,7 @@ int launch_layer_tail(tandem_handle* h, int li, cudaStream_t s) {
 // Every kernel is launched once for the two models (Pair arguments): the models advance layer by layer in lock-step on
 // one stream, each launch carrying the senior's and the junior's half of the work.
 template <typename T>
-int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaStream_t s, bool score = false, float score_inv_t = 1.f) {
+int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaStream_t s, bool score = false, float score_inv_t = 1.f, cudaStream_t s2 = nullptr) {
   const tandem_config& c = h->cfg;
   const int H = c.hidden, nq = c.n_q_heads, nkv = c.n_kv_heads, d = c.head_dim, I = c.intermediate, V = c.vocab;
   const int qkv_n = (nq + 2 * nkv) * d;
@@ -321,6 +337,155 @@ int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaS
     for (int m = 0; m < 2; ++m) ea.m[m] = EmbedArgs<T>{h->tab[m].counts, h->tab[m].row_tok, (const T*)h->w[m].embed, (const T*)h->w[m].attn_norm[0], h->ws[m].x, (T*)h->ws[m].act, H, c.rms_eps};
     KL(h, TANDEM_KC_EMBED, s, launch_ex(embed_norm_kernel<T, 256>, dim3(row_grid, 2), dim3(256), 0, s, false, ea));
   }
+
+  // The chain of a layer in three parts and the head, each launched for the models m0 .. m0 + nm - 1 on stream st:
+  // nm = 2 is one launch for both models (Pair arguments, the model is a grid dimension), nm = 1 a launch for one model
+  // (the staggered two-stream mode of launch_step). Entry i >= nm of a Pair is never indexed by a grid of nm models;
+  // the attention kernel's shared unit space sees a zero item count for it.
+  auto mi = [](int i, int m0, int nm) { return i < nm ? m0 + i : m0; };
+  auto pre_attn = [&](int l, int m0, int nm, cudaStream_t st) -> int {
+    int ns; size_t ss; int rc;
+    // S3 QKV projection
+    for (int i = 0; i < 2; ++i) { const int m = mi(i, m0, nm); set_gemm(i, h->ws[m].act, h->w[m].wqkv[l], h->ws[m].gemm_out, h->tab[m].counts + C_ROWS); }
+    if ((rc = launch_gemm<T>(h, 0, A, W, qkv_n, H, O, RP, h->row_cap, &ns, &ss, st, kTcEpiPartial, nm))) return rc;
+    // S4 RoPE + KV append
+    if (mma) {
+      Pair<RopeArgs<T, bf16>> ra;
+      for (int i = 0; i < 2; ++i) {
+        const int m = mi(i, m0, nm);
+        T* kpool = (T*)h->ws[m].kv + (size_t)l * layer_kv;
+        ra.m[i] = RopeArgs<T, bf16>{h->tab[m].counts, h->tab[m].row_pos, h->tab[m].row_kvslot, h->ws[m].gemm_out, ns, ss, h->rope_cs, (bf16*)h->ws[m].q, kpool, kpool + half_kv, nq, nkv, d};
+      }
+      KL(h, TANDEM_KC_ROPE_APPEND, st, launch_ex(rope_append_kernel<T, bf16, 256>, dim3(row_grid * 4, nm), dim3(256), 0, st, pdl, ra));
+    } else {
+      Pair<RopeArgs<T, float>> ra;
+      for (int i = 0; i < 2; ++i) {
+        const int m = mi(i, m0, nm);
+        T* kpool = (T*)h->ws[m].kv + (size_t)l * layer_kv;
+        ra.m[i] = RopeArgs<T, float>{h->tab[m].counts, h->tab[m].row_pos, h->tab[m].row_kvslot, h->ws[m].gemm_out, ns, ss, h->rope_cs, (float*)h->ws[m].q, kpool, kpool + half_kv, nq, nkv, d};
+      }
+      KL(h, TANDEM_KC_ROPE_APPEND, st, launch_ex(rope_append_kernel<T, float, 256>, dim3(row_grid * 4, nm), dim3(256), 0, st, pdl, ra));
+    }
+    return TANDEM_OK;
+  };
+  // S5 attention (decode splits + catch-up rows); apdl = false when the launch also waits on another stream's event
+  auto attention = [&](int l, int m0, int nm, cudaStream_t st, bool apdl) -> int {
+    bool ok = true;
+    if (mma) {
+      const long long rows_per_half = (long long)h->pool_pages * nkv * kPageTokens;
+      Pair<AttnMmaArgs> ma; Pair<CUtensorMap> maps;
+      for (int i = 0; i < 2; ++i) {
+        const int m = mi(i, m0, nm);
+        const StepTab& tb = h->tab[m];
+        // one work counter per (layer, launch): the staggered mode's second model takes the counters past the first L
+        ma.m[i] = AttnMmaArgs{i < nm ? tb.counts : h->zero_counts, tb.item_row0, tb.item_ntok, tb.item_kv0, tb.item_kv1, tb.item_part, tb.row_slot, tb.row_pos, h->pt[m].bt, h->max_pages,
+                              (const bf16*)h->ws[m].q, (bf16*)h->ws[m].attn_out, h->ws[m].part_acc, h->ws[m].part_ml, nq, nkv, 1.0f / sqrtf((float)d),
+                              (int)((2ll * l) * rows_per_half), (int)((2ll * l + 1) * rows_per_half), h->work_ctr + l + (nm == 1 && m0 == 1 ? c.n_layers : 0)};
+        maps.m[i] = h->kv_map_store[m];
+      }
+      const int ctas = (nm == 1 ? h->stagger_attn_ctas_per_sm : h->attn_ctas_per_sm) * h->n_sms;
+      KL(h, TANDEM_KC_ATTENTION, st, ok = run_attn_mma(maps, ma, d, nq / nkv, ctas, st, false, apdl, nm == 1 && h->stagger_attn_ctas_per_sm == 1 && h->stagger_deep));
+    } else {
+      Pair<AttnArgs<T>> aa;
+      for (int i = 0; i < 2; ++i) {
+        const int m = mi(i, m0, nm);
+        const StepTab& tb = h->tab[m];
+        T* kpool = (T*)h->ws[m].kv + (size_t)l * layer_kv;
+        aa.m[i] = AttnArgs<T>{tb.counts, tb.item_row0, tb.item_ntok, tb.item_kv0, tb.item_kv1, tb.item_part, tb.row_slot, tb.row_pos, h->pt[m].bt, h->max_pages,
+                              (const float*)h->ws[m].q, kpool, kpool + half_kv, (T*)h->ws[m].attn_out, h->ws[m].part_acc, h->ws[m].part_ml, nq, nkv, 1.0f / sqrtf((float)d)};
+      }
+      KL(h, TANDEM_KC_ATTENTION, st, ok = AttnDispatch<T>::run(aa, d, nq / nkv, 148 * 2, st, apdl, nm));
+    }
+    if (!ok) return fail(h, TANDEM_EINVAL, "unsupported (head_dim, group) for attention");
+    return TANDEM_OK;
+  };
+  auto post_attn = [&](int l, int m0, int nm, cudaStream_t st) -> int {
+    int ns; size_t ss; int rc;
+    {
+      Pair<CombineArgs<T>> ca;
+      for (int i = 0; i < 2; ++i) {
+        const int m = mi(i, m0, nm);
+        const StepTab& tb = h->tab[m];
+        ca.m[i] = CombineArgs<T>{tb.counts, tb.comb_row, tb.comb_part0, tb.comb_n, tb.comb_stride, h->ws[m].part_acc, h->ws[m].part_ml, (T*)h->ws[m].attn_out, nq, d};
+      }
+      KL(h, TANDEM_KC_ATTN_COMBINE, st, launch_ex(attn_combine_kernel<T>, dim3(148 * 4, nm), dim3(256), 0, st, pdl, ca));
+    }
+    // S6 O projection + residual + RMSNorm(mlp)
+    for (int i = 0; i < 2; ++i) { const int m = mi(i, m0, nm); set_gemm(i, h->ws[m].attn_out, h->w[m].wo[l], h->ws[m].gemm_out, h->tab[m].counts + C_ROWS); }
+    if ((rc = launch_gemm<T>(h, 1, A, W, H, nq * d, O, RP, h->row_cap, &ns, &ss, st, kTcEpiPartial, nm))) return rc;
+    {
+      Pair<ResNormArgs<T>> na;
+      for (int i = 0; i < 2; ++i) {
+        const int m = mi(i, m0, nm);
+        na.m[i] = ResNormArgs<T>{h->tab[m].counts, h->ws[m].gemm_out, ns, ss, h->ws[m].x, (const T*)h->w[m].mlp_norm[l], (T*)h->ws[m].act, nullptr, H, c.rms_eps};
+      }
+      launch_residual_norm<T>(h, st, row_grid, na, nm);
+    }
+    // S7 gate/up + SwiGLU, down + residual + RMSNorm(next layer | final)
+    if (h->gemm_impl == TANDEM_GEMM_TCGEN05) {   // SwiGLU in the GEMM epilogue (gate/up rows interleaved at load time)
+      for (int i = 0; i < 2; ++i) { const int m = mi(i, m0, nm); set_gemm(i, h->ws[m].act, h->w[m].wgu[l], (float*)h->ws[m].mlp_act, h->tab[m].counts + C_ROWS); }
+      if ((rc = launch_gemm<T>(h, 2, A, W, 2 * I, H, O, RP, h->row_cap, &ns, &ss, st, kTcEpiSwiGLU, nm))) return rc;
+    } else {
+      for (int i = 0; i < 2; ++i) { const int m = mi(i, m0, nm); set_gemm(i, h->ws[m].act, h->w[m].wgu[l], h->ws[m].gemm_out, h->tab[m].counts + C_ROWS); }
+      if ((rc = launch_gemm<T>(h, 2, A, W, 2 * I, H, O, RP, h->row_cap, &ns, &ss, st, kTcEpiPartial, nm))) return rc;
+      Pair<SwigluArgs<T>> sg;
+      for (int i = 0; i < 2; ++i) { const int m = mi(i, m0, nm); sg.m[i] = SwigluArgs<T>{h->tab[m].counts, h->ws[m].gemm_out, ns, ss, (T*)h->ws[m].mlp_act, I}; }
+      KL(h, TANDEM_KC_SWIGLU, st, launch_ex(swiglu_kernel<T, 256>, dim3(row_grid, nm), dim3(256), 0, st, pdl, sg));
+    }
+    for (int i = 0; i < 2; ++i) { const int m = mi(i, m0, nm); set_gemm(i, h->ws[m].mlp_act, h->w[m].wdown[l], h->ws[m].gemm_out, h->tab[m].counts + C_ROWS); }
+    if ((rc = launch_gemm<T>(h, 3, A, W, H, I, O, RP, h->row_cap, &ns, &ss, st, kTcEpiPartial, nm))) return rc;
+    const bool last = l == c.n_layers - 1;
+    {
+      Pair<ResNormArgs<T>> na;
+      for (int i = 0; i < 2; ++i) {
+        const int m = mi(i, m0, nm);
+        na.m[i] = ResNormArgs<T>{h->tab[m].counts, h->ws[m].gemm_out, ns, ss, h->ws[m].x, (const T*)(last ? h->w[m].final_norm : h->w[m].attn_norm[l + 1]),
+                                 (T*)(last ? (score ? h->ws[m].score_lm_in : h->ws[m].lm_in) : h->ws[m].act), last ? h->tab[m].row_emit : nullptr, H, c.rms_eps};
+      }
+      launch_residual_norm<T>(h, st, row_grid, na, nm);
+    }
+    return TANDEM_OK;
+  };
+  // S8 LM head on the emitting rows only, then sample + switch + emit
+  auto head = [&](int m0, int nm, cudaStream_t st) -> int {
+    int ns; size_t ss; int rc;
+    for (int i = 0; i < 2; ++i) { const int m = mi(i, m0, nm); set_gemm(i, h->ws[m].lm_in, h->w[m].lm_head, h->ws[m].logits, h->tab[m].counts + C_EMIT); }
+    if ((rc = launch_gemm<T>(h, 4, A, W, V, H, O, RP, c.max_seqs, &ns, &ss, st, kTcEpiPartial, nm))) return rc;
+    Pair<SampleArgs> sa;
+    const int n_chunk = std::max(1, std::min(kSampleMaxChunks, V / 8192));   // ~8k ids per CTA: 18 slices at V = 151,936
+    for (int i = 0; i < 2; ++i) {
+      const int m = mi(i, m0, nm);
+      sa.m[i] = SampleArgs{h->st, h->tab[m], io, rp, h->ws[m].logits, h->word_start_dev, h->tokens, h->out_owner, h->out_logp, V, c.max_seq_len, m,
+                           h->ws[m].chunk_part, h->ws[m].chunk_ctr, n_chunk};
+    }
+    const size_t nucleus_smem = (rp.temperature > 0.f && (rp.top_p < 1.f || (rp.top_k > 0 && rp.top_k < V))) ? sizeof(NucleusSmem<256>) : 0;
+    if (nucleus_smem) KL(h, TANDEM_KC_SAMPLE, st, launch_ex(sample_switch_emit_kernel<256, true>, dim3(c.max_seqs, n_chunk, nm), dim3(256), nucleus_smem, st, pdl, sa));
+    else KL(h, TANDEM_KC_SAMPLE, st, launch_ex(sample_switch_emit_kernel<256, false>, dim3(c.max_seqs, n_chunk, nm), dim3(256), 0, st, pdl, sa));
+    return TANDEM_OK;
+  };
+
+  if (s2) {
+    // Staggered mode: one chain per model on its own stream, offset by half a layer. A model's attention (pure KV streaming,
+    // one CTA per SM) runs while the other model's projections (weight streaming with exposed prologues and epilogues) occupy
+    // the second CTA slot of every SM; events order the attention launches senior(l), junior(l), senior(l+1), ... so the two
+    // chains cannot drift into phase. The caller forked s2 from s after the scheduler and joins it before finalize.
+    cudaStream_t sm[2] = {s, s2};
+    const bool ev = s2 != s;   // profile mode passes s2 == s: same launches, serialised on one stream
+    if (ev) { CU(h, cudaEventRecord(h->ev_fork, s)); CU(h, cudaStreamWaitEvent(s2, h->ev_fork, 0)); }
+    for (int l = 0; l < c.n_layers; ++l)
+      for (int m = 0; m < 2; ++m) {
+        if ((rc = pre_attn(l, m, 1, sm[m]))) return rc;
+        const bool wait = ev && h->stagger_events && (m == 1 || l > 0);
+        if (wait) CU(h, cudaStreamWaitEvent(sm[m], h->stagger_ev[m == 1 ? 2 * l : 2 * (l - 1) + 1], 0));
+        if ((rc = attention(l, m, 1, sm[m], pdl && !wait))) return rc;
+        if (ev && h->stagger_events) CU(h, cudaEventRecord(h->stagger_ev[2 * l + m], sm[m]));
+        if ((rc = post_attn(l, m, 1, sm[m]))) return rc;
+      }
+    for (int m = 0; m < 2; ++m) if ((rc = head(m, 1, sm[m]))) return rc;
+    if (ev) { CU(h, cudaEventRecord(h->ev_join, s2)); CU(h, cudaStreamWaitEvent(s, h->ev_join, 0)); }
+    return TANDEM_OK;
+  }
+
   const bool tail = h->use_tail && sizeof(T) == 2 && !score;
   if (tail && (rc = launch_layer_tail(h, 0, s))) return rc;
   for (int l = 0; l < c.n_layers; ++l) {
@@ -342,88 +507,8 @@ int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaS
       if ((rc = launch_layer_tail(h, l + 1, s))) return rc;
       continue;
     }
-    // S3 QKV projection
-    for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].act, h->w[m].wqkv[l], h->ws[m].gemm_out, h->tab[m].counts + C_ROWS);
-    if ((rc = launch_gemm<T>(h, 0, A, W, qkv_n, H, O, RP, h->row_cap, &ns, &ss, s))) return rc;
-    // S4 RoPE + KV append
-    if (mma) {
-      Pair<RopeArgs<T, bf16>> ra;
-      for (int m = 0; m < 2; ++m) {
-        T* kpool = (T*)h->ws[m].kv + (size_t)l * layer_kv;
-        ra.m[m] = RopeArgs<T, bf16>{h->tab[m].counts, h->tab[m].row_pos, h->tab[m].row_kvslot, h->ws[m].gemm_out, ns, ss, h->rope_cs, (bf16*)h->ws[m].q, kpool, kpool + half_kv, nq, nkv, d};
-      }
-      KL(h, TANDEM_KC_ROPE_APPEND, s, launch_ex(rope_append_kernel<T, bf16, 256>, dim3(row_grid * 4, 2), dim3(256), 0, s, pdl, ra));
-    } else {
-      Pair<RopeArgs<T, float>> ra;
-      for (int m = 0; m < 2; ++m) {
-        T* kpool = (T*)h->ws[m].kv + (size_t)l * layer_kv;
-        ra.m[m] = RopeArgs<T, float>{h->tab[m].counts, h->tab[m].row_pos, h->tab[m].row_kvslot, h->ws[m].gemm_out, ns, ss, h->rope_cs, (float*)h->ws[m].q, kpool, kpool + half_kv, nq, nkv, d};
-      }
-      KL(h, TANDEM_KC_ROPE_APPEND, s, launch_ex(rope_append_kernel<T, float, 256>, dim3(row_grid * 4, 2), dim3(256), 0, s, pdl, ra));
-    }
-    // S5 attention (decode splits + catch-up rows), then combine
-    bool ok = true;
-    if (mma) {
-      const long long rows_per_half = (long long)h->pool_pages * nkv * kPageTokens;
-      Pair<AttnMmaArgs> ma; Pair<CUtensorMap> maps;
-      for (int m = 0; m < 2; ++m) {
-        const StepTab& tb = h->tab[m];
-        ma.m[m] = AttnMmaArgs{tb.counts, tb.item_row0, tb.item_ntok, tb.item_kv0, tb.item_kv1, tb.item_part, tb.row_slot, tb.row_pos, h->pt[m].bt, h->max_pages,
-                              (const bf16*)h->ws[m].q, (bf16*)h->ws[m].attn_out, h->ws[m].part_acc, h->ws[m].part_ml, nq, nkv, 1.0f / sqrtf((float)d),
-                              (int)((2ll * l) * rows_per_half), (int)((2ll * l + 1) * rows_per_half), h->work_ctr + l};
-        maps.m[m] = h->kv_map_store[m];
-      }
-      KL(h, TANDEM_KC_ATTENTION, s, ok = run_attn_mma(maps, ma, d, nq / nkv, h->attn_ctas_per_sm * h->n_sms, s, false, pdl));
-    } else {
-      Pair<AttnArgs<T>> aa;
-      for (int m = 0; m < 2; ++m) {
-        const StepTab& tb = h->tab[m];
-        T* kpool = (T*)h->ws[m].kv + (size_t)l * layer_kv;
-        aa.m[m] = AttnArgs<T>{tb.counts, tb.item_row0, tb.item_ntok, tb.item_kv0, tb.item_kv1, tb.item_part, tb.row_slot, tb.row_pos, h->pt[m].bt, h->max_pages,
-                              (const float*)h->ws[m].q, kpool, kpool + half_kv, (T*)h->ws[m].attn_out, h->ws[m].part_acc, h->ws[m].part_ml, nq, nkv, 1.0f / sqrtf((float)d)};
-      }
-      KL(h, TANDEM_KC_ATTENTION, s, ok = AttnDispatch<T>::run(aa, d, nq / nkv, 148 * 2, s, pdl));
-    }
-    if (!ok) return fail(h, TANDEM_EINVAL, "unsupported (head_dim, group) for attention");
-    {
-      Pair<CombineArgs<T>> ca;
-      for (int m = 0; m < 2; ++m) {
-        const StepTab& tb = h->tab[m];
-        ca.m[m] = CombineArgs<T>{tb.counts, tb.comb_row, tb.comb_part0, tb.comb_n, tb.comb_stride, h->ws[m].part_acc, h->ws[m].part_ml, (T*)h->ws[m].attn_out, nq, d};
-      }
-      KL(h, TANDEM_KC_ATTN_COMBINE, s, launch_ex(attn_combine_kernel<T>, dim3(148 * 4, 2), dim3(256), 0, s, pdl, ca));
-    }
-    // S6 O projection + residual + RMSNorm(mlp)
-    for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].attn_out, h->w[m].wo[l], h->ws[m].gemm_out, h->tab[m].counts + C_ROWS);
-    if ((rc = launch_gemm<T>(h, 1, A, W, H, nq * d, O, RP, h->row_cap, &ns, &ss, s))) return rc;
-    {
-      Pair<ResNormArgs<T>> na;
-      for (int m = 0; m < 2; ++m) na.m[m] = ResNormArgs<T>{h->tab[m].counts, h->ws[m].gemm_out, ns, ss, h->ws[m].x, (const T*)h->w[m].mlp_norm[l], (T*)h->ws[m].act, nullptr, H, c.rms_eps};
-      launch_residual_norm<T>(h, s, row_grid, na);
-    }
-    // S7 gate/up + SwiGLU, down + residual + RMSNorm(next layer | final)
-    if (h->gemm_impl == TANDEM_GEMM_TCGEN05) {   // SwiGLU in the GEMM epilogue (gate/up rows interleaved at load time)
-      for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].act, h->w[m].wgu[l], (float*)h->ws[m].mlp_act, h->tab[m].counts + C_ROWS);
-      if ((rc = launch_gemm<T>(h, 2, A, W, 2 * I, H, O, RP, h->row_cap, &ns, &ss, s, kTcEpiSwiGLU))) return rc;
-    } else {
-      for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].act, h->w[m].wgu[l], h->ws[m].gemm_out, h->tab[m].counts + C_ROWS);
-      if ((rc = launch_gemm<T>(h, 2, A, W, 2 * I, H, O, RP, h->row_cap, &ns, &ss, s))) return rc;
-      Pair<SwigluArgs<T>> sg;
-      for (int m = 0; m < 2; ++m) sg.m[m] = SwigluArgs<T>{h->tab[m].counts, h->ws[m].gemm_out, ns, ss, (T*)h->ws[m].mlp_act, I};
-      KL(h, TANDEM_KC_SWIGLU, s, launch_ex(swiglu_kernel<T, 256>, dim3(row_grid, 2), dim3(256), 0, s, pdl, sg));
-    }
-    for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].mlp_act, h->w[m].wdown[l], h->ws[m].gemm_out, h->tab[m].counts + C_ROWS);
-    if ((rc = launch_gemm<T>(h, 3, A, W, H, I, O, RP, h->row_cap, &ns, &ss, s))) return rc;
-    const bool last = l == c.n_layers - 1;
-    {
-      Pair<ResNormArgs<T>> na;
-      for (int m = 0; m < 2; ++m)
-        na.m[m] = ResNormArgs<T>{h->tab[m].counts, h->ws[m].gemm_out, ns, ss, h->ws[m].x, (const T*)(last ? h->w[m].final_norm : h->w[m].attn_norm[l + 1]),
-                                 (T*)(last ? (score ? h->ws[m].score_lm_in : h->ws[m].lm_in) : h->ws[m].act), last ? h->tab[m].row_emit : nullptr, H, c.rms_eps};
-      launch_residual_norm<T>(h, s, row_grid, na);
-    }
+    if ((rc = pre_attn(l, 0, 2, s)) || (rc = attention(l, 0, 2, s, pdl)) || (rc = post_attn(l, 0, 2, s))) return rc;
   }
-  // S8 LM head on the emitting rows only, then sample + switch + emit
   if (score) {   // every row reaches the LM head (the scheduler set row_emit[r] = r); the dual-scoring kernel replaces the sampler
     for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].score_lm_in, h->w[m].lm_head, h->ws[m].score_logits, h->tab[m].counts + C_EMIT);
     if ((rc = launch_gemm<T>(h, 4, A, W, V, H, O, RP, h->row_cap, &ns, &ss, s))) return rc;
@@ -432,17 +517,7 @@ int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaS
     KL(h, TANDEM_KC_SCORE, s, launch_ex(score_kernel<512>, dim3(h->row_cap), dim3(512), 0, s, pdl, sc));
     return TANDEM_OK;
   }
-  for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].lm_in, h->w[m].lm_head, h->ws[m].logits, h->tab[m].counts + C_EMIT);
-  if ((rc = launch_gemm<T>(h, 4, A, W, V, H, O, RP, c.max_seqs, &ns, &ss, s))) return rc;
-  Pair<SampleArgs> sa;
-  const int n_chunk = std::max(1, std::min(kSampleMaxChunks, V / 8192));   // ~8k ids per CTA: 18 slices at V = 151,936
-  for (int m = 0; m < 2; ++m)
-    sa.m[m] = SampleArgs{h->st, h->tab[m], io, rp, h->ws[m].logits, h->word_start_dev, h->tokens, h->out_owner, h->out_logp, V, c.max_seq_len, m,
-                         h->ws[m].chunk_part, h->ws[m].chunk_ctr, n_chunk};
-  const size_t nucleus_smem = (rp.temperature > 0.f && (rp.top_p < 1.f || (rp.top_k > 0 && rp.top_k < V))) ? sizeof(NucleusSmem<256>) : 0;
-  if (nucleus_smem) KL(h, TANDEM_KC_SAMPLE, s, launch_ex(sample_switch_emit_kernel<256, true>, dim3(c.max_seqs, n_chunk, 2), dim3(256), nucleus_smem, s, pdl, sa));
-  else KL(h, TANDEM_KC_SAMPLE, s, launch_ex(sample_switch_emit_kernel<256, false>, dim3(c.max_seqs, n_chunk, 2), dim3(256), 0, s, pdl, sa));
-  return TANDEM_OK;
+  return head(0, 2, s);
 }
 
 int launch_step(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaStream_t s, bool score = false, float score_inv_t = 1.f) {
@@ -454,7 +529,9 @@ int launch_step(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaSt
   sa.work_ctr = h->work_ctr; sa.n_work_ctr = c.n_layers + (c.n_layers + 1) * LT_NPHASE;
   sa.score = score ? 1 : 0;
   KL(h, TANDEM_KC_SCHED, s, (sched_kernel<<<1, 1024, 0, s>>>(sa)));
-  const int rc = (c.dtype == TANDEM_F32) ? forward_pair<float>(h, io, rp, s, score, score_inv_t) : forward_pair<bf16>(h, io, rp, s, score, score_inv_t);
+  // staggered mode: the junior's chain on the second internal stream (profile mode: same launches, serialised on s)
+  cudaStream_t s2 = (h->use_stagger && !score) ? (h->profile ? s : h->gs2) : nullptr;
+  const int rc = (c.dtype == TANDEM_F32) ? forward_pair<float>(h, io, rp, s, score, score_inv_t, s2) : forward_pair<bf16>(h, io, rp, s, score, score_inv_t, s2);
   if (rc) return rc;
   FinalArgs fa{h->st, {h->pt[0], h->pt[1]}, io, h->stats, h->n_active, c.max_seqs, h->max_pages, h->pool_pages};
   KL(h, TANDEM_KC_FINALIZE, s, (finalize_kernel<<<1, 1024, 0, s>>>(fa)));
@@ -771,6 +848,17 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
   INIT_CU(cudaEventCreateWithFlags(&h->ev_in, cudaEventDisableTiming));
   INIT_CU(cudaEventCreateWithFlags(&h->ev_out, cudaEventDisableTiming));
   INIT_CU(cudaStreamCreateWithFlags(&h->gs, cudaStreamNonBlocking));
+  INIT_CU(cudaStreamCreateWithFlags(&h->gs2, cudaStreamNonBlocking));
+  INIT_CU(cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));
+  INIT_CU(cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming));
+  for (int i = 0; i < 2 * c.n_layers; ++i) { cudaEvent_t e; INIT_CU(cudaEventCreateWithFlags(&e, cudaEventDisableTiming)); h->stagger_ev.push_back(e); }
+  INIT_TRY(dmalloc(h, &h->zero_counts, (size_t)C_NUM * 4));
+  INIT_CU(cudaMemset(h->zero_counts, 0, (size_t)C_NUM * 4));
+  if (const char* e = getenv("TANDEM_STAGGER")) h->use_stagger = atoi(e) != 0;
+  if (const char* e = getenv("TANDEM_STAGGER_ATTN_CTAS")) h->stagger_attn_ctas_per_sm = std::max(1, std::min(2, atoi(e)));
+  if (const char* e = getenv("TANDEM_STAGGER_EVENTS")) h->stagger_events = atoi(e) != 0;
+  if (const char* e = getenv("TANDEM_STAGGER_DEEP")) h->stagger_deep = atoi(e) != 0;
+  if (const char* e = getenv("TANDEM_STAGGER_RING_KB")) h->stagger_ring_kb = std::max(32, std::min(200, atoi(e)));
   if (const char* e = getenv("TANDEM_ATTN_CTAS_PER_SM")) h->attn_ctas_per_sm = std::max(1, std::min(2, atoi(e)));
   if (const char* e = getenv("TANDEM_PDL")) h->use_pdl = atoi(e) != 0;
   // The persistent layer-tail kernel (layer_tail.cuh) is correct and tested but, at 157 us per layer against ~150 us for the
@@ -1134,6 +1222,11 @@ void tandem_free(tandem_handle* h) {
   if (h->ev_in) cudaEventDestroy(h->ev_in);
   if (h->ev_out) cudaEventDestroy(h->ev_out);
   if (h->gs) cudaStreamDestroy(h->gs);
+  if (h->gs2) cudaStreamDestroy(h->gs2);
+  if (h->ev_fork) cudaEventDestroy(h->ev_fork);
+  if (h->ev_join) cudaEventDestroy(h->ev_join);
+  for (cudaEvent_t e : h->stagger_ev) cudaEventDestroy(e);
+  fr(h->zero_counts);
   fr(h->score_out[0]); fr(h->score_out[1]); fr(h->st_mem); fr(h->st_mem8); fr(h->tokens); fr(h->out_owner); fr(h->out_logp); fr(h->rope_cs); fr(h->word_start_dev); fr(h->stats);
   fr(h->lt_wmaps); fr(h->lt_amaps); fr(h->lt_ts); fr(h->n_active); fr(h->work_ctr); fr(h->stage_tokens); fr(h->stage_off); fr(h->stage_i32);
   cudaGetLastError();
