@@ -67,6 +67,8 @@ def parse_args():
                     help="instead of timed steps: run the WHOLE workload through tandem_generate (host buffers, admission queue) with "
                          "every max_new multiplied by SCALE (1.0 = the workload as specified) and report tokens/s of the call")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-share-prompt-pages", action="store_true",
+                    help="every rollout computes and stores its own copy of the prompt's KV (default: the G rollouts of a prompt share its full pages)")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-new", type=int, default=8, help="new tokens of the oracle's bounded sample")
     return ap.parse_args()
@@ -219,7 +221,8 @@ def run_full_rollout(args):
     kv_per_model = int(min((free - wbytes - 4.5e9) / 2, need + (64 << 20)))            # workspaces and the CUDA context stay free
     max_seqs = min(B, 256)
     eng = T.Tandem(T.TandemConfig(shape, max_seqs=max_seqs, max_seq_len=(max(len(p) for p in prompts) + int(max_new.max()) + 31) // 16 * 16,
-                                  kv_bytes_per_model=kv_per_model, max_rows_per_step=4096, use_graph=1))
+                                  kv_bytes_per_model=kv_per_model, max_rows_per_step=4096, use_graph=1,
+                                  share_prompt_pages=0 if args.no_share_prompt_pages else 1))
     for m in range(2):
         eng.load_weights(m, w_host[m])
     del w_host
@@ -244,6 +247,7 @@ def run_full_rollout(args):
                                  "sequences": B, "max_new_scale": args.full_rollout, "mean_new": float(max_new.mean()), "tokens": tok, "seconds": dt,
                                  "max_seqs": max_seqs, "peak_resident": int(st["peak_resident"]), "kv_gb_per_model": kv_per_model / 1e9,
                                  "peak_pages": [int(st["peak_pages_senior"]), int(st["peak_pages_junior"])],
+                                 "share_prompt_pages": not args.no_share_prompt_pages, "shared_prompt_rows": int(st["shared_prompt_rows"]),
                                  "senior_share": float(g["mask"].sum() / max(1, tok))},
                       "gpu_launches": int(st["kernel_launches"]),
                       "step_roofline": {"bound": "hbm", "achieved": gbs, "unit": "GB/s", "frac_of_measured": gbs / pk["hbm_gbs"], "frac_of_8TBs": gbs / NOMINAL_HBM_GBS},
@@ -386,7 +390,8 @@ def run_ours(args):
     prefill_steps = (prefill_rows + row_cap - 1) // row_cap + 2
     gen_budget = prefill_steps + max(args.ramp, int(8.0 / max(wl.p * wl.word_start_frac, 1e-3))) + args.max_drain + W + K + args.profile_steps + 64
     max_seq_len = ((max_prompt + max(gen_budget, args.e2e_new) + 15) // 16) * 16
-    eng = T.Tandem(T.TandemConfig(shape, max_seqs=B, max_seq_len=max_seq_len, device=local, max_rows_per_step=row_cap, use_graph=1))
+    eng = T.Tandem(T.TandemConfig(shape, max_seqs=B, max_seq_len=max_seq_len, device=local, max_rows_per_step=row_cap, use_graph=1,
+                                  share_prompt_pages=0 if args.no_share_prompt_pages else 1))
     w_cpu = []
     for m, seed in enumerate((wl.seeds["senior"], wl.seeds["junior"])):
         w = make_weights(shape, seed, device="cuda")
@@ -526,7 +531,9 @@ def run_ours(args):
         d2h = B * new * (4 + 1 + 4) + B * 4
         res["e2e"] = {"value": tok / dt, "unit": "tokens/s", "h2d_bytes_per_step": h2d / steps_e, "d2h_bytes_per_step": d2h / steps_e,
                       "call": "tandem_generate(B=%d host prompts of the workload, max_new=%d): prompt prefill + %d engine steps, host buffers in and out"
-                              % (B, new, steps_e), "seconds": dt, "device_seconds": g["stats"]["seconds_total"]}
+                              % (B, new, steps_e), "seconds": dt, "device_seconds": g["stats"]["seconds_total"],
+                      "share_prompt_pages": not args.no_share_prompt_pages, "prompt_rows": e_rows, "shared_prompt_rows": g["stats"]["shared_prompt_rows"],
+                      "rows_computed": g["stats"]["rows_senior"] + g["stats"]["rows_junior"]}
     eng.free()
     torch.cuda.empty_cache()
 

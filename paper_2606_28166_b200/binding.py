@@ -31,7 +31,7 @@ class _Config(C.Structure):
     _fields_ = [(n, C.c_int32) for n in ("n_layers", "hidden", "n_q_heads", "n_kv_heads", "head_dim", "intermediate", "vocab")] + \
                [("rms_eps", C.c_float), ("rope_theta", C.c_float), ("dtype", C.c_int32), ("page_tokens", C.c_int32),
                 ("max_seqs", C.c_int32), ("max_seq_len", C.c_int32), ("kv_bytes_per_model", C.c_int64), ("device", C.c_int32),
-                ("max_rows_per_step", C.c_int32), ("gemm_impl", C.c_int32), ("use_graph", C.c_int32), ("attn_impl", C.c_int32), ("reserved", C.c_int32 * 3)]
+                ("max_rows_per_step", C.c_int32), ("gemm_impl", C.c_int32), ("use_graph", C.c_int32), ("attn_impl", C.c_int32), ("share_prompt_pages", C.c_int32), ("reserved", C.c_int32 * 2)]
 
 
 _PP = C.POINTER(C.c_void_p)
@@ -67,7 +67,7 @@ class _StepOut(C.Structure):
 class _Stats(C.Structure):
     _fields_ = [(n, C.c_int64) for n in ("steps", "tokens_emitted", "rows_senior", "rows_junior", "catchup_rows", "kv_bytes_read", "weight_bytes_read")] + \
                [("peak_pages_senior", C.c_int32), ("peak_pages_junior", C.c_int32), ("peak_resident", C.c_int32), ("seconds_total", C.c_double),
-                ("kernel_launches", C.c_int64)]
+                ("kernel_launches", C.c_int64), ("shared_prompt_rows", C.c_int64)]
 
 
 _lib = None
@@ -112,11 +112,12 @@ class TandemConfig:
     """Mirror of tandem_config. `shape` is any object with the model dimensions (e.g. workloads.ModelShape)."""
 
     def __init__(self, shape, max_seqs, max_seq_len, kv_bytes_per_model=0, device=0, max_rows_per_step=0,
-                 gemm_impl=GEMM_AUTO, use_graph=0, page_tokens=16, attn_impl=ATTN_AUTO):
+                 gemm_impl=GEMM_AUTO, use_graph=0, page_tokens=16, attn_impl=ATTN_AUTO, share_prompt_pages=0):
         self.shape = shape
         self.c = _Config(shape.n_layers, shape.hidden, shape.n_q_heads, shape.n_kv_heads, shape.head_dim, shape.intermediate,
                          shape.vocab, shape.rms_eps, shape.rope_theta, F32 if shape.dtype == "f32" else BF16, page_tokens,
-                         max_seqs, max_seq_len, kv_bytes_per_model, device, max_rows_per_step, gemm_impl, use_graph, attn_impl)
+                         max_seqs, max_seq_len, kv_bytes_per_model, device, max_rows_per_step, gemm_impl, use_graph, attn_impl,
+                         share_prompt_pages)
 
 
 class TandemParams:

@@ -80,6 +80,7 @@ struct StepTab {
 struct SeqState {       // all [max_seqs]
   int32_t* seq_id; int32_t* prompt_len; int32_t* n_ctx; int32_t* ing[2]; int32_t* cap_c;
   int32_t* max_new; int32_t* n_emit; uint8_t* active; uint8_t* owner; uint8_t* done;
+  int32_t* grp;         // prompt-sharing group of the sequence (index into GroupTab), -1 = none
 };
 
 struct PageTab {        // per model
@@ -87,10 +88,23 @@ struct PageTab {        // per model
   int32_t* npages;      // [max_seqs]
   int32_t* free_pages;  // [pool_pages] stack of free page ids (page 0 is a dummy page, never handed out)
   int32_t* free_top;    // scalar: number of free pages on the stack
+  int32_t* nshared;     // [max_seqs] leading entries of the sequence's block table that belong to its group (GroupTab), not to it
+};
+
+// Prompt-page sharing ("pages": the G rollouts of a GRPO group have identical prompts): the full pages of the
+// common prompt are computed once per model - by the first member that runs that model, the donor - and referenced read-only from
+// every member's block table. The group owns those pages; the last member to finish returns them. All [max_seqs] except pages.
+struct GroupTab {
+  int32_t* state[2];    // per model: 0 = nobody has started the shared prefix, 1 = the donor is ingesting it, 2 = pages[] valid
+  int32_t* donor[2];    // slot of the donor while state == 1
+  int32_t* pages[2];    // [max_seqs, max_pages] the group's page ids, npg[g] of them
+  int32_t* npg;         // shared pages = floor((prompt_len - 1) / 16): every member keeps at least one prompt row of its own
+  int32_t* ref;         // members that have not finished
 };
 
 struct DevStats {       // device-side accumulators (unsigned long long for atomicAdd)
   unsigned long long steps, tokens_emitted, rows[2], catchup_rows, kv_tokens_read, model_steps;
+  unsigned long long shared_rows;   // prompt positions taken over from a group's shared pages instead of being recomputed
   int peak_pages_used[2]; int peak_resident; int err_oom;
 };
 

@@ -12,7 +12,7 @@ namespace tandem {
 // written for the kernels downstream. PAPER.md L257 (per-step attention metadata: slot mappings, block tables,
 // position indices) - here per model, since the two models are no longer in lock-step.
 struct SchedArgs {
-  SeqState st; PageTab pt[2]; StepTab tab[2]; StepIO io; DevStats* stats;
+  SeqState st; PageTab pt[2]; GroupTab gt; StepTab tab[2]; StepIO io; DevStats* stats;
   const int32_t* tokens; int max_seqs, max_seq_len, max_pages, row_cap, tile_tok;
   int32_t* work_ctr; int n_work_ctr;   // dynamic-scheduling counters of the attention launches of this step
   int score;                           // teacher-forced dual scoring (tandem_score): both models ingest every sequence, every row reaches the LM head
@@ -71,8 +71,31 @@ __global__ void __launch_bounds__(1024) sched_kernel(SchedArgs a) {
     const StepTab& tb = a.tab[M];
     const PageTab& pt = a.pt[M];
     const bool mine = a.score ? live : owner == M;
-    const int ing = mine ? a.st.ing[M][s] : 0;
-    const int want = mine ? nfeed - ing : 0;
+    int ing = mine ? a.st.ing[M][s] : 0;
+    // Prompt-page sharing: a member of a group that has not started with this model links the group's prompt pages if they are
+    // ready, becomes the donor if nobody has started them, and otherwise waits (no rows this step) for the donor to finish.
+    // g_state is read here, before the scans below; the donor publishes after them, so a step sees the state of its start.
+    const int g = (mine && !a.score) ? a.st.grp[s] : -1;
+    bool donor = false, waits = false;
+    if (g >= 0 && ing == 0) {
+      const int gs = a.gt.state[M][g];
+      donor = gs == 1 && a.gt.donor[M][g] == s;
+      if (gs == 2) {
+        const int npg = a.gt.npg[g];
+        for (int i = 0; i < npg; ++i) pt.bt[(size_t)s * a.max_pages + i] = a.gt.pages[M][(size_t)g * a.max_pages + i];
+        pt.npages[s] = npg; pt.nshared[s] = npg;
+        ing = npg * kPageTokens;
+        a.st.ing[M][s] = ing;
+        atomicAdd(&a.stats->shared_rows, (unsigned long long)ing);
+      } else if (gs == 0) {
+        if (atomicCAS(&a.gt.state[M][g], 0, 1) == 0) { a.gt.donor[M][g] = s; donor = true; } else waits = true;
+      } else if (!donor) {
+        waits = true;
+      }
+    } else if (g >= 0 && a.gt.state[M][g] == 1 && a.gt.donor[M][g] == s) {
+      donor = true;   // a donor whose prefill is chunked over several steps
+    }
+    const int want = (mine && !waits) ? nfeed - ing : 0;
     int total_want;
     const int pre = block_excl_scan_1024(want, &total_want, wsum);
     const int rows = min(want, max(0, a.row_cap - pre));
@@ -140,6 +163,12 @@ __global__ void __launch_bounds__(1024) sched_kernel(SchedArgs a) {
       }
     }
     if (rows > 0) a.st.ing[M][s] = ing + rows;  // commit: the forward below always runs
+    if (donor && ing + rows >= a.gt.npg[g] * kPageTokens) {   // the shared prefix is stored after this step: hand its pages to the group
+      const int npg = a.gt.npg[g];
+      for (int i = 0; i < npg; ++i) a.gt.pages[M][(size_t)g * a.max_pages + i] = pt.bt[(size_t)s * a.max_pages + i];
+      pt.nshared[s] = npg;
+      a.gt.state[M][g] = 2;
+    }
     __syncthreads();
 
     for (int r = threadIdx.x; r < n_rows; r += blockDim.x) {
@@ -198,8 +227,9 @@ __global__ void __launch_bounds__(1024) sched_kernel(SchedArgs a) {
 
 // ============================================================================================ admission
 struct AdmitArgs {
-  SeqState st; PageTab pt[2]; int32_t* tokens; int max_seq_len;
+  SeqState st; PageTab pt[2]; GroupTab gt; int32_t* tokens; int max_seq_len;
   const int32_t* stage_tokens; const long long* stage_off; const int32_t* slots; const int32_t* seq_ids; const int32_t* max_new;
+  const int32_t* grp; const int32_t* grp_members;   // per admitted sequence: its group (-1 = none); members of the group if it is the group's first, else 0
   int n; int start_owner; float p; unsigned long long seed; const float* u_switch; long long u_switch_stride;
 };
 __global__ void admit_kernel(AdmitArgs a) {
@@ -219,29 +249,49 @@ __global__ void admit_kernel(AdmitArgs a) {
     a.st.ing[0][s] = 0; a.st.ing[1][s] = 0; a.st.cap_c[s] = 0; a.st.max_new[s] = a.max_new[i]; a.st.n_emit[s] = 0;
     a.st.owner[s] = (uint8_t)owner; a.st.done[s] = 0; a.st.active[s] = 1;
     a.pt[0].npages[s] = 0; a.pt[1].npages[s] = 0;
+    a.pt[0].nshared[s] = 0; a.pt[1].nshared[s] = 0;
+    const int g = a.grp ? a.grp[i] : -1;
+    a.st.grp[s] = g;
+    if (g >= 0 && a.grp_members[i] > 0) {   // first member: reset the group's entry
+      a.gt.state[0][g] = 0; a.gt.state[1][g] = 0; a.gt.donor[0][g] = -1; a.gt.donor[1][g] = -1;
+      a.gt.npg[g] = ((int)(o1 - o0) - 1) / kPageTokens;
+      a.gt.ref[g] = a.grp_members[i];
+    }
   }
 }
 
 // ============================================================================================ finalize
 // After both models' samplers: release the pages of sequences that finished this step and count the rest.
-struct FinalArgs { SeqState st; PageTab pt[2]; StepIO io; DevStats* stats; int32_t* n_active; int max_seqs, max_pages, pool_pages; };
+struct FinalArgs { SeqState st; PageTab pt[2]; GroupTab gt; StepIO io; DevStats* stats; int32_t* n_active; int max_seqs, max_pages, pool_pages; };
 __global__ void __launch_bounds__(1024) finalize_kernel(FinalArgs a) {
   __shared__ int wsum[32];
   const int s = threadIdx.x;
   bool live = false;
   if (s < a.max_seqs && a.st.active[s]) {
     if (a.st.done[s]) {
-      for (int M = 0; M < 2; ++M) {
-        const int n = a.pt[M].npages[s];
+      for (int M = 0; M < 2; ++M) {   // the sequence's own pages; the leading nshared entries belong to its group
+        const int n0 = a.pt[M].nshared[s], n = a.pt[M].npages[s] - n0;
         if (n > 0) {
           const int pos = atomicAdd(a.pt[M].free_top, n);
           for (int i = 0; i < n; ++i) {
-            const int pg = a.pt[M].bt[(size_t)s * a.max_pages + i];
+            const int pg = a.pt[M].bt[(size_t)s * a.max_pages + n0 + i];
             if (pos + i < a.pool_pages) a.pt[M].free_pages[pos + i] = pg;
           }
-          a.pt[M].npages[s] = 0;
+        }
+        a.pt[M].npages[s] = 0; a.pt[M].nshared[s] = 0;
+      }
+      const int g = a.st.grp[s];
+      if (g >= 0 && atomicSub(&a.gt.ref[g], 1) == 1) {   // last member of its group: return the shared prompt pages
+        for (int M = 0; M < 2; ++M) {
+          if (a.gt.state[M][g] != 2) continue;
+          const int n = a.gt.npg[g];
+          const int pos = atomicAdd(a.pt[M].free_top, n);
+          for (int i = 0; i < n; ++i)
+            if (pos + i < a.pool_pages) a.pt[M].free_pages[pos + i] = a.gt.pages[M][(size_t)g * a.max_pages + i];
+          a.gt.state[M][g] = 0;
         }
       }
+      a.st.grp[s] = -1;
       a.st.active[s] = 0;
     } else {
       live = true;

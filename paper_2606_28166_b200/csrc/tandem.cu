@@ -97,6 +97,11 @@ struct tandem_handle {
   int stagger_attn_ctas_per_sm = 1, stagger_ring_kb = 98; bool stagger_events = true, stagger_deep = true;
   int32_t* zero_counts = nullptr;               // C_NUM zeros: the absent second model of a one-model attention launch
   std::vector<uint8_t> slot_busy;           // host view of the slots
+  // prompt-page sharing (cfg.share_prompt_pages): device group table and the host's view of which entries are in use
+  GroupTab gt{};
+  int32_t* gt_mem = nullptr; int32_t* gt_pages_mem = nullptr;
+  std::vector<int> grp_free, grp_live, slot_grp;   // free group indices, members not yet seen finished per group, group of each slot
+  std::vector<int> grp_reserved; int grp_released = 0;   // tandem_generate's page reservation held by each group / given back by finished groups
   // admission staging
   int32_t* stage_tokens = nullptr; size_t stage_cap = 0; long long* stage_off = nullptr; int32_t* stage_i32 = nullptr;
   // graph of one step
@@ -523,7 +528,7 @@ int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaS
 int launch_step(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaStream_t s, bool score = false, float score_inv_t = 1.f) {
   const tandem_config& c = h->cfg;
   SchedArgs sa{};
-  sa.st = h->st; sa.pt[0] = h->pt[0]; sa.pt[1] = h->pt[1]; sa.tab[0] = h->tab[0]; sa.tab[1] = h->tab[1];
+  sa.st = h->st; sa.pt[0] = h->pt[0]; sa.pt[1] = h->pt[1]; sa.gt = h->gt; sa.tab[0] = h->tab[0]; sa.tab[1] = h->tab[1];
   sa.io = io; sa.stats = h->stats; sa.tokens = h->tokens; sa.max_seqs = c.max_seqs; sa.max_seq_len = c.max_seq_len;
   sa.max_pages = h->max_pages; sa.row_cap = h->row_cap; sa.tile_tok = h->tile_tok;
   sa.work_ctr = h->work_ctr; sa.n_work_ctr = c.n_layers + (c.n_layers + 1) * LT_NPHASE;
@@ -533,7 +538,7 @@ int launch_step(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaSt
   cudaStream_t s2 = (h->use_stagger && !score) ? (h->profile ? s : h->gs2) : nullptr;
   const int rc = (c.dtype == TANDEM_F32) ? forward_pair<float>(h, io, rp, s, score, score_inv_t, s2) : forward_pair<bf16>(h, io, rp, s, score, score_inv_t, s2);
   if (rc) return rc;
-  FinalArgs fa{h->st, {h->pt[0], h->pt[1]}, io, h->stats, h->n_active, c.max_seqs, h->max_pages, h->pool_pages};
+  FinalArgs fa{h->st, {h->pt[0], h->pt[1]}, h->gt, io, h->stats, h->n_active, c.max_seqs, h->max_pages, h->pool_pages};
   KL(h, TANDEM_KC_FINALIZE, s, (finalize_kernel<<<1, 1024, 0, s>>>(fa)));
   return TANDEM_OK;
 }
@@ -628,7 +633,14 @@ int refresh_slots(tandem_handle* h, cudaStream_t s) {
   std::vector<uint8_t> act(h->cfg.max_seqs);
   CU(h, cudaStreamSynchronize(s));
   CU(h, cudaMemcpy(act.data(), h->st.active, act.size(), cudaMemcpyDeviceToHost));
-  for (int i = 0; i < h->cfg.max_seqs; ++i) h->slot_busy[i] = act[i];
+  for (int i = 0; i < h->cfg.max_seqs; ++i) {
+    if (h->slot_busy[i] && !act[i] && h->slot_grp[i] >= 0) {   // a member finished: the group's index is reusable after its last one
+      const int g = h->slot_grp[i];
+      if (--h->grp_live[g] == 0) { h->grp_free.push_back(g); h->grp_released += h->grp_reserved[g]; h->grp_reserved[g] = 0; }
+      h->slot_grp[i] = -1;
+    }
+    h->slot_busy[i] = act[i];
+  }
   return TANDEM_OK;
 }
 
@@ -655,16 +667,33 @@ int admit(tandem_handle* h, const tandem_params* p, const tandem_overrides* ovr,
     h->stage_cap = (size_t)total;
   }
   std::vector<long long> o(n + 1);
-  std::vector<int32_t> meta(3 * (size_t)n);
+  std::vector<int32_t> meta(5 * (size_t)n);
   for (int i = 0; i <= n; ++i) o[i] = offs[i] - offs[0];
-  for (int i = 0; i < n; ++i) { meta[i] = slots[i]; meta[n + i] = seq_ids ? seq_ids[i] : slots[i]; meta[2 * n + i] = max_new[i]; }
+  for (int i = 0; i < n; ++i) { meta[i] = slots[i]; meta[n + i] = seq_ids ? seq_ids[i] : slots[i]; meta[2 * n + i] = max_new[i]; meta[3 * n + i] = -1; meta[4 * n + i] = 0; }
+  if (c.share_prompt_pages && !score) {
+    // Groups = runs of consecutive sequences of this call with identical prompts of more than one page (the G rollouts of a
+    // prompt): they share the full pages of the prompt except the one holding its last token.
+    for (int i = 0; i < n;) {
+      const int64_t len = offs[i + 1] - offs[i];
+      int j = i + 1;
+      while (j < n && offs[j + 1] - offs[j] == len && std::memcmp(toks + offs[i], toks + offs[j], (size_t)len * 4) == 0) ++j;
+      if (j - i >= 2 && (len - 1) / kPageTokens >= 1 && !h->grp_free.empty()) {
+        const int g = h->grp_free.back(); h->grp_free.pop_back();
+        h->grp_live[g] = j - i;
+        for (int k = i; k < j; ++k) { meta[3 * n + k] = g; h->slot_grp[slots[k]] = g; }
+        meta[4 * n + i] = j - i;
+      }
+      i = j;
+    }
+  }
   CU(h, cudaStreamSynchronize(s));
   CU(h, cudaMemcpy(h->stage_tokens, toks + offs[0], (size_t)total * 4, cudaMemcpyHostToDevice));
   CU(h, cudaMemcpy(h->stage_off, o.data(), (n + 1) * sizeof(long long), cudaMemcpyHostToDevice));
   CU(h, cudaMemcpy(h->stage_i32, meta.data(), meta.size() * 4, cudaMemcpyHostToDevice));
   AdmitArgs a{};
-  a.st = h->st; a.pt[0] = h->pt[0]; a.pt[1] = h->pt[1]; a.tokens = h->tokens; a.max_seq_len = c.max_seq_len;
+  a.st = h->st; a.pt[0] = h->pt[0]; a.pt[1] = h->pt[1]; a.gt = h->gt; a.tokens = h->tokens; a.max_seq_len = c.max_seq_len;
   a.stage_tokens = h->stage_tokens; a.stage_off = h->stage_off; a.slots = h->stage_i32; a.seq_ids = h->stage_i32 + n; a.max_new = h->stage_i32 + 2 * n;
+  a.grp = h->stage_i32 + 3 * n; a.grp_members = h->stage_i32 + 4 * n;
   a.n = n; a.start_owner = p->start_owner; a.p = p->p; a.seed = p->seed;
   a.u_switch = ovr ? ovr->u_switch : nullptr; a.u_switch_stride = ovr ? ovr->u_switch_stride : 0;
   admit_kernel<<<n, 128, 0, s>>>(a);
@@ -688,6 +717,7 @@ int fill_stats(tandem_handle* h, tandem_stats* stats) {
   stats->peak_pages_senior = d.peak_pages_used[0]; stats->peak_pages_junior = d.peak_pages_used[1]; stats->peak_resident = d.peak_resident;
   stats->seconds_total = 0.0;
   stats->kernel_launches = h->launches;
+  stats->shared_prompt_rows = (int64_t)d.shared_rows;
   return TANDEM_OK;
 }
 
@@ -727,7 +757,8 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
   if (c.max_seqs < 1 || c.max_seqs > kMaxSlots) return bad("max_seqs must be in 1..1024");
   if (c.max_seq_len < 2) return bad("bad max_seq_len");
   if (!attn_supported(c.dtype, c.head_dim, c.n_q_heads / c.n_kv_heads)) return bad("unsupported (head_dim, n_q/n_kv) combination");
-  for (int i = 0; i < 3; ++i) if (c.reserved[i]) return bad("reserved fields must be 0");
+  for (int i = 0; i < 2; ++i) if (c.reserved[i]) return bad("reserved fields must be 0");
+  if (c.share_prompt_pages != 0 && c.share_prompt_pages != 1) return bad("share_prompt_pages must be 0 or 1");
   if (c.attn_impl < 0 || c.attn_impl > 2) return bad("bad attn_impl");
   h->attn_impl = c.attn_impl == TANDEM_ATTN_AUTO ? (c.dtype == TANDEM_BF16 ? TANDEM_ATTN_MMA : TANDEM_ATTN_ALU) : c.attn_impl;
   if (h->attn_impl == TANDEM_ATTN_MMA && c.dtype != TANDEM_BF16) return bad("tensor-core attention needs bf16");
@@ -760,7 +791,7 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
   {
     int32_t* p = h->st_mem;
     h->st.seq_id = p; p += S; h->st.prompt_len = p; p += S; h->st.n_ctx = p; p += S; h->st.ing[0] = p; p += S; h->st.ing[1] = p; p += S;
-    h->st.cap_c = p; p += S; h->st.max_new = p; p += S; h->st.n_emit = p; p += S;
+    h->st.cap_c = p; p += S; h->st.max_new = p; p += S; h->st.n_emit = p; p += S; h->st.grp = p; p += S;
     h->st.active = h->st_mem8; h->st.owner = h->st_mem8 + S; h->st.done = h->st_mem8 + 2 * S;
   }
   INIT_TRY(dmalloc(h, &h->tokens, (size_t)S * c.max_seq_len * 4));
@@ -776,7 +807,7 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
   INIT_TRY(dmalloc(h, &h->n_active, 4));
   INIT_CU(cudaMemset(h->n_active, 0, 4));
   INIT_TRY(dmalloc(h, &h->stage_off, (size_t)(S + 1) * sizeof(long long)));
-  INIT_TRY(dmalloc(h, &h->stage_i32, (size_t)3 * S * 4));
+  INIT_TRY(dmalloc(h, &h->stage_i32, (size_t)5 * S * 4));
 
   // RoPE table: cos/sin of pos * theta^(-2j/d), evaluated in double, stored as fp32
   {
@@ -839,11 +870,19 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
     }
     // page tables
     INIT_TRY(dmalloc(h, &w.bt, (size_t)S * h->max_pages * 4));
-    INIT_TRY(dmalloc(h, &w.npages, (size_t)S * 4));
+    INIT_TRY(dmalloc(h, &w.npages, (size_t)2 * S * 4));   // npages, then nshared
     INIT_TRY(dmalloc(h, &w.free_pages, (size_t)h->pool_pages * 4));
     INIT_TRY(dmalloc(h, &w.free_top, 4));
     INIT_CU(cudaMemset(w.bt, 0, (size_t)S * h->max_pages * 4));
-    h->pt[m].bt = w.bt; h->pt[m].npages = w.npages; h->pt[m].free_pages = w.free_pages; h->pt[m].free_top = w.free_top;
+    h->pt[m].bt = w.bt; h->pt[m].npages = w.npages; h->pt[m].nshared = w.npages + S; h->pt[m].free_pages = w.free_pages; h->pt[m].free_top = w.free_top;
+  }
+  INIT_TRY(dmalloc(h, &h->gt_mem, (size_t)6 * S * 4));
+  INIT_CU(cudaMemset(h->gt_mem, 0, (size_t)6 * S * 4));
+  INIT_TRY(dmalloc(h, &h->gt_pages_mem, (size_t)2 * S * h->max_pages * 4));
+  {
+    int32_t* p = h->gt_mem;
+    for (int m = 0; m < 2; ++m) { h->gt.state[m] = p; p += S; h->gt.donor[m] = p; p += S; h->gt.pages[m] = h->gt_pages_mem + (size_t)m * S * h->max_pages; }
+    h->gt.npg = p; p += S; h->gt.ref = p; p += S;
   }
   INIT_CU(cudaEventCreateWithFlags(&h->ev_in, cudaEventDisableTiming));
   INIT_CU(cudaEventCreateWithFlags(&h->ev_out, cudaEventDisableTiming));
@@ -915,10 +954,13 @@ int tandem_reset(tandem_handle* h) {
   for (int m = 0; m < 2; ++m) {
     CU(h, cudaMemcpy(h->ws[m].free_pages, fp.data(), (size_t)h->pool_pages * 4, cudaMemcpyHostToDevice));
     CU(h, cudaMemcpy(h->ws[m].free_top, &top, 4, cudaMemcpyHostToDevice));
-    CU(h, cudaMemset(h->ws[m].npages, 0, (size_t)S * 4));
+    CU(h, cudaMemset(h->ws[m].npages, 0, (size_t)2 * S * 4));
     CU(h, cudaMemset(h->ws[m].chunk_ctr, 0, (size_t)S * 4));
   }
   std::fill(h->slot_busy.begin(), h->slot_busy.end(), 0);
+  CU(h, cudaMemset(h->gt_mem, 0, (size_t)6 * S * 4));
+  h->slot_grp.assign(S, -1); h->grp_live.assign(S, 0); h->grp_free.clear(); h->grp_reserved.assign(S, 0); h->grp_released = 0;
+  for (int g = S - 1; g >= 0; --g) h->grp_free.push_back(g);
   h->launches = 0;
   return TANDEM_OK;
 }
@@ -1047,6 +1089,11 @@ int tandem_generate(tandem_handle* h, const tandem_params* params, int32_t B, co
   // (prompt + max_new), so a rollout never runs out of pages half-way; the rest waits in the queue (order preserved).
   std::vector<int> slot_pages(c.max_seqs, 0);
   auto pages_of = [&](int b) { return (int)((prompt_offsets[b + 1] - prompt_offsets[b] + max_new[b] + kPageTokens - 1) / kPageTokens); };
+  auto shared_pages_of = [&](int b) { return (int)((prompt_offsets[b + 1] - prompt_offsets[b] - 1) / kPageTokens); };
+  auto same_prompt = [&](int a, int b) {
+    const int64_t la = prompt_offsets[a + 1] - prompt_offsets[a], lb = prompt_offsets[b + 1] - prompt_offsets[b];
+    return la == lb && std::memcmp(prompt_tokens + prompt_offsets[a], prompt_tokens + prompt_offsets[b], (size_t)la * 4) == 0;
+  };
   int pages_reserved = 0;
   const int pages_avail = h->pool_pages - 1;
   for (int b = 0; b < B; ++b) if (pages_of(b) > pages_avail) return fail(h, TANDEM_ENOMEM, "a single sequence needs more KV pages than the pool holds");
@@ -1060,17 +1107,30 @@ int tandem_generate(tandem_handle* h, const tandem_params* params, int32_t B, co
     int nfree = 0;
     for (int i = 0; i < c.max_seqs; ++i) nfree += !h->slot_busy[i];
     int n = 0, add = 0;
-    while (n < std::min(nfree, B - next) && pages_reserved + add + pages_of(next + n) <= pages_avail) { add += pages_of(next + n); ++n; }
+    while (n < std::min(nfree, B - next)) {
+      // with prompt-page sharing a sequence whose prompt equals its predecessor's in this batch joins that group (the rule of
+      // admit()) and needs no pages of its own for the shared prefix
+      const int b = next + n;
+      const int need = pages_of(b) - ((c.share_prompt_pages && n > 0 && same_prompt(b - 1, b)) ? shared_pages_of(b) : 0);
+      if (pages_reserved + add + need > pages_avail) break;
+      add += need; ++n;
+    }
     if (n > 0) {
       std::vector<int32_t> slots(n);
       for (int i = 0; i < n; ++i) ids[i] = seq_ids ? seq_ids[next + i] : next + i;
       if ((rc = admit(h, params, ovr, n, prompt_tokens, prompt_offsets + next, ids.data(), max_new + next, slots.data(), s))) return rc;
-      for (int i = 0; i < n; ++i) { slot_seq[slots[i]] = next + i; slot_pages[slots[i]] = pages_of(next + i); }
+      for (int i = 0; i < n; ++i) {
+        const int b = next + i, g = h->slot_grp[slots[i]];
+        slot_seq[slots[i]] = b;
+        slot_pages[slots[i]] = pages_of(b) - (g >= 0 ? shared_pages_of(b) : 0);   // a group holds its shared pages until its last member finishes
+        if (g >= 0) h->grp_reserved[g] = shared_pages_of(b);
+      }
       pages_reserved += add;
       next += n;
     }
     for (int k = 0; k < poll; ++k) if ((rc = run_step(h, io, rp, s))) return rc;
     if ((rc = refresh_slots(h, s))) return rc;
+    pages_reserved -= h->grp_released; h->grp_released = 0;
     CU(h, cudaMemcpy(nemit.data(), h->st.n_emit, (size_t)c.max_seqs * 4, cudaMemcpyDeviceToHost));
     CU(h, cudaMemcpy(plen.data(), h->st.prompt_len, (size_t)c.max_seqs * 4, cudaMemcpyDeviceToHost));
     for (int i = 0; i < c.max_seqs; ++i) {
@@ -1228,6 +1288,7 @@ void tandem_free(tandem_handle* h) {
   for (cudaEvent_t e : h->stagger_ev) cudaEventDestroy(e);
   fr(h->zero_counts);
   fr(h->score_out[0]); fr(h->score_out[1]); fr(h->st_mem); fr(h->st_mem8); fr(h->tokens); fr(h->out_owner); fr(h->out_logp); fr(h->rope_cs); fr(h->word_start_dev); fr(h->stats);
+  fr(h->gt_mem); fr(h->gt_pages_mem);
   fr(h->lt_wmaps); fr(h->lt_amaps); fr(h->lt_ts); fr(h->n_active); fr(h->work_ctr); fr(h->stage_tokens); fr(h->stage_off); fr(h->stage_i32);
   cudaGetLastError();
   delete h;

@@ -1,0 +1,106 @@
+"""-m gpu: prompt-page sharing across the G rollouts of a prompt (tandem_config.share_prompt_pages; SURVEY.md section 8(a)
+"pages"). The K/V of equal prefixes are equal, so the outputs must be those of the oracle (which knows
+nothing about pages) and of the engine without sharing; what changes is the bookkeeping: prompt rows computed once per model and
+group, fewer pages in use, every page back in the pool at the end."""
+import numpy as np
+import pytest
+import torch
+
+import paper_2606_28166_b200 as T
+from oracle import TandemParams as OParams, tandem_generate
+from oracle.rule import Uniforms
+from workloads import get_workload, make_word_start, ModelShape
+from gpu_util import make_pair
+
+pytestmark = pytest.mark.gpu
+TINY = get_workload("cfg1_tiny_f32").shape
+
+
+def _grouped_prompts(shape, lens, group, seed):
+    rng = np.random.default_rng(seed)
+    out = []
+    for n in lens:
+        ids = rng.integers(0, shape.vocab, size=n).astype(np.int32)
+        out.extend([ids.copy() for _ in range(group)])
+    return out
+
+
+def _same(out, ref, B, logp_tol):
+    for b in range(B):
+        n = out["len"][b]
+        assert n == len(ref["tokens"][b])
+        assert np.array_equal(out["tokens"][b, :n], ref["tokens"][b]), b
+        assert np.array_equal(out["owner"][b, :n], ref["owner"][b]), b
+        assert np.max(np.abs(out["sen_logp"][b, :n] - ref["sen_logp"][b])) < logp_tol
+
+
+@pytest.mark.parametrize("start,rows,graph", [(T.SENIOR, 0, 1), (T.DRAW, 0, 0), (T.SENIOR, 24, 1), (T.JUNIOR, 9, 0)])
+def test_shared_prompt_pages_match_oracle(start, rows, graph):
+    """fp32, 3 prompts x 4 rollouts (lengths 40, 17, 70: 2, 1 and 4 shared pages) plus an ungrouped short prompt; also with
+    a row budget that chunks the donor's prefill over several steps (followers wait) and with drawn start owners."""
+    table = make_word_start(TINY.vocab, 0.3, 5)
+    prompts = _grouped_prompts(TINY, (40, 17, 70), 4, seed=21) + [np.arange(9, dtype=np.int32)]
+    B = len(prompts)
+    max_new = [28] * B
+    eng, orc, _ = make_pair(TINY, (1, 2), max_seqs=B, max_seq_len=112, share_prompt_pages=1, max_rows_per_step=rows, use_graph=graph)
+    ref = tandem_generate(orc, OParams(p=0.5, temperature=1.0, seed=91, start_owner=start), prompts, max_new, table, uni=Uniforms(seed=91))
+    out = eng.generate(T.TandemParams(table, p=0.5, temperature=1.0, seed=91, start_owner=start), prompts, max_new)
+    _same(out, ref, B, 2e-5)
+    st = out["stats"]
+    # the start model computes each group's shared prefix once: the other three members take it over (32 + 16 + 64 positions)
+    assert st["shared_prompt_rows"] >= 3 * (32 + 16 + 64)
+    assert 0 < out["owner"].mean() < 1
+    eng.free()
+    # without sharing: same outputs, more rows, more pages
+    eng0, _, _ = make_pair(TINY, (1, 2), max_seqs=B, max_seq_len=112, share_prompt_pages=0, max_rows_per_step=rows, use_graph=graph)
+    out0 = eng0.generate(T.TandemParams(table, p=0.5, temperature=1.0, seed=91, start_owner=start), prompts, max_new)
+    eng0.free()
+    for k in ("tokens", "owner", "len"):
+        assert np.array_equal(out[k], out0[k])
+    assert np.max(np.abs(out["sen_logp"] - out0["sen_logp"])) < 2e-5
+    st0 = out0["stats"]
+    assert st0["shared_prompt_rows"] == 0
+    assert st["rows_senior"] + st["rows_junior"] + st["shared_prompt_rows"] == st0["rows_senior"] + st0["rows_junior"]
+    assert st["peak_pages_senior"] < st0["peak_pages_senior"] or st["peak_pages_junior"] < st0["peak_pages_junior"]
+
+
+def test_shared_pages_are_returned_and_groups_recycled():
+    """Queued admission with a pool of a few rollouts: groups come and go (their table entries and pages are reused); a leaked
+    page or a stale group entry would end in the pool-exhausted error or in wrong tokens. Some members finish early (EOS)."""
+    table = make_word_start(TINY.vocab, 0.3, 5)
+    prompts = _grouped_prompts(TINY, (36, 20, 50, 33, 41), 3, seed=4)
+    B = len(prompts)
+    max_new = np.array([10 + 3 * (b % 5) for b in range(B)], dtype=np.int32)
+    page_bytes = 2 * TINY.n_layers * TINY.n_kv_heads * 16 * TINY.head_dim * 4
+    eng, orc, _ = make_pair(TINY, (1, 2), max_seqs=4, max_seq_len=96, share_prompt_pages=1, kv_bytes_per_model=21 * page_bytes)
+    op = OParams(p=0.5, temperature=1.0, seed=13, eos_id=7)
+    ref = tandem_generate(orc, op, prompts, max_new, table, uni=Uniforms(seed=13))
+    prm = T.TandemParams(table, p=0.5, temperature=1.0, seed=13, eos_id=7)
+    for _ in range(2):
+        out = eng.generate(prm, prompts, max_new)
+        _same(out, ref, B, 2e-5)
+        assert out["stats"]["peak_resident"] <= 4
+    eng.free()
+
+
+def test_shared_prompt_pages_bf16_step_api():
+    """bf16 (tcgen05 GEMM, tensor-core attention) through tandem_step: members admitted in one call form a group; compared with the
+    engine without sharing on the same forced token stream (owners exact, log-probs up to bf16 rounding of a different q-tiling)."""
+    shape = ModelShape(3, 256, 4, 2, 64, 512, 2048, 1e-6, 1e6, "bf16")
+    table = make_word_start(shape.vocab, 0.3, 5)
+    prompts = _grouped_prompts(shape, (45, 70), 4, seed=2)
+    B, n_new = len(prompts), 24
+    prm = T.TandemParams(table, p=0.5, temperature=1.0, seed=5)
+    res = []
+    forced = None
+    for share in (0, 1):
+        eng, _, _ = make_pair(shape, (1, 2), max_seqs=B, max_seq_len=128, share_prompt_pages=share, use_graph=1)
+        out = eng.generate(prm, prompts, [n_new] * B, forced_tokens=forced)
+        res.append(out)
+        if forced is None:
+            forced = torch.as_tensor(out["tokens"].astype(np.int32)).cuda()
+        eng.free()
+    a, b = res
+    assert np.array_equal(a["tokens"], b["tokens"]) and np.array_equal(a["owner"], b["owner"])
+    assert np.max(np.abs(a["sen_logp"] - b["sen_logp"])) < 0.02
+    assert a["stats"]["shared_prompt_rows"] == 0 and b["stats"]["shared_prompt_rows"] >= 3 * (32 + 64)
