@@ -48,7 +48,7 @@ def parse_args():
     ap.add_argument("--grpo", action="store_true", help="time tandem_grpo_objective (senior-masked GRPO forward, NEXT-3) on the workload's batch x max_new")
     ap.add_argument("--score", type=int, default=0, help="N > 0: time tandem_score (teacher-forced dual scoring, NEXT-1) on N synthetic streams instead of the rollout")
     ap.add_argument("--score-len", type=int, default=2048, help="tokens per stream for --score")
-    ap.add_argument("--score-rows", type=int, default=512, help="rows per step and model for --score (max_rows_per_step)")
+    ap.add_argument("--score-rows", type=int, default=2048, help="rows per step and model for --score (max_rows_per_step)")
     ap.add_argument("--top-k", type=int, default=0, help="top-k filter of the sampler (0 = off; the paper evaluates with 20)")
     ap.add_argument("--temperature", type=float, default=None, help="override the workload's sampling temperature")
     ap.add_argument("--top-p", type=float, default=None, help="override the workload's top-p (the paper trains at 1.0, evaluates at 0.8)")

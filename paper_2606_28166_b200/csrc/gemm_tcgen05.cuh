@@ -172,6 +172,8 @@ struct TcGemmArgs {
   int N, K, n_split;
   size_t split_stride;        // floats between partials
   int ring_bytes;             // shared-memory ring of this launch (200 KB: one CTA per SM; 98 KB: two)
+  int chunk_grid;             // >= 1: the 256-row chunks of the token rows are dealt round-robin to this many CTAs per (tile, split)
+                              // (gridDim.y = n_split * chunk_grid); 1 = one CTA walks all chunks
 };
 
 // ---------------------------------------------------------------------------------------------- the kernel
@@ -203,7 +205,8 @@ gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__
   const uint32_t rank = PAIR ? ptx::cluster_ctarank() : 0u;
   const bool leader = rank == 0;
   const int n0 = blockIdx.x * kTcTileN;
-  const int split = blockIdx.y;
+  const int split = (int)blockIdx.y % g.n_split;
+  const int cslice = (int)blockIdx.y / g.n_split, cstep = g.chunk_grid;   // this CTA's chunks: cslice, cslice + cstep, ...
   const int kb_total = (g.K + kTcBlockK - 1) / kTcBlockK;
   const int kb0 = (int)((long long)kb_total * split / g.n_split);
   const int kb1 = (int)((long long)kb_total * (split + 1) / g.n_split);
@@ -243,7 +246,7 @@ gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__
     {
       const uint64_t pol_w = ptx::policy_evict_first();
       int it = 0;
-      for (int c = 0; c < n_chunks; ++c)
+      for (int c = cslice; c < n_chunks; c += cstep)
         for (int kb = kb0; kb < kb1; ++kb, ++it) {
           const int s = it % n_stages;
           ptx::mbar_wait(empty_bar(s), ((uint32_t)(it / n_stages) & 1u) ^ 1u);
@@ -265,7 +268,7 @@ gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__
       const uint64_t pol_a = ptx::policy_evict_last();
       pdl_wait();                                            // the activations come from the predecessor kernel
       int it = 0;
-      for (int c = 0; c < n_chunks; ++c) {
+      for (int c = cslice; c < n_chunks; c += cstep) {
         const int cols = chunk_cols(c * kTcMaxRows);
         const int nbox = cols / kTcRowBox / (PAIR ? 2 : 1);
         const int r0 = c * kTcMaxRows + (PAIR ? (int)rank * (cols / 2) : 0);   // a pair: this CTA's half of the token rows
@@ -296,10 +299,10 @@ gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__
     // ===== MMA issuer: one elected lane drives the tensor core for the whole CTA (for both CTAs of a pair: the leader's)
     if (leader) {
       int it = 0;
-      for (int c = 0; c < n_chunks; ++c) {
+      for (int c = cslice, ci = 0; c < n_chunks; c += cstep, ++ci) {
         const int ncols = chunk_cols(c * kTcMaxRows);
         const uint32_t idesc = umma_idesc_bf16(ncols, PAIR ? 2 * kTcTileN : kTcTileN);
-        ptx::mbar_wait(tmem_empty_bar, ((uint32_t)c & 1u) ^ 1u);
+        ptx::mbar_wait(tmem_empty_bar, ((uint32_t)ci & 1u) ^ 1u);
         ptx::tc_fence_after();
         for (int kb = kb0; kb < kb1; ++kb, ++it) {
           const int s = it % n_stages;
@@ -331,10 +334,10 @@ gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__
     float* outp = g.out + (size_t)split * g.split_stride;
     const uint32_t te_bar = PAIR ? ptx::mapa_rank(tmem_empty_bar, 0) : tmem_empty_bar;
     pdl_wait();                                            // the predecessor may still be reading the buffer this kernel writes
-    for (int c = 0; c < n_chunks; ++c) {
+    for (int c = cslice, ci = 0; c < n_chunks; c += cstep, ++ci) {
       const int r0 = c * kTcMaxRows;
       const int crow = min(rows - r0, kTcMaxRows);
-      ptx::mbar_wait(tmem_full_bar, (uint32_t)c & 1u);
+      ptx::mbar_wait(tmem_full_bar, (uint32_t)ci & 1u);
       ptx::tc_fence_after();
       for (int c0 = 32 * half; c0 < crow; c0 += 64) {
         uint32_t v[32];
@@ -445,7 +448,7 @@ inline int tc_gemm_launch_epi(const TcMaps& maps, const Pair<TcGemmArgs>& g, dim
   if (pair) return launch_ex_cluster(gemm_tcgen05_kernel<EPI, true>, grid, dim3(kTcThreads), smem, s, pdl, 2, maps, g) == cudaSuccess ? 0 : -3;
   return launch_ex(gemm_tcgen05_kernel<EPI, false>, grid, dim3(kTcThreads), smem, s, pdl, maps, g) == cudaSuccess ? 0 : -3;
 }
-struct TcGemmTune { int ring_kb = 0, splits = 0; bool pdl = false; int pair = 0; };   // pair: 1 = CTA pairs (cta_group::2), 0 = single CTAs   // 0 = automatic; overrides for tuning / tandem_test_gemm_time
+struct TcGemmTune { int ring_kb = 0, splits = 0; bool pdl = false; int pair = 0; int chunk_grid = 1; };   // pair: 1 = CTA pairs (cta_group::2), 0 = single CTAs   // 0 = automatic; overrides for tuning / tandem_test_gemm_time
 // One launch for n_models (1 or 2) problems of the same shape: out[m] = A[m] W[m]^T, rows of model m from rows_ptr[m].
 inline int tc_gemm_launch(TcGemmPlans* p, int n_models, int which, const void* const* A, const void* const* W, int N, int K, float* const* out,
                           const int32_t* const* rows_ptr, int rows_cap, int* n_split, size_t* split_stride, cudaStream_t s, int epi = kTcEpiPartial,
@@ -460,8 +463,11 @@ inline int tc_gemm_launch(TcGemmPlans* p, int n_models, int which, const void* c
   const int tiles_pad = pair ? (tiles + 1) & ~1 : tiles;   // a pair takes two adjacent weight tiles (a tile past N reads zeros and writes nothing)
   TcMaps maps;
   Pair<TcGemmArgs> g;
+  // many token rows (scoring, prefill): the 256-row chunks go to different CTAs, so the launch has more and shorter CTAs and a
+  // shorter tail (ncu, 512 rows, gate/up as 304 CTAs on 296 slots: SMs active 60% of the kernel's duration)
+  const int CG = (tune && tune->chunk_grid > 1) ? std::min(tune->chunk_grid, (rows_cap + kTcMaxRows - 1) / kTcMaxRows) : 1;
   const int ring = (tune && tune->ring_kb > 0) ? tune->ring_kb * 1024
-                                                : (tiles_pad * S * n_models > 148 ? 109 * 1024 : kTcRingBytes);   // more CTAs than SMs: two share an SM
+                                                : (tiles_pad * S * CG * n_models > 148 ? 109 * 1024 : kTcRingBytes);   // more CTAs than SMs: two share an SM
   for (int m = 0; m < 2; ++m) {
     const int mm = m < n_models ? m : 0;
     const CUtensorMap* mw = tc_gemm_map(p, W[mm], N, K, kTcTileN);
@@ -472,9 +478,9 @@ inline int tc_gemm_launch(TcGemmPlans* p, int n_models, int which, const void* c
       if (!ma) return -3;
       maps.a[m][b] = *ma;
     }
-    g.m[m] = TcGemmArgs{out[mm], rows_ptr ? rows_ptr[mm] : nullptr, rows_cap, N, K, S, *split_stride, ring};
+    g.m[m] = TcGemmArgs{out[mm], rows_ptr ? rows_ptr[mm] : nullptr, rows_cap, N, K, S, *split_stride, ring, CG};
   }
-  dim3 grid(tiles_pad, S, n_models);
+  dim3 grid(tiles_pad, S * CG, n_models);
   const bool pdl = tune && tune->pdl;
   if (epi == kTcEpiSwiGLU) return tc_gemm_launch_epi<1>(maps, g, grid, s, pdl, pair);
   return tc_gemm_launch_epi<0>(maps, g, grid, s, pdl, pair);
