@@ -83,9 +83,55 @@ def test_shared_pages_are_returned_and_groups_recycled():
     eng.free()
 
 
-def test_shared_prompt_pages_bf16_step_api():
-    """bf16 (tcgen05 GEMM, tensor-core attention) through tandem_step: members admitted in one call form a group; compared with the
-    engine without sharing on the same forced token stream (owners exact, log-probs up to bf16 rounding of a different q-tiling)."""
+def test_shared_prompt_pages_through_tandem_step():
+    """The step call with two admissions: a group admitted at step 1, a second group (same prompt as an unrelated single) a few
+    steps later while the first is running; a waiting member emits nothing (token -1) until its donor has stored the prefix.
+    Per-sequence streams equal the oracle's."""
+    table = make_word_start(TINY.vocab, 0.3, 5)
+    first = _grouped_prompts(TINY, (40,), 3, seed=6)
+    second = [np.arange(30, dtype=np.int32)] + _grouped_prompts(TINY, (52,), 2, seed=7)
+    n_new = 20
+    eng, orc, _ = make_pair(TINY, (1, 2), max_seqs=6, max_seq_len=96, share_prompt_pages=1, use_graph=1)
+    prm = T.TandemParams(table, p=0.5, temperature=1.0, seed=3)
+    o = dict(token=torch.zeros(6, dtype=torch.int32, device="cuda"), owner=torch.zeros(6, dtype=torch.uint8, device="cuda"),
+             done=torch.zeros(6, dtype=torch.uint8, device="cuda"))
+    streams = {i: [] for i in range(6)}
+    owners = {i: [] for i in range(6)}
+    slot_of = {}
+    waited = 0
+    for t in range(80):
+        admit = None
+        if t == 0:
+            admit = (first, [10, 11, 12], [n_new] * 3)
+        elif t == 5:
+            admit = (second, [20, 21, 22], [n_new] * 3)
+        slots = eng.step(prm, admit=admit, out=o)
+        torch.cuda.synchronize()
+        if admit is not None:
+            for sid, sl in zip(admit[1], slots):
+                slot_of[int(sl)] = sid
+        tok = o["token"].cpu().numpy(); own = o["owner"].cpu().numpy()
+        for sl, sid in slot_of.items():
+            if tok[sl] >= 0:
+                streams[sl].append(int(tok[sl])); owners[sl].append(int(own[sl]))
+            elif len(streams[sl]) < n_new:
+                waited += 1
+        if all(len(streams[sl]) == n_new for sl in slot_of) and len(slot_of) == 6:
+            break
+    assert waited >= 2          # the followers of both groups sat out the donor's prefill step
+    ref = tandem_generate(orc, OParams(p=0.5, temperature=1.0, seed=3), first + second, [n_new] * 6, table,
+                          uni=Uniforms(seed=3, seq_ids=[10, 11, 12, 20, 21, 22]))
+    sid_to_b = {10: 0, 11: 1, 12: 2, 20: 3, 21: 4, 22: 5}
+    for sl, sid in slot_of.items():
+        b = sid_to_b[sid]
+        assert streams[sl] == list(ref["tokens"][b]) and owners[sl] == list(ref["owner"][b]), sid
+    assert eng.get_stats()["shared_prompt_rows"] >= 2 * 32 + 48
+    eng.free()
+
+
+def test_shared_prompt_pages_bf16():
+    """bf16 (tcgen05 GEMM, tensor-core attention): compared with the engine without sharing on the same forced token stream
+    (owners exact, log-probs up to bf16 rounding of a different q-tiling)."""
     shape = ModelShape(3, 256, 4, 2, 64, 512, 2048, 1e-6, 1e6, "bf16")
     table = make_word_start(shape.vocab, 0.3, 5)
     prompts = _grouped_prompts(shape, (45, 70), 4, seed=2)
