@@ -324,7 +324,9 @@ int launch_layer_tail(tandem_handle* h, int li, cudaStream_t s) {
 
 // ------------------------------------------------------------------------------------------ both models' forward (S1..S8)
 // Every kernel is launched once for the two models (Pair arguments): the models advance layer by layer in lock-step on
-// one stream, each launch carrying the senior's and the junior's half of the work.
+// one stream, each launch carrying the senior's and the junior's half of the work. s2 != nullptr selects the opt-in staggered
+// mode instead (TANDEM_STAGGER=1: one chain of single-model launches per model, the junior's on s2; same results, measured
+// slower - DESIGN.md section 9).
 template <typename T>
 int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaStream_t s, bool score = false, float score_inv_t = 1.f, cudaStream_t s2 = nullptr) {
   const tandem_config& c = h->cfg;
