@@ -72,6 +72,7 @@ struct tandem_handle {
   int gemm_pair = -1;                            // tcgen05 projections as CTA pairs (cta_group::2): -1 = automatic (while scoring: hundreds of
                                                  // rows per launch, +5%; no gain at the rollout's ~128 rows), 0 / 1 = env TANDEM_GEMM_PAIR
   bool scoring = false;
+  bool score_nosplit = true;
   int score_chunk_grid = 8;                      // scoring: CTAs per (weight tile, K split) along the token rows (env TANDEM_SCORE_CHUNK_GRID; 1 = off)
   bool use_tail = false;                        // persistent layer-tail kernel (bf16 + tcgen05 + tensor-core attention; env TANDEM_TAIL=1 enables)
   LtWMaps* lt_wmaps = nullptr; LtAMaps* lt_amaps = nullptr; bool lt_maps_ready = false;   // device tensor-map tables of the layer-tail kernel
@@ -175,7 +176,11 @@ int launch_gemm(tandem_handle* h, int which, const void* const* A, const void* c
     int rc = 0;
     TcGemmTune tune; tune.ring_kb = h->gemm_ring_kb; tune.pdl = h->use_pdl;
  tune.pair = h->gemm_pair >= 0 ? h->gemm_pair : (h->scoring ? 1 : 0);
-    if (h->scoring && which != 4) tune.chunk_grid = h->score_chunk_grid;   // hundreds of rows per launch: one CTA per 256-row chunk
+    if (h->scoring && which != 4) {
+      tune.chunk_grid = h->score_chunk_grid;   // hundreds of rows per launch: one CTA per 256-row chunk
+      // with >= 4 chunks per weight tile the launch is wide enough without K-splits: a third of the fp32 partials to write and re-read
+      if (h->score_nosplit && std::min(tune.chunk_grid, (rows_cap + kTcMaxRows - 1) / kTcMaxRows) >= 4) tune.splits = 1;
+    }
     if (nm == 1) {   // staggered mode: the K-splits of the paired launch (same reduction order, bit-identical results) and a ring that leaves
                      // room for the other model's attention CTA on the same SM
       if (which != 4 && epi != kTcEpiSwiGLU) tune.splits = tc_gemm_splits(N, K, 2);
@@ -910,6 +915,7 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
   if (const char* e = getenv("TANDEM_TAIL"))
     h->use_tail = atoi(e) != 0 && c.dtype == TANDEM_BF16 && h->gemm_impl == TANDEM_GEMM_TCGEN05 && h->attn_impl == TANDEM_ATTN_MMA;
   if (const char* e = getenv("TANDEM_GEMM_RING_KB")) h->gemm_ring_kb = std::max(0, std::min(200, atoi(e)));
+  if (const char* e = getenv("TANDEM_SCORE_NOSPLIT")) h->score_nosplit = atoi(e) != 0;
   if (const char* e = getenv("TANDEM_SCORE_CHUNK_GRID")) h->score_chunk_grid = std::max(1, std::min(16, atoi(e)));
   if (const char* e = getenv("TANDEM_GEMM_PAIR")) h->gemm_pair = atoi(e) != 0 ? 1 : 0;
   {
