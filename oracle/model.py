@@ -26,6 +26,12 @@ Two evaluation orders of the same definition, which must agree (pin 4, tests/tes
 `round_bf16=True` is the rounding-point-faithful mode (DESIGN.md §3 R-V): float64 arithmetic with
 round-to-nearest-even bf16 applied at exactly the points where the bf16 CUDA path stores bf16
 (GEMM A-operands and the KV cache). It is used only for the sharp kernel-correctness check.
+`round_qp=True` (only with `round_bf16`) adds the two rounding points of the tensor-core attention path
+that R-V names: the RoPE'd queries are stored as bf16, and the softmax numerators exp(s - max) enter
+the P.V product as bf16 while the denominator is summed from the unrounded values:
+o_i = sum_j bf16(e_ij) v_j / sum_j e_ij. (A tiled online softmax rounds e relative to its running
+maximum, which is the same relative rounding, not the same bits; so this mode is statistically, not
+bitwise, faithful for P.)
 """
 import numpy as np
 
@@ -96,10 +102,11 @@ class KVState:
 
 
 class OracleModel:
-    def __init__(self, cfg, weights, round_bf16=False, cache=True):
+    def __init__(self, cfg, weights, round_bf16=False, cache=True, round_qp=False):
         self.cfg = cfg
         self.w = weights
         self.round_bf16 = bool(round_bf16)
+        self.round_qp = bool(round_qp) and self.round_bf16
         self._cache = {} if cache else None
 
     # -- weight access: float64 view of the values as given ------------------------------------
@@ -131,6 +138,8 @@ class OracleModel:
             k = (u @ self._W("wk", l).T).reshape(n_new, nkv, d)
             v = (u @ self._W("wv", l).T).reshape(n_new, nkv, d)
             q = rope(q, positions, c.rope_theta)
+            if self.round_qp:
+                q = round_to_bf16(q)
             k = self._rb(rope(k, positions, c.rope_theta))
             v = self._rb(v)
             if state is not None:
@@ -150,8 +159,12 @@ class OracleModel:
                 g = a // group
                 s = (q[:, a, :] @ kk[:, g, :].T) / np.sqrt(d)          # [n_new, n_ctx]
                 s = np.where(causal, s, -np.inf)
-                p = softmax_rows(s)
-                o[:, a, :] = p @ vv[:, g, :]
+                if self.round_qp:                                      # bf16 numerators, unrounded denominator (R-V)
+                    e = np.exp(s - np.max(s, axis=-1, keepdims=True))
+                    o[:, a, :] = (round_to_bf16(e) @ vv[:, g, :]) / np.sum(e, axis=-1, keepdims=True)
+                else:
+                    p = softmax_rows(s)
+                    o[:, a, :] = p @ vv[:, g, :]
             o = self._rb(o.reshape(n_new, nq * d))
             h = h + o @ self._W("wo", l).T
             u = self._rb(rms_norm(h, self._W("mlp_norm", l), c.rms_eps))

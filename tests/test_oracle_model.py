@@ -249,3 +249,49 @@ def test_round_to_bf16_matches_torch():
     m = OracleModel(MICRO, make_weights(MICRO, 3), round_bf16=True)
     t = np.arange(6)
     assert 0 < np.max(np.abs(m.forward_full(t) - OracleModel(MICRO, m.w).forward_full(t))) < 0.05
+
+
+def test_round_qp_mode_pins():
+    """`round_qp` (DESIGN.md section 3 R-V: bf16 queries, bf16 softmax numerators over an unrounded denominator).
+    (a) a single key has softmax 1 whatever the query, and 1 is a bf16 number: identical to `round_bf16` alone;
+    (b) with an independent torch composition of one attention head (bf16 casts by torch) on values chosen so
+        that nothing else rounds; (c) the perturbation of the logits is of the size of a bf16 ulp, not zero."""
+    m0 = OracleModel(MICRO, make_weights(MICRO, 3), round_bf16=True)
+    m1 = OracleModel(MICRO, m0.w, round_bf16=True, round_qp=True)
+    assert np.array_equal(m0.forward_full([5]), m1.forward_full([5]))
+    assert not OracleModel(MICRO, m0.w, round_qp=True).round_qp                      # needs round_bf16
+    t = np.arange(9)
+    d = np.max(np.abs(m0.forward_full(t) - m1.forward_full(t)))
+    assert 0 < d < 0.05
+    # (b) one layer, one head, identity projections except W_v; W_o = W_down = 0 would hide the head, so read the
+    # attention output through W_o = I and a zero MLP: h1 = h0 + o.
+    s = ModelShape(1, 4, 1, 1, 4, 4, 4, 0.0, 1e4, "f32")
+    w = make_weights(s, 0)
+    L = w["layers"][0]
+    rng = np.random.default_rng(5)
+    E = torch.as_tensor(rng.standard_normal((4, 4)))
+    w["embed"] = E.clone()
+    for n in ("attn_norm", "mlp_norm"):
+        L[n] = torch.ones(4, dtype=torch.float64)
+    w["final_norm"] = torch.ones(4, dtype=torch.float64)
+    L["wq"] = torch.eye(4, dtype=torch.float64); L["wk"] = torch.eye(4, dtype=torch.float64); L["wv"] = torch.eye(4, dtype=torch.float64)
+    L["wo"] = torch.eye(4, dtype=torch.float64)
+    L["w_gate"] = torch.zeros(4, 4, dtype=torch.float64); L["w_up"] = torch.zeros(4, 4, dtype=torch.float64); L["w_down"] = torch.zeros(4, 4, dtype=torch.float64)
+    w["lm_head"] = torch.eye(4, dtype=torch.float64)
+    toks = [0, 1, 2, 3]
+    z = OracleModel(s, w, round_bf16=True, round_qp=True).forward_full(toks)
+    bf = lambda x: x.to(torch.float32).to(torch.bfloat16).to(torch.float64)
+    h = E[toks]
+    u = bf(h / torch.sqrt((h * h).mean(-1, keepdim=True)))
+    pos = torch.arange(4, dtype=torch.float64)
+    inv = torch.as_tensor([1e4 ** (-2.0 * j / 4) for j in range(2)], dtype=torch.float64)
+    ang = pos[:, None] * inv[None, :]
+    rot = lambda x: torch.cat([x[:, :2] * torch.cos(ang) - x[:, 2:] * torch.sin(ang), x[:, 2:] * torch.cos(ang) + x[:, :2] * torch.sin(ang)], -1)
+    q, k, v = bf(rot(u)), bf(rot(u)), bf(u)
+    sc = (q @ k.T) / 2.0
+    sc = sc.masked_fill(torch.triu(torch.ones(4, 4, dtype=torch.bool), 1), float("-inf"))
+    e = torch.exp(sc - sc.max(-1, keepdim=True).values)
+    o = bf((bf(e) @ v) / e.sum(-1, keepdim=True))
+    h1 = h + o
+    f = bf(h1 / torch.sqrt((h1 * h1).mean(-1, keepdim=True)))        # MLP is zero; final norm, then the identity head
+    assert np.allclose(z, f.numpy(), atol=1e-12)
