@@ -17,8 +17,9 @@ _ERR = {0: "OK", -1: "EINVAL", -2: "ENOMEM", -3: "ECUDA", -4: "ESTATE", -5: "EFU
 
 EXPORTED_SYMBOLS = ["tandem_init", "tandem_load_weights", "tandem_step", "tandem_generate", "tandem_score", "tandem_grpo_objective", "tandem_reset",
                     "tandem_free", "tandem_last_error", "tandem_get_stats", "tandem_set_profile", "tandem_get_profile",
-                    "tandem_kernel_class_name", "tandem_debug_lt_times", "tandem_test_uniforms", "tandem_test_nucleus", "tandem_test_philox", "tandem_test_gemm", "tandem_test_gemm_time"]
-KC_NUM = 16
+                    "tandem_kernel_class_name", "tandem_test_set_option", "tandem_test_set_page_order", "tandem_test_uniforms", "tandem_test_nucleus", "tandem_test_philox",
+                    "tandem_test_gemm", "tandem_test_gemm_time"]
+KC_NUM = 15
 
 
 class TandemError(RuntimeError):
@@ -102,8 +103,9 @@ def lib():
         L.tandem_test_nucleus.argtypes = [C.c_int32, C.c_float, C.c_float, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.tandem_test_philox.argtypes = [C.POINTER(C.c_uint32), C.POINTER(C.c_uint32), C.POINTER(C.c_uint32)]
         L.tandem_test_gemm.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
-        L.tandem_debug_lt_times.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
-        L.tandem_test_gemm_time.argtypes = [C.c_int32] * 8 + [C.POINTER(C.c_float)]
+        L.tandem_test_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_int32]
+        L.tandem_test_set_page_order.argtypes = [C.c_void_p, C.c_uint64]
+        L.tandem_test_gemm_time.argtypes = [C.c_int32] * 7 + [C.POINTER(C.c_float)]
         _lib = L
     return _lib
 
@@ -247,11 +249,13 @@ class Tandem:
     def set_profile(self, enable):
         self._check(lib().tandem_set_profile(self._h, 1 if enable else 0))
 
-    def debug_lt_times(self):
-        n = (self.config.shape.n_layers + 1) * 32
-        out = np.zeros(n, np.uint64)
-        self._check(lib().tandem_debug_lt_times(self._h, out.ctypes.data, n))
-        return out.reshape(-1, 32)
+    def set_option(self, name, value):
+        """A/B knob for measurements (tandem_test.h: tandem_test_set_option)."""
+        self._check(lib().tandem_test_set_option(self._h, name.encode(), int(value)))
+
+    def set_page_order(self, seed):
+        """Test hook: hand KV pages out in a seeded pseudo-random order from the next reset on (0 = ascending)."""
+        self._check(lib().tandem_test_set_page_order(self._h, int(seed)))
 
     def get_profile(self):
         """dict kernel class name -> (device milliseconds, launches) accumulated while profiling was enabled."""
@@ -321,9 +325,9 @@ def tandem_test_gemm(dtype, impl, A, W, out):
         raise TandemError(rc)
 
 
-def tandem_test_gemm_time(rows, N, K, iters=50, cluster=0, ring_kb=0, splits=0, swiglu=0, pdl=0):
+def tandem_test_gemm_time(rows, N, K, iters=50, ring_kb=0, splits=0, swiglu=0, pdl=0, pair=0):
     ms = C.c_float()
-    rc = lib().tandem_test_gemm_time(rows, N, K, iters, cluster, ring_kb, splits, (1 if swiglu else 0) | (2 if pdl else 0), C.byref(ms))
+    rc = lib().tandem_test_gemm_time(rows, N, K, iters, ring_kb, splits, (1 if swiglu else 0) | (2 if pdl else 0) | (4 if pair else 0), C.byref(ms))
     if rc:
         raise TandemError(rc)
     return ms.value

@@ -16,6 +16,7 @@ struct SchedArgs {
   const int32_t* tokens; int max_seqs, max_seq_len, max_pages, row_cap, tile_tok;
   int32_t* work_ctr; int n_work_ctr;   // dynamic-scheduling counters of the attention launches of this step
   int score;                           // teacher-forced dual scoring (tandem_score): both models ingest every sequence, every row reaches the LM head
+  int32_t* oom_flag;                   // mapped host word, set when a pool runs dry (the host reads it without synchronising)
 };
 
 __device__ __forceinline__ int block_excl_scan_1024(int v, int* total, int* wsum) {
@@ -117,6 +118,7 @@ __global__ void __launch_bounds__(1024) sched_kernel(SchedArgs a) {
           atomicAdd(pt.free_top, k);
           for (int i = 0; i < k; ++i) pt.bt[(size_t)s * a.max_pages + have + i] = 0;
           a.stats->err_oom = 1;
+          if (a.oom_flag) *a.oom_flag = 1;
         }
         pt.npages[s] = need;
       }
@@ -275,7 +277,7 @@ __global__ void __launch_bounds__(1024) finalize_kernel(FinalArgs a) {
           const int pos = atomicAdd(a.pt[M].free_top, n);
           for (int i = 0; i < n; ++i) {
             const int pg = a.pt[M].bt[(size_t)s * a.max_pages + n0 + i];
-            if (pos + i < a.pool_pages) a.pt[M].free_pages[pos + i] = pg;
+            if (pos + i < a.pool_pages) a.pt[M].free_pages[pos + i] = pg;   // after a pool exhaustion entries may name the dummy page 0: the handle then needs tandem_reset (tandem.h)
           }
         }
         a.pt[M].npages[s] = 0; a.pt[M].nshared[s] = 0;
@@ -921,7 +923,7 @@ __global__ void __launch_bounds__(NT) sample_switch_emit_kernel(const __grid_con
   int y = greedy ? raw.i : gum.i;
   if (a.io.forced_tokens) {
     const int f = a.io.forced_tokens[(size_t)s * a.io.forced_stride + (t - 1)];
-    if (f >= 0) y = f;
+    if (f >= 0 && f < V) y = f;   // an id outside the vocabulary is ignored (it would index the logits and the embedding out of bounds)
   }
   const float logp = z[y] * invT - (m + logf(sum));
   const int M = a.model;

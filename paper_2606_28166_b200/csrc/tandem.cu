@@ -2,6 +2,7 @@
 // (S0 scheduler -> S1..S8 for both models, every kernel launched once for the pair -> finalize) and whole-rollout generation. All arithmetic of the path
 // runs in the kernels of this directory; there is no CPU fallback.
 #include "../../include/tandem.h"
+#include "../../include/tandem_test.h"
 
 #include <cuda_runtime.h>
 #include <cuda_bf16.h>
@@ -20,7 +21,6 @@
 #include "attention_mma.cuh"
 #include "gemm_simt.cuh"
 #include "gemm_tcgen05.cuh"
-#include "layer_tail.cuh"
 #include "grpo.cuh"
 
 using namespace tandem;
@@ -68,17 +68,14 @@ struct tandem_handle {
   int esize = 4;
   int row_cap = 0, max_pages = 0, pool_pages = 0, tile_tok = 0, max_items = 0, max_comb = 0, part_cap = 0, gemm_impl = TANDEM_GEMM_SIMT, attn_impl = TANDEM_ATTN_ALU;
   int n_sms = 148;
-  int attn_ctas_per_sm = 2, gemm_ring_kb = 0;   // tuning knobs (env TANDEM_ATTN_CTAS_PER_SM, TANDEM_GEMM_RING_KB; 0 = automatic)
+  // tuning knobs (tandem_test_set_option; the defaults are what every measured number uses)
+  int attn_ctas_per_sm = 2, gemm_ring_kb = 0;   // 0 = automatic ring size
   int gemm_pair = -1;                            // tcgen05 projections as CTA pairs (cta_group::2): -1 = automatic (while scoring: hundreds of
-                                                 // rows per launch, +5%; no gain at the rollout's ~128 rows), 0 / 1 = env TANDEM_GEMM_PAIR
+                                                 // rows per launch, +5%; no gain at the rollout's ~128 rows), 0 / 1 = forced
   bool scoring = false;
   bool score_nosplit = true;
-  int score_chunk_grid = 8;                      // scoring: CTAs per (weight tile, K split) along the token rows (env TANDEM_SCORE_CHUNK_GRID; 1 = off)
-  bool use_tail = false;                        // persistent layer-tail kernel (bf16 + tcgen05 + tensor-core attention; env TANDEM_TAIL=1 enables)
-  LtWMaps* lt_wmaps = nullptr; LtAMaps* lt_amaps = nullptr; bool lt_maps_ready = false;   // device tensor-map tables of the layer-tail kernel
-  unsigned long long* lt_ts = nullptr;          // env TANDEM_LT_DEBUG=1: per-phase timestamps of the layer-tail launches (tandem_debug_lt_times)
-  int32_t* lt_bar = nullptr;                    // grid-barrier counters of the layer-tail launches, zeroed by the scheduler
-  bool use_pdl = true;                          // programmatic dependent launch along each model's kernel chain (env TANDEM_PDL=0 disables)
+  int score_chunk_grid = 8;                      // scoring: CTAs per (weight tile, K split) along the token rows (1 = off)
+  bool use_pdl = true;                          // programmatic dependent launch along the kernel chain
   size_t gemm_out_cols = 0;
   ModelWeights w[2];
   Workspace ws[2];
@@ -91,13 +88,9 @@ struct tandem_handle {
   float2* rope_cs = nullptr;
   uint8_t* word_start_dev = nullptr; std::vector<uint8_t> word_start_host;
   DevStats* stats = nullptr; int32_t* n_active = nullptr; int32_t* work_ctr = nullptr;
+  int32_t* oom_host = nullptr; int32_t* oom_dev = nullptr;   // mapped pinned word the scheduler raises when a page pool runs dry: read by every call without a sync
+  uint64_t page_order_seed = 0;                 // tandem_test_set_page_order: != 0 = pages are handed out in a seeded pseudo-random order
   cudaStream_t gs{}; cudaEvent_t ev_in{}, ev_out{};   // internal stream of the captured step graph and its fork / join events
-  // staggered two-stream mode (forward_pair): the junior's chain runs on gs2, half a layer behind the senior's
-  bool use_stagger = false;
-  cudaStream_t gs2{}; cudaEvent_t ev_fork{}, ev_join{};
-  std::vector<cudaEvent_t> stagger_ev;          // [2 * layer + model]: that model's attention launch of that layer has been issued and is complete
-  int stagger_attn_ctas_per_sm = 1, stagger_ring_kb = 98; bool stagger_events = true, stagger_deep = true;
-  int32_t* zero_counts = nullptr;               // C_NUM zeros: the absent second model of a one-model attention launch
   std::vector<uint8_t> slot_busy;           // host view of the slots
   // prompt-page sharing (cfg.share_prompt_pages): device group table and the host's view of which entries are in use
   GroupTab gt{};
@@ -122,7 +115,6 @@ struct tandem_handle {
 
 namespace {
 
-int build_layer_tail_maps(tandem_handle* h);
 int fail(tandem_handle* h, int code, const std::string& msg) {
   if (h) h->err = msg;
   return code;
@@ -168,7 +160,8 @@ cudaEvent_t prof_event(tandem_handle* h) {
 // read from rows_ptr[m] on the device.
 template <typename T>
 int launch_gemm(tandem_handle* h, int which, const void* const* A, const void* const* W, int N, int K, float* const* out,
-                const int32_t* const* rows_ptr, int rows_cap, int* n_split, size_t* split_stride, cudaStream_t s, int epi = kTcEpiPartial, int nm = 2) {
+                const int32_t* const* rows_ptr, int rows_cap, int* n_split, size_t* split_stride, cudaStream_t s, int epi = kTcEpiPartial) {
+  const int nm = 2;
   *n_split = 1;
   *split_stride = (size_t)rows_cap * N;
   static const int cls_of[5] = {TANDEM_KC_GEMM_QKV, TANDEM_KC_GEMM_O, TANDEM_KC_GEMM_GATEUP, TANDEM_KC_GEMM_DOWN, TANDEM_KC_GEMM_LMHEAD};
@@ -181,11 +174,6 @@ int launch_gemm(tandem_handle* h, int which, const void* const* A, const void* c
       // with >= 4 chunks per weight tile the launch is wide enough without K-splits: a third of the fp32 partials to write and re-read
       if (h->score_nosplit && std::min(tune.chunk_grid, (rows_cap + kTcMaxRows - 1) / kTcMaxRows) >= 4) tune.splits = 1;
     }
-    if (nm == 1) {   // staggered mode: the K-splits of the paired launch (same reduction order, bit-identical results) and a ring that leaves
-                     // room for the other model's attention CTA on the same SM
-      if (which != 4 && epi != kTcEpiSwiGLU) tune.splits = tc_gemm_splits(N, K, 2);
-      if (tune.ring_kb == 0) tune.ring_kb = h->stagger_ring_kb;
-    }
     KL(h, cls_of[which], s, rc = tc_gemm_launch(h->tc, nm, which, A, W, N, K, out, rows_ptr, rows_cap, n_split, split_stride, s, epi, &tune));
     return rc == 0 ? TANDEM_OK : fail(h, rc, "tcgen05 GEMM launch failed (tensor map encode or K % 8 != 0)");
   }
@@ -197,7 +185,8 @@ int launch_gemm(tandem_handle* h, int which, const void* const* A, const void* c
 }
 
 template <typename T>
-void launch_residual_norm(tandem_handle* h, cudaStream_t s, int grid_x, const Pair<ResNormArgs<T>>& a, int nm = 2) {
+void launch_residual_norm(tandem_handle* h, cudaStream_t s, int grid_x, const Pair<ResNormArgs<T>>& a) {
+  const int nm = 2;
   const int v = (a.m[0].H / 4 + 255) / 256;   // float4 per thread; tandem_init guarantees H % 8 == 0 and H <= 8192
   const dim3 grid(grid_x, nm);
   if (v <= 1) KL(h, TANDEM_KC_RESIDUAL_NORM, s, launch_ex(residual_norm_kernel<T, 256, 1>, grid, dim3(256), 0, s, h->use_pdl, a));
@@ -207,21 +196,21 @@ void launch_residual_norm(tandem_handle* h, cudaStream_t s, int grid_x, const Pa
 }
 
 template <typename T, int D, int G>
-void launch_attn_dg(const Pair<AttnArgs<T>>& a, int grid, cudaStream_t s, bool pdl, int nm) {
-  launch_ex(paged_attention_kernel<T, D, G>, dim3(grid, nm), dim3(kAttnThreads), 0, s, pdl, a);
+void launch_attn_dg(const Pair<AttnArgs<T>>& a, int grid, cudaStream_t s, bool pdl) {
+  launch_ex(paged_attention_kernel<T, D, G>, dim3(grid, 2), dim3(kAttnThreads), 0, s, pdl, a);
 }
 template <typename T> struct AttnDispatch;
 template <> struct AttnDispatch<float> {
-  static bool run(const Pair<AttnArgs<float>>& a, int D, int G, int grid, cudaStream_t s, bool pdl, int nm = 2) {
-#define TD_CASE(d, g) if (D == d && G == g) { launch_attn_dg<float, d, g>(a, grid, s, pdl, nm); return true; }
+  static bool run(const Pair<AttnArgs<float>>& a, int D, int G, int grid, cudaStream_t s, bool pdl) {
+#define TD_CASE(d, g) if (D == d && G == g) { launch_attn_dg<float, d, g>(a, grid, s, pdl); return true; }
     TD_CASE(32, 1) TD_CASE(32, 2) TD_CASE(32, 4) TD_CASE(64, 1) TD_CASE(64, 2) TD_CASE(64, 4) TD_CASE(128, 1) TD_CASE(128, 2) TD_CASE(128, 4)
 #undef TD_CASE
     return false;
   }
 };
 template <> struct AttnDispatch<bf16> {
-  static bool run(const Pair<AttnArgs<bf16>>& a, int D, int G, int grid, cudaStream_t s, bool pdl, int nm = 2) {
-#define TD_CASE(d, g) if (D == d && G == g) { launch_attn_dg<bf16, d, g>(a, grid, s, pdl, nm); return true; }
+  static bool run(const Pair<AttnArgs<bf16>>& a, int D, int G, int grid, cudaStream_t s, bool pdl) {
+#define TD_CASE(d, g) if (D == d && G == g) { launch_attn_dg<bf16, d, g>(a, grid, s, pdl); return true; }
     TD_CASE(64, 1) TD_CASE(64, 2) TD_CASE(64, 4) TD_CASE(64, 7) TD_CASE(64, 8) TD_CASE(128, 1) TD_CASE(128, 2) TD_CASE(128, 4) TD_CASE(128, 8)
 #undef TD_CASE
     return false;
@@ -229,20 +218,15 @@ template <> struct AttnDispatch<bf16> {
 };
 template <int D, int G> struct AmStages { static constexpr int value = D == 128 ? 2 : 4; };
 template <int D, int G>
-bool launch_attn_mma_dg(const Pair<CUtensorMap>& map, const Pair<AttnMmaArgs>& a, int grid, cudaStream_t s, bool set_attr, bool pdl, bool deep) {
+bool launch_attn_mma_dg(const Pair<CUtensorMap>& map, const Pair<AttnMmaArgs>& a, int grid, cudaStream_t s, bool set_attr, bool pdl) {
   constexpr int ST = AmStages<D, G>::value;
   constexpr int smem = attn_mma_smem_bytes<D, ST>();
-  // deep = the staggered mode's one-CTA-per-SM launch: a ring of 1.5x the stages (the second CTA slot of the SM belongs to a GEMM CTA)
-  constexpr int STD = ST + ST / 2;
-  constexpr int smem_deep = attn_mma_smem_bytes<D, STD>();
-  if (set_attr) return cudaFuncSetAttribute(paged_attention_mma_kernel<D, G, ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) == cudaSuccess &&
-                       cudaFuncSetAttribute(paged_attention_mma_kernel<D, G, STD>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_deep) == cudaSuccess;
-  if (deep) return launch_ex(paged_attention_mma_kernel<D, G, STD>, dim3(grid), dim3(kAmThreads), smem_deep, s, pdl, map, a) == cudaSuccess;
+  if (set_attr) return cudaFuncSetAttribute(paged_attention_mma_kernel<D, G, ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) == cudaSuccess;
   return launch_ex(paged_attention_mma_kernel<D, G, ST>, dim3(grid), dim3(kAmThreads), smem, s, pdl, map, a) == cudaSuccess;
 }
 // set_attr = true: only raise the kernel's dynamic shared memory limit (called once from tandem_init)
-bool run_attn_mma(const Pair<CUtensorMap>& map, const Pair<AttnMmaArgs>& a, int D, int G, int grid, cudaStream_t s, bool set_attr, bool pdl = false, bool deep = false) {
-#define TD_CASE(d, g) if (D == d && G == g) return launch_attn_mma_dg<d, g>(map, a, grid, s, set_attr, pdl, deep);
+bool run_attn_mma(const Pair<CUtensorMap>& map, const Pair<AttnMmaArgs>& a, int D, int G, int grid, cudaStream_t s, bool set_attr, bool pdl = false) {
+#define TD_CASE(d, g) if (D == d && G == g) return launch_attn_mma_dg<d, g>(map, a, grid, s, set_attr, pdl);
   TD_CASE(64, 1) TD_CASE(64, 2) TD_CASE(64, 4) TD_CASE(64, 7) TD_CASE(64, 8) TD_CASE(128, 1) TD_CASE(128, 2) TD_CASE(128, 4) TD_CASE(128, 8)
 #undef TD_CASE
   return false;
@@ -252,92 +236,15 @@ bool attn_supported(int dtype, int D, int G) {
   return (D == 64 && (G == 1 || G == 2 || G == 4 || G == 7 || G == 8)) || (D == 128 && (G == 1 || G == 2 || G == 4 || G == 8));
 }
 
-// ------------------------------------------------------------------------------------------ persistent layer tail
-// Launch li = 0: QKV + RoPE of layer 0 (after embed_norm). Launch li = l + 1: O .. NORM2 of layer l and, unless l is the last
-// layer, QKV + RoPE of layer l + 1.
-int build_layer_tail_maps(tandem_handle* h) {
-  const tandem_config& c = h->cfg;
-  const int H = c.hidden, nq = c.n_q_heads, nkv = c.n_kv_heads, d = c.head_dim, I = c.intermediate, L = c.n_layers;
-  const int qkv_n = (nq + 2 * nkv) * d;
-  std::vector<LtWMaps> wm(L);
-  LtAMaps am;
-  std::memset(wm.data(), 0, sizeof(LtWMaps) * L); std::memset(&am, 0, sizeof(am));
-  bool ok = true;
-  auto put = [&](CUtensorMap& dst, const void* base, int rows, int K, int box) {
-    const CUtensorMap* mp = tc_gemm_map(h->tc, base, rows, K, box);
-    if (!mp) { ok = false; return; }
-    dst = *mp;
-  };
-  for (int m = 0; m < 2; ++m) {
-    const ModelWeights& w = h->w[m]; Workspace& ws = h->ws[m];
-    for (int l = 0; l < L; ++l)
-      for (int b = 0; b < 2; ++b) {
-        const int box = b == 0 ? 256 : 128;
-        put(wm[l].w[0][m][b], w.wo[l], H, nq * d, box); put(wm[l].w[1][m][b], w.wgu[l], 2 * I, H, box);
-        put(wm[l].w[2][m][b], w.wdown[l], H, I, box);   put(wm[l].w[3][m][b], w.wqkv[l], qkv_n, H, box);
-      }
-    for (int b = 0; b < 4; ++b) {
-      const int box = 128 >> b;
-      put(am.a[0][m][b], ws.attn_out, h->row_cap, nq * d, box); put(am.a[1][m][b], ws.act, h->row_cap, H, box);
-      put(am.a[2][m][b], ws.mlp_act, h->row_cap, I, box);
-    }
-  }
-  if (!ok) return fail(h, TANDEM_ECUDA, "tensor map encode failed (layer tail)");
-  tc_gemm_invalidate(h->tc, 0);   // the per-launch cache is not needed for these
-  if (!h->lt_wmaps) { DM(h, &h->lt_wmaps, sizeof(LtWMaps) * L); DM(h, &h->lt_amaps, sizeof(LtAMaps)); }
-  CU(h, cudaMemcpy(h->lt_wmaps, wm.data(), sizeof(LtWMaps) * L, cudaMemcpyHostToDevice));
-  CU(h, cudaMemcpy(h->lt_amaps, &am, sizeof(am), cudaMemcpyHostToDevice));
-  h->lt_maps_ready = true;
-  return TANDEM_OK;
-}
-
-int launch_layer_tail(tandem_handle* h, int li, cudaStream_t s) {
-  const tandem_config& c = h->cfg;
-  const int H = c.hidden, nq = c.n_q_heads, nkv = c.n_kv_heads, d = c.head_dim, I = c.intermediate, L = c.n_layers;
-  const int qkv_n = (nq + 2 * nkv) * d;
-  const int l = li - 1;                   // layer whose attention output this launch consumes (-1: none)
-  const int ln = li;                      // layer whose QKV / RoPE this launch produces (== L: none)
-  const size_t layer_kv = (size_t)2 * h->pool_pages * nkv * kPageTokens * d;
-  const size_t half_kv = (size_t)h->pool_pages * nkv * kPageTokens * d;
-  LtArgs a{};
-  for (int m = 0; m < 2; ++m) {
-    const ModelWeights& w = h->w[m]; Workspace& ws = h->ws[m]; const StepTab& tb = h->tab[m];
-    LtModel& M = a.m[m];
-    M.counts = tb.counts; M.x = ws.x; M.gemm_out = ws.gemm_out; M.act = (bf16*)ws.act; M.mlp_act = (bf16*)ws.mlp_act; M.lm_in = (bf16*)ws.lm_in;
-    M.row_pos = tb.row_pos; M.row_kvslot = tb.row_kvslot; M.q = (bf16*)ws.q;
-    if (l >= 0) {
-      M.g_mlp = (const bf16*)w.mlp_norm[l];
-      M.g_next = (const bf16*)(l == L - 1 ? w.final_norm : w.attn_norm[l + 1]);
-      M.row_emit = l == L - 1 ? tb.row_emit : nullptr;
-    }
-    if (ln < L) {
-      bf16* kpool = (bf16*)ws.kv + (size_t)ln * layer_kv;
-      M.kpool = kpool; M.vpool = kpool + half_kv;
-    }
-  }
-  a.H = H; a.I = I; a.nq = nq; a.nkv = nkv; a.d = d; a.eps = c.rms_eps; a.rope_cs = h->rope_cs;
-  a.S_o = tc_gemm_splits(H, nq * d, 2); a.S_down = tc_gemm_splits(H, I, 2); a.S_qkv = tc_gemm_splits(qkv_n, H, 2); a.row_cap = h->row_cap;
-  a.bar = h->lt_bar + li * LT_NPHASE;
-  a.dbg_ts = h->lt_ts ? h->lt_ts + (size_t)li * 32 : nullptr;
-  a.wm_l = h->lt_wmaps + (l >= 0 ? l : 0); a.wm_ln = h->lt_wmaps + (ln < L ? ln : 0); a.am = h->lt_amaps;
-  a.phase_mask = (l >= 0 ? (1 << LT_O) | (1 << LT_NORM1) | (1 << LT_GU) | (1 << LT_DOWN) | (1 << LT_NORM2) : 0) |
-                 (ln < L ? (1 << LT_QKV) | (1 << LT_ROPE) : 0);
-  cudaError_t e = cudaSuccess;
-  KL(h, TANDEM_KC_LAYER_TAIL, s, e = launch_ex(layer_tail_kernel, dim3(h->n_sms), dim3(kLtThreads), kLtSmemBytes, s, h->use_pdl, a));
-  return e == cudaSuccess ? TANDEM_OK : fail(h, TANDEM_ECUDA, std::string("layer_tail launch: ") + cudaGetErrorString(e));
-}
-
 // ------------------------------------------------------------------------------------------ both models' forward (S1..S8)
 // Every kernel is launched once for the two models (Pair arguments): the models advance layer by layer in lock-step on
-// one stream, each launch carrying the senior's and the junior's half of the work. s2 != nullptr selects the opt-in staggered
-// mode instead (TANDEM_STAGGER=1: one chain of single-model launches per model, the junior's on s2; same results, measured
-// slower - DESIGN.md section 9).
+// one stream, each launch carrying the senior's and the junior's half of the work.
 template <typename T>
-int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaStream_t s, bool score = false, float score_inv_t = 1.f, cudaStream_t s2 = nullptr) {
+int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaStream_t s, bool score = false, float score_inv_t = 1.f) {
   const tandem_config& c = h->cfg;
   const int H = c.hidden, nq = c.n_q_heads, nkv = c.n_kv_heads, d = c.head_dim, I = c.intermediate, V = c.vocab;
   const int qkv_n = (nq + 2 * nkv) * d;
-  const int row_grid = 148 * 2;
+  const int row_grid = h->n_sms * 2;
   const size_t layer_kv = (size_t)2 * h->pool_pages * nkv * kPageTokens * d;
   const size_t half_kv = (size_t)h->pool_pages * nkv * kPageTokens * d;
   const bool mma = h->attn_impl == TANDEM_ATTN_MMA;
@@ -352,176 +259,90 @@ int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaS
     KL(h, TANDEM_KC_EMBED, s, launch_ex(embed_norm_kernel<T, 256>, dim3(row_grid, 2), dim3(256), 0, s, false, ea));
   }
 
-  // The chain of a layer in three parts and the head, each launched for the models m0 .. m0 + nm - 1 on stream st:
-  // nm = 2 is one launch for both models (Pair arguments, the model is a grid dimension), nm = 1 a launch for one model
-  // (the staggered two-stream mode of launch_step). Entry i >= nm of a Pair is never indexed by a grid of nm models;
-  // the attention kernel's shared unit space sees a zero item count for it.
-  auto mi = [](int i, int m0, int nm) { return i < nm ? m0 + i : m0; };
-  auto pre_attn = [&](int l, int m0, int nm, cudaStream_t st) -> int {
-    int ns; size_t ss; int rc;
+  for (int l = 0; l < c.n_layers; ++l) {
     // S3 QKV projection
-    for (int i = 0; i < 2; ++i) { const int m = mi(i, m0, nm); set_gemm(i, h->ws[m].act, h->w[m].wqkv[l], h->ws[m].gemm_out, h->tab[m].counts + C_ROWS); }
-    if ((rc = launch_gemm<T>(h, 0, A, W, qkv_n, H, O, RP, h->row_cap, &ns, &ss, st, kTcEpiPartial, nm))) return rc;
+    for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].act, h->w[m].wqkv[l], h->ws[m].gemm_out, h->tab[m].counts + C_ROWS);
+    if ((rc = launch_gemm<T>(h, 0, A, W, qkv_n, H, O, RP, h->row_cap, &ns, &ss, s))) return rc;
     // S4 RoPE + KV append
     if (mma) {
       Pair<RopeArgs<T, bf16>> ra;
-      for (int i = 0; i < 2; ++i) {
-        const int m = mi(i, m0, nm);
+      for (int m = 0; m < 2; ++m) {
         T* kpool = (T*)h->ws[m].kv + (size_t)l * layer_kv;
-        ra.m[i] = RopeArgs<T, bf16>{h->tab[m].counts, h->tab[m].row_pos, h->tab[m].row_kvslot, h->ws[m].gemm_out, ns, ss, h->rope_cs, (bf16*)h->ws[m].q, kpool, kpool + half_kv, nq, nkv, d};
+        ra.m[m] = RopeArgs<T, bf16>{h->tab[m].counts, h->tab[m].row_pos, h->tab[m].row_kvslot, h->ws[m].gemm_out, ns, ss, h->rope_cs, (bf16*)h->ws[m].q, kpool, kpool + half_kv, nq, nkv, d};
       }
-      KL(h, TANDEM_KC_ROPE_APPEND, st, launch_ex(rope_append_kernel<T, bf16, 256>, dim3(row_grid * 4, nm), dim3(256), 0, st, pdl, ra));
+      KL(h, TANDEM_KC_ROPE_APPEND, s, launch_ex(rope_append_kernel<T, bf16, 256>, dim3(row_grid * 4, 2), dim3(256), 0, s, pdl, ra));
     } else {
       Pair<RopeArgs<T, float>> ra;
-      for (int i = 0; i < 2; ++i) {
-        const int m = mi(i, m0, nm);
+      for (int m = 0; m < 2; ++m) {
         T* kpool = (T*)h->ws[m].kv + (size_t)l * layer_kv;
-        ra.m[i] = RopeArgs<T, float>{h->tab[m].counts, h->tab[m].row_pos, h->tab[m].row_kvslot, h->ws[m].gemm_out, ns, ss, h->rope_cs, (float*)h->ws[m].q, kpool, kpool + half_kv, nq, nkv, d};
+        ra.m[m] = RopeArgs<T, float>{h->tab[m].counts, h->tab[m].row_pos, h->tab[m].row_kvslot, h->ws[m].gemm_out, ns, ss, h->rope_cs, (float*)h->ws[m].q, kpool, kpool + half_kv, nq, nkv, d};
       }
-      KL(h, TANDEM_KC_ROPE_APPEND, st, launch_ex(rope_append_kernel<T, float, 256>, dim3(row_grid * 4, nm), dim3(256), 0, st, pdl, ra));
+      KL(h, TANDEM_KC_ROPE_APPEND, s, launch_ex(rope_append_kernel<T, float, 256>, dim3(row_grid * 4, 2), dim3(256), 0, s, pdl, ra));
     }
-    return TANDEM_OK;
-  };
-  // S5 attention (decode splits + catch-up rows); apdl = false when the launch also waits on another stream's event
-  auto attention = [&](int l, int m0, int nm, cudaStream_t st, bool apdl) -> int {
-    bool ok = true;
-    if (mma) {
-      const long long rows_per_half = (long long)h->pool_pages * nkv * kPageTokens;
-      Pair<AttnMmaArgs> ma; Pair<CUtensorMap> maps;
-      for (int i = 0; i < 2; ++i) {
-        const int m = mi(i, m0, nm);
-        const StepTab& tb = h->tab[m];
-        // one work counter per (layer, launch): the staggered mode's second model takes the counters past the first L
-        ma.m[i] = AttnMmaArgs{i < nm ? tb.counts : h->zero_counts, tb.item_row0, tb.item_ntok, tb.item_kv0, tb.item_kv1, tb.item_part, tb.row_slot, tb.row_pos, h->pt[m].bt, h->max_pages,
-                              (const bf16*)h->ws[m].q, (bf16*)h->ws[m].attn_out, h->ws[m].part_acc, h->ws[m].part_ml, nq, nkv, 1.0f / sqrtf((float)d),
-                              (int)((2ll * l) * rows_per_half), (int)((2ll * l + 1) * rows_per_half), h->work_ctr + l + (nm == 1 && m0 == 1 ? c.n_layers : 0)};
-        maps.m[i] = h->kv_map_store[m];
+    // S5 attention (decode splits + catch-up rows)
+    {
+      bool ok = true;
+      if (mma) {
+        const long long rows_per_half = (long long)h->pool_pages * nkv * kPageTokens;
+        Pair<AttnMmaArgs> ma; Pair<CUtensorMap> maps;
+        for (int m = 0; m < 2; ++m) {
+          const StepTab& tb = h->tab[m];
+          ma.m[m] = AttnMmaArgs{tb.counts, tb.item_row0, tb.item_ntok, tb.item_kv0, tb.item_kv1, tb.item_part, tb.row_slot, tb.row_pos, h->pt[m].bt, h->max_pages,
+                                (const bf16*)h->ws[m].q, (bf16*)h->ws[m].attn_out, h->ws[m].part_acc, h->ws[m].part_ml, nq, nkv, 1.0f / sqrtf((float)d),
+                                (int)((2ll * l) * rows_per_half), (int)((2ll * l + 1) * rows_per_half), h->work_ctr + l};
+          maps.m[m] = h->kv_map_store[m];
+        }
+        KL(h, TANDEM_KC_ATTENTION, s, ok = run_attn_mma(maps, ma, d, nq / nkv, h->attn_ctas_per_sm * h->n_sms, s, false, pdl));
+      } else {
+        Pair<AttnArgs<T>> aa;
+        for (int m = 0; m < 2; ++m) {
+          const StepTab& tb = h->tab[m];
+          T* kpool = (T*)h->ws[m].kv + (size_t)l * layer_kv;
+          aa.m[m] = AttnArgs<T>{tb.counts, tb.item_row0, tb.item_ntok, tb.item_kv0, tb.item_kv1, tb.item_part, tb.row_slot, tb.row_pos, h->pt[m].bt, h->max_pages,
+                                (const float*)h->ws[m].q, kpool, kpool + half_kv, (T*)h->ws[m].attn_out, h->ws[m].part_acc, h->ws[m].part_ml, nq, nkv, 1.0f / sqrtf((float)d)};
+        }
+        KL(h, TANDEM_KC_ATTENTION, s, ok = AttnDispatch<T>::run(aa, d, nq / nkv, h->n_sms * 2, s, pdl));
       }
-      const int ctas = (nm == 1 ? h->stagger_attn_ctas_per_sm : h->attn_ctas_per_sm) * h->n_sms;
-      KL(h, TANDEM_KC_ATTENTION, st, ok = run_attn_mma(maps, ma, d, nq / nkv, ctas, st, false, apdl, nm == 1 && h->stagger_attn_ctas_per_sm == 1 && h->stagger_deep));
-    } else {
-      Pair<AttnArgs<T>> aa;
-      for (int i = 0; i < 2; ++i) {
-        const int m = mi(i, m0, nm);
-        const StepTab& tb = h->tab[m];
-        T* kpool = (T*)h->ws[m].kv + (size_t)l * layer_kv;
-        aa.m[i] = AttnArgs<T>{tb.counts, tb.item_row0, tb.item_ntok, tb.item_kv0, tb.item_kv1, tb.item_part, tb.row_slot, tb.row_pos, h->pt[m].bt, h->max_pages,
-                              (const float*)h->ws[m].q, kpool, kpool + half_kv, (T*)h->ws[m].attn_out, h->ws[m].part_acc, h->ws[m].part_ml, nq, nkv, 1.0f / sqrtf((float)d)};
-      }
-      KL(h, TANDEM_KC_ATTENTION, st, ok = AttnDispatch<T>::run(aa, d, nq / nkv, 148 * 2, st, apdl, nm));
+      if (!ok) return fail(h, TANDEM_EINVAL, "unsupported (head_dim, group) for attention");
     }
-    if (!ok) return fail(h, TANDEM_EINVAL, "unsupported (head_dim, group) for attention");
-    return TANDEM_OK;
-  };
-  auto post_attn = [&](int l, int m0, int nm, cudaStream_t st) -> int {
-    int ns; size_t ss; int rc;
     {
       Pair<CombineArgs<T>> ca;
-      for (int i = 0; i < 2; ++i) {
-        const int m = mi(i, m0, nm);
+      for (int m = 0; m < 2; ++m) {
         const StepTab& tb = h->tab[m];
-        ca.m[i] = CombineArgs<T>{tb.counts, tb.comb_row, tb.comb_part0, tb.comb_n, tb.comb_stride, h->ws[m].part_acc, h->ws[m].part_ml, (T*)h->ws[m].attn_out, nq, d};
+        ca.m[m] = CombineArgs<T>{tb.counts, tb.comb_row, tb.comb_part0, tb.comb_n, tb.comb_stride, h->ws[m].part_acc, h->ws[m].part_ml, (T*)h->ws[m].attn_out, nq, d};
       }
-      KL(h, TANDEM_KC_ATTN_COMBINE, st, launch_ex(attn_combine_kernel<T>, dim3(148 * 4, nm), dim3(256), 0, st, pdl, ca));
+      KL(h, TANDEM_KC_ATTN_COMBINE, s, launch_ex(attn_combine_kernel<T>, dim3(h->n_sms * 4, 2), dim3(256), 0, s, pdl, ca));
     }
     // S6 O projection + residual + RMSNorm(mlp)
-    for (int i = 0; i < 2; ++i) { const int m = mi(i, m0, nm); set_gemm(i, h->ws[m].attn_out, h->w[m].wo[l], h->ws[m].gemm_out, h->tab[m].counts + C_ROWS); }
-    if ((rc = launch_gemm<T>(h, 1, A, W, H, nq * d, O, RP, h->row_cap, &ns, &ss, st, kTcEpiPartial, nm))) return rc;
+    for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].attn_out, h->w[m].wo[l], h->ws[m].gemm_out, h->tab[m].counts + C_ROWS);
+    if ((rc = launch_gemm<T>(h, 1, A, W, H, nq * d, O, RP, h->row_cap, &ns, &ss, s))) return rc;
     {
       Pair<ResNormArgs<T>> na;
-      for (int i = 0; i < 2; ++i) {
-        const int m = mi(i, m0, nm);
-        na.m[i] = ResNormArgs<T>{h->tab[m].counts, h->ws[m].gemm_out, ns, ss, h->ws[m].x, (const T*)h->w[m].mlp_norm[l], (T*)h->ws[m].act, nullptr, H, c.rms_eps};
-      }
-      launch_residual_norm<T>(h, st, row_grid, na, nm);
+      for (int m = 0; m < 2; ++m)
+        na.m[m] = ResNormArgs<T>{h->tab[m].counts, h->ws[m].gemm_out, ns, ss, h->ws[m].x, (const T*)h->w[m].mlp_norm[l], (T*)h->ws[m].act, nullptr, H, c.rms_eps};
+      launch_residual_norm<T>(h, s, row_grid, na);
     }
     // S7 gate/up + SwiGLU, down + residual + RMSNorm(next layer | final)
     if (h->gemm_impl == TANDEM_GEMM_TCGEN05) {   // SwiGLU in the GEMM epilogue (gate/up rows interleaved at load time)
-      for (int i = 0; i < 2; ++i) { const int m = mi(i, m0, nm); set_gemm(i, h->ws[m].act, h->w[m].wgu[l], (float*)h->ws[m].mlp_act, h->tab[m].counts + C_ROWS); }
-      if ((rc = launch_gemm<T>(h, 2, A, W, 2 * I, H, O, RP, h->row_cap, &ns, &ss, st, kTcEpiSwiGLU, nm))) return rc;
+      for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].act, h->w[m].wgu[l], (float*)h->ws[m].mlp_act, h->tab[m].counts + C_ROWS);
+      if ((rc = launch_gemm<T>(h, 2, A, W, 2 * I, H, O, RP, h->row_cap, &ns, &ss, s, kTcEpiSwiGLU))) return rc;
     } else {
-      for (int i = 0; i < 2; ++i) { const int m = mi(i, m0, nm); set_gemm(i, h->ws[m].act, h->w[m].wgu[l], h->ws[m].gemm_out, h->tab[m].counts + C_ROWS); }
-      if ((rc = launch_gemm<T>(h, 2, A, W, 2 * I, H, O, RP, h->row_cap, &ns, &ss, st, kTcEpiPartial, nm))) return rc;
+      for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].act, h->w[m].wgu[l], h->ws[m].gemm_out, h->tab[m].counts + C_ROWS);
+      if ((rc = launch_gemm<T>(h, 2, A, W, 2 * I, H, O, RP, h->row_cap, &ns, &ss, s))) return rc;
       Pair<SwigluArgs<T>> sg;
-      for (int i = 0; i < 2; ++i) { const int m = mi(i, m0, nm); sg.m[i] = SwigluArgs<T>{h->tab[m].counts, h->ws[m].gemm_out, ns, ss, (T*)h->ws[m].mlp_act, I}; }
-      KL(h, TANDEM_KC_SWIGLU, st, launch_ex(swiglu_kernel<T, 256>, dim3(row_grid, nm), dim3(256), 0, st, pdl, sg));
+      for (int m = 0; m < 2; ++m) sg.m[m] = SwigluArgs<T>{h->tab[m].counts, h->ws[m].gemm_out, ns, ss, (T*)h->ws[m].mlp_act, I};
+      KL(h, TANDEM_KC_SWIGLU, s, launch_ex(swiglu_kernel<T, 256>, dim3(row_grid, 2), dim3(256), 0, s, pdl, sg));
     }
-    for (int i = 0; i < 2; ++i) { const int m = mi(i, m0, nm); set_gemm(i, h->ws[m].mlp_act, h->w[m].wdown[l], h->ws[m].gemm_out, h->tab[m].counts + C_ROWS); }
-    if ((rc = launch_gemm<T>(h, 3, A, W, H, I, O, RP, h->row_cap, &ns, &ss, st, kTcEpiPartial, nm))) return rc;
+    for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].mlp_act, h->w[m].wdown[l], h->ws[m].gemm_out, h->tab[m].counts + C_ROWS);
+    if ((rc = launch_gemm<T>(h, 3, A, W, H, I, O, RP, h->row_cap, &ns, &ss, s))) return rc;
     const bool last = l == c.n_layers - 1;
     {
       Pair<ResNormArgs<T>> na;
-      for (int i = 0; i < 2; ++i) {
-        const int m = mi(i, m0, nm);
-        na.m[i] = ResNormArgs<T>{h->tab[m].counts, h->ws[m].gemm_out, ns, ss, h->ws[m].x, (const T*)(last ? h->w[m].final_norm : h->w[m].attn_norm[l + 1]),
+      for (int m = 0; m < 2; ++m)
+        na.m[m] = ResNormArgs<T>{h->tab[m].counts, h->ws[m].gemm_out, ns, ss, h->ws[m].x, (const T*)(last ? h->w[m].final_norm : h->w[m].attn_norm[l + 1]),
                                  (T*)(last ? (score ? h->ws[m].score_lm_in : h->ws[m].lm_in) : h->ws[m].act), last ? h->tab[m].row_emit : nullptr, H, c.rms_eps};
-      }
-      launch_residual_norm<T>(h, st, row_grid, na, nm);
+      launch_residual_norm<T>(h, s, row_grid, na);
     }
-    return TANDEM_OK;
-  };
-  // S8 LM head on the emitting rows only, then sample + switch + emit
-  auto head = [&](int m0, int nm, cudaStream_t st) -> int {
-    int ns; size_t ss; int rc;
-    for (int i = 0; i < 2; ++i) { const int m = mi(i, m0, nm); set_gemm(i, h->ws[m].lm_in, h->w[m].lm_head, h->ws[m].logits, h->tab[m].counts + C_EMIT); }
-    if ((rc = launch_gemm<T>(h, 4, A, W, V, H, O, RP, c.max_seqs, &ns, &ss, st, kTcEpiPartial, nm))) return rc;
-    Pair<SampleArgs> sa;
-    const int n_chunk = std::max(1, std::min(kSampleMaxChunks, V / 8192));   // ~8k ids per CTA: 18 slices at V = 151,936
-    for (int i = 0; i < 2; ++i) {
-      const int m = mi(i, m0, nm);
-      sa.m[i] = SampleArgs{h->st, h->tab[m], io, rp, h->ws[m].logits, h->word_start_dev, h->tokens, h->out_owner, h->out_logp, V, c.max_seq_len, m,
-                           h->ws[m].chunk_part, h->ws[m].chunk_ctr, n_chunk};
-    }
-    const size_t nucleus_smem = (rp.temperature > 0.f && (rp.top_p < 1.f || (rp.top_k > 0 && rp.top_k < V))) ? sizeof(NucleusSmem<256>) : 0;
-    if (nucleus_smem) KL(h, TANDEM_KC_SAMPLE, st, launch_ex(sample_switch_emit_kernel<256, true>, dim3(c.max_seqs, n_chunk, nm), dim3(256), nucleus_smem, st, pdl, sa));
-    else KL(h, TANDEM_KC_SAMPLE, st, launch_ex(sample_switch_emit_kernel<256, false>, dim3(c.max_seqs, n_chunk, nm), dim3(256), 0, st, pdl, sa));
-    return TANDEM_OK;
-  };
-
-  if (s2) {
-    // Staggered mode: one chain per model on its own stream, offset by half a layer. A model's attention (pure KV streaming,
-    // one CTA per SM) runs while the other model's projections (weight streaming with exposed prologues and epilogues) occupy
-    // the second CTA slot of every SM; events order the attention launches senior(l), junior(l), senior(l+1), ... so the two
-    // chains cannot drift into phase. The caller forked s2 from s after the scheduler and joins it before finalize.
-    cudaStream_t sm[2] = {s, s2};
-    const bool ev = s2 != s;   // profile mode passes s2 == s: same launches, serialised on one stream
-    if (ev) { CU(h, cudaEventRecord(h->ev_fork, s)); CU(h, cudaStreamWaitEvent(s2, h->ev_fork, 0)); }
-    for (int l = 0; l < c.n_layers; ++l)
-      for (int m = 0; m < 2; ++m) {
-        if ((rc = pre_attn(l, m, 1, sm[m]))) return rc;
-        const bool wait = ev && h->stagger_events && (m == 1 || l > 0);
-        if (wait) CU(h, cudaStreamWaitEvent(sm[m], h->stagger_ev[m == 1 ? 2 * l : 2 * (l - 1) + 1], 0));
-        if ((rc = attention(l, m, 1, sm[m], pdl && !wait))) return rc;
-        if (ev && h->stagger_events) CU(h, cudaEventRecord(h->stagger_ev[2 * l + m], sm[m]));
-        if ((rc = post_attn(l, m, 1, sm[m]))) return rc;
-      }
-    for (int m = 0; m < 2; ++m) if ((rc = head(m, 1, sm[m]))) return rc;
-    if (ev) { CU(h, cudaEventRecord(h->ev_join, s2)); CU(h, cudaStreamWaitEvent(s, h->ev_join, 0)); }
-    return TANDEM_OK;
-  }
-
-  const bool tail = h->use_tail && sizeof(T) == 2 && !score;
-  if (tail && (rc = launch_layer_tail(h, 0, s))) return rc;
-  for (int l = 0; l < c.n_layers; ++l) {
-    if (tail) {   // attention + combine, then everything up to the next attention in one persistent kernel
-      const long long rows_per_half = (long long)h->pool_pages * nkv * kPageTokens;
-      Pair<AttnMmaArgs> ma; Pair<CUtensorMap> kmaps; Pair<CombineArgs<T>> ca;
-      for (int m = 0; m < 2; ++m) {
-        const StepTab& tb = h->tab[m];
-        ma.m[m] = AttnMmaArgs{tb.counts, tb.item_row0, tb.item_ntok, tb.item_kv0, tb.item_kv1, tb.item_part, tb.row_slot, tb.row_pos, h->pt[m].bt, h->max_pages,
-                              (const bf16*)h->ws[m].q, (bf16*)h->ws[m].attn_out, h->ws[m].part_acc, h->ws[m].part_ml, nq, nkv, 1.0f / sqrtf((float)d),
-                              (int)((2ll * l) * rows_per_half), (int)((2ll * l + 1) * rows_per_half), h->work_ctr + l};
-        kmaps.m[m] = h->kv_map_store[m];
-        ca.m[m] = CombineArgs<T>{tb.counts, tb.comb_row, tb.comb_part0, tb.comb_n, tb.comb_stride, h->ws[m].part_acc, h->ws[m].part_ml, (T*)h->ws[m].attn_out, nq, d};
-      }
-      bool ok = true;
-      KL(h, TANDEM_KC_ATTENTION, s, ok = run_attn_mma(kmaps, ma, d, nq / nkv, h->attn_ctas_per_sm * h->n_sms, s, false, pdl));
-      if (!ok) return fail(h, TANDEM_EINVAL, "unsupported (head_dim, group) for attention");
-      KL(h, TANDEM_KC_ATTN_COMBINE, s, launch_ex(attn_combine_kernel<T>, dim3(148 * 4, 2), dim3(256), 0, s, pdl, ca));
-      if ((rc = launch_layer_tail(h, l + 1, s))) return rc;
-      continue;
-    }
-    if ((rc = pre_attn(l, 0, 2, s)) || (rc = attention(l, 0, 2, s, pdl)) || (rc = post_attn(l, 0, 2, s))) return rc;
   }
   if (score) {   // every row reaches the LM head (the scheduler set row_emit[r] = r); the dual-scoring kernel replaces the sampler
     for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].score_lm_in, h->w[m].lm_head, h->ws[m].score_logits, h->tab[m].counts + C_EMIT);
@@ -531,7 +352,18 @@ int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaS
     KL(h, TANDEM_KC_SCORE, s, launch_ex(score_kernel<512>, dim3(h->row_cap), dim3(512), 0, s, pdl, sc));
     return TANDEM_OK;
   }
-  return head(0, 2, s);
+  // S8 LM head on the emitting rows only, then sample + switch + emit
+  for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].lm_in, h->w[m].lm_head, h->ws[m].logits, h->tab[m].counts + C_EMIT);
+  if ((rc = launch_gemm<T>(h, 4, A, W, V, H, O, RP, c.max_seqs, &ns, &ss, s))) return rc;
+  Pair<SampleArgs> sa;
+  const int n_chunk = std::max(1, std::min(kSampleMaxChunks, V / 8192));   // ~8k ids per CTA: 18 slices at V = 151,936
+  for (int m = 0; m < 2; ++m)
+    sa.m[m] = SampleArgs{h->st, h->tab[m], io, rp, h->ws[m].logits, h->word_start_dev, h->tokens, h->out_owner, h->out_logp, V, c.max_seq_len, m,
+                         h->ws[m].chunk_part, h->ws[m].chunk_ctr, n_chunk};
+  const size_t nucleus_smem = (rp.temperature > 0.f && (rp.top_p < 1.f || (rp.top_k > 0 && rp.top_k < V))) ? sizeof(NucleusSmem<256>) : 0;
+  if (nucleus_smem) KL(h, TANDEM_KC_SAMPLE, s, launch_ex(sample_switch_emit_kernel<256, true>, dim3(c.max_seqs, n_chunk, 2), dim3(256), nucleus_smem, s, pdl, sa));
+  else KL(h, TANDEM_KC_SAMPLE, s, launch_ex(sample_switch_emit_kernel<256, false>, dim3(c.max_seqs, n_chunk, 2), dim3(256), 0, s, pdl, sa));
+  return TANDEM_OK;
 }
 
 int launch_step(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaStream_t s, bool score = false, float score_inv_t = 1.f) {
@@ -540,12 +372,10 @@ int launch_step(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaSt
   sa.st = h->st; sa.pt[0] = h->pt[0]; sa.pt[1] = h->pt[1]; sa.gt = h->gt; sa.tab[0] = h->tab[0]; sa.tab[1] = h->tab[1];
   sa.io = io; sa.stats = h->stats; sa.tokens = h->tokens; sa.max_seqs = c.max_seqs; sa.max_seq_len = c.max_seq_len;
   sa.max_pages = h->max_pages; sa.row_cap = h->row_cap; sa.tile_tok = h->tile_tok;
-  sa.work_ctr = h->work_ctr; sa.n_work_ctr = c.n_layers + (c.n_layers + 1) * LT_NPHASE;
-  sa.score = score ? 1 : 0;
+  sa.work_ctr = h->work_ctr; sa.n_work_ctr = c.n_layers;
+  sa.score = score ? 1 : 0; sa.oom_flag = h->oom_dev;
   KL(h, TANDEM_KC_SCHED, s, (sched_kernel<<<1, 1024, 0, s>>>(sa)));
-  // staggered mode: the junior's chain on the second internal stream (profile mode: same launches, serialised on s)
-  cudaStream_t s2 = (h->use_stagger && !score) ? (h->profile ? s : h->gs2) : nullptr;
-  const int rc = (c.dtype == TANDEM_F32) ? forward_pair<float>(h, io, rp, s, score, score_inv_t, s2) : forward_pair<bf16>(h, io, rp, s, score, score_inv_t, s2);
+  const int rc = (c.dtype == TANDEM_F32) ? forward_pair<float>(h, io, rp, s, score, score_inv_t) : forward_pair<bf16>(h, io, rp, s, score, score_inv_t);
   if (rc) return rc;
   FinalArgs fa{h->st, {h->pt[0], h->pt[1]}, h->gt, io, h->stats, h->n_active, c.max_seqs, h->max_pages, h->pool_pages};
   KL(h, TANDEM_KC_FINALIZE, s, (finalize_kernel<<<1, 1024, 0, s>>>(fa)));
@@ -734,7 +564,19 @@ int check_ready(tandem_handle* h) {
   if (!h) return TANDEM_EINVAL;
   if (h->cuda_fault) return fail(h, TANDEM_ECUDA, "a previous CUDA error is sticky: " + h->err);
   if (!h->w[0].loaded || !h->w[1].loaded) return fail(h, TANDEM_ESTATE, "weights of both models must be loaded first");
-  if (h->use_tail && !h->lt_maps_ready) return build_layer_tail_maps(h);
+  return TANDEM_OK;
+}
+
+struct EventPair {   // timing events of tandem_generate / tandem_score, destroyed on every exit path
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  ~EventPair() { if (e0) cudaEventDestroy(e0); if (e1) cudaEventDestroy(e1); }
+};
+
+// KV-pool exhaustion seen by the scheduler of an earlier step (mapped host word, no synchronisation): sticky until tandem_reset
+int check_oom_flag(tandem_handle* h) {
+  if (h->oom_host && *(volatile int32_t*)h->oom_host)
+    return fail(h, TANDEM_ENOMEM, "KV page pool exhausted during generation (results of the starved sequences are invalid); tandem_reset the handle, "
+                                  "then enlarge kv_bytes_per_model or lower max_seqs");
   return TANDEM_OK;
 }
 
@@ -742,7 +584,8 @@ int check_oom(tandem_handle* h, cudaStream_t s) {
   DevStats st;
   CU(h, cudaStreamSynchronize(s));
   CU(h, cudaMemcpy(&st, h->stats, sizeof(st), cudaMemcpyDeviceToHost));
-  if (st.err_oom) return fail(h, TANDEM_ENOMEM, "KV page pool exhausted during generation (results invalid); enlarge kv_bytes_per_model or lower max_seqs");
+  if (st.err_oom) return fail(h, TANDEM_ENOMEM, "KV page pool exhausted during generation (results of the starved sequences are invalid); tandem_reset the handle, "
+                                                "then enlarge kv_bytes_per_model or lower max_seqs");
   return TANDEM_OK;
 }
 
@@ -810,9 +653,10 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
   INIT_TRY(dmalloc(h, &h->word_start_dev, (size_t)V));
   INIT_TRY(dmalloc(h, &h->stats, sizeof(DevStats)));
   INIT_CU(cudaMemset(h->stats, 0, sizeof(DevStats)));
-  INIT_TRY(dmalloc(h, &h->work_ctr, (size_t)(c.n_layers + (c.n_layers + 1) * LT_NPHASE) * 4));
-  h->lt_bar = h->work_ctr + c.n_layers;
-  if (getenv("TANDEM_LT_DEBUG")) { INIT_TRY(dmalloc(h, &h->lt_ts, (size_t)(c.n_layers + 1) * 32 * 8)); INIT_CU(cudaMemset(h->lt_ts, 0, (size_t)(c.n_layers + 1) * 32 * 8)); }
+  INIT_TRY(dmalloc(h, &h->work_ctr, (size_t)c.n_layers * 4));
+  INIT_CU(cudaHostAlloc((void**)&h->oom_host, 4, cudaHostAllocMapped));
+  *h->oom_host = 0;
+  INIT_CU(cudaHostGetDevicePointer((void**)&h->oom_dev, h->oom_host, 0));
   INIT_TRY(dmalloc(h, &h->n_active, 4));
   INIT_CU(cudaMemset(h->n_active, 0, 4));
   INIT_TRY(dmalloc(h, &h->stage_off, (size_t)(S + 1) * sizeof(long long)));
@@ -896,28 +740,6 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
   INIT_CU(cudaEventCreateWithFlags(&h->ev_in, cudaEventDisableTiming));
   INIT_CU(cudaEventCreateWithFlags(&h->ev_out, cudaEventDisableTiming));
   INIT_CU(cudaStreamCreateWithFlags(&h->gs, cudaStreamNonBlocking));
-  INIT_CU(cudaStreamCreateWithFlags(&h->gs2, cudaStreamNonBlocking));
-  INIT_CU(cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));
-  INIT_CU(cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming));
-  for (int i = 0; i < 2 * c.n_layers; ++i) { cudaEvent_t e; INIT_CU(cudaEventCreateWithFlags(&e, cudaEventDisableTiming)); h->stagger_ev.push_back(e); }
-  INIT_TRY(dmalloc(h, &h->zero_counts, (size_t)C_NUM * 4));
-  INIT_CU(cudaMemset(h->zero_counts, 0, (size_t)C_NUM * 4));
-  if (const char* e = getenv("TANDEM_STAGGER")) h->use_stagger = atoi(e) != 0;
-  if (const char* e = getenv("TANDEM_STAGGER_ATTN_CTAS")) h->stagger_attn_ctas_per_sm = std::max(1, std::min(2, atoi(e)));
-  if (const char* e = getenv("TANDEM_STAGGER_EVENTS")) h->stagger_events = atoi(e) != 0;
-  if (const char* e = getenv("TANDEM_STAGGER_DEEP")) h->stagger_deep = atoi(e) != 0;
-  if (const char* e = getenv("TANDEM_STAGGER_RING_KB")) h->stagger_ring_kb = std::max(32, std::min(200, atoi(e)));
-  if (const char* e = getenv("TANDEM_ATTN_CTAS_PER_SM")) h->attn_ctas_per_sm = std::max(1, std::min(2, atoi(e)));
-  if (const char* e = getenv("TANDEM_PDL")) h->use_pdl = atoi(e) != 0;
-  // The persistent layer-tail kernel (layer_tail.cuh) is correct and tested but, at 157 us per layer against ~150 us for the
-  // PDL-chained separate kernels, not yet faster: opt-in with TANDEM_TAIL=1.
-  h->use_tail = false;
-  if (const char* e = getenv("TANDEM_TAIL"))
-    h->use_tail = atoi(e) != 0 && c.dtype == TANDEM_BF16 && h->gemm_impl == TANDEM_GEMM_TCGEN05 && h->attn_impl == TANDEM_ATTN_MMA;
-  if (const char* e = getenv("TANDEM_GEMM_RING_KB")) h->gemm_ring_kb = std::max(0, std::min(200, atoi(e)));
-  if (const char* e = getenv("TANDEM_SCORE_NOSPLIT")) h->score_nosplit = atoi(e) != 0;
-  if (const char* e = getenv("TANDEM_SCORE_CHUNK_GRID")) h->score_chunk_grid = std::max(1, std::min(16, atoi(e)));
-  if (const char* e = getenv("TANDEM_GEMM_PAIR")) h->gemm_pair = atoi(e) != 0 ? 1 : 0;
   {
     int dev_sms = 0;
     if (cudaDeviceGetAttribute(&dev_sms, cudaDevAttrMultiProcessorCount, c.device) == cudaSuccess && dev_sms > 0) h->n_sms = dev_sms;
@@ -928,9 +750,6 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
   }
   if (cudaFuncSetAttribute(sample_switch_emit_kernel<256, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(NucleusSmem<256>)) != cudaSuccess)
     return bad("cannot reserve shared memory for the nucleus sampler");
-  if (h->use_tail && cudaFuncSetAttribute(layer_tail_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kLtSmemBytes) != cudaSuccess) {
-    cudaGetLastError(); h->use_tail = false;
-  }
   if (h->attn_impl == TANDEM_ATTN_MMA) {
     const long long total_rows = 2ll * c.n_layers * h->pool_pages * nkv * kPageTokens;
     if (total_rows >= (1ll << 31)) return bad("KV pool too large for the attention tensor map (2^31 rows)");
@@ -959,8 +778,14 @@ int tandem_reset(tandem_handle* h) {
   CU(h, cudaMemset(h->st_mem8, 0, (size_t)3 * S));
   CU(h, cudaMemset(h->stats, 0, sizeof(DevStats)));
   CU(h, cudaMemset(h->n_active, 0, 4));
+  if (h->oom_host) *h->oom_host = 0;
   std::vector<int32_t> fp(h->pool_pages);
   for (int i = 0; i < h->pool_pages - 1; ++i) fp[i] = h->pool_pages - 1 - i;   // pages 1..pool-1; popped in ascending order
+  if (h->page_order_seed) {   // test hook: a seeded Fisher-Yates shuffle of the hand-out order (splitmix64)
+    uint64_t x = h->page_order_seed;
+    auto next = [&x]() { x += 0x9E3779B97F4A7C15ull; uint64_t z = x; z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull; z = (z ^ (z >> 27)) * 0x94D049BB133111EBull; return z ^ (z >> 31); };
+    for (int i = h->pool_pages - 2; i > 0; --i) std::swap(fp[i], fp[(size_t)(next() % (uint64_t)(i + 1))]);
+  }
   const int32_t top = h->pool_pages - 1;
   for (int m = 0; m < 2; ++m) {
     CU(h, cudaMemcpy(h->ws[m].free_pages, fp.data(), (size_t)h->pool_pages * 4, cudaMemcpyHostToDevice));
@@ -996,16 +821,9 @@ int tandem_get_profile(tandem_handle* h, double* ms, int64_t* launches) {
   return TANDEM_OK;
 }
 
-int tandem_debug_lt_times(tandem_handle* h, unsigned long long* out, int n) {
-  if (!h || !out || !h->lt_ts) return TANDEM_ESTATE;
-  CU(h, cudaDeviceSynchronize());
-  CU(h, cudaMemcpy(out, h->lt_ts, (size_t)std::min(n, (h->cfg.n_layers + 1) * 32) * 8, cudaMemcpyDeviceToHost));
-  return TANDEM_OK;
-}
-
 const char* tandem_kernel_class_name(int kc) {
   static const char* names[TANDEM_KC_NUM] = {"sched", "embed_norm", "gemm_qkv", "rope_append", "attention", "attn_combine", "gemm_o",
-                                             "residual_norm", "gemm_gateup", "swiglu", "gemm_down", "gemm_lmhead", "sample_switch_emit", "finalize", "layer_tail", "score"};
+                                             "residual_norm", "gemm_gateup", "swiglu", "gemm_down", "gemm_lmhead", "sample_switch_emit", "finalize", "score"};
   return (kc >= 0 && kc < TANDEM_KC_NUM) ? names[kc] : "?";
 }
 
@@ -1053,7 +871,6 @@ int tandem_load_weights(tandem_handle* h, int model, const tandem_weights* w) {
   mw.loaded = true;
   if (h->graph) { cudaGraphExecDestroy(h->graph); h->graph = nullptr; h->gkey.valid = false; }
   if (h->tc) tc_gemm_invalidate(h->tc, model);
-  h->lt_maps_ready = false;
   return TANDEM_OK;
 }
 
@@ -1063,6 +880,7 @@ int tandem_step(tandem_handle* h, const tandem_step_in* in, tandem_step_out* out
   if (!in) return fail(h, TANDEM_EINVAL, "step_in is NULL");
   if ((rc = check_params(h, in->params))) return rc;
   cudaStream_t s = (cudaStream_t)cuda_stream;
+  if ((rc = check_oom_flag(h))) return rc;
   if ((rc = sync_word_start(h, in->params, s))) return rc;
   if (in->n_admit > 0) {
     if ((rc = check_oom(h, s))) return rc;
@@ -1089,9 +907,9 @@ int tandem_generate(tandem_handle* h, const tandem_params* params, int32_t B, co
   if (out_tokens) std::memset(out_tokens, 0, (size_t)B * out_stride * 4);
   if (out_owner) std::memset(out_owner, 0, (size_t)B * out_stride);
   if (out_sen_logp) std::memset(out_sen_logp, 0, (size_t)B * out_stride * 4);
-  cudaEvent_t e0, e1;
-  CU(h, cudaEventCreate(&e0)); CU(h, cudaEventCreate(&e1));
-  CU(h, cudaEventRecord(e0, s));
+  EventPair ev;
+  CU(h, cudaEventCreate(&ev.e0)); CU(h, cudaEventCreate(&ev.e1));
+  CU(h, cudaEventRecord(ev.e0, s));
   const StepIO io = make_io(nullptr, ovr);
   const RuleParams rp = make_rule(params);
   std::vector<int> slot_seq(c.max_seqs, -1);
@@ -1126,6 +944,7 @@ int tandem_generate(tandem_handle* h, const tandem_params* params, int32_t B, co
       if (pages_reserved + add + need > pages_avail) break;
       add += need; ++n;
     }
+    if (ovr && n < B) return fail(h, TANDEM_ENOMEM, "overrides are addressed by slot = batch index: the whole batch must fit the KV pools at once");
     if (n > 0) {
       std::vector<int32_t> slots(n);
       for (int i = 0; i < n; ++i) ids[i] = seq_ids ? seq_ids[next + i] : next + i;
@@ -1156,11 +975,10 @@ int tandem_generate(tandem_handle* h, const tandem_params* params, int32_t B, co
       ++finished;
     }
   }
-  CU(h, cudaEventRecord(e1, s));
-  CU(h, cudaEventSynchronize(e1));
+  CU(h, cudaEventRecord(ev.e1, s));
+  CU(h, cudaEventSynchronize(ev.e1));
   float ms = 0.f;
-  CU(h, cudaEventElapsedTime(&ms, e0, e1));
-  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  CU(h, cudaEventElapsedTime(&ms, ev.e0, ev.e1));
   if ((rc = check_oom(h, s))) return rc;
   if (stats) {
     if ((rc = fill_stats(h, stats))) return rc;
@@ -1185,9 +1003,9 @@ int tandem_score(tandem_handle* h, int32_t n_seqs, const int32_t* tokens, const 
   if ((rc = tandem_reset(h))) return rc;
   const int64_t total = n_seqs > 0 ? offsets[n_seqs] - offsets[0] : 0;
   for (float* o : {sen_logp, jun_logp, overlap}) if (o && total > 0) std::memset(o + offsets[0], 0, (size_t)total * sizeof(float));
-  cudaEvent_t e0, e1;
-  CU(h, cudaEventCreate(&e0)); CU(h, cudaEventCreate(&e1));
-  CU(h, cudaEventRecord(e0, s));
+  EventPair ev;
+  CU(h, cudaEventCreate(&ev.e0)); CU(h, cudaEventCreate(&ev.e1));
+  CU(h, cudaEventRecord(ev.e0, s));
   tandem_params prm{};   // admission only needs an owner; the rule never runs while scoring
   prm.p = 0.f; prm.switch_mode = TANDEM_TOGGLE; prm.start_owner = TANDEM_SENIOR; prm.temperature = temperature; prm.top_p = 1.f; prm.top_k = 0; prm.eos_id = -1;
   const StepIO io = make_io(nullptr, nullptr);
@@ -1247,11 +1065,10 @@ int tandem_score(tandem_handle* h, int32_t n_seqs, const int32_t* tokens, const 
       ++finished;
     }
   }
-  CU(h, cudaEventRecord(e1, s));
-  CU(h, cudaEventSynchronize(e1));
+  CU(h, cudaEventRecord(ev.e1, s));
+  CU(h, cudaEventSynchronize(ev.e1));
   float ms = 0.f;
-  CU(h, cudaEventElapsedTime(&ms, e0, e1));
-  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  CU(h, cudaEventElapsedTime(&ms, ev.e0, ev.e1));
   if ((rc = check_oom(h, s))) return rc;
   if (stats) {
     if ((rc = fill_stats(h, stats))) return rc;
@@ -1293,14 +1110,10 @@ void tandem_free(tandem_handle* h) {
   if (h->ev_in) cudaEventDestroy(h->ev_in);
   if (h->ev_out) cudaEventDestroy(h->ev_out);
   if (h->gs) cudaStreamDestroy(h->gs);
-  if (h->gs2) cudaStreamDestroy(h->gs2);
-  if (h->ev_fork) cudaEventDestroy(h->ev_fork);
-  if (h->ev_join) cudaEventDestroy(h->ev_join);
-  for (cudaEvent_t e : h->stagger_ev) cudaEventDestroy(e);
-  fr(h->zero_counts);
   fr(h->score_out[0]); fr(h->score_out[1]); fr(h->st_mem); fr(h->st_mem8); fr(h->tokens); fr(h->out_owner); fr(h->out_logp); fr(h->rope_cs); fr(h->word_start_dev); fr(h->stats);
   fr(h->gt_mem); fr(h->gt_pages_mem);
-  fr(h->lt_wmaps); fr(h->lt_amaps); fr(h->lt_ts); fr(h->n_active); fr(h->work_ctr); fr(h->stage_tokens); fr(h->stage_off); fr(h->stage_i32);
+  if (h->oom_host) cudaFreeHost(h->oom_host);
+  fr(h->n_active); fr(h->work_ctr); fr(h->stage_tokens); fr(h->stage_off); fr(h->stage_i32);
   cudaGetLastError();
   delete h;
 }
@@ -1365,11 +1178,32 @@ int tandem_test_gemm(int32_t dtype, int32_t impl, int32_t rows, int32_t N, int32
   return cudaDeviceSynchronize() == cudaSuccess ? TANDEM_OK : TANDEM_ECUDA;
 }
 
-int tandem_test_gemm_time(int32_t rows, int32_t N, int32_t K, int32_t iters, int32_t cluster, int32_t ring_kb, int32_t splits, int32_t flags,
-                          float* ms_per_launch) {
+int tandem_test_gemm_time(int32_t rows, int32_t N, int32_t K, int32_t iters, int32_t ring_kb, int32_t splits, int32_t flags, float* ms_per_launch) {
   if (rows <= 0 || N <= 0 || K <= 0 || iters <= 0 || !ms_per_launch) return TANDEM_EINVAL;
-  TcGemmTune t; t.ring_kb = ring_kb; t.splits = splits; t.pdl = (flags & 2) != 0; t.pair = cluster == 2 ? 1 : 0;
+  TcGemmTune t; t.ring_kb = ring_kb; t.splits = splits; t.pdl = (flags & 2) != 0; t.pair = (flags & 4) ? 1 : 0;
   return tc_gemm_time(rows, N, K, iters, t, (flags & 1) ? kTcEpiSwiGLU : kTcEpiPartial, ms_per_launch);
+}
+
+int tandem_test_set_option(tandem_handle* h, const char* name, int32_t value) {
+  if (!h || !name) return TANDEM_EINVAL;
+  const std::string n(name);
+  auto in = [&](int lo, int hi) { return value >= lo && value <= hi; };
+  if (n == "pdl" && in(0, 1)) h->use_pdl = value != 0;
+  else if (n == "attn_ctas_per_sm" && in(1, 2)) h->attn_ctas_per_sm = value;
+  else if (n == "gemm_ring_kb" && in(0, 200)) h->gemm_ring_kb = value;
+  else if (n == "gemm_pair" && in(-1, 1)) h->gemm_pair = value;
+  else if (n == "score_nosplit" && in(0, 1)) h->score_nosplit = value != 0;
+  else if (n == "score_chunk_grid" && in(1, 16)) h->score_chunk_grid = value;
+  else return fail(h, TANDEM_EINVAL, "unknown option or value out of range: " + n);
+  CU(h, cudaDeviceSynchronize());
+  if (h->graph) { cudaGraphExecDestroy(h->graph); h->graph = nullptr; h->gkey.valid = false; }
+  return TANDEM_OK;
+}
+
+int tandem_test_set_page_order(tandem_handle* h, uint64_t seed) {
+  if (!h) return TANDEM_EINVAL;
+  h->page_order_seed = seed;
+  return TANDEM_OK;
 }
 
 }  // extern "C"

@@ -10,9 +10,3 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
-
-
-def pytest_collection_modifyitems(config, items):
-    """GPU tests fail loudly (not skip) when selected on a box whose CUDA extension cannot load;
-    on a CPU-only box they are deselected by `-m "not gpu"`."""
-    return

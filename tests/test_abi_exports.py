@@ -1,4 +1,4 @@
-"""CPU-only: the C-ABI library builds for sm_100a, loads, and exports every symbol include/tandem.h declares.
+"""CPU-only: the C-ABI library builds for sm_100a, loads, and exports every symbol include/*.h declares.
 No compute call is made (there is no GPU here)."""
 import os
 import re
@@ -9,9 +9,12 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 def _declared():
-    src = open(os.path.join(ROOT, "include", "tandem.h")).read()
-    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(tandem_[a-z0-9_]+)\s*\(", src)))
+    names = set()
+    for hdr in sorted(os.listdir(os.path.join(ROOT, "include"))):      # every header under include/: the product API and the test hooks
+        src = open(os.path.join(ROOT, "include", hdr)).read()
+        src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+        names |= set(re.findall(r"\b(tandem_[a-z0-9_]+)\s*\(", src))
+    return sorted(names)
 
 
 def test_library_builds_loads_and_exports_every_declared_symbol():

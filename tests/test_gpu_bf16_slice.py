@@ -78,9 +78,6 @@ def _run_slice(name, gemm_impl, n_new=64, seed=4242):
                          top1_margin_ge_0p1=float(np.mean(top1[margins >= 0.1])) if (margins >= 0.1).any() else 1.0,
                          worst_margin_at_disagreement=float(margins[~top1].max()) if (~top1).any() else 0.0,
                          sampled_agreement=float(np.mean(samp)), junior_share=float(own.mean()))
-    os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
-    with open(os.path.join(ROOT, "gpurun_out", f"parity_bf16_{name}_impl{gemm_impl}.json"), "w") as f:
-        json.dump(res, f, indent=1)
     print(name, gemm_impl, json.dumps(res))
     return res
 

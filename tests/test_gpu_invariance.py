@@ -55,30 +55,6 @@ def test_batch_composition_and_determinism():
     eng2.free()
 
 
-@pytest.mark.parametrize("dtype", ["f32", "bf16"])
-def test_staggered_two_stream_mode_is_bit_identical(monkeypatch, dtype):
-    """TANDEM_STAGGER=1 (one chain of single-model launches per model on two streams, the junior half a layer behind; DESIGN.md
-    section 9) computes exactly what the paired launches compute: same K-splits, same kernels, hence identical bytes - with and
-    without the step graph."""
-    from workloads import ModelShape
-    shape = SHAPE if dtype == "f32" else ModelShape(3, 256, 4, 2, 64, 512, 2048, 1e-6, 1e6, "bf16")
-    ws = make_word_start(shape.vocab, 0.3, 4)
-    rng = np.random.default_rng(3)
-    prompts = [rng.integers(0, shape.vocab, size=n).astype(np.int32) for n in (9, 33, 17, 40, 5)]
-    prm = T.TandemParams(ws, p=0.5, temperature=1.0, seed=31)
-    eng, _, _ = make_pair(shape, max_seqs=5, max_seq_len=128)
-    a = eng.generate(prm, prompts, [40] * 5)
-    eng.free()
-    monkeypatch.setenv("TANDEM_STAGGER", "1")
-    for graph in (1, 0):
-        eng2, _, _ = make_pair(shape, max_seqs=5, max_seq_len=128, use_graph=graph)
-        b = eng2.generate(prm, prompts, [40] * 5)
-        eng2.free()
-        assert a["owner"].any() and not a["owner"].all()
-        for k in ("tokens", "owner", "sen_logp", "len"):
-            assert np.array_equal(a[k], b[k]), (k, graph)
-
-
 def test_api_errors():
     ws = make_word_start(SHAPE.vocab, 0.3, 4)
     eng = T.Tandem(T.TandemConfig(SHAPE, max_seqs=2, max_seq_len=32))
