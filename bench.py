@@ -60,7 +60,9 @@ def parse_args():
     ap.add_argument("--ramp", type=int, default=48, help="untimed steps after prefill so that both models own KV")
     ap.add_argument("--max-drain", type=int, default=256, help="upper bound on the extra untimed steps that drain the first catch-ups")
     ap.add_argument("--profile-steps", type=int, default=4)
-    ap.add_argument("--e2e-new", type=int, default=64, help="new tokens per sequence in the end-to-end tandem_generate leg")
+    ap.add_argument("--e2e-new", type=int, default=64, help="new tokens per sequence in the SHORT end-to-end tandem_generate leg (e2e_short)")
+    ap.add_argument("--no-e2e-full", action="store_true",
+                    help="skip the whole-workload tandem_generate call (e2e: every sequence to its max_new, ~50 s for cfg 3); e2e then falls back to the short leg")
     ap.add_argument("--profiler-range", action="store_true",
                     help="cudaProfilerStart/Stop around the timed region (for `ncu --profile-from-start off`)")
     ap.add_argument("--full-rollout", type=float, default=0.0, metavar="SCALE",
@@ -72,6 +74,16 @@ def parse_args():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-new", type=int, default=8, help="new tokens of the oracle's bounded sample")
     return ap.parse_args()
+
+
+def code_state():
+    """sha256 over the sources of the dominant kernel (the paged attention kernel and what it includes): `roofline.traffic` is an
+    ncu measurement stored beside this hash (profiles/traffic_r2.json) and is reported only while the hash still matches."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in ("attention_mma.cuh", "common.cuh"):
+        h.update(open(os.path.join(ROOT, "paper_2606_28166_b200", "csrc", f), "rb").read())
+    return h.hexdigest()[:16]
 
 
 def peaks():
@@ -369,7 +381,11 @@ def run_ours(args):
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    T.build()
+    if local == 0:
+        T.build()                     # one rank per node compiles (a stale pushed .so would otherwise be rebuilt by N ranks at once)
+    if dist:
+        dist.barrier()
+    T.lib()
     wl = get_workload(args.workload)
     if args.p is not None:
         wl = wl.with_(p=args.p)
@@ -389,18 +405,30 @@ def run_ours(args):
     row_cap = 4096
     prefill_steps = (prefill_rows + row_cap - 1) // row_cap + 2
     gen_budget = prefill_steps + max(args.ramp, int(8.0 / max(wl.p * wl.word_start_frac, 1e-3))) + args.max_drain + W + K + args.profile_steps + 64
-    max_seq_len = ((max_prompt + max(gen_budget, args.e2e_new) + 15) // 16) * 16
+    e2e_len = args.e2e_new if (args.no_e2e or args.no_e2e_full) else max(args.e2e_new, wl.max_new)
+    max_seq_len = ((max_prompt + max(gen_budget, e2e_len) + 15) // 16) * 16
+    # weights are drawn on the GPU, parked on the host and loaded from there, so that no staging copy competes with the KV pools
+    to_cpu = lambda w: dict(embed=w["embed"].cpu(), lm_head=w["lm_head"].cpu(), final_norm=w["final_norm"].cpu(),
+                            layers=[{k: v.cpu() for k, v in l.items()} for l in w["layers"]])
+    w_host = []
+    for seed in (wl.seeds["senior"], wl.seeds["junior"]):
+        w = make_weights(shape, seed, device="cuda"); w_host.append(to_cpu(w)); del w; torch.cuda.empty_cache()
+    # KV pools: what the timed steps need and, for the e2e leg, the whole workload (every sequence at prompt + max_new), as far as
+    # the device allows beside 2 x (layers + LM head + embedding) of weights and the workspaces; what does not fit queues in tandem_generate
+    from workloads import make_max_new
+    page_bytes = shape.kv_elems_per_token * 2 * 16
+    need_pages = B * ((max_prompt + gen_budget + 15) // 16 + 1)
+    if not (args.no_e2e or args.no_e2e_full):
+        need_pages = max(need_pages, sum((len(p) + int(n) + 15) // 16 + 1 for p, n in zip(build_inputs(wl, 0, rank)[0], make_max_new(wl))))
+    free, _ = torch.cuda.mem_get_info()
+    wbytes = 2 * (shape.params_read_per_step + shape.vocab * shape.hidden) * 2
+    kv_per_model = int(min((free - wbytes - 5.5e9) / 2, (need_pages + 64) * page_bytes))
     eng = T.Tandem(T.TandemConfig(shape, max_seqs=B, max_seq_len=max_seq_len, device=local, max_rows_per_step=row_cap, use_graph=1,
-                                  share_prompt_pages=0 if args.no_share_prompt_pages else 1))
-    w_cpu = []
-    for m, seed in enumerate((wl.seeds["senior"], wl.seeds["junior"])):
-        w = make_weights(shape, seed, device="cuda")
-        eng.load_weights(m, w)
-        if rank == 0 and world == 1 and not args.no_cpu:
-            w_cpu.append(dict(embed=w["embed"].cpu(), lm_head=w["lm_head"].cpu(), final_norm=w["final_norm"].cpu(),
-                              layers=[{k: v.cpu() for k, v in l.items()} for l in w["layers"]]))
-        del w
-        torch.cuda.empty_cache()
+                                  kv_bytes_per_model=kv_per_model, share_prompt_pages=0 if args.no_share_prompt_pages else 1))
+    for m in range(2):
+        eng.load_weights(m, w_host[m])
+    w_cpu = w_host if (rank == 0 and world == 1 and not args.no_cpu) else []
+    del w_host
     prm = T.TandemParams(table, p=wl.p, switch_mode=wl.switch_mode, temperature=wl.temperature, top_p=wl.top_p, top_k=args.top_k or wl.top_k, seed=20260628)
     out = dict(token=torch.zeros(B, dtype=torch.int32, device="cuda"), owner=torch.zeros(B, dtype=torch.uint8, device="cuda"),
                sen_logp=torch.zeros(B, device="cuda"), done=torch.zeros(B, dtype=torch.uint8, device="cuda"))
@@ -488,15 +516,20 @@ def run_ours(args):
                              "alg_bytes_per_launch": b, "gbs": b / (kms / n * 1e-3) / 1e9 if kms > 0 else None}
         top = max(kernels, key=lambda k: kernels[k]["share"])
         kt = kernels[top]
-        traffic = None        # DRAM bytes per launch of that kernel from the committed `ncu --set full` capture of this workload
-        tpath = os.path.join(ROOT, "profiles", "traffic_r1.json")
+        # DRAM bytes per launch of that kernel from the committed `ncu --set full` capture of this workload - valid only for the code
+        # state it was captured on: the entry carries the hash of the kernel's sources, and a mismatch reports null
+        traffic, traffic_note = None, "no capture for this workload"
+        tpath = os.path.join(ROOT, "profiles", "traffic_r2.json")
         if os.path.exists(tpath):
             tj = json.load(open(tpath))
             for kname, tv in tj.items():
                 if top == "attention" and "attention" in kname and tv.get("workload") == wl.name and tv.get("fast_forward") == args.fast_forward:
-                    traffic = tv["dram_bytes_per_launch"]
+                    if tv.get("code_sha") == code_state():
+                        traffic, traffic_note = tv["dram_bytes_per_launch"], "ncu --set full, %s" % tv.get("source", "profiles/")
+                    else:
+                        traffic_note = "stale: kernel sources changed since the capture (%s)" % tv.get("source", "profiles/")
         roofline = {"kernel": top, "bound": "hbm", "achieved": kt["gbs"], "peak": pk["hbm_gbs"], "unit": "GB/s",
-                    "frac": kt["gbs"] / pk["hbm_gbs"], "traffic": traffic, "alg_bytes_per_launch": kt["alg_bytes_per_launch"], "peak_source": pk["source"] + " burst copy (kernel timed alone)",
+                    "frac": kt["gbs"] / pk["hbm_gbs"], "traffic": traffic, "traffic_source": traffic_note, "alg_bytes_per_launch": kt["alg_bytes_per_launch"], "peak_source": pk["source"] + " burst copy (kernel timed alone)",
                     "share_of_step": kt["share"], "rows_per_launch": rows, "profile_steps": args.profile_steps,
                     "profile_ms_per_step": total_ms / args.profile_steps}
 
@@ -506,7 +539,7 @@ def run_ours(args):
                       "ctx_mean_timed": ctx_mean, "p": wl.p, "word_start_frac": wl.word_start_frac, "temperature": wl.temperature, "top_p": wl.top_p, "top_k": args.top_k or wl.top_k, "switch_mode": "REDRAW" if wl.switch_mode else "TOGGLE",
                       "page_tokens": 16, "parallelism": "dp%d (independent sequences, replicated weights, no collective)" % world,
                       "l2": "inputs larger than L2 (16.1 GB of weights + KV streamed per step vs 126 MB L2)",
-                      "setup_steps": n_setup + ramp + n_drain, "setup_seconds": setup_s, "cuda_graph": True},
+                      "setup_steps": n_setup + ramp + n_drain, "setup_seconds": setup_s, "cuda_graph": True, "kv_gb_per_model": kv_per_model / 1e9},
            "clocks": clk, "gpu_launches": int(d["kernel_launches"]),
            "step_roofline": {"bound": "hbm", "alg_bytes_per_step": step_bytes, "weights_bytes_per_step": d["weight_bytes_read"] / K,
                              "kv_bytes_per_step": d["kv_bytes_read"] / K, "achieved": step_gbs, "unit": "GB/s",
@@ -514,26 +547,43 @@ def run_ours(args):
                              "rows_per_step": (d["rows_senior"] + d["rows_junior"]) / K, "catchup_rows_per_step": d["catchup_rows"] / K},
            "roofline": roofline, "kernels": kernels}
 
-    # ---- end to end through tandem_generate with HOST buffers
+    # ---- end to end through tandem_generate with HOST buffers: prompts in (H2D), tokens / owner flags / senior log-probs out (D2H),
+    # prefill and admission inside the timed region. e2e_short: max_new capped (first call warms the graph of this parameter set);
+    # e2e: the WHOLE workload as BASELINE.json specifies it (every sequence to its max_new) - the metric itself.
     if not args.no_e2e:
-        new = args.e2e_new
-        e_prompts = build_inputs(wl, 0, rank)[0]   # the workload's own prompts: a rollout from its start, max_new capped
+        from workloads import make_max_new
+        e_prompts = build_inputs(wl, 0, rank)[0]   # the workload's own prompts: rollouts from their start
         e_rows = sum(len(p) for p in e_prompts)
-        for it in range(2):                      # first call warms the graph for this parameter set
+
+        def e2e_call(max_new_list):
             if dist: dist.barrier()
             t0 = time.perf_counter()
-            g = eng.generate(prm, e_prompts, [new] * B, seq_ids=seq_ids, stream=stream)
+            g = eng.generate(prm, e_prompts, max_new_list, seq_ids=seq_ids, stream=stream)
             torch.cuda.synchronize()
             dt = time.perf_counter() - t0
-        dt, tok = reduce_over_ranks(dist, dt, float(g["len"].sum()), "cuda")
-        steps_e = max(1, g["stats"]["steps"])
-        h2d = e_rows * 4 + (B + 1) * 8 + 3 * B * 4 + shape.vocab
-        d2h = B * new * (4 + 1 + 4) + B * 4
-        res["e2e"] = {"value": tok / dt, "unit": "tokens/s", "h2d_bytes_per_step": h2d / steps_e, "d2h_bytes_per_step": d2h / steps_e,
-                      "call": "tandem_generate(B=%d host prompts of the workload, max_new=%d): prompt prefill + %d engine steps, host buffers in and out"
-                              % (B, new, steps_e), "seconds": dt, "device_seconds": g["stats"]["seconds_total"],
-                      "share_prompt_pages": not args.no_share_prompt_pages, "prompt_rows": e_rows, "shared_prompt_rows": g["stats"]["shared_prompt_rows"],
-                      "rows_computed": g["stats"]["rows_senior"] + g["stats"]["rows_junior"]}
+            new_tot = int(np.sum(max_new_list))
+            dt_all, tok = reduce_over_ranks(dist, dt, float(g["len"].sum()), "cuda")
+            steps_e = max(1, g["stats"]["steps"])
+            h2d = e_rows * 4 + (B + 1) * 8 + 3 * B * 4 + shape.vocab
+            d2h = new_tot * (4 + 1 + 4) + B * 4
+            st = g["stats"]
+            gbs = (st["kv_bytes_read"] + st["weight_bytes_read"]) / max(st["seconds_total"], 1e-9) / 1e9
+            return {"value": tok / dt_all, "unit": "tokens/s", "h2d_bytes_per_step": h2d / steps_e, "d2h_bytes_per_step": d2h / steps_e,
+                    "call": "tandem_generate(B=%d host prompts of the workload, max_new=%d): prompt prefill + %d engine steps, host buffers in and out"
+                            % (B, int(np.max(max_new_list)), steps_e),
+                    "seconds": dt_all, "device_seconds": st["seconds_total"], "steps": int(st["steps"]), "tokens": int(tok),
+                    "ms_per_step": st["seconds_total"] / steps_e * 1e3,
+                    "senior_share": float(g["mask"].sum() / max(1, g["len"].sum())),
+                    "step_roofline": {"bound": "hbm", "achieved": gbs, "unit": "GB/s", "frac_of_measured": gbs / pk["hbm_gbs"], "frac_of_8TBs": gbs / NOMINAL_HBM_GBS},
+                    "share_prompt_pages": not args.no_share_prompt_pages, "prompt_rows": e_rows, "shared_prompt_rows": st["shared_prompt_rows"],
+                    "rows_computed": st["rows_senior"] + st["rows_junior"], "peak_resident": int(st["peak_resident"])}
+
+        for it in range(2):
+            res["e2e_short"] = e2e_call([args.e2e_new] * B)
+        if args.no_e2e_full or max_seq_len < max_prompt + wl.max_new:
+            res["e2e"] = res["e2e_short"]
+        else:
+            res["e2e"] = e2e_call([int(x) for x in make_max_new(wl)])
     eng.free()
     torch.cuda.empty_cache()
 

@@ -19,7 +19,7 @@ EXPORTED_SYMBOLS = ["tandem_init", "tandem_load_weights", "tandem_step", "tandem
                     "tandem_free", "tandem_last_error", "tandem_get_stats", "tandem_set_profile", "tandem_get_profile",
                     "tandem_kernel_class_name", "tandem_test_set_option", "tandem_test_set_page_order", "tandem_test_layer_times", "tandem_test_uniforms", "tandem_test_nucleus", "tandem_test_philox",
                     "tandem_test_gemm", "tandem_test_gemm_time"]
-KC_NUM = 16
+KC_NUM = 17
 
 
 class TandemError(RuntimeError):
@@ -68,7 +68,7 @@ class _StepOut(C.Structure):
 class _Stats(C.Structure):
     _fields_ = [(n, C.c_int64) for n in ("steps", "tokens_emitted", "rows_senior", "rows_junior", "catchup_rows", "kv_bytes_read", "weight_bytes_read")] + \
                [("peak_pages_senior", C.c_int32), ("peak_pages_junior", C.c_int32), ("peak_resident", C.c_int32), ("seconds_total", C.c_double),
-                ("kernel_launches", C.c_int64), ("shared_prompt_rows", C.c_int64)]
+                ("kernel_launches", C.c_int64), ("shared_prompt_rows", C.c_int64), ("starved", C.c_int64), ("preemptions", C.c_int64)]
 
 
 _lib = None

@@ -34,6 +34,7 @@ struct AttnMmaArgs {
   int nq, nkv; float scale;
   int row_base_k, row_base_v;  // tensor-map row of (page 0, kv head 0, token 0) of this layer's K / V pool
   int32_t* work_ctr;           // zeroed by the scheduler every step: units beyond the first gridDim.x are claimed dynamically
+  int min_ntok;                // measurement only (bench.py, cfg 5): items with fewer query tokens are skipped; 0 = all items
 };
 
 namespace ptx {
@@ -107,7 +108,7 @@ __global__ void __launch_bounds__(kAmThreads, 2) paged_attention_mma_kernel(cons
         const int item = ul / nkv, kvh = ul - item * nkv;
         const int slot = a.row_slot[a.item_row0[item]];
         const int kv0 = a.item_kv0[item], kv1 = a.item_kv1[item];
-        const int n_tiles = (kv1 - kv0 + kAmTileTok - 1) / kAmTileTok;
+        const int n_tiles = a.item_ntok[item] >= a.min_ntok ? (kv1 - kv0 + kAmTileTok - 1) / kAmTileTok : 0;   // a skipped item loads nothing: the consumers never see it
         const int32_t* btp = a.bt + (size_t)slot * a.max_pages + kv0 / kPageTokens;
         for (int ti = 0; ti < n_tiles; ++ti, ++it) {
           const int npg = min(4, (kv1 - kv0 - ti * kAmTileTok + kPageTokens - 1) / kPageTokens);

@@ -105,6 +105,7 @@ struct GroupTab {
 struct DevStats {       // device-side accumulators (unsigned long long for atomicAdd)
   unsigned long long steps, tokens_emitted, rows[2], catchup_rows, kv_tokens_read, model_steps;
   unsigned long long shared_rows;   // prompt positions taken over from a group's shared pages instead of being recomputed
+  unsigned long long starved;       // (sequence, step) pairs not scheduled because the model's page pool had no page left
   int peak_pages_used[2]; int peak_resident; int err_oom;
 };
 

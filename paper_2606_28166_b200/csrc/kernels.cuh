@@ -67,6 +67,7 @@ __global__ void __launch_bounds__(1024) sched_kernel(SchedArgs a) {
   block_excl_scan_1024(live ? 1 : 0, &resident_total, wsum);
   const int nfeed = a.score ? nctx - 1 : nctx;   // scoring: the last token is only a target
   int fed[2] = {0, 0};
+  int sched_rows_total = 0;   // thread 0 only
 
   for (int M = 0; M < 2; ++M) {
     const StepTab& tb = a.tab[M];
@@ -99,30 +100,34 @@ __global__ void __launch_bounds__(1024) sched_kernel(SchedArgs a) {
     const int want = (mine && !waits) ? nfeed - ing : 0;
     int total_want;
     const int pre = block_excl_scan_1024(want, &total_want, wsum);
-    const int rows = min(want, max(0, a.row_cap - pre));
-    const int cu = min(pre, a.row_cap);
-    const int n_rows = min(total_want, a.row_cap);
-    const bool emits = !a.score && mine && rows == want && want > 0;
-    fed[M] = ing + rows;
-
-    // pages for positions [ing, ing + rows)
-    if (rows > 0) {
-      const int need = (ing + rows + kPageTokens - 1) / kPageTokens;
-      const int have = pt.npages[s];
-      const int k = need - have;
-      if (k > 0) {
-        const int old = atomicSub(pt.free_top, k);
-        if (old >= k) {
-          for (int i = 0; i < k; ++i) pt.bt[(size_t)s * a.max_pages + have + i] = pt.free_pages[old - 1 - i];
-        } else {  // pool exhausted: point at the dummy page (no fault), flag the error for the host
-          atomicAdd(pt.free_top, k);
-          for (int i = 0; i < k; ++i) pt.bt[(size_t)s * a.max_pages + have + i] = 0;
-          a.stats->err_oom = 1;
-          if (a.oom_flag) *a.oom_flag = 1;
-        }
+    int rows = min(want, max(0, a.row_cap - pre));   // tentative: the row budget in slot order
+    // Pages for positions [ing, ing + rows), granted in slot order from the model's free stack. A sequence whose pages do not fit
+    // any more is NOT scheduled this step (it stalls, nothing is written for it) and neither is any later slot that needs pages:
+    // the pool never hands out a page twice and never points a block table at the dummy page. The host sees the stall through
+    // DevStats::starved / the mapped flag: tandem_generate preempts a resident sequence, tandem_step reports a dead lock.
+    {
+      const int have = mine ? pt.npages[s] : 0;
+      const int need = rows > 0 ? (ing + rows + kPageTokens - 1) / kPageTokens : 0;
+      const int k = max(0, need - have);
+      int total_k, total_g;
+      const int kpre = block_excl_scan_1024(k, &total_k, wsum);
+      const int free0 = *pt.free_top;                 // only this kernel and finalize_kernel (later in the stream) touch the stack
+      const bool granted = kpre + k <= free0;
+      block_excl_scan_1024(granted ? k : 0, &total_g, wsum);   // also orders every read of free_top before the write below
+      if (k > 0 && granted) {
+        for (int i = 0; i < k; ++i) pt.bt[(size_t)s * a.max_pages + have + i] = pt.free_pages[free0 - 1 - kpre - i];
         pt.npages[s] = need;
       }
+      if (k > 0 && !granted) { rows = 0; atomicAdd(&a.stats->starved, 1ull); }
+      if (threadIdx.x == 0 && total_k > 0) {
+        *pt.free_top = free0 - total_g;
+        if (total_g < total_k) { a.stats->err_oom = 1; if (a.oom_flag && *a.oom_flag < 1) *a.oom_flag = 1; }
+      }
     }
+    int n_rows;
+    const int cu = block_excl_scan_1024(rows, &n_rows, wsum);
+    const bool emits = !a.score && mine && rows == want && want > 0;
+    fed[M] = ing + rows;
     int n_emit;
     const int j = block_excl_scan_1024(emits ? 1 : 0, &n_emit, wsum);
     // attention items (S5): the rows of a sequence are cut into q-tiles of tile_tok tokens; q-tile t attends to the KV
@@ -207,6 +212,7 @@ __global__ void __launch_bounds__(1024) sched_kernel(SchedArgs a) {
       }
     }
     if (threadIdx.x == 0) {
+      sched_rows_total += n_rows;
       tb.counts[C_ROWS] = n_rows; tb.counts[C_SCHED] = n_sched; tb.counts[C_EMIT] = a.score ? n_rows : n_emit;
       tb.counts[C_ITEMS] = n_items; tb.counts[C_COMB] = n_comb; tb.counts[C_PARTS] = n_parts;
       a.stats->rows[M] += (unsigned long long)n_rows;
@@ -224,6 +230,8 @@ __global__ void __launch_bounds__(1024) sched_kernel(SchedArgs a) {
   if (threadIdx.x == 0) {
     a.stats->steps += 1ull;
     a.stats->peak_resident = max(a.stats->peak_resident, resident_total);
+    // live sequences, not a single row scheduled, and pages were refused: no step can make progress any more without the host
+    if (resident_total > 0 && sched_rows_total == 0 && a.stats->err_oom && a.oom_flag) *a.oom_flag = 2;
   }
 }
 

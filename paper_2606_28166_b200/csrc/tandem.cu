@@ -112,8 +112,8 @@ struct tandem_handle {
   CUtensorMap kv_map_store[2];
   const CUtensorMap* kv_map[2] = {nullptr, nullptr};   // each model's whole KV pool as rows of head_dim bf16 (tensor-core attention)
   // launch accounting and the optional per-kernel-class timing mode (tandem_set_profile)
-  int64_t launches = 0, graph_launches = 0;
-  bool profile = false;
+  int64_t launches = 0, graph_launches = 0, preemptions = 0;
+  bool profile = false, profile_catchup_attn = false;
   std::vector<cudaEvent_t> ev_pool; size_t ev_used = 0;
   struct ProfRec { int cls; cudaEvent_t e0, e1; };
   std::vector<ProfRec> prof_pending;
@@ -369,7 +369,7 @@ int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaS
         const StepTab& tb = h->tab[m];
         ma.m[m] = AttnMmaArgs{tb.counts, tb.item_row0, tb.item_ntok, tb.item_kv0, tb.item_kv1, tb.item_part, tb.row_slot, tb.row_pos, h->pt[m].bt, h->max_pages,
                               (const bf16*)h->ws[m].q, (bf16*)h->ws[m].attn_out, h->ws[m].part_acc, h->ws[m].part_ml, nq, nkv, 1.0f / sqrtf((float)d),
-                              (int)((2ll * l) * rows_per_half), (int)((2ll * l + 1) * rows_per_half), h->work_ctr + l};
+                              (int)((2ll * l) * rows_per_half), (int)((2ll * l + 1) * rows_per_half), h->work_ctr + l, 0};
         kmaps.m[m] = h->kv_map_store[m];
         ca.m[m] = CombineArgs<T>{tb.counts, tb.comb_row, tb.comb_part0, tb.comb_n, tb.comb_stride, h->ws[m].part_acc, h->ws[m].part_ml, (T*)h->ws[m].attn_out, nq, d};
       }
@@ -409,10 +409,16 @@ int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaS
           const StepTab& tb = h->tab[m];
           ma.m[m] = AttnMmaArgs{tb.counts, tb.item_row0, tb.item_ntok, tb.item_kv0, tb.item_kv1, tb.item_part, tb.row_slot, tb.row_pos, h->pt[m].bt, h->max_pages,
                                 (const bf16*)h->ws[m].q, (bf16*)h->ws[m].attn_out, h->ws[m].part_acc, h->ws[m].part_ml, nq, nkv, 1.0f / sqrtf((float)d),
-                                (int)((2ll * l) * rows_per_half), (int)((2ll * l + 1) * rows_per_half), h->work_ctr + l};
+                                (int)((2ll * l) * rows_per_half), (int)((2ll * l + 1) * rows_per_half), h->work_ctr + l, 0};
           maps.m[m] = h->kv_map_store[m];
         }
         KL(h, TANDEM_KC_ATTENTION, s, ok = run_attn_mma(maps, ma, d, nq / nkv, h->attn_ctas_per_sm * h->n_sms, s, false, pdl));
+        if (ok && h->profile && h->profile_catchup_attn) {
+          // measurement (BASELINE.json configs[4], "catch-up-prefill share of step time"): the same launch again, restricted to the items
+          // with more than one query token (S5b); it rewrites the same values, so results are unchanged
+          for (int m = 0; m < 2; ++m) { ma.m[m].min_ntok = 2; ma.m[m].work_ctr = h->work_ctr + c.n_layers + l; }
+          KL(h, TANDEM_KC_ATTN_CATCHUP, s, ok = run_attn_mma(maps, ma, d, nq / nkv, h->attn_ctas_per_sm * h->n_sms, s, false, pdl));
+        }
       } else {
         Pair<AttnArgs<T>> aa;
         for (int m = 0; m < 2; ++m) {
@@ -492,7 +498,7 @@ int launch_step(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaSt
   sa.st = h->st; sa.pt[0] = h->pt[0]; sa.pt[1] = h->pt[1]; sa.gt = h->gt; sa.tab[0] = h->tab[0]; sa.tab[1] = h->tab[1];
   sa.io = io; sa.stats = h->stats; sa.tokens = h->tokens; sa.max_seqs = c.max_seqs; sa.max_seq_len = c.max_seq_len;
   sa.max_pages = h->max_pages; sa.row_cap = h->row_cap; sa.tile_tok = h->tile_tok;
-  sa.work_ctr = h->work_ctr; sa.n_work_ctr = c.n_layers + (c.n_layers + 1) * h->lk_sync_per_launch;
+  sa.work_ctr = h->work_ctr; sa.n_work_ctr = 2 * c.n_layers + (c.n_layers + 1) * h->lk_sync_per_launch;
   sa.score = score ? 1 : 0; sa.oom_flag = h->oom_dev;
   KL(h, TANDEM_KC_SCHED, s, (sched_kernel<<<1, 1024, 0, s>>>(sa)));
   const int rc = (c.dtype == TANDEM_F32) ? forward_pair<float>(h, io, rp, s, score, score_inv_t) : forward_pair<bf16>(h, io, rp, s, score, score_inv_t);
@@ -677,6 +683,7 @@ int fill_stats(tandem_handle* h, tandem_stats* stats) {
   stats->seconds_total = 0.0;
   stats->kernel_launches = h->launches;
   stats->shared_prompt_rows = (int64_t)d.shared_rows;
+  stats->starved = (int64_t)d.starved; stats->preemptions = h->preemptions;
   return TANDEM_OK;
 }
 
@@ -695,9 +702,9 @@ struct EventPair {   // timing events of tandem_generate / tandem_score, destroy
 
 // KV-pool exhaustion seen by the scheduler of an earlier step (mapped host word, no synchronisation): sticky until tandem_reset
 int check_oom_flag(tandem_handle* h) {
-  if (h->oom_host && *(volatile int32_t*)h->oom_host)
-    return fail(h, TANDEM_ENOMEM, "KV page pool exhausted during generation (results of the starved sequences are invalid); tandem_reset the handle, "
-                                  "then enlarge kv_bytes_per_model or lower max_seqs");
+  if (h->oom_host && *(volatile int32_t*)h->oom_host >= 2)
+    return fail(h, TANDEM_ENOMEM, "KV page pools exhausted: every resident sequence is stalled and no step can make progress (nothing was corrupted); "
+                                  "tandem_reset the handle, then enlarge kv_bytes_per_model or admit fewer sequences");
   return TANDEM_OK;
 }
 
@@ -705,14 +712,26 @@ int check_oom(tandem_handle* h, cudaStream_t s) {
   DevStats st;
   CU(h, cudaStreamSynchronize(s));
   CU(h, cudaMemcpy(&st, h->stats, sizeof(st), cudaMemcpyDeviceToHost));
-  if (st.err_oom) return fail(h, TANDEM_ENOMEM, "KV page pool exhausted during generation (results of the starved sequences are invalid); tandem_reset the handle, "
-                                                "then enlarge kv_bytes_per_model or lower max_seqs");
+  if (h->oom_host && *(volatile int32_t*)h->oom_host >= 2) return check_oom_flag(h);
+  (void)st;
   if (h->lk_abort) {
     int32_t ab = 0;
     CU(h, cudaMemcpy(&ab, h->lk_abort, 4, cudaMemcpyDeviceToHost));
     if (ab) return fail(h, TANDEM_ECUDA, "a wait inside the layer kernel timed out (results invalid); tandem_reset the handle");
   }
   return TANDEM_OK;
+}
+
+// Preemption: the sequence in `slot` gives its pages back (its own ones at once, its group's shared prompt pages with the group's last
+// member) and the slot becomes free - the finalize kernel's path for a finished sequence, taken early.
+int preempt_slot(tandem_handle* h, int slot, cudaStream_t s) {
+  const tandem_config& c = h->cfg;
+  const uint8_t one = 1;
+  CU(h, cudaMemcpyAsync(h->st.done + slot, &one, 1, cudaMemcpyHostToDevice, s));
+  FinalArgs fa{h->st, {h->pt[0], h->pt[1]}, h->gt, StepIO{}, h->stats, h->n_active, c.max_seqs, h->max_pages, h->pool_pages};
+  finalize_kernel<<<1, 1024, 0, s>>>(fa);
+  CU(h, cudaGetLastError());
+  return refresh_slots(h, s);
 }
 
 }  // namespace
@@ -786,9 +805,9 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
   const bool lk_ok = c.dtype == TANDEM_BF16 && h->gemm_impl == TANDEM_GEMM_TCGEN05 && h->attn_impl == TANDEM_ATTN_MMA && h->n_sms >= 2 && c.hidden <= 4096;
   h->use_layer = false;   // opt-in (tandem_test_set_option "layer_kernel"): measured slower than the PDL-chained separate kernels so far
   h->lk_sync_per_launch = lk_ok ? kLkMaxPhases + 4 * (h->n_sms / 2) : 0;
-  INIT_TRY(dmalloc(h, &h->work_ctr, (size_t)(c.n_layers + (c.n_layers + 1) * h->lk_sync_per_launch) * 4));
-  INIT_CU(cudaMemset(h->work_ctr, 0, (size_t)(c.n_layers + (c.n_layers + 1) * h->lk_sync_per_launch) * 4));
-  h->lk_sync = h->work_ctr + c.n_layers;
+  INIT_TRY(dmalloc(h, &h->work_ctr, (size_t)(2 * c.n_layers + (c.n_layers + 1) * h->lk_sync_per_launch) * 4));
+  INIT_CU(cudaMemset(h->work_ctr, 0, (size_t)(2 * c.n_layers + (c.n_layers + 1) * h->lk_sync_per_launch) * 4));
+  h->lk_sync = h->work_ctr + 2 * c.n_layers;
   INIT_TRY(dmalloc(h, &h->lk_abort, 4));
   INIT_CU(cudaMemset(h->lk_abort, 0, 4));
   INIT_CU(cudaHostAlloc((void**)&h->oom_host, 4, cudaHostAllocMapped));
@@ -940,7 +959,7 @@ int tandem_reset(tandem_handle* h) {
   CU(h, cudaMemset(h->gt_mem, 0, (size_t)6 * S * 4));
   h->slot_grp.assign(S, -1); h->grp_live.assign(S, 0); h->grp_free.clear(); h->grp_reserved.assign(S, 0); h->grp_released = 0;
   for (int g = S - 1; g >= 0; --g) h->grp_free.push_back(g);
-  h->launches = 0;
+  h->launches = 0; h->preemptions = 0;
   return TANDEM_OK;
 }
 
@@ -966,7 +985,7 @@ int tandem_get_profile(tandem_handle* h, double* ms, int64_t* launches) {
 
 const char* tandem_kernel_class_name(int kc) {
   static const char* names[TANDEM_KC_NUM] = {"sched", "embed_norm", "gemm_qkv", "rope_append", "attention", "attn_combine", "gemm_o",
-                                             "residual_norm", "gemm_gateup", "swiglu", "gemm_down", "gemm_lmhead", "sample_switch_emit", "finalize", "score", "layer_kernel"};
+                                             "residual_norm", "gemm_gateup", "swiglu", "gemm_down", "gemm_lmhead", "sample_switch_emit", "finalize", "score", "layer_kernel", "attention_catchup"};
   return (kc >= 0 && kc < TANDEM_KC_NUM) ? names[kc] : "?";
 }
 
@@ -1056,57 +1075,86 @@ int tandem_generate(tandem_handle* h, const tandem_params* params, int32_t B, co
   CU(h, cudaEventRecord(ev.e0, s));
   const StepIO io = make_io(nullptr, ovr);
   const RuleParams rp = make_rule(params);
+  // Continuous batching: a sequence is admitted on its CURRENT need - the pages of
+  // its prompt in both pools - plus a watermark (the pages every resident sequence can grow by until the next poll), not on
+  // prompt + max_new. Pages come from the device-side free stacks on demand; when a pool runs dry the scheduler stalls the
+  // sequences it cannot serve (nothing is corrupted) and the host preempts the youngest resident sequence: its pages are freed,
+  // it goes back to the head of the queue and is redone from its prompt - bit-identically, since every random draw is addressed
+  // by (seed, seq_id, t, vocabulary id) and no result depends on the batch composition.
   std::vector<int> slot_seq(c.max_seqs, -1);
-  std::vector<int32_t> ids(c.max_seqs), nemit(c.max_seqs), plen(c.max_seqs);
-  // Admission by reservation: a sequence is admitted only if each model's page pool can hold its whole context
-  // (prompt + max_new), so a rollout never runs out of pages half-way; the rest waits in the queue (order preserved).
-  std::vector<int> slot_pages(c.max_seqs, 0);
-  auto pages_of = [&](int b) { return (int)((prompt_offsets[b + 1] - prompt_offsets[b] + max_new[b] + kPageTokens - 1) / kPageTokens); };
+  std::vector<int32_t> nemit(c.max_seqs), plen(c.max_seqs);
+  auto prompt_pages = [&](int b) { return (int)((prompt_offsets[b + 1] - prompt_offsets[b] + kPageTokens - 1) / kPageTokens) + 1; };
+  auto total_pages = [&](int b) { return (int)((prompt_offsets[b + 1] - prompt_offsets[b] + max_new[b] + kPageTokens - 1) / kPageTokens); };
   auto shared_pages_of = [&](int b) { return (int)((prompt_offsets[b + 1] - prompt_offsets[b] - 1) / kPageTokens); };
   auto same_prompt = [&](int a, int b) {
     const int64_t la = prompt_offsets[a + 1] - prompt_offsets[a], lb = prompt_offsets[b + 1] - prompt_offsets[b];
     return la == lb && std::memcmp(prompt_tokens + prompt_offsets[a], prompt_tokens + prompt_offsets[b], (size_t)la * 4) == 0;
   };
-  int pages_reserved = 0;
   const int pages_avail = h->pool_pages - 1;
-  for (int b = 0; b < B; ++b) if (pages_of(b) > pages_avail) return fail(h, TANDEM_ENOMEM, "a single sequence needs more KV pages than the pool holds");
-  int next = 0, finished = 0;
-  const int poll = 16;
+  for (int b = 0; b < B; ++b) if (total_pages(b) > pages_avail) return fail(h, TANDEM_ENOMEM, "a single sequence needs more KV pages than the pool holds");
+  std::vector<int> requeue;               // preempted sequences, admitted before the rest of the queue
+  int next = 0, finished = 0, resident = 0;
+  const int max_poll = 16;
   int64_t budget = 0;   // generous bound on the number of steps: guards against a stuck sequence
   for (int b = 0; b < B; ++b) budget += max_new[b] + (prompt_offsets[b + 1] - prompt_offsets[b]) / std::max(1, h->row_cap / 4) + 4;
-  budget = 4 * budget + 1024;
+  budget = 8 * budget + 4096;
+  int free_pages_now = pages_avail;       // min over the two pools, as of the last poll
+  bool starving = false;
   while (finished < B) {
-    if ((budget -= poll) < 0) return fail(h, TANDEM_ESTATE, "generation made no progress (internal error)");
+    // ---- admission
+    const int growth = max_poll / kPageTokens + 1;                // pages a resident sequence may take per model until the next poll
     int nfree = 0;
     for (int i = 0; i < c.max_seqs; ++i) nfree += !h->slot_busy[i];
-    int n = 0, add = 0;
-    while (n < std::min(nfree, B - next)) {
-      // with prompt-page sharing a sequence whose prompt equals its predecessor's in this batch joins that group (the rule of
-      // admit()) and needs no pages of its own for the shared prefix
-      const int b = next + n;
-      const int need = pages_of(b) - ((c.share_prompt_pages && n > 0 && same_prompt(b - 1, b)) ? shared_pages_of(b) : 0);
-      if (pages_reserved + add + need > pages_avail) break;
-      add += need; ++n;
-    }
-    if (ovr && next == 0 && n < B) return fail(h, TANDEM_ENOMEM, "overrides are addressed by slot = batch index: the whole batch must fit the KV pools at once");
-    if (n > 0) {
-      std::vector<int32_t> slots(n);
-      for (int i = 0; i < n; ++i) ids[i] = seq_ids ? seq_ids[next + i] : next + i;
-      if ((rc = admit(h, params, ovr, n, prompt_tokens, prompt_offsets + next, ids.data(), max_new + next, slots.data(), s))) return rc;
-      for (int i = 0; i < n; ++i) {
-        const int b = next + i, g = h->slot_grp[slots[i]];
-        slot_seq[slots[i]] = b;
-        slot_pages[slots[i]] = pages_of(b) - (g >= 0 ? shared_pages_of(b) : 0);   // a group holds its shared pages until its last member finishes
-        if (g >= 0) h->grp_reserved[g] = shared_pages_of(b);
+    // what the resident sequences may still take until the next poll (never more than the rest of their context)
+    int avail = free_pages_now;
+    for (int i = 0; i < c.max_seqs; ++i)
+      if (slot_seq[i] >= 0) {
+        const int b = slot_seq[i];
+        const int held = (int)((prompt_offsets[b + 1] - prompt_offsets[b] + nemit[i] + kPageTokens - 1) / kPageTokens);
+        avail -= std::min(growth, std::max(0, total_pages(b) - held));
       }
-      pages_reserved += add;
-      next += n;
+    auto admit_need = [&](int b) { return std::min(prompt_pages(b) + growth, total_pages(b)); };
+    if (!starving) {
+      while (!requeue.empty() && nfree > 0 && (avail >= admit_need(requeue.back()) || resident == 0)) {
+        const int b = requeue.back(); requeue.pop_back();
+        int32_t slot = -1; const int32_t id = seq_ids ? seq_ids[b] : b;
+        if ((rc = admit(h, params, ovr, 1, prompt_tokens, prompt_offsets + b, &id, max_new + b, &slot, s))) return rc;
+        slot_seq[slot] = b; --nfree; ++resident; avail -= admit_need(b);
+      }
+      int n = 0;
+      while (requeue.empty() && n < std::min(nfree, B - next)) {
+        const int b = next + n;
+        const int need = admit_need(b) - ((c.share_prompt_pages && n > 0 && same_prompt(b - 1, b)) ? std::min(shared_pages_of(b), admit_need(b)) : 0);
+        if (avail < need && resident + n > 0) break;              // an empty engine always takes the next sequence (it fits: checked above)
+        avail -= need; ++n;
+      }
+      if (ovr && next == 0 && n < B) return fail(h, TANDEM_ENOMEM, "overrides are addressed by slot = batch index: the whole batch must fit the KV pools at once");
+      if (n > 0) {
+        std::vector<int32_t> slots(n), ids(n);
+        for (int i = 0; i < n; ++i) ids[i] = seq_ids ? seq_ids[next + i] : next + i;
+        if ((rc = admit(h, params, ovr, n, prompt_tokens, prompt_offsets + next, ids.data(), max_new + next, slots.data(), s))) return rc;
+        for (int i = 0; i < n; ++i) slot_seq[slots[i]] = next + i;
+        next += n; resident += n;
+      }
     }
+    // ---- steps until the next poll: no longer than the soonest possible finish when there is no EOS to end a sequence early
+    int poll = starving ? 2 : max_poll;
+    if (params->eos_id < 0) {
+      int soonest = max_poll;
+      for (int i = 0; i < c.max_seqs; ++i) if (slot_seq[i] >= 0) soonest = std::min(soonest, std::max(1, max_new[slot_seq[i]] - nemit[i]));
+      poll = std::min(poll, soonest);
+    }
+    if ((budget -= poll) < 0) return fail(h, TANDEM_ESTATE, "generation made no progress (internal error)");
     for (int k = 0; k < poll; ++k) if ((rc = run_step(h, io, rp, s))) return rc;
-    if ((rc = refresh_slots(h, s))) return rc;
-    pages_reserved -= h->grp_released; h->grp_released = 0;
+    if ((rc = refresh_slots(h, s))) return rc;                   // synchronises the stream
     CU(h, cudaMemcpy(nemit.data(), h->st.n_emit, (size_t)c.max_seqs * 4, cudaMemcpyDeviceToHost));
     CU(h, cudaMemcpy(plen.data(), h->st.prompt_len, (size_t)c.max_seqs * 4, cudaMemcpyDeviceToHost));
+    {
+      int32_t ft[2];
+      for (int m = 0; m < 2; ++m) CU(h, cudaMemcpy(&ft[m], h->ws[m].free_top, 4, cudaMemcpyDeviceToHost));
+      free_pages_now = std::min(ft[0], ft[1]);
+    }
+    // ---- finished sequences: results to the caller's buffers
     for (int i = 0; i < c.max_seqs; ++i) {
       if (slot_seq[i] < 0 || h->slot_busy[i]) continue;
       const int b = slot_seq[i], len = nemit[i];
@@ -1114,9 +1162,27 @@ int tandem_generate(tandem_handle* h, const tandem_params* params, int32_t B, co
       if (out_tokens) CU(h, cudaMemcpy(out_tokens + (size_t)b * out_stride, h->tokens + (size_t)i * c.max_seq_len + plen[i], (size_t)len * 4, cudaMemcpyDeviceToHost));
       if (out_owner) CU(h, cudaMemcpy(out_owner + (size_t)b * out_stride, h->out_owner + (size_t)i * c.max_seq_len, (size_t)len, cudaMemcpyDeviceToHost));
       if (out_sen_logp) CU(h, cudaMemcpy(out_sen_logp + (size_t)b * out_stride, h->out_logp + (size_t)i * c.max_seq_len, (size_t)len * 4, cudaMemcpyDeviceToHost));
-      slot_seq[i] = -1;
-      pages_reserved -= slot_pages[i]; slot_pages[i] = 0;
-      ++finished;
+      slot_seq[i] = -1; nemit[i] = 0;
+      ++finished; --resident;
+    }
+    // ---- a pool ran dry since the last poll: preempt the youngest resident sequence (the least work to redo)
+    starving = false;
+    if (h->oom_host && *(volatile int32_t*)h->oom_host) {
+      *h->oom_host = 0;
+      CU(h, cudaMemset(&h->stats->err_oom, 0, sizeof(int)));
+      if (resident > 0) {
+        if (ovr) return fail(h, TANDEM_ENOMEM, "KV pool exhausted and overrides are addressed by slot: a sequence cannot be preempted");
+        int victim = -1;
+        for (int i = 0; i < c.max_seqs; ++i)
+          if (slot_seq[i] >= 0 && (victim < 0 || nemit[i] < nemit[victim] || (nemit[i] == nemit[victim] && slot_seq[i] > slot_seq[victim]))) victim = i;
+        if (resident == 1) return fail(h, TANDEM_ENOMEM, "KV pool exhausted by a single sequence (internal error: its whole context was checked to fit)");
+        if ((rc = preempt_slot(h, victim, s))) return rc;
+        requeue.push_back(slot_seq[victim]);
+        slot_seq[victim] = -1; nemit[victim] = 0; --resident;
+        ++h->preemptions;
+        starving = true;                    // poll soon: more may have to go before the stalled sequences move again
+        for (int m = 0; m < 2; ++m) { int32_t ft; CU(h, cudaMemcpy(&ft, h->ws[m].free_top, 4, cudaMemcpyDeviceToHost)); free_pages_now = m ? std::min(free_pages_now, ft) : ft; }
+      }
     }
   }
   CU(h, cudaEventRecord(ev.e1, s));
@@ -1341,6 +1407,7 @@ int tandem_test_set_option(tandem_handle* h, const char* name, int32_t value) {
   if (n == "pdl" && in(0, 1)) h->use_pdl = value != 0;
   else if (n == "attn_ctas_per_sm" && in(1, 2)) h->attn_ctas_per_sm = value;
   else if (n == "gemm_ring_kb" && in(0, 200)) h->gemm_ring_kb = value;
+  else if (n == "profile_catchup_attention" && in(0, 1)) h->profile_catchup_attn = value != 0;
   else if (n == "layer_debug" && in(0, 1)) {
     const size_t nb = (size_t)(h->cfg.n_layers + 1) * (32 * h->n_sms + 384) * 8;
     if (value && !h->lk_dbg) { DM(h, &h->lk_dbg, nb); CU(h, cudaMemset(h->lk_dbg, 0, nb)); }

@@ -198,3 +198,66 @@ def test_generate_queues_when_the_kv_pool_is_short():
         eng2.generate(T.TandemParams(ws, p=0.5, temperature=1.0, seed=77), [np.zeros(40, np.int32)], [16])   # 56 positions = 4 pages
     assert e.value.code == -2
     eng2.free()
+
+
+def test_generate_preempts_when_a_pool_runs_dry_and_redoes_bit_identically():
+    """Continuous batching: admission on current need + a watermark lets all four sequences in, their
+    growth then exhausts a 16-page pool (each needs 7 pages per model at the end), the scheduler stalls what it cannot serve and
+    tandem_generate preempts the youngest sequence and redoes it later from its prompt. Position-addressed random draws make the
+    redo bit-identical: tokens, owners, lengths equal the oracle's, which knows nothing of pages."""
+    shape = get_workload("cfg1_tiny_f32").shape
+    ws = make_word_start(shape.vocab, 0.3, 11)
+    rng = np.random.default_rng(18)
+    B = 4
+    prompts = [rng.integers(0, shape.vocab, size=10).astype(np.int32) for _ in range(B)]
+    max_new = np.array([100, 100, 100, 100], dtype=np.int32)
+    page_bytes = 2 * shape.n_layers * shape.n_kv_heads * 16 * shape.head_dim * 4
+    eng, orc, _ = make_pair(shape, (1, 2), max_seqs=4, max_seq_len=128, kv_bytes_per_model=17 * page_bytes)   # 16 usable pages
+    op = OParams(p=0.5, temperature=1.0, seed=5)
+    ref = tandem_generate(orc, op, prompts, max_new, ws, uni=Uniforms(seed=5))
+    out = eng.generate(T.TandemParams(ws, p=0.5, temperature=1.0, seed=5), prompts, max_new)
+    _compare(out, ref, B, logp_tol=2e-5)
+    st = out["stats"]
+    assert st["preemptions"] >= 1 and st["starved"] >= 1, st
+    assert st["peak_resident"] == 4 and max(st["peak_pages_senior"], st["peak_pages_junior"]) <= 16
+    again = eng.generate(T.TandemParams(ws, p=0.5, temperature=1.0, seed=5), prompts, max_new)      # and the call is repeatable
+    for k in ("tokens", "owner", "sen_logp", "len"):
+        assert np.array_equal(out[k], again[k])
+    eng.free()
+
+
+def test_step_stalls_on_an_empty_pool_and_reports_the_dead_lock():
+    """tandem_step on a pool too small for the admitted sequences: the scheduler stalls sequences instead of handing out the dummy
+    page (tokens emitted so far equal the oracle's), `starved` counts the stalls, and once nothing can move the next call returns
+    TANDEM_ENOMEM. tandem_reset makes the handle usable again."""
+    shape = get_workload("cfg1_tiny_f32").shape
+    ws = make_word_start(shape.vocab, 0.3, 11)
+    rng = np.random.default_rng(19)
+    B = 3
+    prompts = [rng.integers(0, shape.vocab, size=12).astype(np.int32) for _ in range(B)]
+    page_bytes = 2 * shape.n_layers * shape.n_kv_heads * 16 * shape.head_dim * 4
+    eng, orc, _ = make_pair(shape, (1, 2), max_seqs=B, max_seq_len=128, kv_bytes_per_model=7 * page_bytes)    # 6 usable pages = 96 positions
+    prm = T.TandemParams(ws, p=0.5, temperature=1.0, seed=6)
+    ref = tandem_generate(orc, OParams(p=0.5, temperature=1.0, seed=6), prompts, [100] * B, ws, uni=Uniforms(seed=6))
+    o = dict(token=torch.zeros(B, dtype=torch.int32, device="cuda"), owner=torch.zeros(B, dtype=torch.uint8, device="cuda"))
+    got = [[] for _ in range(B)]
+    err = None
+    for t in range(200):
+        try:
+            eng.step(prm, admit=(prompts, None, [100] * B) if t == 0 else None, out=o)
+        except T.TandemError as e:
+            err = e
+            break
+        torch.cuda.synchronize()
+        tok = o["token"].cpu().numpy()
+        for b in range(B):
+            if tok[b] >= 0:
+                got[b].append(int(tok[b]))
+    assert err is not None and err.code == -2, "the dead lock must surface as TANDEM_ENOMEM"
+    for b in range(B):                                       # everything emitted before the stall is right
+        assert len(got[b]) > 0 and got[b] == [int(x) for x in ref["tokens"][b][:len(got[b])]]
+    assert sum(len(g) for g in got) < 3 * 100
+    eng.reset()
+    out = eng.generate(prm, [prompts[0]], [20])
+    assert np.array_equal(out["tokens"][0, :20], ref["tokens"][0][:20])
+    eng.free()
