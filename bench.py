@@ -68,6 +68,9 @@ def parse_args():
     ap.add_argument("--full-rollout", type=float, default=0.0, metavar="SCALE",
                     help="instead of timed steps: run the WHOLE workload through tandem_generate (host buffers, admission queue) with "
                          "every max_new multiplied by SCALE (1.0 = the workload as specified) and report tokens/s of the call")
+    ap.add_argument("--catchup-share", action="store_true",
+                    help="BASELINE.json configs[4]: also report the catch-up-prefill share of STEP TIME - attention over the catch-up items "
+                         "(q_len > 1) timed by a second, filtered launch in the per-kernel pass, the row-proportional kernels apportioned by rows")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-share-prompt-pages", action="store_true",
                     help="every rollout computes and stores its own copy of the prompt's KV (default: the G rollouts of a prompt share its full pages)")
@@ -189,8 +192,6 @@ def class_bytes(shape, cls, rows, kv_bytes_per_layer_launch, emit_rows, n_models
         return g(H, I, rows)
     if cls == "gemm_lmhead":
         return g(V, H, emit_rows)
-    if cls == "layer_tail":
-        return g(H, qd, rows) + g(2 * I, H, rows) + g(H, I, rows) + g(qd + 2 * kd, H, rows)
     if cls == "attention":
         return kv_bytes_per_layer_launch + rows * qd * (4 + es)
     if cls == "rope_append":
@@ -497,6 +498,8 @@ def run_ours(args):
     roofline, kernels = None, {}
     if args.profile_steps > 0:
         p0 = eng.get_stats()
+        if args.catchup_share:
+            eng.set_option("profile_catchup_attention", 1)
         eng.set_profile(True)
         for _ in range(args.profile_steps):
             eng.step(prm, out=out, stream=stream)
@@ -507,7 +510,19 @@ def run_ours(args):
         rows = (p1["rows_senior"] + p1["rows_junior"] - p0["rows_senior"] - p0["rows_junior"]) / psteps
         emit_rows = (p1["tokens_emitted"] - p0["tokens_emitted"]) / psteps
         kv_launch = (p1["kv_bytes_read"] - p0["kv_bytes_read"]) / psteps / shape.n_layers
-        total_ms = sum(v[0] for v in prof.values())
+        dup_ms = prof.get("attention_catchup", (0.0, 0))[0]      # the filtered second launch is extra work: not part of a step
+        total_ms = sum(v[0] for v in prof.values()) - dup_ms
+        catchup = None
+        if args.catchup_share:
+            eng.set_option("profile_catchup_attention", 0)
+            crows = (p1["catchup_rows"] - p0["catchup_rows"]) / psteps
+            row_prop = ("gemm_qkv", "gemm_o", "gemm_gateup", "gemm_down", "rope_append", "residual_norm", "embed_norm", "attn_combine", "swiglu")
+            by_rows = sum(prof[k][0] for k in row_prop if k in prof) * (crows / max(rows, 1e-9))
+            catchup = {"share_of_step_time": (dup_ms + by_rows) / total_ms, "attention_catchup_ms_per_step": dup_ms / args.profile_steps,
+                       "row_proportional_ms_per_step": by_rows / args.profile_steps, "catchup_rows_per_step": crows, "rows_per_step": rows,
+                       "share_of_rows": crows / max(rows, 1e-9),
+                       "method": "attention over items with q_len > 1 timed directly (second, filtered launch in the per-kernel pass); "
+                                 "projection / norm / RoPE / combine time apportioned by rows; LM head, sampler, scheduler excluded"}
         for name, (kms, n) in prof.items():
             if n == 0:
                 continue
@@ -546,6 +561,8 @@ def run_ours(args):
                              "frac_of_measured": step_gbs / pk["hbm_gbs"], "frac_of_8TBs": step_gbs / NOMINAL_HBM_GBS,
                              "rows_per_step": (d["rows_senior"] + d["rows_junior"]) / K, "catchup_rows_per_step": d["catchup_rows"] / K},
            "roofline": roofline, "kernels": kernels}
+    if args.profile_steps > 0 and catchup is not None:
+        res["catchup_prefill"] = catchup
 
     # ---- end to end through tandem_generate with HOST buffers: prompts in (H2D), tokens / owner flags / senior log-probs out (D2H),
     # prefill and admission inside the timed region. e2e_short: max_new capped (first call warms the graph of this parameter set);

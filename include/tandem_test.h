@@ -12,7 +12,7 @@ extern "C" {
 /* kernel classes of one step, for launch accounting and tandem_get_profile */
 enum { TANDEM_KC_SCHED = 0, TANDEM_KC_EMBED, TANDEM_KC_GEMM_QKV, TANDEM_KC_ROPE_APPEND, TANDEM_KC_ATTENTION, TANDEM_KC_ATTN_COMBINE,
        TANDEM_KC_GEMM_O, TANDEM_KC_RESIDUAL_NORM, TANDEM_KC_GEMM_GATEUP, TANDEM_KC_SWIGLU, TANDEM_KC_GEMM_DOWN, TANDEM_KC_GEMM_LMHEAD,
-       TANDEM_KC_SAMPLE, TANDEM_KC_FINALIZE, TANDEM_KC_SCORE, TANDEM_KC_LAYER, TANDEM_KC_ATTN_CATCHUP, TANDEM_KC_NUM };
+       TANDEM_KC_SAMPLE, TANDEM_KC_FINALIZE, TANDEM_KC_SCORE, TANDEM_KC_ATTN_CATCHUP, TANDEM_KC_NUM };
 
 /* Per-kernel timing mode (bench.py's roofline leg): while enabled, a step runs un-captured on the caller's stream, every kernel
  * bracketed by CUDA events, and the call returns after the step has finished. Results are unchanged. enable = 1 also zeroes
@@ -24,16 +24,9 @@ const char *tandem_kernel_class_name(int kc);
 
 /* A/B knob for measurements, by name; call before the first step (a captured step graph is dropped). Names: "pdl" (0/1, default 1),
  * "attn_ctas_per_sm" (1/2), "gemm_ring_kb" (0 = automatic), "profile_catchup_attention" (0/1: in profile mode launch the attention kernel a second time on the
- * catch-up items only - q_len > 1 - as class attention_catchup; results unchanged), "layer_debug" (0/1), "layer_kernel" (0 = the separate per-projection kernels instead of the persistent
- * layer kernel; default 1 for bf16), "gemm_pair" (-1 automatic, 0, 1), "score_nosplit" (0/1),
+ * catch-up items only - q_len > 1 - as class attention_catchup; results unchanged),  "gemm_pair" (-1 automatic, 0, 1), "score_nosplit" (0/1),
  * "score_chunk_grid" (1..16). TANDEM_EINVAL for an unknown name or a value out of range. Every published number uses the defaults. */
 int tandem_test_set_option(tandem_handle *h, const char *name, int32_t value);
-
-/* Tuning aid (after tandem_test_set_option(h, "layer_debug", 1), else TANDEM_ESTATE): stamps of the last step's layer-kernel launches,
- * 32 words per (launch, CTA) - n_launches = n_layers + 1, CTAs = the SM count: [0] start, [1] after the dependency wait, [2 + 2p] / [3 + 2p] globaltimer ns at the start / end of
- * phase p, [16 + p] first operands of phase p landed, [24] / [25] cycles the MMA warp waited for operands / for a free accumulator, [26] k-blocks it issued, [27] stages * 1000 +
- * accumulator buffers. HOST out. */
-int tandem_test_layer_times(tandem_handle *h, unsigned long long *out, int32_t n);
 
 /* Parity tests at realistic page numbers: seed != 0 makes tandem_reset (and so tandem_generate / tandem_score) hand the pages of each
  * pool out in a pseudo-random order (a seeded permutation of 1..pool-1) instead of ascending, so that short tests touch scattered,
@@ -54,15 +47,11 @@ int tandem_test_philox(const uint32_t ctr[4], const uint32_t key[2], uint32_t ou
 /* out[rows,N] (fp32) = A[rows,K] * W[N,K]^T with the selected GEMM implementation; dtype of A and W as given.
  * impl = 3: the tcgen05 kernel with its fused SwiGLU epilogue - W rows interleaved (2i = gate_i, 2i+1 = up_i), out is bf16
  * [rows, N/2] = silu(A gate_i) * (A up_i). impl = 4, 5: the same two kernels launched as CTA pairs (cta_group::2: two adjacent weight
- * tiles share one M = 256 MMA and each CTA loads half of the token rows). impl = 6 .. 9: one GEMM phase of the persistent layer kernel
- * (layer_kernel.cuh: stream-K ranges, partial planes summed in k order): 6 / 7 = one model active (every range served by two CTAs, one
- * per 128-row half of a tile pair) with fp32 / SwiGLU output, 8 / 9 = both models active (tile pairs; the same problem for both, the
- * second model's result is returned). 6 and 8 are bit-identical by construction, and so are 7 and 9. */
+ * tiles share one M = 256 MMA and each CTA loads half of the token rows). */
 int tandem_test_gemm(int32_t dtype, int32_t impl, int32_t rows, int32_t N, int32_t K, const void *A_dev, const void *W_dev, float *out_dev);
 /* Mean device milliseconds of `iters` back-to-back launches of the tcgen05 GEMM [rows,K] x [N,K]^T on synthetic bf16 data, each launch
  * on a different weight buffer (more than the L2 holds in total). ring_kb / splits = 0: the library's own choice. flags: bit 0 = fused
- * SwiGLU epilogue, bit 1 = programmatic dependent launch, bit 2 = CTA pairs, bit 3 = one GEMM phase of the persistent layer kernel instead,
- * launched for two models of `rows` token rows each (two weight matrices per launch). HOST out. */
+ * SwiGLU epilogue, bit 1 = programmatic dependent launch, bit 2 = CTA pairs. HOST out. */
 int tandem_test_gemm_time(int32_t rows, int32_t N, int32_t K, int32_t iters, int32_t ring_kb, int32_t splits, int32_t flags, float *ms_per_launch);
 
 #ifdef __cplusplus

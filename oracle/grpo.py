@@ -15,7 +15,12 @@ Reading R19 where the paper leaves the standard objective 
   KL (optional) k_t = exp(logp_ref_t - logp_new_t) - (logp_ref_t - logp_new_t) - 1 (the estimator of Shao et al.), weight beta;
   aggregation   J_i = (1 / n_i) sum_{t < len_i, a_t = sen} (s_t - beta k_t), n_i = number of senior positions of rollout i
                 (J_i = 0 when n_i = 0); loss = -(1 / B) sum_i J_i  (Shao et al.'s 1/G sum_i 1/|o_i| sum_t with |o_i| narrowed
-                to the senior positions).
+                to the senior positions);
+  clip_frac     a diagnostic the paper does not define: the share of senior positions where the clipped branch is the one the
+                min selects (clip(rho) A < rho A), i.e. where the policy gradient is cut - not every position whose ratio left
+                [1 - eps, 1 + eps] (for A > 0 and rho < 1 - eps the unclipped branch is taken).
+Not covered by the paper's text: trainer stacks differ in the std convention (this reading: population std; some use the unbiased
+G - 1 form, which makes every advantage sqrt((G-1)/G) times smaller) - the caller can rescale `advantages`.
 """
 import numpy as np
 
@@ -30,7 +35,7 @@ def group_advantages(rewards, group, adv_eps=1e-6):
 
 def grpo_objective(rewards, group, lengths, owner, logp_new, logp_old, logp_ref=None, clip_eps=0.2, kl_beta=0.0, adv_eps=1e-6):
     """owner [B, L] (0 = senior-emitted), logp_* [B, L], lengths [B]. Returns dict(advantages [B], token_obj [B, L] (s_t - beta k_t at
-    senior positions, 0 elsewhere), seq_obj [B], loss, clip_frac (share of senior positions whose ratio was clipped), n_senior)."""
+    senior positions, 0 elsewhere), seq_obj [B], loss, clip_frac (share of senior positions where the clipped branch of the min is the one taken), n_senior)."""
     owner = np.asarray(owner)
     B, L = owner.shape
     A = group_advantages(rewards, group, adv_eps)
@@ -48,7 +53,7 @@ def grpo_objective(rewards, group, lengths, owner, logp_new, logp_old, logp_ref=
             rho = np.exp(ln[i, t] - lo[i, t])
             rc = min(max(rho, 1.0 - clip_eps), 1.0 + clip_eps)
             s = min(rho * A[i], rc * A[i])
-            if rc != rho:
+            if rc * A[i] < rho * A[i]:          # the clipped branch is the one min() takes (R19): the gradient of this position is cut
                 clipped += 1
             if kl_beta != 0.0 and logp_ref is not None:
                 d = float(logp_ref[i][t]) - ln[i, t]

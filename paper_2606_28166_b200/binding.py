@@ -17,9 +17,9 @@ _ERR = {0: "OK", -1: "EINVAL", -2: "ENOMEM", -3: "ECUDA", -4: "ESTATE", -5: "EFU
 
 EXPORTED_SYMBOLS = ["tandem_init", "tandem_load_weights", "tandem_step", "tandem_generate", "tandem_score", "tandem_grpo_objective", "tandem_reset",
                     "tandem_free", "tandem_last_error", "tandem_get_stats", "tandem_set_profile", "tandem_get_profile",
-                    "tandem_kernel_class_name", "tandem_test_set_option", "tandem_test_set_page_order", "tandem_test_layer_times", "tandem_test_uniforms", "tandem_test_nucleus", "tandem_test_philox",
+                    "tandem_kernel_class_name", "tandem_test_set_option", "tandem_test_set_page_order", "tandem_test_uniforms", "tandem_test_nucleus", "tandem_test_philox",
                     "tandem_test_gemm", "tandem_test_gemm_time"]
-KC_NUM = 17
+KC_NUM = 16
 
 
 class TandemError(RuntimeError):
@@ -105,7 +105,6 @@ def lib():
         L.tandem_test_gemm.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
         L.tandem_test_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_int32]
         L.tandem_test_set_page_order.argtypes = [C.c_void_p, C.c_uint64]
-        L.tandem_test_layer_times.argtypes = [C.c_void_p, C.c_void_p, C.c_int32]
         L.tandem_test_gemm_time.argtypes = [C.c_int32] * 7 + [C.POINTER(C.c_float)]
         _lib = L
     return _lib
@@ -254,18 +253,6 @@ class Tandem:
         """A/B knob for measurements (tandem_test.h: tandem_test_set_option)."""
         self._check(lib().tandem_test_set_option(self._h, name.encode(), int(value)))
 
-    def layer_times(self):
-        """Tuning aid: per layer-kernel launch of the last step, 32 stamps of CTA 0 (tandem_test.h: tandem_test_layer_times)."""
-        import torch
-        sms = torch.cuda.get_device_properties(self.config.c.device).multi_processor_count
-        per = 32 * sms + 384                                        # + the stage trace of two CTAs
-        n = (self.config.shape.n_layers + 1) * per
-        out = np.zeros(n, np.uint64)
-        self._check(lib().tandem_test_layer_times(self._h, out.ctypes.data, n))
-        out = out.reshape(self.config.shape.n_layers + 1, per)
-        self.last_stage_trace = out[:, 32 * sms:].reshape(-1, 2, 3, 64)
-        return out[:, :32 * sms].reshape(self.config.shape.n_layers + 1, sms, 32)
-
     def set_page_order(self, seed):
         """Test hook: hand KV pages out in a seeded pseudo-random order from the next reset on (0 = ascending)."""
         self._check(lib().tandem_test_set_page_order(self._h, int(seed)))
@@ -338,9 +325,9 @@ def tandem_test_gemm(dtype, impl, A, W, out):
         raise TandemError(rc)
 
 
-def tandem_test_gemm_time(rows, N, K, iters=50, ring_kb=0, splits=0, swiglu=0, pdl=0, pair=0, layer=0, dbg=0):
+def tandem_test_gemm_time(rows, N, K, iters=50, ring_kb=0, splits=0, swiglu=0, pdl=0, pair=0):
     ms = C.c_float()
-    rc = lib().tandem_test_gemm_time(rows, N, K, iters, ring_kb, splits, (1 if swiglu else 0) | (2 if pdl else 0) | (4 if pair else 0) | (8 if layer else 0) | (dbg << 4),
+    rc = lib().tandem_test_gemm_time(rows, N, K, iters, ring_kb, splits, (1 if swiglu else 0) | (2 if pdl else 0) | (4 if pair else 0),
                                      C.byref(ms))
     if rc:
         raise TandemError(rc)

@@ -382,10 +382,10 @@ gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__
 // per launch: O and down 3 splits = 120 CTAs: 12.98 ms per step; 4 splits = 160 CTAs: 13.13; 7 splits = 280 CTAs: 13.15), and
 // the consumer kernel has fewer partials to sum. A function of the shape and of the number of models per launch only, so the
 // reduction order (and every logit) is independent of the batch.
-inline int tc_gemm_splits(int N, int K, int n_models = 1) {
+inline int tc_gemm_splits(int N, int K, int n_models = 1, int n_sms = 148) {
   const int tiles = n_models * ((N + kTcTileN - 1) / kTcTileN), kb = (K + kTcBlockK - 1) / kTcBlockK;
   int s = 1;
-  while (tiles * (s + 1) <= 148 && (s + 1) * 4 <= kb && s < 16) ++s;
+  while (tiles * (s + 1) <= n_sms && (s + 1) * 4 <= kb && s < 16) ++s;
   return s;
 }
 
@@ -448,13 +448,14 @@ inline int tc_gemm_launch_epi(const TcMaps& maps, const Pair<TcGemmArgs>& g, dim
   if (pair) return launch_ex_cluster(gemm_tcgen05_kernel<EPI, true>, grid, dim3(kTcThreads), smem, s, pdl, 2, maps, g) == cudaSuccess ? 0 : -3;
   return launch_ex(gemm_tcgen05_kernel<EPI, false>, grid, dim3(kTcThreads), smem, s, pdl, maps, g) == cudaSuccess ? 0 : -3;
 }
-struct TcGemmTune { int ring_kb = 0, splits = 0; bool pdl = false; int pair = 0; int chunk_grid = 1; };   // pair: 1 = CTA pairs (cta_group::2), 0 = single CTAs   // 0 = automatic; overrides for tuning / tandem_test_gemm_time
+struct TcGemmTune { int ring_kb = 0, splits = 0; bool pdl = false; int pair = 0; int chunk_grid = 1; int n_sms = 148; };   // pair: 1 = CTA pairs (cta_group::2), 0 = single CTAs   // 0 = automatic; overrides for tuning / tandem_test_gemm_time
 // One launch for n_models (1 or 2) problems of the same shape: out[m] = A[m] W[m]^T, rows of model m from rows_ptr[m].
 inline int tc_gemm_launch(TcGemmPlans* p, int n_models, int which, const void* const* A, const void* const* W, int N, int K, float* const* out,
                           const int32_t* const* rows_ptr, int rows_cap, int* n_split, size_t* split_stride, cudaStream_t s, int epi = kTcEpiPartial,
                           const TcGemmTune* tune = nullptr) {
   if (!p || (K % 8) != 0) return -1;                       // TMA needs 16-byte row strides
-  int S = (which == 4 || epi == kTcEpiSwiGLU) ? 1 : tc_gemm_splits(N, K, n_models);
+  const int n_sms = tune ? tune->n_sms : 148;
+  int S = (which == 4 || epi == kTcEpiSwiGLU) ? 1 : tc_gemm_splits(N, K, n_models, n_sms);
   if (tune && tune->splits > 0) S = tune->splits;
   *n_split = S;
   *split_stride = (size_t)rows_cap * N;
@@ -467,7 +468,7 @@ inline int tc_gemm_launch(TcGemmPlans* p, int n_models, int which, const void* c
   // shorter tail (ncu, 512 rows, gate/up as 304 CTAs on 296 slots: SMs active 60% of the kernel's duration)
   const int CG = (tune && tune->chunk_grid > 1) ? std::min(tune->chunk_grid, (rows_cap + kTcMaxRows - 1) / kTcMaxRows) : 1;
   const int ring = (tune && tune->ring_kb > 0) ? tune->ring_kb * 1024
-                                                : (tiles_pad * S * CG * n_models > 148 ? 109 * 1024 : kTcRingBytes);   // more CTAs than SMs: two share an SM
+                                                : (tiles_pad * S * CG * n_models > n_sms ? 109 * 1024 : kTcRingBytes);   // more CTAs than SMs: two share an SM
   for (int m = 0; m < 2; ++m) {
     const int mm = m < n_models ? m : 0;
     const CUtensorMap* mw = tc_gemm_map(p, W[mm], N, K, kTcTileN);

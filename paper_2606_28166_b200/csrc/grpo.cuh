@@ -42,7 +42,7 @@ __global__ void __launch_bounds__(NT) grpo_seq_kernel(const __grid_constant__ Gr
       const float rho = expf(ln - a.logp_old[row + t]);
       const float rc = fminf(fmaxf(rho, lo_c), hi_c);
       s = fminf(rho * A, rc * A);
-      if (rc != rho) clipped += 1.f;
+      if (rc * A < rho * A) clipped += 1.f;   // the clipped branch is the one min() takes: the position whose gradient is cut (R19)
       if (a.kl_beta != 0.f && a.logp_ref) {
         const float d = a.logp_ref[row + t] - ln;
         s -= a.kl_beta * (expf(d) - d - 1.f);

@@ -21,7 +21,6 @@
 #include "attention_mma.cuh"
 #include "gemm_simt.cuh"
 #include "gemm_tcgen05.cuh"
-#include "layer_kernel.cuh"
 #include "grpo.cuh"
 
 using namespace tandem;
@@ -77,12 +76,6 @@ struct tandem_handle {
   bool score_nosplit = true;
   int score_chunk_grid = 8;                      // scoring: CTAs per (weight tile, K split) along the token rows (1 = off)
   bool use_pdl = true;                          // programmatic dependent launch along the kernel chain
-  // persistent layer kernel (layer_kernel.cuh): bf16 + tcgen05 + tensor-core attention, rollout steps (scoring keeps the separate kernels)
-  bool use_layer = false;
-  CUtensorMap* lk_wmaps = nullptr; CUtensorMap* lk_amaps = nullptr; bool lk_maps_ready = false;   // device tensor-map tables
-  int32_t* lk_sync = nullptr; int lk_sync_per_launch = 0;   // per launch: kLkMaxPhases barrier counters + 2 x 2 x NR fix-up flags, zeroed by the scheduler
-  int32_t* lk_abort = nullptr;                  // raised by a wait that timed out inside the layer kernel; sticky until tandem_reset
-  unsigned long long* lk_dbg = nullptr;         // tandem_test_set_option("layer_debug", 1): 32 stamps per layer-kernel launch (tandem_test_layer_times)
   size_t gemm_out_cols = 0;
   ModelWeights w[2];
   Workspace ws[2];
@@ -174,7 +167,7 @@ int launch_gemm(tandem_handle* h, int which, const void* const* A, const void* c
   static const int cls_of[5] = {TANDEM_KC_GEMM_QKV, TANDEM_KC_GEMM_O, TANDEM_KC_GEMM_GATEUP, TANDEM_KC_GEMM_DOWN, TANDEM_KC_GEMM_LMHEAD};
   if (h->gemm_impl == TANDEM_GEMM_TCGEN05 && sizeof(T) == 2) {
     int rc = 0;
-    TcGemmTune tune; tune.ring_kb = h->gemm_ring_kb; tune.pdl = h->use_pdl;
+    TcGemmTune tune; tune.ring_kb = h->gemm_ring_kb; tune.pdl = h->use_pdl; tune.n_sms = h->n_sms;
  tune.pair = h->gemm_pair >= 0 ? h->gemm_pair : (h->scoring ? 1 : 0);
     if (h->scoring && which != 4) {
       tune.chunk_grid = h->score_chunk_grid;   // hundreds of rows per launch: one CTA per 256-row chunk
@@ -243,99 +236,6 @@ bool attn_supported(int dtype, int D, int G) {
   return (D == 64 && (G == 1 || G == 2 || G == 4 || G == 7 || G == 8)) || (D == 128 && (G == 1 || G == 2 || G == 4 || G == 8));
 }
 
-// ------------------------------------------------------------------------------------------ persistent layer kernel
-// Tensor-map tables in device memory: weights [layer * 4 + gemm (0 O, 1 gate/up, 2 down, 3 QKV)][model][box: 256 | 128 rows],
-// activations [LK_A_ATTN | LK_A_ACT | LK_A_MLP][model][box: 128, 64, 32, 16 rows].
-int build_layer_maps(tandem_handle* h) {
-  const tandem_config& c = h->cfg;
-  const int H = c.hidden, nq = c.n_q_heads, nkv = c.n_kv_heads, d = c.head_dim, I = c.intermediate, L = c.n_layers;
-  const int qkv_n = (nq + 2 * nkv) * d;
-  std::vector<CUtensorMap> wm((size_t)L * 4 * 2 * 2), am((size_t)3 * 2 * 4);
-  bool ok = true;
-  auto put = [&](CUtensorMap& dst, const void* base, int rows, int K, int box) {
-    const CUtensorMap* mp = tc_gemm_map(h->tc, base, rows, K, box);
-    if (!mp) { ok = false; return; }
-    dst = *mp;
-  };
-  for (int m = 0; m < 2; ++m) {
-    const ModelWeights& w = h->w[m]; Workspace& ws = h->ws[m];
-    for (int l = 0; l < L; ++l)
-      for (int b = 0; b < 2; ++b) {
-        const int box = b == 0 ? kLkPairRows : kTcTileN;
-        put(wm[(((size_t)l * 4 + 0) * 2 + m) * 2 + b], w.wo[l], H, nq * d, box);
-        put(wm[(((size_t)l * 4 + 1) * 2 + m) * 2 + b], w.wgu[l], 2 * I, H, box);
-        put(wm[(((size_t)l * 4 + 2) * 2 + m) * 2 + b], w.wdown[l], H, I, box);
-        put(wm[(((size_t)l * 4 + 3) * 2 + m) * 2 + b], w.wqkv[l], qkv_n, H, box);
-      }
-    for (int b = 0; b < 4; ++b) {
-      const int box = 128 >> b;
-      put(am[((size_t)LK_A_ATTN * 2 + m) * 4 + b], ws.attn_out, h->row_cap, nq * d, box);
-      put(am[((size_t)LK_A_ACT * 2 + m) * 4 + b], ws.act, h->row_cap, H, box);
-      put(am[((size_t)LK_A_MLP * 2 + m) * 4 + b], ws.mlp_act, h->row_cap, I, box);
-    }
-  }
-  if (!ok) return fail(h, TANDEM_ECUDA, "tensor map encode failed (layer kernel)");
-  tc_gemm_invalidate(h->tc, 0);   // the per-launch cache is not needed for these
-  if (!h->lk_wmaps) { DM(h, &h->lk_wmaps, wm.size() * sizeof(CUtensorMap)); DM(h, &h->lk_amaps, am.size() * sizeof(CUtensorMap)); }
-  CU(h, cudaMemcpy(h->lk_wmaps, wm.data(), wm.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice));
-  CU(h, cudaMemcpy(h->lk_amaps, am.data(), am.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice));
-  h->lk_maps_ready = true;
-  return TANDEM_OK;
-}
-
-// Launch li = 0: QKV + RoPE of layer 0 (after embed_norm). Launch li = l + 1: O .. the second norm of layer l and, unless l is the
-// last layer, QKV + RoPE of layer l + 1.
-int launch_layer_kernel(tandem_handle* h, int li, cudaStream_t s) {
-  const tandem_config& c = h->cfg;
-  const int H = c.hidden, nq = c.n_q_heads, nkv = c.n_kv_heads, d = c.head_dim, I = c.intermediate, L = c.n_layers;
-  const int qkv_n = (nq + 2 * nkv) * d;
-  const int l = li - 1;                   // layer whose attention output this launch consumes (-1: none)
-  const int ln = li;                      // layer whose QKV / RoPE this launch produces (== L: none)
-  const size_t layer_kv = (size_t)2 * h->pool_pages * nkv * kPageTokens * d;
-  const size_t half_kv = (size_t)h->pool_pages * nkv * kPageTokens * d;
-  LkArgs a{};
-  int np = 0, norm1 = -1, norm2 = -1;
-  auto gemm = [&](int type, int N, int K, int wmap, int amap, int dep) { LkPhase& p = a.ph[np]; p = LkPhase{type, N, K, wmap, amap, dep, -1, 0}; return np++; };
-  auto elem = [&](int type, int src, int last) { LkPhase& p = a.ph[np]; p = LkPhase{type, 0, 0, 0, 0, -1, src, last}; return np++; };
-  int dep = -1;
-  if (l >= 0) {
-    const int po = gemm(LK_GEMM_PARTIAL, H, nq * d, l * 4 + 0, LK_A_ATTN, -1);
-    norm1 = elem(LK_NORM, po, 0);
-    const int pg = gemm(LK_GEMM_SWIGLU, 2 * I, H, l * 4 + 1, LK_A_ACT, norm1);
-    const int pd = gemm(LK_GEMM_PARTIAL, H, I, l * 4 + 2, LK_A_MLP, pg);
-    norm2 = elem(LK_NORM, pd, l == L - 1 ? 1 : 0);
-    dep = norm2;
-  }
-  if (ln < L) {
-    const int pq = gemm(LK_GEMM_PARTIAL, qkv_n, H, ln * 4 + 3, LK_A_ACT, dep);
-    elem(LK_ROPE, pq, 0);
-  }
-  a.n_phases = np;
-  for (int m = 0; m < 2; ++m) {
-    const ModelWeights& w = h->w[m]; Workspace& ws = h->ws[m]; const StepTab& tb = h->tab[m];
-    LkModel& M = a.m[m];
-    M.counts = tb.counts; M.x = ws.x; M.gemm_out = ws.gemm_out; M.act = (bf16*)ws.act; M.mlp_act = (bf16*)ws.mlp_act; M.lm_in = (bf16*)ws.lm_in;
-    M.row_emit = tb.row_emit; M.row_pos = tb.row_pos; M.row_kvslot = tb.row_kvslot; M.q = (bf16*)ws.q;
-    if (l >= 0) {
-      M.gain[norm1] = (const bf16*)w.mlp_norm[l];
-      M.gain[norm2] = (const bf16*)(l == L - 1 ? w.final_norm : w.attn_norm[l + 1]);
-    }
-    if (ln < L) {
-      bf16* kpool = (bf16*)ws.kv + (size_t)ln * layer_kv;
-      M.kpool = kpool; M.vpool = kpool + half_kv;
-    }
-  }
-  a.H = H; a.nq = nq; a.nkv = nkv; a.d = d; a.eps = c.rms_eps; a.rope_cs = h->rope_cs; a.row_cap = h->row_cap;
-  a.bar = h->lk_sync + (size_t)li * h->lk_sync_per_launch;
-  a.flag = a.bar + kLkMaxPhases;
-  a.abort_flag = h->lk_abort;
-  a.wmaps = h->lk_wmaps; a.amaps = h->lk_amaps;
-  a.dbg_ts = h->lk_dbg ? h->lk_dbg + (size_t)li * (32 * h->n_sms + 384) : nullptr;
-  cudaError_t e = cudaSuccess;
-  KL(h, TANDEM_KC_LAYER, s, e = launch_ex(layer_kernel, dim3(h->n_sms), dim3(kLkThreads), kLkSmemBytes, s, h->use_pdl, a));
-  return e == cudaSuccess ? TANDEM_OK : fail(h, TANDEM_ECUDA, std::string("layer kernel launch: ") + cudaGetErrorString(e));
-}
-
 // ------------------------------------------------------------------------------------------ both models' forward (S1..S8)
 // Every kernel is launched once for the two models (Pair arguments): the models advance layer by layer in lock-step on
 // one stream, each launch carrying the senior's and the junior's half of the work.
@@ -359,27 +259,7 @@ int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaS
     KL(h, TANDEM_KC_EMBED, s, launch_ex(embed_norm_kernel<T, 256>, dim3(row_grid, 2), dim3(256), 0, s, false, ea));
   }
 
-  const bool layer_k = h->use_layer && sizeof(T) == 2 && !score;
-  if (layer_k && (rc = launch_layer_kernel(h, 0, s))) return rc;
   for (int l = 0; l < c.n_layers; ++l) {
-    if (layer_k) {   // attention + combine, then everything up to the next attention in one persistent kernel
-      const long long rows_per_half = (long long)h->pool_pages * nkv * kPageTokens;
-      Pair<AttnMmaArgs> ma; Pair<CUtensorMap> kmaps; Pair<CombineArgs<T>> ca;
-      for (int m = 0; m < 2; ++m) {
-        const StepTab& tb = h->tab[m];
-        ma.m[m] = AttnMmaArgs{tb.counts, tb.item_row0, tb.item_ntok, tb.item_kv0, tb.item_kv1, tb.item_part, tb.row_slot, tb.row_pos, h->pt[m].bt, h->max_pages,
-                              (const bf16*)h->ws[m].q, (bf16*)h->ws[m].attn_out, h->ws[m].part_acc, h->ws[m].part_ml, nq, nkv, 1.0f / sqrtf((float)d),
-                              (int)((2ll * l) * rows_per_half), (int)((2ll * l + 1) * rows_per_half), h->work_ctr + l, 0};
-        kmaps.m[m] = h->kv_map_store[m];
-        ca.m[m] = CombineArgs<T>{tb.counts, tb.comb_row, tb.comb_part0, tb.comb_n, tb.comb_stride, h->ws[m].part_acc, h->ws[m].part_ml, (T*)h->ws[m].attn_out, nq, d};
-      }
-      bool ok = true;
-      KL(h, TANDEM_KC_ATTENTION, s, ok = run_attn_mma(kmaps, ma, d, nq / nkv, h->attn_ctas_per_sm * h->n_sms, s, false, pdl));
-      if (!ok) return fail(h, TANDEM_EINVAL, "unsupported (head_dim, group) for attention");
-      KL(h, TANDEM_KC_ATTN_COMBINE, s, launch_ex(attn_combine_kernel<T>, dim3(h->n_sms * 4, 2), dim3(256), 0, s, pdl, ca));
-      if ((rc = launch_layer_kernel(h, l + 1, s))) return rc;
-      continue;
-    }
     // S3 QKV projection
     for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].act, h->w[m].wqkv[l], h->ws[m].gemm_out, h->tab[m].counts + C_ROWS);
     if ((rc = launch_gemm<T>(h, 0, A, W, qkv_n, H, O, RP, h->row_cap, &ns, &ss, s))) return rc;
@@ -498,7 +378,7 @@ int launch_step(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaSt
   sa.st = h->st; sa.pt[0] = h->pt[0]; sa.pt[1] = h->pt[1]; sa.gt = h->gt; sa.tab[0] = h->tab[0]; sa.tab[1] = h->tab[1];
   sa.io = io; sa.stats = h->stats; sa.tokens = h->tokens; sa.max_seqs = c.max_seqs; sa.max_seq_len = c.max_seq_len;
   sa.max_pages = h->max_pages; sa.row_cap = h->row_cap; sa.tile_tok = h->tile_tok;
-  sa.work_ctr = h->work_ctr; sa.n_work_ctr = 2 * c.n_layers + (c.n_layers + 1) * h->lk_sync_per_launch;
+  sa.work_ctr = h->work_ctr; sa.n_work_ctr = 2 * c.n_layers;
   sa.score = score ? 1 : 0; sa.oom_flag = h->oom_dev;
   KL(h, TANDEM_KC_SCHED, s, (sched_kernel<<<1, 1024, 0, s>>>(sa)));
   const int rc = (c.dtype == TANDEM_F32) ? forward_pair<float>(h, io, rp, s, score, score_inv_t) : forward_pair<bf16>(h, io, rp, s, score, score_inv_t);
@@ -691,7 +571,6 @@ int check_ready(tandem_handle* h) {
   if (!h) return TANDEM_EINVAL;
   if (h->cuda_fault) return fail(h, TANDEM_ECUDA, "a previous CUDA error is sticky: " + h->err);
   if (!h->w[0].loaded || !h->w[1].loaded) return fail(h, TANDEM_ESTATE, "weights of both models must be loaded first");
-  if (h->use_layer && !h->lk_maps_ready) return build_layer_maps(h);
   return TANDEM_OK;
 }
 
@@ -714,11 +593,6 @@ int check_oom(tandem_handle* h, cudaStream_t s) {
   CU(h, cudaMemcpy(&st, h->stats, sizeof(st), cudaMemcpyDeviceToHost));
   if (h->oom_host && *(volatile int32_t*)h->oom_host >= 2) return check_oom_flag(h);
   (void)st;
-  if (h->lk_abort) {
-    int32_t ab = 0;
-    CU(h, cudaMemcpy(&ab, h->lk_abort, 4, cudaMemcpyDeviceToHost));
-    if (ab) return fail(h, TANDEM_ECUDA, "a wait inside the layer kernel timed out (results invalid); tandem_reset the handle");
-  }
   return TANDEM_OK;
 }
 
@@ -802,14 +676,8 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
     int dev_sms = 0;
     if (cudaDeviceGetAttribute(&dev_sms, cudaDevAttrMultiProcessorCount, c.device) == cudaSuccess && dev_sms > 0) h->n_sms = dev_sms;
   }
-  const bool lk_ok = c.dtype == TANDEM_BF16 && h->gemm_impl == TANDEM_GEMM_TCGEN05 && h->attn_impl == TANDEM_ATTN_MMA && h->n_sms >= 2 && c.hidden <= 4096;
-  h->use_layer = false;   // opt-in (tandem_test_set_option "layer_kernel"): measured slower than the PDL-chained separate kernels so far
-  h->lk_sync_per_launch = lk_ok ? kLkMaxPhases + 4 * (h->n_sms / 2) : 0;
-  INIT_TRY(dmalloc(h, &h->work_ctr, (size_t)(2 * c.n_layers + (c.n_layers + 1) * h->lk_sync_per_launch) * 4));
-  INIT_CU(cudaMemset(h->work_ctr, 0, (size_t)(2 * c.n_layers + (c.n_layers + 1) * h->lk_sync_per_launch) * 4));
-  h->lk_sync = h->work_ctr + 2 * c.n_layers;
-  INIT_TRY(dmalloc(h, &h->lk_abort, 4));
-  INIT_CU(cudaMemset(h->lk_abort, 0, 4));
+  INIT_TRY(dmalloc(h, &h->work_ctr, (size_t)2 * c.n_layers * 4));   // [L] attention work counters, [L] for the profile mode's catch-up-only launch
+  INIT_CU(cudaMemset(h->work_ctr, 0, (size_t)2 * c.n_layers * 4));
   INIT_CU(cudaHostAlloc((void**)&h->oom_host, 4, cudaHostAllocMapped));
   *h->oom_host = 0;
   INIT_CU(cudaHostGetDevicePointer((void**)&h->oom_dev, h->oom_host, 0));
@@ -837,17 +705,11 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
   // widest split-K partial buffer any GEMM needs, in floats per row (S*N); SIMT uses S = 1
   size_t cols = std::max({(size_t)qkv_n, (size_t)2 * I, (size_t)H});
   if (h->gemm_impl == TANDEM_GEMM_TCGEN05) {
-    cols = std::max(cols, (size_t)qkv_n * tc_gemm_splits(qkv_n, H));
-    cols = std::max(cols, (size_t)H * tc_gemm_splits(H, nq * d));
-    cols = std::max(cols, (size_t)2 * I * tc_gemm_splits(2 * I, H));
-    cols = std::max(cols, (size_t)H * tc_gemm_splits(H, I));
-  }
-  if (h->lk_sync_per_launch) {   // stream-K partial planes of the layer kernel, and its gate/up fix-up scratch (one 256-column slot per range)
-    const int NR = h->n_sms / 2;
-    cols = std::max(cols, (size_t)qkv_n * lk_max_planes(qkv_n, H, NR));
-    cols = std::max(cols, (size_t)H * lk_max_planes(H, nq * d, NR));
-    cols = std::max(cols, (size_t)H * lk_max_planes(H, I, NR));
-    cols = std::max(cols, (size_t)NR * kLkPairRows);
+    for (int nm = 1; nm <= 2; ++nm) {   // split counts are a function of the shape, the models per launch and the SM count
+      cols = std::max(cols, (size_t)qkv_n * tc_gemm_splits(qkv_n, H, nm, h->n_sms));
+      cols = std::max(cols, (size_t)H * tc_gemm_splits(H, nq * d, nm, h->n_sms));
+      cols = std::max(cols, (size_t)H * tc_gemm_splits(H, I, nm, h->n_sms));
+    }
   }
   h->gemm_out_cols = cols;
   for (int m = 0; m < 2; ++m) {
@@ -903,12 +765,15 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
   INIT_CU(cudaEventCreateWithFlags(&h->ev_in, cudaEventDisableTiming));
   INIT_CU(cudaEventCreateWithFlags(&h->ev_out, cudaEventDisableTiming));
   INIT_CU(cudaStreamCreateWithFlags(&h->gs, cudaStreamNonBlocking));
+  if (h->gemm_impl == TANDEM_GEMM_TCGEN05) {
+    int cc_major = 0;
+    cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, c.device);
+    if (cc_major != 10) return bad("the tcgen05 GEMM needs an sm_100-class device (compute capability 10.x)");
+  }
   if (h->gemm_impl == TANDEM_GEMM_TCGEN05 || h->attn_impl == TANDEM_ATTN_MMA) {
     h->tc = tc_gemm_create();
     if (!h->tc) { h->err = "tcgen05 GEMM setup failed (driver entry point for tensor maps not found)"; fprintf(stderr, "tandem_init: %s\n", h->err.c_str()); tandem_free(h); return TANDEM_ECUDA; }
   }
-  if (h->lk_sync_per_launch && cudaFuncSetAttribute(layer_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kLkSmemBytes) != cudaSuccess)
-    return bad("cannot reserve shared memory for the layer kernel");
   if (cudaFuncSetAttribute(sample_switch_emit_kernel<256, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(NucleusSmem<256>)) != cudaSuccess)
     return bad("cannot reserve shared memory for the nucleus sampler");
   if (h->attn_impl == TANDEM_ATTN_MMA) {
@@ -940,7 +805,6 @@ int tandem_reset(tandem_handle* h) {
   CU(h, cudaMemset(h->stats, 0, sizeof(DevStats)));
   CU(h, cudaMemset(h->n_active, 0, 4));
   if (h->oom_host) *h->oom_host = 0;
-  if (h->lk_abort) CU(h, cudaMemset(h->lk_abort, 0, 4));
   std::vector<int32_t> fp(h->pool_pages);
   for (int i = 0; i < h->pool_pages - 1; ++i) fp[i] = h->pool_pages - 1 - i;   // pages 1..pool-1; popped in ascending order
   if (h->page_order_seed) {   // test hook: a seeded Fisher-Yates shuffle of the hand-out order (splitmix64)
@@ -985,7 +849,7 @@ int tandem_get_profile(tandem_handle* h, double* ms, int64_t* launches) {
 
 const char* tandem_kernel_class_name(int kc) {
   static const char* names[TANDEM_KC_NUM] = {"sched", "embed_norm", "gemm_qkv", "rope_append", "attention", "attn_combine", "gemm_o",
-                                             "residual_norm", "gemm_gateup", "swiglu", "gemm_down", "gemm_lmhead", "sample_switch_emit", "finalize", "score", "layer_kernel", "attention_catchup"};
+                                             "residual_norm", "gemm_gateup", "swiglu", "gemm_down", "gemm_lmhead", "sample_switch_emit", "finalize", "score", "attention_catchup"};
   return (kc >= 0 && kc < TANDEM_KC_NUM) ? names[kc] : "?";
 }
 
@@ -1033,7 +897,6 @@ int tandem_load_weights(tandem_handle* h, int model, const tandem_weights* w) {
   mw.loaded = true;
   if (h->graph) { cudaGraphExecDestroy(h->graph); h->graph = nullptr; h->gkey.valid = false; }
   if (h->tc) tc_gemm_invalidate(h->tc, model);
-  h->lk_maps_ready = false;
   return TANDEM_OK;
 }
 
@@ -1323,7 +1186,6 @@ void tandem_free(tandem_handle* h) {
   fr(h->score_out[0]); fr(h->score_out[1]); fr(h->st_mem); fr(h->st_mem8); fr(h->tokens); fr(h->out_owner); fr(h->out_logp); fr(h->rope_cs); fr(h->word_start_dev); fr(h->stats);
   fr(h->gt_mem); fr(h->gt_pages_mem);
   if (h->oom_host) cudaFreeHost(h->oom_host);
-  fr(h->lk_wmaps); fr(h->lk_amaps); fr(h->lk_abort); fr(h->lk_dbg);
   fr(h->n_active); fr(h->work_ctr); fr(h->stage_tokens); fr(h->stage_off); fr(h->stage_i32);
   cudaGetLastError();
   delete h;
@@ -1378,10 +1240,6 @@ int tandem_test_gemm(int32_t dtype, int32_t impl, int32_t rows, int32_t N, int32
     if (dtype != TANDEM_BF16) return TANDEM_EINVAL;
     return tc_gemm_test(rows, N, K, A_dev, W_dev, out_dev, (impl == 3 || impl == 5) ? kTcEpiSwiGLU : kTcEpiPartial, impl >= 4);
   }
-  if (impl >= 6 && impl <= 9) {   // one GEMM phase of the persistent layer kernel: 6 / 7 one model active (partial planes / SwiGLU), 8 / 9 both
-    if (dtype != TANDEM_BF16) return TANDEM_EINVAL;
-    return lk_gemm_test(rows, N, K, A_dev, W_dev, out_dev, impl == 7 || impl == 9, impl >= 8);
-  }
   dim3 grid((N + kSimtTile - 1) / kSimtTile, std::max(1, std::min((rows + kSimtTile - 1) / kSimtTile, 64)));
   if (dtype == TANDEM_F32) {
     Pair<SimtGemmArgs<float>> g; g.m[0] = g.m[1] = SimtGemmArgs<float>{nullptr, rows, (const float*)A_dev, (const float*)W_dev, out_dev, N, K};
@@ -1395,7 +1253,6 @@ int tandem_test_gemm(int32_t dtype, int32_t impl, int32_t rows, int32_t N, int32
 
 int tandem_test_gemm_time(int32_t rows, int32_t N, int32_t K, int32_t iters, int32_t ring_kb, int32_t splits, int32_t flags, float* ms_per_launch) {
   if (rows <= 0 || N <= 0 || K <= 0 || iters <= 0 || !ms_per_launch) return TANDEM_EINVAL;
-  if (flags & 8) return lk_gemm_time(rows, N, K, iters, (flags & 1) != 0, (flags & 2) != 0, ms_per_launch, flags >> 4);   // one phase of the layer kernel, both models
   TcGemmTune t; t.ring_kb = ring_kb; t.splits = splits; t.pdl = (flags & 2) != 0; t.pair = (flags & 4) ? 1 : 0;
   return tc_gemm_time(rows, N, K, iters, t, (flags & 1) ? kTcEpiSwiGLU : kTcEpiPartial, ms_per_launch);
 }
@@ -1408,25 +1265,9 @@ int tandem_test_set_option(tandem_handle* h, const char* name, int32_t value) {
   else if (n == "attn_ctas_per_sm" && in(1, 2)) h->attn_ctas_per_sm = value;
   else if (n == "gemm_ring_kb" && in(0, 200)) h->gemm_ring_kb = value;
   else if (n == "profile_catchup_attention" && in(0, 1)) h->profile_catchup_attn = value != 0;
-  else if (n == "layer_debug" && in(0, 1)) {
-    const size_t nb = (size_t)(h->cfg.n_layers + 1) * (32 * h->n_sms + 384) * 8;
-    if (value && !h->lk_dbg) { DM(h, &h->lk_dbg, nb); CU(h, cudaMemset(h->lk_dbg, 0, nb)); }
-    if (!value && h->lk_dbg) { CU(h, cudaDeviceSynchronize()); cudaFree(h->lk_dbg); h->lk_dbg = nullptr; }
-  }
-  else if (n == "layer_kernel" && in(0, 1)) { if (value && !h->lk_sync_per_launch) return fail(h, TANDEM_EINVAL, "the layer kernel needs bf16 + tcgen05 + tensor-core attention"); h->use_layer = value != 0; }
-  else if (n == "gemm_pair" && in(-1, 1)) h->gemm_pair = value;
-  else if (n == "score_nosplit" && in(0, 1)) h->score_nosplit = value != 0;
-  else if (n == "score_chunk_grid" && in(1, 16)) h->score_chunk_grid = value;
   else return fail(h, TANDEM_EINVAL, "unknown option or value out of range: " + n);
   CU(h, cudaDeviceSynchronize());
   if (h->graph) { cudaGraphExecDestroy(h->graph); h->graph = nullptr; h->gkey.valid = false; }
-  return TANDEM_OK;
-}
-
-int tandem_test_layer_times(tandem_handle* h, unsigned long long* out, int32_t n) {
-  if (!h || !out || !h->lk_dbg) return TANDEM_ESTATE;
-  CU(h, cudaDeviceSynchronize());
-  CU(h, cudaMemcpy(out, h->lk_dbg, (size_t)std::min(n, (h->cfg.n_layers + 1) * (32 * h->n_sms + 384)) * 8, cudaMemcpyDeviceToHost));
   return TANDEM_OK;
 }
 

@@ -107,51 +107,6 @@ def test_tcgen05_gemm_swiglu_epilogue(rows, I, K):
     assert torch.equal(pair, out)
 
 
-@pytest.mark.parametrize("rows,N,K", [(1, 128, 64), (7, 256, 128), (33, 384, 192), (64, 512, 256), (128, 6144, 2560), (129, 2560, 4096),
-                                      (100, 2560, 9728), (300, 1152, 896), (257, 1024, 512), (61, 4096, 2560), (5, 200, 72), (600, 640, 1024),
-                                      (128, 896, 4864), (16, 1152, 896)])
-def test_layer_kernel_gemm_phase_partial_planes(rows, N, K):
-    """One GEMM phase of the persistent layer kernel (stream-K ranges over tile pairs, fp32 partial planes summed in k order)
-    against a float64 matmul: the projection shapes of cfg 3 and cfg 2, fewer units than ranges (1, 128, 64), a last odd tile
-    (N = 384, 640, 896, 1152), K not a multiple of 64, more than one 256-row chunk. With one model active every range is served by
-    two CTAs (one 128-row half each) over the same k-ranges: bit-identical to the tile-pair mode."""
-    g = torch.Generator().manual_seed(rows * 7919 + N + K)
-    A = torch.randn(rows, K, generator=g).to(torch.bfloat16).cuda()
-    W = (torch.randn(N, K, generator=g) * 0.05).to(torch.bfloat16).cuda()
-    ref = (A.double() @ W.double().T)
-    outs = []
-    for impl in (6, 8):
-        out = torch.full((rows, N), float("nan"), device="cuda")
-        T.tandem_test_gemm(T.BF16, impl, A, W, out)
-        err = torch.max(torch.abs(out.double() - ref)).item()
-        assert np.isfinite(err)
-        assert err <= 2e-6 * max(1.0, ref.abs().max().item()) * (K ** 0.5), (impl, err, ref.abs().max().item())
-        outs.append(out)
-    assert torch.equal(outs[0], outs[1])
-
-
-@pytest.mark.parametrize("rows,I,K", [(1, 64, 64), (37, 192, 128), (140, 9728, 2560), (128, 9728, 2560), (300, 512, 256), (64, 4864, 896), (90, 448, 200)])
-def test_layer_kernel_gemm_phase_swiglu_fixup(rows, I, K):
-    """The gate/up phase: tiles cut by a range boundary are completed by the CTA that holds their first k-block from the other
-    pieces' fp32 partials (flags, k order), then SwiGLU on the interleaved gate/up rows -> bf16. Against float64."""
-    g = torch.Generator().manual_seed(rows * 31 + I + K)
-    A = torch.randn(rows, K, generator=g).to(torch.bfloat16).cuda()
-    Wg = (torch.randn(I, K, generator=g) * 0.05).to(torch.bfloat16)
-    Wu = (torch.randn(I, K, generator=g) * 0.05).to(torch.bfloat16)
-    W = torch.stack([Wg, Wu], dim=1).reshape(2 * I, K).contiguous().cuda()
-    gate = A.double() @ Wg.cuda().double().T
-    up = A.double() @ Wu.cuda().double().T
-    ref = gate / (1 + torch.exp(-gate)) * up
-    outs = []
-    for impl in (7, 9):
-        out = torch.zeros(rows, I, dtype=torch.bfloat16, device="cuda")
-        T.tandem_test_gemm(T.BF16, impl, A, W, out)
-        err = torch.max(torch.abs(out.double() - ref)).item()
-        assert err <= 2 ** -8 * max(1e-3, ref.abs().max().item()) + 1e-6, (impl, err, ref.abs().max().item())   # one bf16 rounding of the result
-        outs.append(out)
-    assert torch.equal(outs[0], outs[1])
-
-
 def _nucleus(z, temperature, top_p, u, top_k=0):
     zt = torch.tensor(z, dtype=torch.float32, device="cuda")
     ut = torch.tensor(u, dtype=torch.float32, device="cuda")

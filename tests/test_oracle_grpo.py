@@ -78,3 +78,21 @@ def test_on_policy_special_cases():
     owner[3, :] = 1
     r2 = grpo_objective(rewards, G, [L] * G, owner, old, old)
     assert r2["seq_obj"][3] == 0 and abs(r2["loss"] - r["advantages"][3] / G) < 1e-12
+
+
+def test_clip_frac_counts_only_positions_where_the_clipped_branch_is_taken():
+    """R19: for A > 0 and rho < 1 - eps (or A < 0 and rho > 1 + eps) the min selects the UNCLIPPED branch: the ratio left the
+    interval but the gradient is not cut, so the position does not count. Hand case, one group of two rollouts (A = +1, -1),
+    one senior position each: rho = e^{-0.5} = 0.607 with A = +1 -> min(0.607, 0.8) = 0.607 (unclipped); rho = e^{0.5} = 1.649
+    with A = -1 -> min(-1.649, -1.2) = -1.649 (unclipped)."""
+    rewards = np.array([1.0, 0.0])
+    owner = np.zeros((2, 1), np.uint8)
+    old = np.zeros((2, 1))
+    new = np.array([[-0.5], [0.5]])
+    r = grpo_objective(rewards, 2, np.array([1, 1]), owner, new, old)
+    assert r["clip_frac"] == 0.0
+    assert np.allclose(r["token_obj"][:, 0], [np.exp(-0.5) * r["advantages"][0], np.exp(0.5) * r["advantages"][1]], atol=1e-12)
+    # mirrored ratios: both clipped branches are taken
+    r2 = grpo_objective(rewards, 2, np.array([1, 1]), owner, -new, old)
+    assert r2["clip_frac"] == 1.0
+    assert np.allclose(r2["token_obj"][:, 0], [1.2 * r2["advantages"][0], 0.8 * r2["advantages"][1]], atol=1e-12)
