@@ -190,8 +190,8 @@ def class_bytes(shape, cls, rows, kv_bytes_per_layer_launch, emit_rows, n_models
         return g(2 * I, H, rows)
     if cls == "gemm_down":
         return g(H, I, rows)
-    if cls == "gemm_lmhead":
-        return g(V, H, emit_rows)
+    if cls == "gemm_lmhead":   # fused S8: the output is one 32-byte partial per (128-id tile, row), not fp32 logits
+        return n_models * V * H * es + emit_rows * H * es + emit_rows * ((V + 127) // 128) * 32
     if cls == "attention":
         return kv_bytes_per_layer_launch + rows * qd * (4 + es)
     if cls == "rope_append":
@@ -202,8 +202,8 @@ def class_bytes(shape, cls, rows, kv_bytes_per_layer_launch, emit_rows, n_models
         return rows * 2 * I * 4 + rows * I * es
     if cls == "embed_norm":
         return rows * H * (es + 4 + es)
-    if cls == "sample_switch_emit":
-        return emit_rows * V * 4
+    if cls == "sample_switch_emit":   # fused S8: the merge reads the partials
+        return emit_rows * ((V + 127) // 128) * 32
     return 0
 
 
@@ -510,8 +510,10 @@ def run_ours(args):
         rows = (p1["rows_senior"] + p1["rows_junior"] - p0["rows_senior"] - p0["rows_junior"]) / psteps
         emit_rows = (p1["tokens_emitted"] - p0["tokens_emitted"]) / psteps
         kv_launch = (p1["kv_bytes_read"] - p0["kv_bytes_read"]) / psteps / shape.n_layers
-        dup_ms = prof.get("attention_catchup", (0.0, 0))[0]      # the filtered second launch is extra work: not part of a step
-        total_ms = sum(v[0] for v in prof.values()) - dup_ms
+        empty_ms = prof.get("attention_empty", (0.0, 0))[0]     # a launch that finds no item: the fixed cost of the extra launches
+        dup_all = prof.get("attention_catchup", (0.0, 0))[0] + empty_ms   # the filtered launches are extra work: not part of a step
+        dup_ms = max(0.0, prof.get("attention_catchup", (0.0, 0))[0] - empty_ms)
+        total_ms = sum(v[0] for v in prof.values()) - dup_all
         catchup = None
         if args.catchup_share:
             eng.set_option("profile_catchup_attention", 0)
@@ -522,7 +524,8 @@ def run_ours(args):
                        "row_proportional_ms_per_step": by_rows / args.profile_steps, "catchup_rows_per_step": crows, "rows_per_step": rows,
                        "share_of_rows": crows / max(rows, 1e-9),
                        "method": "attention over items with q_len > 1 timed directly (second, filtered launch in the per-kernel pass); "
-                                 "projection / norm / RoPE / combine time apportioned by rows; LM head, sampler, scheduler excluded"}
+                                 "less the time of the same launch with no item at all; projection / norm / RoPE / combine time apportioned by rows; "
+                                 "LM head, sampler, scheduler excluded"}
         for name, (kms, n) in prof.items():
             if n == 0:
                 continue

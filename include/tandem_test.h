@@ -12,7 +12,7 @@ extern "C" {
 /* kernel classes of one step, for launch accounting and tandem_get_profile */
 enum { TANDEM_KC_SCHED = 0, TANDEM_KC_EMBED, TANDEM_KC_GEMM_QKV, TANDEM_KC_ROPE_APPEND, TANDEM_KC_ATTENTION, TANDEM_KC_ATTN_COMBINE,
        TANDEM_KC_GEMM_O, TANDEM_KC_RESIDUAL_NORM, TANDEM_KC_GEMM_GATEUP, TANDEM_KC_SWIGLU, TANDEM_KC_GEMM_DOWN, TANDEM_KC_GEMM_LMHEAD,
-       TANDEM_KC_SAMPLE, TANDEM_KC_FINALIZE, TANDEM_KC_SCORE, TANDEM_KC_ATTN_CATCHUP, TANDEM_KC_NUM };
+       TANDEM_KC_SAMPLE, TANDEM_KC_FINALIZE, TANDEM_KC_SCORE, TANDEM_KC_ATTN_CATCHUP, TANDEM_KC_ATTN_EMPTY, TANDEM_KC_NUM };
 
 /* Per-kernel timing mode (bench.py's roofline leg): while enabled, a step runs un-captured on the caller's stream, every kernel
  * bracketed by CUDA events, and the call returns after the step has finished. Results are unchanged. enable = 1 also zeroes
@@ -23,8 +23,10 @@ int tandem_get_profile(tandem_handle *h, double *ms, int64_t *launches);
 const char *tandem_kernel_class_name(int kc);
 
 /* A/B knob for measurements, by name; call before the first step (a captured step graph is dropped). Names: "pdl" (0/1, default 1),
- * "attn_ctas_per_sm" (1/2), "gemm_ring_kb" (0 = automatic), "profile_catchup_attention" (0/1: in profile mode launch the attention kernel a second time on the
- * catch-up items only - q_len > 1 - as class attention_catchup; results unchanged),  "gemm_pair" (-1 automatic, 0, 1), "score_nosplit" (0/1),
+ * "attn_ctas_per_sm" (1/2), "gemm_ring_kb" (0 = automatic), "fused_sampler" (0 = always materialise the logits and run the
+ * separate sampler kernel; default 1: S8 in the LM head's epilogue when no filter / override / logits tap needs them), "profile_catchup_attention" (0/1: in profile mode launch the attention kernel a second time on the
+ * catch-up items only - q_len > 1 - as class attention_catchup, and a third time with no item at all - class attention_empty, the
+ * fixed cost of such a launch; results unchanged),  "gemm_pair" (-1 automatic, 0, 1), "score_nosplit" (0/1),
  * "score_chunk_grid" (1..16). TANDEM_EINVAL for an unknown name or a value out of range. Every published number uses the defaults. */
 int tandem_test_set_option(tandem_handle *h, const char *name, int32_t value);
 

@@ -19,7 +19,7 @@ EXPORTED_SYMBOLS = ["tandem_init", "tandem_load_weights", "tandem_step", "tandem
                     "tandem_free", "tandem_last_error", "tandem_get_stats", "tandem_set_profile", "tandem_get_profile",
                     "tandem_kernel_class_name", "tandem_test_set_option", "tandem_test_set_page_order", "tandem_test_uniforms", "tandem_test_nucleus", "tandem_test_philox",
                     "tandem_test_gemm", "tandem_test_gemm_time"]
-KC_NUM = 16
+KC_NUM = 17
 
 
 class TandemError(RuntimeError):

@@ -153,6 +153,18 @@ __device__ __forceinline__ float u_switch_counter(unsigned long long seed, int s
 // Gumbel variate from a uniform: E = -log1p(-u) (unit exponential), g = -ln E. Accurate libm calls, not intrinsics.
 __device__ __forceinline__ float gumbel_from_uniform(float u) { return -logf(-log1pf(-u)); }
 
+// Fused S8: what the LM head's epilogue keeps of a range of vocabulary ids for one emitting row (gemm_tcgen05.cuh, kTcEpiSample), and how
+// two ranges combine. Symmetric (a + b == b + a bit for bit), ties go to the lower id: any merge tree gives the same ids, a fixed tree
+// the same sums.
+struct SamplePart { float m, s, gv, gz; int raw_id, g_id; };   // max z, sum exp((z - m) / T), best Gumbel-perturbed value and its z; argmax ids
+__device__ __forceinline__ void sample_part_merge(SamplePart& a, const SamplePart& b, float inv_t) {
+  const float mn = fmaxf(a.m, b.m);
+  const float sa = a.m == -INFINITY ? 0.f : a.s * expf((a.m - mn) * inv_t), sb = b.m == -INFINITY ? 0.f : b.s * expf((b.m - mn) * inv_t);
+  if (b.m > a.m || (b.m == a.m && b.raw_id < a.raw_id)) a.raw_id = b.raw_id;
+  a.m = mn; a.s = sa + sb;
+  if (b.gv > a.gv || (b.gv == a.gv && b.g_id < a.g_id)) { a.gv = b.gv; a.gz = b.gz; a.g_id = b.g_id; }
+}
+
 // ------------------------------------------------------------------------------------------------------------
 // Programmatic dependent launch (PDL): a kernel launched with the attribute may start while its predecessor in the stream
 // is still running; pdl_wait() blocks until the predecessor has completed and its writes are visible, pdl_trigger() lets

@@ -502,6 +502,35 @@ __device__ __forceinline__ ArgBest better(ArgBest a, ArgBest b) {  // larger val
   return (b.v > a.v || (b.v == a.v && b.i < a.i)) ? b : a;
 }
 
+// The tail of S8 for one emitting sequence (slot s, token index t): append y, record owner flag and senior log-prob, then the rule of
+// PAPER.md L61 / Alg. 1 lines 9-15 / L271: EOS or length => done; boundary = word_start[y]; cap counter; the coin decides a_{t+1}.
+__device__ __forceinline__ void emit_token_and_switch(const SampleArgs& a, int s, int t, int sid, int y, float logp, int raw_id) {
+  const int M = a.model;
+  const int n = a.st.n_ctx[s];
+  a.tokens[(size_t)s * a.max_seq_len + n] = y;
+  a.out_owner[(size_t)s * a.max_seq_len + (t - 1)] = (uint8_t)M;
+  a.out_logp[(size_t)s * a.max_seq_len + (t - 1)] = (M == 0) ? logp : 0.f;
+  a.st.n_ctx[s] = n + 1;
+  a.st.n_emit[s] = t;
+  if (a.io.token) a.io.token[s] = y;
+  if (a.io.owner) a.io.owner[s] = (uint8_t)M;
+  if (a.io.sen_logp) a.io.sen_logp[s] = (M == 0) ? logp : 0.f;
+  if (a.io.argmax) a.io.argmax[s] = raw_id;
+  if ((a.rp.eos_id >= 0 && y == a.rp.eos_id) || t >= a.st.max_new[s]) { a.st.done[s] = 1; return; }
+  // the rule: the coin after y_t decides the author of y_{t+1}
+  const bool boundary = a.word_start[y] != 0;
+  int c = boundary ? 0 : a.st.cap_c[s] + 1;
+  int owner = M;
+  if (boundary || (a.rp.cap_k > 0 && c >= a.rp.cap_k)) {
+    const float u = a.io.u_switch ? a.io.u_switch[(size_t)s * a.io.u_switch_stride + t] : u_switch_counter(a.rp.seed, sid, t);
+    const bool hit = u < a.rp.p;
+    owner = (a.rp.switch_mode == 0) ? (hit ? 1 - M : M) : (hit ? 0 : 1);
+    c = 0;
+  }
+  a.st.cap_c[s] = c;
+  a.st.owner[s] = (uint8_t)owner;
+}
+
 // Nucleus (top-p) filtering, then the Gumbel argmax over the kept set (reading R10; off the fast path: a few passes over the
 // L2-resident row by the CTA that merges it). Masses are fixed-point integers (exp(x - m) * 2^40), so every sum is exact and
 // independent of the order of accumulation. Each id has a 24-bit depth T = floor(2^18 * min(log2e * (m - x), 64)), monotone in
@@ -933,31 +962,53 @@ __global__ void __launch_bounds__(NT) sample_switch_emit_kernel(const __grid_con
     const int f = a.io.forced_tokens[(size_t)s * a.io.forced_stride + (t - 1)];
     if (f >= 0 && f < V) y = f;   // an id outside the vocabulary is ignored (it would index the logits and the embedding out of bounds)
   }
-  const float logp = z[y] * invT - (m + logf(sum));
-  const int M = a.model;
-  const int n = a.st.n_ctx[s];
-  a.tokens[(size_t)s * a.max_seq_len + n] = y;
-  a.out_owner[(size_t)s * a.max_seq_len + (t - 1)] = (uint8_t)M;
-  a.out_logp[(size_t)s * a.max_seq_len + (t - 1)] = (M == 0) ? logp : 0.f;
-  a.st.n_ctx[s] = n + 1;
-  a.st.n_emit[s] = t;
-  if (a.io.token) a.io.token[s] = y;
-  if (a.io.owner) a.io.owner[s] = (uint8_t)M;
-  if (a.io.sen_logp) a.io.sen_logp[s] = (M == 0) ? logp : 0.f;
-  if (a.io.argmax) a.io.argmax[s] = raw.i;
-  if ((a.rp.eos_id >= 0 && y == a.rp.eos_id) || t >= a.st.max_new[s]) { a.st.done[s] = 1; return; }
-  // the rule: the coin after y_t decides the author of y_{t+1}
-  const bool boundary = a.word_start[y] != 0;
-  int c = boundary ? 0 : a.st.cap_c[s] + 1;
-  int owner = M;
-  if (boundary || (a.rp.cap_k > 0 && c >= a.rp.cap_k)) {
-    const float u = a.io.u_switch ? a.io.u_switch[(size_t)s * a.io.u_switch_stride + t] : u_switch_counter(a.rp.seed, sid, t);
-    const bool hit = u < a.rp.p;
-    owner = (a.rp.switch_mode == 0) ? (hit ? 1 - M : M) : (hit ? 0 : 1);
-    c = 0;
+  emit_token_and_switch(a, s, t, sid, y, z[y] * invT - (m + logf(sum)), raw.i);
+}
+
+// ============================================================================================ S8, fused path: merge + emit
+// The LM head's epilogue (gemm_tcgen05.cuh, kTcEpiSample) left one SamplePart per (emitting row, 128-id weight tile): [row][tile][8]
+// fp32. One warp per emitting row merges the tiles - each lane its tiles in ascending order (eight loads in flight), then a butterfly over the lanes: a fixed
+// tree, and sample_part_merge is symmetric, so every lane ends with the same bits - and lane 0 applies the rule. The logits never
+// reached HBM: 38 KB of partials per row instead of 608 KB written and read.
+struct SampleMergeArgs { SampleArgs sa; const float* part; int n_tiles; int row_cap; };
+template <int NT>
+__global__ void __launch_bounds__(NT) sample_merge_emit_kernel(const __grid_constant__ Pair<SampleMergeArgs> pp) {
+  pdl_trigger(); pdl_wait();
+  const SampleMergeArgs& ma = pp.m[blockIdx.y];
+  const SampleArgs& a = ma.sa;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int j = blockIdx.x * (NT / 32) + warp;
+  if (j >= a.tab.counts[C_EMIT]) return;
+  const bool greedy = !(a.rp.temperature > 0.f);
+  const float invT = greedy ? 1.f : 1.f / a.rp.temperature;
+  SamplePart acc{-INFINITY, 0.f, -INFINITY, 0.f, 0x7fffffff, 0x7fffffff};
+  const float4* row = reinterpret_cast<const float4*>(ma.part + (size_t)j * ma.n_tiles * 8);
+  for (int t0 = lane; t0 < ma.n_tiles; t0 += 8 * 32) {
+    float4 p0[8], p1[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+      const int t = t0 + 32 * k;
+      p0[k] = make_float4(-INFINITY, 0.f, __int_as_float(0x7fffffff), -INFINITY); p1[k] = make_float4(__int_as_float(0x7fffffff), 0.f, 0.f, 0.f);
+      if (t < ma.n_tiles) { p0[k] = __ldcg(row + 2 * t); p1[k] = __ldcg(row + 2 * t + 1); }
+    }
+#pragma unroll
+    for (int k = 0; k < 8; ++k)
+      sample_part_merge(acc, SamplePart{p0[k].x, p0[k].y, p0[k].w, p1[k].y, __float_as_int(p0[k].z), __float_as_int(p1[k].x)}, invT);
   }
-  a.st.cap_c[s] = c;
-  a.st.owner[s] = (uint8_t)owner;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    SamplePart b;
+    b.m = __shfl_xor_sync(0xffffffffu, acc.m, o); b.s = __shfl_xor_sync(0xffffffffu, acc.s, o);
+    b.gv = __shfl_xor_sync(0xffffffffu, acc.gv, o); b.gz = __shfl_xor_sync(0xffffffffu, acc.gz, o);
+    b.raw_id = __shfl_xor_sync(0xffffffffu, acc.raw_id, o); b.g_id = __shfl_xor_sync(0xffffffffu, acc.g_id, o);
+    sample_part_merge(acc, b, invT);
+  }
+  if (lane != 0) return;
+  const int s = a.tab.emit_slot[j];
+  const int t = a.st.n_emit[s] + 1;
+  const int y = greedy ? acc.raw_id : acc.g_id;
+  const float zy = greedy ? acc.m : acc.gz;
+  emit_token_and_switch(a, s, t, a.st.seq_id[s], y, zy * invT - (acc.m * invT + logf(acc.s)), acc.raw_id);
 }
 
 // ============================================================================================ dual scoring (NEXT-1)

@@ -45,6 +45,7 @@ struct Workspace {  // per model, sized for row_cap rows
   float* logits = nullptr;     // [max_seqs, V]
   void* score_lm_in = nullptr; float* score_logits = nullptr;   // tandem_score: [row_cap, H] and [row_cap, V], allocated at its first call
   float* chunk_part = nullptr; int32_t* chunk_ctr = nullptr;   // sampler: per-slice partials and arrival counters
+  float* spart = nullptr;      // fused S8: the LM head's per-(row, weight tile) sampling partials [max_seqs][V / 128][8]
   float* part_acc = nullptr; float2* part_ml = nullptr;
   void* kv = nullptr;          // page pool: [layer][K|V][page][nkv][16][d]
   int32_t* tab_mem = nullptr;  // backing store of the StepTab arrays
@@ -76,6 +77,7 @@ struct tandem_handle {
   bool score_nosplit = true;
   int score_chunk_grid = 8;                      // scoring: CTAs per (weight tile, K split) along the token rows (1 = off)
   bool use_pdl = true;                          // programmatic dependent launch along the kernel chain
+  bool fused_sampler = true;                    // S8 in the LM head's epilogue whenever the sampler needs no materialised logits
   size_t gemm_out_cols = 0;
   ModelWeights w[2];
   Workspace ws[2];
@@ -160,14 +162,15 @@ cudaEvent_t prof_event(tandem_handle* h) {
 // read from rows_ptr[m] on the device.
 template <typename T>
 int launch_gemm(tandem_handle* h, int which, const void* const* A, const void* const* W, int N, int K, float* const* out,
-                const int32_t* const* rows_ptr, int rows_cap, int* n_split, size_t* split_stride, cudaStream_t s, int epi = kTcEpiPartial) {
+                const int32_t* const* rows_ptr, int rows_cap, int* n_split, size_t* split_stride, cudaStream_t s, int epi = kTcEpiPartial,
+                const TcSampleCfg* sample = nullptr) {
   const int nm = 2;
   *n_split = 1;
   *split_stride = (size_t)rows_cap * N;
   static const int cls_of[5] = {TANDEM_KC_GEMM_QKV, TANDEM_KC_GEMM_O, TANDEM_KC_GEMM_GATEUP, TANDEM_KC_GEMM_DOWN, TANDEM_KC_GEMM_LMHEAD};
   if (h->gemm_impl == TANDEM_GEMM_TCGEN05 && sizeof(T) == 2) {
     int rc = 0;
-    TcGemmTune tune; tune.ring_kb = h->gemm_ring_kb; tune.pdl = h->use_pdl; tune.n_sms = h->n_sms;
+    TcGemmTune tune; tune.ring_kb = h->gemm_ring_kb; tune.pdl = h->use_pdl; tune.n_sms = h->n_sms; tune.sample = sample;
  tune.pair = h->gemm_pair >= 0 ? h->gemm_pair : (h->scoring ? 1 : 0);
     if (h->scoring && which != 4) {
       tune.chunk_grid = h->score_chunk_grid;   // hundreds of rows per launch: one CTA per 256-row chunk
@@ -298,6 +301,9 @@ int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaS
           // with more than one query token (S5b); it rewrites the same values, so results are unchanged
           for (int m = 0; m < 2; ++m) { ma.m[m].min_ntok = 2; ma.m[m].work_ctr = h->work_ctr + c.n_layers + l; }
           KL(h, TANDEM_KC_ATTN_CATCHUP, s, ok = run_attn_mma(maps, ma, d, nq / nkv, h->attn_ctas_per_sm * h->n_sms, s, false, pdl));
+          // and once more with every item filtered out: the fixed cost of such a launch, to be subtracted
+          for (int m = 0; m < 2; ++m) { ma.m[m].min_ntok = 1 << 30; ma.m[m].work_ctr = h->work_ctr + 2 * c.n_layers + l; }
+          KL(h, TANDEM_KC_ATTN_EMPTY, s, ok = ok && run_attn_mma(maps, ma, d, nq / nkv, h->attn_ctas_per_sm * h->n_sms, s, false, pdl));
         }
       } else {
         Pair<AttnArgs<T>> aa;
@@ -359,6 +365,21 @@ int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaS
     return TANDEM_OK;
   }
   // S8 LM head on the emitting rows only, then sample + switch + emit
+  const bool want_nucleus = rp.temperature > 0.f && (rp.top_p < 1.f || (rp.top_k > 0 && rp.top_k < V));
+  if (h->fused_sampler && h->gemm_impl == TANDEM_GEMM_TCGEN05 && sizeof(T) == 2 && !want_nucleus && !io.u_sample && !io.dbg_logits && !io.forced_tokens) {
+    // the default sampling path: (max, sum exp, argmax, Gumbel-max) are reduced in the LM head's epilogue per 128-id weight tile and merged
+    // by one warp per row - no [rows, V] logits in HBM. Filters, explicit uniforms, forced tokens and the logits tap need the logits.
+    const bool greedy = !(rp.temperature > 0.f);
+    const TcSampleCfg sc{{h->tab[0].emit_slot, h->tab[1].emit_slot}, h->st.n_emit, h->st.seq_id, greedy ? 1.f : 1.f / rp.temperature, greedy ? 1 : 0, rp.seed};
+    for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].lm_in, h->w[m].lm_head, h->ws[m].spart, h->tab[m].counts + C_EMIT);
+    if ((rc = launch_gemm<T>(h, 4, A, W, V, H, O, RP, c.max_seqs, &ns, &ss, s, kTcEpiSample, &sc))) return rc;
+    Pair<SampleMergeArgs> sm;
+    for (int m = 0; m < 2; ++m)
+      sm.m[m] = SampleMergeArgs{SampleArgs{h->st, h->tab[m], io, rp, nullptr, h->word_start_dev, h->tokens, h->out_owner, h->out_logp, V, c.max_seq_len, m, nullptr, nullptr, 0},
+                                h->ws[m].spart, (V + kTcTileN - 1) / kTcTileN, c.max_seqs};
+    KL(h, TANDEM_KC_SAMPLE, s, launch_ex(sample_merge_emit_kernel<128>, dim3((c.max_seqs + 3) / 4, 2), dim3(128), 0, s, pdl, sm));
+    return TANDEM_OK;
+  }
   for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].lm_in, h->w[m].lm_head, h->ws[m].logits, h->tab[m].counts + C_EMIT);
   if ((rc = launch_gemm<T>(h, 4, A, W, V, H, O, RP, c.max_seqs, &ns, &ss, s))) return rc;
   Pair<SampleArgs> sa;
@@ -366,7 +387,7 @@ int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaS
   for (int m = 0; m < 2; ++m)
     sa.m[m] = SampleArgs{h->st, h->tab[m], io, rp, h->ws[m].logits, h->word_start_dev, h->tokens, h->out_owner, h->out_logp, V, c.max_seq_len, m,
                          h->ws[m].chunk_part, h->ws[m].chunk_ctr, n_chunk};
-  const size_t nucleus_smem = (rp.temperature > 0.f && (rp.top_p < 1.f || (rp.top_k > 0 && rp.top_k < V))) ? sizeof(NucleusSmem<256>) : 0;
+  const size_t nucleus_smem = want_nucleus ? sizeof(NucleusSmem<256>) : 0;
   if (nucleus_smem) KL(h, TANDEM_KC_SAMPLE, s, launch_ex(sample_switch_emit_kernel<256, true>, dim3(c.max_seqs, n_chunk, 2), dim3(256), nucleus_smem, s, pdl, sa));
   else KL(h, TANDEM_KC_SAMPLE, s, launch_ex(sample_switch_emit_kernel<256, false>, dim3(c.max_seqs, n_chunk, 2), dim3(256), 0, s, pdl, sa));
   return TANDEM_OK;
@@ -378,7 +399,7 @@ int launch_step(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaSt
   sa.st = h->st; sa.pt[0] = h->pt[0]; sa.pt[1] = h->pt[1]; sa.gt = h->gt; sa.tab[0] = h->tab[0]; sa.tab[1] = h->tab[1];
   sa.io = io; sa.stats = h->stats; sa.tokens = h->tokens; sa.max_seqs = c.max_seqs; sa.max_seq_len = c.max_seq_len;
   sa.max_pages = h->max_pages; sa.row_cap = h->row_cap; sa.tile_tok = h->tile_tok;
-  sa.work_ctr = h->work_ctr; sa.n_work_ctr = 2 * c.n_layers;
+  sa.work_ctr = h->work_ctr; sa.n_work_ctr = 3 * c.n_layers;
   sa.score = score ? 1 : 0; sa.oom_flag = h->oom_dev;
   KL(h, TANDEM_KC_SCHED, s, (sched_kernel<<<1, 1024, 0, s>>>(sa)));
   const int rc = (c.dtype == TANDEM_F32) ? forward_pair<float>(h, io, rp, s, score, score_inv_t) : forward_pair<bf16>(h, io, rp, s, score, score_inv_t);
@@ -676,8 +697,8 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
     int dev_sms = 0;
     if (cudaDeviceGetAttribute(&dev_sms, cudaDevAttrMultiProcessorCount, c.device) == cudaSuccess && dev_sms > 0) h->n_sms = dev_sms;
   }
-  INIT_TRY(dmalloc(h, &h->work_ctr, (size_t)2 * c.n_layers * 4));   // [L] attention work counters, [L] for the profile mode's catch-up-only launch
-  INIT_CU(cudaMemset(h->work_ctr, 0, (size_t)2 * c.n_layers * 4));
+  INIT_TRY(dmalloc(h, &h->work_ctr, (size_t)3 * c.n_layers * 4));   // [L] attention work counters, 2 x [L] for the profile mode's filtered launches
+  INIT_CU(cudaMemset(h->work_ctr, 0, (size_t)3 * c.n_layers * 4));
   INIT_CU(cudaHostAlloc((void**)&h->oom_host, 4, cudaHostAllocMapped));
   *h->oom_host = 0;
   INIT_CU(cudaHostGetDevicePointer((void**)&h->oom_dev, h->oom_host, 0));
@@ -724,6 +745,7 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
     INIT_TRY(dmalloc(h, &w.gemm_out, (size_t)R * cols * 4));
     INIT_TRY(dmalloc(h, &w.logits, (size_t)S * V * 4));
     INIT_TRY(dmalloc(h, &w.chunk_part, (size_t)S * kSampleMaxChunks * 6 * 4));
+    if (h->gemm_impl == TANDEM_GEMM_TCGEN05) INIT_TRY(dmalloc(h, &w.spart, (size_t)((V + kTcTileN - 1) / kTcTileN) * S * kTcSampleVals * 4));
     INIT_TRY(dmalloc(h, &w.chunk_ctr, (size_t)S * 4));
     INIT_CU(cudaMemset(w.chunk_ctr, 0, (size_t)S * 4));
     INIT_TRY(dmalloc(h, &w.part_acc, (size_t)h->part_cap * nq * d * 4));
@@ -849,7 +871,7 @@ int tandem_get_profile(tandem_handle* h, double* ms, int64_t* launches) {
 
 const char* tandem_kernel_class_name(int kc) {
   static const char* names[TANDEM_KC_NUM] = {"sched", "embed_norm", "gemm_qkv", "rope_append", "attention", "attn_combine", "gemm_o",
-                                             "residual_norm", "gemm_gateup", "swiglu", "gemm_down", "gemm_lmhead", "sample_switch_emit", "finalize", "score", "attention_catchup"};
+                                             "residual_norm", "gemm_gateup", "swiglu", "gemm_down", "gemm_lmhead", "sample_switch_emit", "finalize", "score", "attention_catchup", "attention_empty"};
   return (kc >= 0 && kc < TANDEM_KC_NUM) ? names[kc] : "?";
 }
 
@@ -1173,7 +1195,7 @@ void tandem_free(tandem_handle* h) {
   auto fr = [](void* p) { if (p) cudaFree(p); };
   for (int m = 0; m < 2; ++m) {
     Workspace& w = h->ws[m];
-    fr(w.score_lm_in); fr(w.score_logits); fr(w.chunk_part); fr(w.chunk_ctr); fr(w.x); fr(w.act); fr(w.q); fr(w.attn_out); fr(w.mlp_act); fr(w.lm_in); fr(w.gemm_out); fr(w.logits); fr(w.part_acc); fr(w.part_ml); fr(w.kv);
+    fr(w.score_lm_in); fr(w.score_logits); fr(w.spart); fr(w.chunk_part); fr(w.chunk_ctr); fr(w.x); fr(w.act); fr(w.q); fr(w.attn_out); fr(w.mlp_act); fr(w.lm_in); fr(w.gemm_out); fr(w.logits); fr(w.part_acc); fr(w.part_ml); fr(w.kv);
     fr(w.tab_mem); fr(w.bt); fr(w.npages); fr(w.free_pages); fr(w.free_top);
     ModelWeights& mw = h->w[m];
     fr(mw.embed); fr(mw.lm_head); fr(mw.final_norm);
@@ -1264,6 +1286,7 @@ int tandem_test_set_option(tandem_handle* h, const char* name, int32_t value) {
   if (n == "pdl" && in(0, 1)) h->use_pdl = value != 0;
   else if (n == "attn_ctas_per_sm" && in(1, 2)) h->attn_ctas_per_sm = value;
   else if (n == "gemm_ring_kb" && in(0, 200)) h->gemm_ring_kb = value;
+  else if (n == "fused_sampler" && in(0, 1)) h->fused_sampler = value != 0;
   else if (n == "profile_catchup_attention" && in(0, 1)) h->profile_catchup_attn = value != 0;
   else return fail(h, TANDEM_EINVAL, "unknown option or value out of range: " + n);
   CU(h, cudaDeviceSynchronize());
