@@ -16,7 +16,7 @@ ATTN_AUTO, ATTN_ALU, ATTN_MMA = 0, 1, 2
 _ERR = {0: "OK", -1: "EINVAL", -2: "ENOMEM", -3: "ECUDA", -4: "ESTATE", -5: "EFULL"}
 
 EXPORTED_SYMBOLS = ["tandem_init", "tandem_load_weights", "tandem_step", "tandem_generate", "tandem_score", "tandem_grpo_objective", "tandem_reset",
-                    "tandem_free", "tandem_last_error", "tandem_get_stats", "tandem_set_profile", "tandem_get_profile",
+                    "tandem_free", "tandem_last_error", "tandem_get_stats", "tandem_evict", "tandem_set_profile", "tandem_get_profile",
                     "tandem_kernel_class_name", "tandem_test_set_option", "tandem_test_set_page_order", "tandem_test_uniforms", "tandem_test_nucleus", "tandem_test_philox",
                     "tandem_test_gemm", "tandem_test_gemm_time"]
 KC_NUM = 17
@@ -90,6 +90,7 @@ def lib():
                                       C.POINTER(_Overrides), C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                       C.POINTER(_Stats), C.c_void_p]
         L.tandem_reset.argtypes = [C.c_void_p]
+        L.tandem_evict.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
         L.tandem_get_stats.argtypes = [C.c_void_p, C.POINTER(_Stats)]
         L.tandem_set_profile.argtypes = [C.c_void_p, C.c_int]
         L.tandem_get_profile.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
@@ -240,6 +241,10 @@ class Tandem:
 
     def reset(self):
         self._check(lib().tandem_reset(self._h))
+
+    def evict(self, slot, stream=None):
+        """Remove the sequence in `slot` (pages back to the pools, slot free): resolves a stall / dead lock for tandem_step callers."""
+        self._check(lib().tandem_evict(self._h, int(slot), stream))
 
     def get_stats(self):
         st = _Stats()

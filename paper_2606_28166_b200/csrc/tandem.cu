@@ -939,6 +939,20 @@ int tandem_step(tandem_handle* h, const tandem_step_in* in, tandem_step_out* out
   return run_step(h, make_io(out, in->ovr), make_rule(in->params), s);
 }
 
+int tandem_evict(tandem_handle* h, int32_t slot, void* cuda_stream) {
+  if (!h) return TANDEM_EINVAL;
+  if (h->cuda_fault) return fail(h, TANDEM_ECUDA, "a previous CUDA error is sticky: " + h->err);
+  if (slot < 0 || slot >= h->cfg.max_seqs) return fail(h, TANDEM_EINVAL, "slot out of range");
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  int rc = refresh_slots(h, s);
+  if (rc) return rc;
+  if (!h->slot_busy[slot]) return fail(h, TANDEM_EINVAL, "slot holds no sequence");
+  if ((rc = preempt_slot(h, slot, s))) return rc;
+  if (h->oom_host) *h->oom_host = 0;             // pages came back: a stall or dead lock reported so far is history
+  CU(h, cudaMemset(&h->stats->err_oom, 0, sizeof(int)));
+  return TANDEM_OK;
+}
+
 int tandem_generate(tandem_handle* h, const tandem_params* params, int32_t B, const int32_t* prompt_tokens, const int64_t* prompt_offsets,
                     const int32_t* max_new, const int32_t* seq_ids, const tandem_overrides* ovr, int32_t out_stride, int32_t* out_tokens,
                     uint8_t* out_owner, float* out_sen_logp, int32_t* out_len, tandem_stats* stats, void* cuda_stream) {

@@ -257,6 +257,25 @@ def test_step_stalls_on_an_empty_pool_and_reports_the_dead_lock():
     for b in range(B):                                       # everything emitted before the stall is right
         assert len(got[b]) > 0 and got[b] == [int(x) for x in ref["tokens"][b][:len(got[b])]]
     assert sum(len(g) for g in got) < 3 * 100
+    # tandem_evict gives the pages of one sequence back: the others move again and stay on the oracle's token streams
+    eng.evict(2)
+    before = [len(g) for g in got]
+    for t in range(40):
+        try:
+            eng.step(prm, out=o)
+        except T.TandemError:
+            break
+        torch.cuda.synchronize()
+        tok = o["token"].cpu().numpy()
+        assert tok[2] < 0
+        for b in range(2):
+            if tok[b] >= 0:
+                got[b].append(int(tok[b]))
+    assert len(got[0]) + len(got[1]) > before[0] + before[1]
+    for b in range(2):
+        assert got[b] == [int(x) for x in ref["tokens"][b][:len(got[b])]]
+    with pytest.raises(T.TandemError):
+        eng.evict(2)                                          # the slot is empty now
     eng.reset()
     out = eng.generate(prm, [prompts[0]], [20])
     assert np.array_equal(out["tokens"][0, :20], ref["tokens"][0][:20])
