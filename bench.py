@@ -48,6 +48,7 @@ def parse_args():
     ap.add_argument("--grpo", action="store_true", help="time tandem_grpo_objective (senior-masked GRPO forward, NEXT-3) on the workload's batch x max_new")
     ap.add_argument("--score", type=int, default=0, help="N > 0: time tandem_score (teacher-forced dual scoring, NEXT-1) on N synthetic streams instead of the rollout")
     ap.add_argument("--score-len", type=int, default=2048, help="tokens per stream for --score")
+    ap.add_argument("--attn-prefill-tc", type=int, default=1, help="--score: 0 = attention on the mma.sync kernel of the rollout instead of the tcgen05 kernel (A/B)")
     ap.add_argument("--score-rows", type=int, default=2048, help="rows per step and model for --score (max_rows_per_step)")
     ap.add_argument("--top-k", type=int, default=0, help="top-k filter of the sampler (0 = off; the paper evaluates with 20)")
     ap.add_argument("--temperature", type=float, default=None, help="override the workload's sampling temperature")
@@ -338,6 +339,8 @@ def run_score(args):
     eng = T.Tandem(T.TandemConfig(shape, max_seqs=max_seqs, max_seq_len=(L + 15) // 16 * 16, kv_bytes_per_model=kv, max_rows_per_step=args.score_rows))
     for m, seed in enumerate((wl.seeds["senior"], wl.seeds["junior"])):
         w = make_weights(shape, seed, device="cuda"); eng.load_weights(m, w); del w; torch.cuda.empty_cache()
+    if not args.attn_prefill_tc:
+        eng.set_option("attn_prefill_tc", 0)
     eng.score(streams[:min(N, 2)])                       # warm-up: buffers, tensor maps
     t0 = time.perf_counter()
     out = eng.score(streams)
@@ -360,7 +363,7 @@ def run_score(args):
                       "steps": int(st["steps"]), "warmup": 1, "ms_per_step": dt / max(1, st["steps"]) * 1e3, "higher_is_better": True, "scaling": "weak",
                       "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
                       "config": {"workload": wl.name, "mode": "tandem_score (host buffers)", "streams": N, "tokens_per_stream": L,
-                                 "rows_per_step_and_model": args.score_rows, "seconds": dt, "mean_alpha": alpha, "junior_cross_entropy": ce},
+                                 "rows_per_step_and_model": args.score_rows, "attention": "tcgen05" if args.attn_prefill_tc else "mma.sync", "seconds": dt, "mean_alpha": alpha, "junior_cross_entropy": ce},
                       "gpu_launches": int(st["kernel_launches"]), "kernels": kernels,
                       "step_roofline": {"tensor_tflops": flops / dt / 1e12, "tensor_peak": pk.get("bf16_tflops_sustained", pk.get("bf16_tflops")),
                                         "weights_gbs": wbytes / dt / 1e9, "hbm_peak": pk["hbm_gbs"]},

@@ -27,7 +27,8 @@ const char *tandem_kernel_class_name(int kc);
  * separate sampler kernel; default 1: S8 in the LM head's epilogue when no filter / override / logits tap needs them), "profile_catchup_attention" (0/1: in profile mode launch the attention kernel a second time on the
  * catch-up items only - q_len > 1 - as class attention_catchup, and a third time with no item at all - class attention_empty, the
  * fixed cost of such a launch; results unchanged),  "gemm_pair" (-1 automatic, 0, 1), "score_nosplit" (0/1),
- * "score_chunk_grid" (1..16). TANDEM_EINVAL for an unknown name or a value out of range. Every published number uses the defaults. */
+ * "score_chunk_grid" (1..16), "attn_prefill_tc" (0 = tandem_score runs its attention on the mma.sync kernel of the rollout; default 1:
+ * the tcgen05 kernel over 128-row q-tiles, csrc/attention_tcgen05.cuh). TANDEM_EINVAL for an unknown name or a value out of range. Every published number uses the defaults. */
 int tandem_test_set_option(tandem_handle *h, const char *name, int32_t value);
 
 /* Parity tests at realistic page numbers: seed != 0 makes tandem_reset (and so tandem_generate / tandem_score) hand the pages of each

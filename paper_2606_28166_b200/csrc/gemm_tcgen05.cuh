@@ -583,6 +583,17 @@ inline const CUtensorMap* tc_gemm_map(TcGemmPlans* p, const void* base, int n_ro
   return &(p->maps[key] = m);
 }
 
+// Descriptor of a q buffer [n_rows][n_heads][D] bf16 in boxes of tok_box tokens x G heads x 64 elements (one 64-dim half of an attention
+// q-tile whose rows are (token, head of the group) pairs), 128-byte swizzle; rows beyond n_rows read as zero.
+inline bool tc_map_q3d(TcGemmPlans* p, CUtensorMap* out, const void* base, int D, int n_heads, int n_rows, int G, int tok_box) {
+  const cuuint64_t dims[3] = {(cuuint64_t)D, (cuuint64_t)n_heads, (cuuint64_t)n_rows};
+  const cuuint64_t strides[2] = {(cuuint64_t)D * 2, (cuuint64_t)n_heads * D * 2};
+  const cuuint32_t box[3] = {64u, (cuuint32_t)G, (cuuint32_t)tok_box};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  return p->encode(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                   CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 // Launch on `s`. out receives *n_split partials, *split_stride floats apart (epi = kTcEpiPartial), or the bf16 SwiGLU
 // activations [rows, N/2] (epi = kTcEpiSwiGLU; W rows interleaved gate/up). Returns 0, or -1 (TANDEM_EINVAL) / -3 (TANDEM_ECUDA).
 // which == 4 (LM head) never splits: the sampler reads the logits in place.

@@ -16,6 +16,7 @@ struct SchedArgs {
   const int32_t* tokens; int max_seqs, max_seq_len, max_pages, row_cap, tile_tok;
   int32_t* work_ctr; int n_work_ctr;   // dynamic-scheduling counters of the attention launches of this step
   int score;                           // teacher-forced dual scoring (tandem_score): both models ingest every sequence, every row reaches the LM head
+  int no_parts;                        // tcgen05 scoring attention: every q-tile covers its whole causal KV range (no KV splits, no combine)
   int32_t* oom_flag;                   // mapped host word, set when a pool runs dry (the host reads it without synchronising)
 };
 
@@ -137,7 +138,7 @@ __global__ void __launch_bounds__(1024) sched_kernel(SchedArgs a) {
     const int kv_len = ing + rows;
     const int n_qt = (rows + a.tile_tok - 1) / a.tile_tok;
     const int chunk = attn_chunk(kv_len);
-    const bool use_parts = rows > 0 && n_qt <= kAttnSplitTiles && kv_len > chunk;
+    const bool use_parts = rows > 0 && n_qt <= kAttnSplitTiles && kv_len > chunk && !a.no_parts;
     int items = rows > 0 ? n_qt : 0, parts = 0;
     if (use_parts) {
       items = 0;

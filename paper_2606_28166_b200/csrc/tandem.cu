@@ -19,6 +19,7 @@
 #include "kernels.cuh"
 #include "attention.cuh"
 #include "attention_mma.cuh"
+#include "attention_tcgen05.cuh"
 #include "gemm_simt.cuh"
 #include "gemm_tcgen05.cuh"
 #include "grpo.cuh"
@@ -77,6 +78,7 @@ struct tandem_handle {
   bool score_nosplit = true;
   int score_chunk_grid = 8;                      // scoring: CTAs per (weight tile, K split) along the token rows (1 = off)
   bool use_pdl = true;                          // programmatic dependent launch along the kernel chain
+  bool attn_prefill_tc = true;                  // tandem_score: tcgen05 attention over 128-row q-tiles (attention_tcgen05.cuh); false = the mma.sync kernel
   bool fused_sampler = true;                    // S8 in the LM head's epilogue whenever the sampler needs no materialised logits
   size_t gemm_out_cols = 0;
   ModelWeights w[2];
@@ -105,6 +107,8 @@ struct tandem_handle {
   cudaGraphExec_t graph = nullptr; GraphKey gkey;
   TcGemmPlans* tc = nullptr;
   CUtensorMap kv_map_store[2];
+  CUtensorMap q_map_store[2];                          // each model's q buffer as [row][q-head][head_dim] in boxes of one q-tile (tcgen05 attention)
+  bool q_map_ok = false;
   const CUtensorMap* kv_map[2] = {nullptr, nullptr};   // each model's whole KV pool as rows of head_dim bf16 (tensor-core attention)
   // launch accounting and the optional per-kernel-class timing mode (tandem_set_profile)
   int64_t launches = 0, graph_launches = 0, preemptions = 0;
@@ -234,6 +238,19 @@ bool run_attn_mma(const Pair<CUtensorMap>& map, const Pair<AttnMmaArgs>& a, int 
 #undef TD_CASE
   return false;
 }
+// tcgen05 attention for scoring (attention_tcgen05.cuh): set_attr = true raises the dynamic shared memory limit only
+bool run_attn_tc(const Pair<CUtensorMap>& kv, const Pair<CUtensorMap>& q, const Pair<AttnMmaArgs>& a, int D, int G, int grid, cudaStream_t s, bool set_attr, bool pdl = false) {
+  if (D == 128) {
+    if (set_attr) return cudaFuncSetAttribute(prefill_attention_tc_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_tc_smem_bytes<128>()) == cudaSuccess;
+    return launch_ex(prefill_attention_tc_kernel<128>, dim3(grid), dim3(kAtThreads), attn_tc_smem_bytes<128>(), s, pdl, kv, q, a, G) == cudaSuccess;
+  }
+  if (D == 64) {
+    if (set_attr) return cudaFuncSetAttribute(prefill_attention_tc_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_tc_smem_bytes<64>()) == cudaSuccess;
+    return launch_ex(prefill_attention_tc_kernel<64>, dim3(grid), dim3(kAtThreads), attn_tc_smem_bytes<64>(), s, pdl, kv, q, a, G) == cudaSuccess;
+  }
+  return false;
+}
+bool use_attn_tc(const tandem_handle* h) { return h->attn_prefill_tc && h->attn_impl == TANDEM_ATTN_MMA && h->q_map_ok; }
 bool attn_supported(int dtype, int D, int G) {
   if (dtype == TANDEM_F32) return (D == 32 || D == 64 || D == 128) && (G == 1 || G == 2 || G == 4);
   return (D == 64 && (G == 1 || G == 2 || G == 4 || G == 7 || G == 8)) || (D == 128 && (G == 1 || G == 2 || G == 4 || G == 8));
@@ -295,6 +312,10 @@ int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaS
                                 (int)((2ll * l) * rows_per_half), (int)((2ll * l + 1) * rows_per_half), h->work_ctr + l, 0};
           maps.m[m] = h->kv_map_store[m];
         }
+        if (score && use_attn_tc(h)) {
+          Pair<CUtensorMap> qm; qm.m[0] = h->q_map_store[0]; qm.m[1] = h->q_map_store[1];
+          KL(h, TANDEM_KC_ATTENTION, s, ok = run_attn_tc(maps, qm, ma, d, nq / nkv, 2 * h->n_sms, s, false, pdl));
+        } else
         KL(h, TANDEM_KC_ATTENTION, s, ok = run_attn_mma(maps, ma, d, nq / nkv, h->attn_ctas_per_sm * h->n_sms, s, false, pdl));
         if (ok && h->profile && h->profile_catchup_attn) {
           // measurement (BASELINE.json configs[4], "catch-up-prefill share of step time"): the same launch again, restricted to the items
@@ -399,6 +420,7 @@ int launch_step(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaSt
   sa.st = h->st; sa.pt[0] = h->pt[0]; sa.pt[1] = h->pt[1]; sa.gt = h->gt; sa.tab[0] = h->tab[0]; sa.tab[1] = h->tab[1];
   sa.io = io; sa.stats = h->stats; sa.tokens = h->tokens; sa.max_seqs = c.max_seqs; sa.max_seq_len = c.max_seq_len;
   sa.max_pages = h->max_pages; sa.row_cap = h->row_cap; sa.tile_tok = h->tile_tok;
+  if (score && use_attn_tc(h)) { sa.tile_tok = kAtTileKv / (c.n_q_heads / c.n_kv_heads); sa.no_parts = 1; }   // 128-row q-tiles, each over its whole causal range
   sa.work_ctr = h->work_ctr; sa.n_work_ctr = 3 * c.n_layers;
   sa.score = score ? 1 : 0; sa.oom_flag = h->oom_dev;
   KL(h, TANDEM_KC_SCHED, s, (sched_kernel<<<1, 1024, 0, s>>>(sa)));
@@ -806,6 +828,14 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
       if (!mp) { h->err = "tensor map encode failed for the KV pool"; fprintf(stderr, "tandem_init: %s\n", h->err.c_str()); tandem_free(h); return TANDEM_ECUDA; }
       h->kv_map_store[m] = *mp;
       h->kv_map[m] = &h->kv_map_store[m];
+    }
+    {  // tcgen05 attention for scoring: q-tile boxes of 128 / G tokens x G heads x 64 dims; unsupported shapes keep the mma.sync kernel
+      const int G = nq / nkv;
+      Pair<AttnMmaArgs> dummy{}; Pair<CUtensorMap> dmaps{};
+      bool ok = (d == 64 || d == 128) && G >= 1 && G <= 16 && run_attn_tc(dmaps, dmaps, dummy, d, G, 1, 0, true);
+      for (int m = 0; m < 2 && ok; ++m) ok = tc_map_q3d(h->tc, &h->q_map_store[m], h->ws[m].q, d, nq, h->row_cap, G, kAtTileKv / G);
+      if (!ok) cudaGetLastError();
+      h->q_map_ok = ok;
     }
     Pair<AttnMmaArgs> dummy{}; Pair<CUtensorMap> dmaps{};
     if (!run_attn_mma(dmaps, dummy, d, nq / nkv, 1, 0, true)) {
@@ -1301,6 +1331,7 @@ int tandem_test_set_option(tandem_handle* h, const char* name, int32_t value) {
   else if (n == "attn_ctas_per_sm" && in(1, 2)) h->attn_ctas_per_sm = value;
   else if (n == "gemm_ring_kb" && in(0, 200)) h->gemm_ring_kb = value;
   else if (n == "fused_sampler" && in(0, 1)) h->fused_sampler = value != 0;
+  else if (n == "attn_prefill_tc" && in(0, 1)) h->attn_prefill_tc = value != 0;
   else if (n == "profile_catchup_attention" && in(0, 1)) h->profile_catchup_attn = value != 0;
   else return fail(h, TANDEM_EINVAL, "unknown option or value out of range: " + n);
   CU(h, cudaDeviceSynchronize());
