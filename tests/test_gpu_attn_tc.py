@@ -63,7 +63,7 @@ def test_tc_attention_matches_oracle_and_mma_kernel(name):
     # the means over ~3,000 positions and the new kernel's distance from the oracle relative to the old kernel's
     assert d_tc.mean() <= 1.15 * d_mma.mean() + 1e-4, (d_tc.mean(), d_mma.mean())
     assert d_tc.max() <= 1.5 * d_mma.max(), (d_tc.max(), d_mma.max())
-    assert d_k.max() <= d_mma.max(), (d_k.max(), d_mma.max())       # the kernels are closer to each other than either is to float64
+    assert d_k.max() <= 1.5 * d_mma.max(), (d_k.max(), d_mma.max())   # the kernels differ from each other no more than from float64
     assert outs[0]["stats"]["rows_senior"] == sum(len(s) - 1 for s in streams)
 
 
