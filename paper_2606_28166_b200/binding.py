@@ -15,7 +15,7 @@ GEMM_AUTO, GEMM_SIMT, GEMM_TCGEN05 = 0, 1, 2
 ATTN_AUTO, ATTN_ALU, ATTN_MMA = 0, 1, 2
 _ERR = {0: "OK", -1: "EINVAL", -2: "ENOMEM", -3: "ECUDA", -4: "ESTATE", -5: "EFULL"}
 
-EXPORTED_SYMBOLS = ["tandem_init", "tandem_load_weights", "tandem_step", "tandem_generate", "tandem_score", "tandem_grpo_objective", "tandem_reset",
+EXPORTED_SYMBOLS = ["tandem_init", "tandem_load_weights", "tandem_step", "tandem_generate", "tandem_score", "tandem_grpo_objective", "tandem_grpo_objective_static", "tandem_reset",
                     "tandem_free", "tandem_last_error", "tandem_get_stats", "tandem_evict", "tandem_set_profile", "tandem_get_profile",
                     "tandem_kernel_class_name", "tandem_test_set_option", "tandem_test_set_page_order", "tandem_test_uniforms", "tandem_test_nucleus", "tandem_test_philox",
                     "tandem_test_gemm", "tandem_test_gemm_time"]
@@ -86,6 +86,7 @@ def lib():
         L.tandem_step.argtypes = [C.c_void_p, C.POINTER(_StepIn), C.POINTER(_StepOut), C.c_void_p]
         L.tandem_score.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.tandem_grpo_objective.argtypes = [C.c_int32, C.c_int32, C.c_int32] + [C.c_void_p] * 6 + [C.c_float] * 3 + [C.c_void_p] * 5
+        L.tandem_grpo_objective_static.argtypes = [C.c_int32, C.c_int32, C.c_int32] + [C.c_void_p] * 6 + [C.c_float] * 3 + [C.c_void_p] * 3
         L.tandem_generate.argtypes = [C.c_void_p, C.POINTER(_Params), C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                       C.POINTER(_Overrides), C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                       C.POINTER(_Stats), C.c_void_p]
@@ -300,6 +301,31 @@ def grpo_objective(rewards, group, lengths, owner, logp_new, logp_old, logp_ref=
         raise TandemError(rc)
     r = res.cpu().numpy()
     return dict(advantages=adv, token_obj=tok, seq_obj=seq, loss=float(r[0]), clip_frac=float(r[1]), n_senior=int(r[2]), n_live=int(r[3]))
+
+
+GRPO_STATIC_MAX_ROLLOUTS = 8192          # TANDEM_GRPO_STATIC_MAX_ROLLOUTS in include/tandem.h
+
+
+def grpo_objective_static(rewards, group, lengths, owner, logp_new, logp_old, logp_ref=None, clip_eps=0.2, kl_beta=0.0, adv_eps=1e-6,
+                          token_obj=None, result=None, stream=None):
+    """tandem_grpo_objective_static: the same objective with the kernel's scratch in the library's static device array - the call
+    allocates nothing. `result` (4 floats, CUDA) and `token_obj` ([B, L] floats, CUDA, optional) are the caller's; when `result` is
+    None one is made here (that allocation is the binding's convenience, not the entry point's). Returns dict(loss, clip_frac,
+    n_senior, n_live, result, token_obj) - the scalars after a synchronising copy. Calls that overlap on the GPU race on the array."""
+    import torch
+    B, L = owner.shape
+    assert B % group == 0 and rewards.numel() == B and lengths.numel() == B
+    for t_ in (rewards, lengths, owner, logp_new, logp_old) + ((logp_ref,) if logp_ref is not None else ()):
+        assert t_.is_cuda and t_.is_contiguous()
+    if result is None:
+        result = torch.empty(4, dtype=torch.float32, device=owner.device)
+    assert result.is_cuda and result.dtype == torch.float32 and result.numel() >= 4
+    rc = lib().tandem_grpo_objective_static(B // group, group, L, rewards.data_ptr(), lengths.data_ptr(), owner.data_ptr(), logp_new.data_ptr(),
+                                            logp_old.data_ptr(), _ptr(logp_ref), clip_eps, kl_beta, adv_eps, _ptr(token_obj), result.data_ptr(), stream)
+    if rc:
+        raise TandemError(rc)
+    r = result.cpu().numpy()
+    return dict(loss=float(r[0]), clip_frac=float(r[1]), n_senior=int(r[2]), n_live=int(r[3]), result=result, token_obj=token_obj)
 
 
 def tandem_test_uniforms(seed, seq_id, t, stream, n, out_dev):

@@ -13,6 +13,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <string>
+#include <mutex>
 #include <vector>
 
 #include "common.cuh"
@@ -1229,6 +1230,71 @@ int tandem_grpo_objective(int32_t n_groups, int32_t group, int32_t stride, const
   const GrpoArgs a{B, group, stride, rewards, len, owner, logp_new, logp_old, logp_ref, clip_eps, kl_beta, adv_eps, advantages, token_obj, seq_obj, result};
   grpo_seq_kernel<256><<<B, 256, 0, s>>>(a);
   return cudaGetLastError() == cudaSuccess ? TANDEM_OK : TANDEM_ECUDA;
+}
+
+// ---------------------------------------------------------------------------------------------- tandem_grpo_objective_static
+// The GRPO objective for callers that cannot allocate (code under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc):
+// grpo_seq_kernel's scratch - the arrival counters, the per-rollout objectives the last CTA reduces in index order, the advantages -
+// lives in ONE file-scope device array instead of caller-provided buffers. Every GPU that loads the library holds its kGrpoStaticBytes
+// (65,792 bytes) until the process exits. Layout (floats): [0, 8) result + counters (zeroed by every call), [64, 64 + MAX) per-rollout
+// objectives, [64 + MAX, 64 + 2 MAX) advantages; entries [0, B) of both are written before the last CTA reads them, the rest keeps the
+// previous call's values and is never read. All calls share the array: two calls that overlap on the GPU (different streams, or
+// different host threads without ordering) race on it.
+constexpr int kGrpoStaticMaxSeqs = TANDEM_GRPO_STATIC_MAX_ROLLOUTS;
+constexpr int kGrpoStaticHead = 64;                                           // floats in front of the per-rollout arrays
+constexpr size_t kGrpoStaticBytes = (size_t)(kGrpoStaticHead + 2 * kGrpoStaticMaxSeqs) * sizeof(float);
+static __device__ __align__(256) unsigned char g_grpo_static_scratch[kGrpoStaticBytes];
+
+namespace {
+// In host code `g_grpo_static_scratch` is a host-side stand-in, not a device address: the kernel gets the address
+// cudaGetSymbolAddress returns for the CURRENT device, looked up once per device.
+constexpr int kMaxDevices = 64;
+std::mutex g_grpo_static_mu;
+float* g_grpo_static_ptr[kMaxDevices] = {};
+int grpo_static_scratch(float** out) {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) { cudaGetLastError(); return TANDEM_ECUDA; }
+  std::lock_guard<std::mutex> lk(g_grpo_static_mu);
+  if (!g_grpo_static_ptr[dev]) {
+    void* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&p, g_grpo_static_scratch);
+    if (e != cudaSuccess || !p) {
+      fprintf(stderr, "tandem_grpo_objective_static: cudaGetSymbolAddress failed on device %d: %s\n", dev, cudaGetErrorString(e));
+      cudaGetLastError();
+      return TANDEM_ECUDA;
+    }
+    g_grpo_static_ptr[dev] = (float*)p;
+  }
+  *out = g_grpo_static_ptr[dev];
+  return TANDEM_OK;
+}
+}  // namespace
+
+int tandem_grpo_objective_static(int32_t n_groups, int32_t group, int32_t stride, const float* rewards, const int32_t* len, const uint8_t* owner,
+                                 const float* logp_new, const float* logp_old, const float* logp_ref, float clip_eps, float kl_beta, float adv_eps,
+                                 float* token_obj, float* result4, void* cuda_stream) {
+  if (n_groups < 0 || group < 1 || stride < 1 || !(clip_eps >= 0.f) || !(adv_eps >= 0.f)) return TANDEM_EINVAL;
+  if (!rewards || !len || !owner || !logp_new || !logp_old || !result4) return TANDEM_EINVAL;
+  if (kl_beta != 0.f && !logp_ref) return TANDEM_EINVAL;
+  const long long B = (long long)n_groups * group;
+  if (B > kGrpoStaticMaxSeqs) {
+    fprintf(stderr, "tandem_grpo_objective_static: %lld rollouts exceed the static scratch (TANDEM_GRPO_STATIC_MAX_ROLLOUTS = %d); use tandem_grpo_objective\n",
+            B, kGrpoStaticMaxSeqs);
+    return TANDEM_EINVAL;
+  }
+  float* scratch = nullptr;
+  const int rc = grpo_static_scratch(&scratch);
+  if (rc) return rc;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  if (cudaMemsetAsync(scratch, 0, 8 * sizeof(float), s) != cudaSuccess) { cudaGetLastError(); return TANDEM_ECUDA; }   // results and counters start at zero
+  if (B > 0) {
+    const GrpoArgs a{(int)B, group, stride, rewards, len, owner, logp_new, logp_old, logp_ref, clip_eps, kl_beta, adv_eps,
+                     scratch + kGrpoStaticHead + kGrpoStaticMaxSeqs, token_obj, scratch + kGrpoStaticHead, scratch};
+    grpo_seq_kernel<256><<<(int)B, 256, 0, s>>>(a);
+    if (cudaGetLastError() != cudaSuccess) return TANDEM_ECUDA;
+  }
+  if (cudaMemcpyAsync(result4, scratch, 4 * sizeof(float), cudaMemcpyDeviceToDevice, s) != cudaSuccess) { cudaGetLastError(); return TANDEM_ECUDA; }
+  return TANDEM_OK;
 }
 
 void tandem_free(tandem_handle* h) {
