@@ -603,6 +603,13 @@ def run_ours(args):
 
         for it in range(2):
             res["e2e_short"] = e2e_call([args.e2e_new] * B)
+        # the prefill part of a rollout on its own: the same call with one new token per sequence (prompt ingestion by both models,
+        # admission, one sampled token); second call of two, like e2e_short
+        for it in range(2):
+            pf = e2e_call([1] * B)
+        res["e2e_prefill"] = {"seconds": pf["seconds"], "steps": pf["steps"], "prompt_tokens": e_rows, "rows_computed": pf["rows_computed"],
+                              "shared_prompt_rows": pf["shared_prompt_rows"], "prompt_tokens_per_s": e_rows / pf["seconds"],
+                              "call": "tandem_generate(B=%d host prompts, max_new=1)" % B}
         if args.no_e2e_full or max_seq_len < max_prompt + wl.max_new:
             res["e2e"] = res["e2e_short"]
         else:
