@@ -48,6 +48,8 @@ def parse_args():
     ap.add_argument("--grpo", action="store_true", help="time tandem_grpo_objective (senior-masked GRPO forward, NEXT-3) on the workload's batch x max_new")
     ap.add_argument("--score", type=int, default=0, help="N > 0: time tandem_score (teacher-forced dual scoring, NEXT-1) on N synthetic streams instead of the rollout")
     ap.add_argument("--score-len", type=int, default=2048, help="tokens per stream for --score")
+    ap.add_argument("--dual-forward", action="store_true",
+                    help="measurement: the paper's lock-step engine (both models forward every token, no catch-up prefill) instead of the owner split")
     ap.add_argument("--attn-prefill-tc", type=int, default=1, help="--score: 0 = attention on the mma.sync kernel of the rollout instead of the tcgen05 kernel (A/B)")
     ap.add_argument("--score-rows", type=int, default=2048, help="rows per step and model for --score (max_rows_per_step)")
     ap.add_argument("--top-k", type=int, default=0, help="top-k filter of the sampler (0 = off; the paper evaluates with 20)")
@@ -431,6 +433,8 @@ def run_ours(args):
                                   kv_bytes_per_model=kv_per_model, share_prompt_pages=0 if args.no_share_prompt_pages else 1))
     for m in range(2):
         eng.load_weights(m, w_host[m])
+    if args.dual_forward:
+        eng.set_option("dual_forward", 1)
     w_cpu = w_host if (rank == 0 and world == 1 and not args.no_cpu) else []
     del w_host
     prm = T.TandemParams(table, p=wl.p, switch_mode=wl.switch_mode, temperature=wl.temperature, top_p=wl.top_p, top_k=args.top_k or wl.top_k, seed=20260628)
@@ -558,6 +562,7 @@ def run_ours(args):
            "ms_per_step": ms_all / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
            "config": {"workload": wl.name, "batch_per_gpu": B, "prompt_len": list(wl.prompt_len), "fast_forward": args.fast_forward,
                       "ctx_mean_timed": ctx_mean, "p": wl.p, "word_start_frac": wl.word_start_frac, "temperature": wl.temperature, "top_p": wl.top_p, "top_k": args.top_k or wl.top_k, "switch_mode": "REDRAW" if wl.switch_mode else "TOGGLE",
+                      "engine": "dual forward, lock-step (the paper's engine, measurement mode)" if args.dual_forward else "owner split + catch-up prefill",
                       "page_tokens": 16, "parallelism": "dp%d (independent sequences, replicated weights, no collective)" % world,
                       "l2": "inputs larger than L2 (16.1 GB of weights + KV streamed per step vs 126 MB L2)",
                       "setup_steps": n_setup + ramp + n_drain, "setup_seconds": setup_s, "cuda_graph": True, "kv_gb_per_model": kv_per_model / 1e9},

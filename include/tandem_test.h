@@ -28,7 +28,10 @@ const char *tandem_kernel_class_name(int kc);
  * catch-up items only - q_len > 1 - as class attention_catchup, and a third time with no item at all - class attention_empty, the
  * fixed cost of such a launch; results unchanged),  "gemm_pair" (-1 automatic, 0, 1), "score_nosplit" (0/1),
  * "score_chunk_grid" (1..16), "attn_prefill_tc" (0 = tandem_score runs its attention on the mma.sync kernel of the rollout; default 1:
- * the tcgen05 kernel over 128-row q-tiles, csrc/attention_tcgen05.cuh). TANDEM_EINVAL for an unknown name or a value out of range. Every published number uses the defaults. */
+ * the tcgen05 kernel over 128-row q-tiles, csrc/attention_tcgen05.cuh), "dual_forward" (1 = the paper's own engine for an on-box
+ * comparison, PAPER.md L257 / SURVEY.md section 8(f)-1: BOTH models ingest every token in the step after it is emitted, so there is
+ * no catch-up prefill and each model reads its whole KV cache every step; only the owner's row reaches the LM head and the sampler, so
+ * tokens, owner flags and log-probs follow the same rule and the same random numbers; default 0 = owner split). TANDEM_EINVAL for an unknown name or a value out of range. Every published number uses the defaults. */
 int tandem_test_set_option(tandem_handle *h, const char *name, int32_t value);
 
 /* Parity tests at realistic page numbers: seed != 0 makes tandem_reset (and so tandem_generate / tandem_score) hand the pages of each

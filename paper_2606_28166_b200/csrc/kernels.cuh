@@ -17,6 +17,7 @@ struct SchedArgs {
   int32_t* work_ctr; int n_work_ctr;   // dynamic-scheduling counters of the attention launches of this step
   int score;                           // teacher-forced dual scoring (tandem_score): both models ingest every sequence, every row reaches the LM head
   int no_parts;                        // tcgen05 scoring attention: every q-tile covers its whole causal KV range (no KV splits, no combine)
+  int lockstep;                        // measurement (paper's engine): BOTH models ingest every token as it is emitted; only the owner samples
   int32_t* oom_flag;                   // mapped host word, set when a pool runs dry (the host reads it without synchronising)
 };
 
@@ -73,7 +74,7 @@ __global__ void __launch_bounds__(1024) sched_kernel(SchedArgs a) {
   for (int M = 0; M < 2; ++M) {
     const StepTab& tb = a.tab[M];
     const PageTab& pt = a.pt[M];
-    const bool mine = a.score ? live : owner == M;
+    const bool mine = (a.score || a.lockstep) ? live : owner == M;
     int ing = mine ? a.st.ing[M][s] : 0;
     // Prompt-page sharing: a member of a group that has not started with this model links the group's prompt pages if they are
     // ready, becomes the donor if nobody has started them, and otherwise waits (no rows this step) for the donor to finish.
@@ -127,7 +128,7 @@ __global__ void __launch_bounds__(1024) sched_kernel(SchedArgs a) {
     }
     int n_rows;
     const int cu = block_excl_scan_1024(rows, &n_rows, wsum);
-    const bool emits = !a.score && mine && rows == want && want > 0;
+    const bool emits = !a.score && owner == M && mine && rows == want && want > 0;
     fed[M] = ing + rows;
     int n_emit;
     const int j = block_excl_scan_1024(emits ? 1 : 0, &n_emit, wsum);

@@ -79,6 +79,7 @@ struct tandem_handle {
   bool score_nosplit = true;
   int score_chunk_grid = 8;                      // scoring: CTAs per (weight tile, K split) along the token rows (1 = off)
   bool use_pdl = true;                          // programmatic dependent launch along the kernel chain
+  bool dual_forward = false;                    // measurement: the paper's lock-step engine (both models forward every token), see tandem_test.h
   bool attn_prefill_tc = true;                  // tandem_score: tcgen05 attention over 128-row q-tiles (attention_tcgen05.cuh); false = the mma.sync kernel
   bool fused_sampler = true;                    // S8 in the LM head's epilogue whenever the sampler needs no materialised logits
   size_t gemm_out_cols = 0;
@@ -423,7 +424,7 @@ int launch_step(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaSt
   sa.max_pages = h->max_pages; sa.row_cap = h->row_cap; sa.tile_tok = h->tile_tok;
   if (score && use_attn_tc(h)) { sa.tile_tok = kAtTileKv / (c.n_q_heads / c.n_kv_heads); sa.no_parts = 1; }   // 128-row q-tiles, each over its whole causal range
   sa.work_ctr = h->work_ctr; sa.n_work_ctr = 3 * c.n_layers;
-  sa.score = score ? 1 : 0; sa.oom_flag = h->oom_dev;
+  sa.score = score ? 1 : 0; sa.oom_flag = h->oom_dev; sa.lockstep = (h->dual_forward && !score) ? 1 : 0;
   KL(h, TANDEM_KC_SCHED, s, (sched_kernel<<<1, 1024, 0, s>>>(sa)));
   const int rc = (c.dtype == TANDEM_F32) ? forward_pair<float>(h, io, rp, s, score, score_inv_t) : forward_pair<bf16>(h, io, rp, s, score, score_inv_t);
   if (rc) return rc;
@@ -1397,6 +1398,7 @@ int tandem_test_set_option(tandem_handle* h, const char* name, int32_t value) {
   else if (n == "attn_ctas_per_sm" && in(1, 2)) h->attn_ctas_per_sm = value;
   else if (n == "gemm_ring_kb" && in(0, 200)) h->gemm_ring_kb = value;
   else if (n == "fused_sampler" && in(0, 1)) h->fused_sampler = value != 0;
+  else if (n == "dual_forward" && in(0, 1)) h->dual_forward = value != 0;
   else if (n == "attn_prefill_tc" && in(0, 1)) h->attn_prefill_tc = value != 0;
   else if (n == "profile_catchup_attention" && in(0, 1)) h->profile_catchup_attn = value != 0;
   else return fail(h, TANDEM_EINVAL, "unknown option or value out of range: " + n);

@@ -280,3 +280,33 @@ def test_step_stalls_on_an_empty_pool_and_reports_the_dead_lock():
     out = eng.generate(prm, [prompts[0]], [20])
     assert np.array_equal(out["tokens"][0, :20], ref["tokens"][0][:20])
     eng.free()
+
+
+@pytest.mark.parametrize("mode,start,p,share", [(T.TOGGLE, T.SENIOR, 0.5, 0), (T.REDRAW, T.DRAW, 0.5, 1), (T.TOGGLE, T.JUNIOR, 1.0, 0)])
+def test_dual_forward_measurement_mode_follows_the_same_rule(mode, start, p, share):
+    """The paper's own engine as a measurement mode (tandem_test_set_option "dual_forward"):
+    both models ingest every emitted token in lock-step and only the owner samples, so the rollout is the oracle's, token for token,
+    while each model computes one row per resident sequence and step (no catch-up bursts) - both models end up with the same row count."""
+    shape = get_workload("cfg1_tiny_f32").shape
+    ws = make_word_start(shape.vocab, 0.3, 11)
+    rng = np.random.default_rng(6)
+    B = 6
+    base = [rng.integers(0, shape.vocab, size=int(n)).astype(np.int32) for n in (3, 17, 33)]
+    prompts = [base[i // 2] for i in range(B)]                      # groups of two rollouts per prompt
+    max_new = np.array([30, 12, 33, 5, 20, 37], dtype=np.int32)
+    eng, orc, _ = make_pair(shape, (1, 2), max_seqs=6, max_seq_len=96, gain_jitter=0.1, max_rows_per_step=24, share_prompt_pages=share)
+    eng.set_option("dual_forward", 1)
+    op = OParams(p=p, switch_mode=mode, start_owner=start, temperature=1.0, eos_id=3, seed=77)
+    ref = tandem_generate(orc, op, prompts, max_new, ws, uni=Uniforms(seed=77, seq_ids=np.arange(B, dtype=np.int32)))
+    out = eng.generate(T.TandemParams(ws, p=p, switch_mode=mode, start_owner=start, temperature=1.0, eos_id=3, seed=77), prompts, max_new)
+    _compare(out, ref, B, logp_tol=2e-5)
+    st = out["stats"]
+    # every model ingested every prompt (less what it took from shared pages) and every emitted token but each sequence's last one
+    ingested = sum(len(p_) for p_ in prompts) + int(out["len"].sum()) - B
+    assert st["rows_senior"] == st["rows_junior"] == ingested - st["shared_prompt_rows"] // 2
+    # the default engine on the same problem computes fewer rows (a model that never takes a sequence over again skips its tail)
+    eng.set_option("dual_forward", 0)
+    out2 = eng.generate(T.TandemParams(ws, p=p, switch_mode=mode, start_owner=start, temperature=1.0, eos_id=3, seed=77), prompts, max_new)
+    _compare(out2, ref, B, logp_tol=2e-5)
+    assert out2["stats"]["rows_senior"] + out2["stats"]["rows_junior"] <= st["rows_senior"] + st["rows_junior"]
+    eng.free()
