@@ -45,6 +45,7 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg3_4b_bf16")
     ap.add_argument("--p", type=float, default=None, help="override the workload's switch probability (cfg5 sweep)")
+    ap.add_argument("--switch-mode", default=None, choices=["TOGGLE", "REDRAW"], help="override the workload's meaning of p (cfg5: REDRAW p = 1 is solo senior decoding too)")
     ap.add_argument("--grpo", action="store_true", help="time tandem_grpo_objective (senior-masked GRPO forward, NEXT-3) on the workload's batch x max_new")
     ap.add_argument("--score", type=int, default=0, help="N > 0: time tandem_score (teacher-forced dual scoring, NEXT-1) on N synthetic streams instead of the rollout")
     ap.add_argument("--score-len", type=int, default=2048, help="tokens per stream for --score")
@@ -395,6 +396,8 @@ def run_ours(args):
     wl = get_workload(args.workload)
     if args.p is not None:
         wl = wl.with_(p=args.p)
+    if args.switch_mode is not None:
+        wl = wl.with_(switch_mode=1 if args.switch_mode == "REDRAW" else 0)
     if args.word_start_frac is not None:
         wl = wl.with_(word_start_frac=args.word_start_frac)
     if args.top_p is not None:
