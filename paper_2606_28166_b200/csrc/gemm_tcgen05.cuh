@@ -176,25 +176,6 @@ __device__ __forceinline__ uint32_t umma_idesc_bf16(int n, int m = kTcTileN) {
 }
 
 
-// ---- kTcEpiSample helpers: 16 token columns per lane (lane = vocabulary id), reduced across the 32 lanes of a warp by recursive
-// halving - after four exchange rounds a lane holds ONE column reduced over 16 lanes, a fifth round finishes it: 16 shuffles per
-// quantity instead of 80. The column a lane ends up with is lane >> 1. The combination tree is fixed: results are deterministic.
-template <typename Op>
-__device__ __forceinline__ float tc_reduce16(float (&a)[16], int lane, Op op) {
-  bool hi = lane & 16;
-#pragma unroll
-  for (int i = 0; i < 8; ++i) { const float send = hi ? a[i] : a[i + 8], keep = hi ? a[i + 8] : a[i]; a[i] = op(keep, __shfl_xor_sync(0xffffffffu, send, 16)); }
-  hi = lane & 8;
-#pragma unroll
-  for (int i = 0; i < 4; ++i) { const float send = hi ? a[i] : a[i + 4], keep = hi ? a[i + 4] : a[i]; a[i] = op(keep, __shfl_xor_sync(0xffffffffu, send, 8)); }
-  hi = lane & 4;
-#pragma unroll
-  for (int i = 0; i < 2; ++i) { const float send = hi ? a[i] : a[i + 2], keep = hi ? a[i + 2] : a[i]; a[i] = op(keep, __shfl_xor_sync(0xffffffffu, send, 4)); }
-  hi = lane & 2;
-  { const float send = hi ? a[0] : a[1], keep = hi ? a[1] : a[0]; a[0] = op(keep, __shfl_xor_sync(0xffffffffu, send, 2)); }
-  return op(a[0], __shfl_xor_sync(0xffffffffu, a[0], 1));
-}
-
 struct TcMaps { CUtensorMap w[2], a[2][4]; };   // per model: weight descriptor; activation descriptors with 128/64/32/16-row boxes
 
 struct TcGemmArgs {
@@ -206,13 +187,12 @@ struct TcGemmArgs {
   int ring_bytes;             // shared-memory ring of this launch (200 KB: one CTA per SM; 98 KB: two)
   int chunk_grid;             // >= 1: the 256-row chunks of the token rows are dealt round-robin to this many CTAs per (tile, split)
                               // (gridDim.y = n_split * chunk_grid); 1 = one CTA walks all chunks
-  // EPI = kTcEpiSample (the LM head of the default sampling path, S8): the logits never reach HBM
+  // kTcEpiSample (lmhead_sample_kernel: the LM head of the default sampling path, S8): the logits never reach HBM
   const int32_t* emit_slot;   // [rows] slot of emitting row j
   const int32_t* n_emit;      // [max_seqs] tokens emitted so far (t = n_emit + 1 addresses the uniforms)
   const int32_t* seq_id;      // [max_seqs]
   float inv_t; int greedy; uint32_t key0, key1;   // 1 / temperature (1 if greedy), Philox key = seed
 };
-constexpr int kTcSampleSmem = 8192;    // kTcEpiSample: (t, seq_id) of a chunk's rows + the per-quarter partials of two 16-column groups, double-buffered
 constexpr int kTcSampleVals = 8;       // floats per (weight tile, row) partial: max z, sum exp, raw best id, Gumbel best value, its id, its z, 2 spare
 
 // ---------------------------------------------------------------------------------------------- the kernel
@@ -220,10 +200,8 @@ enum { kTcEpiPartial = 0, kTcEpiSwiGLU = 1, kTcEpiSample = 2 };
 
 // EPI  = kTcEpiPartial: fp32 partial out[split][r][n];
 //        kTcEpiSwiGLU : W rows interleaved (2i = gate_i, 2i+1 = up_i), n_split = 1: act[r][i] = silu(gate) * up as bf16.
-//        kTcEpiSample : the LM head when the sampler needs no materialised logits (S8; "logits never need to
-//                       reach HBM if the softmax stats + Gumbel-argmax are reduced in the GEMM epilogue"): per (128-id weight tile,
-//                       emitting row) the epilogue writes (max z, sum exp((z - max) / T), raw argmax, Gumbel-max value / id / z) -
-//                       out[row][tile][8] fp32 - and sample_merge_emit_kernel merges the tiles of a row.
+// (kTcEpiSample, the LM head of the default sampling path with S8's reductions in its epilogue, is a kernel of its own:
+//  lmhead_sample.cuh - persistent, two TMEM accumulators.)
 // Cluster launches with TMA multicast of the activation boxes (2 and 4 CTAs) were built and measured: no gain at any of
 // the projection shapes on B200 (profiles/gemm_sweep_r1.md): multicast does not lower what each SM has to ingest. The CTA pair does.
 // PAIR = true: launched in clusters of two CTAs along x (adjacent weight tiles). The pair runs one cta_group::2 MMA with M = 256:
@@ -380,106 +358,6 @@ gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__
     for (int c = cslice, ci = 0; c < n_chunks; c += cstep, ++ci) {
       const int r0 = c * kTcMaxRows;
       const int crow = min(rows - r0, kTcMaxRows);
-      if constexpr (EPI == kTcEpiSample) {
-        // ---- S8 in the epilogue: lane = vocabulary id n, 16 emitting rows (columns) at a time; the two warps of a lane quarter take
-        // alternate 16-column groups; the four quarters of a half are combined through shared memory into ONE partial per (tile, row)
-        uint8_t* extra = tc_smem_raw + (ring - ptx::smem_u32(tc_smem_raw)) + g.ring_bytes;
-        int* s_t = reinterpret_cast<int*>(extra);                 // [256] t = index of the token being emitted by the row's sequence
-        int* s_sid = s_t + kTcMaxRows;                            // [256] its sequence id
-        float* s_part = reinterpret_cast<float*>(extra + 2048);   // [half 2][buffer 2][quarter 4][16 columns][6]
-        const int et = (warp >= 7 ? warp - 3 : warp - 2) * 32 + lane;   // 0..255 over the eight epilogue warps
-        ptx::bar_sync_id<1>(256);                                 // the previous chunk's readers of s_t are done
-        {
-          const int j = r0 + et;
-          const int slot = j < rows ? g.emit_slot[j] : 0;
-          s_t[et] = j < rows ? g.n_emit[slot] + 1 : 0;
-          s_sid[et] = j < rows ? g.seq_id[slot] : 0;
-        }
-        ptx::bar_sync_id<1>(256);
-        ptx::mbar_wait(tmem_full_bar, (uint32_t)ci & 1u);
-        ptx::tc_fence_after();
-        const bool n_ok = n < g.N;
-        const float inv_t = g.inv_t;
-        const int tile = blockIdx.x;
-        int it16 = 0;
-        for (int c0 = 16 * half; c0 < crow; c0 += 32, ++it16) {
-          uint32_t v[16];
-          ptx::tmem_ld16(tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)c0, v);
-          ptx::tmem_ld_wait();
-          float z[16], w[16];
-#pragma unroll
-          for (int k = 0; k < 16; ++k) { z[k] = (n_ok && c0 + k < crow) ? __uint_as_float(v[k]) : -INFINITY; w[k] = z[k]; }
-          // column maxima of z, then known to every lane
-          const float mine_m = tc_reduce16(w, lane, [](float x, float y) { return fmaxf(x, y); });
-          float M[16];
-#pragma unroll
-          for (int k = 0; k < 16; ++k) M[k] = __shfl_sync(0xffffffffu, mine_m, 2 * k);
-          // raw argmax: the lowest lane (= lowest id) that holds the maximum; sum of exp((z - max) / T)
-          int my_raw = 0;
-#pragma unroll
-          for (int k = 0; k < 16; ++k) {
-            const unsigned b = __ballot_sync(0xffffffffu, z[k] == M[k] && z[k] != -INFINITY);
-            if (k == (lane >> 1)) my_raw = b ? __ffs(b) - 1 : 0;
-            w[k] = z[k] == -INFINITY ? 0.f : expf((z[k] - M[k]) * inv_t);
-          }
-          const float mine_s = tc_reduce16(w, lane, [](float x, float y) { return x + y; });
-          // Gumbel-max: g = -ln(-log1p(-u)), u from Philox-4x32-10 at counter (n >> 2, t, seq_id, 0), word n & 3 - the block of four ids is
-          // computed by the lane whose (lane & 3) equals (column & 3) and handed to its three neighbours
-          float mine_gv = -INFINITY, mine_gz = 0.f; int my_g = 0;
-          if (!g.greedy) {
-            uint32_t blk[4][4];
-#pragma unroll
-            for (int kk = 0; kk < 4; ++kk) {
-              const int k = 4 * kk + (lane & 3);
-              blk[kk][0] = (uint32_t)(n >> 2); blk[kk][1] = (uint32_t)s_t[c0 + k]; blk[kk][2] = (uint32_t)s_sid[c0 + k]; blk[kk][3] = 0u;
-              philox4x32_10(blk[kk], g.key0, g.key1);
-            }
-#pragma unroll
-            for (int k = 0; k < 16; ++k) {
-              const int src = (lane & ~3) | (k & 3);
-              const uint32_t w0 = __shfl_sync(0xffffffffu, blk[k >> 2][0], src), w1 = __shfl_sync(0xffffffffu, blk[k >> 2][1], src);
-              const uint32_t w2 = __shfl_sync(0xffffffffu, blk[k >> 2][2], src), w3 = __shfl_sync(0xffffffffu, blk[k >> 2][3], src);
-              const uint32_t r = (lane & 2) ? ((lane & 1) ? w3 : w2) : ((lane & 1) ? w1 : w0);
-              w[k] = z[k] == -INFINITY ? -INFINITY : z[k] * inv_t + gumbel_from_uniform(uniform_from_bits(r));
-            }
-            float gg[16];
-#pragma unroll
-            for (int k = 0; k < 16; ++k) gg[k] = w[k];
-            mine_gv = tc_reduce16(w, lane, [](float x, float y) { return fmaxf(x, y); });
-#pragma unroll
-            for (int k = 0; k < 16; ++k) {
-              const float Gk = __shfl_sync(0xffffffffu, mine_gv, 2 * k);
-              const unsigned b = __ballot_sync(0xffffffffu, gg[k] == Gk && gg[k] != -INFINITY);
-              const int wl = b ? __ffs(b) - 1 : 0;
-              const float zw = __shfl_sync(0xffffffffu, z[k], wl);
-              if (k == (lane >> 1)) { my_g = wl; mine_gz = zw; }
-            }
-          }
-          // this quarter's partial of column lane >> 1 -> shared memory; four quarters -> one partial per (tile, row)
-          float* sp = s_part + ((size_t)(half * 2 + (it16 & 1)) * 4 + q) * 16 * 6;
-          if ((lane & 1) == 0) {
-            float* e = sp + (lane >> 1) * 6;
-            e[0] = mine_m; e[1] = mine_s; e[2] = __int_as_float(n0 + q * 32 + my_raw); e[3] = mine_gv; e[4] = __int_as_float(n0 + q * 32 + my_g); e[5] = mine_gz;
-          }
-          if (half) ptx::bar_sync_id<3>(128); else ptx::bar_sync_id<2>(128);
-          if (q == 0 && lane < 16 && c0 + lane < crow) {
-            const float* e0 = s_part + ((size_t)(half * 2 + (it16 & 1)) * 4) * 16 * 6 + lane * 6;
-            SamplePart a{e0[0], e0[1], e0[3], e0[5], __float_as_int(e0[2]), __float_as_int(e0[4])};
-#pragma unroll
-            for (int qq = 1; qq < 4; ++qq) {
-              const float* e = e0 + qq * 16 * 6;
-              sample_part_merge(a, SamplePart{e[0], e[1], e[3], e[5], __float_as_int(e[2]), __float_as_int(e[4])}, inv_t);
-            }
-            float4* dst = reinterpret_cast<float4*>(g.out + ((size_t)(r0 + c0 + lane) * gridDim.x + tile) * kTcSampleVals);   // [row][tile][8]
-            dst[0] = make_float4(a.m, a.s, __int_as_float(a.raw_id), a.gv);
-            dst[1] = make_float4(__int_as_float(a.g_id), a.gz, 0.f, 0.f);
-          }
-        }
-        ptx::tc_fence_before();
-        __syncwarp();
-        if (lane == 0) { if (PAIR) ptx::mbar_arrive_cluster(te_bar); else ptx::mbar_arrive(te_bar); }
-        continue;
-      }
       ptx::mbar_wait(tmem_full_bar, (uint32_t)ci & 1u);
       ptx::tc_fence_after();
       for (int c0 = 32 * half; c0 < crow; c0 += 64) {
@@ -519,6 +397,8 @@ gemm_tcgen05_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__
   if (warp == 2) { if (PAIR) ptx::tmem_dealloc_pair<kTcMaxRows>(tmem_base); else ptx::tmem_dealloc<kTcMaxRows>(tmem_base); }
 }
 
+#include "lmhead_sample.cuh"   // lmhead_sample_kernel (kTcEpiSample); needs everything above
+
 // ---------------------------------------------------------------------------------------------- host side
 // K-splits: as many as keep the whole launch (all tiles of all models in it) within one CTA per SM, each slice >= 4 k-blocks.
 // One CTA per SM with the deep 200 KB ring beats two per SM with an uneven second layer (measured on the 4B shape, both models
@@ -551,7 +431,7 @@ inline TcGemmPlans* tc_gemm_create() {
   bool ok = true;
   ok &= cudaFuncSetAttribute(gemm_tcgen05_kernel<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes) == cudaSuccess;
   ok &= cudaFuncSetAttribute(gemm_tcgen05_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes) == cudaSuccess;
-  ok &= cudaFuncSetAttribute(gemm_tcgen05_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes) == cudaSuccess;
+  ok &= cudaFuncSetAttribute(lmhead_sample_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kLmSmemBytes) == cudaSuccess;
   ok &= cudaFuncSetAttribute(gemm_tcgen05_kernel<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes) == cudaSuccess;
   ok &= cudaFuncSetAttribute(gemm_tcgen05_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes) == cudaSuccess;
   if (!ok) {
@@ -599,9 +479,8 @@ inline bool tc_map_q3d(TcGemmPlans* p, CUtensorMap* out, const void* base, int D
 // which == 4 (LM head) never splits: the sampler reads the logits in place.
 template <int EPI>
 inline int tc_gemm_launch_epi(const TcMaps& maps, const Pair<TcGemmArgs>& g, dim3 grid, cudaStream_t s, bool pdl, bool pair) {
-  const size_t smem = (size_t)g.m[0].ring_bytes + 1024 + (EPI == kTcEpiSample ? kTcSampleSmem : 0);
-  if constexpr (EPI == kTcEpiSample) return launch_ex(gemm_tcgen05_kernel<EPI, false>, grid, dim3(kTcThreads), smem, s, pdl, maps, g) == cudaSuccess ? 0 : -3;
-  else if (pair) return launch_ex_cluster(gemm_tcgen05_kernel<EPI, true>, grid, dim3(kTcThreads), smem, s, pdl, 2, maps, g) == cudaSuccess ? 0 : -3;
+  const size_t smem = (size_t)g.m[0].ring_bytes + 1024;
+  if (pair) return launch_ex_cluster(gemm_tcgen05_kernel<EPI, true>, grid, dim3(kTcThreads), smem, s, pdl, 2, maps, g) == cudaSuccess ? 0 : -3;
   return launch_ex(gemm_tcgen05_kernel<EPI, false>, grid, dim3(kTcThreads), smem, s, pdl, maps, g) == cudaSuccess ? 0 : -3;
 }
 struct TcSampleCfg { const int32_t* emit_slot[2]; const int32_t* n_emit; const int32_t* seq_id; float inv_t; int greedy; unsigned long long seed; };
@@ -637,7 +516,7 @@ inline int tc_gemm_launch(TcGemmPlans* p, int n_models, int which, const void* c
       maps.a[m][b] = *ma;
     }
     g.m[m] = TcGemmArgs{out[mm], rows_ptr ? rows_ptr[mm] : nullptr, rows_cap, N, K, S, *split_stride,
-                        epi == kTcEpiSample ? ring - kTcSampleSmem : ring, CG, nullptr, nullptr, nullptr, 1.f, 1, 0u, 0u};
+                        epi == kTcEpiSample ? kLmRingBytes : ring, CG, nullptr, nullptr, nullptr, 1.f, 1, 0u, 0u};
     if (epi == kTcEpiSample) {
       if (!tune || !tune->sample) return -1;
       const TcSampleCfg& sc = *tune->sample;
@@ -648,7 +527,8 @@ inline int tc_gemm_launch(TcGemmPlans* p, int n_models, int which, const void* c
   dim3 grid(tiles_pad, S * CG, n_models);
   const bool pdl = tune && tune->pdl;
   if (epi == kTcEpiSwiGLU) return tc_gemm_launch_epi<1>(maps, g, grid, s, pdl, pair);
-  if (epi == kTcEpiSample) return tc_gemm_launch_epi<2>(maps, g, grid, s, pdl, false);
+  if (epi == kTcEpiSample)   // persistent: one CTA per SM walks the (weight tile, model) units
+    return launch_ex(lmhead_sample_kernel, dim3(std::min(n_sms, tiles * n_models)), dim3(kLmThreads), (size_t)kLmSmemBytes, s, pdl, maps, g) == cudaSuccess ? 0 : -3;
   return tc_gemm_launch_epi<0>(maps, g, grid, s, pdl, pair);
 }
 
