@@ -23,6 +23,7 @@
 #include "attention_tcgen05.cuh"
 #include "gemm_simt.cuh"
 #include "gemm_tcgen05.cuh"
+#include "gemm_streamk.cuh"
 #include "grpo.cuh"
 
 using namespace tandem;
@@ -82,6 +83,9 @@ struct tandem_handle {
   bool dual_forward = false;                    // measurement: the paper's lock-step engine (both models forward every token), see tandem_test.h
   bool attn_prefill_tc = true;                  // tandem_score: tcgen05 attention over 128-row q-tiles (attention_tcgen05.cuh); false = the mma.sync kernel
   bool fused_sampler = true;                    // S8 in the LM head's epilogue whenever the sampler needs no materialised logits
+  bool gateup_streamk = true;                   // gate/up + SwiGLU as the persistent stream-K kernel (gemm_streamk.cuh) when the shape allows; false = one tile per CTA
+  float* sk_scratch = nullptr; int sk_rows = 0; int32_t* sk_flags = nullptr;   // its tail partials [n_sms][2][sk_rows][128] and flag / acknowledge counters [2][n_sms]
+  int32_t* fault_host = nullptr; int32_t* fault_dev = nullptr;   // mapped pinned word a kernel raises when a bounded wait on another CTA expired
   size_t gemm_out_cols = 0;
   ModelWeights w[2];
   Workspace ws[2];
@@ -360,7 +364,13 @@ int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaS
     // S7 gate/up + SwiGLU, down + residual + RMSNorm(next layer | final)
     if (h->gemm_impl == TANDEM_GEMM_TCGEN05) {   // SwiGLU in the GEMM epilogue (gate/up rows interleaved at load time)
       for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].act, h->w[m].wgu[l], (float*)h->ws[m].mlp_act, h->tab[m].counts + C_ROWS);
-      if ((rc = launch_gemm<T>(h, 2, A, W, 2 * I, H, O, RP, h->row_cap, &ns, &ss, s, kTcEpiSwiGLU))) return rc;
+      if (h->sk_scratch && h->gateup_streamk && !h->scoring) {   // decode-sized steps: stream-K over tile pairs, both models, one CTA per SM
+        void* outs[2] = {h->ws[0].mlp_act, h->ws[1].mlp_act};
+        int src = 0;
+        KL(h, TANDEM_KC_GEMM_GATEUP, s, src = sk_gateup_launch(h->tc, A, W, 2 * I, H, outs, RP, h->row_cap, h->sk_scratch, h->sk_rows, h->sk_flags,
+                                                              h->sk_flags + h->n_sms, h->fault_dev, h->n_sms, s, pdl));
+        if (src) return fail(h, src, "stream-K gate/up launch failed");
+      } else if ((rc = launch_gemm<T>(h, 2, A, W, 2 * I, H, O, RP, h->row_cap, &ns, &ss, s, kTcEpiSwiGLU))) return rc;
     } else {
       for (int m = 0; m < 2; ++m) set_gemm(m, h->ws[m].act, h->w[m].wgu[l], h->ws[m].gemm_out, h->tab[m].counts + C_ROWS);
       if ((rc = launch_gemm<T>(h, 2, A, W, 2 * I, H, O, RP, h->row_cap, &ns, &ss, s))) return rc;
@@ -626,6 +636,8 @@ struct EventPair {   // timing events of tandem_generate / tandem_score, destroy
 
 // KV-pool exhaustion seen by the scheduler of an earlier step (mapped host word, no synchronisation): sticky until tandem_reset
 int check_oom_flag(tandem_handle* h) {
+  if (h->fault_host && *(volatile int32_t*)h->fault_host)
+    return fail(h, TANDEM_ECUDA, "a kernel's bounded wait on another CTA expired (stream-K hand-over): results since then are invalid; tandem_free the handle");
   if (h->oom_host && *(volatile int32_t*)h->oom_host >= 2)
     return fail(h, TANDEM_ENOMEM, "KV page pools exhausted: every resident sequence is stalled and no step can make progress (nothing was corrupted); "
                                   "tandem_reset the handle, then enlarge kv_bytes_per_model or admit fewer sequences");
@@ -726,6 +738,9 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
   INIT_CU(cudaHostAlloc((void**)&h->oom_host, 4, cudaHostAllocMapped));
   *h->oom_host = 0;
   INIT_CU(cudaHostGetDevicePointer((void**)&h->oom_dev, h->oom_host, 0));
+  INIT_CU(cudaHostAlloc((void**)&h->fault_host, 4, cudaHostAllocMapped));
+  *h->fault_host = 0;
+  INIT_CU(cudaHostGetDevicePointer((void**)&h->fault_dev, h->fault_host, 0));
   INIT_TRY(dmalloc(h, &h->n_active, 4));
   INIT_CU(cudaMemset(h->n_active, 0, 4));
   INIT_TRY(dmalloc(h, &h->stage_off, (size_t)(S + 1) * sizeof(long long)));
@@ -757,6 +772,13 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
     }
   }
   h->gemm_out_cols = cols;
+  if (h->gemm_impl == TANDEM_GEMM_TCGEN05 && h->esize == 2 && sk_applicable(2 * I, H, h->n_sms) && sk_gateup_init()) {
+    // stream-K gate/up (gemm_streamk.cuh): one 256-row chunk of tail partials per CTA, flag / acknowledge counters (zero between launches)
+    h->sk_rows = ((std::min(R, kTcMaxRows) + 31) / 32) * 32;
+    INIT_TRY(dmalloc(h, &h->sk_scratch, (size_t)h->n_sms * 2 * h->sk_rows * kTcTileN * 4));
+    INIT_TRY(dmalloc(h, &h->sk_flags, (size_t)2 * h->n_sms * 4));
+    INIT_CU(cudaMemset(h->sk_flags, 0, (size_t)2 * h->n_sms * 4));
+  }
   for (int m = 0; m < 2; ++m) {
     Workspace& w = h->ws[m];
     INIT_TRY(dmalloc(h, &w.x, (size_t)R * H * 4));
@@ -1319,6 +1341,9 @@ void tandem_free(tandem_handle* h) {
   fr(h->score_out[0]); fr(h->score_out[1]); fr(h->st_mem); fr(h->st_mem8); fr(h->tokens); fr(h->out_owner); fr(h->out_logp); fr(h->rope_cs); fr(h->word_start_dev); fr(h->stats);
   fr(h->gt_mem); fr(h->gt_pages_mem);
   if (h->oom_host) cudaFreeHost(h->oom_host);
+  if (h->fault_host) cudaFreeHost(h->fault_host);
+  if (h->sk_scratch) cudaFree(h->sk_scratch);
+  if (h->sk_flags) cudaFree(h->sk_flags);
   fr(h->n_active); fr(h->work_ctr); fr(h->stage_tokens); fr(h->stage_off); fr(h->stage_i32);
   cudaGetLastError();
   delete h;
@@ -1398,6 +1423,7 @@ int tandem_test_set_option(tandem_handle* h, const char* name, int32_t value) {
   else if (n == "attn_ctas_per_sm" && in(1, 2)) h->attn_ctas_per_sm = value;
   else if (n == "gemm_ring_kb" && in(0, 200)) h->gemm_ring_kb = value;
   else if (n == "fused_sampler" && in(0, 1)) h->fused_sampler = value != 0;
+  else if (n == "gateup_streamk" && in(0, 1)) h->gateup_streamk = value != 0;
   else if (n == "dual_forward" && in(0, 1)) h->dual_forward = value != 0;
   else if (n == "attn_prefill_tc" && in(0, 1)) h->attn_prefill_tc = value != 0;
   else if (n == "profile_catchup_attention" && in(0, 1)) h->profile_catchup_attn = value != 0;
