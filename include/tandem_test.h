@@ -31,7 +31,9 @@ const char *tandem_kernel_class_name(int kc);
  * the tcgen05 kernel over 128-row q-tiles, csrc/attention_tcgen05.cuh), "dual_forward" (1 = the paper's own engine for an on-box
  * comparison, PAPER.md L257 / SURVEY.md section 8(f)-1: BOTH models ingest every token in the step after it is emitted, so there is
  * no catch-up prefill and each model reads its whole KV cache every step; only the owner's row reaches the LM head and the sampler, so
- * tokens, owner flags and log-probs follow the same rule and the same random numbers; default 0 = owner split). TANDEM_EINVAL for an unknown name or a value out of range. Every published number uses the defaults. */
+ * tokens, owner flags and log-probs follow the same rule and the same random numbers; default 0 = owner split), "gateup_streamk" (0 = the
+ * gate/up projection always runs on the one-tile-per-CTA kernel; default 1: decode-sized steps of a shape with at least one tile pair per
+ * CTA use the persistent balanced kernel, csrc/gemm_streamk.cuh). TANDEM_EINVAL for an unknown name or a value out of range. Every published number uses the defaults. */
 int tandem_test_set_option(tandem_handle *h, const char *name, int32_t value);
 
 /* Parity tests at realistic page numbers: seed != 0 makes tandem_reset (and so tandem_generate / tandem_score) hand the pages of each
