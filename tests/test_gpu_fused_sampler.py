@@ -17,11 +17,11 @@ from workloads import ModelShape, make_weights, make_word_start
 pytestmark = pytest.mark.gpu
 
 
-def _run(shape, B, n_new, temperature, eos, fused, ws, wj, prompts, max_new, table, seed=9):
+def _run(shape, B, n_new, temperature, eos, fused, ws, wj, prompts, max_new, table, seed=9, p=0.5):
     eng = T.Tandem(T.TandemConfig(shape, max_seqs=B + 3, max_seq_len=160, use_graph=1))
     eng.load_weights(0, ws); eng.load_weights(1, wj)
     eng.set_option("fused_sampler", fused)
-    out = eng.generate(T.TandemParams(table, p=0.5, temperature=temperature, eos_id=eos, seed=seed), prompts, max_new)
+    out = eng.generate(T.TandemParams(table, p=p, temperature=temperature, eos_id=eos, seed=seed), prompts, max_new)
     eng.free()
     return out
 
@@ -39,6 +39,25 @@ def test_fused_sampler_equals_materialised_logits(V, B, temperature, eos):
     assert np.array_equal(a["len"], b["len"]) and np.array_equal(a["tokens"], b["tokens"]) and np.array_equal(a["owner"], b["owner"])
     assert 0.1 < a["owner"][:, :20].mean() < 0.9
     assert np.max(np.abs(a["sen_logp"] - b["sen_logp"])) <= 2e-5
+
+
+def test_fused_sampler_more_than_256_emitting_rows_of_one_model():
+    """The persistent LM head (lmhead_sample.cuh) with one model active and 300 emitting rows: two row chunks per weight tile, the two
+    TMEM accumulators alternate within a tile, the (t, seq_id) table is reloaded per chunk; and, with p = 0.5, both models at ~150 rows
+    (one CTA per model parity, 144-column accumulators)."""
+    V, B = 4100, 300
+    shape = ModelShape(1, 128, 2, 1, 64, 256, V, 1e-6, 1e6, "bf16")
+    ws = make_weights(shape, 1, device="cuda", gain_jitter=0.1); wj = make_weights(shape, 2, device="cuda", gain_jitter=0.1)
+    table = make_word_start(V, 0.3, 3)
+    rng = np.random.default_rng(31)
+    prompts = [rng.integers(0, V, size=int(rng.integers(2, 9))).astype(np.int32) for _ in range(B)]
+    max_new = np.full(B, 6, np.int32)
+    for p in (0.0, 0.5):
+        a = _run(shape, B, 6, 1.0, -1, 1, ws, wj, prompts, max_new, table, p=p)
+        b = _run(shape, B, 6, 1.0, -1, 0, ws, wj, prompts, max_new, table, p=p)
+        assert np.array_equal(a["len"], b["len"]) and np.array_equal(a["tokens"], b["tokens"]) and np.array_equal(a["owner"], b["owner"])
+        assert (a["owner"].sum() == 0) == (p == 0.0)
+        assert np.max(np.abs(a["sen_logp"] - b["sen_logp"])) <= 2e-5
 
 
 def test_fused_sampler_against_the_oracle():
