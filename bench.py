@@ -51,6 +51,9 @@ def parse_args():
     ap.add_argument("--score-len", type=int, default=2048, help="tokens per stream for --score")
     ap.add_argument("--dual-forward", action="store_true",
                     help="measurement: the paper's lock-step engine (both models forward every token, no catch-up prefill) instead of the owner split")
+    ap.add_argument("--skip-class", default=None,
+                    help="measurement: leave the launches of one kernel class (a name of the kernels table, e.g. gemm_gateup) out of the timed steps; the "
+                         "difference to the full step is the class's marginal cost inside the step graph (results of those steps are garbage)")
     ap.add_argument("--attn-prefill-tc", type=int, default=1, help="--score: 0 = attention on the mma.sync kernel of the rollout instead of the tcgen05 kernel (A/B)")
     ap.add_argument("--score-rows", type=int, default=2048, help="rows per step and model for --score (max_rows_per_step)")
     ap.add_argument("--top-k", type=int, default=0, help="top-k filter of the sampler (0 = off; the paper evaluates with 20)")
@@ -471,6 +474,9 @@ def run_ours(args):
         if rows8 <= 8 * 3 * B:
             break
     torch.cuda.synchronize()
+    if args.skip_class:   # after the setup: the state the timed steps start from is the real one
+        names = [T.lib().tandem_kernel_class_name(i).decode() for i in range(T.binding.KC_NUM)]
+        eng.set_option("skip_class", names.index(args.skip_class))
     setup_s = time.perf_counter() - t0
 
     # ---- warmup + timed region
@@ -566,6 +572,7 @@ def run_ours(args):
            "config": {"workload": wl.name, "batch_per_gpu": B, "prompt_len": list(wl.prompt_len), "fast_forward": args.fast_forward,
                       "ctx_mean_timed": ctx_mean, "p": wl.p, "word_start_frac": wl.word_start_frac, "temperature": wl.temperature, "top_p": wl.top_p, "top_k": args.top_k or wl.top_k, "switch_mode": "REDRAW" if wl.switch_mode else "TOGGLE",
                       "engine": "dual forward, lock-step (the paper's engine, measurement mode)" if args.dual_forward else "owner split + catch-up prefill",
+                      **({"skip_class": args.skip_class + " (measurement: this kernel class was left out of the timed steps; not a throughput number)"} if args.skip_class else {}),
                       "page_tokens": 16, "parallelism": "dp%d (independent sequences, replicated weights, no collective)" % world,
                       "l2": "inputs larger than L2 (16.1 GB of weights + KV streamed per step vs 126 MB L2)",
                       "setup_steps": n_setup + ramp + n_drain, "setup_seconds": setup_s, "cuda_graph": True, "kv_gb_per_model": kv_per_model / 1e9},

@@ -960,6 +960,7 @@ __global__ void __launch_bounds__(NT) sample_switch_emit_kernel(const __grid_con
   }
   if (!searched && !last) return;
   int y = greedy ? raw.i : gum.i;
+  if ((unsigned)y >= (unsigned)V) y = 0;   // all logits non-finite (NaN weights): no id ever won a comparison - emit id 0 rather than index out of bounds
   if (a.io.forced_tokens) {
     const int f = a.io.forced_tokens[(size_t)s * a.io.forced_stride + (t - 1)];
     if (f >= 0 && f < V) y = f;   // an id outside the vocabulary is ignored (it would index the logits and the embedding out of bounds)
@@ -1008,7 +1009,8 @@ __global__ void __launch_bounds__(NT) sample_merge_emit_kernel(const __grid_cons
   if (lane != 0) return;
   const int s = a.tab.emit_slot[j];
   const int t = a.st.n_emit[s] + 1;
-  const int y = greedy ? acc.raw_id : acc.g_id;
+  int y = greedy ? acc.raw_id : acc.g_id;
+  if ((unsigned)y >= (unsigned)a.vocab) y = 0;   // all logits non-finite: see sample_switch_emit_kernel
   const float zy = greedy ? acc.m : acc.gz;
   emit_token_and_switch(a, s, t, a.st.seq_id[s], y, zy * invT - (acc.m * invT + logf(acc.s)), acc.raw_id);
 }

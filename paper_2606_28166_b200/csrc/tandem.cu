@@ -83,6 +83,7 @@ struct tandem_handle {
   bool dual_forward = false;                    // measurement: the paper's lock-step engine (both models forward every token), see tandem_test.h
   bool attn_prefill_tc = true;                  // tandem_score: tcgen05 attention over 128-row q-tiles (attention_tcgen05.cuh); false = the mma.sync kernel
   bool fused_sampler = true;                    // S8 in the LM head's epilogue whenever the sampler needs no materialised logits
+  int skip_class = -1;                          // measurement (tandem_test.h "skip_class"): the launches of this kernel class are left out of the step
   bool gateup_streamk = true;                   // gate/up + SwiGLU as the persistent stream-K kernel (gemm_streamk.cuh) when the shape allows; false = one tile per CTA
   float* sk_scratch = nullptr; int sk_rows = 0; int32_t* sk_flags = nullptr;   // its tail partials [n_sms][2][sk_rows][128] and flag / acknowledge counters [2][n_sms]
   int32_t* fault_host = nullptr; int32_t* fault_dev = nullptr;   // mapped pinned word a kernel raises when a bounded wait on another CTA expired
@@ -155,6 +156,7 @@ cudaEvent_t prof_event(tandem_handle* h) {
 }
 #define KL(h, cls, stream, ...)                                                   \
   do {                                                                            \
+    if ((h)->skip_class == (cls)) break; /* measurement: this class is left out */ \
     ++(h)->launches;                                                              \
     if ((h)->profile) {                                                           \
       cudaEvent_t e0__ = prof_event(h), e1__ = prof_event(h);                     \
@@ -1424,6 +1426,7 @@ int tandem_test_set_option(tandem_handle* h, const char* name, int32_t value) {
   else if (n == "gemm_ring_kb" && in(0, 200)) h->gemm_ring_kb = value;
   else if (n == "fused_sampler" && in(0, 1)) h->fused_sampler = value != 0;
   else if (n == "gateup_streamk" && in(0, 1)) h->gateup_streamk = value != 0;
+  else if (n == "skip_class" && in(-1, TANDEM_KC_NUM - 1)) h->skip_class = value;
   else if (n == "dual_forward" && in(0, 1)) h->dual_forward = value != 0;
   else if (n == "attn_prefill_tc" && in(0, 1)) h->attn_prefill_tc = value != 0;
   else if (n == "profile_catchup_attention" && in(0, 1)) h->profile_catchup_attn = value != 0;

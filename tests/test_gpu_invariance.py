@@ -4,7 +4,7 @@ import pytest
 import torch
 
 import paper_2606_28166_b200 as T
-from workloads import get_workload, make_word_start, ModelShape
+from workloads import get_workload, make_weights, make_word_start, ModelShape
 from gpu_util import make_pair
 
 pytestmark = pytest.mark.gpu
@@ -92,4 +92,24 @@ def test_kv_pool_exhaustion_is_reported():
     with pytest.raises(T.TandemError) as e:
         eng.generate(T.TandemParams(ws), _prompts(4), [60] * 4)
     assert e.value.code == -2
+    eng.free()
+
+
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+def test_non_finite_logits_cannot_index_out_of_bounds(dtype):
+    """Weights with a NaN (here: the final norm's gains) make every logit NaN, no id ever wins an argmax comparison and the merged id keeps its
+    'none yet' value: the samplers (materialised-logits kernel for fp32, the LM head's fused epilogue + merge kernel for bf16) then emit an id
+    inside the vocabulary (0 where nothing won) instead of using that value as an index into the logits, the word-start table and the embedding.
+    The call returns and the device is healthy (before the guard: an illegal memory access, which is expensive to clear on a shared pool)."""
+    shape = ModelShape(2, 256, 4, 2, 64, 512, 4100, 1e-6, 1e6, dtype)
+    w = [make_weights(shape, s, device="cuda") for s in (1, 2)]
+    for x in w:
+        x["final_norm"] = torch.full_like(x["final_norm"], float("nan"))
+    eng = T.Tandem(T.TandemConfig(shape, max_seqs=3, max_seq_len=48))
+    eng.load_weights(0, w[0]); eng.load_weights(1, w[1])
+    table = make_word_start(shape.vocab, 0.3, 4)
+    for temperature in (1.0, 0.0):
+        out = eng.generate(T.TandemParams(table, p=0.5, temperature=temperature, seed=3), [np.arange(5, 14, dtype=np.int32)] * 3, [6] * 3)
+        assert out["len"].tolist() == [6, 6, 6] and (out["tokens"] >= 0).all() and (out["tokens"] < shape.vocab).all()
+    torch.cuda.synchronize()
     eng.free()
