@@ -51,6 +51,8 @@ def parse_args():
     ap.add_argument("--score-len", type=int, default=2048, help="tokens per stream for --score")
     ap.add_argument("--dual-forward", action="store_true",
                     help="measurement: the paper's lock-step engine (both models forward every token, no catch-up prefill) instead of the owner split")
+    ap.add_argument("--set-option", action="append", default=[], metavar="NAME=VALUE",
+                    help="measurement: a tandem_test_set_option knob (include/tandem_test.h) for an A/B on one box, e.g. gateup_cluster=0; repeatable")
     ap.add_argument("--skip-class", default=None,
                     help="measurement: leave the launches of one kernel class (a name of the kernels table, e.g. gemm_gateup) out of the timed steps; the "
                          "difference to the full step is the class's marginal cost inside the step graph (results of those steps are garbage)")
@@ -441,6 +443,8 @@ def run_ours(args):
         eng.load_weights(m, w_host[m])
     if args.dual_forward:
         eng.set_option("dual_forward", 1)
+    for kv in args.set_option:
+        eng.set_option(kv.split("=")[0], int(kv.split("=")[1]))
     w_cpu = w_host if (rank == 0 and world == 1 and not args.no_cpu) else []
     del w_host
     prm = T.TandemParams(table, p=wl.p, switch_mode=wl.switch_mode, temperature=wl.temperature, top_p=wl.top_p, top_k=args.top_k or wl.top_k, seed=20260628)
@@ -572,6 +576,7 @@ def run_ours(args):
            "config": {"workload": wl.name, "batch_per_gpu": B, "prompt_len": list(wl.prompt_len), "fast_forward": args.fast_forward,
                       "ctx_mean_timed": ctx_mean, "p": wl.p, "word_start_frac": wl.word_start_frac, "temperature": wl.temperature, "top_p": wl.top_p, "top_k": args.top_k or wl.top_k, "switch_mode": "REDRAW" if wl.switch_mode else "TOGGLE",
                       "engine": "dual forward, lock-step (the paper's engine, measurement mode)" if args.dual_forward else "owner split + catch-up prefill",
+                      **({"set_option": args.set_option} if args.set_option else {}),
                       **({"skip_class": args.skip_class + " (measurement: this kernel class was left out of the timed steps; not a throughput number)"} if args.skip_class else {}),
                       "page_tokens": 16, "parallelism": "dp%d (independent sequences, replicated weights, no collective)" % world,
                       "l2": "inputs larger than L2 (16.1 GB of weights + KV streamed per step vs 126 MB L2)",
