@@ -51,6 +51,10 @@ def parse_args():
     ap.add_argument("--score-len", type=int, default=2048, help="tokens per stream for --score")
     ap.add_argument("--dual-forward", action="store_true",
                     help="measurement: the paper's lock-step engine (both models forward every token, no catch-up prefill) instead of the owner split")
+    ap.add_argument("--max-rows", type=int, default=0,
+                    help="tandem_config.max_rows_per_step: row budget of a step per model (prefills and catch-ups beyond it are chunked). 0 = 4096, except 256 for a "
+                         "whole rollout with >= 256 resident sequences (cfg 4): the projections pass over the weights once per 256 token rows, and with ~256 rows "
+                         "per model and step a budget of 256 keeps every step at one pass (160.1 -> 151.1 s measured)")
     ap.add_argument("--set-option", action="append", default=[], metavar="NAME=VALUE",
                     help="measurement: a tandem_test_set_option knob (include/tandem_test.h) for an A/B on one box, e.g. gateup_cluster=0; repeatable")
     ap.add_argument("--skip-class", default=None,
@@ -242,8 +246,9 @@ def run_full_rollout(args):
     need = sum((len(p) + int(n) + 15) // 16 + 1 for p, n in zip(prompts, max_new)) * shape.kv_elems_per_token * 2 * 16
     kv_per_model = int(min((free - wbytes - 4.5e9) / 2, need + (64 << 20)))            # workspaces and the CUDA context stay free
     max_seqs = min(B, 256)
+    max_rows = args.max_rows or (256 if max_seqs >= 256 else 4096)
     eng = T.Tandem(T.TandemConfig(shape, max_seqs=max_seqs, max_seq_len=(max(len(p) for p in prompts) + int(max_new.max()) + 31) // 16 * 16,
-                                  kv_bytes_per_model=kv_per_model, max_rows_per_step=4096, use_graph=1,
+                                  kv_bytes_per_model=kv_per_model, max_rows_per_step=max_rows, use_graph=1,
                                   share_prompt_pages=0 if args.no_share_prompt_pages else 1))
     for m in range(2):
         eng.load_weights(m, w_host[m])
@@ -267,7 +272,7 @@ def run_full_rollout(args):
                       "data": "synthetic",
                       "config": {"workload": wl.name, "mode": "full rollout through tandem_generate (prefill, admission queue, host buffers)",
                                  "sequences": B, "max_new_scale": args.full_rollout, "mean_new": float(max_new.mean()), "tokens": tok, "seconds": dt,
-                                 "max_seqs": max_seqs, "peak_resident": int(st["peak_resident"]), "kv_gb_per_model": kv_per_model / 1e9,
+                                 "max_seqs": max_seqs, "max_rows_per_step": max_rows, "peak_resident": int(st["peak_resident"]), "kv_gb_per_model": kv_per_model / 1e9,
                                  "peak_pages": [int(st["peak_pages_senior"]), int(st["peak_pages_junior"])],
                                  "share_prompt_pages": not args.no_share_prompt_pages, "shared_prompt_rows": int(st["shared_prompt_rows"]),
                                  "senior_share": float(g["mask"].sum() / max(1, tok))},
@@ -416,7 +421,7 @@ def run_ours(args):
     prompts, table, seq_ids = build_inputs(wl, args.fast_forward, rank)
     max_prompt = max(len(p) for p in prompts)
     prefill_rows = sum(len(p) for p in prompts)
-    row_cap = 4096
+    row_cap = args.max_rows or 4096
     prefill_steps = (prefill_rows + row_cap - 1) // row_cap + 2
     gen_budget = prefill_steps + max(args.ramp, int(8.0 / max(wl.p * wl.word_start_frac, 1e-3))) + args.max_drain + W + K + args.profile_steps + 64
     e2e_len = args.e2e_new if (args.no_e2e or args.no_e2e_full) else max(args.e2e_new, wl.max_new)

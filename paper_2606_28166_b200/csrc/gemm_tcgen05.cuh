@@ -10,8 +10,10 @@
 //   fp32 partial out[s][r][n]; the consumer kernel sums the S partials in a fixed order (deterministic, no atomics).
 //   warp 0: weight TMA   warp 6: activation TMA   warp 1: MMA issuer   warps 2-5, 7-10: epilogue (tcgen05.ld -> coalesced global
 //   stores; two warps per TMEM lane quarter: the epilogue is an exposed tail, every CTA owns a single tile)
-//   smem ring: stage = 16 KB of W (128 x 64 bf16, 128B swizzle) + nbox x 4 KB of A (32-row boxes), as many stages
-//   as fit in 200 KB (4 at 256 rows, 6 at 128 rows, 9 at 32 rows).
+//   smem ring: stage = 16 KB of W (128 x 64 bf16, 128B swizzle) + 2 KB of A per 16 token rows (boxes of 128/64/32/16 rows), as many
+//   stages as fit in 200 KB (4 at 256 rows, 6 at 128 rows, 10 at 32 rows).
+// The gate/up projection of decode-sized steps and the LM head of the default sampling path have persistent kernels of their own
+// (gemm_streamk.cuh, lmhead_sample.cuh); this kernel serves QKV, O, down, the materialised-logits LM head, scoring and prefill-sized launches.
 #pragma once
 #include <cuda.h>   // CUtensorMap and its enums only; the encode entry point is fetched at run time (no libcuda link)
 #include <algorithm>
@@ -31,7 +33,7 @@ constexpr int kTcRingBytes = 200 * 1024;
 constexpr int kTcSmemBytes = kTcRingBytes + 1024;   // + alignment slack
 constexpr int kTcThreads = 352;        // warps: 0 weight TMA, 1 MMA, 2-5 and 7-10 epilogue (two per TMEM lane quarter), 6 activation TMA
 constexpr int kTcWBytes = kTcTileN * kTcBlockK * 2;     // 16384
-constexpr int kTcABoxBytes = kTcRowBox * kTcBlockK * 2; // 4096
+constexpr int kTcABoxBytes = kTcRowBox * kTcBlockK * 2; // 2048
 
 // ---------------------------------------------------------------------------------------------- PTX wrappers
 namespace ptx {
