@@ -87,6 +87,9 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-share-prompt-pages", action="store_true",
                     help="every rollout computes and stores its own copy of the prompt's KV (default: the G rollouts of a prompt share its full pages)")
+    ap.add_argument("--share-mode", type=int, default=2, choices=[1, 2],
+                    help="tandem_config.share_prompt_pages when sharing is on: 1 = the rollouts of a prompt share its full KV pages; 2 = and the members a model "
+                         "serves in a step read them once (shared-prefix runs)")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-new", type=int, default=8, help="new tokens of the oracle's bounded sample")
     return ap.parse_args()
@@ -249,7 +252,7 @@ def run_full_rollout(args):
     max_rows = args.max_rows or (256 if max_seqs >= 256 else 4096)
     eng = T.Tandem(T.TandemConfig(shape, max_seqs=max_seqs, max_seq_len=(max(len(p) for p in prompts) + int(max_new.max()) + 31) // 16 * 16,
                                   kv_bytes_per_model=kv_per_model, max_rows_per_step=max_rows, use_graph=1,
-                                  share_prompt_pages=0 if args.no_share_prompt_pages else 1))
+                                  share_prompt_pages=0 if args.no_share_prompt_pages else args.share_mode))
     for m in range(2):
         eng.load_weights(m, w_host[m])
     del w_host
@@ -274,7 +277,7 @@ def run_full_rollout(args):
                                  "sequences": B, "max_new_scale": args.full_rollout, "mean_new": float(max_new.mean()), "tokens": tok, "seconds": dt,
                                  "max_seqs": max_seqs, "max_rows_per_step": max_rows, "peak_resident": int(st["peak_resident"]), "kv_gb_per_model": kv_per_model / 1e9,
                                  "peak_pages": [int(st["peak_pages_senior"]), int(st["peak_pages_junior"])],
-                                 "share_prompt_pages": not args.no_share_prompt_pages, "shared_prompt_rows": int(st["shared_prompt_rows"]),
+                                 "share_prompt_pages": 0 if args.no_share_prompt_pages else args.share_mode, "shared_prompt_rows": int(st["shared_prompt_rows"]),
                                  "senior_share": float(g["mask"].sum() / max(1, tok))},
                       "gpu_launches": int(st["kernel_launches"]),
                       "step_roofline": {"bound": "hbm", "achieved": gbs, "unit": "GB/s", "frac_of_measured": gbs / pk["hbm_gbs"], "frac_of_8TBs": gbs / NOMINAL_HBM_GBS},
@@ -443,7 +446,7 @@ def run_ours(args):
     wbytes = 2 * (shape.params_read_per_step + shape.vocab * shape.hidden) * 2
     kv_per_model = int(min((free - wbytes - 5.5e9) / 2, (need_pages + 64) * page_bytes))
     eng = T.Tandem(T.TandemConfig(shape, max_seqs=B, max_seq_len=max_seq_len, device=local, max_rows_per_step=row_cap, use_graph=1,
-                                  kv_bytes_per_model=kv_per_model, share_prompt_pages=0 if args.no_share_prompt_pages else 1))
+                                  kv_bytes_per_model=kv_per_model, share_prompt_pages=0 if args.no_share_prompt_pages else args.share_mode))
     for m in range(2):
         eng.load_weights(m, w_host[m])
     if args.dual_forward:
@@ -623,7 +626,7 @@ def run_ours(args):
                     "ms_per_step": st["seconds_total"] / steps_e * 1e3,
                     "senior_share": float(g["mask"].sum() / max(1, g["len"].sum())),
                     "step_roofline": {"bound": "hbm", "achieved": gbs, "unit": "GB/s", "frac_of_measured": gbs / pk["hbm_gbs"], "frac_of_8TBs": gbs / NOMINAL_HBM_GBS},
-                    "share_prompt_pages": not args.no_share_prompt_pages, "prompt_rows": e_rows, "shared_prompt_rows": st["shared_prompt_rows"],
+                    "share_prompt_pages": 0 if args.no_share_prompt_pages else args.share_mode, "prompt_rows": e_rows, "shared_prompt_rows": st["shared_prompt_rows"],
                     "rows_computed": st["rows_senior"] + st["rows_junior"], "peak_resident": int(st["peak_resident"])}
 
         for it in range(2):

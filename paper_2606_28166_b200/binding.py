@@ -68,7 +68,8 @@ class _StepOut(C.Structure):
 class _Stats(C.Structure):
     _fields_ = [(n, C.c_int64) for n in ("steps", "tokens_emitted", "rows_senior", "rows_junior", "catchup_rows", "kv_bytes_read", "weight_bytes_read")] + \
                [("peak_pages_senior", C.c_int32), ("peak_pages_junior", C.c_int32), ("peak_resident", C.c_int32), ("seconds_total", C.c_double),
-                ("kernel_launches", C.c_int64), ("shared_prompt_rows", C.c_int64), ("starved", C.c_int64), ("preemptions", C.c_int64)]
+                ("kernel_launches", C.c_int64), ("shared_prompt_rows", C.c_int64), ("starved", C.c_int64), ("preemptions", C.c_int64),
+                ("kv_bytes_shared_reads", C.c_int64)]
 
 
 _lib = None

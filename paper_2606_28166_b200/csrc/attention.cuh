@@ -206,6 +206,7 @@ __global__ void __launch_bounds__(kAttnThreads) paged_attention_kernel(const __g
 // Combine the splits of a decode row: out = sum_i e^{m_i - m} acc_i / sum_i e^{m_i - m} l_i.
 template <typename T> struct CombineArgs {
   const int32_t* counts; const int32_t* comb_row; const int32_t* comb_part0; const int32_t* comb_n; const int32_t* comb_stride;
+  const int32_t* comb_gpart;   // optional extra partial per row (the row's part of a shared-prefix run), -1 = none
   const float* part_acc; const float2* part_ml; T* out; int nq, d;
 };
 // One warp per (row, head); lane = 4 consecutive dims; all partial loads of a row are independent (n <= kAttnMaxSplits).
@@ -217,23 +218,27 @@ __global__ void __launch_bounds__(256) attn_combine_kernel(const __grid_constant
   const int lane = threadIdx.x & 31;
   for (int unit = blockIdx.x * (blockDim.x / 32) + (threadIdx.x >> 5); unit < n_units; unit += gridDim.x * (blockDim.x / 32)) {
     const int c = unit / a.nq, head = unit - c * a.nq;
-    const int row = a.comb_row[c], p0 = a.comb_part0[c], n = a.comb_n[c], ps = a.comb_stride[c];
-    float2 ml[kAttnMaxSplits];
+    const int row = a.comb_row[c], p0 = a.comb_part0[c], n = a.comb_n[c], ps = a.comb_stride[c], gp = a.comb_gpart[c];
+    // entry 0 = the shared-prefix partial (if any), entries 1.. = the row's own splits, in KV order
+    float2 ml[kAttnMaxSplits + 1];
+    int pi[kAttnMaxSplits + 1];
     float m = -INFINITY;
 #pragma unroll
-    for (int i = 0; i < kAttnMaxSplits; ++i) {
-      ml[i] = i < n ? a.part_ml[(size_t)(p0 + i * ps) * a.nq + head] : make_float2(-INFINITY, 0.f);
+    for (int i = 0; i <= kAttnMaxSplits; ++i) {
+      const bool on = i == 0 ? gp >= 0 : i - 1 < n;
+      pi[i] = i == 0 ? gp : p0 + (i - 1) * ps;
+      ml[i] = on ? a.part_ml[(size_t)pi[i] * a.nq + head] : make_float2(-INFINITY, 0.f);
       m = fmaxf(m, ml[i].x);
     }
-    float l = 0.f, w[kAttnMaxSplits];
+    float l = 0.f, w[kAttnMaxSplits + 1];
 #pragma unroll
-    for (int i = 0; i < kAttnMaxSplits; ++i) { w[i] = i < n ? __expf(ml[i].x - m) : 0.f; l += w[i] * ml[i].y; }
+    for (int i = 0; i <= kAttnMaxSplits; ++i) { w[i] = ml[i].x == -INFINITY ? 0.f : __expf(ml[i].x - m); l += w[i] * ml[i].y; }
     for (int e = 4 * lane; e < a.d; e += 128) {
       float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
-      for (int i = 0; i < kAttnMaxSplits; ++i) {
-        if (i < n) {
-          const float4 t = ld4(a.part_acc + ((size_t)(p0 + i * ps) * a.nq + head) * a.d + e);
+      for (int i = 0; i <= kAttnMaxSplits; ++i) {
+        if (i == 0 ? gp >= 0 : i - 1 < n) {
+          const float4 t = ld4(a.part_acc + ((size_t)pi[i] * a.nq + head) * a.d + e);
           v.x += w[i] * t.x; v.y += w[i] * t.y; v.z += w[i] * t.z; v.w += w[i] * t.w;
         }
       }

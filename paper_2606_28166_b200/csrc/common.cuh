@@ -75,6 +75,7 @@ struct StepTab {
   int32_t* comb_part0;  // [C] first partial of that row
   int32_t* comb_n;      // [C] number of partials
   int32_t* comb_stride; // [C] distance between consecutive partials of that row
+  int32_t* comb_gpart;  // [C] one more partial of that row: its share of a shared-prefix run's item (share_prompt_pages = 2), or -1
 };
 
 struct SeqState {       // all [max_seqs]
@@ -106,6 +107,7 @@ struct DevStats {       // device-side accumulators (unsigned long long for atom
   unsigned long long steps, tokens_emitted, rows[2], catchup_rows, kv_tokens_read, model_steps;
   unsigned long long shared_rows;   // prompt positions taken over from a group's shared pages instead of being recomputed
   unsigned long long starved;       // (sequence, step) pairs not scheduled because the model's page pool had no page left
+  unsigned long long kv_tokens_shared;   // shared-prefix runs: KV positions the run's members after the first did not stream again
   int peak_pages_used[2]; int peak_resident; int err_oom;
 };
 

@@ -18,6 +18,7 @@ struct SchedArgs {
   int score;                           // teacher-forced dual scoring (tandem_score): both models ingest every sequence, every row reaches the LM head
   int no_parts;                        // tcgen05 scoring attention: every q-tile covers its whole causal KV range (no KV splits, no combine)
   int lockstep;                        // measurement (paper's engine): BOTH models ingest every token as it is emitted; only the owner samples
+  int cascade;                         // share_prompt_pages = 2: the members of a group that a model serves in a step read the group's shared prompt pages ONCE (see below)
   int32_t* oom_flag;                   // mapped host word, set when a pool runs dry (the host reads it without synchronising)
 };
 
@@ -51,6 +52,11 @@ __device__ __forceinline__ int find_owner_slot(const int* cu, int n, int r) {
 __global__ void __launch_bounds__(1024) sched_kernel(SchedArgs a) {
   __shared__ int cu_rows[kMaxSlots + 1], cu_items[kMaxSlots + 1];
   __shared__ int sm_rows[kMaxSlots], sm_ing[kMaxSlots], sm_part0[kMaxSlots], sm_emit[kMaxSlots];
+  // shared-prefix runs (cascade): per row-bearing index the run's group id (-1 = none) and the slot; per slot the shared length, the slot's
+  // own item count, for a run's head its rows, and the index of the slot's first shared-prefix partial
+  __shared__ short comp_eg[kMaxSlots], comp_slot[kMaxSlots];
+  __shared__ unsigned short sm_ls[kMaxSlots], sm_oitems[kMaxSlots], sm_grows[kMaxSlots];
+  __shared__ int sm_gp[kMaxSlots];
   __shared__ int wsum[32];
   const int s = threadIdx.x;
   const bool in_range = s < a.max_seqs;
@@ -139,34 +145,66 @@ __global__ void __launch_bounds__(1024) sched_kernel(SchedArgs a) {
     const int kv_len = ing + rows;
     const int n_qt = (rows + a.tile_tok - 1) / a.tile_tok;
     const int chunk = attn_chunk(kv_len);
-    const bool use_parts = rows > 0 && n_qt <= kAttnSplitTiles && kv_len > chunk && !a.no_parts;
+    int n_sched;
+    const int ridx = block_excl_scan_1024(rows > 0 ? 1 : 0, &n_sched, wsum);   // index among the slots that have rows in this model
+    // Shared-prefix runs (share_prompt_pages = 2; the 8 rollouts of a GRPO group, hold the same prompt KV): the members of a group
+    // that this model serves this step with all their rows past the shared prompt pages, and whose rows are neighbours in the row table, form
+    // a run. The run's rows attend to the shared positions [0, Ls) TOGETHER - q-tiles over the run's rows, one partial per row - so those
+    // pages are streamed once per run instead of once per member; every member's own items start at Ls, and the combine kernel merges the
+    // shared partial with the member's own splits. Same sums up to the order of the softmax merge (the split point Ls).
+    const int Ls_mine = (a.cascade && g >= 0) ? pt.nshared[s] * kPageTokens : 0;
+    const bool elig = Ls_mine > 0 && rows > 0 && ing >= Ls_mine && n_qt <= kAttnSplitTiles && !a.no_parts;
+    sm_rows[s] = rows;
+    if (rows > 0) { comp_eg[ridx] = (short)(elig ? g : -1); comp_slot[ridx] = (short)s; }
+    __syncthreads();
+    const bool in_run = elig && ((ridx > 0 && comp_eg[ridx - 1] == g) || (ridx + 1 < n_sched && comp_eg[ridx + 1] == g));
+    const bool head = in_run && !(ridx > 0 && comp_eg[ridx - 1] == g);
+    int run_off = 0, run_rows = 0, head_slot = s;          // rows of the run before this member; head: rows of the whole run
+    if (in_run) {
+      for (int j2 = ridx - 1; j2 >= 0 && comp_eg[j2] == g; --j2) { run_off += sm_rows[comp_slot[j2]]; head_slot = comp_slot[j2]; }
+      if (head) {
+        int members = 0;
+        for (int j2 = ridx; j2 < n_sched && comp_eg[j2] == g; ++j2) { run_rows += sm_rows[comp_slot[j2]]; ++members; }
+        atomicAdd(&a.stats->kv_tokens_shared, (unsigned long long)(members - 1) * (unsigned long long)Ls_mine);
+      }
+    }
+    const int Ls = in_run ? Ls_mine : 0;
+    const int k_first = Ls / chunk;                          // own splits that lie wholly inside the shared prefix are not created
+    const bool use_parts = rows > 0 && ((n_qt <= kAttnSplitTiles && kv_len > chunk && !a.no_parts) || in_run);
     int items = rows > 0 ? n_qt : 0, parts = 0;
     if (use_parts) {
       items = 0;
       for (int t = 0; t < n_qt; ++t) {
         const int t0 = t * a.tile_tok, nt = min(a.tile_tok, rows - t0);
-        const int ns = (ing + t0 + nt + chunk - 1) / chunk;
+        const int ns = (ing + t0 + nt + chunk - 1) / chunk - k_first;
         items += ns; parts += ns * nt;
       }
     }
-    int n_items, n_parts, n_comb, n_sched;
+    const int own_items = items, own_parts = parts;
+    const int g_items = head ? (run_rows + a.tile_tok - 1) / a.tile_tok : 0;
+    items += g_items; parts += head ? run_rows : 0;
+    int n_items, n_parts, n_comb;
     const int icu = block_excl_scan_1024(items, &n_items, wsum);
     const int pcu = block_excl_scan_1024(parts, &n_parts, wsum);
     const int ccu = block_excl_scan_1024(use_parts ? rows : 0, &n_comb, wsum);
-    block_excl_scan_1024(rows > 0 ? 1 : 0, &n_sched, wsum);
 
     cu_rows[s] = cu; cu_items[s] = icu;
-    sm_rows[s] = rows; sm_ing[s] = ing; sm_part0[s] = use_parts ? pcu : -1; sm_emit[s] = emits ? j : -1;
+    sm_ing[s] = ing; sm_part0[s] = use_parts ? pcu : -1; sm_emit[s] = emits ? j : -1;
+    sm_ls[s] = (unsigned short)Ls; sm_oitems[s] = (unsigned short)own_items; sm_grows[s] = (unsigned short)(head ? run_rows : 0);
+    sm_gp[s] = pcu + own_parts;                              // a head's shared-prefix partials follow its own
     if (s == 0) { cu_rows[kMaxSlots] = n_rows; cu_items[kMaxSlots] = n_items; }
     if (emits) tb.emit_slot[j] = s;
+    __syncthreads();
     if (use_parts) {
+      const int gp = in_run ? sm_gp[head_slot] + run_off : -1;
       int poff = 0;
       for (int t = 0; t < n_qt; ++t) {
         const int t0 = t * a.tile_tok, nt = min(a.tile_tok, rows - t0);
-        const int ns = (ing + t0 + nt + chunk - 1) / chunk;
+        const int ns = (ing + t0 + nt + chunk - 1) / chunk - k_first;
         for (int k = 0; k < nt; ++k) {
           tb.comb_row[ccu + t0 + k] = cu + t0 + k; tb.comb_part0[ccu + t0 + k] = pcu + poff + k;
           tb.comb_n[ccu + t0 + k] = ns; tb.comb_stride[ccu + t0 + k] = nt;
+          tb.comb_gpart[ccu + t0 + k] = in_run ? gp + t0 + k : -1;
         }
         poff += ns * nt;
       }
@@ -194,17 +232,22 @@ __global__ void __launch_bounds__(1024) sched_kernel(SchedArgs a) {
       const int q = find_owner_slot(cu_items, kMaxSlots, i);
       const int off = i - cu_items[q];
       const int qrows = sm_rows[q], qkv = sm_ing[q] + qrows;
-      if (sm_part0[q] >= 0) {             // split sequence: walk its q-tiles to find (q-tile, split) number `off`
-        const int ch = attn_chunk(qkv);
+      if (off >= (int)sm_oitems[q]) {     // head of a shared-prefix run: q-tile t of the run's rows against the shared positions [0, Ls)
+        const int t0 = (off - (int)sm_oitems[q]) * a.tile_tok, nt = min(a.tile_tok, (int)sm_grows[q] - t0);
+        tb.item_row0[i] = cu_rows[q] + t0; tb.item_ntok[i] = nt;
+        tb.item_kv0[i] = 0; tb.item_kv1[i] = (int)sm_ls[q];
+        tb.item_part[i] = sm_gp[q] + t0;
+      } else if (sm_part0[q] >= 0) {      // split sequence: walk its q-tiles to find (q-tile, split) number `off`
+        const int ch = attn_chunk(qkv), ls = (int)sm_ls[q], kf = ls / ch;   // member of a run: its own items start at the shared length
         int rem = off, poff = 0, t0 = 0, nt = 0, ns = 0;
         for (;; t0 += a.tile_tok) {
           nt = min(a.tile_tok, qrows - t0);
-          ns = (sm_ing[q] + t0 + nt + ch - 1) / ch;
+          ns = (sm_ing[q] + t0 + nt + ch - 1) / ch - kf;
           if (rem < ns) break;
           rem -= ns; poff += ns * nt;
         }
         tb.item_row0[i] = cu_rows[q] + t0; tb.item_ntok[i] = nt;
-        tb.item_kv0[i] = rem * ch; tb.item_kv1[i] = min(sm_ing[q] + t0 + nt, (rem + 1) * ch);
+        tb.item_kv0[i] = max((rem + kf) * ch, ls); tb.item_kv1[i] = min(sm_ing[q] + t0 + nt, (rem + kf + 1) * ch);
         tb.item_part[i] = sm_part0[q] + poff + rem * nt;
       } else {                            // q-tile `off`, whole causal range, written directly
         const int t0 = off * a.tile_tok, nt = min(a.tile_tok, qrows - t0);

@@ -350,7 +350,7 @@ int forward_pair(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaS
       Pair<CombineArgs<T>> ca;
       for (int m = 0; m < 2; ++m) {
         const StepTab& tb = h->tab[m];
-        ca.m[m] = CombineArgs<T>{tb.counts, tb.comb_row, tb.comb_part0, tb.comb_n, tb.comb_stride, h->ws[m].part_acc, h->ws[m].part_ml, (T*)h->ws[m].attn_out, nq, d};
+        ca.m[m] = CombineArgs<T>{tb.counts, tb.comb_row, tb.comb_part0, tb.comb_n, tb.comb_stride, tb.comb_gpart, h->ws[m].part_acc, h->ws[m].part_ml, (T*)h->ws[m].attn_out, nq, d};
       }
       KL(h, TANDEM_KC_ATTN_COMBINE, s, launch_ex(attn_combine_kernel<T>, dim3(h->n_sms * 4, 2), dim3(256), 0, s, pdl, ca));
     }
@@ -436,6 +436,7 @@ int launch_step(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaSt
   sa.max_pages = h->max_pages; sa.row_cap = h->row_cap; sa.tile_tok = h->tile_tok;
   if (score && use_attn_tc(h)) { sa.tile_tok = kAtTileKv / (c.n_q_heads / c.n_kv_heads); sa.no_parts = 1; }   // 128-row q-tiles, each over its whole causal range
   sa.work_ctr = h->work_ctr; sa.n_work_ctr = 3 * c.n_layers;
+  sa.cascade = (c.share_prompt_pages == 2 && !score) ? 1 : 0;
   sa.score = score ? 1 : 0; sa.oom_flag = h->oom_dev; sa.lockstep = (h->dual_forward && !score) ? 1 : 0;
   KL(h, TANDEM_KC_SCHED, s, (sched_kernel<<<1, 1024, 0, s>>>(sa)));
   const int rc = (c.dtype == TANDEM_F32) ? forward_pair<float>(h, io, rp, s, score, score_inv_t) : forward_pair<bf16>(h, io, rp, s, score, score_inv_t);
@@ -620,6 +621,7 @@ int fill_stats(tandem_handle* h, tandem_stats* stats) {
   stats->seconds_total = 0.0;
   stats->kernel_launches = h->launches;
   stats->shared_prompt_rows = (int64_t)d.shared_rows;
+  stats->kv_bytes_shared_reads = (int64_t)d.kv_tokens_shared * 2ll * c.n_layers * kd * h->esize;
   stats->starved = (int64_t)d.starved; stats->preemptions = h->preemptions;
   return TANDEM_OK;
 }
@@ -688,7 +690,8 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
   if (c.max_seq_len < 2) return bad("bad max_seq_len");
   if (!attn_supported(c.dtype, c.head_dim, c.n_q_heads / c.n_kv_heads)) return bad("unsupported (head_dim, n_q/n_kv) combination");
   for (int i = 0; i < 2; ++i) if (c.reserved[i]) return bad("reserved fields must be 0");
-  if (c.share_prompt_pages != 0 && c.share_prompt_pages != 1) return bad("share_prompt_pages must be 0 or 1");
+  if (c.share_prompt_pages < 0 || c.share_prompt_pages > 2) return bad("share_prompt_pages must be 0, 1 or 2");
+  if (c.share_prompt_pages == 2 && c.max_seq_len > 65535) return bad("share_prompt_pages = 2 needs max_seq_len <= 65535");
   if (c.attn_impl < 0 || c.attn_impl > 2) return bad("bad attn_impl");
   h->attn_impl = c.attn_impl == TANDEM_ATTN_AUTO ? (c.dtype == TANDEM_BF16 ? TANDEM_ATTN_MMA : TANDEM_ATTN_ALU) : c.attn_impl;
   if (h->attn_impl == TANDEM_ATTN_MMA && c.dtype != TANDEM_BF16) return bad("tensor-core attention needs bf16");
@@ -700,9 +703,9 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
   h->row_cap = std::max(h->row_cap, c.max_seqs);   // every owned sequence must be able to decode in one step
   h->max_pages = (c.max_seq_len + kPageTokens - 1) / kPageTokens;
   h->tile_tok = std::max(1, kAttnTileRows / (c.n_q_heads / c.n_kv_heads));
-  h->max_items = c.max_seqs * kAttnSplitTiles * kAttnMaxSplits + h->row_cap;   // (q-tile, split) of short runs + q-tiles of longer ones
+  h->max_items = c.max_seqs * kAttnSplitTiles * (kAttnMaxSplits + 1) + h->row_cap;   // (q-tile, split) of short runs + the q-tiles of shared-prefix runs + q-tiles of longer ones
   h->max_comb = std::min(c.max_seqs * kAttnSplitTiles * h->tile_tok, h->row_cap);   // rows whose splits are combined
-  h->part_cap = h->max_comb * kAttnMaxSplits;                       // (row, split) partials
+  h->part_cap = h->max_comb * (kAttnMaxSplits + 1);                 // (row, split) partials + one shared-prefix partial per row
   const int H = c.hidden, nq = c.n_q_heads, nkv = c.n_kv_heads, d = c.head_dim, I = c.intermediate, V = c.vocab, R = h->row_cap, S = c.max_seqs;
   const size_t page_bytes = (size_t)2 * c.n_layers * nkv * kPageTokens * d * h->esize;
   h->pool_pages = c.kv_bytes_per_model > 0 ? (int)std::min<int64_t>(c.kv_bytes_per_model / (int64_t)page_bytes, (int64_t)1 << 30)
@@ -806,7 +809,7 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
     INIT_CU(cudaMemset(w.lm_in, 0, (size_t)std::max(S, 256) * H * h->esize));
     INIT_CU(cudaMemset(w.kv, 0, (size_t)h->pool_pages * page_bytes));
     // step tables
-    const size_t tab_ints = (size_t)C_NUM + 5 * (size_t)R + (size_t)S + 5 * (size_t)h->max_items + 4 * (size_t)h->max_comb;
+    const size_t tab_ints = (size_t)C_NUM + 5 * (size_t)R + (size_t)S + 5 * (size_t)h->max_items + 5 * (size_t)h->max_comb;
     INIT_TRY(dmalloc(h, &w.tab_mem, tab_ints * 4));
     INIT_CU(cudaMemset(w.tab_mem, 0, tab_ints * 4));
     {
@@ -814,7 +817,7 @@ int tandem_init(const tandem_config* cfg, tandem_handle** out) {
       t.counts = p; p += C_NUM; t.row_slot = p; p += R; t.row_pos = p; p += R; t.row_tok = p; p += R; t.row_kvslot = p; p += R; t.row_emit = p; p += R;
       t.emit_slot = p; p += S; t.item_row0 = p; p += h->max_items; t.item_ntok = p; p += h->max_items; t.item_kv0 = p; p += h->max_items;
       t.item_kv1 = p; p += h->max_items; t.item_part = p; p += h->max_items;
-      t.comb_row = p; p += h->max_comb; t.comb_part0 = p; p += h->max_comb; t.comb_n = p; p += h->max_comb; t.comb_stride = p; p += h->max_comb;
+      t.comb_row = p; p += h->max_comb; t.comb_part0 = p; p += h->max_comb; t.comb_n = p; p += h->max_comb; t.comb_stride = p; p += h->max_comb; t.comb_gpart = p; p += h->max_comb;
     }
     // page tables
     INIT_TRY(dmalloc(h, &w.bt, (size_t)S * h->max_pages * 4));

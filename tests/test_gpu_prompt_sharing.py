@@ -34,21 +34,25 @@ def _same(out, ref, B, logp_tol):
         assert np.max(np.abs(out["sen_logp"][b, :n] - ref["sen_logp"][b])) < logp_tol
 
 
+@pytest.mark.parametrize("share", [1, 2])
 @pytest.mark.parametrize("start,rows,graph", [(T.SENIOR, 0, 1), (T.DRAW, 0, 0), (T.SENIOR, 24, 1), (T.JUNIOR, 9, 0)])
-def test_shared_prompt_pages_match_oracle(start, rows, graph):
+def test_shared_prompt_pages_match_oracle(start, rows, graph, share):
     """fp32, 3 prompts x 4 rollouts (lengths 40, 17, 70: 2, 1 and 4 shared pages) plus an ungrouped short prompt; also with
-    a row budget that chunks the donor's prefill over several steps (followers wait) and with drawn start owners."""
+    a row budget that chunks the donor's prefill over several steps (followers wait) and with drawn start owners.
+    share = 2: the members of a group that a model serves in a step also READ the shared pages once (shared-prefix runs: q-tiles over
+    the members' rows against positions [0, Ls), merged with each member's own splits by the combine kernel)."""
     table = make_word_start(TINY.vocab, 0.3, 5)
     prompts = _grouped_prompts(TINY, (40, 17, 70), 4, seed=21) + [np.arange(9, dtype=np.int32)]
     B = len(prompts)
     max_new = [28] * B
-    eng, orc, _ = make_pair(TINY, (1, 2), max_seqs=B, max_seq_len=112, share_prompt_pages=1, max_rows_per_step=rows, use_graph=graph)
+    eng, orc, _ = make_pair(TINY, (1, 2), max_seqs=B, max_seq_len=112, share_prompt_pages=share, max_rows_per_step=rows, use_graph=graph)
     ref = tandem_generate(orc, OParams(p=0.5, temperature=1.0, seed=91, start_owner=start), prompts, max_new, table, uni=Uniforms(seed=91))
     out = eng.generate(T.TandemParams(table, p=0.5, temperature=1.0, seed=91, start_owner=start), prompts, max_new)
     _same(out, ref, B, 2e-5)
     st = out["stats"]
     # the start model computes each group's shared prefix once: the other three members take it over (32 + 16 + 64 positions)
     assert st["shared_prompt_rows"] >= 3 * (32 + 16 + 64)
+    assert (st["kv_bytes_shared_reads"] > 0) == (share == 2)      # runs of members were formed and read the shared pages together
     assert 0 < out["owner"].mean() < 1
     eng.free()
     # without sharing: same outputs, more rows, more pages
@@ -91,7 +95,7 @@ def test_shared_prompt_pages_through_tandem_step():
     first = _grouped_prompts(TINY, (40,), 3, seed=6)
     second = [np.arange(30, dtype=np.int32)] + _grouped_prompts(TINY, (52,), 2, seed=7)
     n_new = 20
-    eng, orc, _ = make_pair(TINY, (1, 2), max_seqs=6, max_seq_len=96, share_prompt_pages=1, use_graph=1)
+    eng, orc, _ = make_pair(TINY, (1, 2), max_seqs=6, max_seq_len=96, share_prompt_pages=2, use_graph=1)   # 2: with shared-prefix runs
     prm = T.TandemParams(table, p=0.5, temperature=1.0, seed=3)
     o = dict(token=torch.zeros(6, dtype=torch.int32, device="cuda"), owner=torch.zeros(6, dtype=torch.uint8, device="cuda"),
              done=torch.zeros(6, dtype=torch.uint8, device="cuda"))
@@ -139,14 +143,16 @@ def test_shared_prompt_pages_bf16():
     prm = T.TandemParams(table, p=0.5, temperature=1.0, seed=5)
     res = []
     forced = None
-    for share in (0, 1):
+    for share in (0, 1, 2):
         eng, _, _ = make_pair(shape, (1, 2), max_seqs=B, max_seq_len=128, share_prompt_pages=share, use_graph=1)
         out = eng.generate(prm, prompts, [n_new] * B, forced_tokens=forced)
         res.append(out)
         if forced is None:
             forced = torch.as_tensor(out["tokens"].astype(np.int32)).cuda()
         eng.free()
-    a, b = res
-    assert np.array_equal(a["tokens"], b["tokens"]) and np.array_equal(a["owner"], b["owner"])
-    assert np.max(np.abs(a["sen_logp"] - b["sen_logp"])) < 0.02
-    assert a["stats"]["shared_prompt_rows"] == 0 and b["stats"]["shared_prompt_rows"] >= 3 * (32 + 64)
+    a, b, c = res
+    for x in (b, c):                                       # 1: shared pages; 2: shared pages read once per run of members as well
+        assert np.array_equal(a["tokens"], x["tokens"]) and np.array_equal(a["owner"], x["owner"])
+        assert np.max(np.abs(a["sen_logp"] - x["sen_logp"])) < 0.02
+        assert x["stats"]["shared_prompt_rows"] >= 3 * (32 + 64)
+    assert a["stats"]["shared_prompt_rows"] == 0 and b["stats"]["kv_bytes_shared_reads"] == 0 and c["stats"]["kv_bytes_shared_reads"] > 0
