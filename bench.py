@@ -278,6 +278,7 @@ def run_full_rollout(args):
                                  "max_seqs": max_seqs, "max_rows_per_step": max_rows, "peak_resident": int(st["peak_resident"]), "kv_gb_per_model": kv_per_model / 1e9,
                                  "peak_pages": [int(st["peak_pages_senior"]), int(st["peak_pages_junior"])],
                                  "share_prompt_pages": 0 if args.no_share_prompt_pages else args.share_mode, "shared_prompt_rows": int(st["shared_prompt_rows"]),
+                                 "kv_bytes_shared_reads": int(st["kv_bytes_shared_reads"]), "kv_bytes_read": int(st["kv_bytes_read"]),
                                  "senior_share": float(g["mask"].sum() / max(1, tok))},
                       "gpu_launches": int(st["kernel_launches"]),
                       "step_roofline": {"bound": "hbm", "achieved": gbs, "unit": "GB/s", "frac_of_measured": gbs / pk["hbm_gbs"], "frac_of_8TBs": gbs / NOMINAL_HBM_GBS},
@@ -627,6 +628,7 @@ def run_ours(args):
                     "senior_share": float(g["mask"].sum() / max(1, g["len"].sum())),
                     "step_roofline": {"bound": "hbm", "achieved": gbs, "unit": "GB/s", "frac_of_measured": gbs / pk["hbm_gbs"], "frac_of_8TBs": gbs / NOMINAL_HBM_GBS},
                     "share_prompt_pages": 0 if args.no_share_prompt_pages else args.share_mode, "prompt_rows": e_rows, "shared_prompt_rows": st["shared_prompt_rows"],
+                    "kv_bytes_read": int(st["kv_bytes_read"]), "kv_bytes_shared_reads": int(st["kv_bytes_shared_reads"]),
                     "rows_computed": st["rows_senior"] + st["rows_junior"], "peak_resident": int(st["peak_resident"])}
 
         for it in range(2):
