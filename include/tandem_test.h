@@ -33,7 +33,8 @@ const char *tandem_kernel_class_name(int kc);
  * no catch-up prefill and each model reads its whole KV cache every step; only the owner's row reaches the LM head and the sampler, so
  * tokens, owner flags and log-probs follow the same rule and the same random numbers; default 0 = owner split), "gateup_streamk" (0 = the
  * gate/up projection always runs on the one-tile-per-CTA kernel; default 1: decode-sized steps of a shape with at least one tile pair per
- * CTA use the persistent balanced kernel, csrc/gemm_streamk.cuh), "skip_class" (-1 = none; a TANDEM_KC_* value: the launches of that
+ * CTA use the persistent balanced kernel, csrc/gemm_streamk.cuh), "attn_min_chunk" (0 = by shape: 1024 KV positions per split for
+ * models with >= 8 KV heads, else 256; or a multiple of 64), "skip_class" (-1 = none; a TANDEM_KC_* value: the launches of that
  * kernel class are left out of every step - the step's results are then garbage, its time less the full step's time is the class's
  * marginal cost inside the step graph, PDL overlap included; bench.py --skip-class). TANDEM_EINVAL for an unknown name or a value out of range. Every published number uses the defaults. */
 int tandem_test_set_option(tandem_handle *h, const char *name, int32_t value);

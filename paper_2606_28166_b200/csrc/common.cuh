@@ -9,15 +9,16 @@
 namespace tandem {
 
 constexpr int kPageTokens = 16;      // KV page size (BASELINE.json configs[2]: "paged KV with 16-token blocks")
-constexpr int kAttnMinChunk = 256;   // smallest KV split of an attention item
+constexpr int kAttnMinChunk = 256;   // smallest KV split of an attention item (models with few KV heads: the splits are the parallelism)
+constexpr int kAttnMinChunkWide = 1024;   // ... with >= 8 KV heads (sequences x heads already fill the SMs; a short context in one piece needs no combine)
 constexpr int kAttnMaxSplits = 4;    // an item is split along KV into at most this many chunks
 constexpr int kAttnTileRows = 64;    // (query token, q-head of the group) rows per attention item = 4 MMA m-tiles
 constexpr int kAttnSplitTiles = 4;   // sequences with at most this many q-tiles this step are also split along KV
 // KV positions per split for a context of kv_len positions: a function of kv_len only, so the reduction order of a row
 // never depends on what else is in the batch (batch invariance).
-__host__ __device__ __forceinline__ int attn_chunk(int kv_len) {
+__host__ __device__ __forceinline__ int attn_chunk(int kv_len, int min_chunk) {
   const int c = ((kv_len + kAttnMaxSplits - 1) / kAttnMaxSplits + 63) & ~63;
-  return c > kAttnMinChunk ? c : kAttnMinChunk;
+  return c > min_chunk ? c : min_chunk;
 }
 constexpr int kMaxSlots = 1024;      // scheduler is one CTA with one thread per slot
 

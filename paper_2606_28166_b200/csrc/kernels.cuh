@@ -18,6 +18,7 @@ struct SchedArgs {
   int score;                           // teacher-forced dual scoring (tandem_score): both models ingest every sequence, every row reaches the LM head
   int no_parts;                        // tcgen05 scoring attention: every q-tile covers its whole causal KV range (no KV splits, no combine)
   int lockstep;                        // measurement (paper's engine): BOTH models ingest every token as it is emitted; only the owner samples
+  int min_chunk;                       // smallest KV split (a function of the model shape only: kAttnMinChunk / kAttnMinChunkWide)
   int cascade;                         // share_prompt_pages = 2: the members of a group that a model serves in a step read the group's shared prompt pages ONCE (see below)
   int32_t* oom_flag;                   // mapped host word, set when a pool runs dry (the host reads it without synchronising)
 };
@@ -144,7 +145,7 @@ __global__ void __launch_bounds__(1024) sched_kernel(SchedArgs a) {
     // longer runs (prompt prefill) get their parallelism from the q-tiles and write their output directly.
     const int kv_len = ing + rows;
     const int n_qt = (rows + a.tile_tok - 1) / a.tile_tok;
-    const int chunk = attn_chunk(kv_len);
+    const int chunk = attn_chunk(kv_len, a.min_chunk);
     int n_sched;
     const int ridx = block_excl_scan_1024(rows > 0 ? 1 : 0, &n_sched, wsum);   // index among the slots that have rows in this model
     // Shared-prefix runs (share_prompt_pages = 2; the 8 rollouts of a GRPO group, hold the same prompt KV): the members of a group
@@ -238,7 +239,7 @@ __global__ void __launch_bounds__(1024) sched_kernel(SchedArgs a) {
         tb.item_kv0[i] = 0; tb.item_kv1[i] = (int)sm_ls[q];
         tb.item_part[i] = sm_gp[q] + t0;
       } else if (sm_part0[q] >= 0) {      // split sequence: walk its q-tiles to find (q-tile, split) number `off`
-        const int ch = attn_chunk(qkv), ls = (int)sm_ls[q], kf = ls / ch;   // member of a run: its own items start at the shared length
+        const int ch = attn_chunk(qkv, a.min_chunk), ls = (int)sm_ls[q], kf = ls / ch;   // member of a run: its own items start at the shared length
         int rem = off, poff = 0, t0 = 0, nt = 0, ns = 0;
         for (;; t0 += a.tile_tok) {
           nt = min(a.tile_tok, qrows - t0);

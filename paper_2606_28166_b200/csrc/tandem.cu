@@ -83,6 +83,7 @@ struct tandem_handle {
   bool dual_forward = false;                    // measurement: the paper's lock-step engine (both models forward every token), see tandem_test.h
   bool attn_prefill_tc = true;                  // tandem_score: tcgen05 attention over 128-row q-tiles (attention_tcgen05.cuh); false = the mma.sync kernel
   bool fused_sampler = true;                    // S8 in the LM head's epilogue whenever the sampler needs no materialised logits
+  int attn_min_chunk = 0;                       // 0 = by shape; "attn_min_chunk" knob for A/B
   int skip_class = -1;                          // measurement (tandem_test.h "skip_class"): the launches of this kernel class are left out of the step
   bool gateup_streamk = true;                   // gate/up + SwiGLU as the persistent stream-K kernel (gemm_streamk.cuh) when the shape allows; false = one tile per CTA
   float* sk_scratch = nullptr; int sk_rows = 0; int32_t* sk_flags = nullptr;   // its tail partials [n_sms][2][sk_rows][128] and flag / acknowledge counters [2][n_sms]
@@ -437,6 +438,7 @@ int launch_step(tandem_handle* h, const StepIO& io, const RuleParams& rp, cudaSt
   if (score && use_attn_tc(h)) { sa.tile_tok = kAtTileKv / (c.n_q_heads / c.n_kv_heads); sa.no_parts = 1; }   // 128-row q-tiles, each over its whole causal range
   sa.work_ctr = h->work_ctr; sa.n_work_ctr = 3 * c.n_layers;
   sa.cascade = (c.share_prompt_pages == 2 && !score) ? 1 : 0;
+  sa.min_chunk = h->attn_min_chunk > 0 ? h->attn_min_chunk : (c.n_kv_heads >= 8 ? kAttnMinChunkWide : kAttnMinChunk);
   sa.score = score ? 1 : 0; sa.oom_flag = h->oom_dev; sa.lockstep = (h->dual_forward && !score) ? 1 : 0;
   KL(h, TANDEM_KC_SCHED, s, (sched_kernel<<<1, 1024, 0, s>>>(sa)));
   const int rc = (c.dtype == TANDEM_F32) ? forward_pair<float>(h, io, rp, s, score, score_inv_t) : forward_pair<bf16>(h, io, rp, s, score, score_inv_t);
@@ -1429,6 +1431,7 @@ int tandem_test_set_option(tandem_handle* h, const char* name, int32_t value) {
   else if (n == "gemm_ring_kb" && in(0, 200)) h->gemm_ring_kb = value;
   else if (n == "fused_sampler" && in(0, 1)) h->fused_sampler = value != 0;
   else if (n == "gateup_streamk" && in(0, 1)) h->gateup_streamk = value != 0;
+  else if (n == "attn_min_chunk" && (value == 0 || (value >= 64 && value % 64 == 0))) h->attn_min_chunk = value;
   else if (n == "skip_class" && in(-1, TANDEM_KC_NUM - 1)) h->skip_class = value;
   else if (n == "dual_forward" && in(0, 1)) h->dual_forward = value != 0;
   else if (n == "attn_prefill_tc" && in(0, 1)) h->attn_prefill_tc = value != 0;
