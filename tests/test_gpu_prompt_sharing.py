@@ -156,3 +156,44 @@ def test_shared_prompt_pages_bf16():
         assert np.max(np.abs(a["sen_logp"] - x["sen_logp"])) < 0.02
         assert x["stats"]["shared_prompt_rows"] >= 3 * (32 + 64)
     assert a["stats"]["shared_prompt_rows"] == 0 and b["stats"]["kv_bytes_shared_reads"] == 0 and c["stats"]["kv_bytes_shared_reads"] > 0
+
+
+def test_shared_prefix_runs_at_the_4b_width():
+    """share_prompt_pages = 2 at the head geometry the benchmark runs (32 q / 8 kv heads of 128: G = 4, 16-token q-tiles, KV splits of 1024
+    positions): 2 prompts x 8 rollouts (lengths 150 and 333: 9 and 20 shared pages), one layer of the 4B shape. The engine without sharing and
+    the engine with shared-prefix runs follow the same forced token stream; owners are exact, and BOTH are compared with the float64 oracle:
+    the runs change where the softmax is cut (at the shared length) and with it the bf16 rounding of P, not the sums - their error against
+    the oracle must be the error of the plain path (one layer of this width: max 0.02 / mean 0.006, tests/test_gpu_full_width.py)."""
+    from workloads import get_workload
+    from oracle import replay_owner_logits
+    from oracle.sampler import log_softmax
+    f = get_workload("cfg3_4b_bf16").shape
+    shape = ModelShape(1, f.hidden, f.n_q_heads, f.n_kv_heads, f.head_dim, f.intermediate, 4096, f.rms_eps, f.rope_theta, "bf16")
+    table = make_word_start(shape.vocab, 0.3, 5)
+    prompts = _grouped_prompts(shape, (150, 333), 8, seed=4)
+    B, n_new = len(prompts), 24
+    prm = T.TandemParams(table, p=0.5, temperature=1.0, seed=15)
+    res, forced = [], None
+    for share in (0, 2):
+        eng, models, _ = make_pair(shape, (1, 2), max_seqs=B, max_seq_len=400, share_prompt_pages=share, use_graph=1)
+        out = eng.generate(prm, prompts, [n_new] * B, forced_tokens=forced)
+        res.append(out)
+        if forced is None:
+            forced = torch.as_tensor(out["tokens"].astype(np.int32)).cuda()
+        eng.free()
+    a, c = res
+    assert np.array_equal(a["tokens"], c["tokens"]) and np.array_equal(a["owner"], c["owner"]) and 0.2 < a["owner"].mean() < 0.8
+    assert c["stats"]["kv_bytes_shared_reads"] > 0.3 * c["stats"]["kv_bytes_read"]
+    err = {0: [], 2: []}
+    for b in (0, 3, 8, 13):                                 # two members of each group
+        z = replay_owner_logits(models, prompts[b], a["tokens"][b], a["owner"][b])
+        for t in range(n_new):
+            if a["owner"][b, t] == 0:
+                ref = log_softmax(z[t])[int(a["tokens"][b, t])]
+                err[0].append(abs(float(a["sen_logp"][b, t]) - ref)); err[2].append(abs(float(c["sen_logp"][b, t]) - ref))
+    e0, e2 = np.array(err[0]), np.array(err[2])
+    print("4B width, 1 layer, vs float64 oracle over %d senior positions: no sharing max %.4f mean %.4f; shared-prefix runs max %.4f mean %.4f; shared reads %.0f%% of the KV bytes"
+          % (e0.size, e0.max(), e0.mean(), e2.max(), e2.mean(), 100.0 * c["stats"]["kv_bytes_shared_reads"] / c["stats"]["kv_bytes_read"]))
+    # measured on B200: no sharing max 0.0201 / mean 0.0059, shared-prefix runs max 0.0191 / mean 0.0056, 69% of the KV bytes read shared
+    assert e0.max() <= 0.04 and e0.mean() <= 0.012          # the bars of tests/test_gpu_full_width.py for one layer
+    assert e2.max() <= 0.04 and e2.mean() <= 0.012 and e2.mean() <= 1.3 * e0.mean() + 1e-3
