@@ -42,12 +42,14 @@ def test_cfg3_full_batch_sampled_sequences_and_integer_outputs():
     max_len = max(len(p) for p in prompts) + N_NEW + 1
     prm = T.TandemParams(table, p=wl.p, temperature=1.0, seed=SEED)
 
-    eng = T.Tandem(T.TandemConfig(shape, max_seqs=B, max_seq_len=max_len, use_graph=1))   # what bench.py runs: step graph, paired launches
+    # what bench.py runs: step graph, paired launches, the rollouts of a prompt sharing its KV pages and reading them once per run (share_prompt_pages = 2)
+    eng = T.Tandem(T.TandemConfig(shape, max_seqs=B, max_seq_len=max_len, use_graph=1, share_prompt_pages=2))
     eng.load_weights(0, ws_)
     eng.load_weights(1, wj_)
     out = eng.generate(prm, prompts, [N_NEW] * B)
     eng.free()
     toks, own, lp, n = out["tokens"], out["owner"], out["sen_logp"], out["len"]
+    assert out["stats"]["shared_prompt_rows"] > 0 and out["stats"]["kv_bytes_shared_reads"] > 0
 
     # ---- all 128 sequences: integer outputs bit-exact against the oracle's rule on the GPU's own token stream
     assert (n == N_NEW).all()
